@@ -1,0 +1,265 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the tropical transfer sweep (BASELINE.json metric:
+"Sweep time per instance & achieved HBM GB/s (frac. of peak), LxL tropical sweep").
+
+Workload at N=1: BASELINE.json configs[3] -- 32x32 +-J Ising, h=0, Tropical<f32> energy, one
+2^32-entry (16 GiB) state swept in place -- the configuration north_star's ">= 60 % of the HBM
+roofline on the 2^28..2^32-entry sweeps" is quoted on.  A "step" is one whole sweep (every pass
+kernel + the final reduction) of one instance per GPU.  With N GPUs each rank sweeps its own
+instance (seed 4000 + rank): replicas, no data-path collective, "scaling": "weak".
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--L 32] [--impl ours|reference]
+
+`value`  : ms per instance, device-timed with CUDA events on the launching stream, couplings
+           already resident in HBM (ttn_plan_launch only), max over ranks / instances per step.
+`e2e`    : the same through the one-call C ABI (ttn_sweep_energy) with HOST coupling buffers:
+           plan + host->device upload + sweep + device->host result, timed on the host clock
+           around the synchronising call.
+`roofline`: HBM roofline as north_star defines it: algorithmic bytes = (L-1)*2*4*2^L per sweep
+           (row 0 write-only, last row read-only) over the measured sweep time,
+           against the measured copy bandwidth in MEASURED_PEAKS.json.
+`cpu_baseline`: the CPU oracle (oracle/, unmodified) timed on the host cores on a bounded
+           sample, scaled to the metric's unit by the update count (L-1)*L*2^L.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from ttn_inputs import make_batch  # noqa: E402
+
+METRIC = "sweep_time_per_instance"
+UNIT = "ms"
+
+
+def updates(L: int) -> float:
+    """el-gate updates of one sweep: (L-1) rows x L gates x 2^L elements."""
+    return float(L - 1) * L * 2.0 ** L
+
+
+def bytes_min(L: int) -> float:
+    """north_star's minimum traffic: one read + one write of the f32 state per row, row 0
+    write-only and the last row read-only."""
+    return float(L - 1) * 2 * 4 * 2.0 ** L
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons during the timed region (nvidia-smi, 200 ms)."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop_evt = threading.Event()
+
+    def run(self):
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        while not self._stop_evt.is_set():
+            try:
+                out = subprocess.check_output(
+                    ["nvidia-smi", f"--id={self.index}", f"--query-gpu={q}", "--format=csv,noheader,nounits"],
+                    text=True, timeout=5).strip().split(",")
+                self.samples.append(float(out[0]))
+                self.max_mhz = float(out[1])
+                for n, v in zip(names, out[2:]):
+                    if v.strip().lower() == "active":
+                        self.reasons.add(n)
+            except Exception:
+                pass
+            self._stop_evt.wait(0.2)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=10)
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle as it stands, on the host cores.  Each step is a bounded
+    sample (a full sweep of a smaller lattice of the same +-J distribution), scaled to the
+    32x32 metric by the update count."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    Ls = args.ref_L
+    Jh, Jv, _ = make_batch(Ls, [4000], "pmj")
+    times = []
+    for i in range(args.warmup + args.steps):
+        t = time.perf_counter()
+        oracle.dp_ising(Ls, Jh[0], Jv[0], None, count=False)
+        if i >= args.warmup:
+            times.append(time.perf_counter() - t)
+    per_update = float(np.mean(times)) / updates(Ls)
+    val = per_update * updates(args.L) * 1e3
+    cores = oracle.num_threads()
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": float(np.mean(times)) * 1e3,
+        "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": f"{args.L}x{args.L} +-J Ising energy sweep (extrapolated from sample)"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": f"full O-dp sweep of a {Ls}x{Ls} +-J instance per step, scaled by "
+                                   f"(L-1)L2^L updates to {args.L}x{args.L}"},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def cpu_baseline(L_target: int, L_sample: int):
+    import oracle
+    Jh, Jv, _ = make_batch(L_sample, [4000], "pmj")
+    t = time.perf_counter()
+    oracle.dp_ising(L_sample, Jh[0], Jv[0], None, count=False)
+    dt = time.perf_counter() - t
+    val = dt / updates(L_sample) * updates(L_target) * 1e3
+    return {"value": val, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"one full O-dp sweep of a {L_sample}x{L_sample} +-J instance ({dt:.1f} s), scaled by "
+                      f"(L-1)L2^L updates to {L_target}x{L_target}",
+            "sample_seconds": dt}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--L", type=int, default=32)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-L", type=int, default=22, dest="ref_L")
+    ap.add_argument("--cpu-L", type=int, default=24, dest="cpu_L")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3                                   # timing rule: W >= 3
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import paper_2008_06888_b200 as ttn
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the sweep has no CPU path)")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    L = args.L
+    Jh, Jv, _ = make_batch(L, [4000 + rank], "pmj")
+    ws = ttn.alloc_workspace(ttn.workspace_bytes(2, L, ttn.TROPICAL_F32, 1), f"cuda:{local_rank}")
+    plan = ttn.Plan(2, ttn.CALL_ENERGY, Jh, Jv, None, workspace=ws)
+    torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        plan.launch()
+    torch.cuda.synchronize()
+    E_dev = plan.read()[0][0]
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    barrier()
+    if sampler:
+        sampler.start()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    ev[0].record()
+    for k in range(args.steps):
+        plan.launch()
+        ev[k + 1].record()
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    total_ms = ev[0].elapsed_time(ev[-1])
+    step_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
+    if dist is not None:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+
+    # ---- end to end through the one-call C ABI with host buffers -----------------------------
+    e2e_times = []
+    for i in range(2 + min(args.steps, 3)):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        E_host = ttn.sweep_energy(Jh, Jv, workspace=ws)[0]
+        if i >= 2:
+            e2e_times.append((time.perf_counter() - t0) * 1e3)
+    e2e_ms = float(np.mean(e2e_times))
+    if dist is not None:
+        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    assert E_host == E_dev, (E_host, E_dev)
+
+    if rank == 0:
+        peak, peak_src = measured_peaks()
+        per_inst_ms = ms_per_step / world
+        achieved = bytes_min(L) / (ms_per_step * 1e-3) / 1e9            # GB/s per GPU
+        sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
+        alu_peak = 148 * 64 * sm_mhz * 1e6                              # FMNMX: 64 lanes/clk/SM (alu pipe)
+        out = {
+            "metric": METRIC, "value": per_inst_ms, "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
+            "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{L}x{L} +-J Ising (p=0.5, h=0) Tropical<f32> energy sweep, "
+                                   f"2^{L}-entry state in place, 1 instance per GPU (seed 4000+rank)",
+                       "L": L, "state_bytes": 4 * 2 ** L, "hbm_passes": plan.num_passes,
+                       "l2_policy": "state (>= 1 GiB) far larger than the 126 MB L2; no flush needed"
+                       if L >= 28 else "state fits L2: flush not applied, number is L2-resident",
+                       "E0": E_dev},
+            "e2e": {"value": e2e_ms / world, "unit": UNIT,
+                    "h2d_bytes_per_step": int(Jh.nbytes + Jv.nbytes), "d2h_bytes_per_step": 4},
+            "gpu_launches": plan.num_launches * args.steps,
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                         "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                         "algorithmic_bytes_per_sweep": bytes_min(L),
+                         "kernel": "ttn::pass_kernel<2,false> (all passes of one sweep)"},
+            "alu_roofline": {"bound": "alu", "achieved": updates(L) / (ms_per_step * 1e-3),
+                             "peak": alu_peak, "unit": "max-plus updates/s",
+                             "frac": updates(L) / (ms_per_step * 1e-3) / alu_peak,
+                             "note": "1 FMNMX per update on the 64-lane/clk/SM alu pipe at the sampled SM clock"},
+            "step_ms": step_ms, "clocks": clocks,
+        }
+        if not args.no_cpu_baseline:
+            out["cpu_baseline"] = cpu_baseline(L, args.cpu_L)
+        print(json.dumps(out))
+    plan.close()
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,129 @@
+/*
+ * ttn.h -- C ABI of the B200 tropical tensor-network sweep (libttn.so).
+ *
+ * The library contracts the tropical tensor network of an L x L open-boundary Ising (q = 2)
+ * or 3-state Potts (q = 3) spin glass as a row-by-row transfer sweep in the paper's circuit
+ * picture (Fig. 1b; App. A (A2)-(A4) PAPER.md:240-252): a state vector of
+ * q^L tropical numbers (Eq. (2)) -- or counting tuples (x, n) (Eq. (4)
+ * PAPER.md:78-83) -- goes through every row; a final (+)-reduction gives -E0
+ * and the ground-state degeneracy.  A checkpointed backward pass returns one
+ * ground-state configuration ("caching intermediate contraction results and backtracking",
+ * PAPER.md:97; footnote [49] PAPER.md:201 for ties).
+ *
+ * Problem statement (Eq. (1)):
+ *     E(sigma) = - sum_<ij> J_ij sigma_i sigma_j - sum_i h_i sigma_i ,   sigma_i = +-1
+ *   site (r,c), r,c in [0,L);  Jh[r][c] (c < L-1) couples (r,c)-(r,c+1);  Jv[r][c] (r < L-1)
+ *   couples (r,c)-(r+1,c);  h[r][c] is the field on (r,c).
+ *   Potts (App. C, in BASELINE.json's reading):
+ *     E(t) = - sum_<ij> J_ij delta(t_i, t_j),  t_i in {0,1,2},  no fields.
+ *
+ * Memory spaces.  Couplings and results are HOST pointers (they are O(L^2) numbers);
+ * `workspace` is a DEVICE pointer owned by the caller (at least ttn_workspace_bytes(...)
+ * bytes, 256-byte aligned), `stream` is a cudaStream_t passed as void* (NULL = default
+ * stream).  The library allocates no device memory and keeps no global state; every step of
+ * the path runs in the library's own sm_100a kernels.  There is NO CPU fallback: without a
+ * CUDA device every compute call returns TTN_ECUDA.
+ *
+ * Layouts (row-major, batch-major):  Jh[batch][L][L-1], Jv[batch][L-1][L], h[batch][L][L]
+ * (h may be NULL = all zero), E0[batch], degeneracy[batch], sigma[batch][L][L] (+1 / -1).
+ *
+ * Numerics.  State elements are f32 (Tropical<f32>); degeneracy counts are f64
+ * (CountingTropical<f32,f64>): exact below 2^53, correctly rounded sums above.  Ties in
+ * Eq. (4) are exact IEEE equality on f32, meaningful for integer-valued couplings.
+ * E0 is returned as the ground-state ENERGY (the sweep yields -E0); -0.0 is normalised to
+ * +0.0.  Under degeneracy sigma is one ground state (lowest state index wins ties).
+ *
+ * Errors.  Every function returns a ttn_status; nothing throws or aborts.
+ * ttn_last_error() gives a thread-local message for the last non-OK status.
+ */
+#ifndef TTN_H_
+#define TTN_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    TTN_OK = 0,
+    TTN_EINVAL = 1,        /* NULL pointer, L < 1, batch < 1, non-finite coupling, bad q/mode   */
+    TTN_EUNSUPPORTED = 2,  /* L beyond the limits below, or the device is not sm_100           */
+    TTN_ENOMEM = 3,        /* workspace_bytes smaller than ttn_workspace_bytes(...)            */
+    TTN_ECUDA = 4          /* a CUDA call failed / no device; see ttn_last_error()             */
+} ttn_status;
+
+typedef enum {
+    TTN_TROPICAL_F32 = 0,      /* Eq. (2): x (+) y = max, x (.) y = x + y                      */
+    TTN_COUNTING_F32_F64 = 1   /* Eq. (4): (x, n) tuples, n summed on exact ties               */
+} ttn_semiring;
+
+/* Limits: Ising tropical L <= 34, Ising counting L <= 32, Potts L <= 20 (index fits 32 bits);
+   ttn_ground_config L <= 28 (L checkpoints of 2^L f32 each). */
+
+/* Bytes of device workspace needed.  q = 2 (Ising) or 3 (Potts).  Returns 0 on bad arguments. */
+size_t ttn_workspace_bytes(int q, int L, ttn_semiring mode, int batch, int want_config);
+
+/* ---- one-call host API (upload + sweep + read-back, synchronises `stream`) -------------- */
+
+/* Ground-state energy, Tropical<f32> sweep. */
+ttn_status ttn_sweep_energy(int L, const float* Jh, const float* Jv, const float* h, int batch,
+                            void* workspace, size_t workspace_bytes, void* stream,
+                            double* E0 /*[batch]*/);
+
+/* Ground-state energy and degeneracy, CountingTropical sweep (Eq. (4)). */
+ttn_status ttn_sweep_count(int L, const float* Jh, const float* Jv, const float* h, int batch,
+                           void* workspace, size_t workspace_bytes, void* stream,
+                           double* E0 /*[batch]*/, double* degeneracy /*[batch]*/);
+
+/* Ground-state energy and one ground-state configuration: forward sweep with row-boundary
+   checkpoints C_r, backward argmax pass (stands in for App. B). */
+ttn_status ttn_ground_config(int L, const float* Jh, const float* Jv, const float* h, int batch,
+                             void* workspace, size_t workspace_bytes, void* stream,
+                             double* E0 /*[batch]*/, int8_t* sigma /*[batch][L][L]*/);
+
+/* 3-state Potts variants (App. C): 3x3 max-plus gates, state 3^L. */
+ttn_status ttn_potts3_sweep_energy(int L, const float* Jh, const float* Jv, int batch,
+                                   void* workspace, size_t workspace_bytes, void* stream,
+                                   double* E0 /*[batch]*/);
+ttn_status ttn_potts3_sweep_count(int L, const float* Jh, const float* Jv, int batch,
+                                  void* workspace, size_t workspace_bytes, void* stream,
+                                  double* E0 /*[batch]*/, double* degeneracy /*[batch]*/);
+
+/* ---- split API: upload once, launch asynchronously, read later ---------------------------
+ * The one-call functions above are ttn_plan_create + ttn_plan_launch + ttn_plan_read +
+ * ttn_plan_destroy.  A plan holds the host-side pass schedule (which gates
+ * and diagonal terms each HBM pass applies) and the addresses of its tables inside
+ * `workspace`; the workspace must stay alive and untouched while the plan is in use.
+ *   ttn_plan_create : validates, plans, copies couplings host->device on `stream` (async).
+ *   ttn_plan_launch : enqueues every kernel of one whole sweep on `stream`; does not
+ *                     synchronise; results stay in the workspace.  May be called repeatedly.
+ *   ttn_plan_read   : device->host copy of the results of the last launch; synchronises.
+ *                     Pointers that do not apply to the plan's call kind must be NULL.      */
+typedef struct ttn_plan ttn_plan;
+typedef enum { TTN_CALL_ENERGY = 0, TTN_CALL_COUNT = 1, TTN_CALL_CONFIG = 2 } ttn_call;
+
+ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const float* Jv,
+                           const float* h, int batch, void* workspace, size_t workspace_bytes,
+                           void* stream, ttn_plan** plan);
+ttn_status ttn_plan_launch(ttn_plan* plan, void* stream);
+ttn_status ttn_plan_read(ttn_plan* plan, void* stream, double* E0, double* degeneracy,
+                         int8_t* sigma);
+void ttn_plan_destroy(ttn_plan* plan);
+
+/* Introspection (host only, no CUDA calls). */
+int ttn_plan_num_launches(const ttn_plan* plan);   /* kernels enqueued by one ttn_plan_launch   */
+int ttn_plan_num_passes(const ttn_plan* plan);     /* HBM passes over the state among them      */
+/* Writes a text description of the pass schedule for (q, L, call) -- one line per pass and
+   one per op -- into buf (NUL-terminated, truncated to n).  Returns the untruncated length,
+   or -1 on bad arguments.  Needs no device: used by the CPU-side schedule validator.          */
+long ttn_plan_describe(int q, int L, ttn_call call, char* buf, size_t n);
+
+const char* ttn_last_error(void);   /* thread-local, static storage */
+int ttn_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TTN_H_ */

@@ -1,0 +1,359 @@
+// ttn_api.cu -- the C ABI of include/ttn.h: argument validation, workspace layout, coupling
+// upload, kernel launches of one whole sweep, result read-back.  No torch types; no CPU path.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/ttn.h"
+#include "planner.h"
+#include "ttn_kernels.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+ttn_status fail(ttn_status st, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return st;
+}
+
+#define TTN_CUDA(call)                                                                        \
+    do {                                                                                      \
+        cudaError_t e_ = (call);                                                              \
+        if (e_ != cudaSuccess)                                                                \
+            return fail(TTN_ECUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_),    \
+                        __FILE__, __LINE__);                                                  \
+    } while (0)
+
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+unsigned long long ipow(int q, int e) {
+    unsigned long long r = 1;
+    for (int i = 0; i < e; ++i) r *= (unsigned long long)q;
+    return r;
+}
+
+// Tile capacity (log_q of elements per CTA tile) and riding digits of the generic path.
+struct TileCfg { int Tmax, ride; };
+TileCfg tile_cfg(int q, bool count) {
+    TileCfg t;
+    if (q == 2) t = count ? TileCfg{13, 3} : TileCfg{14, 3};   // 96 KiB / 64 KiB of smem
+    else t = count ? TileCfg{8, 2} : TileCfg{9, 2};           // 3^8*12 = 77 KiB / 3^9*4 = 77 KiB
+    // Debug/test override (smaller tiles only): lets tiny lattices exercise multi-pass schedules.
+    if (const char* e = getenv("TTN_DEBUG_TMAX")) { int v = atoi(e); if (v >= 2 && v <= t.Tmax) t.Tmax = v; }
+    if (const char* e = getenv("TTN_DEBUG_RIDE")) { int v = atoi(e); if (v >= 0 && v < t.Tmax) t.ride = v; }
+    if (t.ride >= t.Tmax) t.ride = t.Tmax - 1;
+    return t;
+}
+
+bool limits_ok(int q, int L, bool count, bool config) {
+    if (L < 1) return false;
+    if (q == 2) {
+        if (config) return L <= 28;
+        return count ? L <= 32 : L <= 34;
+    }
+    if (q == 3) return !config && L <= 20;
+    return false;
+}
+
+struct Layout {
+    size_t x = 0, n = 0, ckpt = 0, Jh = 0, Jv = 0, h = 0, ops = 0, part_x = 0, part_n = 0,
+           amax_v = 0, amax_s = 0, out_x = 0, out_n = 0, out_s = 0, sigma = 0, total = 0;
+    unsigned long long NS = 0, max_tiles = 0;
+    int amax_blocks = 0;
+};
+
+// The op list length is bounded by L*L gates + 2*L*L diagonals.
+Layout make_layout(int q, int L, bool count, bool config, int batch) {
+    Layout y;
+    y.NS = ipow(q, L);
+    const TileCfg tc = tile_cfg(q, count);
+    // every pass of a plan stages tiles of q^min(L, Tmax) elements
+    y.max_tiles = y.NS / ipow(q, tc.Tmax < L ? tc.Tmax : L);
+    if (y.max_tiles == 0) y.max_tiles = 1;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+    y.x = take((size_t)batch * y.NS * 4);
+    if (count) y.n = take((size_t)batch * y.NS * 8);
+    if (config) y.ckpt = take((size_t)batch * L * y.NS * 4);
+    y.Jh = take((size_t)batch * L * (L - 1) * 4 + 4);
+    y.Jv = take((size_t)batch * (L - 1) * L * 4 + 4);
+    y.h = take((size_t)batch * L * L * 4);
+    y.ops = take((size_t)(3 * L * L + 8) * sizeof(ttn::Op));
+    y.part_x = take((size_t)batch * y.max_tiles * 4);
+    y.part_n = take((size_t)batch * y.max_tiles * 8);
+    unsigned long long nb = (y.NS + 256ull * 16 - 1) / (256ull * 16);
+    y.amax_blocks = (int)(nb < 1 ? 1 : (nb > 1024 ? 1024 : nb));
+    y.amax_v = take((size_t)batch * y.amax_blocks * 4);
+    y.amax_s = take((size_t)batch * y.amax_blocks * 8);
+    y.out_x = take((size_t)batch * 4);
+    y.out_n = take((size_t)batch * 8);
+    y.out_s = take((size_t)batch * 8);
+    y.sigma = take((size_t)batch * L * L);
+    y.total = off;
+    return y;
+}
+
+template <typename K>
+ttn_status set_smem(K kernel, size_t bytes) {
+    TTN_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    return TTN_OK;
+}
+
+}  // namespace
+
+struct ttn_plan {
+    int q, L, batch;
+    ttn_call call;
+    bool count, config, has_field;
+    ttn::Plan plan;
+    Layout lay;
+    unsigned char* ws;
+    std::vector<double> defer;     // per instance: sum of the +J constants factored out of the gates
+    int launches;
+};
+
+static ttn::Plan plan_for(int q, int L, ttn_call call, bool has_field) {
+    const bool count = (call == TTN_CALL_COUNT);
+    const TileCfg tc = tile_cfg(q, count);
+    return ttn::make_plan(q, L, has_field, call == TTN_CALL_CONFIG, tc.Tmax, tc.ride);
+}
+
+template <int Q, bool COUNT>
+static ttn_status launch_pass(const ttn_plan* P, const ttn::Pass& ps, cudaStream_t st) {
+    const Layout& y = P->lay;
+    ttn::PassParams pp{};
+    pp.L = P->L; pp.lo = ps.lo; pp.a = ps.a; pp.b = ps.b; pp.T = ps.lo + (ps.b - ps.a);
+    pp.P_lo = ipow(Q, ps.lo); pp.P_a = ipow(Q, ps.a); pp.P_mid = ipow(Q, ps.a - ps.lo); pp.P_b = ipow(Q, ps.b);
+    pp.n_tile = (unsigned)ipow(Q, pp.T);
+    pp.tiles_per_inst = y.NS / pp.n_tile;
+    float* V = reinterpret_cast<float*>(P->ws + y.x);
+    float* CK = reinterpret_cast<float*>(P->ws + y.ckpt);
+    auto buf = [&](int id, unsigned long long& stride) -> float* {
+        if (id < 0) { stride = y.NS; return V; }
+        stride = (unsigned long long)P->L * y.NS;
+        return CK + (unsigned long long)id * y.NS;
+    };
+    pp.src_x = buf(ps.src_buf, pp.src_stride);
+    pp.dst_x = buf(ps.dst_buf, pp.dst_stride);
+    pp.src_n = pp.dst_n = COUNT ? reinterpret_cast<double*>(P->ws + y.n) : nullptr;
+    pp.ops = reinterpret_cast<const ttn::Op*>(P->ws + y.ops) + ps.op_begin;
+    pp.n_ops = ps.op_end - ps.op_begin;
+    pp.Jh = reinterpret_cast<const float*>(P->ws + y.Jh);
+    pp.Jv = reinterpret_cast<const float*>(P->ws + y.Jv);
+    pp.h = P->has_field ? reinterpret_cast<const float*>(P->ws + y.h) : nullptr;
+    pp.flags = ps.flags;
+    pp.part_x = reinterpret_cast<float*>(P->ws + y.part_x);
+    pp.part_n = reinterpret_cast<double*>(P->ws + y.part_n);
+    const size_t smem = (size_t)pp.n_tile * (COUNT ? 12 : 4);
+    ttn_status s = set_smem(ttn::pass_kernel<Q, COUNT>, smem);
+    if (s != TTN_OK) return s;
+    const unsigned long long grid = pp.tiles_per_inst * (unsigned long long)P->batch;
+    if (grid > 0x7fffffffull) return fail(TTN_EUNSUPPORTED, "grid too large");
+    unsigned threads = pp.n_tile / Q >= 512 ? 512 : (pp.n_tile / Q < 32 ? 32 : ((pp.n_tile / Q + 31) / 32 * 32));
+    ttn::pass_kernel<Q, COUNT><<<(unsigned)grid, threads, smem, st>>>(pp);
+    TTN_CUDA(cudaGetLastError());
+    if (ps.flags & ttn::PASS_REDUCE) {
+        ttn::final_reduce_kernel<COUNT><<<P->batch, 256, 0, st>>>(
+            pp.part_x, pp.part_n, pp.tiles_per_inst, reinterpret_cast<float*>(P->ws + y.out_x),
+            reinterpret_cast<double*>(P->ws + y.out_n));
+        TTN_CUDA(cudaGetLastError());
+    }
+    return TTN_OK;
+}
+
+extern "C" {
+
+const char* ttn_last_error(void) { return g_err; }
+int ttn_version(void) { return 100; }
+
+size_t ttn_workspace_bytes(int q, int L, ttn_semiring mode, int batch, int want_config) {
+    const bool count = (mode == TTN_COUNTING_F32_F64);
+    if ((q != 2 && q != 3) || batch < 1 || (mode != TTN_TROPICAL_F32 && mode != TTN_COUNTING_F32_F64)) return 0;
+    if (!limits_ok(q, L, count, want_config != 0)) return 0;
+    return make_layout(q, L, count, want_config != 0, batch).total;
+}
+
+long ttn_plan_describe(int q, int L, ttn_call call, char* buf, size_t n) {
+    if ((q != 2 && q != 3) || !buf || n == 0) return -1;
+    if (!limits_ok(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) return -1;
+    std::string s = ttn::describe(plan_for(q, L, call, /*has_field=*/q == 2));
+    size_t m = s.size() < n - 1 ? s.size() : n - 1;
+    memcpy(buf, s.data(), m);
+    buf[m] = 0;
+    return (long)s.size();
+}
+
+ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const float* Jv,
+                           const float* h, int batch, void* workspace, size_t workspace_bytes,
+                           void* stream, ttn_plan** out) {
+    if (!out) return fail(TTN_EINVAL, "plan pointer is NULL");
+    *out = nullptr;
+    if (q != 2 && q != 3) return fail(TTN_EINVAL, "q must be 2 or 3");
+    if (L < 1 || batch < 1) return fail(TTN_EINVAL, "L and batch must be >= 1");
+    if (call != TTN_CALL_ENERGY && call != TTN_CALL_COUNT && call != TTN_CALL_CONFIG)
+        return fail(TTN_EINVAL, "bad call kind");
+    if (L > 1 && (!Jh || !Jv)) return fail(TTN_EINVAL, "Jh/Jv is NULL");
+    if (!workspace) return fail(TTN_EINVAL, "workspace is NULL");
+    if (q == 3 && h) return fail(TTN_EINVAL, "the Potts variant takes no fields");
+    const bool count = (call == TTN_CALL_COUNT), config = (call == TTN_CALL_CONFIG);
+    if (!limits_ok(q, L, count, config)) return fail(TTN_EUNSUPPORTED, "L=%d beyond the limits for this call", L);
+    const size_t nh = (size_t)batch * L * (L - 1), nv = (size_t)batch * (L - 1) * L, nf = (size_t)batch * L * L;
+    for (size_t i = 0; i < nh; ++i) if (!std::isfinite(Jh[i])) return fail(TTN_EINVAL, "non-finite Jh[%zu]", i);
+    for (size_t i = 0; i < nv; ++i) if (!std::isfinite(Jv[i])) return fail(TTN_EINVAL, "non-finite Jv[%zu]", i);
+    if (h) for (size_t i = 0; i < nf; ++i) if (!std::isfinite(h[i])) return fail(TTN_EINVAL, "non-finite h[%zu]", i);
+
+    Layout lay = make_layout(q, L, count, config, batch);
+    if (workspace_bytes < lay.total)
+        return fail(TTN_ENOMEM, "workspace too small: %zu < %zu", workspace_bytes, lay.total);
+    if ((uintptr_t)workspace % 256) return fail(TTN_EINVAL, "workspace must be 256-byte aligned");
+
+    int dev = 0, major = 0;
+    TTN_CUDA(cudaGetDevice(&dev));
+    TTN_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10) return fail(TTN_EUNSUPPORTED, "device compute capability %d.x is not sm_100", major);
+
+    ttn_plan* P = new (std::nothrow) ttn_plan();
+    if (!P) return fail(TTN_ENOMEM, "host allocation failed");
+    P->q = q; P->L = L; P->batch = batch; P->call = call; P->count = count; P->config = config;
+    P->has_field = (h != nullptr);
+    P->plan = plan_for(q, L, call, P->has_field);
+    P->lay = lay;
+    P->ws = static_cast<unsigned char*>(workspace);
+    if (P->plan.passes.empty()) { delete P; return fail(TTN_EUNSUPPORTED, "planner produced no schedule"); }
+    if (P->plan.ops.size() > (size_t)(3 * L * L + 8)) { delete P; return fail(TTN_EUNSUPPORTED, "op list too long"); }
+
+    // the +J constants factored out of the Ising gates (kernel comment at OP_GATE), in f64
+    P->defer.assign(batch, 0.0);
+    if (q == 2)
+        for (int b = 0; b < batch; ++b) {
+            double s = 0.0;
+            for (int i = 0; i < (L - 1) * L; ++i) s += (double)Jv[(size_t)b * (L - 1) * L + i];
+            P->defer[b] = s;
+        }
+
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    auto up = [&](size_t off, const void* src, size_t bytes) -> cudaError_t {
+        if (!bytes) return cudaSuccess;
+        return cudaMemcpyAsync(P->ws + off, src, bytes, cudaMemcpyHostToDevice, st);
+    };
+    cudaError_t e = up(lay.Jh, Jh, nh * 4);
+    if (e == cudaSuccess) e = up(lay.Jv, Jv, nv * 4);
+    if (e == cudaSuccess && h) e = up(lay.h, h, nf * 4);
+    if (e == cudaSuccess) e = up(lay.ops, P->plan.ops.data(), P->plan.ops.size() * sizeof(ttn::Op));
+    if (e != cudaSuccess) { delete P; return fail(TTN_ECUDA, "coupling upload failed: %s", cudaGetErrorString(e)); }
+
+    P->launches = (int)P->plan.passes.size() + (config ? 2 * L : 1);
+    *out = P;
+    return TTN_OK;
+}
+
+ttn_status ttn_plan_launch(ttn_plan* P, void* stream) {
+    if (!P) return fail(TTN_EINVAL, "plan is NULL");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    for (const ttn::Pass& ps : P->plan.passes) {
+        ttn_status s;
+        if (P->q == 2) s = P->count ? launch_pass<2, true>(P, ps, st) : launch_pass<2, false>(P, ps, st);
+        else s = P->count ? launch_pass<3, true>(P, ps, st) : launch_pass<3, false>(P, ps, st);
+        if (s != TTN_OK) return s;
+    }
+    if (P->config) {
+        const Layout& y = P->lay;
+        ttn::ArgmaxParams ap{};
+        ap.L = P->L; ap.NS = y.NS; ap.nblk = y.amax_blocks;
+        ap.c_stride = (unsigned long long)P->L * y.NS;
+        ap.Jv = reinterpret_cast<const float*>(P->ws + y.Jv);
+        ap.s_next = ap.s_out = reinterpret_cast<unsigned long long*>(P->ws + y.out_s);
+        ap.part_v = reinterpret_cast<float*>(P->ws + y.amax_v);
+        ap.part_s = reinterpret_cast<unsigned long long*>(P->ws + y.amax_s);
+        ap.v_out = reinterpret_cast<float*>(P->ws + y.out_x);
+        ap.sigma = reinterpret_cast<signed char*>(P->ws + y.sigma);
+        for (int r = P->L - 1; r >= 0; --r) {
+            ap.r = r; ap.has_next = (r < P->L - 1);
+            ap.C = reinterpret_cast<const float*>(P->ws + y.ckpt) + (unsigned long long)r * y.NS;
+            ttn::argmax_partial_kernel<<<dim3(ap.nblk, P->batch), 256, 0, st>>>(ap);
+            TTN_CUDA(cudaGetLastError());
+            ttn::argmax_final_kernel<<<P->batch, 32, 0, st>>>(ap);
+            TTN_CUDA(cudaGetLastError());
+        }
+    }
+    return TTN_OK;
+}
+
+ttn_status ttn_plan_read(ttn_plan* P, void* stream, double* E0, double* degeneracy, int8_t* sigma) {
+    if (!P) return fail(TTN_EINVAL, "plan is NULL");
+    if (!E0) return fail(TTN_EINVAL, "E0 is NULL");
+    if (P->count && !degeneracy) return fail(TTN_EINVAL, "degeneracy is NULL");
+    if (!P->count && degeneracy) return fail(TTN_EINVAL, "degeneracy given for a non-counting plan");
+    if (P->config && !sigma) return fail(TTN_EINVAL, "sigma is NULL");
+    if (!P->config && sigma) return fail(TTN_EINVAL, "sigma given for a non-config plan");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    std::vector<float> x(P->batch);
+    TTN_CUDA(cudaMemcpyAsync(x.data(), P->ws + P->lay.out_x, (size_t)P->batch * 4, cudaMemcpyDeviceToHost, st));
+    if (P->count)
+        TTN_CUDA(cudaMemcpyAsync(degeneracy, P->ws + P->lay.out_n, (size_t)P->batch * 8, cudaMemcpyDeviceToHost, st));
+    if (P->config)
+        TTN_CUDA(cudaMemcpyAsync(sigma, P->ws + P->lay.sigma, (size_t)P->batch * P->L * P->L, cudaMemcpyDeviceToHost, st));
+    TTN_CUDA(cudaStreamSynchronize(st));
+    for (int b = 0; b < P->batch; ++b) {
+        double m = (double)x[b] + P->defer[b];      // max of -E
+        E0[b] = (m == 0.0) ? 0.0 : -m;              // -0.0 -> +0.0
+    }
+    return TTN_OK;
+}
+
+void ttn_plan_destroy(ttn_plan* P) { delete P; }
+int ttn_plan_num_launches(const ttn_plan* P) { return P ? P->launches : 0; }
+int ttn_plan_num_passes(const ttn_plan* P) { return P ? (int)P->plan.passes.size() : 0; }
+
+}  // extern "C"
+
+static ttn_status one_call(int q, int L, ttn_call call, const float* Jh, const float* Jv, const float* h,
+                           int batch, void* ws, size_t wsb, void* stream, double* E0, double* g, int8_t* sigma) {
+    if (!E0) return fail(TTN_EINVAL, "E0 is NULL");
+    if (call == TTN_CALL_COUNT && !g) return fail(TTN_EINVAL, "degeneracy is NULL");
+    if (call == TTN_CALL_CONFIG && !sigma) return fail(TTN_EINVAL, "sigma is NULL");
+    ttn_plan* P = nullptr;
+    ttn_status s = ttn_plan_create(q, L, call, Jh, Jv, h, batch, ws, wsb, stream, &P);
+    if (s != TTN_OK) return s;
+    s = ttn_plan_launch(P, stream);
+    if (s == TTN_OK) s = ttn_plan_read(P, stream, E0, g, sigma);
+    else cudaStreamSynchronize(static_cast<cudaStream_t>(stream));
+    ttn_plan_destroy(P);
+    return s;
+}
+
+extern "C" {
+
+ttn_status ttn_sweep_energy(int L, const float* Jh, const float* Jv, const float* h, int batch,
+                            void* ws, size_t wsb, void* stream, double* E0) {
+    return one_call(2, L, TTN_CALL_ENERGY, Jh, Jv, h, batch, ws, wsb, stream, E0, nullptr, nullptr);
+}
+ttn_status ttn_sweep_count(int L, const float* Jh, const float* Jv, const float* h, int batch,
+                           void* ws, size_t wsb, void* stream, double* E0, double* g) {
+    return one_call(2, L, TTN_CALL_COUNT, Jh, Jv, h, batch, ws, wsb, stream, E0, g, nullptr);
+}
+ttn_status ttn_ground_config(int L, const float* Jh, const float* Jv, const float* h, int batch,
+                             void* ws, size_t wsb, void* stream, double* E0, int8_t* sigma) {
+    return one_call(2, L, TTN_CALL_CONFIG, Jh, Jv, h, batch, ws, wsb, stream, E0, nullptr, sigma);
+}
+ttn_status ttn_potts3_sweep_energy(int L, const float* Jh, const float* Jv, int batch, void* ws,
+                                   size_t wsb, void* stream, double* E0) {
+    return one_call(3, L, TTN_CALL_ENERGY, Jh, Jv, nullptr, batch, ws, wsb, stream, E0, nullptr, nullptr);
+}
+ttn_status ttn_potts3_sweep_count(int L, const float* Jh, const float* Jv, int batch, void* ws,
+                                  size_t wsb, void* stream, double* E0, double* g) {
+    return one_call(3, L, TTN_CALL_COUNT, Jh, Jv, nullptr, batch, ws, wsb, stream, E0, g, nullptr);
+}
+
+}  // extern "C"

@@ -1,0 +1,56 @@
+"""The C-ABI library builds, loads without a GPU and exports every symbol include/ttn.h declares."""
+import ctypes
+import os
+import re
+
+import pytest
+
+import paper_2008_06888_b200 as ttn
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "ttn.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(ttn_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_header_symbols_are_exported():
+    lib = ttn.lib()
+    names = declared_symbols()
+    assert set(names) == set(ttn.EXPORTS)
+    for n in names:
+        assert hasattr(lib, n), n
+
+
+def test_workspace_bytes_and_argument_errors_without_gpu():
+    # 2^32 f32 state = 16 GiB + tables
+    n = ttn.workspace_bytes(2, 32, ttn.TROPICAL_F32, 1)
+    assert 16 * 2**30 <= n < 16 * 2**30 + 2**26
+    n = ttn.workspace_bytes(2, 24, ttn.COUNTING_F32_F64, 16)
+    assert n >= 16 * 2**24 * 12
+    n = ttn.workspace_bytes(2, 16, ttn.TROPICAL_F32, 256, True)
+    assert n >= 256 * 17 * 2**16 * 4
+    n = ttn.workspace_bytes(3, 18, ttn.COUNTING_F32_F64, 1)
+    assert n >= 3**18 * 12
+    lib = ttn.lib()
+    assert lib.ttn_workspace_bytes(5, 8, 0, 1, 0) == 0
+    assert lib.ttn_workspace_bytes(2, 0, 0, 1, 0) == 0
+    assert lib.ttn_workspace_bytes(2, 40, 0, 1, 0) == 0
+    assert lib.ttn_workspace_bytes(3, 21, 0, 1, 0) == 0
+    assert lib.ttn_workspace_bytes(2, 8, 0, 0, 0) == 0
+    # NULL arguments are rejected before any CUDA call
+    e0 = (ctypes.c_double * 1)()
+    st = lib.ttn_sweep_energy(4, None, None, None, 1, None, 0, None, e0)
+    assert st == 1 and b"NULL" in lib.ttn_last_error()
+    assert lib.ttn_version() >= 100
+
+
+def test_no_cpu_fallback():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    import numpy as np
+    with pytest.raises(ttn.TTNError):
+        ttn.sweep_energy(np.ones((3, 2)), np.ones((2, 3)))

@@ -1,0 +1,180 @@
+"""Host logic: the pass schedule (csrc/planner.h, dumped by ttn_plan_describe) is replayed
+(1) against an independent statement of the dependency rule of SURVEY.md 8a-S8
+    (derived from PAPER.md:118 "order ... can be arbitrary" + non-commutation of a gate with
+    anything that reads its digit), and
+(2) numerically, op by op in numpy (float64 + integer counts), against the CPU oracle.
+No GPU is needed: this checks what the kernels are told to do, not the kernels.
+"""
+import os
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_2008_06888_b200 as ttn
+from ttn_inputs import make_instance
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def describe(q, L, call, tmax=None, ride=None):
+    """Run ttn_plan_describe in a subprocess so the debug tile overrides can be set."""
+    env = dict(os.environ)
+    if tmax is not None:
+        env["TTN_DEBUG_TMAX"] = str(tmax)
+    if ride is not None:
+        env["TTN_DEBUG_RIDE"] = str(ride)
+    code = ("import paper_2008_06888_b200 as t, sys; "
+            f"sys.stdout.write(t.plan_describe({q}, {L}, {call}))")
+    return subprocess.check_output([sys.executable, "-c", code], cwd=ROOT, env=env, text=True)
+
+
+def parse(txt):
+    head, passes = None, []
+    for line in txt.splitlines():
+        w = line.split()
+        if w[0] == "plan":
+            head = dict(kv.split("=") for kv in w[1:])
+        elif w[0] == "pass":
+            d = {k: int(v) for k, v in (kv.split("=") for kv in w[2:])}
+            d["ops"] = []
+            passes.append(d)
+        elif w[0] == "op":
+            d = {k: int(v) for k, v in (kv.split("=") for kv in w[2:])}
+            d["type"] = w[1]
+            passes[-1]["ops"].append(d)
+    return head, passes
+
+
+def validate(q, L, passes, fields, row_aligned):
+    g = np.zeros((L, L), dtype=int); g[0, :] = 1          # row 0 needs no gate
+    dh = np.zeros((L, L), dtype=int)
+    dJ = np.zeros((L, max(L - 1, 0)), dtype=int)
+    if not fields:
+        dh[:] = 1
+    rows_done = 0
+    for i, ps in enumerate(passes):
+        lo, a, b = ps["lo"], ps["a"], ps["b"]
+        assert 0 <= lo <= a <= b <= L
+        tile = list(range(lo)) + list(range(a, b))
+        assert len(tile) == len(set(tile)) and len(tile) >= 1
+        assert (ps["flags"] & 1) == (1 if i == 0 else 0)          # INIT only on the first pass
+        for op in ps["ops"]:
+            r, c = op["r"], op["c"]
+            if op["type"] == "g":
+                assert c in tile and tile.index(c) == op["pos"]
+                assert 1 <= r < L and g[r, c] == 0 and g[r - 1, c] == 1
+                assert dh[r - 1, c] == 1
+                if c > 0: assert dJ[r - 1, c - 1] == 1
+                if c < L - 1: assert dJ[r - 1, c] == 1
+                g[r, c] = 1
+            elif op["type"] == "dh":
+                assert fields and dh[r, c] == 0 and g[r, c] == 1
+                assert r == L - 1 or g[r + 1, c] == 0
+                dh[r, c] = 1
+            else:
+                assert dJ[r, c] == 0 and g[r, c] == 1 and g[r, c + 1] == 1
+                assert r == L - 1 or (g[r + 1, c] == 0 and g[r + 1, c + 1] == 0)
+                dJ[r, c] = 1
+        if row_aligned:
+            full = lambda r: g[r].all() and dh[r].all() and dJ[r].all()
+            if rows_done < L and full(rows_done):
+                assert ps["dst"] == rows_done
+                rows_done += 1
+            else:
+                assert ps["dst"] == -1
+            if i > 0:
+                assert ps["src"] == passes[i - 1]["dst"]
+    assert g.all() and dh.all() and dJ.all()
+    if row_aligned:
+        assert rows_done == L
+    else:
+        assert passes[-1]["flags"] & 2 and all(not (p["flags"] & 2) for p in passes[:-1])
+
+
+@pytest.mark.parametrize("q,L,call", [(2, 32, 0), (2, 24, 1), (2, 16, 2), (3, 18, 1), (3, 18, 0),
+                                      (2, 4, 1), (2, 1, 0), (2, 28, 0), (2, 30, 0), (2, 20, 2),
+                                      (3, 12, 0), (2, 34, 0), (2, 15, 0), (2, 14, 1)])
+def test_schedule_obeys_dependency_rule(q, L, call):
+    head, passes = parse(ttn.plan_describe(q, L, call))
+    assert int(head["L"]) == L and int(head["q"]) == q
+    validate(q, L, passes, fields=(q == 2), row_aligned=(call == 2))
+
+
+def test_fusion_cuts_hbm_passes():
+    # cross-row fusion brings L=32 from 3 passes per row (93) to ~0.5 per row
+    _, passes = parse(ttn.plan_describe(2, 32, 0))
+    assert len(passes) <= 18
+    _, passes = parse(ttn.plan_describe(2, 24, 1))
+    assert len(passes) <= 12
+
+
+# ------------------------------------------------------------------------------- numeric replay
+def digits(q, L):
+    s = np.arange(q ** L)
+    return [(s // q ** c) % q for c in range(L)]
+
+
+def replay(q, L, passes, Jh, Jv, h):
+    """Apply the op list to the full state in numpy: x float64, n Python-int (object) counts."""
+    N = q ** L
+    x = np.zeros(N); n = np.ones(N, dtype=object)
+    dig = digits(q, L)
+    idx = np.arange(N)
+    defer = 0.0
+    for ps in passes:
+        for op in ps["ops"]:
+            r, c = op["r"], op["c"]
+            if op["type"] == "dh":
+                if h is not None:
+                    x += h[r, c] * (1 - 2 * dig[c])
+            elif op["type"] == "dJ":
+                if q == 2:
+                    x += Jh[r, c] * (1 - 2 * dig[c]) * (1 - 2 * dig[c + 1])
+                else:
+                    x += Jh[r, c] * (dig[c] == dig[c + 1])
+            else:
+                J = Jv[r - 1, c]
+                st = q ** c
+                base = idx[dig[c] == 0]
+                olds = [(x[base + t * st].copy(), n[base + t * st].copy()) for t in range(q)]
+                for tn in range(q):
+                    bx = None
+                    for t in range(q):
+                        w = J * (1 - 2 * t) * (1 - 2 * tn) if q == 2 else J * (t == tn)
+                        cx, cn = olds[t][0] + w, olds[t][1]
+                        if bx is None:
+                            bx, bn = cx.copy(), cn.copy()
+                        else:
+                            gt, eq = cx > bx, cx == bx
+                            bn = np.where(gt, cn, np.where(eq, bn + cn, bn))
+                            bx = np.maximum(bx, cx)
+                    x[base + tn * st] = bx; n[base + tn * st] = bn
+    m = x.max()
+    return (0.0 if m == 0 else -m), int(sum(n[x == m]))
+
+
+@pytest.mark.parametrize("q,L,call,tmax,ride", [
+    (2, 8, 1, 5, 2), (2, 9, 0, 4, 1), (2, 7, 1, 3, 1), (2, 10, 1, 6, 3), (2, 6, 2, 4, 2),
+    (3, 6, 1, 3, 1), (3, 5, 1, 2, 1), (3, 7, 0, 4, 2), (2, 8, 1, 13, 3),
+])
+def test_schedule_replay_matches_oracle(q, L, call, tmax, ride):
+    head, passes = parse(describe(q, L, call, tmax, ride))
+    validate(q, L, passes, fields=(q == 2), row_aligned=(call == 2))
+    if tmax < L:
+        assert len(passes) > 1
+    for seed in range(3):
+        if q == 2:
+            rng = np.random.default_rng(seed)
+            Jh = rng.integers(-2, 3, size=(L, L - 1)).astype(float)
+            Jv = rng.integers(-2, 3, size=(L - 1, L)).astype(float)
+            h = rng.integers(-1, 2, size=(L, L)).astype(float)
+            E0, g = replay(q, L, passes, Jh, Jv, h)
+            Eo, go, _ = oracle.dp_ising(L, Jh, Jv, h)
+        else:
+            inst = make_instance(L, 900 + seed, "pmj", q=3)
+            E0, g = replay(q, L, passes, inst.Jh, inst.Jv, None)
+            Eo, go, _ = oracle.dp_potts3(L, inst.Jh, inst.Jv)
+        assert (E0, g) == (Eo, go)
