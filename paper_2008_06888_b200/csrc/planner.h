@@ -150,7 +150,7 @@ inline Plan make_plan(int q, int L, bool has_field, bool row_aligned, int Tmax, 
         Scheduler s(L, has_field);
         size_t k = 0; int row = 0; bool first = true; int idle = 0;
         int cur_src = -1;
-        while (!s.done()) {
+        while (first || !s.done()) {   // the INIT pass exists even when there is nothing to apply
             const TileSpec& t = cyc[k % cyc.size()]; ++k;
             Pass ps{t.lo, t.a, t.b, (int)p.ops.size(), 0, 0, -1, -1, 0};
             ps.n_gates = s.run_pass(t, row_aligned ? row : L, p.ops);
