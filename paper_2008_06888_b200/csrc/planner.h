@@ -194,4 +194,245 @@ inline std::string describe(const Plan& p) {
     return out;
 }
 
+
+// =============================================================================================
+// Fused register-phase schedule ("v2", Ising Tropical<f32>).
+//
+// A pass gives every WARP a tile of W = 11 active digits [a, a+11) = 2^11 elements, 64 per
+// thread.  Inside a pass the warp alternates between two register layouts,
+//     A : register digits d0..d5,  lane digits d6..d10
+//     B : register digits d5..d10, lane digits d0..d4          (d_i = column a + i)
+// exchanging through its private shared-memory region.  In a layout, a gate on a register
+// digit is pure register arithmetic.  Diagonal terms are applied as small tables over the 64
+// register combinations (one FADD per element per table); a term can go into a table only if
+// each of its digits is a register digit or the tile's outer neighbour column (a-1 or a+11,
+// constant per warp: the table has one variant per value of that digit).  d5 is a register
+// digit in both layouts so that every in-tile pair (c, c+1) sits inside some layout.
+// The same dependency rule as above decides what is legal; phases are filled greedily.
+// =============================================================================================
+enum MicroCode : uint8_t { MC_END = 0, MC_LOAD_A = 1, MC_LOAD_B = 2, MC_STORE_A = 3, MC_STORE_B = 4,
+                           MC_GATE = 5, MC_TABLE = 6 };
+
+struct MicroOp { uint8_t code; uint8_t k; uint16_t arg; };   // GATE: k = register bit, arg = index
+                                                             // into the pass's gate list; TABLE: arg
+                                                             // = table index inside the pass
+struct TableTerm {        // one diagonal term of a table
+    uint8_t type;         // OP_DH / OP_DJ
+    uint8_t posA, posB;   // bit position (0..5) in the register index, or 6 = the outer neighbour
+    uint8_t pad;
+    uint16_t row, col;    // lattice row, (left) column
+};
+
+struct FusedTable { int term_begin, term_end; int layout; };   // layout 0 = A (outer = a-1), 1 = B (outer = a+W)
+
+struct FusedPass {
+    int a;                       // active digits [a, a+W)
+    int ride;                    // riding low digits (0 for the low tile)
+    int flags;
+    int mop_begin, mop_end;      // into FusedPlan::mops
+    int gate_begin, gate_end;    // into FusedPlan::gate_jv (index into Jv[(r-1)*L + c])
+    int table_begin, table_end;  // into FusedPlan::tables
+    int n_phases;
+};
+
+struct FusedPlan {
+    int L = 0, W = 11;
+    std::vector<FusedPass> passes;
+    std::vector<MicroOp> mops;
+    std::vector<int> gate_jv;
+    std::vector<FusedTable> tables;
+    std::vector<TableTerm> terms;
+    bool ok = false;
+};
+
+class FusedScheduler {
+  public:
+    FusedScheduler(int L, bool has_field, FusedPlan& p) : L_(L), P_(p), grow_(L, 1), dh_(L * L, 0),
+        dj_(L * (L > 1 ? L - 1 : 1), 0) { if (!has_field) for (auto& x : dh_) x = 1; }
+    bool done() const {
+        for (int c = 0; c < L_; ++c) if (grow_[c] != L_) return false;
+        for (auto x : dh_) if (!x) return false;
+        for (int r = 0; r < L_; ++r) for (int c = 0; c + 1 < L_; ++c) if (!dj_[r * (L_ - 1) + c]) return false;
+        return true;
+    }
+    // One pass over active digits [a, a+W).  Returns number of ops applied (gates + terms).
+    int run_pass(int a, int W, int ride, FusedPass& ps) {
+        ps.a = a; ps.ride = ride; ps.flags = 0; ps.n_phases = 0;
+        ps.mop_begin = (int)P_.mops.size(); ps.gate_begin = (int)P_.gate_jv.size();
+        ps.table_begin = (int)P_.tables.size();
+        int total = 0, idle = 0, layout = pick_first_layout(a, W);
+        while (idle < 2) {
+            size_t mark = P_.mops.size();
+            P_.mops.push_back({(uint8_t)(layout == 0 ? MC_LOAD_A : MC_LOAD_B), 0, 0});
+            int n = run_phase(a, W, layout);
+            if (n == 0) { P_.mops.resize(mark); ++idle; }
+            else {
+                P_.mops.push_back({(uint8_t)(layout == 0 ? MC_STORE_A : MC_STORE_B), 0, 0});
+                total += n; idle = 0; ++ps.n_phases;
+            }
+            layout ^= 1;
+        }
+        P_.mops.push_back({MC_END, 0, 0});
+        ps.mop_end = (int)P_.mops.size(); ps.gate_end = (int)P_.gate_jv.size();
+        ps.table_end = (int)P_.tables.size();
+        return total;
+    }
+  private:
+    // register digit i of layout -> tile digit index
+    static int rdig(int layout, int i) { return layout == 0 ? i : 5 + i; }
+    int count_legal(int a, int W, int layout) {   // how many gates are legal right now (ignoring pending tables)
+        int n = 0;
+        for (int i = 0; i < 6; ++i) { int c = a + rdig(layout, i); if (c < a + W && grow_[c] < L_) ++n; }
+        return n;
+    }
+    int pick_first_layout(int, int) { return 0; }
+    // position of column c in the register index of this layout: 0..5, 6 = outer neighbour, -1 = no
+    int pos_in(int a, int W, int layout, int c) const {
+        for (int i = 0; i < 6; ++i) if (a + rdig(layout, i) == c) return i;
+        if (layout == 0 && c == a - 1) return 6;
+        if (layout == 1 && c == a + W) return 6;
+        return -1;
+    }
+    int run_phase(int a, int W, int layout) {
+        int n = 0; bool progress = true;
+        while (progress) {
+            progress = false;
+            // ---- a table with every diagonal term that is legal and expressible here -----------
+            int tb = (int)P_.terms.size();
+            for (int i = 0; i < 6; ++i) {
+                int c = a + rdig(layout, i);
+                int r = grow_[c] - 1;
+                if (!dh_[r * L_ + c]) {
+                    dh_[r * L_ + c] = 1;
+                    P_.terms.push_back({OP_DH, (uint8_t)i, 0, 0, (uint16_t)r, (uint16_t)c});
+                }
+                for (int cc = c - 1; cc <= c; ++cc) {
+                    if (cc < 0 || cc + 1 >= L_) continue;
+                    int pa = pos_in(a, W, layout, cc), pb = pos_in(a, W, layout, cc + 1);
+                    if (pa < 0 || pb < 0 || (pa == 6 && pb == 6)) continue;
+                    if (grow_[cc] != grow_[cc + 1]) continue;
+                    int rr = grow_[cc] - 1;
+                    if (dj_[rr * (L_ - 1) + cc]) continue;
+                    dj_[rr * (L_ - 1) + cc] = 1;
+                    P_.terms.push_back({OP_DJ, (uint8_t)pa, (uint8_t)pb, 0, (uint16_t)rr, (uint16_t)cc});
+                }
+            }
+            if ((int)P_.terms.size() > tb) {
+                P_.tables.push_back({tb, (int)P_.terms.size(), layout});
+                int local = (int)P_.tables.size() - 1 - cur_table_begin();
+                P_.mops.push_back({MC_TABLE, (uint8_t)layout, (uint16_t)local});
+                n += (int)P_.terms.size() - tb; progress = true;
+            }
+            // ---- every legal gate on a register digit ----------------------------------------------
+            for (int i = 0; i < 6; ++i) {
+                int c = a + rdig(layout, i);
+                int r = grow_[c];
+                if (r >= L_) continue;
+                bool ok = dh_[(r - 1) * L_ + c] != 0;
+                if (c > 0) ok = ok && dj_[(r - 1) * (L_ - 1) + c - 1];
+                if (c + 1 < L_) ok = ok && dj_[(r - 1) * (L_ - 1) + c];
+                if (!ok) continue;
+                grow_[c] += 1;
+                int local = (int)P_.gate_jv.size() - cur_gate_begin();
+                P_.gate_jv.push_back((r - 1) * L_ + c);
+                P_.mops.push_back({MC_GATE, (uint8_t)i, (uint16_t)local});
+                ++n; progress = true;
+            }
+        }
+        return n;
+    }
+    int cur_table_begin() const { return pass_table_begin_; }
+    int cur_gate_begin() const { return pass_gate_begin_; }
+  public:
+    void begin_pass() { pass_table_begin_ = (int)P_.tables.size(); pass_gate_begin_ = (int)P_.gate_jv.size(); }
+  private:
+    int L_; FusedPlan& P_;
+    std::vector<int> grow_;
+    std::vector<uint8_t> dh_, dj_;
+    int pass_table_begin_ = 0, pass_gate_begin_ = 0;
+};
+
+// Tile starts: 0, then advancing by `stride`, the last flush with L.  High tiles (a > 0) need
+// a >= ride.  Chooses the stride with the fewest passes (ties: fewest phases).
+inline FusedPlan make_fused_plan(int L, bool has_field, int ride) {
+    const int W = 11;
+    FusedPlan best;
+    if (L < W + ride) return best;
+    long best_cost = -1;
+    for (int stride = 1; stride <= W; ++stride) {
+        std::vector<int> starts;
+        starts.push_back(0);
+        if (L > W) {
+            int x = stride;
+            for (;;) {
+                if (x + W >= L) x = L - W;
+                if (x < ride) x = ride;
+                starts.push_back(x);
+                if (x + W >= L) break;
+                x += stride;
+            }
+        }
+        FusedPlan p; p.L = L; p.W = W;
+        FusedScheduler s(L, has_field, p);
+        size_t k = 0; int idle = 0; bool first = true;
+        while ((first || !s.done()) && p.passes.size() < 4096) {
+            int a = starts[k % starts.size()]; ++k;
+            FusedPass ps{};
+            s.begin_pass();
+            size_t m0 = p.mops.size();
+            int n = s.run_pass(a, W, a == 0 ? 0 : ride, ps);
+            if (n == 0 && !first) { p.mops.resize(m0); if (++idle > (int)starts.size()) break; continue; }
+            idle = 0;
+            if (first) ps.flags |= PASS_INIT;
+            first = false;
+            p.passes.push_back(ps);
+        }
+        if (!s.done()) continue;
+        p.passes.back().flags |= PASS_REDUCE;
+        long phases = 0; for (auto& ps : p.passes) phases += ps.n_phases;
+        long cost = (long)p.passes.size() * 1000 + phases;
+        if (best_cost < 0 || cost < best_cost) { best = p; best_cost = cost; best.ok = true; }
+    }
+    return best;
+}
+
+inline std::string describe_fused(const FusedPlan& p) {
+    std::string out; char line[200];
+    snprintf(line, sizeof line, "fused L=%d W=%d passes=%zu mops=%zu gates=%zu tables=%zu terms=%zu\n", p.L, p.W,
+             p.passes.size(), p.mops.size(), p.gate_jv.size(), p.tables.size(), p.terms.size());
+    out += line;
+    for (size_t i = 0; i < p.passes.size(); ++i) {
+        const FusedPass& ps = p.passes[i];
+        snprintf(line, sizeof line, "fpass %zu a=%d ride=%d flags=%d phases=%d gates=%d tables=%d\n", i, ps.a, ps.ride,
+                 ps.flags, ps.n_phases, ps.gate_end - ps.gate_begin, ps.table_end - ps.table_begin);
+        out += line;
+        for (int k = ps.mop_begin; k < ps.mop_end; ++k) {
+            const MicroOp& m = p.mops[k];
+            switch (m.code) {
+                case MC_LOAD_A: out += "m loadA\n"; break;
+                case MC_LOAD_B: out += "m loadB\n"; break;
+                case MC_STORE_A: out += "m storeA\n"; break;
+                case MC_STORE_B: out += "m storeB\n"; break;
+                case MC_END: out += "m end\n"; break;
+                case MC_GATE: {
+                    int jv = p.gate_jv[ps.gate_begin + m.arg];
+                    snprintf(line, sizeof line, "m gate k=%d r=%d c=%d\n", m.k, jv / p.L + 1, jv % p.L);
+                    out += line; break; }
+                case MC_TABLE: {
+                    const FusedTable& t = p.tables[ps.table_begin + m.arg];
+                    snprintf(line, sizeof line, "m table layout=%d nterms=%d\n", t.layout, t.term_end - t.term_begin);
+                    out += line;
+                    for (int q = t.term_begin; q < t.term_end; ++q) {
+                        const TableTerm& tt = p.terms[q];
+                        snprintf(line, sizeof line, "t %s r=%d c=%d pa=%d pb=%d\n", tt.type == OP_DH ? "dh" : "dJ",
+                                 tt.row, tt.col, tt.posA, tt.posB);
+                        out += line;
+                    }
+                    break; }
+            }
+        }
+    }
+    return out;
+}
+
 }  // namespace ttn

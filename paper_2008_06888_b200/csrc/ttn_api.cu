@@ -14,6 +14,7 @@
 #include "../../include/ttn.h"
 #include "planner.h"
 #include "ttn_kernels.cuh"
+#include "ttn_fused.cuh"
 
 namespace {
 
@@ -69,9 +70,17 @@ bool limits_ok(int q, int L, bool count, bool config) {
 struct Layout {
     size_t x = 0, n = 0, ckpt = 0, Jh = 0, Jv = 0, h = 0, ops = 0, part_x = 0, part_n = 0,
            amax_v = 0, amax_s = 0, out_x = 0, out_n = 0, out_s = 0, sigma = 0, total = 0;
+    size_t f_mops = 0, f_gate_jv = 0, f_tables = 0, f_terms = 0, f_gate_m = 0, f_table_vals = 0;
     unsigned long long NS = 0, max_tiles = 0;
     int amax_blocks = 0;
+    int f_max_gates = 0, f_max_tables = 0, f_max_terms = 0, f_max_mops = 0;
 };
+
+// The fused register-phase path serves the Ising Tropical<f32> energy sweep for L >= 14.
+bool fused_eligible(int q, int L, bool count, bool config) {
+    if (const char* e = getenv("TTN_DEBUG_FUSED")) if (atoi(e) == 0) return false;
+    return q == 2 && !count && !config && L >= ttn::FW + ttn::FRIDE;
+}
 
 // The op list length is bounded by L*L gates + 2*L*L diagonals.
 Layout make_layout(int q, int L, bool count, bool config, int batch) {
@@ -100,6 +109,15 @@ Layout make_layout(int q, int L, bool count, bool config, int batch) {
     y.out_n = take((size_t)batch * 8);
     y.out_s = take((size_t)batch * 8);
     y.sigma = take((size_t)batch * L * L);
+    if (fused_eligible(q, L, count, config)) {
+        y.f_max_gates = L * L; y.f_max_tables = 3 * L * L; y.f_max_terms = 2 * L * L; y.f_max_mops = 8 * L * L + 64;
+        y.f_mops = take((size_t)y.f_max_mops * sizeof(ttn::MicroOp));
+        y.f_gate_jv = take((size_t)y.f_max_gates * 4);
+        y.f_tables = take((size_t)y.f_max_tables * sizeof(ttn::FusedTable));
+        y.f_terms = take((size_t)y.f_max_terms * sizeof(ttn::TableTerm));
+        y.f_gate_m = take((size_t)batch * y.f_max_gates * 4);
+        y.f_table_vals = take((size_t)batch * y.f_max_tables * 128 * 4);
+    }
     y.total = off;
     return y;
 }
@@ -117,6 +135,9 @@ struct ttn_plan {
     ttn_call call;
     bool count, config, has_field;
     ttn::Plan plan;
+    ttn::FusedPlan fplan;
+    bool fused = false;
+    int fused_grid = 0;
     Layout lay;
     unsigned char* ws;
     std::vector<double> defer;     // per instance: sum of the +J constants factored out of the gates
@@ -172,6 +193,75 @@ static ttn_status launch_pass(const ttn_plan* P, const ttn::Pass& ps, cudaStream
     return TTN_OK;
 }
 
+static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps, cudaStream_t st) {
+    const Layout& y = P->lay;
+    const ttn::FusedPlan& fp = P->fplan;
+    ttn::FusedParams pp{};
+    pp.L = P->L; pp.a = ps.a; pp.ride = ps.ride; pp.flags = ps.flags;
+    pp.state = reinterpret_cast<float*>(P->ws + y.x);
+    pp.inst_stride = y.NS;
+    pp.tiles_per_inst = y.NS >> 14;
+    pp.total_tiles = pp.tiles_per_inst * (unsigned long long)P->batch;
+    pp.mops = reinterpret_cast<const ttn::MicroOp*>(P->ws + y.f_mops) + ps.mop_begin;
+    pp.n_mops = ps.mop_end - ps.mop_begin;
+    pp.gate_m = reinterpret_cast<const float*>(P->ws + y.f_gate_m) + ps.gate_begin;
+    pp.n_gates = ps.gate_end - ps.gate_begin;
+    pp.gate_inst_stride = (int)fp.gate_jv.size();
+    pp.tables = reinterpret_cast<const float*>(P->ws + y.f_table_vals) + (size_t)ps.table_begin * 128;
+    pp.table_inst_stride = (unsigned long long)fp.tables.size() * 128;
+    pp.part_x = reinterpret_cast<float*>(P->ws + y.part_x);
+    const size_t smem = (size_t)(ttn::FWARPS * ttn::FREGION + ttn::FMAX_GATES) * 4 + ttn::FMAX_MOPS * sizeof(ttn::MicroOp);
+    unsigned long long grid = (unsigned long long)P->fused_grid;
+    if (grid > pp.total_tiles) grid = pp.total_tiles;
+    ttn::fused_pass_kernel<<<(unsigned)grid, ttn::FWARPS * 32, smem, st>>>(pp);
+    TTN_CUDA(cudaGetLastError());
+    if (ps.flags & ttn::PASS_REDUCE) {
+        ttn::final_reduce_kernel<false><<<P->batch, 256, 0, st>>>(
+            pp.part_x, nullptr, pp.tiles_per_inst, reinterpret_cast<float*>(P->ws + y.out_x), nullptr);
+        TTN_CUDA(cudaGetLastError());
+    }
+    return TTN_OK;
+}
+
+// Uploads the fused program and runs the S0 prep kernel (gate constants + diagonal tables).
+static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
+    const Layout& y = P->lay;
+    ttn::FusedPlan& fp = P->fplan;
+    if ((int)fp.gate_jv.size() > y.f_max_gates || (int)fp.tables.size() > y.f_max_tables ||
+        (int)fp.terms.size() > y.f_max_terms || (int)fp.mops.size() > y.f_max_mops)
+        return fail(TTN_EUNSUPPORTED, "fused plan exceeds its workspace bounds");
+    for (const auto& ps : fp.passes)
+        if (ps.mop_end - ps.mop_begin > ttn::FMAX_MOPS || ps.gate_end - ps.gate_begin > ttn::FMAX_GATES)
+            return fail(TTN_EUNSUPPORTED, "fused pass program too long");
+    TTN_CUDA(cudaMemcpyAsync(P->ws + y.f_mops, fp.mops.data(), fp.mops.size() * sizeof(ttn::MicroOp), cudaMemcpyHostToDevice, st));
+    TTN_CUDA(cudaMemcpyAsync(P->ws + y.f_gate_jv, fp.gate_jv.data(), fp.gate_jv.size() * 4, cudaMemcpyHostToDevice, st));
+    TTN_CUDA(cudaMemcpyAsync(P->ws + y.f_tables, fp.tables.data(), fp.tables.size() * sizeof(ttn::FusedTable), cudaMemcpyHostToDevice, st));
+    TTN_CUDA(cudaMemcpyAsync(P->ws + y.f_terms, fp.terms.data(), fp.terms.size() * sizeof(ttn::TableTerm), cudaMemcpyHostToDevice, st));
+    ttn::FusedPrepParams q{};
+    q.L = P->L; q.n_gates = (int)fp.gate_jv.size(); q.n_tables = (int)fp.tables.size();
+    q.gate_jv = reinterpret_cast<const int*>(P->ws + y.f_gate_jv);
+    q.tables = reinterpret_cast<const ttn::FusedTable*>(P->ws + y.f_tables);
+    q.terms = reinterpret_cast<const ttn::TableTerm*>(P->ws + y.f_terms);
+    q.Jh = reinterpret_cast<const float*>(P->ws + y.Jh);
+    q.Jv = reinterpret_cast<const float*>(P->ws + y.Jv);
+    q.h = P->has_field ? reinterpret_cast<const float*>(P->ws + y.h) : nullptr;
+    q.gate_m = reinterpret_cast<float*>(P->ws + y.f_gate_m);
+    q.table_out = reinterpret_cast<float*>(P->ws + y.f_table_vals);
+    long work = (long)q.n_tables * 128; if (q.n_gates > work) work = q.n_gates;
+    dim3 grid((unsigned)((work + 255) / 256), (unsigned)P->batch);
+    ttn::fused_prep_kernel<<<grid, 256, 0, st>>>(q);
+    TTN_CUDA(cudaGetLastError());
+    const size_t smem = (size_t)(ttn::FWARPS * ttn::FREGION + ttn::FMAX_GATES) * 4 + ttn::FMAX_MOPS * sizeof(ttn::MicroOp);
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int dev = 0, sms = 0, per_sm = 0;
+    TTN_CUDA(cudaGetDevice(&dev));
+    TTN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    TTN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ttn::fused_pass_kernel, ttn::FWARPS * 32, smem));
+    if (per_sm < 1) return fail(TTN_ECUDA, "fused kernel does not fit on an SM");
+    P->fused_grid = sms * per_sm;
+    return TTN_OK;
+}
+
 extern "C" {
 
 const char* ttn_last_error(void) { return g_err; }
@@ -187,7 +277,12 @@ size_t ttn_workspace_bytes(int q, int L, ttn_semiring mode, int batch, int want_
 long ttn_plan_describe(int q, int L, ttn_call call, char* buf, size_t n) {
     if ((q != 2 && q != 3) || !buf || n == 0) return -1;
     if (!limits_ok(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) return -1;
-    std::string s = ttn::describe(plan_for(q, L, call, /*has_field=*/q == 2));
+    std::string s;
+    if (fused_eligible(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) {
+        ttn::FusedPlan fp = ttn::make_fused_plan(L, /*has_field=*/true, ttn::FRIDE);
+        if (fp.ok) s = ttn::describe_fused(fp);
+    }
+    if (s.empty()) s = ttn::describe(plan_for(q, L, call, /*has_field=*/q == 2));
     size_t m = s.size() < n - 1 ? s.size() : n - 1;
     memcpy(buf, s.data(), m);
     buf[m] = 0;
@@ -227,10 +322,14 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     if (!P) return fail(TTN_ENOMEM, "host allocation failed");
     P->q = q; P->L = L; P->batch = batch; P->call = call; P->count = count; P->config = config;
     P->has_field = (h != nullptr);
-    P->plan = plan_for(q, L, call, P->has_field);
     P->lay = lay;
     P->ws = static_cast<unsigned char*>(workspace);
-    if (P->plan.passes.empty()) { delete P; return fail(TTN_EUNSUPPORTED, "planner produced no schedule"); }
+    if (fused_eligible(q, L, count, config)) {
+        P->fplan = ttn::make_fused_plan(L, P->has_field, ttn::FRIDE);
+        P->fused = P->fplan.ok;
+    }
+    if (!P->fused) P->plan = plan_for(q, L, call, P->has_field);
+    if (!P->fused && P->plan.passes.empty()) { delete P; return fail(TTN_EUNSUPPORTED, "planner produced no schedule"); }
     if (P->plan.ops.size() > (size_t)(3 * L * L + 8)) { delete P; return fail(TTN_EUNSUPPORTED, "op list too long"); }
 
     // the +J constants factored out of the Ising gates (kernel comment at OP_GATE), in f64
@@ -253,7 +352,13 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     if (e == cudaSuccess) e = up(lay.ops, P->plan.ops.data(), P->plan.ops.size() * sizeof(ttn::Op));
     if (e != cudaSuccess) { delete P; return fail(TTN_ECUDA, "coupling upload failed: %s", cudaGetErrorString(e)); }
 
-    P->launches = (int)P->plan.passes.size() + (config ? 2 * L : 1);
+    if (P->fused) {
+        ttn_status fs = setup_fused(P, st);
+        if (fs != TTN_OK) { delete P; return fs; }
+        P->launches = (int)P->fplan.passes.size() + 1;
+    } else {
+        P->launches = (int)P->plan.passes.size() + (config ? 2 * L : 1);
+    }
     *out = P;
     return TTN_OK;
 }
@@ -261,6 +366,13 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
 ttn_status ttn_plan_launch(ttn_plan* P, void* stream) {
     if (!P) return fail(TTN_EINVAL, "plan is NULL");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (P->fused) {
+        for (const ttn::FusedPass& ps : P->fplan.passes) {
+            ttn_status s = launch_fused_pass(P, ps, st);
+            if (s != TTN_OK) return s;
+        }
+        return TTN_OK;
+    }
     for (const ttn::Pass& ps : P->plan.passes) {
         ttn_status s;
         if (P->q == 2) s = P->count ? launch_pass<2, true>(P, ps, st) : launch_pass<2, false>(P, ps, st);
@@ -314,7 +426,7 @@ ttn_status ttn_plan_read(ttn_plan* P, void* stream, double* E0, double* degenera
 
 void ttn_plan_destroy(ttn_plan* P) { delete P; }
 int ttn_plan_num_launches(const ttn_plan* P) { return P ? P->launches : 0; }
-int ttn_plan_num_passes(const ttn_plan* P) { return P ? (int)P->plan.passes.size() : 0; }
+int ttn_plan_num_passes(const ttn_plan* P) { return P ? (int)(P->fused ? P->fplan.passes.size() : P->plan.passes.size()) : 0; }
 
 }  // extern "C"
 

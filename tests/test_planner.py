@@ -19,9 +19,10 @@ from ttn_inputs import make_instance
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def describe(q, L, call, tmax=None, ride=None):
+def describe(q, L, call, tmax=None, ride=None, fused=False):
     """Run ttn_plan_describe in a subprocess so the debug tile overrides can be set."""
     env = dict(os.environ)
+    env["TTN_DEBUG_FUSED"] = "1" if fused else "0"
     if tmax is not None:
         env["TTN_DEBUG_TMAX"] = str(tmax)
     if ride is not None:
@@ -98,17 +99,111 @@ def validate(q, L, passes, fields, row_aligned):
                                       (2, 4, 1), (2, 1, 0), (2, 28, 0), (2, 30, 0), (2, 20, 2),
                                       (3, 12, 0), (2, 34, 0), (2, 15, 0), (2, 14, 1)])
 def test_schedule_obeys_dependency_rule(q, L, call):
-    head, passes = parse(ttn.plan_describe(q, L, call))
+    head, passes = parse(describe(q, L, call))
     assert int(head["L"]) == L and int(head["q"]) == q
     validate(q, L, passes, fields=(q == 2), row_aligned=(call == 2))
 
 
 def test_fusion_cuts_hbm_passes():
     # cross-row fusion brings L=32 from 3 passes per row (93) to ~0.5 per row
-    _, passes = parse(ttn.plan_describe(2, 32, 0))
+    _, passes = parse(describe(2, 32, 0))
     assert len(passes) <= 18
-    _, passes = parse(ttn.plan_describe(2, 24, 1))
+    _, passes = parse(describe(2, 24, 1))
     assert len(passes) <= 12
+    head, fpasses = parse_fused(describe(2, 32, 0, fused=True))
+    assert len(fpasses) <= 20
+
+
+# ------------------------------------------------------------------ fused register-phase schedule
+W = 11
+
+
+def parse_fused(txt):
+    head, passes = None, []
+    for line in txt.splitlines():
+        w = line.split()
+        if w[0] == "fused":
+            head = dict(kv.split("=") for kv in w[1:])
+        elif w[0] == "fpass":
+            d = {k: int(v) for k, v in (kv.split("=") for kv in w[2:])}
+            d["mops"] = []
+            passes.append(d)
+        elif w[0] == "m":
+            d = {"code": w[1]}
+            d.update({k: int(v) for k, v in (kv.split("=") for kv in w[2:])})
+            d["terms"] = []
+            passes[-1]["mops"].append(d)
+        elif w[0] == "t":
+            d = {"type": w[1]}
+            d.update({k: int(v) for k, v in (kv.split("=") for kv in w[2:])})
+            passes[-1]["mops"][-1]["terms"].append(d)
+    return head, passes
+
+
+def fused_to_ops(L, fpasses, fields):
+    """Check the structure of the micro-op program (layouts, register bits, table positions) and
+    flatten it to the (type, r, c) op sequence, validated against the same dependency rule."""
+    flat = []
+    for i, ps in enumerate(fpasses):
+        a = ps["a"]
+        assert 0 <= a and a + W <= L and (a == 0 or a >= ps["ride"])
+        assert (ps["flags"] & 1) == (1 if i == 0 else 0)
+        layout, ops = None, []
+        assert ps["mops"][-1]["code"] == "end"
+        for m in ps["mops"][:-1]:
+            code = m["code"]
+            if code in ("loadA", "loadB"):
+                assert layout is None
+                layout = 0 if code == "loadA" else 1
+            elif code in ("storeA", "storeB"):
+                assert layout == (0 if code == "storeA" else 1)
+                layout = None
+            elif code == "gate":
+                assert layout is not None and 0 <= m["k"] < 6
+                assert m["c"] == a + (m["k"] if layout == 0 else 5 + m["k"])      # register bit <-> column
+                ops.append({"type": "g", "r": m["r"], "c": m["c"], "pos": 0})
+            elif code == "table":
+                assert layout == m["layout"] and m["nterms"] == len(m["terms"]) > 0
+                rcols = [a + (k if layout == 0 else 5 + k) for k in range(6)]
+                outer = a - 1 if layout == 0 else a + W
+                def col_of(pos):
+                    return outer if pos == 6 else rcols[pos]
+                for t in m["terms"]:
+                    if t["type"] == "dh":
+                        assert col_of(t["pa"]) == t["c"] and t["pa"] < 6
+                    else:
+                        assert col_of(t["pa"]) == t["c"] and col_of(t["pb"]) == t["c"] + 1
+                        assert not (t["pa"] == 6 and t["pb"] == 6) and 0 <= t["c"] < L - 1
+                    ops.append({"type": t["type"], "r": t["r"], "c": t["c"]})
+        assert layout is None
+        # re-use validate(): a pass whose tile is the active range
+        flat.append({"lo": 0, "a": a, "b": a + W, "flags": ps["flags"], "src": -1, "dst": -1, "ops": ops})
+    for ps in flat:          # validate() checks tile membership via lo/a/b and pos; give pos its value
+        for op in ps["ops"]:
+            if op["type"] == "g":
+                op["pos"] = op["c"] - ps["a"]
+    validate(2, L, flat, fields=fields, row_aligned=False)
+    return flat
+
+
+@pytest.mark.parametrize("L", [14, 15, 16, 20, 24, 28, 32, 34])
+def test_fused_schedule_obeys_dependency_rule(L):
+    head, fpasses = parse_fused(describe(2, L, 0, fused=True))
+    assert int(head["L"]) == L
+    fused_to_ops(L, fpasses, fields=True)
+
+
+@pytest.mark.parametrize("L", [14, 16])
+def test_fused_schedule_replay_matches_oracle(L):
+    _, fpasses = parse_fused(describe(2, L, 0, fused=True))
+    flat = fused_to_ops(L, fpasses, fields=True)
+    rng = np.random.default_rng(L)
+    Jh = rng.integers(-2, 3, size=(L, L - 1)).astype(float)
+    Jv = rng.integers(-2, 3, size=(L - 1, L)).astype(float)
+    h = rng.integers(-1, 2, size=(L, L)).astype(float)
+    E0, g = replay(2, L, flat, Jh, Jv, h)
+    Eo, go, _ = oracle.dp_ising(L, Jh, Jv, h)
+    assert (E0, g) == (Eo, go)
 
 
 # ------------------------------------------------------------------------------- numeric replay
