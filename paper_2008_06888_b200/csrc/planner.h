@@ -198,37 +198,56 @@ inline std::string describe(const Plan& p) {
 // =============================================================================================
 // Fused register-phase schedule ("v2", Ising Tropical<f32>).
 //
-// A pass gives every WARP a tile of W = 11 active digits [a, a+11) = 2^11 elements, 64 per
-// thread.  Inside a pass the warp alternates between two register layouts,
-//     A : register digits d0..d5,  lane digits d6..d10
-//     B : register digits d5..d10, lane digits d0..d4          (d_i = column a + i)
-// exchanging through its private shared-memory region.  In a layout, a gate on a register
-// digit is pure register arithmetic.  Diagonal terms are applied as small tables over the 64
-// register combinations (one FADD per element per table); a term can go into a table only if
-// each of its digits is a register digit or the tile's outer neighbour column (a-1 or a+11,
-// constant per warp: the table has one variant per value of that digit).  d5 is a register
-// digit in both layouts so that every in-tile pair (c, c+1) sits inside some layout.
-// The same dependency rule as above decides what is legal; phases are filled greedily.
+// Every WARP owns a tile of 2^12 state elements, 128 per thread (7 "register digits"), and runs
+// the pass's micro-op program on it with no CTA-level cooperation:
+//   LOW  tile (a = 0): 12 active digits d0..d11 = columns 0..11, a contiguous 16 KiB chunk.
+//        layout A: register digits d0..d6, lane digits d7..d11
+//        layout B: register digits d5..d11, lane digits d0..d4     (loads/stores: 128 B coalesced)
+//   HIGH tile (a >= 4): 9 active digits d0..d8 = columns a..a+8 plus the 3 riding digits 0..2,
+//        which sit on the low 3 lane bits so that every global request moves whole 32-byte runs.
+//        layout A: register digits d0..d6, lanes (riding, d7, d8)
+//        layout B: register digits d2..d8, lanes (riding, d0, d1)
+// A gate on a register digit is pure register arithmetic.  Diagonal terms are applied as
+// 128-entry tables over the register combinations; a term can go into a table only if each of
+// its digits is a register digit or the tile's outer neighbour column (a-1 for layout A, a+W for
+// layout B; constant per warp: one table variant per value).  Layout exchanges go through the
+// warp's private shared-memory region.  The dependency rule above decides what is legal;
+// phases are filled greedily.  The bit position of a digit inside the 7-bit register index is
+// layout specific (the two digits shared by both layouts are bits 0,1 so that exchanges and
+// FADD2 pairs are 128-bit / 64-bit register vectors): see fused_bitpos().
 // =============================================================================================
-enum MicroCode : uint8_t { MC_END = 0, MC_LOAD_A = 1, MC_LOAD_B = 2, MC_STORE_A = 3, MC_STORE_B = 4,
-                           MC_GATE = 5, MC_TABLE = 6 };
+enum MicroCode : uint8_t { MC_END = 0, MC_XAB = 1, MC_XBA = 2, MC_GATE = 3, MC_TABLE = 4 };
 
-struct MicroOp { uint8_t code; uint8_t k; uint16_t arg; };   // GATE: k = register bit, arg = index
-                                                             // into the pass's gate list; TABLE: arg
-                                                             // = table index inside the pass
+struct MicroOp { uint8_t code; uint8_t k; uint16_t arg; };   // GATE: k = register-index bit, arg = index
+                                                             // into the pass's gate list; TABLE: k = layout,
+                                                             // arg = table index inside the pass
 struct TableTerm {        // one diagonal term of a table
     uint8_t type;         // OP_DH / OP_DJ
-    uint8_t posA, posB;   // bit position (0..5) in the register index, or 6 = the outer neighbour
+    uint8_t posA, posB;   // bit position (0..6) in the register index, or 7 = the outer neighbour
     uint8_t pad;
     uint16_t row, col;    // lattice row, (left) column
 };
 
 struct FusedTable { int term_begin, term_end; int layout; };   // layout 0 = A (outer = a-1), 1 = B (outer = a+W)
 
+constexpr int F_RB = 7;          // register digits
+constexpr int F_WLOW = 12;       // active digits of the low tile
+constexpr int F_WHIGH = 9;       // active digits of a high tile
+constexpr int F_RIDE = 3;        // riding digits of a high tile
+constexpr int F_AMIN = 4;        // smallest start of a high tile (its outer neighbour must not ride)
+
+// tile digit (0..W-1) held by register-index bit `bit` in `layout` of a low/high tile
+inline int fused_digit_of_bit(bool low, int layout, int bit) {
+    static const int lowA[7] = {5, 6, 0, 1, 2, 3, 4}, lowB[7] = {5, 6, 7, 8, 9, 10, 11};
+    static const int highA[7] = {2, 3, 0, 1, 4, 5, 6}, highB[7] = {2, 3, 4, 5, 6, 7, 8};
+    return low ? (layout == 0 ? lowA[bit] : lowB[bit]) : (layout == 0 ? highA[bit] : highB[bit]);
+}
+
 struct FusedPass {
-    int a;                       // active digits [a, a+W)
-    int ride;                    // riding low digits (0 for the low tile)
+    int a, W;                    // active digits [a, a+W)
+    int low;                     // 1 = low tile
     int flags;
+    int first_layout, last_layout;
     int mop_begin, mop_end;      // into FusedPlan::mops
     int gate_begin, gate_end;    // into FusedPlan::gate_jv (index into Jv[(r-1)*L + c])
     int table_begin, table_end;  // into FusedPlan::tables
@@ -236,7 +255,7 @@ struct FusedPass {
 };
 
 struct FusedPlan {
-    int L = 0, W = 11;
+    int L = 0;
     std::vector<FusedPass> passes;
     std::vector<MicroOp> mops;
     std::vector<int> gate_jv;
@@ -256,60 +275,63 @@ class FusedScheduler {
         return true;
     }
     // One pass over active digits [a, a+W).  Returns number of ops applied (gates + terms).
-    int run_pass(int a, int W, int ride, FusedPass& ps) {
-        ps.a = a; ps.ride = ride; ps.flags = 0; ps.n_phases = 0;
+    int run_pass(int a, bool low, int max_tables, FusedPass& ps) {
+        const int W = low ? F_WLOW : F_WHIGH;
+        ps.a = a; ps.W = W; ps.low = low; ps.flags = 0; ps.n_phases = 0;
         ps.mop_begin = (int)P_.mops.size(); ps.gate_begin = (int)P_.gate_jv.size();
         ps.table_begin = (int)P_.tables.size();
-        int total = 0, idle = 0, layout = pick_first_layout(a, W);
+        pass_table_begin_ = ps.table_begin; pass_gate_begin_ = ps.gate_begin;
+        // the low tile loads and stores in layout B (coalesced); high tiles may start in either
+        int layout = low ? 1 : 0;
+        ps.first_layout = layout;
+        int total = 0, idle = 0;
+        bool pending_x = false;                        // an exchange is owed before the next non-empty phase
         while (idle < 2) {
             size_t mark = P_.mops.size();
-            P_.mops.push_back({(uint8_t)(layout == 0 ? MC_LOAD_A : MC_LOAD_B), 0, 0});
-            int n = run_phase(a, W, layout);
-            if (n == 0) { P_.mops.resize(mark); ++idle; }
-            else {
-                P_.mops.push_back({(uint8_t)(layout == 0 ? MC_STORE_A : MC_STORE_B), 0, 0});
-                total += n; idle = 0; ++ps.n_phases;
-            }
-            layout ^= 1;
+            if (pending_x) P_.mops.push_back({(uint8_t)(layout == 1 ? MC_XAB : MC_XBA), 0, 0});
+            int n = run_phase(a, W, low, layout, max_tables);
+            if (n == 0) { P_.mops.resize(mark); ++idle; layout ^= 1; pending_x = !pending_x; continue; }
+            total += n; idle = 0; ++ps.n_phases;
+            layout ^= 1; pending_x = true;
         }
+        // `layout` was toggled `idle`(=2) times past the last productive phase plus once after it
+        int last = layout ^ 1;                          // undo: toggles after last productive phase = 1 + 2
+        if (ps.n_phases == 0) last = ps.first_layout;
+        if (low && last != 1) { P_.mops.push_back({MC_XAB, 0, 0}); last = 1; }
+        ps.last_layout = last;
         P_.mops.push_back({MC_END, 0, 0});
         ps.mop_end = (int)P_.mops.size(); ps.gate_end = (int)P_.gate_jv.size();
         ps.table_end = (int)P_.tables.size();
         return total;
     }
   private:
-    // register digit i of layout -> tile digit index
-    static int rdig(int layout, int i) { return layout == 0 ? i : 5 + i; }
-    int count_legal(int a, int W, int layout) {   // how many gates are legal right now (ignoring pending tables)
-        int n = 0;
-        for (int i = 0; i < 6; ++i) { int c = a + rdig(layout, i); if (c < a + W && grow_[c] < L_) ++n; }
-        return n;
-    }
-    int pick_first_layout(int, int) { return 0; }
-    // position of column c in the register index of this layout: 0..5, 6 = outer neighbour, -1 = no
-    int pos_in(int a, int W, int layout, int c) const {
-        for (int i = 0; i < 6; ++i) if (a + rdig(layout, i) == c) return i;
-        if (layout == 0 && c == a - 1) return 6;
-        if (layout == 1 && c == a + W) return 6;
+    // position of column c in the register index of this layout: 0..6, 7 = outer neighbour, -1 = no
+    int pos_in(int a, int W, bool low, int layout, int c) const {
+        for (int b = 0; b < F_RB; ++b) if (a + fused_digit_of_bit(low, layout, b) == c) return b;
+        if (layout == 0 && c == a - 1) return 7;
+        if (layout == 1 && c == a + W) return 7;
         return -1;
     }
-    int run_phase(int a, int W, int layout) {
+    int run_phase(int a, int W, bool low, int layout, int max_tables) {
         int n = 0; bool progress = true;
+        int cols[F_RB];
+        for (int b = 0; b < F_RB; ++b) cols[b] = a + fused_digit_of_bit(low, layout, b);
         while (progress) {
             progress = false;
+            if ((int)P_.tables.size() - pass_table_begin_ >= max_tables) break;
             // ---- a table with every diagonal term that is legal and expressible here -----------
             int tb = (int)P_.terms.size();
-            for (int i = 0; i < 6; ++i) {
-                int c = a + rdig(layout, i);
+            for (int b = 0; b < F_RB; ++b) {
+                int c = cols[b];
                 int r = grow_[c] - 1;
                 if (!dh_[r * L_ + c]) {
                     dh_[r * L_ + c] = 1;
-                    P_.terms.push_back({OP_DH, (uint8_t)i, 0, 0, (uint16_t)r, (uint16_t)c});
+                    P_.terms.push_back({OP_DH, (uint8_t)b, 0, 0, (uint16_t)r, (uint16_t)c});
                 }
                 for (int cc = c - 1; cc <= c; ++cc) {
                     if (cc < 0 || cc + 1 >= L_) continue;
-                    int pa = pos_in(a, W, layout, cc), pb = pos_in(a, W, layout, cc + 1);
-                    if (pa < 0 || pb < 0 || (pa == 6 && pb == 6)) continue;
+                    int pa = pos_in(a, W, low, layout, cc), pb = pos_in(a, W, low, layout, cc + 1);
+                    if (pa < 0 || pb < 0 || (pa == 7 && pb == 7)) continue;
                     if (grow_[cc] != grow_[cc + 1]) continue;
                     int rr = grow_[cc] - 1;
                     if (dj_[rr * (L_ - 1) + cc]) continue;
@@ -319,13 +341,13 @@ class FusedScheduler {
             }
             if ((int)P_.terms.size() > tb) {
                 P_.tables.push_back({tb, (int)P_.terms.size(), layout});
-                int local = (int)P_.tables.size() - 1 - cur_table_begin();
+                int local = (int)P_.tables.size() - 1 - pass_table_begin_;
                 P_.mops.push_back({MC_TABLE, (uint8_t)layout, (uint16_t)local});
                 n += (int)P_.terms.size() - tb; progress = true;
             }
             // ---- every legal gate on a register digit ----------------------------------------------
-            for (int i = 0; i < 6; ++i) {
-                int c = a + rdig(layout, i);
+            for (int b = 0; b < F_RB; ++b) {
+                int c = cols[b];
                 int r = grow_[c];
                 if (r >= L_) continue;
                 bool ok = dh_[(r - 1) * L_ + c] != 0;
@@ -333,54 +355,47 @@ class FusedScheduler {
                 if (c + 1 < L_) ok = ok && dj_[(r - 1) * (L_ - 1) + c];
                 if (!ok) continue;
                 grow_[c] += 1;
-                int local = (int)P_.gate_jv.size() - cur_gate_begin();
+                int local = (int)P_.gate_jv.size() - pass_gate_begin_;
                 P_.gate_jv.push_back((r - 1) * L_ + c);
-                P_.mops.push_back({MC_GATE, (uint8_t)i, (uint16_t)local});
+                P_.mops.push_back({MC_GATE, (uint8_t)b, (uint16_t)local});
                 ++n; progress = true;
             }
         }
         return n;
     }
-    int cur_table_begin() const { return pass_table_begin_; }
-    int cur_gate_begin() const { return pass_gate_begin_; }
-  public:
-    void begin_pass() { pass_table_begin_ = (int)P_.tables.size(); pass_gate_begin_ = (int)P_.gate_jv.size(); }
-  private:
     int L_; FusedPlan& P_;
     std::vector<int> grow_;
     std::vector<uint8_t> dh_, dj_;
     int pass_table_begin_ = 0, pass_gate_begin_ = 0;
 };
 
-// Tile starts: 0, then advancing by `stride`, the last flush with L.  High tiles (a > 0) need
-// a >= ride.  Chooses the stride with the fewest passes (ties: fewest phases).
-inline FusedPlan make_fused_plan(int L, bool has_field, int ride) {
-    const int W = 11;
+// Tile cycle: the low tile [0,12), then high tiles [x, x+9) advancing by `stride`, the last
+// flush with L.  Chooses the stride with the lowest estimated cost.
+inline FusedPlan make_fused_plan(int L, bool has_field, int max_tables) {
     FusedPlan best;
-    if (L < W + ride) return best;
-    long best_cost = -1;
-    for (int stride = 1; stride <= W; ++stride) {
+    if (L < F_WLOW) return best;
+    double best_cost = -1;
+    for (int stride = 1; stride <= F_WHIGH; ++stride) {
         std::vector<int> starts;
         starts.push_back(0);
-        if (L > W) {
-            int x = stride;
+        if (L > F_WLOW) {
+            int x = F_WLOW - (F_WHIGH - stride);
             for (;;) {
-                if (x + W >= L) x = L - W;
-                if (x < ride) x = ride;
+                if (x + F_WHIGH >= L) x = L - F_WHIGH;
+                if (x < F_AMIN) x = F_AMIN;
                 starts.push_back(x);
-                if (x + W >= L) break;
+                if (x + F_WHIGH >= L) break;
                 x += stride;
             }
         }
-        FusedPlan p; p.L = L; p.W = W;
+        FusedPlan p; p.L = L;
         FusedScheduler s(L, has_field, p);
         size_t k = 0; int idle = 0; bool first = true;
         while ((first || !s.done()) && p.passes.size() < 4096) {
             int a = starts[k % starts.size()]; ++k;
             FusedPass ps{};
-            s.begin_pass();
             size_t m0 = p.mops.size();
-            int n = s.run_pass(a, W, a == 0 ? 0 : ride, ps);
+            int n = s.run_pass(a, a == 0, max_tables, ps);
             if (n == 0 && !first) { p.mops.resize(m0); if (++idle > (int)starts.size()) break; continue; }
             idle = 0;
             if (first) ps.flags |= PASS_INIT;
@@ -389,8 +404,12 @@ inline FusedPlan make_fused_plan(int L, bool has_field, int ride) {
         }
         if (!s.done()) continue;
         p.passes.back().flags |= PASS_REDUCE;
-        long phases = 0; for (auto& ps : p.passes) phases += ps.n_phases;
-        long cost = (long)p.passes.size() * 1000 + phases;
+        // cost model (issue slots per thread, 128 elements): gate 192, table 96, exchange 64,
+        // dispatch 6 per micro-op; one HBM pass ~ 2500 (5.7 ms at 6 TB/s vs 64 updates/clk/SM)
+        double cost = 0;
+        for (auto& ps : p.passes)
+            cost += 2500.0 + 192.0 * (ps.gate_end - ps.gate_begin) + 96.0 * (ps.table_end - ps.table_begin) +
+                    64.0 * ps.n_phases + 6.0 * (ps.mop_end - ps.mop_begin);
         if (best_cost < 0 || cost < best_cost) { best = p; best_cost = cost; best.ok = true; }
     }
     return best;
@@ -398,21 +417,20 @@ inline FusedPlan make_fused_plan(int L, bool has_field, int ride) {
 
 inline std::string describe_fused(const FusedPlan& p) {
     std::string out; char line[200];
-    snprintf(line, sizeof line, "fused L=%d W=%d passes=%zu mops=%zu gates=%zu tables=%zu terms=%zu\n", p.L, p.W,
+    snprintf(line, sizeof line, "fused L=%d passes=%zu mops=%zu gates=%zu tables=%zu terms=%zu\n", p.L,
              p.passes.size(), p.mops.size(), p.gate_jv.size(), p.tables.size(), p.terms.size());
     out += line;
     for (size_t i = 0; i < p.passes.size(); ++i) {
         const FusedPass& ps = p.passes[i];
-        snprintf(line, sizeof line, "fpass %zu a=%d ride=%d flags=%d phases=%d gates=%d tables=%d\n", i, ps.a, ps.ride,
-                 ps.flags, ps.n_phases, ps.gate_end - ps.gate_begin, ps.table_end - ps.table_begin);
+        snprintf(line, sizeof line, "fpass %zu a=%d W=%d low=%d flags=%d first=%d last=%d phases=%d gates=%d tables=%d\n", i,
+                 ps.a, ps.W, ps.low, ps.flags, ps.first_layout, ps.last_layout, ps.n_phases,
+                 ps.gate_end - ps.gate_begin, ps.table_end - ps.table_begin);
         out += line;
         for (int k = ps.mop_begin; k < ps.mop_end; ++k) {
             const MicroOp& m = p.mops[k];
             switch (m.code) {
-                case MC_LOAD_A: out += "m loadA\n"; break;
-                case MC_LOAD_B: out += "m loadB\n"; break;
-                case MC_STORE_A: out += "m storeA\n"; break;
-                case MC_STORE_B: out += "m storeB\n"; break;
+                case MC_XAB: out += "m xAB\n"; break;
+                case MC_XBA: out += "m xBA\n"; break;
                 case MC_END: out += "m end\n"; break;
                 case MC_GATE: {
                     int jv = p.gate_jv[ps.gate_begin + m.arg];

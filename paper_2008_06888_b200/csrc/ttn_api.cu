@@ -76,10 +76,10 @@ struct Layout {
     int f_max_gates = 0, f_max_tables = 0, f_max_terms = 0, f_max_mops = 0;
 };
 
-// The fused register-phase path serves the Ising Tropical<f32> energy sweep for L >= 14.
+// The fused register-phase path serves the Ising Tropical<f32> energy sweep for L >= 12.
 bool fused_eligible(int q, int L, bool count, bool config) {
     if (const char* e = getenv("TTN_DEBUG_FUSED")) if (atoi(e) == 0) return false;
-    return q == 2 && !count && !config && L >= ttn::FW + ttn::FRIDE;
+    return q == 2 && !count && !config && L >= ttn::F_WLOW;
 }
 
 // The op list length is bounded by L*L gates + 2*L*L diagonals.
@@ -89,6 +89,7 @@ Layout make_layout(int q, int L, bool count, bool config, int batch) {
     const TileCfg tc = tile_cfg(q, count);
     // every pass of a plan stages tiles of q^min(L, Tmax) elements
     y.max_tiles = y.NS / ipow(q, tc.Tmax < L ? tc.Tmax : L);
+    if (fused_eligible(q, L, count, config) && (y.NS >> 12) > y.max_tiles) y.max_tiles = y.NS >> 12;
     if (y.max_tiles == 0) y.max_tiles = 1;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
@@ -116,7 +117,7 @@ Layout make_layout(int q, int L, bool count, bool config, int batch) {
         y.f_tables = take((size_t)y.f_max_tables * sizeof(ttn::FusedTable));
         y.f_terms = take((size_t)y.f_max_terms * sizeof(ttn::TableTerm));
         y.f_gate_m = take((size_t)batch * y.f_max_gates * 4);
-        y.f_table_vals = take((size_t)batch * y.f_max_tables * 128 * 4);
+        y.f_table_vals = take((size_t)batch * y.f_max_tables * 256 * 4);
     }
     y.total = off;
     return y;
@@ -197,23 +198,24 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
     const Layout& y = P->lay;
     const ttn::FusedPlan& fp = P->fplan;
     ttn::FusedParams pp{};
-    pp.L = P->L; pp.a = ps.a; pp.ride = ps.ride; pp.flags = ps.flags;
+    pp.L = P->L; pp.a = ps.a; pp.low = ps.low; pp.flags = ps.flags; pp.batch = P->batch;
+    pp.first_layout = ps.first_layout; pp.last_layout = ps.last_layout;
     pp.state = reinterpret_cast<float*>(P->ws + y.x);
     pp.inst_stride = y.NS;
-    pp.tiles_per_inst = y.NS >> 14;
-    pp.total_tiles = pp.tiles_per_inst * (unsigned long long)P->batch;
+    pp.tiles_per_inst = y.NS >> 12;
     pp.mops = reinterpret_cast<const ttn::MicroOp*>(P->ws + y.f_mops) + ps.mop_begin;
     pp.n_mops = ps.mop_end - ps.mop_begin;
     pp.gate_m = reinterpret_cast<const float*>(P->ws + y.f_gate_m) + ps.gate_begin;
-    pp.n_gates = ps.gate_end - ps.gate_begin;
     pp.gate_inst_stride = (int)fp.gate_jv.size();
-    pp.tables = reinterpret_cast<const float*>(P->ws + y.f_table_vals) + (size_t)ps.table_begin * 128;
-    pp.table_inst_stride = (unsigned long long)fp.tables.size() * 128;
+    pp.tables = reinterpret_cast<const float*>(P->ws + y.f_table_vals) + (size_t)ps.table_begin * 256;
+    pp.n_tables = ps.table_end - ps.table_begin;
+    pp.table_inst_stride = (unsigned long long)fp.tables.size() * 256;
     pp.part_x = reinterpret_cast<float*>(P->ws + y.part_x);
-    const size_t smem = (size_t)(ttn::FWARPS * ttn::FREGION + ttn::FMAX_GATES) * 4 + ttn::FMAX_MOPS * sizeof(ttn::MicroOp);
     unsigned long long grid = (unsigned long long)P->fused_grid;
-    if (grid > pp.total_tiles) grid = pp.total_tiles;
-    ttn::fused_pass_kernel<<<(unsigned)grid, ttn::FWARPS * 32, smem, st>>>(pp);
+    const unsigned long long need = (pp.tiles_per_inst + ttn::FWARPS - 1) / ttn::FWARPS;
+    if (grid > need) grid = need;
+    if (ps.low) ttn::fused_pass_kernel<true><<<(unsigned)grid, ttn::FWARPS * 32, ttn::FSMEM_BYTES, st>>>(pp);
+    else ttn::fused_pass_kernel<false><<<(unsigned)grid, ttn::FWARPS * 32, ttn::FSMEM_BYTES, st>>>(pp);
     TTN_CUDA(cudaGetLastError());
     if (ps.flags & ttn::PASS_REDUCE) {
         ttn::final_reduce_kernel<false><<<P->batch, 256, 0, st>>>(
@@ -231,8 +233,9 @@ static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
         (int)fp.terms.size() > y.f_max_terms || (int)fp.mops.size() > y.f_max_mops)
         return fail(TTN_EUNSUPPORTED, "fused plan exceeds its workspace bounds");
     for (const auto& ps : fp.passes)
-        if (ps.mop_end - ps.mop_begin > ttn::FMAX_MOPS || ps.gate_end - ps.gate_begin > ttn::FMAX_GATES)
-            return fail(TTN_EUNSUPPORTED, "fused pass program too long");
+        if (ps.mop_end - ps.mop_begin > ttn::FMAX_MOPS || ps.table_end - ps.table_begin > ttn::FMAX_TABLES ||
+            (ps.low && (ps.first_layout != 1 || ps.last_layout != 1)))
+            return fail(TTN_EUNSUPPORTED, "fused pass program out of bounds");
     TTN_CUDA(cudaMemcpyAsync(P->ws + y.f_mops, fp.mops.data(), fp.mops.size() * sizeof(ttn::MicroOp), cudaMemcpyHostToDevice, st));
     TTN_CUDA(cudaMemcpyAsync(P->ws + y.f_gate_jv, fp.gate_jv.data(), fp.gate_jv.size() * 4, cudaMemcpyHostToDevice, st));
     TTN_CUDA(cudaMemcpyAsync(P->ws + y.f_tables, fp.tables.data(), fp.tables.size() * sizeof(ttn::FusedTable), cudaMemcpyHostToDevice, st));
@@ -247,16 +250,18 @@ static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
     q.h = P->has_field ? reinterpret_cast<const float*>(P->ws + y.h) : nullptr;
     q.gate_m = reinterpret_cast<float*>(P->ws + y.f_gate_m);
     q.table_out = reinterpret_cast<float*>(P->ws + y.f_table_vals);
-    long work = (long)q.n_tables * 128; if (q.n_gates > work) work = q.n_gates;
+    long work = (long)q.n_tables * 256; if (q.n_gates > work) work = q.n_gates;
     dim3 grid((unsigned)((work + 255) / 256), (unsigned)P->batch);
     ttn::fused_prep_kernel<<<grid, 256, 0, st>>>(q);
     TTN_CUDA(cudaGetLastError());
-    const size_t smem = (size_t)(ttn::FWARPS * ttn::FREGION + ttn::FMAX_GATES) * 4 + ttn::FMAX_MOPS * sizeof(ttn::MicroOp);
-    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    int dev = 0, sms = 0, per_sm = 0;
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::FSMEM_BYTES));
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::FSMEM_BYTES));
+    int dev = 0, sms = 0, per_sm = 0, per_sm2 = 0;
     TTN_CUDA(cudaGetDevice(&dev));
     TTN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    TTN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ttn::fused_pass_kernel, ttn::FWARPS * 32, smem));
+    TTN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ttn::fused_pass_kernel<true>, ttn::FWARPS * 32, ttn::FSMEM_BYTES));
+    TTN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm2, ttn::fused_pass_kernel<false>, ttn::FWARPS * 32, ttn::FSMEM_BYTES));
+    if (per_sm2 < per_sm) per_sm = per_sm2;
     if (per_sm < 1) return fail(TTN_ECUDA, "fused kernel does not fit on an SM");
     P->fused_grid = sms * per_sm;
     return TTN_OK;
@@ -279,7 +284,7 @@ long ttn_plan_describe(int q, int L, ttn_call call, char* buf, size_t n) {
     if (!limits_ok(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) return -1;
     std::string s;
     if (fused_eligible(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) {
-        ttn::FusedPlan fp = ttn::make_fused_plan(L, /*has_field=*/true, ttn::FRIDE);
+        ttn::FusedPlan fp = ttn::make_fused_plan(L, /*has_field=*/true, ttn::FMAX_TABLES);
         if (fp.ok) s = ttn::describe_fused(fp);
     }
     if (s.empty()) s = ttn::describe(plan_for(q, L, call, /*has_field=*/q == 2));
@@ -325,7 +330,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     P->lay = lay;
     P->ws = static_cast<unsigned char*>(workspace);
     if (fused_eligible(q, L, count, config)) {
-        P->fplan = ttn::make_fused_plan(L, P->has_field, ttn::FRIDE);
+        P->fplan = ttn::make_fused_plan(L, P->has_field, ttn::FMAX_TABLES);
         P->fused = P->fplan.ok;
     }
     if (!P->fused) P->plan = plan_for(q, L, call, P->has_field);

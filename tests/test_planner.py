@@ -111,11 +111,13 @@ def test_fusion_cuts_hbm_passes():
     _, passes = parse(describe(2, 24, 1))
     assert len(passes) <= 12
     head, fpasses = parse_fused(describe(2, 32, 0, fused=True))
-    assert len(fpasses) <= 20
+    assert len(fpasses) <= 24
 
 
 # ------------------------------------------------------------------ fused register-phase schedule
-W = 11
+# register-index bit -> tile digit, as documented in csrc/planner.h (fused_digit_of_bit)
+DIGIT_OF_BIT = {(1, 0): [5, 6, 0, 1, 2, 3, 4], (1, 1): [5, 6, 7, 8, 9, 10, 11],
+                (0, 0): [2, 3, 0, 1, 4, 5, 6], (0, 1): [2, 3, 4, 5, 6, 7, 8]}
 
 
 def parse_fused(txt):
@@ -145,55 +147,58 @@ def fused_to_ops(L, fpasses, fields):
     flatten it to the (type, r, c) op sequence, validated against the same dependency rule."""
     flat = []
     for i, ps in enumerate(fpasses):
-        a = ps["a"]
-        assert 0 <= a and a + W <= L and (a == 0 or a >= ps["ride"])
+        a, Wt, low = ps["a"], ps["W"], ps["low"]
+        assert (low == 1 and a == 0 and Wt == 12) or (low == 0 and a >= 4 and Wt == 9)
+        assert a + Wt <= L
         assert (ps["flags"] & 1) == (1 if i == 0 else 0)
-        layout, ops = None, []
+        if low:
+            assert ps["first"] == 1 and ps["last"] == 1     # coalesced global layout
+        layout, ops = ps["first"], []
         assert ps["mops"][-1]["code"] == "end"
+        assert len(ps["mops"]) <= 256
+        ntab = 0
         for m in ps["mops"][:-1]:
             code = m["code"]
-            if code in ("loadA", "loadB"):
-                assert layout is None
-                layout = 0 if code == "loadA" else 1
-            elif code in ("storeA", "storeB"):
-                assert layout == (0 if code == "storeA" else 1)
-                layout = None
+            if code == "xAB":
+                assert layout == 0
+                layout = 1
+            elif code == "xBA":
+                assert layout == 1
+                layout = 0
             elif code == "gate":
-                assert layout is not None and 0 <= m["k"] < 6
-                assert m["c"] == a + (m["k"] if layout == 0 else 5 + m["k"])      # register bit <-> column
-                ops.append({"type": "g", "r": m["r"], "c": m["c"], "pos": 0})
+                assert 0 <= m["k"] < 7
+                assert m["c"] == a + DIGIT_OF_BIT[(low, layout)][m["k"]]      # register bit <-> column
+                ops.append({"type": "g", "r": m["r"], "c": m["c"], "pos": m["c"] - a})
             elif code == "table":
+                ntab += 1
                 assert layout == m["layout"] and m["nterms"] == len(m["terms"]) > 0
-                rcols = [a + (k if layout == 0 else 5 + k) for k in range(6)]
-                outer = a - 1 if layout == 0 else a + W
+                outer = a - 1 if layout == 0 else a + Wt
+
                 def col_of(pos):
-                    return outer if pos == 6 else rcols[pos]
+                    return outer if pos == 7 else a + DIGIT_OF_BIT[(low, layout)][pos]
                 for t in m["terms"]:
                     if t["type"] == "dh":
-                        assert col_of(t["pa"]) == t["c"] and t["pa"] < 6
+                        assert t["pa"] < 7 and col_of(t["pa"]) == t["c"]
                     else:
                         assert col_of(t["pa"]) == t["c"] and col_of(t["pb"]) == t["c"] + 1
-                        assert not (t["pa"] == 6 and t["pb"] == 6) and 0 <= t["c"] < L - 1
+                        assert not (t["pa"] == 7 and t["pb"] == 7) and 0 <= t["c"] < L - 1
+                        if low == 0:
+                            assert outer >= 3       # the outer neighbour must not be a riding digit
                     ops.append({"type": t["type"], "r": t["r"], "c": t["c"]})
-        assert layout is None
-        # re-use validate(): a pass whose tile is the active range
-        flat.append({"lo": 0, "a": a, "b": a + W, "flags": ps["flags"], "src": -1, "dst": -1, "ops": ops})
-    for ps in flat:          # validate() checks tile membership via lo/a/b and pos; give pos its value
-        for op in ps["ops"]:
-            if op["type"] == "g":
-                op["pos"] = op["c"] - ps["a"]
+        assert layout == ps["last"] and ntab <= 32
+        flat.append({"lo": 0, "a": a, "b": a + Wt, "flags": ps["flags"], "src": -1, "dst": -1, "ops": ops})
     validate(2, L, flat, fields=fields, row_aligned=False)
     return flat
 
 
-@pytest.mark.parametrize("L", [14, 15, 16, 20, 24, 28, 32, 34])
+@pytest.mark.parametrize("L", [12, 13, 14, 16, 17, 20, 24, 28, 32, 34])
 def test_fused_schedule_obeys_dependency_rule(L):
     head, fpasses = parse_fused(describe(2, L, 0, fused=True))
     assert int(head["L"]) == L
     fused_to_ops(L, fpasses, fields=True)
 
 
-@pytest.mark.parametrize("L", [14, 16])
+@pytest.mark.parametrize("L", [12, 13, 16])
 def test_fused_schedule_replay_matches_oracle(L):
     _, fpasses = parse_fused(describe(2, L, 0, fused=True))
     flat = fused_to_ops(L, fpasses, fields=True)
