@@ -371,7 +371,7 @@ class FusedScheduler {
 
 // Tile cycle: the low tile [0,12), then high tiles [x, x+9) advancing by `stride`, the last
 // flush with L.  Chooses the stride with the lowest estimated cost.
-inline FusedPlan make_fused_plan(int L, bool has_field, int max_tables) {
+inline FusedPlan make_fused_plan(int L, bool has_field, int max_tables_low, int max_tables_high) {
     FusedPlan best;
     if (L < F_WLOW) return best;
     double best_cost = -1;
@@ -395,7 +395,7 @@ inline FusedPlan make_fused_plan(int L, bool has_field, int max_tables) {
             int a = starts[k % starts.size()]; ++k;
             FusedPass ps{};
             size_t m0 = p.mops.size();
-            int n = s.run_pass(a, a == 0, max_tables, ps);
+            int n = s.run_pass(a, a == 0, a == 0 ? max_tables_low : max_tables_high, ps);
             if (n == 0 && !first) { p.mops.resize(m0); if (++idle > (int)starts.size()) break; continue; }
             idle = 0;
             if (first) ps.flags |= PASS_INIT;

@@ -212,10 +212,11 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
     pp.table_inst_stride = (unsigned long long)fp.tables.size() * 256;
     pp.part_x = reinterpret_cast<float*>(P->ws + y.part_x);
     unsigned long long grid = (unsigned long long)P->fused_grid;
-    const unsigned long long need = (pp.tiles_per_inst + ttn::FWARPS - 1) / ttn::FWARPS;
+    const int nw = ttn::fwarps(ps.low != 0);
+    const unsigned long long need = (pp.tiles_per_inst + nw - 1) / nw;
     if (grid > need) grid = need;
-    if (ps.low) ttn::fused_pass_kernel<true><<<(unsigned)grid, ttn::FWARPS * 32, ttn::FSMEM_BYTES, st>>>(pp);
-    else ttn::fused_pass_kernel<false><<<(unsigned)grid, ttn::FWARPS * 32, ttn::FSMEM_BYTES, st>>>(pp);
+    if (ps.low) ttn::fused_pass_kernel<true><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(true), st>>>(pp);
+    else ttn::fused_pass_kernel<false><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(false), st>>>(pp);
     TTN_CUDA(cudaGetLastError());
     if (ps.flags & ttn::PASS_REDUCE) {
         ttn::final_reduce_kernel<false><<<P->batch, 256, 0, st>>>(
@@ -233,7 +234,7 @@ static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
         (int)fp.terms.size() > y.f_max_terms || (int)fp.mops.size() > y.f_max_mops)
         return fail(TTN_EUNSUPPORTED, "fused plan exceeds its workspace bounds");
     for (const auto& ps : fp.passes)
-        if (ps.mop_end - ps.mop_begin > ttn::FMAX_MOPS || ps.table_end - ps.table_begin > ttn::FMAX_TABLES ||
+        if (ps.mop_end - ps.mop_begin > ttn::FMAX_MOPS || ps.table_end - ps.table_begin > ttn::fmax_tables(ps.low != 0) ||
             (ps.low && (ps.first_layout != 1 || ps.last_layout != 1)))
             return fail(TTN_EUNSUPPORTED, "fused pass program out of bounds");
     TTN_CUDA(cudaMemcpyAsync(P->ws + y.f_mops, fp.mops.data(), fp.mops.size() * sizeof(ttn::MicroOp), cudaMemcpyHostToDevice, st));
@@ -254,13 +255,13 @@ static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
     dim3 grid((unsigned)((work + 255) / 256), (unsigned)P->batch);
     ttn::fused_prep_kernel<<<grid, 256, 0, st>>>(q);
     TTN_CUDA(cudaGetLastError());
-    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::FSMEM_BYTES));
-    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::FSMEM_BYTES));
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));
     int dev = 0, sms = 0, per_sm = 0, per_sm2 = 0;
     TTN_CUDA(cudaGetDevice(&dev));
     TTN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    TTN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ttn::fused_pass_kernel<true>, ttn::FWARPS * 32, ttn::FSMEM_BYTES));
-    TTN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm2, ttn::fused_pass_kernel<false>, ttn::FWARPS * 32, ttn::FSMEM_BYTES));
+    TTN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ttn::fused_pass_kernel<true>, ttn::FWARPS_LOW * 32, ttn::fsmem_bytes(true)));
+    TTN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm2, ttn::fused_pass_kernel<false>, ttn::FWARPS_HIGH * 32, ttn::fsmem_bytes(false)));
     if (per_sm2 < per_sm) per_sm = per_sm2;
     if (per_sm < 1) return fail(TTN_ECUDA, "fused kernel does not fit on an SM");
     P->fused_grid = sms * per_sm;
@@ -284,7 +285,7 @@ long ttn_plan_describe(int q, int L, ttn_call call, char* buf, size_t n) {
     if (!limits_ok(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) return -1;
     std::string s;
     if (fused_eligible(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) {
-        ttn::FusedPlan fp = ttn::make_fused_plan(L, /*has_field=*/true, ttn::FMAX_TABLES);
+        ttn::FusedPlan fp = ttn::make_fused_plan(L, /*has_field=*/true, ttn::FMAX_TABLES_LOW, ttn::FMAX_TABLES_HIGH);
         if (fp.ok) s = ttn::describe_fused(fp);
     }
     if (s.empty()) s = ttn::describe(plan_for(q, L, call, /*has_field=*/q == 2));
@@ -330,7 +331,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     P->lay = lay;
     P->ws = static_cast<unsigned char*>(workspace);
     if (fused_eligible(q, L, count, config)) {
-        P->fplan = ttn::make_fused_plan(L, P->has_field, ttn::FMAX_TABLES);
+        P->fplan = ttn::make_fused_plan(L, P->has_field, ttn::FMAX_TABLES_LOW, ttn::FMAX_TABLES_HIGH);
         P->fused = P->fplan.ok;
     }
     if (!P->fused) P->plan = plan_for(q, L, call, P->has_field);
