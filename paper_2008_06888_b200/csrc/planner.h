@@ -196,10 +196,24 @@ inline std::string describe(const Plan& p) {
 
 
 // =============================================================================================
-// Fused register-phase schedule ("v2", Ising Tropical<f32>).
+// Fused register-phase schedule in the DIAGONAL FRAME ("v3", Ising Tropical<f32>).
 //
-// Every WARP owns a tile of 2^12 state elements, 128 per thread (7 "register digits"), and runs
-// the pass's micro-op program on it with no CTA-level cooperation:
+// Diagonal frame.  Let D_r be the product of all diagonal gates of row r ((A3), (A4)
+// PAPER.md:247-252) and A_r = D_0 D_1 ... D_r (diagonal operators commute).  With
+// G_r(c) the max-plus gate (A2) PAPER.md:242 of row r on digit c, the sweep
+//     V = D_{L-1} G_{L-1} ... D_1 G_1 D_0 1         equals        V = A_{L-1} G''_{L-1} ... G''_1 1,
+//     G''_r(c) = A_{r-1}^{-1} G_r(c) A_{r-1}        (a similarity transform of every gate).
+// A_{r-1}(s) = sum_c H_c sigma_c + sum_c K_c sigma_c sigma_{c+1} with H_c = sum_{r'<r} h[r'][c],
+// K_c = sum_{r'<r} Jh[r'][c], so G''_r(c) is still a 2x2 max-plus gate on digit c, whose two
+// off-diagonal entries depend on the neighbour bits c-1 and c+1 of the element's own index:
+//     a' = max(a, b + m - 2 rho),  b' = max(b, a + m + 2 rho),   m = -2 Jv[r-1][c],
+//     rho = H_c + K_{c-1} sigma_{c-1} + K_c sigma_{c+1}          (8 constants per gate).
+// No diagonal pass over the state is ever made; the last pass adds A_{L-1}(s) before the final
+// (+)-reduction.  Dependency rule in this frame: g''(r,c) needs g''(r-1,c-1), g''(r-1,c),
+// g''(r-1,c+1); gates of one row commute with each other (same conjugation), gates on
+// non-adjacent digits always commute.
+//
+// Every WARP owns a tile of 2^12 state elements, 128 per thread (7 "register digits"):
 //   LOW  tile (a = 0): 12 active digits d0..d11 = columns 0..11, a contiguous 16 KiB chunk.
 //        layout A: register digits d0..d6, lane digits d7..d11
 //        layout B: register digits d5..d11, lane digits d0..d4     (loads/stores: 128 B coalesced)
@@ -207,28 +221,16 @@ inline std::string describe(const Plan& p) {
 //        which sit on the low 3 lane bits so that every global request moves whole 32-byte runs.
 //        layout A: register digits d0..d6, lanes (riding, d7, d8)
 //        layout B: register digits d2..d8, lanes (riding, d0, d1)
-// A gate on a register digit is pure register arithmetic.  Diagonal terms are applied as
-// 128-entry tables over the register combinations; a term can go into a table only if each of
-// its digits is a register digit or the tile's outer neighbour column (a-1 for layout A, a+W for
-// layout B; constant per warp: one table variant per value).  Layout exchanges go through the
-// warp's private shared-memory region.  The dependency rule above decides what is legal;
-// phases are filled greedily.  The bit position of a digit inside the 7-bit register index is
-// layout specific (the two digits shared by both layouts are bits 0,1 so that exchanges and
-// FADD2 pairs are 128-bit / 64-bit register vectors): see fused_bitpos().
+// A gate on a register digit is pure register arithmetic; its neighbour bits are register-index
+// bits (compile-time per unrolled element) or constant per thread (lane / tile bits).  A phase is
+// a list of ROUNDS; a round applies, for a 7-bit mask of register digits, the next gate of each
+// of them (all legal at the start of the round), in ascending bit order.  Layout exchanges go
+// through the warp's private shared-memory region.
 // =============================================================================================
-enum MicroCode : uint8_t { MC_END = 0, MC_XAB = 1, MC_XBA = 2, MC_GATE = 3, MC_TABLE = 4 };
+enum MicroCode : uint8_t { MC_END = 0, MC_XAB = 1, MC_XBA = 2, MC_ROUND = 3, MC_FINAL = 4 };
 
-struct MicroOp { uint8_t code; uint8_t k; uint16_t arg; };   // GATE: k = register-index bit, arg = index
-                                                             // into the pass's gate list; TABLE: k = layout,
-                                                             // arg = table index inside the pass
-struct TableTerm {        // one diagonal term of a table
-    uint8_t type;         // OP_DH / OP_DJ
-    uint8_t posA, posB;   // bit position (0..6) in the register index, or 7 = the outer neighbour
-    uint8_t pad;
-    uint16_t row, col;    // lattice row, (left) column
-};
-
-struct FusedTable { int term_begin, term_end; int layout; };   // layout 0 = A (outer = a-1), 1 = B (outer = a+W)
+struct MicroOp { uint8_t code; uint8_t mask; uint16_t arg; };   // ROUND: mask = register bits, arg = index of
+                                                                // its first gate in the pass's gate list
 
 constexpr int F_RB = 7;          // register digits
 constexpr int F_WLOW = 12;       // active digits of the low tile
@@ -237,10 +239,21 @@ constexpr int F_RIDE = 3;        // riding digits of a high tile
 constexpr int F_AMIN = 4;        // smallest start of a high tile (its outer neighbour must not ride)
 
 // tile digit (0..W-1) held by register-index bit `bit` in `layout` of a low/high tile
-inline int fused_digit_of_bit(bool low, int layout, int bit) {
-    static const int lowA[7] = {5, 6, 0, 1, 2, 3, 4}, lowB[7] = {5, 6, 7, 8, 9, 10, 11};
-    static const int highA[7] = {2, 3, 0, 1, 4, 5, 6}, highB[7] = {2, 3, 4, 5, 6, 7, 8};
-    return low ? (layout == 0 ? lowA[bit] : lowB[bit]) : (layout == 0 ? highA[bit] : highB[bit]);
+#if defined(__CUDACC__)
+__host__ __device__
+#endif
+constexpr int fused_digit_of_bit(bool low, int layout, int bit) {
+    // lowA {5,6,0,1,2,3,4}  lowB {5,..,11}  highA {2,3,0,1,4,5,6}  highB {2,..,8}
+    return low ? (layout == 0 ? (bit < 2 ? 5 + bit : bit - 2) : 5 + bit)
+               : (layout == 0 ? (bit < 2 ? 2 + bit : (bit < 4 ? bit - 2 : bit)) : 2 + bit);
+}
+// register-index bit holding tile digit d in this layout, or -1 (lane / tile digit)
+#if defined(__CUDACC__)
+__host__ __device__
+#endif
+constexpr int fused_bit_of_digit(bool low, int layout, int d) {
+    for (int b = 0; b < F_RB; ++b) if (fused_digit_of_bit(low, layout, b) == d) return b;
+    return -1;
 }
 
 struct FusedPass {
@@ -249,39 +262,32 @@ struct FusedPass {
     int flags;
     int first_layout, last_layout;
     int mop_begin, mop_end;      // into FusedPlan::mops
-    int gate_begin, gate_end;    // into FusedPlan::gate_jv (index into Jv[(r-1)*L + c])
-    int table_begin, table_end;  // into FusedPlan::tables
-    int n_phases;
+    int gate_begin, gate_end;    // into FusedPlan::gate_rc
+    int n_phases, n_rounds;
 };
 
 struct FusedPlan {
     int L = 0;
     std::vector<FusedPass> passes;
     std::vector<MicroOp> mops;
-    std::vector<int> gate_jv;
-    std::vector<FusedTable> tables;
-    std::vector<TableTerm> terms;
+    std::vector<int> gate_rc;    // r * 64 + c of every gate, in execution order
     bool ok = false;
 };
 
 class FusedScheduler {
   public:
-    FusedScheduler(int L, bool has_field, FusedPlan& p) : L_(L), P_(p), grow_(L, 1), dh_(L * L, 0),
-        dj_(L * (L > 1 ? L - 1 : 1), 0) { if (!has_field) for (auto& x : dh_) x = 1; }
+    FusedScheduler(int L, FusedPlan& p) : L_(L), P_(p), grow_(L, 1) {}
     bool done() const {
         for (int c = 0; c < L_; ++c) if (grow_[c] != L_) return false;
-        for (auto x : dh_) if (!x) return false;
-        for (int r = 0; r < L_; ++r) for (int c = 0; c + 1 < L_; ++c) if (!dj_[r * (L_ - 1) + c]) return false;
         return true;
     }
-    // One pass over active digits [a, a+W).  Returns number of ops applied (gates + terms).
-    int run_pass(int a, bool low, int max_tables, FusedPass& ps) {
+    // One pass over active digits [a, a+W).  Returns number of gates applied.
+    int run_pass(int a, bool low, int max_gates, FusedPass& ps) {
         const int W = low ? F_WLOW : F_WHIGH;
-        ps.a = a; ps.W = W; ps.low = low; ps.flags = 0; ps.n_phases = 0;
-        ps.mop_begin = (int)P_.mops.size(); ps.gate_begin = (int)P_.gate_jv.size();
-        ps.table_begin = (int)P_.tables.size();
-        pass_table_begin_ = ps.table_begin; pass_gate_begin_ = ps.gate_begin;
-        // the low tile loads and stores in layout B (coalesced); high tiles may start in either
+        ps.a = a; ps.W = W; ps.low = low; ps.flags = 0; ps.n_phases = 0; ps.n_rounds = 0;
+        ps.mop_begin = (int)P_.mops.size(); ps.gate_begin = (int)P_.gate_rc.size();
+        pass_gate_begin_ = ps.gate_begin; max_gates_ = max_gates;
+        // the low tile loads and stores in layout B (coalesced); high tiles start in A
         int layout = low ? 1 : 0;
         ps.first_layout = layout;
         int total = 0, idle = 0;
@@ -289,89 +295,54 @@ class FusedScheduler {
         while (idle < 2) {
             size_t mark = P_.mops.size();
             if (pending_x) P_.mops.push_back({(uint8_t)(layout == 1 ? MC_XAB : MC_XBA), 0, 0});
-            int n = run_phase(a, W, low, layout, max_tables);
+            int rounds = 0;
+            int n = run_phase(a, low, layout, rounds);
             if (n == 0) { P_.mops.resize(mark); ++idle; layout ^= 1; pending_x = !pending_x; continue; }
-            total += n; idle = 0; ++ps.n_phases;
+            total += n; idle = 0; ++ps.n_phases; ps.n_rounds += rounds;
             layout ^= 1; pending_x = true;
         }
-        // `layout` was toggled `idle`(=2) times past the last productive phase plus once after it
-        int last = layout ^ 1;                          // undo: toggles after last productive phase = 1 + 2
+        int last = layout ^ 1;                          // the layout of the last productive phase
         if (ps.n_phases == 0) last = ps.first_layout;
         if (low && last != 1) { P_.mops.push_back({MC_XAB, 0, 0}); last = 1; }
         ps.last_layout = last;
         P_.mops.push_back({MC_END, 0, 0});
-        ps.mop_end = (int)P_.mops.size(); ps.gate_end = (int)P_.gate_jv.size();
-        ps.table_end = (int)P_.tables.size();
+        ps.mop_end = (int)P_.mops.size(); ps.gate_end = (int)P_.gate_rc.size();
         return total;
     }
   private:
-    // position of column c in the register index of this layout: 0..6, 7 = outer neighbour, -1 = no
-    int pos_in(int a, int W, bool low, int layout, int c) const {
-        for (int b = 0; b < F_RB; ++b) if (a + fused_digit_of_bit(low, layout, b) == c) return b;
-        if (layout == 0 && c == a - 1) return 7;
-        if (layout == 1 && c == a + W) return 7;
-        return -1;
+    bool legal(int c) const {
+        const int r = grow_[c];
+        if (r >= L_) return false;
+        if (c > 0 && grow_[c - 1] < r) return false;
+        if (c + 1 < L_ && grow_[c + 1] < r) return false;
+        return true;
     }
-    int run_phase(int a, int W, bool low, int layout, int max_tables) {
-        int n = 0; bool progress = true;
-        int cols[F_RB];
-        for (int b = 0; b < F_RB; ++b) cols[b] = a + fused_digit_of_bit(low, layout, b);
-        while (progress) {
-            progress = false;
-            if ((int)P_.tables.size() - pass_table_begin_ >= max_tables) break;
-            // ---- a table with every diagonal term that is legal and expressible here -----------
-            int tb = (int)P_.terms.size();
-            for (int b = 0; b < F_RB; ++b) {
-                int c = cols[b];
-                int r = grow_[c] - 1;
-                if (!dh_[r * L_ + c]) {
-                    dh_[r * L_ + c] = 1;
-                    P_.terms.push_back({OP_DH, (uint8_t)b, 0, 0, (uint16_t)r, (uint16_t)c});
-                }
-                for (int cc = c - 1; cc <= c; ++cc) {
-                    if (cc < 0 || cc + 1 >= L_) continue;
-                    int pa = pos_in(a, W, low, layout, cc), pb = pos_in(a, W, low, layout, cc + 1);
-                    if (pa < 0 || pb < 0 || (pa == 7 && pb == 7)) continue;
-                    if (grow_[cc] != grow_[cc + 1]) continue;
-                    int rr = grow_[cc] - 1;
-                    if (dj_[rr * (L_ - 1) + cc]) continue;
-                    dj_[rr * (L_ - 1) + cc] = 1;
-                    P_.terms.push_back({OP_DJ, (uint8_t)pa, (uint8_t)pb, 0, (uint16_t)rr, (uint16_t)cc});
-                }
+    int run_phase(int a, bool low, int layout, int& rounds) {
+        int n = 0;
+        for (;;) {
+            if ((int)P_.gate_rc.size() - pass_gate_begin_ + F_RB > max_gates_) break;
+            unsigned mask = 0;
+            for (int b = 0; b < F_RB; ++b) if (legal(a + fused_digit_of_bit(low, layout, b))) mask |= 1u << b;
+            if (!mask) break;
+            P_.mops.push_back({MC_ROUND, (uint8_t)mask, (uint16_t)((int)P_.gate_rc.size() - pass_gate_begin_)});
+            for (int b = 0; b < F_RB; ++b) if (mask >> b & 1) {
+                const int c = a + fused_digit_of_bit(low, layout, b);
+                P_.gate_rc.push_back(grow_[c] * 64 + c);
+                ++n;
             }
-            if ((int)P_.terms.size() > tb) {
-                P_.tables.push_back({tb, (int)P_.terms.size(), layout});
-                int local = (int)P_.tables.size() - 1 - pass_table_begin_;
-                P_.mops.push_back({MC_TABLE, (uint8_t)layout, (uint16_t)local});
-                n += (int)P_.terms.size() - tb; progress = true;
-            }
-            // ---- every legal gate on a register digit ----------------------------------------------
-            for (int b = 0; b < F_RB; ++b) {
-                int c = cols[b];
-                int r = grow_[c];
-                if (r >= L_) continue;
-                bool ok = dh_[(r - 1) * L_ + c] != 0;
-                if (c > 0) ok = ok && dj_[(r - 1) * (L_ - 1) + c - 1];
-                if (c + 1 < L_) ok = ok && dj_[(r - 1) * (L_ - 1) + c];
-                if (!ok) continue;
-                grow_[c] += 1;
-                int local = (int)P_.gate_jv.size() - pass_gate_begin_;
-                P_.gate_jv.push_back((r - 1) * L_ + c);
-                P_.mops.push_back({MC_GATE, (uint8_t)b, (uint16_t)local});
-                ++n; progress = true;
-            }
+            for (int b = 0; b < F_RB; ++b) if (mask >> b & 1) grow_[a + fused_digit_of_bit(low, layout, b)] += 1;
+            ++rounds;
         }
         return n;
     }
     int L_; FusedPlan& P_;
-    std::vector<int> grow_;
-    std::vector<uint8_t> dh_, dj_;
-    int pass_table_begin_ = 0, pass_gate_begin_ = 0;
+    std::vector<int> grow_;      // grow[c] = rows complete on digit c (row 0 needs no gate)
+    int pass_gate_begin_ = 0, max_gates_ = 1 << 30;
 };
 
 // Tile cycle: the low tile [0,12), then high tiles [x, x+9) advancing by `stride`, the last
 // flush with L.  Chooses the stride with the lowest estimated cost.
-inline FusedPlan make_fused_plan(int L, bool has_field, int max_tables_low, int max_tables_high) {
+inline FusedPlan make_fused_plan(int L, int max_gates_per_pass) {
     FusedPlan best;
     if (L < F_WLOW) return best;
     double best_cost = -1;
@@ -389,13 +360,13 @@ inline FusedPlan make_fused_plan(int L, bool has_field, int max_tables_low, int 
             }
         }
         FusedPlan p; p.L = L;
-        FusedScheduler s(L, has_field, p);
+        FusedScheduler s(L, p);
         size_t k = 0; int idle = 0; bool first = true;
         while ((first || !s.done()) && p.passes.size() < 4096) {
             int a = starts[k % starts.size()]; ++k;
             FusedPass ps{};
             size_t m0 = p.mops.size();
-            int n = s.run_pass(a, a == 0, a == 0 ? max_tables_low : max_tables_high, ps);
+            int n = s.run_pass(a, a == 0, max_gates_per_pass, ps);
             if (n == 0 && !first) { p.mops.resize(m0); if (++idle > (int)starts.size()) break; continue; }
             idle = 0;
             if (first) ps.flags |= PASS_INIT;
@@ -403,13 +374,14 @@ inline FusedPlan make_fused_plan(int L, bool has_field, int max_tables_low, int 
             p.passes.push_back(ps);
         }
         if (!s.done()) continue;
+        // the last pass adds A_{L-1}(s) and reduces: MC_FINAL replaces its MC_END
         p.passes.back().flags |= PASS_REDUCE;
-        // cost model (issue slots per thread, 128 elements): gate 192, table 96, exchange 64,
-        // dispatch 6 per micro-op; one HBM pass ~ 2500 (5.7 ms at 6 TB/s vs 64 updates/clk/SM)
+        p.mops.back().code = MC_FINAL;
+        // cost model (issue slots per thread, 128 elements): gate 192, round 12, exchange 80;
+        // one HBM pass ~ 2500 (5.7 ms at 6 TB/s vs 64 updates/clk/SM)
         double cost = 0;
         for (auto& ps : p.passes)
-            cost += 2500.0 + 192.0 * (ps.gate_end - ps.gate_begin) + 96.0 * (ps.table_end - ps.table_begin) +
-                    64.0 * ps.n_phases + 6.0 * (ps.mop_end - ps.mop_begin);
+            cost += 2500.0 + 192.0 * (ps.gate_end - ps.gate_begin) + 12.0 * ps.n_rounds + 80.0 * ps.n_phases;
         if (best_cost < 0 || cost < best_cost) { best = p; best_cost = cost; best.ok = true; }
     }
     return best;
@@ -417,14 +389,14 @@ inline FusedPlan make_fused_plan(int L, bool has_field, int max_tables_low, int 
 
 inline std::string describe_fused(const FusedPlan& p) {
     std::string out; char line[200];
-    snprintf(line, sizeof line, "fused L=%d passes=%zu mops=%zu gates=%zu tables=%zu terms=%zu\n", p.L,
-             p.passes.size(), p.mops.size(), p.gate_jv.size(), p.tables.size(), p.terms.size());
+    snprintf(line, sizeof line, "fused L=%d passes=%zu mops=%zu gates=%zu\n", p.L,
+             p.passes.size(), p.mops.size(), p.gate_rc.size());
     out += line;
     for (size_t i = 0; i < p.passes.size(); ++i) {
         const FusedPass& ps = p.passes[i];
-        snprintf(line, sizeof line, "fpass %zu a=%d W=%d low=%d flags=%d first=%d last=%d phases=%d gates=%d tables=%d\n", i,
-                 ps.a, ps.W, ps.low, ps.flags, ps.first_layout, ps.last_layout, ps.n_phases,
-                 ps.gate_end - ps.gate_begin, ps.table_end - ps.table_begin);
+        snprintf(line, sizeof line, "fpass %zu a=%d W=%d low=%d flags=%d first=%d last=%d phases=%d rounds=%d gates=%d\n", i,
+                 ps.a, ps.W, ps.low, ps.flags, ps.first_layout, ps.last_layout, ps.n_phases, ps.n_rounds,
+                 ps.gate_end - ps.gate_begin);
         out += line;
         for (int k = ps.mop_begin; k < ps.mop_end; ++k) {
             const MicroOp& m = p.mops[k];
@@ -432,18 +404,14 @@ inline std::string describe_fused(const FusedPlan& p) {
                 case MC_XAB: out += "m xAB\n"; break;
                 case MC_XBA: out += "m xBA\n"; break;
                 case MC_END: out += "m end\n"; break;
-                case MC_GATE: {
-                    int jv = p.gate_jv[ps.gate_begin + m.arg];
-                    snprintf(line, sizeof line, "m gate k=%d r=%d c=%d\n", m.k, jv / p.L + 1, jv % p.L);
-                    out += line; break; }
-                case MC_TABLE: {
-                    const FusedTable& t = p.tables[ps.table_begin + m.arg];
-                    snprintf(line, sizeof line, "m table layout=%d nterms=%d\n", t.layout, t.term_end - t.term_begin);
+                case MC_FINAL: out += "m final\n"; break;
+                case MC_ROUND: {
+                    snprintf(line, sizeof line, "m round mask=%d first=%d\n", m.mask, m.arg);
                     out += line;
-                    for (int q = t.term_begin; q < t.term_end; ++q) {
-                        const TableTerm& tt = p.terms[q];
-                        snprintf(line, sizeof line, "t %s r=%d c=%d pa=%d pb=%d\n", tt.type == OP_DH ? "dh" : "dJ",
-                                 tt.row, tt.col, tt.posA, tt.posB);
+                    int g = ps.gate_begin + m.arg;
+                    for (int b = 0; b < F_RB; ++b) if (m.mask >> b & 1) {
+                        const int rc = p.gate_rc[g++];
+                        snprintf(line, sizeof line, "g k=%d r=%d c=%d\n", b, rc / 64, rc % 64);
                         out += line;
                     }
                     break; }

@@ -70,10 +70,10 @@ bool limits_ok(int q, int L, bool count, bool config) {
 struct Layout {
     size_t x = 0, n = 0, ckpt = 0, Jh = 0, Jv = 0, h = 0, ops = 0, part_x = 0, part_n = 0,
            amax_v = 0, amax_s = 0, out_x = 0, out_n = 0, out_s = 0, sigma = 0, total = 0;
-    size_t f_mops = 0, f_gate_jv = 0, f_tables = 0, f_terms = 0, f_gate_m = 0, f_table_vals = 0;
+    size_t f_mops = 0, f_gate_rc = 0, f_gate_k = 0, f_final = 0;
     unsigned long long NS = 0, max_tiles = 0;
     int amax_blocks = 0;
-    int f_max_gates = 0, f_max_tables = 0, f_max_terms = 0, f_max_mops = 0;
+    int f_max_gates = 0, f_max_mops = 0;
 };
 
 // The fused register-phase path serves the Ising Tropical<f32> energy sweep for L >= 12.
@@ -111,13 +111,11 @@ Layout make_layout(int q, int L, bool count, bool config, int batch) {
     y.out_s = take((size_t)batch * 8);
     y.sigma = take((size_t)batch * L * L);
     if (fused_eligible(q, L, count, config)) {
-        y.f_max_gates = L * L; y.f_max_tables = 3 * L * L; y.f_max_terms = 2 * L * L; y.f_max_mops = 8 * L * L + 64;
+        y.f_max_gates = L * L; y.f_max_mops = 4 * L * L + 64;
         y.f_mops = take((size_t)y.f_max_mops * sizeof(ttn::MicroOp));
-        y.f_gate_jv = take((size_t)y.f_max_gates * 4);
-        y.f_tables = take((size_t)y.f_max_tables * sizeof(ttn::FusedTable));
-        y.f_terms = take((size_t)y.f_max_terms * sizeof(ttn::TableTerm));
-        y.f_gate_m = take((size_t)batch * y.f_max_gates * 4);
-        y.f_table_vals = take((size_t)batch * y.f_max_tables * 256 * 4);
+        y.f_gate_rc = take((size_t)y.f_max_gates * 4);
+        y.f_gate_k = take((size_t)batch * y.f_max_gates * 8 * 4);
+        y.f_final = take((size_t)batch * ttn::FFINAL_FLOATS * 4);
     }
     y.total = off;
     return y;
@@ -205,12 +203,16 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
     pp.tiles_per_inst = y.NS >> 12;
     pp.mops = reinterpret_cast<const ttn::MicroOp*>(P->ws + y.f_mops) + ps.mop_begin;
     pp.n_mops = ps.mop_end - ps.mop_begin;
-    pp.gate_m = reinterpret_cast<const float*>(P->ws + y.f_gate_m) + ps.gate_begin;
-    pp.gate_inst_stride = (int)fp.gate_jv.size();
-    pp.tables = reinterpret_cast<const float*>(P->ws + y.f_table_vals) + (size_t)ps.table_begin * 256;
-    pp.n_tables = ps.table_end - ps.table_begin;
-    pp.table_inst_stride = (unsigned long long)fp.tables.size() * 256;
+    pp.gate_k = reinterpret_cast<const float*>(P->ws + y.f_gate_k) + (size_t)ps.gate_begin * 8;
+    pp.n_gates = ps.gate_end - ps.gate_begin;
+    pp.gate_inst_stride = (unsigned long long)fp.gate_rc.size() * 8;
+    pp.final_tab = reinterpret_cast<const float*>(P->ws + y.f_final);
     pp.part_x = reinterpret_cast<float*>(P->ws + y.part_x);
+    {   // one tile's gate phase when a warp has the alu pipe to itself: 128 FMNMX x 2 cycles per gate
+        unsigned st = (unsigned)(ps.gate_end - ps.gate_begin) * 256u;
+        if (const char* e = getenv("TTN_DEBUG_STAGGER")) st = (unsigned)(atof(e) * st);
+        pp.stagger_cycles = st;
+    }
     unsigned long long grid = (unsigned long long)P->fused_grid;
     const int nw = ttn::fwarps(ps.low != 0);
     const unsigned long long need = (pp.tiles_per_inst + nw - 1) / nw;
@@ -219,39 +221,37 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
     else ttn::fused_pass_kernel<false><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(false), st>>>(pp);
     TTN_CUDA(cudaGetLastError());
     if (ps.flags & ttn::PASS_REDUCE) {
+        // one partial per CTA and instance
         ttn::final_reduce_kernel<false><<<P->batch, 256, 0, st>>>(
-            pp.part_x, nullptr, pp.tiles_per_inst, reinterpret_cast<float*>(P->ws + y.out_x), nullptr);
+            pp.part_x, nullptr, grid, reinterpret_cast<float*>(P->ws + y.out_x), nullptr);
         TTN_CUDA(cudaGetLastError());
     }
     return TTN_OK;
 }
 
-// Uploads the fused program and runs the S0 prep kernel (gate constants + diagonal tables).
+// Uploads the fused program and runs the S0 prep kernel (gate constants + final table).
 static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
     const Layout& y = P->lay;
     ttn::FusedPlan& fp = P->fplan;
-    if ((int)fp.gate_jv.size() > y.f_max_gates || (int)fp.tables.size() > y.f_max_tables ||
-        (int)fp.terms.size() > y.f_max_terms || (int)fp.mops.size() > y.f_max_mops)
+    if ((int)fp.gate_rc.size() > y.f_max_gates || (int)fp.mops.size() > y.f_max_mops)
         return fail(TTN_EUNSUPPORTED, "fused plan exceeds its workspace bounds");
     for (const auto& ps : fp.passes)
-        if (ps.mop_end - ps.mop_begin > ttn::FMAX_MOPS || ps.table_end - ps.table_begin > ttn::fmax_tables(ps.low != 0) ||
+        if (ps.mop_end - ps.mop_begin > ttn::FMAX_MOPS || ps.gate_end - ps.gate_begin > ttn::FMAX_GATES ||
             (ps.low && (ps.first_layout != 1 || ps.last_layout != 1)))
             return fail(TTN_EUNSUPPORTED, "fused pass program out of bounds");
     TTN_CUDA(cudaMemcpyAsync(P->ws + y.f_mops, fp.mops.data(), fp.mops.size() * sizeof(ttn::MicroOp), cudaMemcpyHostToDevice, st));
-    TTN_CUDA(cudaMemcpyAsync(P->ws + y.f_gate_jv, fp.gate_jv.data(), fp.gate_jv.size() * 4, cudaMemcpyHostToDevice, st));
-    TTN_CUDA(cudaMemcpyAsync(P->ws + y.f_tables, fp.tables.data(), fp.tables.size() * sizeof(ttn::FusedTable), cudaMemcpyHostToDevice, st));
-    TTN_CUDA(cudaMemcpyAsync(P->ws + y.f_terms, fp.terms.data(), fp.terms.size() * sizeof(ttn::TableTerm), cudaMemcpyHostToDevice, st));
+    TTN_CUDA(cudaMemcpyAsync(P->ws + y.f_gate_rc, fp.gate_rc.data(), fp.gate_rc.size() * 4, cudaMemcpyHostToDevice, st));
     ttn::FusedPrepParams q{};
-    q.L = P->L; q.n_gates = (int)fp.gate_jv.size(); q.n_tables = (int)fp.tables.size();
-    q.gate_jv = reinterpret_cast<const int*>(P->ws + y.f_gate_jv);
-    q.tables = reinterpret_cast<const ttn::FusedTable*>(P->ws + y.f_tables);
-    q.terms = reinterpret_cast<const ttn::TableTerm*>(P->ws + y.f_terms);
+    q.L = P->L; q.n_gates = (int)fp.gate_rc.size();
+    q.gate_rc = reinterpret_cast<const int*>(P->ws + y.f_gate_rc);
     q.Jh = reinterpret_cast<const float*>(P->ws + y.Jh);
     q.Jv = reinterpret_cast<const float*>(P->ws + y.Jv);
     q.h = P->has_field ? reinterpret_cast<const float*>(P->ws + y.h) : nullptr;
-    q.gate_m = reinterpret_cast<float*>(P->ws + y.f_gate_m);
-    q.table_out = reinterpret_cast<float*>(P->ws + y.f_table_vals);
-    long work = (long)q.n_tables * 256; if (q.n_gates > work) work = q.n_gates;
+    q.gate_k = reinterpret_cast<float*>(P->ws + y.f_gate_k);
+    q.final_tab = reinterpret_cast<float*>(P->ws + y.f_final);
+    const ttn::FusedPass& lastp = fp.passes.back();
+    q.fin_low = lastp.low; q.fin_layout = lastp.last_layout; q.fin_a = lastp.a;
+    long work = ttn::FFINAL_FLOATS; if (q.n_gates > work) work = q.n_gates;
     dim3 grid((unsigned)((work + 255) / 256), (unsigned)P->batch);
     ttn::fused_prep_kernel<<<grid, 256, 0, st>>>(q);
     TTN_CUDA(cudaGetLastError());
@@ -285,7 +285,7 @@ long ttn_plan_describe(int q, int L, ttn_call call, char* buf, size_t n) {
     if (!limits_ok(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) return -1;
     std::string s;
     if (fused_eligible(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) {
-        ttn::FusedPlan fp = ttn::make_fused_plan(L, /*has_field=*/true, ttn::FMAX_TABLES_LOW, ttn::FMAX_TABLES_HIGH);
+        ttn::FusedPlan fp = ttn::make_fused_plan(L, ttn::FMAX_GATES);
         if (fp.ok) s = ttn::describe_fused(fp);
     }
     if (s.empty()) s = ttn::describe(plan_for(q, L, call, /*has_field=*/q == 2));
@@ -331,7 +331,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     P->lay = lay;
     P->ws = static_cast<unsigned char*>(workspace);
     if (fused_eligible(q, L, count, config)) {
-        P->fplan = ttn::make_fused_plan(L, P->has_field, ttn::FMAX_TABLES_LOW, ttn::FMAX_TABLES_HIGH);
+        P->fplan = ttn::make_fused_plan(L, ttn::FMAX_GATES);
         P->fused = P->fplan.ok;
     }
     if (!P->fused) P->plan = plan_for(q, L, call, P->has_field);

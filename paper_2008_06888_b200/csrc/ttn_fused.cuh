@@ -1,18 +1,20 @@
-// ttn_fused.cuh -- fused register-phase pass kernel for the Ising Tropical<f32> sweep ("v2").
+// ttn_fused.cuh -- fused register-phase pass kernel for the Ising Tropical<f32> sweep ("v3",
+// diagonal frame; see planner.h for the frame and the schedule).
 //
 // One launch = one HBM pass.  Each WARP owns a tile of 2^12 state elements,
-// 128 per thread, and runs the pass's micro-op program (planner.h, FusedPlan) on it with no
-// CTA-level cooperation:
-//   * max-plus gates (A2) PAPER.md:242 on a register digit:  v[j] = max(v[j], v[j ^ bit] + m),
-//     m = -2 J, the common +J deferred to a scalar (ttn_api.cu): 1 FMNMX + 1/2 FADD2 per element;
-//   * diagonal gates (A3), (A4) PAPER.md:247-252 as 128-entry tables in shared memory:
-//     v[j] += T[j]  (1/2 FADD2 + 1/4 LDS.128 per element);
+// 128 per thread, and runs the pass's micro-op program on it with no CTA-level cooperation:
+//   * conjugated max-plus gates (A2) PAPER.md:242 on a register digit:
+//         a' = max(a, b + ka[n]),  b' = max(b, a + kb[n]),   n = (bit c-1, bit c+1) of the index,
+//     the row diagonals (A3), (A4) PAPER.md:247-252 folded into the 8 constants of the gate and
+//     the common +Jv deferred to a scalar (ttn_api.cu): 1 FMNMX + 1/2 FADD2 per element;
 //   * layout exchanges A <-> B through the warp's private shared-memory region with 128-bit,
-//     bank-conflict-free accesses, synchronised with __syncwarp only.
+//     bank-conflict-free accesses, synchronised with __syncwarp only;
+//   * the last pass adds the accumulated diagonal A_{L-1}(s) (a 128-entry table over the
+//     register digits in 4 boundary variants + a per-thread scalar) and max-reduces.
 // Global traffic goes straight between HBM and registers: the LOW tile (columns 0..11) moves
 // 128-byte lines; HIGH tiles (columns a..a+8 plus the riding columns 0..2 on the low lane bits)
 // move whole 32-byte sectors, four per request.  The kernel is persistent (one CTA per SM);
-// programs, gate constants and tables are staged in shared memory once per launch.
+// programs and gate constants are staged in shared memory once per launch and instance.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -20,18 +22,18 @@
 
 namespace ttn {
 
-// Warps per CTA (one CTA per SM) and table budget per pass.  The LOW kernel's global accesses
-// need no address registers, so it fits 12 warps of 168 registers (3 per scheduler: 87 % of the
-// FMNMX peak in the gate phases vs 78 % with 2); the HIGH kernel keeps 8 warps of 255 registers
-// so that all 128 strided loads of a tile stay in flight.
+// Warps per CTA (one CTA per SM).  The LOW kernel's global accesses need no address registers,
+// so it fits 12 warps of 168 registers (3 per scheduler); the HIGH kernel keeps 8 warps of 255
+// registers so that all 128 strided loads of a tile stay in flight.
 constexpr int FWARPS_LOW = 12, FWARPS_HIGH = 8;
-constexpr int FMAX_TABLES_LOW = 24, FMAX_TABLES_HIGH = 32;   // 1 KiB each: 2 variants x 128
 constexpr int FREGION_F4 = 33 * 32;       // float4 per warp exchange region (low tile: padded rows)
-constexpr int FMAX_MOPS = 256;            // micro-ops per pass
+constexpr int FMAX_MOPS = 128;            // micro-ops per pass
+constexpr int FMAX_GATES = 160;           // gates per pass (8 constants each)
+constexpr int FFINAL_FLOATS = 4 * 128 + 2 * 64;   // final table (4 variants) + H[64] + K[64]
 __host__ __device__ constexpr int fwarps(bool low) { return low ? FWARPS_LOW : FWARPS_HIGH; }
-__host__ __device__ constexpr int fmax_tables(bool low) { return low ? FMAX_TABLES_LOW : FMAX_TABLES_HIGH; }
 __host__ __device__ constexpr size_t fsmem_bytes(bool low) {
-    return (size_t)fwarps(low) * FREGION_F4 * 16 + (size_t)fmax_tables(low) * 1024 + (size_t)FMAX_MOPS * 8;
+    return (size_t)fwarps(low) * FREGION_F4 * 16 + (size_t)FMAX_GATES * 32 + (size_t)FFINAL_FLOATS * 4 +
+           (size_t)FMAX_MOPS * 4 + 64;
 }
 
 struct FusedParams {
@@ -40,12 +42,12 @@ struct FusedParams {
     unsigned long long inst_stride;     // elements between instances
     unsigned long long tiles_per_inst;  // warp tiles (2^12 elements) per instance
     const MicroOp* mops; int n_mops;    // this pass's program
-    const float* gate_m; int gate_inst_stride;                    // this pass's slice, instance 0
-    const float* tables; int n_tables; unsigned long long table_inst_stride;   // this pass's slice
-    float* part_x;                      // [batch][tiles_per_inst] (REDUCE)
+    const float* gate_k; int n_gates;   // [inst][all gates][8]; this pass's slice of instance 0
+    unsigned long long gate_inst_stride;          // floats between instances
+    const float* final_tab;             // [inst][FFINAL_FLOATS] (REDUCE pass only)
+    float* part_x;                      // [batch][gridDim.x] (REDUCE)
+    unsigned stagger_cycles;            // start delay per warp group (warp / 4), see the kernel
 };
-
-struct FMop { unsigned ctrl; float m; };  // predecoded: ctrl = code | k << 8 | arg << 16
 
 // (o0, o1) = (a0 + b0, a1 + b1) in one FADD2
 __device__ __forceinline__ void add2(float& o0, float& o1, float a0, float a1, float b0, float b1) {
@@ -57,15 +59,29 @@ __device__ __forceinline__ void add2(float& o0, float& o1, float a0, float a1, f
         : "=f"(o0), "=f"(o1) : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
 }
 
-// ---- gate on register-index bit K: v[j] <- max(v[j], v[j^bit] + m) ---------------------------
-template <int K>
-__device__ __forceinline__ void fgate(float (&v)[128], const float m) {
+// ---- conjugated gate on register-index bit K ------------------------------------------------------
+// NL / NH: register-index bit holding the left / right neighbour column, or -1 when that
+// neighbour is constant per thread (its value is then tl / th).  k[0..3] = ka[nl][nh],
+// k[4..7] = kb[nl][nh].
+template <int K, int NL, int NH>
+__device__ __forceinline__ void cgate(float (&v)[128], const float4 c0, const float4 c1, const int tl, const int th) {
+    float ka[2][2] = {{c0.x, c0.y}, {c0.z, c0.w}}, kb[2][2] = {{c1.x, c1.y}, {c1.z, c1.w}};
+    if (NL < 0) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) { ka[0][h] = tl ? ka[1][h] : ka[0][h]; kb[0][h] = tl ? kb[1][h] : kb[0][h]; }
+    }
+    if (NH < 0) {
+#pragma unroll
+        for (int l = 0; l < 2; ++l) { ka[l][0] = th ? ka[l][1] : ka[l][0]; kb[l][0] = th ? kb[l][1] : kb[l][0]; }
+    }
     constexpr int B = 1 << K;
+#define TTN_NL(j) (NL < 0 ? 0 : (((j) >> (NL < 0 ? 0 : NL)) & 1))
+#define TTN_NH(j) (NH < 0 ? 0 : (((j) >> (NH < 0 ? 0 : NH)) & 1))
     if (K == 0) {
 #pragma unroll
         for (int j = 0; j < 128; j += 2) {
-            float t0, t1;
-            add2(t0, t1, v[j], v[j + 1], m, m);
+            float t0, t1;     // t0 = a + kb (candidate for b), t1 = b + ka (candidate for a)
+            add2(t0, t1, v[j], v[j + 1], kb[TTN_NL(j)][TTN_NH(j)], ka[TTN_NL(j)][TTN_NH(j)]);
             v[j] = fmaxf(v[j], t1);
             v[j + 1] = fmaxf(v[j + 1], t0);
         }
@@ -74,22 +90,36 @@ __device__ __forceinline__ void fgate(float (&v)[128], const float m) {
         for (int j = 0; j < 128; j += 2) {
             if ((j & B) == 0) {
                 float a0, a1, b0, b1;
-                add2(a0, a1, v[j], v[j + 1], m, m);
-                add2(b0, b1, v[j + B], v[j + B + 1], m, m);
+                add2(a0, a1, v[j], v[j + 1], kb[TTN_NL(j)][TTN_NH(j)], kb[TTN_NL(j + 1)][TTN_NH(j + 1)]);
+                add2(b0, b1, v[j + B], v[j + B + 1], ka[TTN_NL(j)][TTN_NH(j)], ka[TTN_NL(j + 1)][TTN_NH(j + 1)]);
                 v[j] = fmaxf(v[j], b0); v[j + 1] = fmaxf(v[j + 1], b1);
                 v[j + B] = fmaxf(v[j + B], a0); v[j + B + 1] = fmaxf(v[j + B + 1], a1);
             }
         }
     }
+#undef TTN_NL
+#undef TTN_NH
 }
 
-__device__ __forceinline__ void ftable(float (&v)[128], const float4* __restrict__ T) {
-#pragma unroll
-    for (int q = 0; q < 32; ++q) {
-        const float4 t = T[q];
-        add2(v[4 * q], v[4 * q + 1], v[4 * q], v[4 * q + 1], t.x, t.y);
-        add2(v[4 * q + 2], v[4 * q + 3], v[4 * q + 2], v[4 * q + 3], t.z, t.w);
+// register bit of the left / right neighbour of the digit held by register bit K (-1: per thread)
+template <bool LOW, int LAYOUT, int K> struct Nbr {
+    static constexpr int d = fused_digit_of_bit(LOW, LAYOUT, K);
+    static constexpr int W = LOW ? F_WLOW : F_WHIGH;
+    static constexpr int NL = d == 0 ? -1 : fused_bit_of_digit(LOW, LAYOUT, d - 1);
+    static constexpr int NH = d == W - 1 ? -1 : fused_bit_of_digit(LOW, LAYOUT, d + 1);
+};
+
+// One round: for every set bit of `mask` (ascending) the next gate of that register digit.
+template <bool LOW, int LAYOUT>
+__device__ __forceinline__ void fround(float (&v)[128], const unsigned mask, const float4* __restrict__ gk,
+                                       const int tl, const int th) {
+#define TTN_G(Kk)                                                                                   \
+    if (mask & (1u << Kk)) {                                                                        \
+        const float4 c0 = gk[0], c1 = gk[1]; gk += 2;                                               \
+        cgate<Kk, Nbr<LOW, LAYOUT, Kk>::NL, Nbr<LOW, LAYOUT, Kk>::NH>(v, c0, c1, tl, th);           \
     }
+    TTN_G(0) TTN_G(1) TTN_G(2) TTN_G(3) TTN_G(4) TTN_G(5) TTN_G(6)
+#undef TTN_G
 }
 
 // ---- exchange addressing: float4 index of register quad q for this lane -------------------------
@@ -153,51 +183,89 @@ __device__ __forceinline__ void gmove(float (&v)[128], float* tile, int lane, in
     }
 }
 
+// ---- last pass: v[j] += A_{L-1}(s) -------------------------------------------------------------------
+// s_fin = [4 variants][128] table over the register digits (variant = tl + 2 th: the two boundary
+// couplings to the per-thread neighbours) followed by H[64], K[64] (accumulated fields and
+// horizontal couplings).  x0 = first register column; sthr = the element index with the register
+// digits cleared.
+__device__ __forceinline__ float final_thread_const(const float* s_fin, int L, int x0, unsigned long long sthr) {
+    const float* H = s_fin + 512; const float* Kc = s_fin + 576;
+    float acc = 0.f;
+    for (int c = 0; c < L; ++c) {
+        const bool in_r = (c >= x0 && c < x0 + F_RB);
+        const int bc = (int)((sthr >> c) & 1ull);
+        if (!in_r) acc += bc ? -H[c] : H[c];
+        if (c + 1 < L) {
+            const bool in_r1 = (c + 1 >= x0 && c + 1 < x0 + F_RB);
+            if (!in_r && !in_r1) {
+                const int b1 = (int)((sthr >> (c + 1)) & 1ull);
+                acc += (bc == b1) ? Kc[c] : -Kc[c];
+            }
+        }
+    }
+    return acc;
+}
+
 template <bool LOW>
 __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const FusedParams p) {
     constexpr int FWARPS = fwarps(LOW);
-    constexpr int FMAX_TABLES = fmax_tables(LOW);
     extern __shared__ __align__(16) unsigned char fsm_raw[];
     float4* regions = reinterpret_cast<float4*>(fsm_raw);                              // FWARPS * FREGION_F4
-    float* s_tab = reinterpret_cast<float*>(fsm_raw + (size_t)FWARPS * FREGION_F4 * 16); // FMAX_TABLES * 256
-    FMop* s_mops = reinterpret_cast<FMop*>(fsm_raw + (size_t)FWARPS * FREGION_F4 * 16 + (size_t)FMAX_TABLES * 1024);
+    float4* s_gk = reinterpret_cast<float4*>(fsm_raw + (size_t)FWARPS * FREGION_F4 * 16);   // FMAX_GATES * 2
+    float* s_fin = reinterpret_cast<float*>(s_gk + FMAX_GATES * 2);                     // FFINAL_FLOATS
+    unsigned* s_mops = reinterpret_cast<unsigned*>(s_fin + FFINAL_FLOATS);              // FMAX_MOPS
+    float* s_red = reinterpret_cast<float*>(s_mops + FMAX_MOPS);                        // FWARPS (<= 16)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     float4* myreg = regions + warp * FREGION_F4;
     const unsigned long long gw = (unsigned long long)blockIdx.x * FWARPS + warp;
     const unsigned long long nw = (unsigned long long)gridDim.x * FWARPS;
     const unsigned long long estride = 1ull << p.a;
 
+    // De-phase the warps of one scheduler (warps w, w+4, w+8 share SM sub-partition w % 4).  All
+    // tiles cost the same and the schedulers share the alu pipe fairly, so warps that start
+    // together stay in lock-step: they all compute, then all wait on memory, and the two never
+    // overlap.  Starting group g one gate-phase later keeps one group in its memory phase while
+    // the others compute.
+    if (p.stagger_cycles && warp >= 4) {
+        const long long t_end = clock64() + (long long)(warp >> 2) * p.stagger_cycles;
+        while (clock64() < t_end) __nanosleep(256);
+    }
+
     for (int inst = 0; inst < p.batch; ++inst) {
-        // ---- stage this instance's program constants and tables (S0 outputs) into shared memory
+        // ---- stage this instance's program and gate constants (S0 outputs) into shared memory
         __syncthreads();
         for (int i = tid; i < p.n_mops; i += blockDim.x) {
             const MicroOp mo = p.mops[i];
-            FMop f;
-            f.ctrl = (unsigned)mo.code | ((unsigned)mo.k << 8) | ((unsigned)mo.arg << 16);
-            f.m = (mo.code == MC_GATE) ? p.gate_m[(size_t)inst * p.gate_inst_stride + mo.arg] : 0.f;
-            s_mops[i] = f;
+            s_mops[i] = (unsigned)mo.code | ((unsigned)mo.mask << 8) | ((unsigned)mo.arg << 16);
         }
         {
-            const float4* src = reinterpret_cast<const float4*>(p.tables + (size_t)inst * p.table_inst_stride);
-            float4* dst = reinterpret_cast<float4*>(s_tab);
-            for (int i = tid; i < p.n_tables * 64; i += blockDim.x) dst[i] = src[i];
+            const float4* src = reinterpret_cast<const float4*>(p.gate_k + (size_t)inst * p.gate_inst_stride);
+            for (int i = tid; i < p.n_gates * 2; i += blockDim.x) s_gk[i] = src[i];
         }
+        if (p.flags & PASS_REDUCE)
+            for (int i = tid; i < FFINAL_FLOATS; i += blockDim.x) s_fin[i] = p.final_tab[(size_t)inst * FFINAL_FLOATS + i];
         __syncthreads();
         float* S = p.state + (unsigned long long)inst * p.inst_stride;
+        float wmax = -INFINITY;
 
         for (unsigned long long wt = gw; wt < p.tiles_per_inst; wt += nw) {
-            // ---- tile geometry ------------------------------------------------------------------
+            // ---- tile geometry: base index, per-thread neighbour bits ------------------------------
             unsigned long long base;
-            int vA = 0, vB = 0;
+            int tlA, thA, tlB, thB;     // per-thread left / right neighbour bit in layout A / B
             if (LOW) {
                 base = wt << 12;
-                vB = (p.L > F_WLOW) ? (int)(wt & 1ull) : 0;                       // column 12
+                tlA = 0;                                   // column -1 does not exist
+                thA = lane & 1;                            // d7 (lane bit 0 in layout A)
+                tlB = (lane >> 4) & 1;                     // d4 (lane bit 4 in layout B)
+                thB = (p.L > F_WLOW) ? (int)(wt & 1ull) : 0;                      // column 12
             } else {
                 const int amid = p.a - F_RIDE;
                 const unsigned long long tmid = wt & ((1ull << amid) - 1), ttop = wt >> amid;
                 base = (tmid << F_RIDE) + (ttop << (p.a + F_WHIGH));
-                vA = (int)((base >> (p.a - 1)) & 1ull);                           // column a-1 (>= 3)
-                vB = (p.a + F_WHIGH < p.L) ? (int)(ttop & 1ull) : 0;              // column a+9
+                tlA = (int)((base >> (p.a - 1)) & 1ull);                          // column a-1 (>= 3)
+                thA = (lane >> 3) & 1;                     // d7
+                tlB = (lane >> 4) & 1;                     // d1
+                thB = (p.a + F_WHIGH < p.L) ? (int)(ttop & 1ull) : 0;             // column a+9
             }
             float v[128];
             if (p.flags & PASS_INIT) {
@@ -207,88 +275,122 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
                 gmove<LOW, false>(v, S + base, lane, p.first_layout, estride);
             }
             // ---- run the program ------------------------------------------------------------------
-            int pc = 0;
-            FMop op = s_mops[0];
+            int pc = 0, layout = p.first_layout;
+            unsigned op = s_mops[0];
             for (;;) {
-                const unsigned code = op.ctrl & 0xffu;
-                if (code == MC_END) break;
-                const FMop nxt = s_mops[pc + 1];
-                switch (code) {
-                    case MC_GATE:
-                        switch ((op.ctrl >> 8) & 0xffu) {
-                            case 0: fgate<0>(v, op.m); break;
-                            case 1: fgate<1>(v, op.m); break;
-                            case 2: fgate<2>(v, op.m); break;
-                            case 3: fgate<3>(v, op.m); break;
-                            case 4: fgate<4>(v, op.m); break;
-                            case 5: fgate<5>(v, op.m); break;
-                            default: fgate<6>(v, op.m); break;
-                        }
-                        break;
-                    case MC_TABLE: {
-                        const int var = ((op.ctrl >> 8) & 0xffu) ? vB : vA;
-                        ftable(v, reinterpret_cast<const float4*>(s_tab + ((op.ctrl >> 16) * 2 + var) * 128));
-                        break;
-                    }
-                    case MC_XAB:
-                        __syncwarp(); xstore<LOW, 0>(v, myreg, lane); __syncwarp(); xload<LOW, 1>(v, myreg, lane);
-                        break;
-                    case MC_XBA:
-                        __syncwarp(); xstore<LOW, 1>(v, myreg, lane); __syncwarp(); xload<LOW, 0>(v, myreg, lane);
-                        break;
-                    default: break;
+                const unsigned code = op & 0xffu;
+                if (code == MC_END || code == MC_FINAL) break;
+                const unsigned nxt = s_mops[pc + 1];
+                if (code == MC_ROUND) {
+                    const float4* gk = s_gk + 2 * (op >> 16);
+                    if (layout == 0) fround<LOW, 0>(v, (op >> 8) & 0x7fu, gk, tlA, thA);
+                    else fround<LOW, 1>(v, (op >> 8) & 0x7fu, gk, tlB, thB);
+                } else if (code == MC_XAB) {
+                    __syncwarp(); xstore<LOW, 0>(v, myreg, lane); __syncwarp(); xload<LOW, 1>(v, myreg, lane);
+                    layout = 1;
+                } else {
+                    __syncwarp(); xstore<LOW, 1>(v, myreg, lane); __syncwarp(); xload<LOW, 0>(v, myreg, lane);
+                    layout = 0;
                 }
                 op = nxt; ++pc;
             }
-            // ---- store, or reduce ------------------------------------------------------------------
+            // ---- store, or add A_{L-1}(s) and reduce ---------------------------------------------
             if (p.flags & PASS_REDUCE) {
-                float mx = v[0];
+                // element index with the register digits cleared, first register column, variant
+                unsigned long long sthr; int x0, var;
+                if (LOW) {
+                    if (layout == 0) { sthr = base + ((unsigned long long)lane << 7); x0 = 0; var = tlA + 2 * thA; }
+                    else { sthr = base + lane; x0 = 5; var = tlB + 2 * thB; }
+                } else {
+                    if (layout == 0) { sthr = base + (lane & 7) + ((unsigned long long)(lane >> 3) << (p.a + 7)); x0 = p.a; var = tlA + 2 * thA; }
+                    else { sthr = base + (lane & 7) + ((unsigned long long)(lane >> 3) << p.a); x0 = p.a + 2; var = tlB + 2 * thB; }
+                }
+                const float cthr = final_thread_const(s_fin, p.L, x0, sthr);
+                const float4* T = reinterpret_cast<const float4*>(s_fin + var * 128);
+                float mx = -INFINITY;
 #pragma unroll
-                for (int j = 1; j < 128; ++j) mx = fmaxf(mx, v[j]);
-                for (int o = 16; o; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-                if (lane == 0) p.part_x[(unsigned long long)inst * p.tiles_per_inst + wt] = mx;
+                for (int q = 0; q < 32; ++q) {
+                    const float4 t = T[q];
+                    mx = fmaxf(mx, fmaxf(fmaxf(v[4 * q] + t.x, v[4 * q + 1] + t.y), fmaxf(v[4 * q + 2] + t.z, v[4 * q + 3] + t.w)));
+                }
+                wmax = fmaxf(wmax, mx + cthr);
             } else {
                 gmove<LOW, true>(v, S + base, lane, p.last_layout, estride);
+            }
+        }
+        if (p.flags & PASS_REDUCE) {
+            for (int o = 16; o; o >>= 1) wmax = fmaxf(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
+            if (lane == 0) s_red[warp] = wmax;
+            __syncthreads();
+            if (tid == 0) {
+                float m = s_red[0];
+                for (int w = 1; w < FWARPS; ++w) m = fmaxf(m, s_red[w]);
+                p.part_x[(size_t)inst * gridDim.x + blockIdx.x] = m;
             }
         }
     }
 }
 
-// ---- S0: per-instance gate constants and diagonal tables from the couplings ----------------------
+// ---- S0: per-instance gate constants and the final table from the couplings ------------------------
 struct FusedPrepParams {
-    int L, n_gates, n_tables;
-    const int* gate_jv;            // [n_gates]
-    const FusedTable* tables;      // [n_tables]
-    const TableTerm* terms;
+    int L, n_gates;
+    const int* gate_rc;            // [n_gates]  r * 64 + c
     const float* Jh; const float* Jv; const float* h;   // device couplings, per instance
-    float* gate_m;                 // [inst][n_gates]
-    float* table_out;              // [inst][n_tables][2][128]
+    float* gate_k;                 // [inst][n_gates][8]
+    float* final_tab;              // [inst][FFINAL_FLOATS]
+    int fin_low, fin_layout, fin_a;   // tile kind, layout and start column of the last pass's end
 };
 
 __global__ void __launch_bounds__(256) fused_prep_kernel(const FusedPrepParams p) {
     const unsigned long long inst = blockIdx.y;
-    const float* Jh = p.Jh + inst * (unsigned long long)(p.L * (p.L - 1));
-    const float* Jv = p.Jv + inst * (unsigned long long)((p.L - 1) * p.L);
-    const float* hh = p.h ? p.h + inst * (unsigned long long)(p.L * p.L) : nullptr;
+    const int L = p.L;
+    const float* Jh = p.Jh + inst * (unsigned long long)(L * (L - 1));
+    const float* Jv = p.Jv + inst * (unsigned long long)((L - 1) * L);
+    const float* hh = p.h ? p.h + inst * (unsigned long long)(L * L) : nullptr;
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx < p.n_gates) p.gate_m[inst * p.n_gates + idx] = -2.f * Jv[p.gate_jv[idx]];
-    if (idx < (long)p.n_tables * 256) {
-        const int t = (int)(idx >> 8), var = (int)(idx >> 7) & 1, j = (int)idx & 127;
-        const FusedTable tb = p.tables[t];
-        float acc = 0.f;
-        for (int q = tb.term_begin; q < tb.term_end; ++q) {
-            const TableTerm tt = p.terms[q];
-            const int ba = tt.posA == 7 ? var : (j >> tt.posA) & 1;
-            if (tt.type == OP_DH) {
-                const float hv = hh ? hh[tt.row * p.L + tt.col] : 0.f;
-                acc += ba ? -hv : hv;
-            } else {
-                const int bb = tt.posB == 7 ? var : (j >> tt.posB) & 1;
-                const float Jc = Jh[tt.row * (p.L - 1) + tt.col];
-                acc += (ba == bb) ? Jc : -Jc;
+    // accumulated diagonal coefficients through row R-1 (A_{R-1}), in double
+    auto Hacc = [&](int R, int c) { double s = 0; if (hh) for (int r = 0; r < R; ++r) s += (double)hh[r * L + c]; return s; };
+    auto Kacc = [&](int R, int c) { double s = 0; if (c < 0 || c >= L - 1) return s; for (int r = 0; r < R; ++r) s += (double)Jh[r * (L - 1) + c]; return s; };
+    if (idx < p.n_gates) {
+        const int r = p.gate_rc[idx] >> 6, c = p.gate_rc[idx] & 63;
+        const double m = -2.0 * (double)Jv[(r - 1) * L + c];
+        const double H = Hacc(r, c), Kl = Kacc(r, c - 1), Kr = Kacc(r, c);
+        float* out = p.gate_k + (inst * p.n_gates + idx) * 8;
+        for (int nl = 0; nl < 2; ++nl)
+            for (int nh = 0; nh < 2; ++nh) {
+                const double rho = H + (nl ? -Kl : Kl) + (nh ? -Kr : Kr);
+                out[nl * 2 + nh] = (float)(m - 2.0 * rho);         // ka: a' = max(a, b + ka)
+                out[4 + nl * 2 + nh] = (float)(m + 2.0 * rho);     // kb: b' = max(b, a + kb)
             }
+    }
+    if (idx < FFINAL_FLOATS) {
+        float* out = p.final_tab + inst * FFINAL_FLOATS;
+        if (idx < 512) {
+            const int var = (int)idx >> 7, j = (int)idx & 127, tl = var & 1, th = var >> 1;
+            const bool low = p.fin_low != 0;
+            const int W = low ? F_WLOW : F_WHIGH;
+            // register columns are consecutive: x0 .. x0+6
+            const int d0 = low ? (p.fin_layout == 0 ? 0 : 5) : (p.fin_layout == 0 ? 0 : 2);
+            const int x0 = p.fin_a + d0;
+            (void)W;
+            double acc = 0;
+            int bits[F_RB];
+            for (int i = 0; i < F_RB; ++i) bits[i] = (j >> fused_bit_of_digit(low, p.fin_layout, d0 + i)) & 1;
+            for (int i = 0; i < F_RB; ++i) {
+                const int c = x0 + i;
+                acc += bits[i] ? -Hacc(L, c) : Hacc(L, c);
+                if (i + 1 < F_RB) acc += (bits[i] == bits[i + 1]) ? Kacc(L, c) : -Kacc(L, c);
+            }
+            acc += (tl == bits[0]) ? Kacc(L, x0 - 1) : -Kacc(L, x0 - 1);              // 0 when x0 = 0
+            acc += (th == bits[F_RB - 1]) ? Kacc(L, x0 + F_RB - 1) : -Kacc(L, x0 + F_RB - 1);   // 0 at the right edge
+            out[idx] = (float)acc;
+        } else if (idx < 576) {
+            const int c = (int)idx - 512;
+            out[idx] = c < L ? (float)Hacc(L, c) : 0.f;
+        } else {
+            const int c = (int)idx - 576;
+            out[idx] = c < L - 1 ? (float)Kacc(L, c) : 0.f;
         }
-        p.table_out[(inst * p.n_tables + t) * 256 + var * 128 + j] = acc;
     }
 }
 

@@ -115,6 +115,12 @@ def test_fusion_cuts_hbm_passes():
 
 
 # ------------------------------------------------------------------ fused register-phase schedule
+# Diagonal frame (csrc/planner.h): the row diagonals are folded into the gates by conjugating
+# every gate with the accumulated diagonal operator, G''_r(c) = A_{r-1}^{-1} G_r(c) A_{r-1}.
+# Restated here independently: with H_c, K_c the sums of h[r'][c], Jh[r'][c] over r' < r,
+#     a' = max(a, b + m - 2 rho), b' = max(b, a + m + 2 rho),  m = -2 Jv[r-1][c],
+#     rho = H_c + K_{c-1} sigma_{c-1} + K_c sigma_{c+1};   result = max_s(V(s) + A_{L-1}(s)).
+# Dependency rule in this frame: g(r,c) after g(r-1,c-1), g(r-1,c), g(r-1,c+1).
 # register-index bit -> tile digit, as documented in csrc/planner.h (fused_digit_of_bit)
 DIGIT_OF_BIT = {(1, 0): [5, 6, 0, 1, 2, 3, 4], (1, 1): [5, 6, 7, 8, 9, 10, 11],
                 (0, 0): [2, 3, 0, 1, 4, 5, 6], (0, 1): [2, 3, 4, 5, 6, 7, 8]}
@@ -133,30 +139,31 @@ def parse_fused(txt):
         elif w[0] == "m":
             d = {"code": w[1]}
             d.update({k: int(v) for k, v in (kv.split("=") for kv in w[2:])})
-            d["terms"] = []
+            d["gates"] = []
             passes[-1]["mops"].append(d)
-        elif w[0] == "t":
-            d = {"type": w[1]}
-            d.update({k: int(v) for k, v in (kv.split("=") for kv in w[2:])})
-            passes[-1]["mops"][-1]["terms"].append(d)
+        elif w[0] == "g":
+            passes[-1]["mops"][-1]["gates"].append({k: int(v) for k, v in (kv.split("=") for kv in w[1:])})
     return head, passes
 
 
-def fused_to_ops(L, fpasses, fields):
-    """Check the structure of the micro-op program (layouts, register bits, table positions) and
-    flatten it to the (type, r, c) op sequence, validated against the same dependency rule."""
+def fused_to_gates(L, fpasses):
+    """Check the structure of the micro-op program (layouts, register bits, rounds) and the
+    three-point-stencil dependency rule; return the flat (r, c) gate sequence."""
     flat = []
+    grow = [1] * L                                   # rows complete per digit (row 0 needs no gate)
     for i, ps in enumerate(fpasses):
         a, Wt, low = ps["a"], ps["W"], ps["low"]
         assert (low == 1 and a == 0 and Wt == 12) or (low == 0 and a >= 4 and Wt == 9)
         assert a + Wt <= L
         assert (ps["flags"] & 1) == (1 if i == 0 else 0)
+        last = i == len(fpasses) - 1
+        assert bool(ps["flags"] & 2) == last
         if low:
             assert ps["first"] == 1 and ps["last"] == 1     # coalesced global layout
-        layout, ops = ps["first"], []
-        assert ps["mops"][-1]["code"] == "end"
-        assert len(ps["mops"]) <= 256
-        ntab = 0
+        layout = ps["first"]
+        assert ps["mops"][-1]["code"] == ("final" if last else "end")
+        assert len(ps["mops"]) <= 128
+        ngates = 0
         for m in ps["mops"][:-1]:
             code = m["code"]
             if code == "xAB":
@@ -165,29 +172,23 @@ def fused_to_ops(L, fpasses, fields):
             elif code == "xBA":
                 assert layout == 1
                 layout = 0
-            elif code == "gate":
-                assert 0 <= m["k"] < 7
-                assert m["c"] == a + DIGIT_OF_BIT[(low, layout)][m["k"]]      # register bit <-> column
-                ops.append({"type": "g", "r": m["r"], "c": m["c"], "pos": m["c"] - a})
-            elif code == "table":
-                ntab += 1
-                assert layout == m["layout"] and m["nterms"] == len(m["terms"]) > 0
-                outer = a - 1 if layout == 0 else a + Wt
-
-                def col_of(pos):
-                    return outer if pos == 7 else a + DIGIT_OF_BIT[(low, layout)][pos]
-                for t in m["terms"]:
-                    if t["type"] == "dh":
-                        assert t["pa"] < 7 and col_of(t["pa"]) == t["c"]
-                    else:
-                        assert col_of(t["pa"]) == t["c"] and col_of(t["pb"]) == t["c"] + 1
-                        assert not (t["pa"] == 7 and t["pb"] == 7) and 0 <= t["c"] < L - 1
-                        if low == 0:
-                            assert outer >= 3       # the outer neighbour must not be a riding digit
-                    ops.append({"type": t["type"], "r": t["r"], "c": t["c"]})
-        assert layout == ps["last"] and ntab <= 32
-        flat.append({"lo": 0, "a": a, "b": a + Wt, "flags": ps["flags"], "src": -1, "dst": -1, "ops": ops})
-    validate(2, L, flat, fields=fields, row_aligned=False)
+            else:
+                assert code == "round" and 0 < m["mask"] < 128 and m["first"] == ngates
+                bits = [k for k in range(7) if m["mask"] >> k & 1]
+                assert [g["k"] for g in m["gates"]] == bits          # ascending register bits
+                before = list(grow)
+                for g in m["gates"]:
+                    c, r = g["c"], g["r"]
+                    assert c == a + DIGIT_OF_BIT[(low, layout)][g["k"]]      # register bit <-> column
+                    # legal at the START of the round: every gate of a round commutes with the others
+                    assert 1 <= r < L and before[c] == r
+                    assert c == 0 or before[c - 1] >= r
+                    assert c == L - 1 or before[c + 1] >= r
+                    grow[c] += 1
+                    flat.append((r, c))
+                ngates += len(bits)
+        assert layout == ps["last"] and ngates == ps["gates"] <= 160
+    assert grow == [L] * L
     return flat
 
 
@@ -195,20 +196,54 @@ def fused_to_ops(L, fpasses, fields):
 def test_fused_schedule_obeys_dependency_rule(L):
     head, fpasses = parse_fused(describe(2, L, 0, fused=True))
     assert int(head["L"]) == L
-    fused_to_ops(L, fpasses, fields=True)
+    flat = fused_to_gates(L, fpasses)
+    assert len(flat) == L * (L - 1) == len(set(flat))
+
+
+def replay_diagonal_frame(L, gates, Jh, Jv, h):
+    """numpy float64 replay of the conjugated gates in schedule order (Ising, energy only)."""
+    N = 2 ** L
+    s = np.arange(N)
+    sig = [1 - 2 * ((s >> c) & 1) for c in range(L)]
+    Hacc = np.cumsum(h, axis=0) if h is not None else np.zeros((L, L))
+    Kacc = np.cumsum(Jh, axis=0)
+    V = np.zeros(N)
+    defer = 0.0
+    for (r, c) in gates:
+        J = Jv[r - 1, c]
+        defer += J
+        rho = Hacc[r - 1, c] * np.ones(N)
+        if c > 0:
+            rho = rho + Kacc[r - 1, c - 1] * sig[c - 1]
+        if c < L - 1:
+            rho = rho + Kacc[r - 1, c] * sig[c + 1]
+        ia = s[(s >> c) & 1 == 0]
+        ib = ia | (1 << c)
+        xa, xb = V[ia].copy(), V[ib].copy()
+        V[ia] = np.maximum(xa, xb - 2 * J - 2 * rho[ia])
+        V[ib] = np.maximum(xb, xa - 2 * J + 2 * rho[ia])
+    A = np.zeros(N)
+    for c in range(L):
+        A += Hacc[L - 1, c] * sig[c]
+        if c < L - 1:
+            A += Kacc[L - 1, c] * sig[c] * sig[c + 1]
+    m = (V + A).max() + defer
+    return 0.0 if m == 0 else -m
 
 
 @pytest.mark.parametrize("L", [12, 13, 16])
 def test_fused_schedule_replay_matches_oracle(L):
     _, fpasses = parse_fused(describe(2, L, 0, fused=True))
-    flat = fused_to_ops(L, fpasses, fields=True)
+    flat = fused_to_gates(L, fpasses)
     rng = np.random.default_rng(L)
     Jh = rng.integers(-2, 3, size=(L, L - 1)).astype(float)
     Jv = rng.integers(-2, 3, size=(L - 1, L)).astype(float)
     h = rng.integers(-1, 2, size=(L, L)).astype(float)
-    E0, g = replay(2, L, flat, Jh, Jv, h)
-    Eo, go, _ = oracle.dp_ising(L, Jh, Jv, h)
-    assert (E0, g) == (Eo, go)
+    Eo, _, _ = oracle.dp_ising(L, Jh, Jv, h, count=False)
+    assert replay_diagonal_frame(L, flat, Jh, Jv, h) == Eo
+    Jh, Jv, h = rng.normal(size=Jh.shape), rng.normal(size=Jv.shape), rng.normal(size=h.shape)
+    Eo, _, _ = oracle.dp_ising(L, Jh, Jv, h, count=False)
+    assert abs(replay_diagonal_frame(L, flat, Jh, Jv, h) - Eo) <= 1e-9 * abs(Eo)
 
 
 # ------------------------------------------------------------------------------- numeric replay
