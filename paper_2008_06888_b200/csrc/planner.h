@@ -222,10 +222,17 @@ inline std::string describe(const Plan& p) {
 //        layout A: register digits d0..d6, lanes (riding, d7, d8)
 //        layout B: register digits d2..d8, lanes (riding, d0, d1)
 // A gate on a register digit is pure register arithmetic; its neighbour bits are register-index
-// bits (compile-time per unrolled element) or constant per thread (lane / tile bits).  A phase is
-// a list of ROUNDS; a round applies, for a 7-bit mask of register digits, the next gate of each
-// of them (all legal at the start of the round), in ascending bit order.  Layout exchanges go
-// through the warp's private shared-memory region.
+// bits (compile-time per unrolled element) or constant per thread (lane / tile bits).
+// MIRRORED LAYOUTS.  The 7 register digits form a chain p0..p6; in layout A p_i is the i-th
+// register digit from the LEFT, in layout B the i-th from the RIGHT.  Chain positions sit on the
+// same register-index bits in both layouts, so one set of 7 unrolled gate bodies serves both
+// (the instruction footprint is what the SM's instruction cache has to hold): the body of bit K
+// only knows its "P" neighbour (chain position - 1; the tile's outer neighbour column for p0)
+// and its "Q" neighbour (position + 1; a lane digit for p6).  P/Q are left/right in A and
+// right/left in B; the gate constants are stored as k[side][P bit][Q bit].
+// A phase is a list of ROUNDS; a round applies, for a 7-bit mask of register bits, the next gate
+// of each of those digits (all legal at the start of the round), in ascending bit order.  Layout
+// exchanges go through the warp's private shared-memory region.
 // =============================================================================================
 enum MicroCode : uint8_t { MC_END = 0, MC_XAB = 1, MC_XBA = 2, MC_ROUND = 3, MC_FINAL = 4 };
 
@@ -239,13 +246,19 @@ constexpr int F_RIDE = 3;        // riding digits of a high tile
 constexpr int F_AMIN = 4;        // smallest start of a high tile (its outer neighbour must not ride)
 
 // tile digit (0..W-1) held by register-index bit `bit` in `layout` of a low/high tile
+//   lowA {5,6,0,1,2,3,4}   lowB {6,5,11,10,9,8,7}   highA {4,5,6,0,1,2,3}   highB {4,3,2,8,7,6,5}
+// chain position of a bit = its layout-A digit; layout B holds digit (W-1) - position.
+#if defined(__CUDACC__)
+__host__ __device__
+#endif
+constexpr int fused_chain_pos(bool low, int bit) {
+    return low ? (bit < 2 ? 5 + bit : bit - 2) : (bit < 3 ? 4 + bit : bit - 3);
+}
 #if defined(__CUDACC__)
 __host__ __device__
 #endif
 constexpr int fused_digit_of_bit(bool low, int layout, int bit) {
-    // lowA {5,6,0,1,2,3,4}  lowB {5,..,11}  highA {2,3,0,1,4,5,6}  highB {2,..,8}
-    return low ? (layout == 0 ? (bit < 2 ? 5 + bit : bit - 2) : 5 + bit)
-               : (layout == 0 ? (bit < 2 ? 2 + bit : (bit < 4 ? bit - 2 : bit)) : 2 + bit);
+    return layout == 0 ? fused_chain_pos(low, bit) : (low ? 11 : 8) - fused_chain_pos(low, bit);
 }
 // register-index bit holding tile digit d in this layout, or -1 (lane / tile digit)
 #if defined(__CUDACC__)
@@ -270,7 +283,7 @@ struct FusedPlan {
     int L = 0;
     std::vector<FusedPass> passes;
     std::vector<MicroOp> mops;
-    std::vector<int> gate_rc;    // r * 64 + c of every gate, in execution order
+    std::vector<int> gate_rc;    // layout * 4096 + r * 64 + c of every gate, in execution order
     bool ok = false;
 };
 
@@ -327,7 +340,7 @@ class FusedScheduler {
             P_.mops.push_back({MC_ROUND, (uint8_t)mask, (uint16_t)((int)P_.gate_rc.size() - pass_gate_begin_)});
             for (int b = 0; b < F_RB; ++b) if (mask >> b & 1) {
                 const int c = a + fused_digit_of_bit(low, layout, b);
-                P_.gate_rc.push_back(grow_[c] * 64 + c);
+                P_.gate_rc.push_back(layout * 4096 + grow_[c] * 64 + c);
                 ++n;
             }
             for (int b = 0; b < F_RB; ++b) if (mask >> b & 1) grow_[a + fused_digit_of_bit(low, layout, b)] += 1;
@@ -411,7 +424,7 @@ inline std::string describe_fused(const FusedPlan& p) {
                     int g = ps.gate_begin + m.arg;
                     for (int b = 0; b < F_RB; ++b) if (m.mask >> b & 1) {
                         const int rc = p.gate_rc[g++];
-                        snprintf(line, sizeof line, "g k=%d r=%d c=%d\n", b, rc / 64, rc % 64);
+                        snprintf(line, sizeof line, "g k=%d r=%d c=%d layout=%d\n", b, (rc / 64) % 64, rc % 64, rc / 4096);
                         out += line;
                     }
                     break; }

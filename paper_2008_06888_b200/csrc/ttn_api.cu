@@ -208,11 +208,7 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
     pp.gate_inst_stride = (unsigned long long)fp.gate_rc.size() * 8;
     pp.final_tab = reinterpret_cast<const float*>(P->ws + y.f_final);
     pp.part_x = reinterpret_cast<float*>(P->ws + y.part_x);
-    {   // one tile's gate phase when a warp has the alu pipe to itself: 128 FMNMX x 2 cycles per gate
-        unsigned st = (unsigned)(ps.gate_end - ps.gate_begin) * 256u;
-        if (const char* e = getenv("TTN_DEBUG_STAGGER")) st = (unsigned)(atof(e) * st);
-        pp.stagger_cycles = st;
-    }
+    pp.stride_bytes = ps.a <= 20 ? (4u << ps.a) : 0u;
     unsigned long long grid = (unsigned long long)P->fused_grid;
     const int nw = ttn::fwarps(ps.low != 0);
     const unsigned long long need = (pp.tiles_per_inst + nw - 1) / nw;
@@ -373,9 +369,24 @@ ttn_status ttn_plan_launch(ttn_plan* P, void* stream) {
     if (!P) return fail(TTN_EINVAL, "plan is NULL");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if (P->fused) {
+        const bool timing = getenv("TTN_DEBUG_TIMING") != nullptr;     // per-pass device times on stderr
+        std::vector<cudaEvent_t> ev;
+        if (timing) { ev.resize(P->fplan.passes.size() + 1); for (auto& e : ev) cudaEventCreate(&e); cudaEventRecord(ev[0], st); }
+        size_t k = 0;
         for (const ttn::FusedPass& ps : P->fplan.passes) {
             ttn_status s = launch_fused_pass(P, ps, st);
             if (s != TTN_OK) return s;
+            if (timing) cudaEventRecord(ev[++k], st);
+        }
+        if (timing) {
+            cudaStreamSynchronize(st);
+            for (size_t i = 0; i < P->fplan.passes.size(); ++i) {
+                float ms = 0; cudaEventElapsedTime(&ms, ev[i], ev[i + 1]);
+                const ttn::FusedPass& ps = P->fplan.passes[i];
+                fprintf(stderr, "pass %2zu a=%2d low=%d gates=%3d rounds=%2d phases=%d : %.2f ms\n", i, ps.a, ps.low,
+                        ps.gate_end - ps.gate_begin, ps.n_rounds, ps.n_phases, ms);
+            }
+            for (auto& e : ev) cudaEventDestroy(e);
         }
         return TTN_OK;
     }

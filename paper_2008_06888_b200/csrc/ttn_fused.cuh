@@ -1,20 +1,22 @@
-// ttn_fused.cuh -- fused register-phase pass kernel for the Ising Tropical<f32> sweep ("v3",
-// diagonal frame; see planner.h for the frame and the schedule).
+// ttn_fused.cuh -- fused register-phase pass kernel for the Ising Tropical<f32> sweep ("v4":
+// diagonal frame + mirrored layouts; see planner.h for the frame, the layouts and the schedule).
 //
 // One launch = one HBM pass.  Each WARP owns a tile of 2^12 state elements,
 // 128 per thread, and runs the pass's micro-op program on it with no CTA-level cooperation:
 //   * conjugated max-plus gates (A2) PAPER.md:242 on a register digit:
-//         a' = max(a, b + ka[n]),  b' = max(b, a + kb[n]),   n = (bit c-1, bit c+1) of the index,
+//         a' = max(a, b + ka[n]),  b' = max(b, a + kb[n]),   n = the two neighbour bits of the index,
 //     the row diagonals (A3), (A4) PAPER.md:247-252 folded into the 8 constants of the gate and
-//     the common +Jv deferred to a scalar (ttn_api.cu): 1 FMNMX + 1/2 FADD2 per element;
-//   * layout exchanges A <-> B through the warp's private shared-memory region with 128-bit,
-//     bank-conflict-free accesses, synchronised with __syncwarp only;
+//     the common +Jv deferred to a scalar (ttn_api.cu): 1 FMNMX + 1/2 FADD2 per element.  One
+//     set of 7 unrolled bodies (one per register bit) serves both layouts of a tile;
+//   * layout exchanges A <-> B through the warp's private shared-memory region with 128-bit
+//     (LOW) / 64-bit (HIGH) bank-conflict-free accesses, synchronised with __syncwarp only;
 //   * the last pass adds the accumulated diagonal A_{L-1}(s) (a 128-entry table over the
 //     register digits in 4 boundary variants + a per-thread scalar) and max-reduces.
 // Global traffic goes straight between HBM and registers: the LOW tile (columns 0..11) moves
-// 128-byte lines; HIGH tiles (columns a..a+8 plus the riding columns 0..2 on the low lane bits)
-// move whole 32-byte sectors, four per request.  The kernel is persistent (one CTA per SM);
-// programs and gate constants are staged in shared memory once per launch and instance.
+// 128-byte lines with immediate offsets; HIGH tiles (columns a..a+8 plus the riding columns 0..2
+// on the low lane bits) move whole 32-byte sectors, four per request, one IMAD.WIDE per address.
+// The kernel is persistent (one CTA per SM); programs and gate constants are staged in shared
+// memory once per launch and instance.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -22,17 +24,23 @@
 
 namespace ttn {
 
-// Warps per CTA (one CTA per SM).  The LOW kernel's global accesses need no address registers,
-// so it fits 12 warps of 168 registers (3 per scheduler); the HIGH kernel keeps 8 warps of 255
-// registers so that all 128 strided loads of a tile stay in flight.
-constexpr int FWARPS_LOW = 12, FWARPS_HIGH = 8;
+// Warps per CTA (one CTA per SM).  LOW: 12 warps of <= 168 registers, 3 per scheduler.  HIGH: 8 warps;
+// with 12 the scattered 32-byte-sector traffic of the strided tiles collapses (measured: a
+// store-only pass takes 11 ms with 12 warps, 3.6 ms with 8).
+#ifndef TTN_FWARPS_LOW
+#define TTN_FWARPS_LOW 12
+#endif
+#ifndef TTN_FWARPS_HIGH
+#define TTN_FWARPS_HIGH 8
+#endif
+constexpr int FWARPS_LOW = TTN_FWARPS_LOW, FWARPS_HIGH = TTN_FWARPS_HIGH;
 constexpr int FREGION_F4 = 33 * 32;       // float4 per warp exchange region (low tile: padded rows)
 constexpr int FMAX_MOPS = 128;            // micro-ops per pass
 constexpr int FMAX_GATES = 160;           // gates per pass (8 constants each)
 constexpr int FFINAL_FLOATS = 4 * 128 + 2 * 64;   // final table (4 variants) + H[64] + K[64]
 __host__ __device__ constexpr int fwarps(bool low) { return low ? FWARPS_LOW : FWARPS_HIGH; }
 __host__ __device__ constexpr size_t fsmem_bytes(bool low) {
-    return (size_t)fwarps(low) * FREGION_F4 * 16 + (size_t)FMAX_GATES * 32 + (size_t)FFINAL_FLOATS * 4 +
+    return (size_t)fwarps(low) * FREGION_F4 * 16 + (size_t)(FMAX_GATES + 1) * 32 + (size_t)FFINAL_FLOATS * 4 +
            (size_t)FMAX_MOPS * 4 + 64;
 }
 
@@ -46,7 +54,8 @@ struct FusedParams {
     unsigned long long gate_inst_stride;          // floats between instances
     const float* final_tab;             // [inst][FFINAL_FLOATS] (REDUCE pass only)
     float* part_x;                      // [batch][gridDim.x] (REDUCE)
-    unsigned stagger_cycles;            // start delay per warp group (warp / 4), see the kernel
+    unsigned stride_bytes;              // HIGH: 4 << a (a <= 20), passed opaque so that the address
+                                        // math stays one IMAD.WIDE per access; else 0
 };
 
 // (o0, o1) = (a0 + b0, a1 + b1) in one FADD2
@@ -60,28 +69,28 @@ __device__ __forceinline__ void add2(float& o0, float& o1, float a0, float a1, f
 }
 
 // ---- conjugated gate on register-index bit K ------------------------------------------------------
-// NL / NH: register-index bit holding the left / right neighbour column, or -1 when that
-// neighbour is constant per thread (its value is then tl / th).  k[0..3] = ka[nl][nh],
-// k[4..7] = kb[nl][nh].
-template <int K, int NL, int NH>
-__device__ __forceinline__ void cgate(float (&v)[128], const float4 c0, const float4 c1, const int tl, const int th) {
+// PN / QN: register-index bit holding the P / Q neighbour (chain position -1 / +1), or -1 when
+// that neighbour is constant per thread (its bit is then tp / tq).  c0 = ka[pn][qn], c1 = kb[pn][qn]
+// (x: 00, y: 01, z: 10, w: 11);  a = the element whose bit K is 0.
+template <int K, int PN, int QN>
+__device__ __forceinline__ void cgate(float (&v)[128], const float4 c0, const float4 c1, const int tp, const int tq) {
     float ka[2][2] = {{c0.x, c0.y}, {c0.z, c0.w}}, kb[2][2] = {{c1.x, c1.y}, {c1.z, c1.w}};
-    if (NL < 0) {
+    if (PN < 0) {
 #pragma unroll
-        for (int h = 0; h < 2; ++h) { ka[0][h] = tl ? ka[1][h] : ka[0][h]; kb[0][h] = tl ? kb[1][h] : kb[0][h]; }
+        for (int h = 0; h < 2; ++h) { ka[0][h] = tp ? ka[1][h] : ka[0][h]; kb[0][h] = tp ? kb[1][h] : kb[0][h]; }
     }
-    if (NH < 0) {
+    if (QN < 0) {
 #pragma unroll
-        for (int l = 0; l < 2; ++l) { ka[l][0] = th ? ka[l][1] : ka[l][0]; kb[l][0] = th ? kb[l][1] : kb[l][0]; }
+        for (int l = 0; l < 2; ++l) { ka[l][0] = tq ? ka[l][1] : ka[l][0]; kb[l][0] = tq ? kb[l][1] : kb[l][0]; }
     }
     constexpr int B = 1 << K;
-#define TTN_NL(j) (NL < 0 ? 0 : (((j) >> (NL < 0 ? 0 : NL)) & 1))
-#define TTN_NH(j) (NH < 0 ? 0 : (((j) >> (NH < 0 ? 0 : NH)) & 1))
+#define TTN_NP(j) (PN < 0 ? 0 : (((j) >> (PN < 0 ? 0 : PN)) & 1))
+#define TTN_NQ(j) (QN < 0 ? 0 : (((j) >> (QN < 0 ? 0 : QN)) & 1))
     if (K == 0) {
 #pragma unroll
         for (int j = 0; j < 128; j += 2) {
             float t0, t1;     // t0 = a + kb (candidate for b), t1 = b + ka (candidate for a)
-            add2(t0, t1, v[j], v[j + 1], kb[TTN_NL(j)][TTN_NH(j)], ka[TTN_NL(j)][TTN_NH(j)]);
+            add2(t0, t1, v[j], v[j + 1], kb[TTN_NP(j)][TTN_NQ(j)], ka[TTN_NP(j)][TTN_NQ(j)]);
             v[j] = fmaxf(v[j], t1);
             v[j + 1] = fmaxf(v[j + 1], t0);
         }
@@ -90,104 +99,162 @@ __device__ __forceinline__ void cgate(float (&v)[128], const float4 c0, const fl
         for (int j = 0; j < 128; j += 2) {
             if ((j & B) == 0) {
                 float a0, a1, b0, b1;
-                add2(a0, a1, v[j], v[j + 1], kb[TTN_NL(j)][TTN_NH(j)], kb[TTN_NL(j + 1)][TTN_NH(j + 1)]);
-                add2(b0, b1, v[j + B], v[j + B + 1], ka[TTN_NL(j)][TTN_NH(j)], ka[TTN_NL(j + 1)][TTN_NH(j + 1)]);
+                add2(a0, a1, v[j], v[j + 1], kb[TTN_NP(j)][TTN_NQ(j)], kb[TTN_NP(j + 1)][TTN_NQ(j + 1)]);
+                add2(b0, b1, v[j + B], v[j + B + 1], ka[TTN_NP(j)][TTN_NQ(j)], ka[TTN_NP(j + 1)][TTN_NQ(j + 1)]);
                 v[j] = fmaxf(v[j], b0); v[j + 1] = fmaxf(v[j + 1], b1);
                 v[j + B] = fmaxf(v[j + B], a0); v[j + B + 1] = fmaxf(v[j + B + 1], a1);
             }
         }
     }
-#undef TTN_NL
-#undef TTN_NH
+#undef TTN_NP
+#undef TTN_NQ
 }
 
-// register bit of the left / right neighbour of the digit held by register bit K (-1: per thread)
-template <bool LOW, int LAYOUT, int K> struct Nbr {
-    static constexpr int d = fused_digit_of_bit(LOW, LAYOUT, K);
-    static constexpr int W = LOW ? F_WLOW : F_WHIGH;
-    static constexpr int NL = d == 0 ? -1 : fused_bit_of_digit(LOW, LAYOUT, d - 1);
-    static constexpr int NH = d == W - 1 ? -1 : fused_bit_of_digit(LOW, LAYOUT, d + 1);
+// register bit of the P / Q neighbour of the chain position held by register bit K (-1: per thread)
+template <bool LOW, int K> struct Nbr {
+    static constexpr int pos = fused_chain_pos(LOW, K);
+    static constexpr int PN = pos == 0 ? -1 : fused_bit_of_digit(LOW, 0, pos - 1);
+    static constexpr int QN = pos == F_RB - 1 ? -1 : fused_bit_of_digit(LOW, 0, pos + 1);
 };
 
-// One round: for every set bit of `mask` (ascending) the next gate of that register digit.
-template <bool LOW, int LAYOUT>
-__device__ __forceinline__ void fround(float (&v)[128], const unsigned mask, const float4* __restrict__ gk,
-                                       const int tl, const int th) {
+// One round: for every set bit of `mask` (ascending) the next gate of that register digit.  The
+// constants of the gate after the current one are already in flight (n0, n1): the gate list of a
+// pass is contiguous in execution order, so the prefetch simply runs one entry ahead.
+template <bool LOW>
+__device__ __forceinline__ void fround(float (&v)[128], const unsigned mask, const float4* __restrict__& gk,
+                                       float4& n0, float4& n1, const int tp, const int tq) {
 #define TTN_G(Kk)                                                                                   \
     if (mask & (1u << Kk)) {                                                                        \
-        const float4 c0 = gk[0], c1 = gk[1]; gk += 2;                                               \
-        cgate<Kk, Nbr<LOW, LAYOUT, Kk>::NL, Nbr<LOW, LAYOUT, Kk>::NH>(v, c0, c1, tl, th);           \
+        const float4 c0 = n0, c1 = n1;                                                              \
+        gk += 2; n0 = gk[0]; n1 = gk[1];                                                            \
+        cgate<Kk, Nbr<LOW, Kk>::PN, Nbr<LOW, Kk>::QN>(v, c0, c1, tp, tq);                           \
     }
     TTN_G(0) TTN_G(1) TTN_G(2) TTN_G(3) TTN_G(4) TTN_G(5) TTN_G(6)
 #undef TTN_G
 }
 
-// ---- exchange addressing: float4 index of register quad q for this lane -------------------------
-//   LOW : chunk X = (d0..d4) + 32 (d7..d11), row-padded: f4 = X + (X >> 5)
-//         A (lanes d7..d11): 33 lane + q          B (lanes d0..d4): lane + 33 q
-//   HIGH: f4 = rho + 8 Y, Y = d0 + 2 d1 + 4 d4 + 8 d5 + 16 d6 + 32 d7 + 64 d8
-//         A (lanes rho, d7, d8): rho + 256 (lane>>3) + 8 q      B (lanes rho, d0, d1): rho + 8 (lane>>3) + 32 q
-template <bool LOW, int LAYOUT>
-__device__ __forceinline__ int xbase(int lane) {
-    if (LOW) return LAYOUT == 0 ? 33 * lane : lane;
-    return LAYOUT == 0 ? (lane & 7) + 256 * (lane >> 3) : (lane & 7) + 8 * (lane >> 3);
+// ---- layout exchange through the warp's shared-memory region ----------------------------------------
+// LOW (128-bit): a float4 holds the 4 elements differing in (d5, d6), in layout A's register
+//   order (.x: d5=0,d6=0  .y: d5=1  .z: d6=1  .w: both); float4 index = (d0..d4) + 33 (d7..d11).
+//     A (lanes d7..d11, quad bits = d0..d4): 33 lane + q
+//     B (lanes d0..d4, quad bits = d11..d7, register bits 0,1 = d6,d5): lane + 33 rev5(q), and
+//       the two middle elements of the quad swap places.
+// HIGH (64-bit): a float2 holds the 2 elements differing in d4 (register bit 0 in both layouts);
+//   float2 index = rho + 8 (d0^d7) + 16 d7 + 32 d1 + 64 d2 + 128 d3 + 256 d5 + 512 d6 + 1024 d8
+//   (the XOR puts a lane digit of either layout on bank bit 3: conflict-free half-warps).
+//     A (lanes rho,d7,d8; pair bits = d5,d6,d0,d1,d2,d3)   B (lanes rho,d0,d1; pair bits = d3,d2,d8,d7,d6,d5)
+__host__ __device__ constexpr int rev5(int q) {
+    return ((q & 1) << 4) | ((q & 2) << 2) | (q & 4) | ((q & 8) >> 2) | ((q & 16) >> 4);
 }
-template <bool LOW, int LAYOUT>
-__device__ __forceinline__ constexpr int xstep() { return LOW ? (LAYOUT == 0 ? 1 : 33) : (LAYOUT == 0 ? 8 : 32); }
+__host__ __device__ constexpr int xh_imm_a(int pr) {   // pr = j >> 1: bits d5,d6,d0,d1,d2,d3 ; d0 goes to the base
+    return 256 * (pr & 1) + 512 * ((pr >> 1) & 1) + 32 * ((pr >> 3) & 1) + 64 * ((pr >> 4) & 1) + 128 * ((pr >> 5) & 1);
+}
+__host__ __device__ constexpr int xh_imm_b(int pr) {   // pr bits d3,d2,d8,d7,d6,d5 ; d7 goes to the base
+    return 128 * (pr & 1) + 64 * ((pr >> 1) & 1) + 1024 * ((pr >> 2) & 1) + 512 * ((pr >> 4) & 1) + 256 * ((pr >> 5) & 1);
+}
 
-template <bool LOW, int LAYOUT>
-__device__ __forceinline__ void xstore(const float (&v)[128], float4* reg, int lane) {
-    float4* p = reg + xbase<LOW, LAYOUT>(lane);
+template <bool LOW, int LAYOUT, bool STORE>
+__device__ __forceinline__ void xmove(float (&v)[128], float4* reg, int lane) {
+    if (LOW) {
+        if (LAYOUT == 0) {
+            float4* p = reg + 33 * lane;
 #pragma unroll
-    for (int q = 0; q < 32; ++q) p[q * xstep<LOW, LAYOUT>()] = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
-}
-template <bool LOW, int LAYOUT>
-__device__ __forceinline__ void xload(float (&v)[128], const float4* reg, int lane) {
-    const float4* p = reg + xbase<LOW, LAYOUT>(lane);
+            for (int q = 0; q < 32; ++q) {
+                if (STORE) p[q] = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+                else { const float4 t = p[q]; v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w; }
+            }
+        } else {
+            float4* p = reg + lane;
 #pragma unroll
-    for (int q = 0; q < 32; ++q) {
-        const float4 t = p[q * xstep<LOW, LAYOUT>()];
-        v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
+            for (int q = 0; q < 32; ++q) {
+                if (STORE) p[33 * rev5(q)] = make_float4(v[4 * q], v[4 * q + 2], v[4 * q + 1], v[4 * q + 3]);
+                else { const float4 t = p[33 * rev5(q)]; v[4 * q] = t.x; v[4 * q + 1] = t.z; v[4 * q + 2] = t.y; v[4 * q + 3] = t.w; }
+            }
+        }
+    } else {
+        float2* r2 = reinterpret_cast<float2*>(reg);
+        const int rho = lane & 7, l3 = (lane >> 3) & 1, l4 = (lane >> 4) & 1;
+        if (LAYOUT == 0) {          // l3 = d7, l4 = d8; base per d0 (pair bit 2)
+            float2* b0 = r2 + rho + 8 * l3 + 16 * l3 + 1024 * l4;
+            float2* b1 = r2 + rho + 8 * (1 - l3) + 16 * l3 + 1024 * l4;
+#pragma unroll
+            for (int pr = 0; pr < 64; ++pr) {
+                float2* p = (((pr >> 2) & 1) ? b1 : b0) + xh_imm_a(pr);
+                if (STORE) *p = make_float2(v[2 * pr], v[2 * pr + 1]);
+                else { const float2 t = *p; v[2 * pr] = t.x; v[2 * pr + 1] = t.y; }
+            }
+        } else {                    // l3 = d0, l4 = d1; base per d7 (pair bit 3)
+            float2* b0 = r2 + rho + 8 * l3 + 32 * l4;
+            float2* b1 = r2 + rho + 8 * (1 - l3) + 16 + 32 * l4;
+#pragma unroll
+            for (int pr = 0; pr < 64; ++pr) {
+                float2* p = (((pr >> 3) & 1) ? b1 : b0) + xh_imm_b(pr);
+                if (STORE) *p = make_float2(v[2 * pr], v[2 * pr + 1]);
+                else { const float2 t = *p; v[2 * pr] = t.x; v[2 * pr + 1] = t.y; }
+            }
+        }
     }
 }
 
 // ---- global <-> register: element index e (inside the warp tile) of register j ---------------
-//   LOW  B: e = lane + 32 j                      (address = tile base + e; 128 B per request)
-//   HIGH A: e = 4 (j & 3) + ((j >> 2) & 3) + (j & 0x70) + 128 (lane >> 3)
-//   HIGH B: e = (lane >> 3) + 4 j                (address = tile base + rho + (e << a))
-__device__ __forceinline__ constexpr int ereg_high_a(int j) { return 4 * (j & 3) + ((j >> 2) & 3) + (j & 0x70); }
+//   LOW  B: e = lane + 32 (d5 + 2 d6 + ... + 64 d11), register bits = d6,d5,d11,d10,d9,d8,d7
+//   HIGH A: e = 16 b0 + 32 b1 + 64 b2 + b3 + 2 b4 + 4 b5 + 8 b6 + 128 (lane >> 3)
+//   HIGH B: e = 16 b0 +  8 b1 +  4 b2 + 256 b3 + 128 b4 + 64 b5 + 32 b6 + (lane >> 3)
+//   (address = tile base + rho + (e << a) for HIGH)
+__host__ __device__ constexpr int ereg_low_b(int j) {
+    return 2 * (j & 1) + ((j >> 1) & 1) + 64 * ((j >> 2) & 1) + 32 * ((j >> 3) & 1) + 16 * ((j >> 4) & 1) +
+           8 * ((j >> 5) & 1) + 4 * ((j >> 6) & 1);
+}
+__host__ __device__ constexpr int ereg_high(int layout, int j) {
+    return layout == 0
+        ? 16 * (j & 1) + 32 * ((j >> 1) & 1) + 64 * ((j >> 2) & 1) + ((j >> 3) & 1) + 2 * ((j >> 4) & 1) +
+          4 * ((j >> 5) & 1) + 8 * ((j >> 6) & 1)
+        : 16 * (j & 1) + 8 * ((j >> 1) & 1) + 4 * ((j >> 2) & 1) + 256 * ((j >> 3) & 1) + 128 * ((j >> 4) & 1) +
+          64 * ((j >> 5) & 1) + 32 * ((j >> 6) & 1);
+}
 
-template <bool LOW, bool STORE>
-__device__ __forceinline__ void gmove(float (&v)[128], float* tile, int lane, int layout, unsigned long long estride) {
+// address of element offset (imm * stride) from a 64-bit base in ONE fma-pipe instruction
+// (IMAD.WIDE.U32); `sb` is the stride in bytes as an opaque 32-bit value.
+__device__ __forceinline__ float* addr_mad(const float* base, unsigned sb, unsigned imm) {
+    unsigned long long r;
+    asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(r) : "r"(sb), "r"(imm), "l"(reinterpret_cast<unsigned long long>(base)));
+    return reinterpret_cast<float*>(r);
+}
+
+template <bool LOW, int LAYOUT, bool STORE>
+__device__ __forceinline__ void gmove(float (&v)[128], float* tile, int lane, unsigned sb, int a) {
     if (LOW) {
         float* p = tile + lane;                                   // layout B only (planner guarantees)
 #pragma unroll
-        for (int j = 0; j < 128; ++j) { if (STORE) p[32 * j] = v[j]; else v[j] = p[32 * j]; }
-    } else if (layout == 0) {
-        // 32-bit element offsets (e * 2^a < 2^32) keep the address math on the FMA pipe (IMAD.WIDE)
-        const unsigned es = (unsigned)estride;
-        float* p = tile + (lane & 7) + (unsigned long long)(128 * (lane >> 3)) * estride;
+        for (int j = 0; j < 128; ++j) { if (STORE) p[32 * ereg_low_b(j)] = v[j]; else v[j] = p[32 * ereg_low_b(j)]; }
+        return;
+    }
+    // HIGH: element e of the tile sits at tile + rho + (e << a); per-lane part first
+    const unsigned elane = (LAYOUT == 0) ? 128u * (unsigned)(lane >> 3) : (unsigned)(lane >> 3);
+    float* p = tile + (lane & 7) + ((unsigned long long)elane << a);
+    if (sb) {        // a <= 20: 511 * sb < 2^32
 #pragma unroll
         for (int j = 0; j < 128; ++j) {
-            float* q = p + (unsigned)(ereg_high_a(j)) * es;
+            float* q = addr_mad(p, sb, (unsigned)ereg_high(LAYOUT, j));
             if (STORE) *q = v[j]; else v[j] = *q;
         }
-    } else {
-        const unsigned es = (unsigned)estride;
-        float* p = tile + (lane & 7) + (unsigned long long)(lane >> 3) * estride;
+    } else {         // e << a = (e << (a - 20)) << 20 keeps the product inside 32 bits
+        const unsigned s20 = 1u << (a - 20);
 #pragma unroll
         for (int j = 0; j < 128; ++j) {
-            float* q = p + (unsigned)(4 * j) * es;
+            unsigned long long off;
+            asm("mul.wide.u32 %0, %1, %2;" : "=l"(off) : "r"(s20), "r"((unsigned)ereg_high(LAYOUT, j)));
+            float* q = p + (off << 20);
             if (STORE) *q = v[j]; else v[j] = *q;
         }
     }
 }
 
 // ---- last pass: v[j] += A_{L-1}(s) -------------------------------------------------------------------
-// s_fin = [4 variants][128] table over the register digits (variant = tl + 2 th: the two boundary
-// couplings to the per-thread neighbours) followed by H[64], K[64] (accumulated fields and
-// horizontal couplings).  x0 = first register column; sthr = the element index with the register
-// digits cleared.
+// s_fin = [4 variants][128] table over the register digits (variant = tl + 2 th: the boundary
+// couplings to the columns left / right of the 7 register columns) followed by H[64], K[64]
+// (accumulated fields and horizontal couplings).  x0 = first register column; sthr = the
+// element index with the register digits cleared.
 __device__ __forceinline__ float final_thread_const(const float* s_fin, int L, int x0, unsigned long long sthr) {
     const float* H = s_fin + 512; const float* Kc = s_fin + 576;
     float acc = 0.f;
@@ -211,25 +278,14 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
     constexpr int FWARPS = fwarps(LOW);
     extern __shared__ __align__(16) unsigned char fsm_raw[];
     float4* regions = reinterpret_cast<float4*>(fsm_raw);                              // FWARPS * FREGION_F4
-    float4* s_gk = reinterpret_cast<float4*>(fsm_raw + (size_t)FWARPS * FREGION_F4 * 16);   // FMAX_GATES * 2
-    float* s_fin = reinterpret_cast<float*>(s_gk + FMAX_GATES * 2);                     // FFINAL_FLOATS
+    float4* s_gk = reinterpret_cast<float4*>(fsm_raw + (size_t)FWARPS * FREGION_F4 * 16);   // (FMAX_GATES + 1) * 2
+    float* s_fin = reinterpret_cast<float*>(s_gk + (FMAX_GATES + 1) * 2);               // FFINAL_FLOATS
     unsigned* s_mops = reinterpret_cast<unsigned*>(s_fin + FFINAL_FLOATS);              // FMAX_MOPS
     float* s_red = reinterpret_cast<float*>(s_mops + FMAX_MOPS);                        // FWARPS (<= 16)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     float4* myreg = regions + warp * FREGION_F4;
     const unsigned long long gw = (unsigned long long)blockIdx.x * FWARPS + warp;
     const unsigned long long nw = (unsigned long long)gridDim.x * FWARPS;
-    const unsigned long long estride = 1ull << p.a;
-
-    // De-phase the warps of one scheduler (warps w, w+4, w+8 share SM sub-partition w % 4).  All
-    // tiles cost the same and the schedulers share the alu pipe fairly, so warps that start
-    // together stay in lock-step: they all compute, then all wait on memory, and the two never
-    // overlap.  Starting group g one gate-phase later keeps one group in its memory phase while
-    // the others compute.
-    if (p.stagger_cycles && warp >= 4) {
-        const long long t_end = clock64() + (long long)(warp >> 2) * p.stagger_cycles;
-        while (clock64() < t_end) __nanosleep(256);
-    }
 
     for (int inst = 0; inst < p.batch; ++inst) {
         // ---- stage this instance's program and gate constants (S0 outputs) into shared memory
@@ -241,6 +297,7 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
         {
             const float4* src = reinterpret_cast<const float4*>(p.gate_k + (size_t)inst * p.gate_inst_stride);
             for (int i = tid; i < p.n_gates * 2; i += blockDim.x) s_gk[i] = src[i];
+            if (tid < 2) s_gk[p.n_gates * 2 + tid] = make_float4(0.f, 0.f, 0.f, 0.f);   // prefetch runs one ahead
         }
         if (p.flags & PASS_REDUCE)
             for (int i = tid; i < FFINAL_FLOATS; i += blockDim.x) s_fin[i] = p.final_tab[(size_t)inst * FFINAL_FLOATS + i];
@@ -249,47 +306,49 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
         float wmax = -INFINITY;
 
         for (unsigned long long wt = gw; wt < p.tiles_per_inst; wt += nw) {
-            // ---- tile geometry: base index, per-thread neighbour bits ------------------------------
+            // ---- tile geometry: base index, per-thread P / Q neighbour bits per layout ---------------
             unsigned long long base;
-            int tlA, thA, tlB, thB;     // per-thread left / right neighbour bit in layout A / B
+            int tpA, tqA, tpB, tqB;
             if (LOW) {
                 base = wt << 12;
-                tlA = 0;                                   // column -1 does not exist
-                thA = lane & 1;                            // d7 (lane bit 0 in layout A)
-                tlB = (lane >> 4) & 1;                     // d4 (lane bit 4 in layout B)
-                thB = (p.L > F_WLOW) ? (int)(wt & 1ull) : 0;                      // column 12
+                tpA = 0;                                   // column -1 does not exist
+                tqA = lane & 1;                            // d7 (lane bit 0 in layout A)
+                tpB = (p.L > F_WLOW) ? (int)(wt & 1ull) : 0;                      // column 12
+                tqB = (lane >> 4) & 1;                     // d4 (lane bit 4 in layout B)
             } else {
                 const int amid = p.a - F_RIDE;
                 const unsigned long long tmid = wt & ((1ull << amid) - 1), ttop = wt >> amid;
                 base = (tmid << F_RIDE) + (ttop << (p.a + F_WHIGH));
-                tlA = (int)((base >> (p.a - 1)) & 1ull);                          // column a-1 (>= 3)
-                thA = (lane >> 3) & 1;                     // d7
-                tlB = (lane >> 4) & 1;                     // d1
-                thB = (p.a + F_WHIGH < p.L) ? (int)(ttop & 1ull) : 0;             // column a+9
+                tpA = (int)((base >> (p.a - 1)) & 1ull);                          // column a-1 (>= 3)
+                tqA = (lane >> 3) & 1;                     // d7
+                tpB = (p.a + F_WHIGH < p.L) ? (int)(ttop & 1ull) : 0;             // column a+9
+                tqB = (lane >> 4) & 1;                     // d1
             }
             float v[128];
             if (p.flags & PASS_INIT) {
 #pragma unroll
                 for (int j = 0; j < 128; ++j) v[j] = 0.f;                         // tropical one
+            } else if (LOW || p.first_layout == 1) {
+                gmove<LOW, 1, false>(v, S + base, lane, p.stride_bytes, p.a);
             } else {
-                gmove<LOW, false>(v, S + base, lane, p.first_layout, estride);
+                gmove<LOW, 0, false>(v, S + base, lane, p.stride_bytes, p.a);
             }
             // ---- run the program ------------------------------------------------------------------
             int pc = 0, layout = p.first_layout;
             unsigned op = s_mops[0];
+            const float4* gk = s_gk;
+            float4 n0 = gk[0], n1 = gk[1];
             for (;;) {
                 const unsigned code = op & 0xffu;
                 if (code == MC_END || code == MC_FINAL) break;
                 const unsigned nxt = s_mops[pc + 1];
                 if (code == MC_ROUND) {
-                    const float4* gk = s_gk + 2 * (op >> 16);
-                    if (layout == 0) fround<LOW, 0>(v, (op >> 8) & 0x7fu, gk, tlA, thA);
-                    else fround<LOW, 1>(v, (op >> 8) & 0x7fu, gk, tlB, thB);
+                    fround<LOW>(v, (op >> 8) & 0x7fu, gk, n0, n1, layout ? tpB : tpA, layout ? tqB : tqA);
                 } else if (code == MC_XAB) {
-                    __syncwarp(); xstore<LOW, 0>(v, myreg, lane); __syncwarp(); xload<LOW, 1>(v, myreg, lane);
+                    __syncwarp(); xmove<LOW, 0, true>(v, myreg, lane); __syncwarp(); xmove<LOW, 1, false>(v, myreg, lane);
                     layout = 1;
                 } else {
-                    __syncwarp(); xstore<LOW, 1>(v, myreg, lane); __syncwarp(); xload<LOW, 0>(v, myreg, lane);
+                    __syncwarp(); xmove<LOW, 1, true>(v, myreg, lane); __syncwarp(); xmove<LOW, 0, false>(v, myreg, lane);
                     layout = 0;
                 }
                 op = nxt; ++pc;
@@ -299,11 +358,11 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
                 // element index with the register digits cleared, first register column, variant
                 unsigned long long sthr; int x0, var;
                 if (LOW) {
-                    if (layout == 0) { sthr = base + ((unsigned long long)lane << 7); x0 = 0; var = tlA + 2 * thA; }
-                    else { sthr = base + lane; x0 = 5; var = tlB + 2 * thB; }
+                    if (layout == 0) { sthr = base + ((unsigned long long)lane << 7); x0 = 0; var = tpA + 2 * tqA; }
+                    else { sthr = base + lane; x0 = 5; var = tqB + 2 * tpB; }
                 } else {
-                    if (layout == 0) { sthr = base + (lane & 7) + ((unsigned long long)(lane >> 3) << (p.a + 7)); x0 = p.a; var = tlA + 2 * thA; }
-                    else { sthr = base + (lane & 7) + ((unsigned long long)(lane >> 3) << p.a); x0 = p.a + 2; var = tlB + 2 * thB; }
+                    if (layout == 0) { sthr = base + (lane & 7) + ((unsigned long long)(lane >> 3) << (p.a + 7)); x0 = p.a; var = tpA + 2 * tqA; }
+                    else { sthr = base + (lane & 7) + ((unsigned long long)(lane >> 3) << p.a); x0 = p.a + 2; var = tqB + 2 * tpB; }
                 }
                 const float cthr = final_thread_const(s_fin, p.L, x0, sthr);
                 const float4* T = reinterpret_cast<const float4*>(s_fin + var * 128);
@@ -314,8 +373,10 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
                     mx = fmaxf(mx, fmaxf(fmaxf(v[4 * q] + t.x, v[4 * q + 1] + t.y), fmaxf(v[4 * q + 2] + t.z, v[4 * q + 3] + t.w)));
                 }
                 wmax = fmaxf(wmax, mx + cthr);
+            } else if (LOW || p.last_layout == 1) {
+                gmove<LOW, 1, true>(v, S + base, lane, p.stride_bytes, p.a);
             } else {
-                gmove<LOW, true>(v, S + base, lane, p.last_layout, estride);
+                gmove<LOW, 0, true>(v, S + base, lane, p.stride_bytes, p.a);
             }
         }
         if (p.flags & PASS_REDUCE) {
@@ -334,7 +395,7 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
 // ---- S0: per-instance gate constants and the final table from the couplings ------------------------
 struct FusedPrepParams {
     int L, n_gates;
-    const int* gate_rc;            // [n_gates]  r * 64 + c
+    const int* gate_rc;            // [n_gates]  layout * 4096 + r * 64 + c
     const float* Jh; const float* Jv; const float* h;   // device couplings, per instance
     float* gate_k;                 // [inst][n_gates][8]
     float* final_tab;              // [inst][FFINAL_FLOATS]
@@ -352,15 +413,17 @@ __global__ void __launch_bounds__(256) fused_prep_kernel(const FusedPrepParams p
     auto Hacc = [&](int R, int c) { double s = 0; if (hh) for (int r = 0; r < R; ++r) s += (double)hh[r * L + c]; return s; };
     auto Kacc = [&](int R, int c) { double s = 0; if (c < 0 || c >= L - 1) return s; for (int r = 0; r < R; ++r) s += (double)Jh[r * (L - 1) + c]; return s; };
     if (idx < p.n_gates) {
-        const int r = p.gate_rc[idx] >> 6, c = p.gate_rc[idx] & 63;
+        const int g = p.gate_rc[idx], mirrored = g >> 12, r = (g >> 6) & 63, c = g & 63;
         const double m = -2.0 * (double)Jv[(r - 1) * L + c];
         const double H = Hacc(r, c), Kl = Kacc(r, c - 1), Kr = Kacc(r, c);
         float* out = p.gate_k + (inst * p.n_gates + idx) * 8;
-        for (int nl = 0; nl < 2; ++nl)
-            for (int nh = 0; nh < 2; ++nh) {
+        // stored as [side][P bit][Q bit]: P = left neighbour in layout A, right neighbour in layout B
+        for (int np = 0; np < 2; ++np)
+            for (int nq = 0; nq < 2; ++nq) {
+                const int nl = mirrored ? nq : np, nh = mirrored ? np : nq;
                 const double rho = H + (nl ? -Kl : Kl) + (nh ? -Kr : Kr);
-                out[nl * 2 + nh] = (float)(m - 2.0 * rho);         // ka: a' = max(a, b + ka)
-                out[4 + nl * 2 + nh] = (float)(m + 2.0 * rho);     // kb: b' = max(b, a + kb)
+                out[np * 2 + nq] = (float)(m - 2.0 * rho);         // ka: a' = max(a, b + ka)
+                out[4 + np * 2 + nq] = (float)(m + 2.0 * rho);     // kb: b' = max(b, a + kb)
             }
     }
     if (idx < FFINAL_FLOATS) {
@@ -368,11 +431,9 @@ __global__ void __launch_bounds__(256) fused_prep_kernel(const FusedPrepParams p
         if (idx < 512) {
             const int var = (int)idx >> 7, j = (int)idx & 127, tl = var & 1, th = var >> 1;
             const bool low = p.fin_low != 0;
-            const int W = low ? F_WLOW : F_WHIGH;
             // register columns are consecutive: x0 .. x0+6
             const int d0 = low ? (p.fin_layout == 0 ? 0 : 5) : (p.fin_layout == 0 ? 0 : 2);
             const int x0 = p.fin_a + d0;
-            (void)W;
             double acc = 0;
             int bits[F_RB];
             for (int i = 0; i < F_RB; ++i) bits[i] = (j >> fused_bit_of_digit(low, p.fin_layout, d0 + i)) & 1;

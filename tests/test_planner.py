@@ -122,8 +122,9 @@ def test_fusion_cuts_hbm_passes():
 #     rho = H_c + K_{c-1} sigma_{c-1} + K_c sigma_{c+1};   result = max_s(V(s) + A_{L-1}(s)).
 # Dependency rule in this frame: g(r,c) after g(r-1,c-1), g(r-1,c), g(r-1,c+1).
 # register-index bit -> tile digit, as documented in csrc/planner.h (fused_digit_of_bit)
-DIGIT_OF_BIT = {(1, 0): [5, 6, 0, 1, 2, 3, 4], (1, 1): [5, 6, 7, 8, 9, 10, 11],
-                (0, 0): [2, 3, 0, 1, 4, 5, 6], (0, 1): [2, 3, 4, 5, 6, 7, 8]}
+# (mirrored layouts: layout B holds the register digits in reverse chain order)
+DIGIT_OF_BIT = {(1, 0): [5, 6, 0, 1, 2, 3, 4], (1, 1): [6, 5, 11, 10, 9, 8, 7],
+                (0, 0): [4, 5, 6, 0, 1, 2, 3], (0, 1): [4, 3, 2, 8, 7, 6, 5]}
 
 
 def parse_fused(txt):
@@ -180,6 +181,7 @@ def fused_to_gates(L, fpasses):
                 for g in m["gates"]:
                     c, r = g["c"], g["r"]
                     assert c == a + DIGIT_OF_BIT[(low, layout)][g["k"]]      # register bit <-> column
+                    assert g["layout"] == layout
                     # legal at the START of the round: every gate of a round commutes with the others
                     assert 1 <= r < L and before[c] == r
                     assert c == 0 or before[c - 1] >= r
