@@ -61,6 +61,32 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def rank_env():
+    """(rank, local_rank, world) from the torchrun environment (1 process per GPU)."""
+    return (int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")),
+            int(os.environ.get("WORLD_SIZE", "1")))
+
+
+def seed_for_rank(rank: int) -> int:
+    """Replicas only: rank r sweeps its own cfg-4 instance."""
+    return 4000 + rank
+
+
+def max_over_ranks(x: float, dist, device="cpu") -> float:
+    """Device-timed numbers are reported as the MAX over ranks (the contract's timing rule)."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([x], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_ms_per_instance(ms_per_step: float, world: int) -> float:
+    """Each rank sweeps one instance per step: `value` = step time / instances in flight."""
+    return ms_per_step / world
+
+
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons during the timed region (nvidia-smi, 200 ms)."""
 
@@ -160,9 +186,7 @@ def main():
     import torch
     import paper_2008_06888_b200 as ttn
 
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank, local_rank, world = rank_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the sweep has no CPU path)")
     torch.cuda.set_device(local_rank)
@@ -172,7 +196,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     L = args.L
-    Jh, Jv, _ = make_batch(L, [4000 + rank], "pmj")
+    Jh, Jv, _ = make_batch(L, [seed_for_rank(rank)], "pmj")
     ws = ttn.alloc_workspace(ttn.workspace_bytes(2, L, ttn.TROPICAL_F32, 1), f"cuda:{local_rank}")
     plan = ttn.Plan(2, ttn.CALL_ENERGY, Jh, Jv, None, workspace=ws)
     torch.cuda.synchronize()
@@ -201,10 +225,7 @@ def main():
     clocks = sampler.stop() if sampler else None
     total_ms = ev[0].elapsed_time(ev[-1])
     step_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
-    if dist is not None:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, dist, "cuda")
     ms_per_step = total_ms / args.steps
 
     # ---- end to end through the one-call C ABI with host buffers -----------------------------
@@ -216,15 +237,12 @@ def main():
         if i >= 2:
             e2e_times.append((time.perf_counter() - t0) * 1e3)
     e2e_ms = float(np.mean(e2e_times))
-    if dist is not None:
-        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms = max_over_ranks(e2e_ms, dist, "cuda")
     assert E_host == E_dev, (E_host, E_dev)
 
     if rank == 0:
         peak, peak_src = measured_peaks()
-        per_inst_ms = ms_per_step / world
+        per_inst_ms = whole_job_ms_per_instance(ms_per_step, world)
         achieved = bytes_min(L) / (ms_per_step * 1e-3) / 1e9            # GB/s per GPU
         sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
         alu_peak = 148 * 64 * sm_mhz * 1e6                              # FMNMX: 64 lanes/clk/SM (alu pipe)
@@ -245,7 +263,7 @@ def main():
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
                          "algorithmic_bytes_per_sweep": bytes_min(L),
-                         "kernel": "ttn::pass_kernel<2,false> (all passes of one sweep)"},
+                         "kernel": "ttn::fused_pass_kernel<LOW|HIGH> (all %d pass launches of one sweep)" % plan.num_passes},
             "alu_roofline": {"bound": "alu", "achieved": updates(L) / (ms_per_step * 1e-3),
                              "peak": alu_peak, "unit": "max-plus updates/s",
                              "frac": updates(L) / (ms_per_step * 1e-3) / alu_peak,
