@@ -208,7 +208,7 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
     pp.gate_inst_stride = (unsigned long long)fp.gate_rc.size() * 8;
     pp.final_tab = reinterpret_cast<const float*>(P->ws + y.f_final);
     pp.part_x = reinterpret_cast<float*>(P->ws + y.part_x);
-    pp.stride_bytes = ps.a <= 20 ? (4u << ps.a) : 0u;
+    pp.stride_bytes = 4u << ps.a;     // a <= L - 9 <= 25
     unsigned long long grid = (unsigned long long)P->fused_grid;
     const int nw = ttn::fwarps(ps.low != 0);
     const unsigned long long need = (pp.tiles_per_inst + nw - 1) / nw;

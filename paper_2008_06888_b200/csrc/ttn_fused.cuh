@@ -24,14 +24,14 @@
 
 namespace ttn {
 
-// Warps per CTA (one CTA per SM).  LOW: 12 warps of <= 168 registers, 3 per scheduler.  HIGH: 8 warps;
-// with 12 the scattered 32-byte-sector traffic of the strided tiles collapses (measured: a
-// store-only pass takes 11 ms with 12 warps, 3.6 ms with 8).
+// Warps per CTA (one CTA per SM): 12 warps of <= 168 registers, 3 per scheduler.  For the HIGH
+// kernel this needs the group barriers below: 12 free-running warps requesting scattered 32-byte
+// sectors take 13-16 ms for a copy-only pass, synchronised 4-warp groups 9 ms.
 #ifndef TTN_FWARPS_LOW
 #define TTN_FWARPS_LOW 12
 #endif
 #ifndef TTN_FWARPS_HIGH
-#define TTN_FWARPS_HIGH 8
+#define TTN_FWARPS_HIGH 12
 #endif
 constexpr int FWARPS_LOW = TTN_FWARPS_LOW, FWARPS_HIGH = TTN_FWARPS_HIGH;
 constexpr int FREGION_F4 = 33 * 32;       // float4 per warp exchange region (low tile: padded rows)
@@ -54,8 +54,8 @@ struct FusedParams {
     unsigned long long gate_inst_stride;          // floats between instances
     const float* final_tab;             // [inst][FFINAL_FLOATS] (REDUCE pass only)
     float* part_x;                      // [batch][gridDim.x] (REDUCE)
-    unsigned stride_bytes;              // HIGH: 4 << a (a <= 20), passed opaque so that the address
-                                        // math stays one IMAD.WIDE per access; else 0
+    unsigned stride_bytes;              // HIGH: 4 << a, passed opaque so that the address math stays
+                                        // one IMAD.WIDE (32 x 32 -> 64 bit) per access
 };
 
 // (o0, o1) = (a0 + b0, a1 + b1) in one FADD2
@@ -214,11 +214,25 @@ __host__ __device__ constexpr int ereg_high(int layout, int j) {
 }
 
 // address of element offset (imm * stride) from a 64-bit base in ONE fma-pipe instruction
-// (IMAD.WIDE.U32); `sb` is the stride in bytes as an opaque 32-bit value.
-__device__ __forceinline__ float* addr_mad(const float* base, unsigned sb, unsigned imm) {
+// (IMAD.WIDE.U32); `sb` is the stride in bytes as an opaque 32-bit value.  The result is a
+// GLOBAL-space address: the accesses below are spelled ld.global / st.global because a pointer
+// that comes out of inline asm is "generic" to the compiler (LD/ST instead of LDG/STG).
+__device__ __forceinline__ unsigned long long addr_mad(unsigned long long gbase, unsigned sb, unsigned imm) {
     unsigned long long r;
-    asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(r) : "r"(sb), "r"(imm), "l"(reinterpret_cast<unsigned long long>(base)));
-    return reinterpret_cast<float*>(r);
+    asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(r) : "r"(sb), "r"(imm), "l"(gbase));
+    return r;
+}
+__device__ __forceinline__ float ldg_f32(unsigned long long ga) {
+    float x;
+#ifdef TTN_HIGH_LD128
+    asm volatile("ld.global.L2::128B.f32 %0, [%1];" : "=f"(x) : "l"(ga));
+#else
+    asm volatile("ld.global.f32 %0, [%1];" : "=f"(x) : "l"(ga));
+#endif
+    return x;
+}
+__device__ __forceinline__ void stg_f32(unsigned long long ga, float x) {
+    asm volatile("st.global.f32 [%0], %1;" :: "l"(ga), "f"(x) : "memory");
 }
 
 template <bool LOW, int LAYOUT, bool STORE>
@@ -231,22 +245,11 @@ __device__ __forceinline__ void gmove(float (&v)[128], float* tile, int lane, un
     }
     // HIGH: element e of the tile sits at tile + rho + (e << a); per-lane part first
     const unsigned elane = (LAYOUT == 0) ? 128u * (unsigned)(lane >> 3) : (unsigned)(lane >> 3);
-    float* p = tile + (lane & 7) + ((unsigned long long)elane << a);
-    if (sb) {        // a <= 20: 511 * sb < 2^32
+    const unsigned long long p = (unsigned long long)__cvta_generic_to_global(tile + (lane & 7) + ((unsigned long long)elane << a));
 #pragma unroll
-        for (int j = 0; j < 128; ++j) {
-            float* q = addr_mad(p, sb, (unsigned)ereg_high(LAYOUT, j));
-            if (STORE) *q = v[j]; else v[j] = *q;
-        }
-    } else {         // e << a = (e << (a - 20)) << 20 keeps the product inside 32 bits
-        const unsigned s20 = 1u << (a - 20);
-#pragma unroll
-        for (int j = 0; j < 128; ++j) {
-            unsigned long long off;
-            asm("mul.wide.u32 %0, %1, %2;" : "=l"(off) : "r"(s20), "r"((unsigned)ereg_high(LAYOUT, j)));
-            float* q = p + (off << 20);
-            if (STORE) *q = v[j]; else v[j] = *q;
-        }
+    for (int j = 0; j < 128; ++j) {      // 32 x 32 -> 64-bit product: valid for sb < 2^32 (a <= 29)
+        const unsigned long long q = addr_mad(p, sb, (unsigned)ereg_high(LAYOUT, j));
+        if (STORE) stg_f32(q, v[j]); else v[j] = ldg_f32(q);
     }
 }
 
@@ -271,6 +274,13 @@ __device__ __forceinline__ float final_thread_const(const float* s_fin, int L, i
         }
     }
     return acc;
+}
+
+// named barrier of one 4-warp group (barrier 0 is __syncthreads)
+__device__ __forceinline__ void group_sync(int warp) {
+#ifndef TTN_NO_GROUPSYNC
+    asm volatile("bar.sync %0, 128;" :: "r"(1 + (warp >> 2)) : "memory");
+#endif
 }
 
 template <bool LOW>
@@ -305,7 +315,20 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
         float* S = p.state + (unsigned long long)inst * p.inst_stride;
         float wmax = -INFINITY;
 
-        for (unsigned long long wt = gw; wt < p.tiles_per_inst; wt += nw) {
+        // HIGH: the 4 warps of a group (one per scheduler) take 4 consecutive tiles -- the 4 sectors
+        // of every 128-byte line -- and meet at a named barrier before their loads and before their
+        // stores, so that the lines are requested whole and at the same time (scattered 32-byte
+        // sectors that arrive at different times cost DRAM efficiency); groups drift freely against
+        // each other, which is what overlaps memory phases with gate phases.
+        for (unsigned long long it = 0;; ++it) {
+            const unsigned long long wt = LOW ? it * nw + gw
+                : 4ull * (it * (nw >> 2) + (gw >> 2)) + (unsigned long long)(warp & 3);
+            if ((LOW ? wt : (wt & ~3ull)) >= p.tiles_per_inst) break;       // uniform per group
+            if (!LOW && wt >= p.tiles_per_inst) {      // L = 13: fewer than 4 tiles; keep the barrier counts equal
+                if (!(p.flags & PASS_INIT)) group_sync(warp);
+                if (!(p.flags & PASS_REDUCE)) group_sync(warp);
+                continue;
+            }
             // ---- tile geometry: base index, per-thread P / Q neighbour bits per layout ---------------
             unsigned long long base;
             int tpA, tqA, tpB, tqB;
@@ -328,10 +351,10 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
             if (p.flags & PASS_INIT) {
 #pragma unroll
                 for (int j = 0; j < 128; ++j) v[j] = 0.f;                         // tropical one
-            } else if (LOW || p.first_layout == 1) {
-                gmove<LOW, 1, false>(v, S + base, lane, p.stride_bytes, p.a);
             } else {
-                gmove<LOW, 0, false>(v, S + base, lane, p.stride_bytes, p.a);
+                if (!LOW) group_sync(warp);
+                if (LOW || p.first_layout == 1) gmove<LOW, 1, false>(v, S + base, lane, p.stride_bytes, p.a);
+                else gmove<LOW, 0, false>(v, S + base, lane, p.stride_bytes, p.a);
             }
             // ---- run the program ------------------------------------------------------------------
             int pc = 0, layout = p.first_layout;
@@ -373,10 +396,10 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
                     mx = fmaxf(mx, fmaxf(fmaxf(v[4 * q] + t.x, v[4 * q + 1] + t.y), fmaxf(v[4 * q + 2] + t.z, v[4 * q + 3] + t.w)));
                 }
                 wmax = fmaxf(wmax, mx + cthr);
-            } else if (LOW || p.last_layout == 1) {
-                gmove<LOW, 1, true>(v, S + base, lane, p.stride_bytes, p.a);
             } else {
-                gmove<LOW, 0, true>(v, S + base, lane, p.stride_bytes, p.a);
+                if (!LOW) group_sync(warp);
+                if (LOW || p.last_layout == 1) gmove<LOW, 1, true>(v, S + base, lane, p.stride_bytes, p.a);
+                else gmove<LOW, 0, true>(v, S + base, lane, p.stride_bytes, p.a);
             }
         }
         if (p.flags & PASS_REDUCE) {
