@@ -7,14 +7,16 @@
 //   dJ(r,c) c < L-1 : the two-site diagonal gate (A4) PAPER.md:251: += Jh[r][c] sigma_c sigma_c+1.
 // "The order of operation of these diagonal gates ... can be arbitrary"; gates on
 // different digits commute.  Two operations fail to commute only when one is a gate on digit c
-// and the other is a gate on c or a diagonal that reads digit c.  Hence the dependency rule
+// and the other is a gate on c or a diagonal that reads digit c:
 //     g(r,c)  before  dh(r,c), dJ(r,c-1), dJ(r,c)  before  g(r+1,c).
+// Both kernel paths run in the DIAGONAL FRAME (defined at the fused section below): all dh / dJ
+// are folded into conjugated gates, and the rule becomes the three-point stencil
+//     g(r,c)  after  g(r-1,c-1), g(r-1,c), g(r-1,c+1);   gates of one row commute.
 // A pass holds a set of digits in its tile (a contiguous low block [0,lo) that "rides" for
-// coalescing plus a high block [a,b)); it may apply, in a legal order, any gate whose digit is
-// in the tile and any diagonal (a diagonal only needs the element's own global index).  The
-// planner visits a cyclic sequence of overlapping tiles and, in each pass, greedily applies
-// every operation that has become legal -- trapezoids/parallelograms over (row, column) as
-// deep as the tile allows -- which cuts HBM passes from ceil(L/T) per row to well below one.
+// coalescing plus a high block [a,b)) and may apply any legal gate whose digit is in the tile.
+// The planner visits a cyclic sequence of overlapping tiles and, in each pass, greedily applies
+// every gate that has become legal -- trapezoids/parallelograms over (row, column) as deep as
+// the tile allows -- which cuts HBM passes from ceil(L/T) per row to well below one.
 //
 // Host only; no CUDA.  The same structures are dumped by ttn_plan_describe() and replayed by
 // tests/test_planner.py against an independent statement of the rule.
@@ -56,65 +58,47 @@ struct Plan {
 
 struct TileSpec { int lo, a, b; };
 
+// Generic-path scheduler in the DIAGONAL FRAME (see the fused section below for the frame): only
+// gates are scheduled; g(r,c) is legal once g(r-1,c-1), g(r-1,c), g(r-1,c+1) are done.
 class Scheduler {
   public:
-    Scheduler(int L, bool has_field) : L_(L), has_field_(has_field), grow_(L, 1),
-        dh_(L * L, 0), dj_(L * (L > 1 ? L - 1 : 1), 0) {
-        if (!has_field_) for (auto& x : dh_) x = 1;   // nothing to apply
-    }
+    explicit Scheduler(int L) : L_(L), grow_(L, 1) {}
     bool done() const {
         for (int c = 0; c < L_; ++c) if (grow_[c] != L_) return false;
-        for (auto x : dh_) if (!x) return false;
-        for (int r = 0; r < L_; ++r) for (int c = 0; c + 1 < L_; ++c) if (!dj_[r * (L_ - 1) + c]) return false;
         return true;
     }
-    bool row_done(int r) const {   // all of row r's gates and diagonals applied
-        for (int c = 0; c < L_; ++c) if (grow_[c] < r + 1 || !dh_[r * L_ + c]) return false;
-        for (int c = 0; c + 1 < L_; ++c) if (!dj_[r * (L_ - 1) + c]) return false;
+    bool row_done(int r) const {   // all of row r's gates applied
+        for (int c = 0; c < L_; ++c) if (grow_[c] < r + 1) return false;
         return true;
     }
     // Greedily apply everything legal for tile digits [0,lo) U [a,b) with rows <= max_row.
     // Appends to ops; returns number of gates applied.
     int run_pass(const TileSpec& t, int max_row, std::vector<Op>& ops) {
         int gates = 0;
-        bool progress = true;
         auto in_tile = [&](int c) { return c < t.lo || (c >= t.a && c < t.b); };
         auto pos_of = [&](int c) { return c < t.lo ? c : t.lo + (c - t.a); };
-        while (progress) {
-            progress = false;
+        for (;;) {
+            std::vector<int> legal;                          // legal at the start of this round
             for (int c = 0; c < L_; ++c) {
                 if (!in_tile(c)) continue;
-                int r = grow_[c] - 1;                       // row currently complete on digit c
-                if (r > max_row) continue;
-                if (!dh_[r * L_ + c]) { dh_[r * L_ + c] = 1; ops.push_back({OP_DH, 0, (uint8_t)c, 0, (uint16_t)r, 0}); progress = true; }
-                for (int cc = c - 1; cc <= c; ++cc) {
-                    if (cc < 0 || cc + 1 >= L_) continue;
-                    if (grow_[cc] == grow_[cc + 1] && grow_[cc] - 1 == r && !dj_[r * (L_ - 1) + cc]) {
-                        dj_[r * (L_ - 1) + cc] = 1;
-                        ops.push_back({OP_DJ, 0, (uint8_t)cc, 0, (uint16_t)r, 0});
-                        progress = true;
-                    }
-                }
-            }
-            for (int c = 0; c < L_; ++c) {
-                if (!in_tile(c)) continue;
-                int r = grow_[c];                           // next gate row on digit c
+                const int r = grow_[c];
                 if (r >= L_ || r > max_row) continue;
-                bool ok = dh_[(r - 1) * L_ + c] != 0;
-                if (c > 0) ok = ok && dj_[(r - 1) * (L_ - 1) + c - 1];
-                if (c + 1 < L_) ok = ok && dj_[(r - 1) * (L_ - 1) + c];
-                if (!ok) continue;
-                grow_[c] += 1;
-                ops.push_back({OP_GATE, (uint8_t)pos_of(c), (uint8_t)c, 0, (uint16_t)r, 0});
-                ++gates; progress = true;
+                if (c > 0 && grow_[c - 1] < r) continue;
+                if (c + 1 < L_ && grow_[c + 1] < r) continue;
+                legal.push_back(c);
             }
+            if (legal.empty()) break;
+            for (int c : legal) {
+                ops.push_back({OP_GATE, (uint8_t)pos_of(c), (uint8_t)c, 0, (uint16_t)grow_[c], 0});
+                ++gates;
+            }
+            for (int c : legal) grow_[c] += 1;
         }
         return gates;
     }
   private:
-    int L_; bool has_field_;
+    int L_;
     std::vector<int> grow_;            // grow[c] = rows complete on digit c (row 0 needs no gate)
-    std::vector<uint8_t> dh_, dj_;
 };
 
 // Tile cycle: first tile [0, w0) (contiguous), then high tiles of `wh` active digits with
@@ -147,7 +131,7 @@ inline Plan make_plan(int q, int L, bool has_field, bool row_aligned, int Tmax, 
     for (int stride = s_lo; stride <= s_hi; ++stride) {
         std::vector<TileSpec> cyc = tile_cycle(L, Tmax, ride, stride);
         Plan p; p.q = q; p.L = L; p.row_aligned = row_aligned;
-        Scheduler s(L, has_field);
+        Scheduler s(L);
         size_t k = 0; int row = 0; bool first = true; int idle = 0;
         int cur_src = -1;
         while (first || !s.done()) {   // the INIT pass exists even when there is nothing to apply

@@ -70,7 +70,7 @@ bool limits_ok(int q, int L, bool count, bool config) {
 struct Layout {
     size_t x = 0, n = 0, ckpt = 0, Jh = 0, Jv = 0, h = 0, ops = 0, part_x = 0, part_n = 0,
            amax_v = 0, amax_s = 0, out_x = 0, out_n = 0, out_s = 0, sigma = 0, total = 0;
-    size_t f_mops = 0, f_gate_rc = 0, f_gate_k = 0, f_final = 0;
+    size_t f_mops = 0, f_gate_rc = 0, f_gate_k = 0, f_final = 0, g_gate_k = 0, g_fin = 0;
     unsigned long long NS = 0, max_tiles = 0;
     int amax_blocks = 0;
     int f_max_gates = 0, f_max_mops = 0;
@@ -99,7 +99,9 @@ Layout make_layout(int q, int L, bool count, bool config, int batch) {
     y.Jh = take((size_t)batch * L * (L - 1) * 4 + 4);
     y.Jv = take((size_t)batch * (L - 1) * L * 4 + 4);
     y.h = take((size_t)batch * L * L * 4);
-    y.ops = take((size_t)(3 * L * L + 8) * sizeof(ttn::Op));
+    y.ops = take((size_t)(L * L + 8) * sizeof(ttn::Op));
+    y.g_gate_k = take((size_t)batch * (L * L + 8) * 8 * 4);
+    y.g_fin = take((size_t)batch * 2 * ttn::GMAX_L * 4);
     y.part_x = take((size_t)batch * y.max_tiles * 4);
     y.part_n = take((size_t)batch * y.max_tiles * 8);
     unsigned long long nb = (y.NS + 256ull * 16 - 1) / (256ull * 16);
@@ -169,9 +171,9 @@ static ttn_status launch_pass(const ttn_plan* P, const ttn::Pass& ps, cudaStream
     pp.src_n = pp.dst_n = COUNT ? reinterpret_cast<double*>(P->ws + y.n) : nullptr;
     pp.ops = reinterpret_cast<const ttn::Op*>(P->ws + y.ops) + ps.op_begin;
     pp.n_ops = ps.op_end - ps.op_begin;
-    pp.Jh = reinterpret_cast<const float*>(P->ws + y.Jh);
-    pp.Jv = reinterpret_cast<const float*>(P->ws + y.Jv);
-    pp.h = P->has_field ? reinterpret_cast<const float*>(P->ws + y.h) : nullptr;
+    pp.gate_k = reinterpret_cast<const float*>(P->ws + y.g_gate_k) + (size_t)ps.op_begin * 8;
+    pp.gate_inst_stride = (unsigned long long)P->plan.ops.size() * 8;
+    pp.fin = reinterpret_cast<const float*>(P->ws + y.g_fin);
     pp.flags = ps.flags;
     pp.part_x = reinterpret_cast<float*>(P->ws + y.part_x);
     pp.part_n = reinterpret_cast<double*>(P->ws + y.part_n);
@@ -332,7 +334,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     }
     if (!P->fused) P->plan = plan_for(q, L, call, P->has_field);
     if (!P->fused && P->plan.passes.empty()) { delete P; return fail(TTN_EUNSUPPORTED, "planner produced no schedule"); }
-    if (P->plan.ops.size() > (size_t)(3 * L * L + 8)) { delete P; return fail(TTN_EUNSUPPORTED, "op list too long"); }
+    if (P->plan.ops.size() > (size_t)(L * L + 8)) { delete P; return fail(TTN_EUNSUPPORTED, "op list too long"); }
 
     // the +J constants factored out of the Ising gates (kernel comment at OP_GATE), in f64
     P->defer.assign(batch, 0.0);
@@ -359,6 +361,18 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
         if (fs != TTN_OK) { delete P; return fs; }
         P->launches = (int)P->fplan.passes.size() + 1;
     } else {
+        ttn::GenericPrepParams gp{};
+        gp.q = q; gp.L = L; gp.n_ops = (int)P->plan.ops.size();
+        gp.ops = reinterpret_cast<const ttn::Op*>(P->ws + lay.ops);
+        gp.Jh = reinterpret_cast<const float*>(P->ws + lay.Jh);
+        gp.Jv = reinterpret_cast<const float*>(P->ws + lay.Jv);
+        gp.h = P->has_field ? reinterpret_cast<const float*>(P->ws + lay.h) : nullptr;
+        gp.gate_k = reinterpret_cast<float*>(P->ws + lay.g_gate_k);
+        gp.fin = reinterpret_cast<float*>(P->ws + lay.g_fin);
+        long work = 2 * ttn::GMAX_L; if (gp.n_ops > work) work = gp.n_ops;
+        ttn::generic_prep_kernel<<<dim3((unsigned)((work + 255) / 256), (unsigned)batch), 256, 0, st>>>(gp);
+        cudaError_t pe = cudaGetLastError();
+        if (pe != cudaSuccess) { delete P; return fail(TTN_ECUDA, "prep launch failed: %s", cudaGetErrorString(pe)); }
         P->launches = (int)P->plan.passes.size() + (config ? 2 * L : 1);
     }
     *out = P;
@@ -402,6 +416,8 @@ ttn_status ttn_plan_launch(ttn_plan* P, void* stream) {
         ap.L = P->L; ap.NS = y.NS; ap.nblk = y.amax_blocks;
         ap.c_stride = (unsigned long long)P->L * y.NS;
         ap.Jv = reinterpret_cast<const float*>(P->ws + y.Jv);
+        ap.Jh = reinterpret_cast<const float*>(P->ws + y.Jh);
+        ap.h = P->has_field ? reinterpret_cast<const float*>(P->ws + y.h) : nullptr;
         ap.s_next = ap.s_out = reinterpret_cast<unsigned long long*>(P->ws + y.out_s);
         ap.part_v = reinterpret_cast<float*>(P->ws + y.amax_v);
         ap.part_s = reinterpret_cast<unsigned long long*>(P->ws + y.amax_s);

@@ -1,12 +1,23 @@
-// ttn_kernels.cuh -- device side of the tropical transfer sweep, generic ("v1") path.
+// ttn_kernels.cuh -- device side of the tropical transfer sweep, generic tile path: every
+// semiring (Tropical<f32>, CountingTropical<f32,f64>), q = 2 (Ising) and q = 3 (Potts), and
+// the checkpointed ground-configuration call.
 //
 // One launch of pass_kernel = one HBM pass over the q^L state: each
-// CTA stages one tile (digits [0,lo) U [a,b) of the state index) in shared memory, runs the
-// pass's op list on it -- max-plus gates (A2) PAPER.md:242 / the 3x3 Potts gate of App. C
-// PAPER.md:296 as butterflies over the gate's digit, diagonal terms (A3), (A4)
-// PAPER.md:247-252 as elementwise adds -- and writes it back in place ("all
-// operations should be performed inplace").  The first pass is write-only (initial state
-// (0,0)^{(x)L}), the last is read-only and fuses the final (+)-reduction.
+// CTA stages one tile (digits [0,lo) U [a,b) of the state index) in shared memory, applies the
+// pass's gate list as butterflies over the gate's digit, and writes the tile back in place
+// ("all operations should be performed inplace").  The first pass is write-only
+// (initial state (0,0)^{(x)L}), the last is read-only and fuses the final
+// (+)-reduction.
+//
+// DIAGONAL FRAME (planner.h): the sweep runs on V'' with V = A_r V'', A_r the accumulated row
+// diagonals (A3), (A4) PAPER.md:247-252, so no diagonal is ever applied to the state; each gate
+// (A2) PAPER.md:242 / the 3x3 Potts gate of App. C PAPER.md:296 is conjugated with A_{r-1}:
+//   Ising:  a' = a (+) (b (.) ka[nl][nr]),  b' = b (+) (a (.) kb[nl][nr])          (8 constants)
+//   Potts:  y[t] = x[t] (.) R(t),  new[t'] = ( (+)_t y[t] (.) Jv delta(t,t') ) (.) (-R(t')),
+//           R(t) = Kl delta(t_{c-1}, t) + Kr delta(t, t_{c+1})                      (3 constants)
+// with nl, nr / t_{c-1}, t_{c+1} the neighbour digits of the element's own index.  The last
+// pass multiplies by A_{L-1}(s) before the reduction; the configuration call keeps V'' in its
+// checkpoints and the backward pass adds A_r(s).
 //
 // Semirings: Tropical<f32>: x (+) y = max, x (.) y = x + y (Eq. (2)
 // PAPER.md:57); CountingTropical<f32,f64>: Eq. (4), counts summed on exact ties.
@@ -17,6 +28,8 @@
 
 namespace ttn {
 
+constexpr int GMAX_L = 64;          // digits (columns) supported by the generic kernels' tables
+
 struct PassParams {
     int L, T, lo, a, b;
     unsigned long long P_lo, P_a, P_mid, P_b;   // q^lo, q^a, q^(a-lo), q^b
@@ -25,26 +38,15 @@ struct PassParams {
     const float* src_x; float* dst_x;             // instance 0 base pointers
     const double* src_n; double* dst_n;           // counting only
     unsigned long long src_stride, dst_stride;    // elements between instances
-    const Op* ops; int n_ops;
-    const float* Jh; const float* Jv; const float* h;   // device, per instance; h may be null
+    const Op* ops; int n_ops;                     // this pass's gates
+    const float* gate_k;                          // [inst][all gates][8]; this pass's slice of instance 0
+    unsigned long long gate_inst_stride;          // floats between instances
+    const float* fin;                             // [inst][2 * GMAX_L]: H_c, K_c of A_{L-1} (REDUCE pass)
     int flags;
     float* part_x; double* part_n;                // [inst][tile] partial reductions
 };
 
 // ---------------------------------------------------------------------------------------------
-template <int Q> struct Radix;
-template <> struct Radix<2> {
-    __device__ static __forceinline__ unsigned digit(unsigned long long s, int c) { return (unsigned)(s >> c) & 1u; }
-};
-template <> struct Radix<3> {
-    __device__ static __forceinline__ unsigned digit(unsigned long long s, int c) {
-        const unsigned p3[21] = {1u, 3u, 9u, 27u, 81u, 243u, 729u, 2187u, 6561u, 19683u, 59049u, 177147u,
-                                 531441u, 1594323u, 4782969u, 14348907u, 43046721u, 129140163u,
-                                 387420489u, 1162261467u, 3486784401u};
-        return ((unsigned)s / p3[c]) % 3u;       // Potts index fits 32 bits (L <= 20)
-    }
-};
-
 __device__ __forceinline__ float warp_max(float v) {
     for (int o = 16; o; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
     return v;
@@ -65,11 +67,27 @@ __device__ __forceinline__ void oplus(float& x, double& n, float cx, double cn) 
     }
 }
 
+// exact n / d for n * d < 2^32 with the host-side magic M = floor(2^32 / d) + 1
+__device__ __forceinline__ unsigned fastdiv(unsigned n, unsigned magic) { return __umulhi(n, magic); }
+__host__ __device__ inline unsigned fastdiv_magic(unsigned d) { return d <= 1 ? 0u : (unsigned)(0x100000000ull / d) + 1u; }
+
+// column held by tile position p
+__device__ __forceinline__ int tile_col(const PassParams& p, int pos) { return pos < p.lo ? pos : p.a + (pos - p.lo); }
+
+// weight of the accumulated diagonal A(s) = sum_c H_c f1(d_c) + sum_c K_c f2(d_c, d_{c+1})
+template <int Q> __device__ __forceinline__ float diag1(float H, int d) { return Q == 2 ? (d ? -H : H) : 0.f; }
+template <int Q> __device__ __forceinline__ float diag2(float K, int d0, int d1) {
+    return Q == 2 ? (d0 == d1 ? K : -K) : (d0 == d1 ? K : 0.f);
+}
+
 template <int Q, bool COUNT>
 __global__ void __launch_bounds__(512) pass_kernel(const PassParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double* sn = reinterpret_cast<double*>(smem_raw);                       // [n_tile] if COUNT
     float* sx = reinterpret_cast<float*>(smem_raw + (COUNT ? (size_t)p.n_tile * 8 : 0));
+    __shared__ int s_dig[GMAX_L];            // digits of this tile's base index (columns outside the tile)
+    __shared__ float s_fin[2 * GMAX_L];      // H_c, K_c of A_{L-1} (REDUCE pass)
+    __shared__ float s_aout;                 // part of A_{L-1} that only involves columns outside the tile
     const unsigned N = p.n_tile;
     const unsigned long long gtile = blockIdx.x;
     const unsigned long long inst = gtile / p.tiles_per_inst;
@@ -89,87 +107,118 @@ __global__ void __launch_bounds__(512) pass_kernel(const PassParams p) {
             if (COUNT) sn[t] = gn[off];
         }
     }
+    for (int i = threadIdx.x; i < p.L; i += blockDim.x) {   // digit c of the base index (0 for the tile's own columns)
+        unsigned long long s = base;
+        for (int c = 0; c < i; ++c) s /= Q;
+        s_dig[i] = (int)(s % Q);
+    }
+    if (p.flags & PASS_REDUCE)
+        for (int i = threadIdx.x; i < 2 * GMAX_L; i += blockDim.x) s_fin[i] = p.fin[inst * (2 * GMAX_L) + i];
     __syncthreads();
 
-    const float* Jh = p.Jh + inst * (unsigned long long)(p.L * (p.L - 1));
-    const float* Jv = p.Jv + inst * (unsigned long long)((p.L - 1) * p.L);
-    const float* hh = p.h ? p.h + inst * (unsigned long long)(p.L * p.L) : nullptr;
-
-    // ---- op list ------------------------------------------------------------------------------
+    // ---- gate list -------------------------------------------------------------------------------
+    const float* GK = p.gate_k + inst * p.gate_inst_stride;
     for (int k = 0; k < p.n_ops; ++k) {
         const Op op = p.ops[k];
-        if (op.type == OP_GATE) {
-            const float J = Jv[(op.row - 1) * p.L + op.c];
-            // stride of the gate's digit inside the tile
-            unsigned st = 1;
-            for (int i = 0; i < op.pos; ++i) st *= Q;
-            const unsigned ngrp = N / Q;
-            for (unsigned g = threadIdx.x; g < ngrp; g += blockDim.x) {
-                unsigned i0 = (g / st) * (st * Q) + (g % st);
-                if (Q == 2) {
-                    // (A2): new[b'] = max_b(old[b] + J s(b) s(b')) = J + max(old[b'], old[1-b'] - 2J);
-                    // the common +J is deferred to a per-instance scalar (see api: defer).
-                    const float m = -2.f * J;
-                    float xa = sx[i0], xb = sx[i0 + st];
-                    float ca = xb + m, cb = xa + m;
-                    if (COUNT) {
-                        double na = sn[i0], nb = sn[i0 + st];
-                        float ya = xa; double ma = na; oplus<true>(ya, ma, ca, nb);
-                        float yb = xb; double mb = nb; oplus<true>(yb, mb, cb, na);
-                        sx[i0] = ya; sx[i0 + st] = yb; sn[i0] = ma; sn[i0 + st] = mb;
-                    } else {
-                        sx[i0] = fmaxf(xa, ca); sx[i0 + st] = fmaxf(xb, cb);
+        const int pos = op.pos, c = op.c;
+        unsigned st = 1;
+        for (int i = 0; i < pos; ++i) st *= Q;
+        const unsigned st_q = pos > 0 ? st / Q : 1;             // weight of the digit at position pos-1
+        const unsigned m_st = fastdiv_magic(st), m_stq = fastdiv_magic(st_q);
+        // neighbour columns: inside the tile (digit taken from the tile-local index) or outside (s_dig)
+        const bool l_in = pos > 0 && tile_col(p, pos - 1) == c - 1;
+        const bool r_in = pos + 1 < p.T && tile_col(p, pos + 1) == c + 1;
+        const int dl_out = c > 0 ? s_dig[c - 1] : 0, dr_out = c + 1 < p.L ? s_dig[c + 1] : 0;
+        const float4 k0 = reinterpret_cast<const float4*>(GK)[2 * k], k1 = reinterpret_cast<const float4*>(GK)[2 * k + 1];
+        const unsigned ngrp = N / Q;
+        for (unsigned g = threadIdx.x; g < ngrp; g += blockDim.x) {
+            const unsigned hi = st == 1 ? g : fastdiv(g, m_st), lo = g - hi * st;
+            const unsigned i0 = hi * (st * Q) + lo;
+            const int dl = l_in ? (int)(st_q == 1 ? lo : fastdiv(lo, m_stq)) : dl_out;   // top digit of lo
+            const int dr = r_in ? (int)(hi % Q) : dr_out;
+            if (Q == 2) {
+                // conjugated (A2): a' = a (+) (b + ka[dl][dr]),  b' = b (+) (a + kb[dl][dr])
+                const int n = dl * 2 + dr;
+                const float ka = n == 0 ? k0.x : (n == 1 ? k0.y : (n == 2 ? k0.z : k0.w));
+                const float kb = n == 0 ? k1.x : (n == 1 ? k1.y : (n == 2 ? k1.z : k1.w));
+                float xa = sx[i0], xb = sx[i0 + st];
+                const float ca = xb + ka, cb = xa + kb;
+                if (COUNT) {
+                    const double na = sn[i0], nb = sn[i0 + st];
+                    float ya = xa; double ma = na; oplus<true>(ya, ma, ca, nb);
+                    float yb = xb; double mb = nb; oplus<true>(yb, mb, cb, na);
+                    sx[i0] = ya; sx[i0 + st] = yb; sn[i0] = ma; sn[i0 + st] = mb;
+                } else {
+                    sx[i0] = fmaxf(xa, ca); sx[i0 + st] = fmaxf(xb, cb);
+                }
+            } else {
+                // conjugated Potts gate: k0 = (Jv, Kl, Kr, -)
+                const float J = k0.x, Kl = k0.y, Kr = k0.z;
+                float R[3], x[3];
+#pragma unroll
+                for (int t = 0; t < 3; ++t) {
+                    R[t] = (t == dl ? Kl : 0.f) + (t == dr ? Kr : 0.f);
+                    x[t] = sx[i0 + t * st] + R[t];
+                }
+                if (COUNT) {
+                    double n[3];
+#pragma unroll
+                    for (int t = 0; t < 3; ++t) n[t] = sn[i0 + t * st];
+#pragma unroll
+                    for (int tn = 0; tn < 3; ++tn) {
+                        float y = x[tn] + J; double m = n[tn];
+#pragma unroll
+                        for (int t = 0; t < 3; ++t) if (t != tn) oplus<true>(y, m, x[t], n[t]);
+                        sx[i0 + tn * st] = y - R[tn]; sn[i0 + tn * st] = m;
                     }
                 } else {
-                    // Potts: new[t'] = max_t(old[t] + J delta(t,t'))
-                    float x0 = sx[i0], x1 = sx[i0 + st], x2 = sx[i0 + 2 * st];
-                    if (COUNT) {
-                        double n0 = sn[i0], n1 = sn[i0 + st], n2 = sn[i0 + 2 * st];
-                        float y0 = x0 + J; double m0 = n0; oplus<true>(y0, m0, x1, n1); oplus<true>(y0, m0, x2, n2);
-                        float y1 = x1 + J; double m1 = n1; oplus<true>(y1, m1, x0, n0); oplus<true>(y1, m1, x2, n2);
-                        float y2 = x2 + J; double m2 = n2; oplus<true>(y2, m2, x0, n0); oplus<true>(y2, m2, x1, n1);
-                        sx[i0] = y0; sx[i0 + st] = y1; sx[i0 + 2 * st] = y2;
-                        sn[i0] = m0; sn[i0 + st] = m1; sn[i0 + 2 * st] = m2;
-                    } else {
-                        sx[i0] = fmaxf(x0 + J, fmaxf(x1, x2));
-                        sx[i0 + st] = fmaxf(x1 + J, fmaxf(x0, x2));
-                        sx[i0 + 2 * st] = fmaxf(x2 + J, fmaxf(x0, x1));
-                    }
+                    sx[i0] = fmaxf(x[0] + J, fmaxf(x[1], x[2])) - R[0];
+                    sx[i0 + st] = fmaxf(x[1] + J, fmaxf(x[0], x[2])) - R[1];
+                    sx[i0 + 2 * st] = fmaxf(x[2] + J, fmaxf(x[0], x[1])) - R[2];
                 }
             }
-            __syncthreads();
-        } else {
-            // a run of diagonal terms: one sweep over the tile applies them all, in list order
-            int k2 = k;
-            while (k2 + 1 < p.n_ops && p.ops[k2 + 1].type != OP_GATE) ++k2;
-            for (unsigned t = threadIdx.x; t < N; t += blockDim.x) {
-                unsigned long long s = base + (unsigned long long)(t % plo) + (unsigned long long)(t / plo) * p.P_a;
-                float v = sx[t];
-                for (int j = k; j <= k2; ++j) {
-                    const Op o = p.ops[j];
-                    if (o.type == OP_DH) {
-                        if (Q == 2 && hh) {
-                            float hv = hh[o.row * p.L + o.c];
-                            v += Radix<Q>::digit(s, o.c) ? -hv : hv;
-                        }
-                    } else {
-                        float Jc = Jh[o.row * (p.L - 1) + o.c];
-                        unsigned d0 = Radix<Q>::digit(s, o.c), d1 = Radix<Q>::digit(s, o.c + 1);
-                        if (Q == 2) v += (d0 == d1) ? Jc : -Jc;
-                        else v += (d0 == d1) ? Jc : 0.f;
-                    }
-                }
-                sx[t] = v;
-            }
-            k = k2;
-            __syncthreads();
         }
+        __syncthreads();
     }
 
-    // ---- store, or reduce ------------------------------------------------------------------
+    // ---- store, or multiply by A_{L-1}(s) and reduce ----------------------------------------------
     if (p.flags & PASS_REDUCE) {
+        const float* H = s_fin; const float* K = s_fin + GMAX_L;
+        if (threadIdx.x == 0) {              // terms whose columns all lie outside the tile
+            float acc = 0.f;
+            for (int c = 0; c < p.L; ++c) {
+                const bool in_c = c < p.lo || (c >= p.a && c < p.b);
+                if (!in_c) acc += diag1<Q>(H[c], s_dig[c]);
+                if (c + 1 < p.L) {
+                    const bool in_n = c + 1 < p.lo || (c + 1 >= p.a && c + 1 < p.b);
+                    if (!in_c && !in_n) acc += diag2<Q>(K[c], s_dig[c], s_dig[c + 1]);
+                }
+            }
+            s_aout = acc;
+        }
+        __syncthreads();
         float mx = -INFINITY;
-        for (unsigned t = threadIdx.x; t < N; t += blockDim.x) mx = fmaxf(mx, sx[t]);
+        for (unsigned t = threadIdx.x; t < N; t += blockDim.x) {
+            // walk the tile-local digits of t: position pos holds column tile_col(pos)
+            float acc = s_aout;
+            unsigned rest = t;
+            int dprev = 0, cprev = -2;
+            for (int pos = 0; pos < p.T; ++pos) {
+                const int d = (int)(rest % Q); rest /= Q;
+                const int c = tile_col(p, pos);
+                acc += diag1<Q>(H[c], d);
+                if (c > 0) {
+                    if (cprev == c - 1) acc += diag2<Q>(K[c - 1], dprev, d);           // left neighbour in the tile
+                    else acc += diag2<Q>(K[c - 1], s_dig[c - 1], d);                   // left neighbour outside
+                }
+                const bool right_in = pos + 1 < p.T && tile_col(p, pos + 1) == c + 1;
+                if (c + 1 < p.L && !right_in) acc += diag2<Q>(K[c], d, s_dig[c + 1]);  // right neighbour outside
+                dprev = d; cprev = c;
+            }
+            const float val = sx[t] + acc;
+            sx[t] = val;
+            mx = fmaxf(mx, val);
+        }
         __shared__ float red_x[16];
         __shared__ double red_n[16];
         mx = warp_max(mx);
@@ -235,14 +284,16 @@ __global__ void __launch_bounds__(256) final_reduce_kernel(const float* part_x, 
 
 // ---------------------------------------------------------------------------------------------
 // Backtrace ("caching intermediate contraction results and
-// backtracking"): s_{L-1} = argmax_s C_{L-1}[s];  s_r = argmax_s ( C_r[s] + sum_c Jv[r][c]
-// sigma_c(s) sigma_c(s_{r+1}) ).  Lowest index wins ties (footnote [49] PAPER.md:201).
+// backtracking").  The checkpoints hold V''_r (diagonal frame), V_r = A_r V''_r, so
+//   s_{L-1} = argmax_s ( C_{L-1}[s] + A_{L-1}(s) ),
+//   s_r     = argmax_s ( C_r[s] + A_r(s) + sum_c Jv[r][c] sigma_c(s) sigma_c(s_{r+1}) ).
+// Lowest index wins ties (footnote [49] PAPER.md:201).
 struct ArgmaxParams {
     int L, r, has_next, nblk;
     unsigned long long NS;
     const float* C;                     // checkpoint C_r of instance 0
     unsigned long long c_stride;        // elements between instances
-    const float* Jv;                    // device couplings (per instance)
+    const float* Jh; const float* Jv; const float* h;   // device couplings (per instance); h may be null
     const unsigned long long* s_next;   // [batch] state of row r+1 (if has_next)
     float* part_v; unsigned long long* part_s;   // [batch][nblk]
     unsigned long long* s_out;          // [batch]
@@ -256,14 +307,22 @@ __device__ __forceinline__ void argmax_combine(float& v, unsigned long long& s, 
 
 __global__ void __launch_bounds__(256) argmax_partial_kernel(const ArgmaxParams p) {
     const unsigned long long inst = blockIdx.y;
-    __shared__ float jsig[64];
+    __shared__ float jsig[GMAX_L];      // coefficient of sigma_c: Jv sigma'_c + H_c (accumulated through row r)
+    __shared__ float kacc[GMAX_L];      // coefficient of sigma_c sigma_{c+1}
     if (threadIdx.x < p.L) {
-        float j = 0.f;
-        if (p.has_next) {
-            j = p.Jv[inst * (unsigned long long)((p.L - 1) * p.L) + p.r * p.L + threadIdx.x];
-            if ((p.s_next[inst] >> threadIdx.x) & 1ull) j = -j;
+        const int c = threadIdx.x, L = p.L;
+        double hs = 0.0, ks = 0.0;
+        for (int rr = 0; rr <= p.r; ++rr) {
+            if (p.h) hs += (double)p.h[inst * (unsigned long long)(L * L) + rr * L + c];
+            if (c + 1 < L) ks += (double)p.Jh[inst * (unsigned long long)(L * (L - 1)) + rr * (L - 1) + c];
         }
-        jsig[threadIdx.x] = j;
+        double j = 0.0;
+        if (p.has_next) {
+            j = (double)p.Jv[inst * (unsigned long long)((L - 1) * L) + p.r * L + c];
+            if ((p.s_next[inst] >> c) & 1ull) j = -j;
+        }
+        jsig[c] = (float)(j + hs);
+        kacc[c] = (float)ks;
     }
     __syncthreads();
     const float* C = p.C + inst * p.c_stride;
@@ -271,8 +330,11 @@ __global__ void __launch_bounds__(256) argmax_partial_kernel(const ArgmaxParams 
     for (unsigned long long s = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; s < p.NS;
          s += (unsigned long long)gridDim.x * blockDim.x) {
         float w = 0.f;
-        if (p.has_next)
-            for (int c = 0; c < p.L; ++c) w += ((s >> c) & 1ull) ? -jsig[c] : jsig[c];
+        const unsigned long long x = s ^ (s >> 1);            // bit c set <=> sigma_c != sigma_{c+1}
+        for (int c = 0; c < p.L; ++c) {
+            w += ((s >> c) & 1ull) ? -jsig[c] : jsig[c];
+            if (c + 1 < p.L) w += ((x >> c) & 1ull) ? -kacc[c] : kacc[c];
+        }
         argmax_combine(bv, bs, C[s] + w, s);
     }
     for (int o = 16; o; o >>= 1) {
@@ -303,6 +365,50 @@ __global__ void __launch_bounds__(32) argmax_final_kernel(const ArgmaxParams p) 
     if (threadIdx.x == 0) { p.s_out[inst] = bs; if (!p.has_next) p.v_out[inst] = bv; }
     if (threadIdx.x < p.L)
         p.sigma[(inst * p.L + p.r) * p.L + threadIdx.x] = ((bs >> threadIdx.x) & 1ull) ? -1 : 1;
+}
+
+// ---- S0 of the generic path: conjugated gate constants and the coefficients of A_{L-1} -------------
+struct GenericPrepParams {
+    int q, L, n_ops;
+    const Op* ops;                 // [n_ops] gates in execution order
+    const float* Jh; const float* Jv; const float* h;   // device couplings, per instance
+    float* gate_k;                 // [inst][n_ops][8]
+    float* fin;                    // [inst][2 * GMAX_L]
+};
+
+__global__ void __launch_bounds__(256) generic_prep_kernel(const GenericPrepParams p) {
+    const unsigned long long inst = blockIdx.y;
+    const int L = p.L;
+    const float* Jh = p.Jh + inst * (unsigned long long)(L * (L - 1));
+    const float* Jv = p.Jv + inst * (unsigned long long)((L - 1) * L);
+    const float* hh = p.h ? p.h + inst * (unsigned long long)(L * L) : nullptr;
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    auto Hacc = [&](int R, int c) { double s = 0; if (hh) for (int r = 0; r < R; ++r) s += (double)hh[r * L + c]; return s; };
+    auto Kacc = [&](int R, int c) { double s = 0; if (c < 0 || c >= L - 1) return s; for (int r = 0; r < R; ++r) s += (double)Jh[r * (L - 1) + c]; return s; };
+    if (idx < p.n_ops) {
+        const Op op = p.ops[idx];
+        const int r = op.row, c = op.c;
+        float* out = p.gate_k + (inst * p.n_ops + idx) * 8;
+        const double J = (double)Jv[(r - 1) * L + c], Kl = Kacc(r, c - 1), Kr = Kacc(r, c);
+        if (p.q == 2) {
+            const double m = -2.0 * J, H = Hacc(r, c);
+            for (int nl = 0; nl < 2; ++nl)
+                for (int nr = 0; nr < 2; ++nr) {
+                    const double rho = H + (nl ? -Kl : Kl) + (nr ? -Kr : Kr);
+                    out[nl * 2 + nr] = (float)(m - 2.0 * rho);          // ka
+                    out[4 + nl * 2 + nr] = (float)(m + 2.0 * rho);      // kb
+                }
+        } else {
+            out[0] = (float)J; out[1] = (float)Kl; out[2] = (float)Kr;
+            for (int i = 3; i < 8; ++i) out[i] = 0.f;
+        }
+    }
+    if (idx < 2 * GMAX_L) {
+        float* out = p.fin + inst * (2 * GMAX_L);
+        const int c = (int)(idx % GMAX_L);
+        if (idx < GMAX_L) out[idx] = c < L ? (float)Hacc(L, c) : 0.f;
+        else out[idx] = c < L - 1 ? (float)Kacc(L, c) : 0.f;
+    }
 }
 
 }  // namespace ttn

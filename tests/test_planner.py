@@ -50,11 +50,8 @@ def parse(txt):
 
 
 def validate(q, L, passes, fields, row_aligned):
+    """Diagonal frame: only gates are scheduled; g(r,c) needs g(r-1,c-1), g(r-1,c), g(r-1,c+1)."""
     g = np.zeros((L, L), dtype=int); g[0, :] = 1          # row 0 needs no gate
-    dh = np.zeros((L, L), dtype=int)
-    dJ = np.zeros((L, max(L - 1, 0)), dtype=int)
-    if not fields:
-        dh[:] = 1
     rows_done = 0
     for i, ps in enumerate(passes):
         lo, a, b = ps["lo"], ps["a"], ps["b"]
@@ -64,31 +61,24 @@ def validate(q, L, passes, fields, row_aligned):
         assert (ps["flags"] & 1) == (1 if i == 0 else 0)          # INIT only on the first pass
         for op in ps["ops"]:
             r, c = op["r"], op["c"]
-            if op["type"] == "g":
-                assert c in tile and tile.index(c) == op["pos"]
-                assert 1 <= r < L and g[r, c] == 0 and g[r - 1, c] == 1
-                assert dh[r - 1, c] == 1
-                if c > 0: assert dJ[r - 1, c - 1] == 1
-                if c < L - 1: assert dJ[r - 1, c] == 1
-                g[r, c] = 1
-            elif op["type"] == "dh":
-                assert fields and dh[r, c] == 0 and g[r, c] == 1
-                assert r == L - 1 or g[r + 1, c] == 0
-                dh[r, c] = 1
-            else:
-                assert dJ[r, c] == 0 and g[r, c] == 1 and g[r, c + 1] == 1
-                assert r == L - 1 or (g[r + 1, c] == 0 and g[r + 1, c + 1] == 0)
-                dJ[r, c] = 1
+            assert op["type"] == "g"                               # no diagonal op is ever scheduled
+            assert c in tile and tile.index(c) == op["pos"]
+            assert 1 <= r < L and g[r, c] == 0 and g[r - 1, c] == 1
+            if c > 0: assert g[r - 1, c - 1] == 1
+            if c < L - 1: assert g[r - 1, c + 1] == 1
+            # the neighbours may be at most one row ahead (same-row gates commute)
+            if c > 0 and r + 1 < L: assert g[r + 1, c - 1] == 0
+            if c < L - 1 and r + 1 < L: assert g[r + 1, c + 1] == 0
+            g[r, c] = 1
         if row_aligned:
-            full = lambda r: g[r].all() and dh[r].all() and dJ[r].all()
-            if rows_done < L and full(rows_done):
+            if rows_done < L and g[rows_done].all():
                 assert ps["dst"] == rows_done
                 rows_done += 1
             else:
                 assert ps["dst"] == -1
             if i > 0:
                 assert ps["src"] == passes[i - 1]["dst"]
-    assert g.all() and dh.all() and dJ.all()
+    assert g.all()
     if row_aligned:
         assert rows_done == L
     else:
@@ -255,40 +245,59 @@ def digits(q, L):
 
 
 def replay(q, L, passes, Jh, Jv, h):
-    """Apply the op list to the full state in numpy: x float64, n Python-int (object) counts."""
+    """Apply the gate list to the full state in numpy in the diagonal frame, restated here from
+    the paper's gates: x float64, n Python-int (object) counts.  With A_{r-1}(s) the sum of all
+    diagonal gates (A3), (A4) of rows < r, gate g(r,c) is  G'' = A^-1 G A:
+        cand(t -> t') = x[t] + w(t,t') + R(t) - R(t'),   R(t) = the terms of A_{r-1} that contain digit c
+    and the result is  (+)_s ( x[s] (.) A_{L-1}(s) )."""
     N = q ** L
     x = np.zeros(N); n = np.ones(N, dtype=object)
     dig = digits(q, L)
     idx = np.arange(N)
-    defer = 0.0
+    H = np.cumsum(h, axis=0) if h is not None else np.zeros((L, L))
+    K = np.cumsum(Jh, axis=0)
+
+    def two(Kc, d0, d1):
+        return Kc * (1 - 2 * d0) * (1 - 2 * d1) if q == 2 else Kc * (d0 == d1)
+
+    def R_of(r, c, t, sel):
+        out = np.zeros(sel.size)
+        if q == 2:
+            out = out + H[r - 1, c] * (1 - 2 * t)
+        if c > 0:
+            out = out + two(K[r - 1, c - 1], dig[c - 1][sel], t)
+        if c < L - 1:
+            out = out + two(K[r - 1, c], t, dig[c + 1][sel])
+        return out
+
     for ps in passes:
         for op in ps["ops"]:
+            assert op["type"] == "g"
             r, c = op["r"], op["c"]
-            if op["type"] == "dh":
-                if h is not None:
-                    x += h[r, c] * (1 - 2 * dig[c])
-            elif op["type"] == "dJ":
-                if q == 2:
-                    x += Jh[r, c] * (1 - 2 * dig[c]) * (1 - 2 * dig[c + 1])
-                else:
-                    x += Jh[r, c] * (dig[c] == dig[c + 1])
-            else:
-                J = Jv[r - 1, c]
-                st = q ** c
-                base = idx[dig[c] == 0]
-                olds = [(x[base + t * st].copy(), n[base + t * st].copy()) for t in range(q)]
-                for tn in range(q):
-                    bx = None
-                    for t in range(q):
-                        w = J * (1 - 2 * t) * (1 - 2 * tn) if q == 2 else J * (t == tn)
-                        cx, cn = olds[t][0] + w, olds[t][1]
-                        if bx is None:
-                            bx, bn = cx.copy(), cn.copy()
-                        else:
-                            gt, eq = cx > bx, cx == bx
-                            bn = np.where(gt, cn, np.where(eq, bn + cn, bn))
-                            bx = np.maximum(bx, cx)
-                    x[base + tn * st] = bx; n[base + tn * st] = bn
+            J = Jv[r - 1, c]
+            st = q ** c
+            base = idx[dig[c] == 0]
+            olds = [(x[base + t * st].copy(), n[base + t * st].copy()) for t in range(q)]
+            Rs = [R_of(r, c, t, base) for t in range(q)]
+            for tn in range(q):
+                bx = None
+                for t in range(q):
+                    w = J * (1 - 2 * t) * (1 - 2 * tn) if q == 2 else J * (t == tn)
+                    cx, cn = olds[t][0] + w + Rs[t] - Rs[tn], olds[t][1]
+                    if bx is None:
+                        bx, bn = cx.copy(), cn.copy()
+                    else:
+                        gt, eq = cx > bx, cx == bx
+                        bn = np.where(gt, cn, np.where(eq, bn + cn, bn))
+                        bx = np.maximum(bx, cx)
+                x[base + tn * st] = bx; n[base + tn * st] = bn
+    A = np.zeros(N)
+    for c in range(L):
+        if q == 2:
+            A = A + H[L - 1, c] * (1 - 2 * dig[c])
+        if c < L - 1:
+            A = A + two(K[L - 1, c], dig[c], dig[c + 1])
+    x = x + A
     m = x.max()
     return (0.0 if m == 0 else -m), int(sum(n[x == m]))
 
