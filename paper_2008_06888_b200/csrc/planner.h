@@ -267,7 +267,7 @@ struct FusedPlan {
     int L = 0;
     std::vector<FusedPass> passes;
     std::vector<MicroOp> mops;
-    std::vector<int> gate_rc;    // layout * 4096 + r * 64 + c of every gate, in execution order
+    std::vector<int> gate_rc;    // low << 16 | register bit << 13 | layout << 12 | r << 6 | c, in execution order
     bool ok = false;
 };
 
@@ -324,7 +324,7 @@ class FusedScheduler {
             P_.mops.push_back({MC_ROUND, (uint8_t)mask, (uint16_t)((int)P_.gate_rc.size() - pass_gate_begin_)});
             for (int b = 0; b < F_RB; ++b) if (mask >> b & 1) {
                 const int c = a + fused_digit_of_bit(low, layout, b);
-                P_.gate_rc.push_back(layout * 4096 + grow_[c] * 64 + c);
+                P_.gate_rc.push_back((low ? 1 << 16 : 0) | (b << 13) | (layout << 12) | (grow_[c] << 6) | c);
                 ++n;
             }
             for (int b = 0; b < F_RB; ++b) if (mask >> b & 1) grow_[a + fused_digit_of_bit(low, layout, b)] += 1;
@@ -408,7 +408,7 @@ inline std::string describe_fused(const FusedPlan& p) {
                     int g = ps.gate_begin + m.arg;
                     for (int b = 0; b < F_RB; ++b) if (m.mask >> b & 1) {
                         const int rc = p.gate_rc[g++];
-                        snprintf(line, sizeof line, "g k=%d r=%d c=%d layout=%d\n", b, (rc / 64) % 64, rc % 64, rc / 4096);
+                        snprintf(line, sizeof line, "g k=%d r=%d c=%d layout=%d\n", (rc >> 13) & 7, (rc >> 6) & 63, rc & 63, (rc >> 12) & 1);
                         out += line;
                     }
                     break; }

@@ -68,39 +68,84 @@ __device__ __forceinline__ void add2(float& o0, float& o1, float a0, float a1, f
         : "=f"(o0), "=f"(o1) : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
 }
 
+// FADD2 against a pre-packed 64-bit constant pair; unpacking of a 64-bit pair into two floats
+__device__ __forceinline__ void add2p(float& o0, float& o1, float a0, float a1, unsigned long long kp) {
+    asm("{ .reg .b64 ra, rc;\n\t"
+        "mov.b64 ra, {%2, %3};\n\t"
+        "add.f32x2 rc, ra, %4;\n\t"
+        "mov.b64 {%0, %1}, rc; }"
+        : "=f"(o0), "=f"(o1) : "f"(a0), "f"(a1), "l"(kp));
+}
+__device__ __forceinline__ void unpack2(unsigned long long p, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(p));
+}
+
 // ---- conjugated gate on register-index bit K ------------------------------------------------------
 // PN / QN: register-index bit holding the P / Q neighbour (chain position -1 / +1), or -1 when
-// that neighbour is constant per thread (its bit is then tp / tq).  c0 = ka[pn][qn], c1 = kb[pn][qn]
-// (x: 00, y: 01, z: 10, w: 11);  a = the element whose bit K is 0.
+// that neighbour is constant per thread (its bit is then tp / tq).  a = the element whose bit K
+// is 0.  The 8 constants ka[pn][qn], kb[pn][qn] arrive as two 128-bit shared-memory loads
+// (c0, c1), stored by the prep kernel in the order this body wants (gate_order()):
+//   ORDER_DEFAULT  c0 = ka[0][0] ka[0][1] ka[1][0] ka[1][1],  c1 = kb likewise
+//   ORDER_K0       c0 = kb00 ka00 kb01 ka01,  c1 = kb10 ka10 kb11 ka11     (K = 0: pair = (a, b))
+//   ORDER_PN0      c0 = ka[0][0] ka[1][0] ka[0][1] ka[1][1],  c1 = kb likewise   (bit 0 = P neighbour)
+// so that whenever the two elements of a register pair (v[j], v[j+1]) take DIFFERENT constants,
+// the constant pair is already an aligned 64-bit register pair straight out of the load (ptxas
+// otherwise rebuilds it with two moves in front of every FADD2: +67 % instructions for K = 0).
+enum GateOrder : int { ORDER_DEFAULT = 0, ORDER_K0 = 1, ORDER_PN0 = 2 };
+__host__ __device__ constexpr int gate_order(int K, int PN) { return K == 0 ? ORDER_K0 : (PN == 0 ? ORDER_PN0 : ORDER_DEFAULT); }
+
 template <int K, int PN, int QN>
-__device__ __forceinline__ void cgate(float (&v)[128], const float4 c0, const float4 c1, const int tp, const int tq) {
-    float ka[2][2] = {{c0.x, c0.y}, {c0.z, c0.w}}, kb[2][2] = {{c1.x, c1.y}, {c1.z, c1.w}};
-    if (PN < 0) {
-#pragma unroll
-        for (int h = 0; h < 2; ++h) { ka[0][h] = tp ? ka[1][h] : ka[0][h]; kb[0][h] = tp ? kb[1][h] : kb[0][h]; }
-    }
-    if (QN < 0) {
-#pragma unroll
-        for (int l = 0; l < 2; ++l) { ka[l][0] = tq ? ka[l][1] : ka[l][0]; kb[l][0] = tq ? kb[l][1] : kb[l][0]; }
-    }
+__device__ __forceinline__ void cgate(float (&v)[128], const ulonglong2 c0, const ulonglong2 c1, const int tp, const int tq) {
     constexpr int B = 1 << K;
 #define TTN_NP(j) (PN < 0 ? 0 : (((j) >> (PN < 0 ? 0 : PN)) & 1))
 #define TTN_NQ(j) (QN < 0 ? 0 : (((j) >> (QN < 0 ? 0 : QN)) & 1))
     if (K == 0) {
+        // pair (v[j], v[j+1]) = (a, b): t0 = a + kb (candidate for b), t1 = b + ka (candidate for a)
+        static_assert(K != 0 || (PN >= 0 && QN >= 0), "bit 0 sits inside the chain");
+        const unsigned long long kp[2][2] = {{c0.x, c0.y}, {c1.x, c1.y}};
 #pragma unroll
         for (int j = 0; j < 128; j += 2) {
-            float t0, t1;     // t0 = a + kb (candidate for b), t1 = b + ka (candidate for a)
-            add2(t0, t1, v[j], v[j + 1], kb[TTN_NP(j)][TTN_NQ(j)], ka[TTN_NP(j)][TTN_NQ(j)]);
+            float t0, t1;
+            add2p(t0, t1, v[j], v[j + 1], kp[TTN_NP(j)][TTN_NQ(j)]);
             v[j] = fmaxf(v[j], t1);
             v[j + 1] = fmaxf(v[j + 1], t0);
         }
-    } else {
+    } else if (PN == 0 || QN == 0) {
+        // bit 0 is a neighbour: (v[j], v[j+1]) take the constants for that neighbour bit = 0 / 1;
+        // the pair index is the OTHER neighbour's bit (a register bit, or tq when it is per thread)
+        unsigned long long pa[2] = {c0.x, c0.y}, pb[2] = {c1.x, c1.y};
+        constexpr int ON = PN == 0 ? QN : PN;          // the other neighbour
+        if (ON < 0) { const int t = PN == 0 ? tq : tp; pa[0] = t ? pa[1] : pa[0]; pb[0] = t ? pb[1] : pb[0]; }
+#define TTN_NO(j) (ON < 0 ? 0 : (((j) >> (ON < 0 ? 0 : ON)) & 1))
 #pragma unroll
         for (int j = 0; j < 128; j += 2) {
             if ((j & B) == 0) {
                 float a0, a1, b0, b1;
-                add2(a0, a1, v[j], v[j + 1], kb[TTN_NP(j)][TTN_NQ(j)], kb[TTN_NP(j + 1)][TTN_NQ(j + 1)]);
-                add2(b0, b1, v[j + B], v[j + B + 1], ka[TTN_NP(j)][TTN_NQ(j)], ka[TTN_NP(j + 1)][TTN_NQ(j + 1)]);
+                add2p(a0, a1, v[j], v[j + 1], pb[TTN_NO(j)]);
+                add2p(b0, b1, v[j + B], v[j + B + 1], pa[TTN_NO(j)]);
+                v[j] = fmaxf(v[j], b0); v[j + 1] = fmaxf(v[j + 1], b1);
+                v[j + B] = fmaxf(v[j + B], a0); v[j + B + 1] = fmaxf(v[j + B + 1], a1);
+            }
+        }
+#undef TTN_NO
+    } else {
+        float ka[2][2], kb[2][2];
+        unpack2(c0.x, ka[0][0], ka[0][1]); unpack2(c0.y, ka[1][0], ka[1][1]);
+        unpack2(c1.x, kb[0][0], kb[0][1]); unpack2(c1.y, kb[1][0], kb[1][1]);
+        if (PN < 0) {
+#pragma unroll
+            for (int h = 0; h < 2; ++h) { ka[0][h] = tp ? ka[1][h] : ka[0][h]; kb[0][h] = tp ? kb[1][h] : kb[0][h]; }
+        }
+        if (QN < 0) {
+#pragma unroll
+            for (int l = 0; l < 2; ++l) { ka[l][0] = tq ? ka[l][1] : ka[l][0]; kb[l][0] = tq ? kb[l][1] : kb[l][0]; }
+        }
+#pragma unroll
+        for (int j = 0; j < 128; j += 2) {
+            if ((j & B) == 0) {
+                float a0, a1, b0, b1;
+                add2(a0, a1, v[j], v[j + 1], kb[TTN_NP(j)][TTN_NQ(j)], kb[TTN_NP(j)][TTN_NQ(j)]);
+                add2(b0, b1, v[j + B], v[j + B + 1], ka[TTN_NP(j)][TTN_NQ(j)], ka[TTN_NP(j)][TTN_NQ(j)]);
                 v[j] = fmaxf(v[j], b0); v[j + 1] = fmaxf(v[j + 1], b1);
                 v[j + B] = fmaxf(v[j + B], a0); v[j + B + 1] = fmaxf(v[j + B + 1], a1);
             }
@@ -121,11 +166,11 @@ template <bool LOW, int K> struct Nbr {
 // constants of the gate after the current one are already in flight (n0, n1): the gate list of a
 // pass is contiguous in execution order, so the prefetch simply runs one entry ahead.
 template <bool LOW>
-__device__ __forceinline__ void fround(float (&v)[128], const unsigned mask, const float4* __restrict__& gk,
-                                       float4& n0, float4& n1, const int tp, const int tq) {
+__device__ __forceinline__ void fround(float (&v)[128], const unsigned mask, const ulonglong2* __restrict__& gk,
+                                       ulonglong2& n0, ulonglong2& n1, const int tp, const int tq) {
 #define TTN_G(Kk)                                                                                   \
     if (mask & (1u << Kk)) {                                                                        \
-        const float4 c0 = n0, c1 = n1;                                                              \
+        const ulonglong2 c0 = n0, c1 = n1;                                                          \
         gk += 2; n0 = gk[0]; n1 = gk[1];                                                            \
         cgate<Kk, Nbr<LOW, Kk>::PN, Nbr<LOW, Kk>::QN>(v, c0, c1, tp, tq);                           \
     }
@@ -359,8 +404,8 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
             // ---- run the program ------------------------------------------------------------------
             int pc = 0, layout = p.first_layout;
             unsigned op = s_mops[0];
-            const float4* gk = s_gk;
-            float4 n0 = gk[0], n1 = gk[1];
+            const ulonglong2* gk = reinterpret_cast<const ulonglong2*>(s_gk);
+            ulonglong2 n0 = gk[0], n1 = gk[1];
             for (;;) {
                 const unsigned code = op & 0xffu;
                 if (code == MC_END || code == MC_FINAL) break;
@@ -418,7 +463,7 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
 // ---- S0: per-instance gate constants and the final table from the couplings ------------------------
 struct FusedPrepParams {
     int L, n_gates;
-    const int* gate_rc;            // [n_gates]  layout * 4096 + r * 64 + c
+    const int* gate_rc;            // [n_gates]  low << 16 | K << 13 | layout << 12 | r << 6 | c
     const float* Jh; const float* Jv; const float* h;   // device couplings, per instance
     float* gate_k;                 // [inst][n_gates][8]
     float* final_tab;              // [inst][FFINAL_FLOATS]
@@ -436,17 +481,28 @@ __global__ void __launch_bounds__(256) fused_prep_kernel(const FusedPrepParams p
     auto Hacc = [&](int R, int c) { double s = 0; if (hh) for (int r = 0; r < R; ++r) s += (double)hh[r * L + c]; return s; };
     auto Kacc = [&](int R, int c) { double s = 0; if (c < 0 || c >= L - 1) return s; for (int r = 0; r < R; ++r) s += (double)Jh[r * (L - 1) + c]; return s; };
     if (idx < p.n_gates) {
-        const int g = p.gate_rc[idx], mirrored = g >> 12, r = (g >> 6) & 63, c = g & 63;
+        const int g = p.gate_rc[idx], mirrored = (g >> 12) & 1, K = (g >> 13) & 7, low = (g >> 16) & 1;
+        const int r = (g >> 6) & 63, c = g & 63;
         const double m = -2.0 * (double)Jv[(r - 1) * L + c];
         const double H = Hacc(r, c), Kl = Kacc(r, c - 1), Kr = Kacc(r, c);
         float* out = p.gate_k + (inst * p.n_gates + idx) * 8;
-        // stored as [side][P bit][Q bit]: P = left neighbour in layout A, right neighbour in layout B
+        // k[side][P bit][Q bit]: P = left neighbour in layout A, right neighbour in layout B
+        float k[2][2][2];
         for (int np = 0; np < 2; ++np)
             for (int nq = 0; nq < 2; ++nq) {
                 const int nl = mirrored ? nq : np, nh = mirrored ? np : nq;
                 const double rho = H + (nl ? -Kl : Kl) + (nh ? -Kr : Kr);
-                out[np * 2 + nq] = (float)(m - 2.0 * rho);         // ka: a' = max(a, b + ka)
-                out[4 + np * 2 + nq] = (float)(m + 2.0 * rho);     // kb: b' = max(b, a + kb)
+                k[0][np][nq] = (float)(m - 2.0 * rho);         // ka: a' = max(a, b + ka)
+                k[1][np][nq] = (float)(m + 2.0 * rho);         // kb: b' = max(b, a + kb)
+            }
+        const int pos = fused_chain_pos(low != 0, K);
+        const int PN = pos == 0 ? -1 : fused_bit_of_digit(low != 0, 0, pos - 1);
+        const int order = gate_order(K, PN);
+        for (int np = 0; np < 2; ++np)
+            for (int nq = 0; nq < 2; ++nq) {
+                if (order == ORDER_K0) { out[(np * 2 + nq) * 2] = k[1][np][nq]; out[(np * 2 + nq) * 2 + 1] = k[0][np][nq]; }
+                else if (order == ORDER_PN0) { out[nq * 2 + np] = k[0][np][nq]; out[4 + nq * 2 + np] = k[1][np][nq]; }
+                else { out[np * 2 + nq] = k[0][np][nq]; out[4 + np * 2 + nq] = k[1][np][nq]; }
             }
     }
     if (idx < FFINAL_FLOATS) {
