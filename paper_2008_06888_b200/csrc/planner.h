@@ -34,7 +34,7 @@ struct Op {            // 8 bytes, uploaded as-is
     uint8_t type;      // OpType
     uint8_t pos;       // GATE: tile position of the digit (0 .. T-1)
     uint8_t c;         // global column (digit) -- DJ: left digit, pair (c, c+1)
-    uint8_t pad;
+    uint8_t first;     // 1 = first gate of a round (the gates of a round commute: all were legal together)
     uint16_t row;      // lattice row r of the operation
     uint16_t pad2;
 };
@@ -88,8 +88,10 @@ class Scheduler {
                 legal.push_back(c);
             }
             if (legal.empty()) break;
+            bool first = true;
             for (int c : legal) {
-                ops.push_back({OP_GATE, (uint8_t)pos_of(c), (uint8_t)c, 0, (uint16_t)grow_[c], 0});
+                ops.push_back({OP_GATE, (uint8_t)pos_of(c), (uint8_t)c, (uint8_t)(first ? 1 : 0), (uint16_t)grow_[c], 0});
+                first = false;
                 ++gates;
             }
             for (int c : legal) grow_[c] += 1;

@@ -371,7 +371,9 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
             if ((LOW ? wt : (wt & ~3ull)) >= p.tiles_per_inst) break;       // uniform per group
             if (!LOW && wt >= p.tiles_per_inst) {      // L = 13: fewer than 4 tiles; keep the barrier counts equal
                 if (!(p.flags & PASS_INIT)) group_sync(warp);
+#ifndef TTN_NO_STORE_SYNC
                 if (!(p.flags & PASS_REDUCE)) group_sync(warp);
+#endif
                 continue;
             }
             // ---- tile geometry: base index, per-thread P / Q neighbour bits per layout ---------------
@@ -442,7 +444,9 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
                 }
                 wmax = fmaxf(wmax, mx + cthr);
             } else {
+#ifndef TTN_NO_STORE_SYNC
                 if (!LOW) group_sync(warp);
+#endif
                 if (LOW || p.last_layout == 1) gmove<LOW, 1, true>(v, S + base, lane, p.stride_bytes, p.a);
                 else gmove<LOW, 0, true>(v, S + base, lane, p.stride_bytes, p.a);
             }

@@ -59,12 +59,11 @@ __device__ __forceinline__ double warp_sum(double v) {
 // tropical / counting (+) of candidate (cx, cn) into accumulator (x, n): Eq. (4)
 template <bool COUNT>
 __device__ __forceinline__ void oplus(float& x, double& n, float cx, double cn) {
-    if (COUNT) {
-        if (cx > x) { x = cx; n = cn; }
-        else if (cx == x) { n += cn; }
-    } else {
-        x = fmaxf(x, cx);
+    if (COUNT) {          // branch-free: the sum is formed always and selected on the exact tie
+        const double s = n + cn;
+        n = cx > x ? cn : (cx == x ? s : n);
     }
+    x = fmaxf(x, cx);
 }
 
 // exact n / d for n * d < 2^32 with the host-side magic M = floor(2^32 / d) + 1
@@ -132,10 +131,17 @@ __global__ void __launch_bounds__(512) pass_kernel(const PassParams p) {
         const float4 k0 = reinterpret_cast<const float4*>(GK)[2 * k], k1 = reinterpret_cast<const float4*>(GK)[2 * k + 1];
         const unsigned ngrp = N / Q;
         for (unsigned g = threadIdx.x; g < ngrp; g += blockDim.x) {
-            const unsigned hi = st == 1 ? g : fastdiv(g, m_st), lo = g - hi * st;
+            unsigned hi, lo; int dl, dr;
+            if (Q == 2) {
+                hi = g >> pos; lo = g & (st - 1);
+                dl = l_in ? (int)(lo >> (pos - 1)) : dl_out;                               // top digit of lo
+                dr = r_in ? (int)(hi & 1u) : dr_out;
+            } else {
+                hi = st == 1 ? g : fastdiv(g, m_st); lo = g - hi * st;
+                dl = l_in ? (int)(st_q == 1 ? lo : fastdiv(lo, m_stq)) : dl_out;
+                dr = r_in ? (int)(hi % Q) : dr_out;
+            }
             const unsigned i0 = hi * (st * Q) + lo;
-            const int dl = l_in ? (int)(st_q == 1 ? lo : fastdiv(lo, m_stq)) : dl_out;   // top digit of lo
-            const int dr = r_in ? (int)(hi % Q) : dr_out;
             if (Q == 2) {
                 // conjugated (A2): a' = a (+) (b + ka[dl][dr]),  b' = b (+) (a + kb[dl][dr])
                 const int n = dl * 2 + dr;
