@@ -213,15 +213,22 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
     pp.stride_bytes = 4u << ps.a;     // a <= L - 9 <= 25
     unsigned long long grid = (unsigned long long)P->fused_grid;
     const int nw = ttn::fwarps(ps.low != 0);
-    const unsigned long long need = (pp.tiles_per_inst + nw - 1) / nw;
-    if (grid > need) grid = need;
+    // batches of small lattices: one CTA per instance at a time instead of the whole grid per instance
+    pp.cta_per_inst = (P->batch > 1 && pp.tiles_per_inst < (unsigned long long)nw * grid) ? 1 : 0;
+    if (pp.cta_per_inst) {
+        if (grid > (unsigned long long)P->batch) grid = (unsigned long long)P->batch;
+    } else {
+        const unsigned long long need = (pp.tiles_per_inst + nw - 1) / nw;
+        if (grid > need) grid = need;
+    }
+    pp.part_stride = pp.cta_per_inst ? 1 : (int)grid;
     if (ps.low) ttn::fused_pass_kernel<true><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(true), st>>>(pp);
     else ttn::fused_pass_kernel<false><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(false), st>>>(pp);
     TTN_CUDA(cudaGetLastError());
     if (ps.flags & ttn::PASS_REDUCE) {
         // one partial per CTA and instance
         ttn::final_reduce_kernel<false><<<P->batch, 256, 0, st>>>(
-            pp.part_x, nullptr, grid, reinterpret_cast<float*>(P->ws + y.out_x), nullptr);
+            pp.part_x, nullptr, (unsigned long long)pp.part_stride, reinterpret_cast<float*>(P->ws + y.out_x), nullptr);
         TTN_CUDA(cudaGetLastError());
     }
     return TTN_OK;
@@ -404,11 +411,25 @@ ttn_status ttn_plan_launch(ttn_plan* P, void* stream) {
         }
         return TTN_OK;
     }
+    const bool gtiming = getenv("TTN_DEBUG_TIMING") != nullptr;      // per-pass device times on stderr
+    std::vector<cudaEvent_t> gev;
+    if (gtiming) { gev.resize(P->plan.passes.size() + 1); for (auto& e : gev) cudaEventCreate(&e); cudaEventRecord(gev[0], st); }
+    size_t gk = 0;
     for (const ttn::Pass& ps : P->plan.passes) {
         ttn_status s;
         if (P->q == 2) s = P->count ? launch_pass<2, true>(P, ps, st) : launch_pass<2, false>(P, ps, st);
         else s = P->count ? launch_pass<3, true>(P, ps, st) : launch_pass<3, false>(P, ps, st);
         if (s != TTN_OK) return s;
+        if (gtiming) cudaEventRecord(gev[++gk], st);
+    }
+    if (gtiming) {
+        cudaStreamSynchronize(st);
+        for (size_t i = 0; i < P->plan.passes.size(); ++i) {
+            float ms = 0; cudaEventElapsedTime(&ms, gev[i], gev[i + 1]);
+            const ttn::Pass& ps = P->plan.passes[i];
+            fprintf(stderr, "gpass %2zu lo=%d a=%d b=%d gates=%3d flags=%d : %.2f ms\n", i, ps.lo, ps.a, ps.b, ps.n_gates, ps.flags, ms);
+        }
+        for (auto& e : gev) cudaEventDestroy(e);
     }
     if (P->config) {
         const Layout& y = P->lay;

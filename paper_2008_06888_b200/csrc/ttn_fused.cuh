@@ -53,7 +53,10 @@ struct FusedParams {
     const float* gate_k; int n_gates;   // [inst][all gates][8]; this pass's slice of instance 0
     unsigned long long gate_inst_stride;          // floats between instances
     const float* final_tab;             // [inst][FFINAL_FLOATS] (REDUCE pass only)
-    float* part_x;                      // [batch][gridDim.x] (REDUCE)
+    float* part_x;                      // [batch][part_stride] (REDUCE)
+    int cta_per_inst;                   // 1: few tiles per instance -- every CTA sweeps whole instances
+                                        // (blockIdx.x, + gridDim.x, ...) with its own warps only
+    int part_stride;                    // partials per instance: gridDim.x, or 1 when cta_per_inst
     unsigned stride_bytes;              // HIGH: 4 << a, passed opaque so that the address math stays
                                         // one IMAD.WIDE (32 x 32 -> 64 bit) per access
 };
@@ -168,10 +171,14 @@ template <bool LOW, int K> struct Nbr {
 template <bool LOW>
 __device__ __forceinline__ void fround(float (&v)[128], const unsigned mask, const ulonglong2* __restrict__& gk,
                                        ulonglong2& n0, ulonglong2& n1, const int tp, const int tq) {
+#ifdef TTN_NO_PREFETCH
+#define TTN_FETCHK const ulonglong2 c0 = gk[0], c1 = gk[1]; gk += 2;
+#else
+#define TTN_FETCHK const ulonglong2 c0 = n0, c1 = n1; gk += 2; n0 = gk[0]; n1 = gk[1];
+#endif
 #define TTN_G(Kk)                                                                                   \
     if (mask & (1u << Kk)) {                                                                        \
-        const ulonglong2 c0 = n0, c1 = n1;                                                          \
-        gk += 2; n0 = gk[0]; n1 = gk[1];                                                            \
+        TTN_FETCHK                                                                                  \
         cgate<Kk, Nbr<LOW, Kk>::PN, Nbr<LOW, Kk>::QN>(v, c0, c1, tp, tq);                           \
     }
     TTN_G(0) TTN_G(1) TTN_G(2) TTN_G(3) TTN_G(4) TTN_G(5) TTN_G(6)
@@ -339,10 +346,10 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
     float* s_red = reinterpret_cast<float*>(s_mops + FMAX_MOPS);                        // FWARPS (<= 16)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     float4* myreg = regions + warp * FREGION_F4;
-    const unsigned long long gw = (unsigned long long)blockIdx.x * FWARPS + warp;
-    const unsigned long long nw = (unsigned long long)gridDim.x * FWARPS;
+    const unsigned long long gw = p.cta_per_inst ? (unsigned long long)warp : (unsigned long long)blockIdx.x * FWARPS + warp;
+    const unsigned long long nw = p.cta_per_inst ? (unsigned long long)FWARPS : (unsigned long long)gridDim.x * FWARPS;
 
-    for (int inst = 0; inst < p.batch; ++inst) {
+    for (int inst = p.cta_per_inst ? (int)blockIdx.x : 0; inst < p.batch; inst += p.cta_per_inst ? (int)gridDim.x : 1) {
         // ---- stage this instance's program and gate constants (S0 outputs) into shared memory
         __syncthreads();
         for (int i = tid; i < p.n_mops; i += blockDim.x) {
@@ -458,7 +465,7 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
             if (tid == 0) {
                 float m = s_red[0];
                 for (int w = 1; w < FWARPS; ++w) m = fmaxf(m, s_red[w]);
-                p.part_x[(size_t)inst * gridDim.x + blockIdx.x] = m;
+                p.part_x[(size_t)inst * p.part_stride + (p.cta_per_inst ? 0 : blockIdx.x)] = m;
             }
         }
     }
