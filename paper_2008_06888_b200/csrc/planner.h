@@ -275,7 +275,8 @@ struct FusedPlan {
 
 class FusedScheduler {
   public:
-    FusedScheduler(int L, FusedPlan& p) : L_(L), P_(p), grow_(L, 1) {}
+    FusedScheduler(int L, FusedPlan& p) : L_(L), Pp_(&p), grow_(L, 1) {}
+    void rebind(FusedPlan& p) { Pp_ = &p; }
     bool done() const {
         for (int c = 0; c < L_; ++c) if (grow_[c] != L_) return false;
         return true;
@@ -284,7 +285,7 @@ class FusedScheduler {
     int run_pass(int a, bool low, int max_gates, FusedPass& ps) {
         const int W = low ? F_WLOW : F_WHIGH;
         ps.a = a; ps.W = W; ps.low = low; ps.flags = 0; ps.n_phases = 0; ps.n_rounds = 0;
-        ps.mop_begin = (int)P_.mops.size(); ps.gate_begin = (int)P_.gate_rc.size();
+        ps.mop_begin = (int)Pp_->mops.size(); ps.gate_begin = (int)Pp_->gate_rc.size();
         pass_gate_begin_ = ps.gate_begin; max_gates_ = max_gates;
         // the low tile loads and stores in layout B (coalesced); high tiles start in A
         int layout = low ? 1 : 0;
@@ -292,20 +293,20 @@ class FusedScheduler {
         int total = 0, idle = 0;
         bool pending_x = false;                        // an exchange is owed before the next non-empty phase
         while (idle < 2) {
-            size_t mark = P_.mops.size();
-            if (pending_x) P_.mops.push_back({(uint8_t)(layout == 1 ? MC_XAB : MC_XBA), 0, 0});
+            size_t mark = Pp_->mops.size();
+            if (pending_x) Pp_->mops.push_back({(uint8_t)(layout == 1 ? MC_XAB : MC_XBA), 0, 0});
             int rounds = 0;
             int n = run_phase(a, low, layout, rounds);
-            if (n == 0) { P_.mops.resize(mark); ++idle; layout ^= 1; pending_x = !pending_x; continue; }
+            if (n == 0) { Pp_->mops.resize(mark); ++idle; layout ^= 1; pending_x = !pending_x; continue; }
             total += n; idle = 0; ++ps.n_phases; ps.n_rounds += rounds;
             layout ^= 1; pending_x = true;
         }
         int last = layout ^ 1;                          // the layout of the last productive phase
         if (ps.n_phases == 0) last = ps.first_layout;
-        if (low && last != 1) { P_.mops.push_back({MC_XAB, 0, 0}); last = 1; }
+        if (low && last != 1) { Pp_->mops.push_back({MC_XAB, 0, 0}); last = 1; }
         ps.last_layout = last;
-        P_.mops.push_back({MC_END, 0, 0});
-        ps.mop_end = (int)P_.mops.size(); ps.gate_end = (int)P_.gate_rc.size();
+        Pp_->mops.push_back({MC_END, 0, 0});
+        ps.mop_end = (int)Pp_->mops.size(); ps.gate_end = (int)Pp_->gate_rc.size();
         return total;
     }
   private:
@@ -319,14 +320,14 @@ class FusedScheduler {
     int run_phase(int a, bool low, int layout, int& rounds) {
         int n = 0;
         for (;;) {
-            if ((int)P_.gate_rc.size() - pass_gate_begin_ + F_RB > max_gates_) break;
+            if ((int)Pp_->gate_rc.size() - pass_gate_begin_ + F_RB > max_gates_) break;
             unsigned mask = 0;
             for (int b = 0; b < F_RB; ++b) if (legal(a + fused_digit_of_bit(low, layout, b))) mask |= 1u << b;
             if (!mask) break;
-            P_.mops.push_back({MC_ROUND, (uint8_t)mask, (uint16_t)((int)P_.gate_rc.size() - pass_gate_begin_)});
+            Pp_->mops.push_back({MC_ROUND, (uint8_t)mask, (uint16_t)((int)Pp_->gate_rc.size() - pass_gate_begin_)});
             for (int b = 0; b < F_RB; ++b) if (mask >> b & 1) {
                 const int c = a + fused_digit_of_bit(low, layout, b);
-                P_.gate_rc.push_back((low ? 1 << 16 : 0) | (b << 13) | (layout << 12) | (grow_[c] << 6) | c);
+                Pp_->gate_rc.push_back((low ? 1 << 16 : 0) | (b << 13) | (layout << 12) | (grow_[c] << 6) | c);
                 ++n;
             }
             for (int b = 0; b < F_RB; ++b) if (mask >> b & 1) grow_[a + fused_digit_of_bit(low, layout, b)] += 1;
@@ -334,17 +335,37 @@ class FusedScheduler {
         }
         return n;
     }
-    int L_; FusedPlan& P_;
+    int L_; FusedPlan* Pp_;
     std::vector<int> grow_;      // grow[c] = rows complete on digit c (row 0 needs no gate)
     int pass_gate_begin_ = 0, max_gates_ = 1 << 30;
 };
 
-// Tile cycle: the low tile [0,12), then high tiles [x, x+9) advancing by `stride`, the last
-// flush with L.  Chooses the stride with the lowest estimated cost.
+// Estimated time of one pass in ms on B200 (fit over the measured launch lists, profiles/r01f.md):
+// 0.267 ms per gate (FMNMX floor 0.231), a fixed part for the memory phases that do not hide, round
+// dispatch and exchanges; a pass cannot beat its memory time.
+inline double fused_pass_cost(const FusedPass& ps) {
+    const int g = ps.gate_end - ps.gate_begin, x = ps.n_phases > 1 ? ps.n_phases - 1 : 0;
+    if (ps.low) { const double t = 1.2 + 0.267 * g + 0.02 * ps.n_rounds + 0.25 * x; return t > 6.5 ? t : 6.5; }
+    const double t = 3.5 + 0.267 * g + 0.08 * ps.n_rounds + 0.25 * x;
+    return t > 9.0 ? t : 9.0;
+}
+
+// Two tile orders are tried and the cheaper plan (by fused_pass_cost) wins:
+//  * cyclic: the low tile [0,12), then high tiles [x, x+9) advancing by `stride`, the last flush
+//    with L, for every stride;
+//  * greedy: at every step the tile (low, or high at any start) that applies the most gates.
 inline FusedPlan make_fused_plan(int L, int max_gates_per_pass) {
     FusedPlan best;
     if (L < F_WLOW) return best;
     double best_cost = -1;
+    auto finish = [&](FusedPlan& p) {
+        // the last pass adds A_{L-1}(s) and reduces: MC_FINAL replaces its MC_END
+        p.passes.back().flags |= PASS_REDUCE;
+        p.mops.back().code = MC_FINAL;
+        double cost = 0;
+        for (auto& ps : p.passes) cost += fused_pass_cost(ps);
+        if (best_cost < 0 || cost < best_cost) { best = p; best_cost = cost; best.ok = true; }
+    };
     for (int stride = 1; stride <= F_WHIGH; ++stride) {
         std::vector<int> starts;
         starts.push_back(0);
@@ -373,15 +394,31 @@ inline FusedPlan make_fused_plan(int L, int max_gates_per_pass) {
             p.passes.push_back(ps);
         }
         if (!s.done()) continue;
-        // the last pass adds A_{L-1}(s) and reduces: MC_FINAL replaces its MC_END
-        p.passes.back().flags |= PASS_REDUCE;
-        p.mops.back().code = MC_FINAL;
-        // cost model (issue slots per thread, 128 elements): gate 192, round 12, exchange 80;
-        // one HBM pass ~ 2500 (5.7 ms at 6 TB/s vs 64 updates/clk/SM)
-        double cost = 0;
-        for (auto& ps : p.passes)
-            cost += 2500.0 + 192.0 * (ps.gate_end - ps.gate_begin) + 12.0 * ps.n_rounds + 80.0 * ps.n_phases;
-        if (best_cost < 0 || cost < best_cost) { best = p; best_cost = cost; best.ok = true; }
+        finish(p);
+    }
+    if (L > F_WLOW) {                               // greedy by gate count
+        FusedPlan p; p.L = L;
+        FusedScheduler s(L, p);
+        bool first = true;
+        while ((first || !s.done()) && p.passes.size() < 4096) {
+            int best_a = -1, best_n = -1; double best_c = 0;
+            for (int a = 0; a + F_WHIGH <= L; a = (a == 0 ? F_AMIN : a + 1)) {
+                FusedScheduler trial = s;                       // dry run on a copy
+                FusedPlan scratch; scratch.L = L;
+                trial.rebind(scratch);
+                FusedPass ps{};
+                const int n = trial.run_pass(a, a == 0, max_gates_per_pass, ps);
+                const double c = fused_pass_cost(ps);
+                if (n > best_n) { best_a = a; best_n = n; best_c = c; }          // ties: the lowest start
+            }
+            if (best_n <= 0 && !first) break;
+            FusedPass ps{};
+            s.run_pass(best_a, best_a == 0, max_gates_per_pass, ps);
+            if (first) ps.flags |= PASS_INIT;
+            first = false;
+            p.passes.push_back(ps);
+        }
+        if (s.done()) finish(p);
     }
     return best;
 }
