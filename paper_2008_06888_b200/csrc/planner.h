@@ -286,7 +286,7 @@ class FusedScheduler {
         const int W = low ? F_WLOW : F_WHIGH;
         ps.a = a; ps.W = W; ps.low = low; ps.flags = 0; ps.n_phases = 0; ps.n_rounds = 0;
         ps.mop_begin = (int)Pp_->mops.size(); ps.gate_begin = (int)Pp_->gate_rc.size();
-        pass_gate_begin_ = ps.gate_begin; max_gates_ = max_gates;
+        pass_gate_begin_ = ps.gate_begin; pass_mop_begin_ = ps.mop_begin; max_gates_ = max_gates;
         // the low tile loads and stores in layout B (coalesced); high tiles start in A
         int layout = low ? 1 : 0;
         ps.first_layout = layout;
@@ -321,6 +321,7 @@ class FusedScheduler {
         int n = 0;
         for (;;) {
             if ((int)Pp_->gate_rc.size() - pass_gate_begin_ + F_RB > max_gates_) break;
+            if ((int)Pp_->mops.size() - pass_mop_begin_ + 8 > max_mops_) break;
             unsigned mask = 0;
             for (int b = 0; b < F_RB; ++b) if (legal(a + fused_digit_of_bit(low, layout, b))) mask |= 1u << b;
             if (!mask) break;
@@ -337,7 +338,8 @@ class FusedScheduler {
     }
     int L_; FusedPlan* Pp_;
     std::vector<int> grow_;      // grow[c] = rows complete on digit c (row 0 needs no gate)
-    int pass_gate_begin_ = 0, max_gates_ = 1 << 30;
+    int pass_gate_begin_ = 0, pass_mop_begin_ = 0, max_gates_ = 1 << 30;
+    int max_mops_ = 120;         // micro-ops per pass the kernel stages (FMAX_MOPS = 128)
 };
 
 // Estimated time of one pass in ms on B200 (fit over the measured launch lists, profiles/r01f.md):

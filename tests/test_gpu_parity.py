@@ -251,7 +251,29 @@ def test_cfg4_32x32_pmj_energy():
     torch.cuda.empty_cache()
 
 
-@pytest.mark.parametrize("L", [24, 28])
+def test_L33_beyond_2_to_32_elements():
+    """2^33-entry state (32 GiB): element indices and byte offsets beyond 2^32.  Pins that need no
+    oracle run: planted (gauge-transformed ferromagnet) E0 = -2L(L-1); transpose invariance."""
+    import torch
+    L = 33
+    free, _ = torch.cuda.mem_get_info()
+    if free < 40 * 2 ** 30:
+        pytest.skip("needs 40 GiB of free device memory")
+    ws = ttn.alloc_workspace(ttn.workspace_bytes(2, L, ttn.TROPICAL_F32, 1))
+    rng = np.random.default_rng(33)
+    eps = rng.choice([-1.0, 1.0], size=(L, L)).astype(np.float32)
+    Ep = ttn.sweep_energy((eps[:, :-1] * eps[:, 1:])[None], (eps[:-1, :] * eps[1:, :])[None], workspace=ws)[0]
+    assert Ep == -2 * L * (L - 1)
+    Jh, Jv, _ = make_batch(L, [4033], "pmj")
+    E0 = ttn.sweep_energy(Jh, Jv, workspace=ws)[0]
+    Et = ttn.sweep_energy(np.ascontiguousarray(Jv.transpose(0, 2, 1)),
+                          np.ascontiguousarray(Jh.transpose(0, 2, 1)), workspace=ws)[0]
+    assert E0 == Et and E0 == round(E0) and -2 * L * (L - 1) <= E0 < 0
+    del ws
+    torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("L", [24, 28, 30])
 def test_large_energy_vs_golden(L):
     gold = golden()
     key = ("ising_energy", L, 4000)
