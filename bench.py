@@ -261,7 +261,13 @@ def main():
                     "h2d_bytes_per_step": int(Jh.nbytes + Jv.nbytes), "d2h_bytes_per_step": 4},
             "gpu_launches": plan.num_launches * args.steps,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                         "frac": achieved / peak,
+                         # dram__bytes_read.sum + dram__bytes_write.sum per pass launch from the ncu
+                         # --set full capture in profiles/r01f_ncu_full_summary.csv (one read + one
+                         # write of the state); algorithmic bytes per launch = bytes_min / passes
+                         "traffic": 17.18e9 + 17.12e9 if L == 32 else None,
+                         "algorithmic_bytes_per_launch": bytes_min(L) / plan.num_passes,
+                         "peak_source": peak_src,
                          "algorithmic_bytes_per_sweep": bytes_min(L),
                          "kernel": "ttn::fused_pass_kernel<LOW|HIGH> (all %d pass launches of one sweep)" % plan.num_passes},
             "alu_roofline": {"bound": "alu", "achieved": updates(L) / (ms_per_step * 1e-3),

@@ -211,6 +211,10 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
     pp.final_tab = reinterpret_cast<const float*>(P->ws + y.f_final);
     pp.part_x = reinterpret_cast<float*>(P->ws + y.part_x);
     pp.stride_bytes = 4u << ps.a;     // a <= L - 9 <= 25
+    pp.prefetch_pc = 0;
+    for (int k = ps.mop_begin; k < ps.mop_end; ++k)
+        if (fp.mops[k].code == ttn::MC_XAB || fp.mops[k].code == ttn::MC_XBA) pp.prefetch_pc = k - ps.mop_begin + 1;
+    if (ps.a > 18) pp.prefetch_pc = -1;      // > 256 distinct 2 MiB pages per tile: synchronous loads
     unsigned long long grid = (unsigned long long)P->fused_grid;
     const int nw = ttn::fwarps(ps.low != 0);
     // batches of small lattices: one CTA per instance at a time instead of the whole grid per instance

@@ -54,6 +54,12 @@ struct FusedParams {
     unsigned long long gate_inst_stride;          // floats between instances
     const float* final_tab;             // [inst][FFINAL_FLOATS] (REDUCE pass only)
     float* part_x;                      // [batch][part_stride] (REDUCE)
+    int prefetch_pc;                    // HIGH: -1 = synchronous loads (tiles spanning > 256 pages of 2 MiB:
+                                        // the burst of a whole tile's translations is slower than 128
+                                        // paced loads); else the micro-op index after the last exchange: from
+                                        // there on the warp's shared-memory region is free, and the NEXT
+                                        // tile is fetched into it asynchronously (cp.async) while the rest
+                                        // of this tile's gates run
     int cta_per_inst;                   // 1: few tiles per instance -- every CTA sweeps whole instances
                                         // (blockIdx.x, + gridDim.x, ...) with its own warps only
     int part_stride;                    // partials per instance: gridDim.x, or 1 when cta_per_inst
@@ -328,6 +334,34 @@ __device__ __forceinline__ float final_thread_const(const float* s_fin, int L, i
     return acc;
 }
 
+// ---- HIGH tiles: asynchronous prefetch of the next tile into the warp's own exchange region -------
+// Layout in the region: row e (512 rows of 8 floats = one 32-byte sector each) at float index
+// 8 (e + (e >> 7)): one slot of skew per 128 rows makes the reads of BOTH layouts bank-conflict
+// free (layout A lanes differ in e by multiples of 128, layout B lanes by 1, 2, 3).
+__device__ __forceinline__ void pf_issue(float4* region, const float* tile, int lane, unsigned sb, int a) {
+    const unsigned sbase = (unsigned)__cvta_generic_to_shared(region) + 32u * (unsigned)(lane >> 1) + 16u * (unsigned)(lane & 1);
+    const unsigned long long g = (unsigned long long)__cvta_generic_to_global(tile + ((unsigned long long)(lane >> 1) << a) + 4 * (lane & 1));
+#pragma unroll
+    for (int i = 0; i < 32; ++i) {       // rows e = 16 i + (lane >> 1), half h = lane & 1
+        const unsigned long long ga = addr_mad(g, sb, 16u * i);
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(sbase + 32u * (16u * i + (i >> 3))), "l"(ga) : "memory");
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+}
+template <int LAYOUT>
+__device__ __forceinline__ void pf_read(float (&v)[128], const float4* region, int lane) {
+    const float* r = reinterpret_cast<const float*>(region);
+    if (LAYOUT == 1) {                   // lanes (rho, d0, d1): e = (lane >> 3) + ereg, no carry into bit 7
+        const float* q = r + lane;
+#pragma unroll
+        for (int j = 0; j < 128; ++j) v[j] = q[8 * (ereg_high(1, j) + (ereg_high(1, j) >> 7))];
+    } else {                             // lanes (rho, d7, d8): e = ereg + 128 k, k = lane >> 3
+        const float* q = r + (lane & 7) + 1032 * (lane >> 3);
+#pragma unroll
+        for (int j = 0; j < 128; ++j) v[j] = q[8 * ereg_high(0, j)];
+    }
+}
+
 // named barrier of one 4-warp group (barrier 0 is __syncthreads)
 __device__ __forceinline__ void group_sync(int warp) {
 #ifndef TTN_NO_GROUPSYNC
@@ -372,15 +406,24 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
         // stores, so that the lines are requested whole and at the same time (scattered 32-byte
         // sectors that arrive at different times cost DRAM efficiency); groups drift freely against
         // each other, which is what overlaps memory phases with gate phases.
+        auto tile_of = [&](unsigned long long it) -> unsigned long long {
+            return LOW ? it * nw + gw : 4ull * (it * (nw >> 2) + (gw >> 2)) + (unsigned long long)(warp & 3);
+        };
+        auto high_base = [&](unsigned long long wt) -> unsigned long long {
+            const int amid = p.a - F_RIDE;
+            return ((wt & ((1ull << amid) - 1)) << F_RIDE) + ((wt >> amid) << (p.a + F_WHIGH));
+        };
+        const bool async_load = !LOW && !(p.flags & PASS_INIT) && p.prefetch_pc >= 0;
+        if (async_load) {                               // the first tile of this warp
+            group_sync(warp);
+            if (tile_of(0) < p.tiles_per_inst) pf_issue(myreg, S + high_base(tile_of(0)), lane, p.stride_bytes, p.a);
+        }
         for (unsigned long long it = 0;; ++it) {
-            const unsigned long long wt = LOW ? it * nw + gw
-                : 4ull * (it * (nw >> 2) + (gw >> 2)) + (unsigned long long)(warp & 3);
+            const unsigned long long wt = tile_of(it);
             if ((LOW ? wt : (wt & ~3ull)) >= p.tiles_per_inst) break;       // uniform per group
             if (!LOW && wt >= p.tiles_per_inst) {      // L = 13: fewer than 4 tiles; keep the barrier counts equal
-                if (!(p.flags & PASS_INIT)) group_sync(warp);
-#ifndef TTN_NO_STORE_SYNC
+                if (!(p.flags & PASS_INIT)) group_sync(warp);      // the load barrier (either flavour)
                 if (!(p.flags & PASS_REDUCE)) group_sync(warp);
-#endif
                 continue;
             }
             // ---- tile geometry: base index, per-thread P / Q neighbour bits per layout ---------------
@@ -405,10 +448,18 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
             if (p.flags & PASS_INIT) {
 #pragma unroll
                 for (int j = 0; j < 128; ++j) v[j] = 0.f;                         // tropical one
-            } else {
-                if (!LOW) group_sync(warp);
-                if (LOW || p.first_layout == 1) gmove<LOW, 1, false>(v, S + base, lane, p.stride_bytes, p.a);
+            } else if (LOW) {
+                gmove<LOW, 1, false>(v, S + base, lane, p.stride_bytes, p.a);
+            } else if (!async_load) {
+                group_sync(warp);
+                if (p.first_layout == 1) gmove<LOW, 1, false>(v, S + base, lane, p.stride_bytes, p.a);
                 else gmove<LOW, 0, false>(v, S + base, lane, p.stride_bytes, p.a);
+            } else {
+                // the tile was fetched into this warp's region while the previous tile was computed
+                asm volatile("cp.async.wait_group 0;" ::: "memory");
+                __syncwarp();
+                if (p.first_layout == 1) pf_read<1>(v, myreg, lane); else pf_read<0>(v, myreg, lane);
+                __syncwarp();
             }
             // ---- run the program ------------------------------------------------------------------
             int pc = 0, layout = p.first_layout;
@@ -416,6 +467,11 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
             const ulonglong2* gk = reinterpret_cast<const ulonglong2*>(s_gk);
             ulonglong2 n0 = gk[0], n1 = gk[1];
             for (;;) {
+                if (async_load && pc == p.prefetch_pc) {    // the region is free from here on: fetch the next tile
+                    const unsigned long long wn = tile_of(it + 1);
+                    group_sync(warp);                       // the group's 4 sectors of every line are requested together
+                    if (wn < p.tiles_per_inst) pf_issue(myreg, S + high_base(wn), lane, p.stride_bytes, p.a);
+                }
                 const unsigned code = op & 0xffu;
                 if (code == MC_END || code == MC_FINAL) break;
                 const unsigned nxt = s_mops[pc + 1];
@@ -451,9 +507,7 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
                 }
                 wmax = fmaxf(wmax, mx + cthr);
             } else {
-#ifndef TTN_NO_STORE_SYNC
                 if (!LOW) group_sync(warp);
-#endif
                 if (LOW || p.last_layout == 1) gmove<LOW, 1, true>(v, S + base, lane, p.stride_bytes, p.a);
                 else gmove<LOW, 0, true>(v, S + base, lane, p.stride_bytes, p.a);
             }
