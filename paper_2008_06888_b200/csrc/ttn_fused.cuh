@@ -177,11 +177,7 @@ template <bool LOW, int K> struct Nbr {
 template <bool LOW>
 __device__ __forceinline__ void fround(float (&v)[128], const unsigned mask, const ulonglong2* __restrict__& gk,
                                        ulonglong2& n0, ulonglong2& n1, const int tp, const int tq) {
-#ifdef TTN_NO_PREFETCH
-#define TTN_FETCHK const ulonglong2 c0 = gk[0], c1 = gk[1]; gk += 2;
-#else
 #define TTN_FETCHK const ulonglong2 c0 = n0, c1 = n1; gk += 2; n0 = gk[0]; n1 = gk[1];
-#endif
 #define TTN_G(Kk)                                                                                   \
     if (mask & (1u << Kk)) {                                                                        \
         TTN_FETCHK                                                                                  \
@@ -282,11 +278,7 @@ __device__ __forceinline__ unsigned long long addr_mad(unsigned long long gbase,
 }
 __device__ __forceinline__ float ldg_f32(unsigned long long ga) {
     float x;
-#ifdef TTN_HIGH_LD128
-    asm volatile("ld.global.L2::128B.f32 %0, [%1];" : "=f"(x) : "l"(ga));
-#else
     asm volatile("ld.global.f32 %0, [%1];" : "=f"(x) : "l"(ga));
-#endif
     return x;
 }
 __device__ __forceinline__ void stg_f32(unsigned long long ga, float x) {
@@ -364,9 +356,7 @@ __device__ __forceinline__ void pf_read(float (&v)[128], const float4* region, i
 
 // named barrier of one 4-warp group (barrier 0 is __syncthreads)
 __device__ __forceinline__ void group_sync(int warp) {
-#ifndef TTN_NO_GROUPSYNC
     asm volatile("bar.sync %0, 128;" :: "r"(1 + (warp >> 2)) : "memory");
-#endif
 }
 
 template <bool LOW>

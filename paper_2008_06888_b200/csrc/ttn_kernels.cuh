@@ -116,18 +116,34 @@ __global__ void __launch_bounds__(512) pass_kernel(const PassParams p) {
     __syncthreads();
 
     // ---- gate list -------------------------------------------------------------------------------
+    // Per-gate index constants (digit weight, division magics, where the neighbour digits come
+    // from) are computed once per gate by ONE thread each into shared memory, not by every thread
+    // (the 64-bit division behind fastdiv_magic is a subroutine call).
+    constexpr int GCHUNK = 256;
+    __shared__ uint4 s_aux[GCHUNK];          // x = st, y = magic(st), z = magic(st / Q), w = flags
     const float* GK = p.gate_k + inst * p.gate_inst_stride;
     for (int k = 0; k < p.n_ops; ++k) {
+        if (k % GCHUNK == 0) {
+            for (int i = threadIdx.x; i < GCHUNK && k + i < p.n_ops; i += blockDim.x) {
+                const Op o = p.ops[k + i];
+                unsigned s_ = 1;
+                for (int j = 0; j < o.pos; ++j) s_ *= Q;
+                const unsigned sq = o.pos > 0 ? s_ / Q : 1;
+                const bool li = o.pos > 0 && tile_col(p, o.pos - 1) == o.c - 1;
+                const bool ri = o.pos + 1 < p.T && tile_col(p, o.pos + 1) == o.c + 1;
+                const int dlo = o.c > 0 ? s_dig[o.c - 1] : 0, dro = o.c + 1 < p.L ? s_dig[o.c + 1] : 0;
+                s_aux[i] = make_uint4(s_, fastdiv_magic(s_), fastdiv_magic(sq),
+                                      (unsigned)li | ((unsigned)ri << 1) | ((unsigned)dlo << 2) | ((unsigned)dro << 4));
+            }
+            __syncthreads();
+        }
         const Op op = p.ops[k];
-        const int pos = op.pos, c = op.c;
-        unsigned st = 1;
-        for (int i = 0; i < pos; ++i) st *= Q;
-        const unsigned st_q = pos > 0 ? st / Q : 1;             // weight of the digit at position pos-1
-        const unsigned m_st = fastdiv_magic(st), m_stq = fastdiv_magic(st_q);
-        // neighbour columns: inside the tile (digit taken from the tile-local index) or outside (s_dig)
-        const bool l_in = pos > 0 && tile_col(p, pos - 1) == c - 1;
-        const bool r_in = pos + 1 < p.T && tile_col(p, pos + 1) == c + 1;
-        const int dl_out = c > 0 ? s_dig[c - 1] : 0, dr_out = c + 1 < p.L ? s_dig[c + 1] : 0;
+        const int pos = op.pos;
+        const uint4 aux = s_aux[k % GCHUNK];
+        const unsigned st = aux.x, m_st = aux.y, m_stq = aux.z;
+        const unsigned st_q = pos > 0 ? st / Q : 1;
+        const bool l_in = aux.w & 1u, r_in = (aux.w >> 1) & 1u;
+        const int dl_out = (int)((aux.w >> 2) & 3u), dr_out = (int)((aux.w >> 4) & 3u);
         const float4 k0 = reinterpret_cast<const float4*>(GK)[2 * k], k1 = reinterpret_cast<const float4*>(GK)[2 * k + 1];
         const unsigned ngrp = N / Q;
         for (unsigned g = threadIdx.x; g < ngrp; g += blockDim.x) {
