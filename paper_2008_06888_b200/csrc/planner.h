@@ -255,6 +255,21 @@ constexpr int fused_bit_of_digit(bool low, int layout, int d) {
     return -1;
 }
 
+// Tile geometry of a fused kernel family.  kind 0: Tropical<f32>, 128 elements per thread (7
+// register digits, maps above).  kind 1: CountingTropical<f32,f64>, 32 elements per thread (5
+// register digits; a tile is 2^10 elements: LOW = columns 0..9, HIGH = 3 riding + 7 active);
+// there register bit i holds chain position i: digit i in layout A, digit W-1-i in layout B.
+struct FusedGeom { int RB, WLOW, WHIGH, RIDE, AMIN, kind; };
+constexpr FusedGeom GEOM_F32{F_RB, F_WLOW, F_WHIGH, F_RIDE, F_AMIN, 0};
+constexpr FusedGeom GEOM_COUNT{5, 10, 7, 3, 4, 1};
+#if defined(__CUDACC__)
+__host__ __device__
+#endif
+constexpr int geom_digit_of_bit(const FusedGeom& g, bool low, int layout, int bit) {
+    return g.kind == 0 ? fused_digit_of_bit(low, layout, bit)
+                       : (layout == 0 ? bit : (low ? g.WLOW : g.WHIGH) - 1 - bit);
+}
+
 struct FusedPass {
     int a, W;                    // active digits [a, a+W)
     int low;                     // 1 = low tile
@@ -275,7 +290,7 @@ struct FusedPlan {
 
 class FusedScheduler {
   public:
-    FusedScheduler(int L, FusedPlan& p) : L_(L), Pp_(&p), grow_(L, 1) {}
+    FusedScheduler(int L, FusedPlan& p, const FusedGeom& g = GEOM_F32) : L_(L), Pp_(&p), G_(g), grow_(L, 1) {}
     void rebind(FusedPlan& p) { Pp_ = &p; }
     bool done() const {
         for (int c = 0; c < L_; ++c) if (grow_[c] != L_) return false;
@@ -283,7 +298,7 @@ class FusedScheduler {
     }
     // One pass over active digits [a, a+W).  Returns number of gates applied.
     int run_pass(int a, bool low, int max_gates, FusedPass& ps) {
-        const int W = low ? F_WLOW : F_WHIGH;
+        const int W = low ? G_.WLOW : G_.WHIGH;
         ps.a = a; ps.W = W; ps.low = low; ps.flags = 0; ps.n_phases = 0; ps.n_rounds = 0;
         ps.mop_begin = (int)Pp_->mops.size(); ps.gate_begin = (int)Pp_->gate_rc.size();
         pass_gate_begin_ = ps.gate_begin; pass_mop_begin_ = ps.mop_begin; max_gates_ = max_gates;
@@ -320,23 +335,23 @@ class FusedScheduler {
     int run_phase(int a, bool low, int layout, int& rounds) {
         int n = 0;
         for (;;) {
-            if ((int)Pp_->gate_rc.size() - pass_gate_begin_ + F_RB > max_gates_) break;
+            if ((int)Pp_->gate_rc.size() - pass_gate_begin_ + G_.RB > max_gates_) break;
             if ((int)Pp_->mops.size() - pass_mop_begin_ + 8 > max_mops_) break;
             unsigned mask = 0;
-            for (int b = 0; b < F_RB; ++b) if (legal(a + fused_digit_of_bit(low, layout, b))) mask |= 1u << b;
+            for (int b = 0; b < G_.RB; ++b) if (legal(a + geom_digit_of_bit(G_, low, layout, b))) mask |= 1u << b;
             if (!mask) break;
             Pp_->mops.push_back({MC_ROUND, (uint8_t)mask, (uint16_t)((int)Pp_->gate_rc.size() - pass_gate_begin_)});
-            for (int b = 0; b < F_RB; ++b) if (mask >> b & 1) {
-                const int c = a + fused_digit_of_bit(low, layout, b);
+            for (int b = 0; b < G_.RB; ++b) if (mask >> b & 1) {
+                const int c = a + geom_digit_of_bit(G_, low, layout, b);
                 Pp_->gate_rc.push_back((low ? 1 << 16 : 0) | (b << 13) | (layout << 12) | (grow_[c] << 6) | c);
                 ++n;
             }
-            for (int b = 0; b < F_RB; ++b) if (mask >> b & 1) grow_[a + fused_digit_of_bit(low, layout, b)] += 1;
+            for (int b = 0; b < G_.RB; ++b) if (mask >> b & 1) grow_[a + geom_digit_of_bit(G_, low, layout, b)] += 1;
             ++rounds;
         }
         return n;
     }
-    int L_; FusedPlan* Pp_;
+    int L_; FusedPlan* Pp_; FusedGeom G_;
     std::vector<int> grow_;      // grow[c] = rows complete on digit c (row 0 needs no gate)
     int pass_gate_begin_ = 0, pass_mop_begin_ = 0, max_gates_ = 1 << 30;
     int max_mops_ = 120;         // micro-ops per pass the kernel stages (FMAX_MOPS = 128)
@@ -356,9 +371,9 @@ inline double fused_pass_cost(const FusedPass& ps) {
 //  * cyclic: the low tile [0,12), then high tiles [x, x+9) advancing by `stride`, the last flush
 //    with L, for every stride;
 //  * greedy: at every step the tile (low, or high at any start) that applies the most gates.
-inline FusedPlan make_fused_plan(int L, int max_gates_per_pass) {
+inline FusedPlan make_fused_plan(int L, int max_gates_per_pass, const FusedGeom& G = GEOM_F32) {
     FusedPlan best;
-    if (L < F_WLOW) return best;
+    if (L < G.WLOW) return best;
     double best_cost = -1;
     auto finish = [&](FusedPlan& p) {
         // the last pass adds A_{L-1}(s) and reduces: MC_FINAL replaces its MC_END
@@ -368,21 +383,21 @@ inline FusedPlan make_fused_plan(int L, int max_gates_per_pass) {
         for (auto& ps : p.passes) cost += fused_pass_cost(ps);
         if (best_cost < 0 || cost < best_cost) { best = p; best_cost = cost; best.ok = true; }
     };
-    for (int stride = 1; stride <= F_WHIGH; ++stride) {
+    for (int stride = 1; stride <= G.WHIGH; ++stride) {
         std::vector<int> starts;
         starts.push_back(0);
-        if (L > F_WLOW) {
-            int x = F_WLOW - (F_WHIGH - stride);
+        if (L > G.WLOW) {
+            int x = G.WLOW - (G.WHIGH - stride);
             for (;;) {
-                if (x + F_WHIGH >= L) x = L - F_WHIGH;
-                if (x < F_AMIN) x = F_AMIN;
+                if (x + G.WHIGH >= L) x = L - G.WHIGH;
+                if (x < G.AMIN) x = G.AMIN;
                 starts.push_back(x);
-                if (x + F_WHIGH >= L) break;
+                if (x + G.WHIGH >= L) break;
                 x += stride;
             }
         }
         FusedPlan p; p.L = L;
-        FusedScheduler s(L, p);
+        FusedScheduler s(L, p, G);
         size_t k = 0; int idle = 0; bool first = true;
         while ((first || !s.done()) && p.passes.size() < 4096) {
             int a = starts[k % starts.size()]; ++k;
@@ -398,13 +413,13 @@ inline FusedPlan make_fused_plan(int L, int max_gates_per_pass) {
         if (!s.done()) continue;
         finish(p);
     }
-    if (L > F_WLOW) {                               // greedy by gate count
+    if (L > G.WLOW) {                               // greedy by gate count
         FusedPlan p; p.L = L;
-        FusedScheduler s(L, p);
+        FusedScheduler s(L, p, G);
         bool first = true;
         while ((first || !s.done()) && p.passes.size() < 4096) {
             int best_a = -1, best_n = -1; double best_c = 0;
-            for (int a = 0; a + F_WHIGH <= L; a = (a == 0 ? F_AMIN : a + 1)) {
+            for (int a = 0; a + G.WHIGH <= L; a = (a == 0 ? G.AMIN : a + 1)) {
                 FusedScheduler trial = s;                       // dry run on a copy
                 FusedPlan scratch; scratch.L = L;
                 trial.rebind(scratch);

@@ -15,6 +15,7 @@
 #include "planner.h"
 #include "ttn_kernels.cuh"
 #include "ttn_fused.cuh"
+#include "ttn_fcount.cuh"
 
 namespace {
 
@@ -76,10 +77,12 @@ struct Layout {
     int f_max_gates = 0, f_max_mops = 0;
 };
 
-// The fused register-phase path serves the Ising Tropical<f32> energy sweep for L >= 12.
+// The fused register-phase paths: Ising Tropical<f32> energy for L >= 12 (ttn_fused.cuh) and Ising
+// CountingTropical<f32,f64> for L >= 10 (ttn_fcount.cuh).
 bool fused_eligible(int q, int L, bool count, bool config) {
     if (const char* e = getenv("TTN_DEBUG_FUSED")) if (atoi(e) == 0) return false;
-    return q == 2 && !count && !config && L >= ttn::F_WLOW;
+    if (q != 2 || config) return false;
+    return count ? L >= ttn::CW_LOW : L >= ttn::F_WLOW;
 }
 
 // The op list length is bounded by L*L gates + 2*L*L diagonals.
@@ -89,7 +92,7 @@ Layout make_layout(int q, int L, bool count, bool config, int batch) {
     const TileCfg tc = tile_cfg(q, count);
     // every pass of a plan stages tiles of q^min(L, Tmax) elements
     y.max_tiles = y.NS / ipow(q, tc.Tmax < L ? tc.Tmax : L);
-    if (fused_eligible(q, L, count, config) && (y.NS >> 12) > y.max_tiles) y.max_tiles = y.NS >> 12;
+    if (fused_eligible(q, L, count, config) && y.max_tiles < 1024) y.max_tiles = 1024;   // one partial per CTA
     if (y.max_tiles == 0) y.max_tiles = 1;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
@@ -238,6 +241,83 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
     return TTN_OK;
 }
 
+static ttn_status launch_fcount_pass(const ttn_plan* P, const ttn::FusedPass& ps, cudaStream_t st) {
+    const Layout& y = P->lay;
+    const ttn::FusedPlan& fp = P->fplan;
+    ttn::CountParams cp{};
+    ttn::FusedParams& pp = cp.f;
+    pp.L = P->L; pp.a = ps.a; pp.low = ps.low; pp.flags = ps.flags; pp.batch = P->batch;
+    pp.first_layout = ps.first_layout; pp.last_layout = ps.last_layout;
+    pp.state = reinterpret_cast<float*>(P->ws + y.x);
+    cp.state_n = reinterpret_cast<double*>(P->ws + y.n);
+    pp.inst_stride = y.NS;
+    pp.tiles_per_inst = y.NS >> 10;
+    pp.mops = reinterpret_cast<const ttn::MicroOp*>(P->ws + y.f_mops) + ps.mop_begin;
+    pp.n_mops = ps.mop_end - ps.mop_begin;
+    pp.gate_k = reinterpret_cast<const float*>(P->ws + y.f_gate_k) + (size_t)ps.gate_begin * 8;
+    pp.n_gates = ps.gate_end - ps.gate_begin;
+    pp.gate_inst_stride = (unsigned long long)fp.gate_rc.size() * 8;
+    pp.final_tab = reinterpret_cast<const float*>(P->ws + y.f_final);
+    pp.part_x = reinterpret_cast<float*>(P->ws + y.part_x);
+    cp.part_n = reinterpret_cast<double*>(P->ws + y.part_n);
+    pp.stride_bytes = 4u << ps.a;
+    pp.prefetch_pc = -1;
+    unsigned long long grid = (unsigned long long)P->fused_grid;
+    const int nw = ttn::CWARPS;
+    pp.cta_per_inst = (P->batch > 1 && pp.tiles_per_inst < (unsigned long long)nw * grid) ? 1 : 0;
+    if (pp.cta_per_inst) {
+        if (grid > (unsigned long long)P->batch) grid = (unsigned long long)P->batch;
+    } else {
+        const unsigned long long need = (pp.tiles_per_inst + nw - 1) / nw;
+        if (grid > need) grid = need;
+    }
+    pp.part_stride = pp.cta_per_inst ? 1 : (int)grid;
+    if (ps.low) ttn::fcount_pass_kernel<true><<<(unsigned)grid, nw * 32, ttn::csmem_bytes(), st>>>(cp);
+    else ttn::fcount_pass_kernel<false><<<(unsigned)grid, nw * 32, ttn::csmem_bytes(), st>>>(cp);
+    TTN_CUDA(cudaGetLastError());
+    if (ps.flags & ttn::PASS_REDUCE) {
+        ttn::final_reduce_kernel<true><<<P->batch, 256, 0, st>>>(
+            pp.part_x, cp.part_n, (unsigned long long)pp.part_stride, reinterpret_cast<float*>(P->ws + y.out_x),
+            reinterpret_cast<double*>(P->ws + y.out_n));
+        TTN_CUDA(cudaGetLastError());
+    }
+    return TTN_OK;
+}
+
+static ttn_status setup_fcount(ttn_plan* P, cudaStream_t st) {
+    const Layout& y = P->lay;
+    ttn::FusedPlan& fp = P->fplan;
+    if ((int)fp.gate_rc.size() > y.f_max_gates || (int)fp.mops.size() > y.f_max_mops)
+        return fail(TTN_EUNSUPPORTED, "fused plan exceeds its workspace bounds");
+    for (const auto& ps : fp.passes)
+        if (ps.mop_end - ps.mop_begin > ttn::FMAX_MOPS || ps.gate_end - ps.gate_begin > ttn::FMAX_GATES ||
+            (ps.low && (ps.first_layout != 1 || ps.last_layout != 1)))
+            return fail(TTN_EUNSUPPORTED, "fused pass program out of bounds");
+    TTN_CUDA(cudaMemcpyAsync(P->ws + y.f_mops, fp.mops.data(), fp.mops.size() * sizeof(ttn::MicroOp), cudaMemcpyHostToDevice, st));
+    TTN_CUDA(cudaMemcpyAsync(P->ws + y.f_gate_rc, fp.gate_rc.data(), fp.gate_rc.size() * 4, cudaMemcpyHostToDevice, st));
+    ttn::CountPrepParams q{};
+    q.L = P->L; q.n_gates = (int)fp.gate_rc.size();
+    q.gate_rc = reinterpret_cast<const int*>(P->ws + y.f_gate_rc);
+    q.Jh = reinterpret_cast<const float*>(P->ws + y.Jh);
+    q.Jv = reinterpret_cast<const float*>(P->ws + y.Jv);
+    q.h = P->has_field ? reinterpret_cast<const float*>(P->ws + y.h) : nullptr;
+    q.gate_k = reinterpret_cast<float*>(P->ws + y.f_gate_k);
+    q.final_tab = reinterpret_cast<float*>(P->ws + y.f_final);
+    const ttn::FusedPass& lastp = fp.passes.back();
+    q.fin_low = lastp.low; q.fin_layout = lastp.last_layout; q.fin_a = lastp.a;
+    long work = ttn::CFINAL_FLOATS; if (q.n_gates > work) work = q.n_gates;
+    dim3 grid((unsigned)((work + 255) / 256), (unsigned)P->batch);
+    ttn::fcount_prep_kernel<<<grid, 256, 0, st>>>(q);
+    TTN_CUDA(cudaGetLastError());
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fcount_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::csmem_bytes()));
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fcount_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::csmem_bytes()));
+    int dev = 0, sms = 0;
+    TTN_CUDA(cudaGetDevice(&dev));
+    TTN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    P->fused_grid = sms;
+    return TTN_OK;
+}
+
 // Uploads the fused program and runs the S0 prep kernel (gate constants + final table).
 static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
     const Layout& y = P->lay;
@@ -294,7 +374,8 @@ long ttn_plan_describe(int q, int L, ttn_call call, char* buf, size_t n) {
     if (!limits_ok(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) return -1;
     std::string s;
     if (fused_eligible(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) {
-        ttn::FusedPlan fp = ttn::make_fused_plan(L, ttn::FMAX_GATES);
+        ttn::FusedPlan fp = call == TTN_CALL_COUNT ? ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_COUNT)
+                                                   : ttn::make_fused_plan(L, ttn::FMAX_GATES);
         if (fp.ok) s = ttn::describe_fused(fp);
     }
     if (s.empty()) s = ttn::describe(plan_for(q, L, call, /*has_field=*/q == 2));
@@ -340,7 +421,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     P->lay = lay;
     P->ws = static_cast<unsigned char*>(workspace);
     if (fused_eligible(q, L, count, config)) {
-        P->fplan = ttn::make_fused_plan(L, ttn::FMAX_GATES);
+        P->fplan = count ? ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_COUNT) : ttn::make_fused_plan(L, ttn::FMAX_GATES);
         P->fused = P->fplan.ok;
     }
     if (!P->fused) P->plan = plan_for(q, L, call, P->has_field);
@@ -368,7 +449,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     if (e != cudaSuccess) { delete P; return fail(TTN_ECUDA, "coupling upload failed: %s", cudaGetErrorString(e)); }
 
     if (P->fused) {
-        ttn_status fs = setup_fused(P, st);
+        ttn_status fs = count ? setup_fcount(P, st) : setup_fused(P, st);
         if (fs != TTN_OK) { delete P; return fs; }
         P->launches = (int)P->fplan.passes.size() + 1;
     } else {
@@ -399,7 +480,7 @@ ttn_status ttn_plan_launch(ttn_plan* P, void* stream) {
         if (timing) { ev.resize(P->fplan.passes.size() + 1); for (auto& e : ev) cudaEventCreate(&e); cudaEventRecord(ev[0], st); }
         size_t k = 0;
         for (const ttn::FusedPass& ps : P->fplan.passes) {
-            ttn_status s = launch_fused_pass(P, ps, st);
+            ttn_status s = P->count ? launch_fcount_pass(P, ps, st) : launch_fused_pass(P, ps, st);
             if (s != TTN_OK) return s;
             if (timing) cudaEventRecord(ev[++k], st);
         }

@@ -137,14 +137,21 @@ def parse_fused(txt):
     return head, passes
 
 
-def fused_to_gates(L, fpasses):
+# counting geometry (csrc/planner.h GEOM_COUNT): 5 register digits, bit i = chain position i
+DIGIT_OF_BIT_COUNT = {(1, 0): [0, 1, 2, 3, 4], (1, 1): [9, 8, 7, 6, 5],
+                      (0, 0): [0, 1, 2, 3, 4], (0, 1): [6, 5, 4, 3, 2]}
+
+
+def fused_to_gates(L, fpasses, count=False):
     """Check the structure of the micro-op program (layouts, register bits, rounds) and the
     three-point-stencil dependency rule; return the flat (r, c) gate sequence."""
     flat = []
     grow = [1] * L                                   # rows complete per digit (row 0 needs no gate)
     for i, ps in enumerate(fpasses):
         a, Wt, low = ps["a"], ps["W"], ps["low"]
-        assert (low == 1 and a == 0 and Wt == 12) or (low == 0 and a >= 4 and Wt == 9)
+        wl, wh, rb = (10, 7, 5) if count else (12, 9, 7)
+        dmap = DIGIT_OF_BIT_COUNT if count else DIGIT_OF_BIT
+        assert (low == 1 and a == 0 and Wt == wl) or (low == 0 and a >= 4 and Wt == wh)
         assert a + Wt <= L
         assert (ps["flags"] & 1) == (1 if i == 0 else 0)
         last = i == len(fpasses) - 1
@@ -164,13 +171,13 @@ def fused_to_gates(L, fpasses):
                 assert layout == 1
                 layout = 0
             else:
-                assert code == "round" and 0 < m["mask"] < 128 and m["first"] == ngates
-                bits = [k for k in range(7) if m["mask"] >> k & 1]
+                assert code == "round" and 0 < m["mask"] < (1 << rb) and m["first"] == ngates
+                bits = [k for k in range(rb) if m["mask"] >> k & 1]
                 assert [g["k"] for g in m["gates"]] == bits          # ascending register bits
                 before = list(grow)
                 for g in m["gates"]:
                     c, r = g["c"], g["r"]
-                    assert c == a + DIGIT_OF_BIT[(low, layout)][g["k"]]      # register bit <-> column
+                    assert c == a + dmap[(low, layout)][g["k"]]      # register bit <-> column
                     assert g["layout"] == layout
                     # legal at the START of the round: every gate of a round commutes with the others
                     assert 1 <= r < L and before[c] == r
@@ -221,6 +228,14 @@ def replay_diagonal_frame(L, gates, Jh, Jv, h):
             A += Kacc[L - 1, c] * sig[c] * sig[c + 1]
     m = (V + A).max() + defer
     return 0.0 if m == 0 else -m
+
+
+@pytest.mark.parametrize("L", [10, 11, 12, 14, 17, 20, 24, 28, 32])
+def test_fused_count_schedule_obeys_dependency_rule(L):
+    head, fpasses = parse_fused(describe(2, L, 1, fused=True))
+    assert int(head["L"]) == L
+    flat = fused_to_gates(L, fpasses, count=True)
+    assert len(flat) == L * (L - 1) == len(set(flat))
 
 
 @pytest.mark.parametrize("L", [12, 13, 16])
