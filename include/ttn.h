@@ -56,7 +56,9 @@ typedef enum {
 
 typedef enum {
     TTN_TROPICAL_F32 = 0,      /* Eq. (2): x (+) y = max, x (.) y = x + y                      */
-    TTN_COUNTING_F32_F64 = 1   /* Eq. (4): (x, n) tuples, n summed on exact ties               */
+    TTN_COUNTING_F32_F64 = 1,  /* Eq. (4): (x, n) tuples, n summed on exact ties               */
+    TTN_TROPICAL_I16 = 2       /* Eq. (2) on 16-bit integers: integer-valued couplings only, the
+                                  paper's own element type for +-J           */
 } ttn_semiring;
 
 /* Limits: Ising tropical L <= 34, Ising counting L <= 32, Potts L <= 20 (index fits 32 bits);
@@ -71,6 +73,14 @@ size_t ttn_workspace_bytes(int q, int L, ttn_semiring mode, int batch, int want_
 ttn_status ttn_sweep_energy(int L, const float* Jh, const float* Jv, const float* h, int batch,
                             void* workspace, size_t workspace_bytes, void* stream,
                             double* E0 /*[batch]*/);
+
+/* Same result as ttn_sweep_energy, computed in Tropical<i16> (two state elements per 32-bit word,
+   packed add-max): half the state (2^L x 2 bytes) and twice the update rate.  EXACT, and only for
+   integer-valued couplings with sum|Jh| + sum|Jv| + sum|h| <= 8000 per instance (every
+   intermediate then fits 16 bits); anything else returns TTN_EINVAL.  L < 13 runs the f32 path. */
+ttn_status ttn_sweep_energy_i16(int L, const float* Jh, const float* Jv, const float* h, int batch,
+                                void* workspace, size_t workspace_bytes, void* stream,
+                                double* E0 /*[batch]*/);
 
 /* Ground-state energy and degeneracy, CountingTropical sweep (Eq. (4)). */
 ttn_status ttn_sweep_count(int L, const float* Jh, const float* Jv, const float* h, int batch,
@@ -102,7 +112,7 @@ ttn_status ttn_potts3_sweep_count(int L, const float* Jh, const float* Jv, int b
  *   ttn_plan_read   : device->host copy of the results of the last launch; synchronises.
  *                     Pointers that do not apply to the plan's call kind must be NULL.      */
 typedef struct ttn_plan ttn_plan;
-typedef enum { TTN_CALL_ENERGY = 0, TTN_CALL_COUNT = 1, TTN_CALL_CONFIG = 2 } ttn_call;
+typedef enum { TTN_CALL_ENERGY = 0, TTN_CALL_COUNT = 1, TTN_CALL_CONFIG = 2, TTN_CALL_ENERGY_I16 = 3 } ttn_call;
 
 ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const float* Jv,
                            const float* h, int batch, void* workspace, size_t workspace_bytes,

@@ -255,19 +255,30 @@ constexpr int fused_bit_of_digit(bool low, int layout, int d) {
     return -1;
 }
 
-// Tile geometry of a fused kernel family.  kind 0: Tropical<f32>, 128 elements per thread (7
-// register digits, maps above).  kind 1: CountingTropical<f32,f64>, 32 elements per thread (5
-// register digits; a tile is 2^10 elements: LOW = columns 0..9, HIGH = 3 riding + 7 active);
-// there register bit i holds chain position i: digit i in layout A, digit W-1-i in layout B.
+// Tile geometry of a fused kernel family.
+//  kind 0: Tropical<f32>, 128 elements per thread (7 register digits, maps above).
+//  kind 1: CountingTropical<f32,f64>, 32 elements per thread (5 register digits; a tile is 2^10
+//          elements: LOW = columns 0..9, HIGH = 3 riding + 7 active); register bit i holds chain
+//          position i: digit i in layout A, digit W-1-i in layout B.
+//  kind 2: Tropical<i16>, two elements per 32-bit word: column 0 is the HALF of a word and the
+//          kind-0 geometry applies to the word index (column c >= 1 = word digit c-1).  The LOW
+//          tile has 13 columns; pseudo register bit 7 is the half digit (in every LOW layout);
+//          HIGH tiles start at column a >= 5 (word digit a-1) and column 0 rides.
 struct FusedGeom { int RB, WLOW, WHIGH, RIDE, AMIN, kind; };
 constexpr FusedGeom GEOM_F32{F_RB, F_WLOW, F_WHIGH, F_RIDE, F_AMIN, 0};
 constexpr FusedGeom GEOM_COUNT{5, 10, 7, 3, 4, 1};
+constexpr FusedGeom GEOM_I16{F_RB, F_WLOW + 1, F_WHIGH, F_RIDE + 1, F_AMIN + 1, 2};
+#if defined(__CUDACC__)
+__host__ __device__
+#endif
+constexpr int geom_bits(const FusedGeom& g, bool low) { return g.kind == 2 && low ? g.RB + 1 : g.RB; }
 #if defined(__CUDACC__)
 __host__ __device__
 #endif
 constexpr int geom_digit_of_bit(const FusedGeom& g, bool low, int layout, int bit) {
     return g.kind == 0 ? fused_digit_of_bit(low, layout, bit)
-                       : (layout == 0 ? bit : (low ? g.WLOW : g.WHIGH) - 1 - bit);
+         : g.kind == 1 ? (layout == 0 ? bit : (low ? g.WLOW : g.WHIGH) - 1 - bit)
+         : (low ? (bit == F_RB ? 0 : 1 + fused_digit_of_bit(true, layout, bit)) : fused_digit_of_bit(false, layout, bit));
 }
 
 struct FusedPass {
@@ -335,18 +346,19 @@ class FusedScheduler {
     int run_phase(int a, bool low, int layout, int& rounds) {
         int n = 0;
         for (;;) {
-            if ((int)Pp_->gate_rc.size() - pass_gate_begin_ + G_.RB > max_gates_) break;
+            const int nb = geom_bits(G_, low);
+            if ((int)Pp_->gate_rc.size() - pass_gate_begin_ + nb > max_gates_) break;
             if ((int)Pp_->mops.size() - pass_mop_begin_ + 8 > max_mops_) break;
             unsigned mask = 0;
-            for (int b = 0; b < G_.RB; ++b) if (legal(a + geom_digit_of_bit(G_, low, layout, b))) mask |= 1u << b;
+            for (int b = 0; b < nb; ++b) if (legal(a + geom_digit_of_bit(G_, low, layout, b))) mask |= 1u << b;
             if (!mask) break;
             Pp_->mops.push_back({MC_ROUND, (uint8_t)mask, (uint16_t)((int)Pp_->gate_rc.size() - pass_gate_begin_)});
-            for (int b = 0; b < G_.RB; ++b) if (mask >> b & 1) {
+            for (int b = 0; b < nb; ++b) if (mask >> b & 1) {
                 const int c = a + geom_digit_of_bit(G_, low, layout, b);
                 Pp_->gate_rc.push_back((low ? 1 << 16 : 0) | (b << 13) | (layout << 12) | (grow_[c] << 6) | c);
                 ++n;
             }
-            for (int b = 0; b < G_.RB; ++b) if (mask >> b & 1) grow_[a + geom_digit_of_bit(G_, low, layout, b)] += 1;
+            for (int b = 0; b < nb; ++b) if (mask >> b & 1) grow_[a + geom_digit_of_bit(G_, low, layout, b)] += 1;
             ++rounds;
         }
         return n;
@@ -462,7 +474,7 @@ inline std::string describe_fused(const FusedPlan& p) {
                     snprintf(line, sizeof line, "m round mask=%d first=%d\n", m.mask, m.arg);
                     out += line;
                     int g = ps.gate_begin + m.arg;
-                    for (int b = 0; b < F_RB; ++b) if (m.mask >> b & 1) {
+                    for (int b = 0; b < 8; ++b) if (m.mask >> b & 1) {
                         const int rc = p.gate_rc[g++];
                         snprintf(line, sizeof line, "g k=%d r=%d c=%d layout=%d\n", (rc >> 13) & 7, (rc >> 6) & 63, rc & 63, (rc >> 12) & 1);
                         out += line;

@@ -79,6 +79,10 @@ struct Layout {
 
 // The fused register-phase paths: Ising Tropical<f32> energy for L >= 12 (ttn_fused.cuh) and Ising
 // CountingTropical<f32,f64> for L >= 10 (ttn_fcount.cuh).
+bool i16_eligible(int q, int L) {
+    if (const char* e = getenv("TTN_DEBUG_FUSED")) if (atoi(e) == 0) return false;
+    return q == 2 && L >= ttn::GEOM_I16.WLOW;
+}
 bool fused_eligible(int q, int L, bool count, bool config) {
     if (const char* e = getenv("TTN_DEBUG_FUSED")) if (atoi(e) == 0) return false;
     if (q != 2 || config) return false;
@@ -86,7 +90,7 @@ bool fused_eligible(int q, int L, bool count, bool config) {
 }
 
 // The op list length is bounded by L*L gates + 2*L*L diagonals.
-Layout make_layout(int q, int L, bool count, bool config, int batch) {
+Layout make_layout(int q, int L, bool count, bool config, int batch, bool i16 = false) {
     Layout y;
     y.NS = ipow(q, L);
     const TileCfg tc = tile_cfg(q, count);
@@ -96,7 +100,7 @@ Layout make_layout(int q, int L, bool count, bool config, int batch) {
     if (y.max_tiles == 0) y.max_tiles = 1;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
-    y.x = take((size_t)batch * y.NS * 4);
+    y.x = take((size_t)batch * y.NS * (i16 ? 2 : 4));
     if (count) y.n = take((size_t)batch * y.NS * 8);
     if (config) y.ckpt = take((size_t)batch * L * y.NS * 4);
     y.Jh = take((size_t)batch * L * (L - 1) * 4 + 4);
@@ -140,7 +144,7 @@ struct ttn_plan {
     bool count, config, has_field;
     ttn::Plan plan;
     ttn::FusedPlan fplan;
-    bool fused = false;
+    bool fused = false, i16 = false;
     int fused_grid = 0;
     Layout lay;
     unsigned char* ws;
@@ -206,6 +210,12 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
     pp.state = reinterpret_cast<float*>(P->ws + y.x);
     pp.inst_stride = y.NS;
     pp.tiles_per_inst = y.NS >> 12;
+    pp.L_cols = P->L;
+    if (P->i16) {           // the kernel sees the lattice of 32-bit words: column c >= 1 = word digit c - 1
+        pp.L = P->L - 1; pp.a = ps.low ? 0 : ps.a - 1;
+        pp.inst_stride = y.NS >> 1; pp.tiles_per_inst = y.NS >> 13;
+    }
+    const int a_mem = pp.a;
     pp.mops = reinterpret_cast<const ttn::MicroOp*>(P->ws + y.f_mops) + ps.mop_begin;
     pp.n_mops = ps.mop_end - ps.mop_begin;
     pp.gate_k = reinterpret_cast<const float*>(P->ws + y.f_gate_k) + (size_t)ps.gate_begin * 8;
@@ -213,11 +223,11 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
     pp.gate_inst_stride = (unsigned long long)fp.gate_rc.size() * 8;
     pp.final_tab = reinterpret_cast<const float*>(P->ws + y.f_final);
     pp.part_x = reinterpret_cast<float*>(P->ws + y.part_x);
-    pp.stride_bytes = 4u << ps.a;     // a <= L - 9 <= 25
+    pp.stride_bytes = 4u << a_mem;    // a <= L - 9 <= 25
     pp.prefetch_pc = 0;
     for (int k = ps.mop_begin; k < ps.mop_end; ++k)
         if (fp.mops[k].code == ttn::MC_XAB || fp.mops[k].code == ttn::MC_XBA) pp.prefetch_pc = k - ps.mop_begin + 1;
-    if (ps.a > 18) pp.prefetch_pc = -1;      // > 256 distinct 2 MiB pages per tile: synchronous loads
+    if (a_mem > 18) pp.prefetch_pc = -1;     // > 256 distinct 2 MiB pages per tile: synchronous loads
     unsigned long long grid = (unsigned long long)P->fused_grid;
     const int nw = ttn::fwarps(ps.low != 0);
     // batches of small lattices: one CTA per instance at a time instead of the whole grid per instance
@@ -229,8 +239,13 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
         if (grid > need) grid = need;
     }
     pp.part_stride = pp.cta_per_inst ? 1 : (int)grid;
-    if (ps.low) ttn::fused_pass_kernel<true><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(true), st>>>(pp);
-    else ttn::fused_pass_kernel<false><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(false), st>>>(pp);
+    if (P->i16) {
+        if (ps.low) ttn::fused_pass_kernel<true, 1><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(true), st>>>(pp);
+        else ttn::fused_pass_kernel<false, 1><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(false), st>>>(pp);
+    } else {
+        if (ps.low) ttn::fused_pass_kernel<true><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(true), st>>>(pp);
+        else ttn::fused_pass_kernel<false><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(false), st>>>(pp);
+    }
     TTN_CUDA(cudaGetLastError());
     if (ps.flags & ttn::PASS_REDUCE) {
         // one partial per CTA and instance
@@ -340,9 +355,17 @@ static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
     q.final_tab = reinterpret_cast<float*>(P->ws + y.f_final);
     const ttn::FusedPass& lastp = fp.passes.back();
     q.fin_low = lastp.low; q.fin_layout = lastp.last_layout; q.fin_a = lastp.a;
+    if (P->i16) q.fin_a = lastp.low ? 0 : lastp.a - 1;                 // word digit
     long work = ttn::FFINAL_FLOATS; if (q.n_gates > work) work = q.n_gates;
     dim3 grid((unsigned)((work + 255) / 256), (unsigned)P->batch);
-    ttn::fused_prep_kernel<<<grid, 256, 0, st>>>(q);
+    if (P->i16) {
+        ttn::fused16_prep_kernel<<<grid, 256, 0, st>>>(q);
+        TTN_CUDA(cudaGetLastError());
+        TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
+        TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));
+    } else {
+        ttn::fused_prep_kernel<<<grid, 256, 0, st>>>(q);
+    }
     TTN_CUDA(cudaGetLastError());
     TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
     TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));
@@ -364,16 +387,23 @@ int ttn_version(void) { return 100; }
 
 size_t ttn_workspace_bytes(int q, int L, ttn_semiring mode, int batch, int want_config) {
     const bool count = (mode == TTN_COUNTING_F32_F64);
-    if ((q != 2 && q != 3) || batch < 1 || (mode != TTN_TROPICAL_F32 && mode != TTN_COUNTING_F32_F64)) return 0;
+    if ((q != 2 && q != 3) || batch < 1 ||
+        (mode != TTN_TROPICAL_F32 && mode != TTN_COUNTING_F32_F64 && mode != TTN_TROPICAL_I16)) return 0;
+    if (mode == TTN_TROPICAL_I16 && (q != 2 || want_config)) return 0;
     if (!limits_ok(q, L, count, want_config != 0)) return 0;
-    return make_layout(q, L, count, want_config != 0, batch).total;
+    return make_layout(q, L, count, want_config != 0, batch, mode == TTN_TROPICAL_I16 && i16_eligible(q, L)).total;
 }
 
 long ttn_plan_describe(int q, int L, ttn_call call, char* buf, size_t n) {
     if ((q != 2 && q != 3) || !buf || n == 0) return -1;
     if (!limits_ok(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) return -1;
     std::string s;
-    if (fused_eligible(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) {
+    if (call == TTN_CALL_ENERGY_I16 && i16_eligible(q, L)) {
+        ttn::FusedPlan fp = ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_I16);
+        if (fp.ok) s = ttn::describe_fused(fp);
+    }
+    if (call == TTN_CALL_ENERGY_I16 && s.empty()) call = TTN_CALL_ENERGY;
+    if (s.empty() && fused_eligible(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) {
         ttn::FusedPlan fp = call == TTN_CALL_COUNT ? ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_COUNT)
                                                    : ttn::make_fused_plan(L, ttn::FMAX_GATES);
         if (fp.ok) s = ttn::describe_fused(fp);
@@ -392,8 +422,13 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     *out = nullptr;
     if (q != 2 && q != 3) return fail(TTN_EINVAL, "q must be 2 or 3");
     if (L < 1 || batch < 1) return fail(TTN_EINVAL, "L and batch must be >= 1");
-    if (call != TTN_CALL_ENERGY && call != TTN_CALL_COUNT && call != TTN_CALL_CONFIG)
+    if (call != TTN_CALL_ENERGY && call != TTN_CALL_COUNT && call != TTN_CALL_CONFIG && call != TTN_CALL_ENERGY_I16)
         return fail(TTN_EINVAL, "bad call kind");
+    bool i16 = false;
+    if (call == TTN_CALL_ENERGY_I16) {
+        if (q != 2) return fail(TTN_EINVAL, "Tropical<i16> is an Ising call");
+        i16 = i16_eligible(q, L);           // small lattices run the f32 path (identical results)
+    }
     if (L > 1 && (!Jh || !Jv)) return fail(TTN_EINVAL, "Jh/Jv is NULL");
     if (!workspace) return fail(TTN_EINVAL, "workspace is NULL");
     if (q == 3 && h) return fail(TTN_EINVAL, "the Potts variant takes no fields");
@@ -404,7 +439,21 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     for (size_t i = 0; i < nv; ++i) if (!std::isfinite(Jv[i])) return fail(TTN_EINVAL, "non-finite Jv[%zu]", i);
     if (h) for (size_t i = 0; i < nf; ++i) if (!std::isfinite(h[i])) return fail(TTN_EINVAL, "non-finite h[%zu]", i);
 
-    Layout lay = make_layout(q, L, count, config, batch);
+    if (call == TTN_CALL_ENERGY_I16) {
+        // exactness: integer-valued couplings whose absolute sum keeps every intermediate inside 16 bits
+        for (int b = 0; b < batch; ++b) {
+            double tot = 0.0;
+            auto scan = [&](const float* a, size_t n_) -> bool {
+                for (size_t i = 0; i < n_; ++i) { if (a[i] != std::nearbyint(a[i])) return false; tot += std::fabs((double)a[i]); }
+                return true;
+            };
+            bool ok = scan(Jh + (size_t)b * L * (L - 1), (size_t)L * (L - 1)) && scan(Jv + (size_t)b * (L - 1) * L, (size_t)(L - 1) * L);
+            if (ok && h) ok = scan(h + (size_t)b * L * L, (size_t)L * L);
+            if (!ok) return fail(TTN_EINVAL, "Tropical<i16> needs integer-valued couplings (instance %d)", b);
+            if (tot > 8000.0) return fail(TTN_EINVAL, "Tropical<i16>: sum of |couplings| = %.0f > 8000 (instance %d)", tot, b);
+        }
+    }
+    Layout lay = make_layout(q, L, count, config, batch, i16);
     if (workspace_bytes < lay.total)
         return fail(TTN_ENOMEM, "workspace too small: %zu < %zu", workspace_bytes, lay.total);
     if ((uintptr_t)workspace % 256) return fail(TTN_EINVAL, "workspace must be 256-byte aligned");
@@ -418,9 +467,14 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     if (!P) return fail(TTN_ENOMEM, "host allocation failed");
     P->q = q; P->L = L; P->batch = batch; P->call = call; P->count = count; P->config = config;
     P->has_field = (h != nullptr);
+    P->i16 = i16;
     P->lay = lay;
     P->ws = static_cast<unsigned char*>(workspace);
-    if (fused_eligible(q, L, count, config)) {
+    if (i16) {
+        P->fplan = ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_I16);
+        P->fused = P->fplan.ok;
+        if (!P->fused) { delete P; return fail(TTN_EUNSUPPORTED, "no Tropical<i16> schedule"); }
+    } else if (fused_eligible(q, L, count, config)) {
         P->fplan = count ? ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_COUNT) : ttn::make_fused_plan(L, ttn::FMAX_GATES);
         P->fused = P->fplan.ok;
     }
@@ -589,6 +643,10 @@ extern "C" {
 ttn_status ttn_sweep_energy(int L, const float* Jh, const float* Jv, const float* h, int batch,
                             void* ws, size_t wsb, void* stream, double* E0) {
     return one_call(2, L, TTN_CALL_ENERGY, Jh, Jv, h, batch, ws, wsb, stream, E0, nullptr, nullptr);
+}
+ttn_status ttn_sweep_energy_i16(int L, const float* Jh, const float* Jv, const float* h, int batch,
+                                void* ws, size_t wsb, void* stream, double* E0) {
+    return one_call(2, L, TTN_CALL_ENERGY_I16, Jh, Jv, h, batch, ws, wsb, stream, E0, nullptr, nullptr);
 }
 ttn_status ttn_sweep_count(int L, const float* Jh, const float* Jv, const float* h, int batch,
                            void* ws, size_t wsb, void* stream, double* E0, double* g) {

@@ -63,6 +63,7 @@ struct FusedParams {
     int cta_per_inst;                   // 1: few tiles per instance -- every CTA sweeps whole instances
                                         // (blockIdx.x, + gridDim.x, ...) with its own warps only
     int part_stride;                    // partials per instance: gridDim.x, or 1 when cta_per_inst
+    int L_cols;                         // Tropical<i16> only: lattice L (p.L = L - 1 word digits)
     unsigned stride_bytes;              // HIGH: 4 << a, passed opaque so that the address math stays
                                         // one IMAD.WIDE (32 x 32 -> 64 bit) per access
 };
@@ -185,6 +186,64 @@ __device__ __forceinline__ void fround(float (&v)[128], const unsigned mask, con
     }
     TTN_G(0) TTN_G(1) TTN_G(2) TTN_G(3) TTN_G(4) TTN_G(5) TTN_G(6)
 #undef TTN_G
+}
+
+// ---- Tropical<i16> (the paper's own Int16 choice for +-J) -----------
+// Two elements per 32-bit word: column 0 of the lattice row is the HALF of a word (low half =
+// bit 0 = sigma +1), the kernel's tile geometry applies to the word index.  One VIADDMNMX.S16x2
+// does max(b + k, a) for both halves: 1 alu-pipe instruction per word and gate, no fma-pipe add.
+// Constants are packed per half (lo = element with column-0 bit 0) by the prep kernel.
+__device__ __forceinline__ float vam2(float b, unsigned k, float a) {
+    return __uint_as_float(__viaddmax_s16x2(__float_as_uint(b), k, __float_as_uint(a)));
+}
+template <int K, int PN, int QN>
+__device__ __forceinline__ void cgate16(float (&v)[128], const uint4 c0, const uint4 c1, const int tp, const int tq) {
+    unsigned ka[2][2] = {{c0.x, c0.y}, {c0.z, c0.w}}, kb[2][2] = {{c1.x, c1.y}, {c1.z, c1.w}};
+    if (PN < 0) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) { ka[0][h] = tp ? ka[1][h] : ka[0][h]; kb[0][h] = tp ? kb[1][h] : kb[0][h]; }
+    }
+    if (QN < 0) {
+#pragma unroll
+        for (int l = 0; l < 2; ++l) { ka[l][0] = tq ? ka[l][1] : ka[l][0]; kb[l][0] = tq ? kb[l][1] : kb[l][0]; }
+    }
+    constexpr int B = 1 << K;
+#pragma unroll
+    for (int j = 0; j < 128; ++j) {
+        if (j & B) continue;
+        const int np = PN < 0 ? 0 : (j >> (PN < 0 ? 0 : PN)) & 1, nq = QN < 0 ? 0 : (j >> (QN < 0 ? 0 : QN)) & 1;
+        const float a = v[j], b = v[j + B];
+        v[j] = vam2(b, ka[np][nq], a);
+        v[j + B] = vam2(a, kb[np][nq], b);
+    }
+}
+// gate on column 0 (the half of a word): partner = the other half of the same word.  kp[n] =
+// (lo: ka, hi: kb) for column-1 bit n; Q1 = register bit holding column 1, or -1 (then t1).
+template <int Q1>
+__device__ __forceinline__ void hgate16(float (&v)[128], const uint4 c0, const int t1) {
+    unsigned kp[2] = {c0.x, c0.y};
+    if (Q1 < 0) kp[0] = t1 ? kp[1] : kp[0];
+#pragma unroll
+    for (int j = 0; j < 128; ++j) {
+        const unsigned w = __float_as_uint(v[j]);
+        const unsigned sw = __byte_perm(w, 0u, 0x1032);           // swap the halves
+        v[j] = __uint_as_float(__viaddmax_s16x2(sw, kp[Q1 < 0 ? 0 : (j >> (Q1 < 0 ? 0 : Q1)) & 1], w));
+    }
+}
+template <bool LOW>
+__device__ __forceinline__ void fround16(float (&v)[128], const unsigned mask, const uint4* __restrict__ gk,
+                                         const int layout, const int tp, const int tq, const int t1) {
+#define TTN_G16(Kk)                                                                                 \
+    if (mask & (1u << Kk)) {                                                                        \
+        const uint4 c0 = gk[0], c1 = gk[1]; gk += 2;                                                \
+        cgate16<Kk, Nbr<LOW, Kk>::PN, Nbr<LOW, Kk>::QN>(v, c0, c1, tp, tq);                         \
+    }
+    TTN_G16(0) TTN_G16(1) TTN_G16(2) TTN_G16(3) TTN_G16(4) TTN_G16(5) TTN_G16(6)
+#undef TTN_G16
+    if (LOW && (mask & 0x80u)) {             // column 0; column 1 = tile digit 0 = register bit 2 in layout A, lane bit 0 in B
+        const uint4 c0 = gk[0];
+        if (layout == 0) hgate16<fused_bit_of_digit(true, 0, 0)>(v, c0, 0); else hgate16<-1>(v, c0, t1);
+    }
 }
 
 // ---- layout exchange through the warp's shared-memory region ----------------------------------------
@@ -359,7 +418,9 @@ __device__ __forceinline__ void group_sync(int warp) {
     asm volatile("bar.sync %0, 128;" :: "r"(1 + (warp >> 2)) : "memory");
 }
 
-template <bool LOW>
+// ELEM = 0: Tropical<f32>.  ELEM = 1: Tropical<i16>, two elements per word; then p.L, p.a and the
+// tile geometry count WORD digits (column c >= 1 = word digit c - 1) and p.L_cols = lattice L.
+template <bool LOW, int ELEM = 0>
 __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const FusedParams p) {
     constexpr int FWARPS = fwarps(LOW);
     extern __shared__ __align__(16) unsigned char fsm_raw[];
@@ -466,7 +527,9 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
                 if (code == MC_END || code == MC_FINAL) break;
                 const unsigned nxt = s_mops[pc + 1];
                 if (code == MC_ROUND) {
-                    fround<LOW>(v, (op >> 8) & 0x7fu, gk, n0, n1, layout ? tpB : tpA, layout ? tqB : tqA);
+                    if (ELEM == 0) fround<LOW>(v, (op >> 8) & 0x7fu, gk, n0, n1, layout ? tpB : tpA, layout ? tqB : tqA);
+                    else fround16<LOW>(v, (op >> 8) & 0xffu, reinterpret_cast<const uint4*>(s_gk) + 2 * (op >> 16), layout,
+                                       layout ? tpB : tpA, layout ? tqB : tqA, lane & 1);
                 } else if (code == MC_XAB) {
                     __syncwarp(); xmove<LOW, 0, true>(v, myreg, lane); __syncwarp(); xmove<LOW, 1, false>(v, myreg, lane);
                     layout = 1;
@@ -487,15 +550,36 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
                     if (layout == 0) { sthr = base + (lane & 7) + ((unsigned long long)(lane >> 3) << (p.a + 7)); x0 = p.a; var = tpA + 2 * tqA; }
                     else { sthr = base + (lane & 7) + ((unsigned long long)(lane >> 3) << p.a); x0 = p.a + 2; var = tqB + 2 * tpB; }
                 }
-                const float cthr = final_thread_const(s_fin, p.L, x0, sthr);
-                const float4* T = reinterpret_cast<const float4*>(s_fin + var * 128);
-                float mx = -INFINITY;
+                if (ELEM == 0) {
+                    const float cthr = final_thread_const(s_fin, p.L, x0, sthr);
+                    const float4* T = reinterpret_cast<const float4*>(s_fin + var * 128);
+                    float mx = -INFINITY;
 #pragma unroll
-                for (int q = 0; q < 32; ++q) {
-                    const float4 t = T[q];
-                    mx = fmaxf(mx, fmaxf(fmaxf(v[4 * q] + t.x, v[4 * q + 1] + t.y), fmaxf(v[4 * q + 2] + t.z, v[4 * q + 3] + t.w)));
+                    for (int q = 0; q < 32; ++q) {
+                        const float4 t = T[q];
+                        mx = fmaxf(mx, fmaxf(fmaxf(v[4 * q] + t.x, v[4 * q + 1] + t.y), fmaxf(v[4 * q + 2] + t.z, v[4 * q + 3] + t.w)));
+                    }
+                    wmax = fmaxf(wmax, mx + cthr);
+                } else {
+                    // per half h: element index = 2 * word index + h, register columns x0+1 .. x0+7; the
+                    // table entries and the thread constants are packed (lo = h 0, hi = h 1), all integers
+                    const int c0 = __float2int_rn(final_thread_const(s_fin, p.L_cols, x0 + 1, sthr << 1));
+                    const int c1 = __float2int_rn(final_thread_const(s_fin, p.L_cols, x0 + 1, (sthr << 1) | 1ull));
+                    const unsigned cpk = ((unsigned)c0 & 0xffffu) | ((unsigned)c1 << 16);
+                    const uint4* T = reinterpret_cast<const uint4*>(s_fin + var * 128);
+                    unsigned m2 = 0x80008000u;                    // (-32768, -32768)
+#pragma unroll
+                    for (int q = 0; q < 32; ++q) {
+                        const uint4 t = T[q];
+                        m2 = __vmaxs2(m2, __vadd2(__float_as_uint(v[4 * q]), t.x));
+                        m2 = __vmaxs2(m2, __vadd2(__float_as_uint(v[4 * q + 1]), t.y));
+                        m2 = __vmaxs2(m2, __vadd2(__float_as_uint(v[4 * q + 2]), t.z));
+                        m2 = __vmaxs2(m2, __vadd2(__float_as_uint(v[4 * q + 3]), t.w));
+                    }
+                    m2 = __vadd2(m2, cpk);
+                    const int lo = (int)(short)(m2 & 0xffffu), hi = (int)(short)(m2 >> 16);
+                    wmax = fmaxf(wmax, (float)(lo > hi ? lo : hi));
                 }
-                wmax = fmaxf(wmax, mx + cthr);
             } else {
                 if (!LOW) group_sync(warp);
                 if (LOW || p.last_layout == 1) gmove<LOW, 1, true>(v, S + base, lane, p.stride_bytes, p.a);
@@ -579,6 +663,76 @@ __global__ void __launch_bounds__(256) fused_prep_kernel(const FusedPrepParams p
             acc += (tl == bits[0]) ? Kacc(L, x0 - 1) : -Kacc(L, x0 - 1);              // 0 when x0 = 0
             acc += (th == bits[F_RB - 1]) ? Kacc(L, x0 + F_RB - 1) : -Kacc(L, x0 + F_RB - 1);   // 0 at the right edge
             out[idx] = (float)acc;
+        } else if (idx < 576) {
+            const int c = (int)idx - 512;
+            out[idx] = c < L ? (float)Hacc(L, c) : 0.f;
+        } else {
+            const int c = (int)idx - 576;
+            out[idx] = c < L - 1 ? (float)Kacc(L, c) : 0.f;
+        }
+    }
+}
+
+}  // namespace ttn
+
+namespace ttn {
+
+// ---- S0 for Tropical<i16>: packed (lo = column-0 bit 0, hi = bit 1) gate constants and final table ------
+// gate_rc: low << 16 | K << 13 | layout << 12 | r << 6 | c with c the lattice COLUMN; K = 7 is the
+// gate on column 0 (the half of a word).  All values are integers (checked on the host).
+__global__ void __launch_bounds__(256) fused16_prep_kernel(const FusedPrepParams p) {
+    const unsigned long long inst = blockIdx.y;
+    const int L = p.L;
+    const float* Jh = p.Jh + inst * (unsigned long long)(L * (L - 1));
+    const float* Jv = p.Jv + inst * (unsigned long long)((L - 1) * L);
+    const float* hh = p.h ? p.h + inst * (unsigned long long)(L * L) : nullptr;
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    auto Hacc = [&](int R, int c) { double s = 0; if (hh) for (int r = 0; r < R; ++r) s += (double)hh[r * L + c]; return s; };
+    auto Kacc = [&](int R, int c) { double s = 0; if (c < 0 || c >= L - 1) return s; for (int r = 0; r < R; ++r) s += (double)Jh[r * (L - 1) + c]; return s; };
+    auto pack = [](double lo, double hi) { return ((unsigned)(int)lo & 0xffffu) | ((unsigned)(int)hi << 16); };
+    if (idx < p.n_gates) {
+        const int g = p.gate_rc[idx], mirrored = (g >> 12) & 1, K = (g >> 13) & 7;
+        const int r = (g >> 6) & 63, c = g & 63;
+        const double m = -2.0 * (double)Jv[(r - 1) * L + c];
+        const double H = Hacc(r, c), Kl = Kacc(r, c - 1), Kr = Kacc(r, c);
+        unsigned* out = reinterpret_cast<unsigned*>(p.gate_k) + (inst * p.n_gates + idx) * 8;
+        auto kval = [&](int side, int nl, int nh) {
+            const double rho = H + (nl ? -Kl : Kl) + (nh ? -Kr : Kr);
+            return side == 0 ? m - 2.0 * rho : m + 2.0 * rho;
+        };
+        if (K == 7) {                 // column 0: kp[n] = (lo: ka, hi: kb), n = bit of column 1
+            for (int i = 0; i < 8; ++i) out[i] = 0u;
+            for (int n = 0; n < 2; ++n) out[n] = pack(kval(0, 0, n), kval(1, 0, n));
+        } else {
+            for (int side = 0; side < 2; ++side)
+                for (int np = 0; np < 2; ++np)
+                    for (int nq = 0; nq < 2; ++nq) {
+                        const int nl = mirrored ? nq : np, nh = mirrored ? np : nq;
+                        // column 1: the left neighbour is the half of the word itself
+                        out[side * 4 + np * 2 + nq] = c == 1 ? pack(kval(side, 0, nh), kval(side, 1, nh))
+                                                             : pack(kval(side, nl, nh), kval(side, nl, nh));
+                    }
+        }
+    }
+    if (idx < FFINAL_FLOATS) {
+        float* out = p.final_tab + inst * FFINAL_FLOATS;
+        if (idx < 512) {
+            const int var = (int)idx >> 7, j = (int)idx & 127, tl = var & 1, th = var >> 1;
+            const bool low = p.fin_low != 0;
+            const int d0 = low ? (p.fin_layout == 0 ? 0 : 5) : (p.fin_layout == 0 ? 0 : 2);
+            const int x0 = 1 + p.fin_a + d0;                    // first register COLUMN (fin_a = word digit)
+            int bits[F_RB];
+            for (int i = 0; i < F_RB; ++i) bits[i] = (j >> fused_bit_of_digit(low, p.fin_layout, d0 + i)) & 1;
+            double acc = 0;
+            for (int i = 0; i < F_RB; ++i) {
+                const int c = x0 + i;
+                acc += bits[i] ? -Hacc(L, c) : Hacc(L, c);
+                if (i + 1 < F_RB) acc += (bits[i] == bits[i + 1]) ? Kacc(L, c) : -Kacc(L, c);
+            }
+            acc += (th == bits[F_RB - 1]) ? Kacc(L, x0 + F_RB - 1) : -Kacc(L, x0 + F_RB - 1);
+            const double kl = Kacc(L, x0 - 1);
+            const int tl0 = x0 == 1 ? 0 : tl, tl1 = x0 == 1 ? 1 : tl;     // column 0 = the half
+            reinterpret_cast<unsigned*>(out)[idx] = pack(acc + ((tl0 == bits[0]) ? kl : -kl), acc + ((tl1 == bits[0]) ? kl : -kl));
         } else if (idx < 576) {
             const int c = (int)idx - 512;
             out[idx] = c < L ? (float)Hacc(L, c) : 0.f;

@@ -14,10 +14,11 @@ from .build import build
 
 TROPICAL_F32 = 0
 COUNTING_F32_F64 = 1
-CALL_ENERGY, CALL_COUNT, CALL_CONFIG = 0, 1, 2
+TROPICAL_I16 = 2
+CALL_ENERGY, CALL_COUNT, CALL_CONFIG, CALL_ENERGY_I16 = 0, 1, 2, 3
 
 EXPORTS = [
-    "ttn_workspace_bytes", "ttn_sweep_energy", "ttn_sweep_count", "ttn_ground_config",
+    "ttn_workspace_bytes", "ttn_sweep_energy", "ttn_sweep_energy_i16", "ttn_sweep_count", "ttn_ground_config",
     "ttn_potts3_sweep_energy", "ttn_potts3_sweep_count", "ttn_plan_create", "ttn_plan_launch",
     "ttn_plan_read", "ttn_plan_destroy", "ttn_plan_num_launches", "ttn_plan_num_passes",
     "ttn_plan_describe", "ttn_last_error", "ttn_version",
@@ -47,6 +48,7 @@ def lib() -> ctypes.CDLL:
         L.ttn_workspace_bytes.argtypes = [ci, ci, ci, ci, ci]
         L.ttn_workspace_bytes.restype = sz
         L.ttn_sweep_energy.argtypes = [ci, fp, fp, fp, ci, vp, sz, vp, dp]
+        L.ttn_sweep_energy_i16.argtypes = [ci, fp, fp, fp, ci, vp, sz, vp, dp]
         L.ttn_sweep_count.argtypes = [ci, fp, fp, fp, ci, vp, sz, vp, dp, dp]
         L.ttn_ground_config.argtypes = [ci, fp, fp, fp, ci, vp, sz, vp, dp, i8]
         L.ttn_potts3_sweep_energy.argtypes = [ci, fp, fp, ci, vp, sz, vp, dp]
@@ -134,7 +136,7 @@ class Plan:
     def __init__(self, q: int, call: int, Jh, Jv, h=None, workspace=None, stream=None):
         self.B, self.L, self.Jh, self.Jv, self.h = _couplings(Jh, Jv, h)
         self.q, self.call = q, call
-        mode = COUNTING_F32_F64 if call == CALL_COUNT else TROPICAL_F32
+        mode = _mode_of(call)
         need = workspace_bytes(q, self.L, mode, self.B, call == CALL_CONFIG)
         self.workspace = workspace if workspace is not None else alloc_workspace(need)
         if self.workspace.numel() * self.workspace.element_size() < need:
@@ -178,9 +180,13 @@ class Plan:
             pass
 
 
+def _mode_of(call: int) -> int:
+    return {CALL_COUNT: COUNTING_F32_F64, CALL_ENERGY_I16: TROPICAL_I16}.get(call, TROPICAL_F32)
+
+
 def _one_call(fn_name, q, call, Jh, Jv, h, workspace, stream):
     B, L, Jh, Jv, h = _couplings(Jh, Jv, h)
-    mode = COUNTING_F32_F64 if call == CALL_COUNT else TROPICAL_F32
+    mode = _mode_of(call)
     need = workspace_bytes(q, L, mode, B, call == CALL_CONFIG)
     ws = workspace if workspace is not None else alloc_workspace(need)
     wsb = ws.numel() * ws.element_size()
@@ -204,6 +210,11 @@ def _one_call(fn_name, q, call, Jh, Jv, h, workspace, stream):
 def sweep_energy(Jh, Jv, h=None, workspace=None, stream=None) -> np.ndarray:
     """ttn_sweep_energy: ground-state energies E0[batch] (Tropical<f32> sweep)."""
     return _one_call("ttn_sweep_energy", 2, CALL_ENERGY, Jh, Jv, h, workspace, stream)[0]
+
+
+def sweep_energy_i16(Jh, Jv, h=None, workspace=None, stream=None) -> np.ndarray:
+    """ttn_sweep_energy_i16: the same E0[batch] in Tropical<i16> (integer-valued couplings only)."""
+    return _one_call("ttn_sweep_energy_i16", 2, CALL_ENERGY_I16, Jh, Jv, h, workspace, stream)[0]
 
 
 def sweep_count(Jh, Jv, h=None, workspace=None, stream=None) -> Tuple[np.ndarray, np.ndarray]:

@@ -319,3 +319,41 @@ def test_plan_split_api_relaunch():
     E_c, s_c = ttn.ground_config(Jh, Jv, h)
     assert np.array_equal(E_a, E_c) and np.array_equal(s_a, s_c)
     p.close()
+
+
+# ------------------------------------------------------------------ Tropical<i16>
+@pytest.mark.parametrize("L", [4, 12, 13, 14, 15, 17, 19])
+def test_i16_energy_vs_oracle(L):
+    """Exact integer arithmetic in 16 bits: bit-exact against the oracle, with and without fields."""
+    rng = np.random.default_rng(1600 + L)
+    B = 3
+    Jh = rng.integers(-2, 3, size=(B, L, L - 1)).astype(np.float32)
+    Jv = rng.integers(-2, 3, size=(B, L - 1, L)).astype(np.float32)
+    h = rng.integers(-1, 2, size=(B, L, L)).astype(np.float32)
+    E_h = ttn.sweep_energy_i16(Jh, Jv, h)
+    Jp, Jq, _ = make_batch(L, [4100, 4101, 4102], "pmj")
+    E_p = ttn.sweep_energy_i16(Jp, Jq)
+    for b in range(B):
+        assert E_h[b] == oracle.dp_ising(L, Jh[b], Jv[b], h[b], count=False)[0]
+        assert E_p[b] == oracle.dp_ising(L, Jp[b], Jq[b], None, count=False)[0]
+    assert np.array_equal(E_p, ttn.sweep_energy(Jp, Jq))
+
+
+@pytest.mark.parametrize("L", [24, 28, 30, 32])
+def test_i16_large_energy_vs_golden(L):
+    gold = golden()
+    key = ("ising_energy", L, 4000)
+    assert key in gold
+    Jh, Jv, _ = make_batch(L, [4000], "pmj")
+    assert ttn.sweep_energy_i16(Jh, Jv)[0] == gold[key][0]
+
+
+def test_i16_rejects_non_integer_and_large_couplings():
+    Jh, Jv, h = make_batch(14, [7], "gauss", fields=True)
+    with pytest.raises(ttn.TTNError) as e:
+        ttn.sweep_energy_i16(Jh, Jv, h)
+    assert e.value.status == 1
+    Jh, Jv, _ = make_batch(14, [7], "pmj")
+    with pytest.raises(ttn.TTNError) as e:
+        ttn.sweep_energy_i16(100 * Jh, 100 * Jv)
+    assert e.value.status == 1

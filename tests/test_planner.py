@@ -142,16 +142,22 @@ DIGIT_OF_BIT_COUNT = {(1, 0): [0, 1, 2, 3, 4], (1, 1): [9, 8, 7, 6, 5],
                       (0, 0): [0, 1, 2, 3, 4], (0, 1): [6, 5, 4, 3, 2]}
 
 
-def fused_to_gates(L, fpasses, count=False):
+# Tropical<i16> geometry (GEOM_I16): column 0 is the half of a 32-bit word (pseudo register bit 7
+# of the LOW tile), column c >= 1 is word digit c - 1 with the f32 maps
+DIGIT_OF_BIT_I16 = {(1, 0): [1 + d for d in [5, 6, 0, 1, 2, 3, 4]] + [0], (1, 1): [1 + d for d in [6, 5, 11, 10, 9, 8, 7]] + [0],
+                    (0, 0): [4, 5, 6, 0, 1, 2, 3], (0, 1): [4, 3, 2, 8, 7, 6, 5]}
+
+
+def fused_to_gates(L, fpasses, count=False, i16=False):
     """Check the structure of the micro-op program (layouts, register bits, rounds) and the
     three-point-stencil dependency rule; return the flat (r, c) gate sequence."""
     flat = []
     grow = [1] * L                                   # rows complete per digit (row 0 needs no gate)
     for i, ps in enumerate(fpasses):
         a, Wt, low = ps["a"], ps["W"], ps["low"]
-        wl, wh, rb = (10, 7, 5) if count else (12, 9, 7)
-        dmap = DIGIT_OF_BIT_COUNT if count else DIGIT_OF_BIT
-        assert (low == 1 and a == 0 and Wt == wl) or (low == 0 and a >= 4 and Wt == wh)
+        wl, wh, rb = (10, 7, 5) if count else ((13, 9, 8 if low else 7) if i16 else (12, 9, 7))
+        dmap = DIGIT_OF_BIT_COUNT if count else (DIGIT_OF_BIT_I16 if i16 else DIGIT_OF_BIT)
+        assert (low == 1 and a == 0 and Wt == wl) or (low == 0 and a >= (5 if i16 else 4) and Wt == wh)
         assert a + Wt <= L
         assert (ps["flags"] & 1) == (1 if i == 0 else 0)
         last = i == len(fpasses) - 1
@@ -235,6 +241,14 @@ def test_fused_count_schedule_obeys_dependency_rule(L):
     head, fpasses = parse_fused(describe(2, L, 1, fused=True))
     assert int(head["L"]) == L
     flat = fused_to_gates(L, fpasses, count=True)
+    assert len(flat) == L * (L - 1) == len(set(flat))
+
+
+@pytest.mark.parametrize("L", [13, 14, 15, 18, 22, 24, 28, 32, 34])
+def test_fused_i16_schedule_obeys_dependency_rule(L):
+    head, fpasses = parse_fused(describe(2, L, 3, fused=True))
+    assert int(head["L"]) == L
+    flat = fused_to_gates(L, fpasses, i16=True)
     assert len(flat) == L * (L - 1) == len(set(flat))
 
 
