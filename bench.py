@@ -240,6 +240,27 @@ def main():
     e2e_ms = max_over_ranks(e2e_ms, dist, "cuda")
     assert E_host == E_dev, (E_host, E_dev)
 
+    # ---- NEXT-1 beside it: the same instance in Tropical<i16> (exact for integer couplings) ------
+    i16 = None
+    try:
+        p16 = ttn.Plan(2, ttn.CALL_ENERGY_I16, Jh, Jv, None, workspace=ws)
+        for _ in range(2):
+            p16.launch()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(3):
+            p16.launch()
+        b.record()
+        torch.cuda.synchronize()
+        E16 = p16.read()[0][0]
+        assert E16 == E_dev, (E16, E_dev)
+        i16 = {"ms_per_instance": a.elapsed_time(b) / 3, "hbm_passes": p16.num_passes, "state_bytes": 2 * 2 ** L,
+               "note": "ttn_sweep_energy_i16 (SURVEY.md NEXT-1), same instance, E0 identical; not the headline metric"}
+        p16.close()
+    except ttn.TTNError as e:      # e.g. L below the i16 path's limits
+        i16 = {"unavailable": str(e)}
+
     if rank == 0:
         peak, peak_src = measured_peaks()
         per_inst_ms = whole_job_ms_per_instance(ms_per_step, world)
@@ -274,7 +295,7 @@ def main():
                              "peak": alu_peak, "unit": "max-plus updates/s",
                              "frac": updates(L) / (ms_per_step * 1e-3) / alu_peak,
                              "note": "1 FMNMX per update on the 64-lane/clk/SM alu pipe at the sampled SM clock"},
-            "step_ms": step_ms, "clocks": clocks,
+            "step_ms": step_ms, "clocks": clocks, "tropical_i16": i16,
         }
         if not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(L, args.cpu_L)

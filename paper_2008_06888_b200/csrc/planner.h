@@ -372,8 +372,16 @@ class FusedScheduler {
 // Estimated time of one pass in ms on B200 (fit over the measured launch lists, profiles/r01f.md):
 // 0.267 ms per gate (FMNMX floor 0.231), a fixed part for the memory phases that do not hide, round
 // dispatch and exchanges; a pass cannot beat its memory time.
-inline double fused_pass_cost(const FusedPass& ps) {
+inline double fused_pass_cost(const FusedPass& ps, const FusedGeom& G = GEOM_F32) {
     const int g = ps.gate_end - ps.gate_begin, x = ps.n_phases > 1 ? ps.n_phases - 1 : 0;
+    if (G.kind == 2) {
+        // Tropical<i16>: half the bytes and half the alu work per element; tiles whose 9 active
+        // word digits reach past bit 18 (> 256 pages of 2 MiB) are bound by address translation
+        if (ps.low) { const double t = 1.2 + 0.19 * g + 0.02 * ps.n_rounds + 0.25 * x; return t > 4.0 ? t : 4.0; }
+        const double t = 3.5 + 0.135 * g + 0.06 * ps.n_rounds + 0.25 * x;
+        const double floor_ = ps.a - 1 > 18 ? 12.5 : 5.0;
+        return t > floor_ ? t : floor_;
+    }
     if (ps.low) { const double t = 1.2 + 0.267 * g + 0.02 * ps.n_rounds + 0.25 * x; return t > 6.5 ? t : 6.5; }
     const double t = 3.5 + 0.267 * g + 0.08 * ps.n_rounds + 0.25 * x;
     return t > 9.0 ? t : 9.0;
@@ -392,7 +400,7 @@ inline FusedPlan make_fused_plan(int L, int max_gates_per_pass, const FusedGeom&
         p.passes.back().flags |= PASS_REDUCE;
         p.mops.back().code = MC_FINAL;
         double cost = 0;
-        for (auto& ps : p.passes) cost += fused_pass_cost(ps);
+        for (auto& ps : p.passes) cost += fused_pass_cost(ps, G);
         if (best_cost < 0 || cost < best_cost) { best = p; best_cost = cost; best.ok = true; }
     };
     for (int stride = 1; stride <= G.WHIGH; ++stride) {
@@ -437,7 +445,7 @@ inline FusedPlan make_fused_plan(int L, int max_gates_per_pass, const FusedGeom&
                 trial.rebind(scratch);
                 FusedPass ps{};
                 const int n = trial.run_pass(a, a == 0, max_gates_per_pass, ps);
-                const double c = fused_pass_cost(ps);
+                const double c = fused_pass_cost(ps, G);
                 if (n > best_n) { best_a = a; best_n = n; best_c = c; }          // ties: the lowest start
             }
             if (best_n <= 0 && !first) break;
