@@ -289,6 +289,7 @@ struct FusedPass {
     int mop_begin, mop_end;      // into FusedPlan::mops
     int gate_begin, gate_end;    // into FusedPlan::gate_rc
     int n_phases, n_rounds;
+    int src_buf = -1, dst_buf = -1;   // -1 = the state V; r >= 0 = checkpoint C_r (row-aligned plans)
 };
 
 struct FusedPlan {
@@ -308,6 +309,11 @@ class FusedScheduler {
         return true;
     }
     // One pass over active digits [a, a+W).  Returns number of gates applied.
+    bool row_done(int r) const {
+        for (int c = 0; c < L_; ++c) if (grow_[c] < r + 1) return false;
+        return true;
+    }
+    void set_max_row(int r) { max_row_ = r; }
     int run_pass(int a, bool low, int max_gates, FusedPass& ps) {
         const int W = low ? G_.WLOW : G_.WHIGH;
         ps.a = a; ps.W = W; ps.low = low; ps.flags = 0; ps.n_phases = 0; ps.n_rounds = 0;
@@ -338,7 +344,7 @@ class FusedScheduler {
   private:
     bool legal(int c) const {
         const int r = grow_[c];
-        if (r >= L_) return false;
+        if (r >= L_ || r > max_row_) return false;
         if (c > 0 && grow_[c - 1] < r) return false;
         if (c + 1 < L_ && grow_[c + 1] < r) return false;
         return true;
@@ -367,6 +373,7 @@ class FusedScheduler {
     std::vector<int> grow_;      // grow[c] = rows complete on digit c (row 0 needs no gate)
     int pass_gate_begin_ = 0, pass_mop_begin_ = 0, max_gates_ = 1 << 30;
     int max_mops_ = 120;         // micro-ops per pass the kernel stages (FMAX_MOPS = 128)
+    int max_row_ = 1 << 30;      // row-aligned plans: no gate of a later row
 };
 
 // Estimated time of one pass in ms on B200 (fit over the measured launch lists, profiles/r01f.md):
@@ -460,6 +467,47 @@ inline FusedPlan make_fused_plan(int L, int max_gates_per_pass, const FusedGeom&
     return best;
 }
 
+// Row-aligned plan for ttn_ground_config (f32 geometry): every row boundary is materialised as a
+// checkpoint C_r = V''_r.  Row r needs one pass per tile of a cover of the columns (the low tile
+// and high tiles up to column L); the pass that completes row r writes C_r, the first pass of
+// row r+1 reads it.  Pass 0 initialises C_0 (no gate: V''_0 is the tropical one everywhere).
+inline FusedPlan make_fused_row_plan(int L, int max_gates_per_pass) {
+    FusedPlan p; p.L = L;
+    if (L < F_WLOW) return p;
+    std::vector<int> starts{0};
+    for (int x = F_WLOW; x < L; x += F_WHIGH) {
+        int a = x + F_WHIGH <= L ? x : L - F_WHIGH;
+        if (a < F_AMIN) a = F_AMIN;
+        starts.push_back(a);
+    }
+    FusedScheduler s(L, p, GEOM_F32);
+    {   // row 0: initialise
+        s.set_max_row(0);
+        FusedPass ps{};
+        s.run_pass(0, true, max_gates_per_pass, ps);
+        ps.flags |= PASS_INIT; ps.src_buf = -1; ps.dst_buf = 0;
+        p.passes.push_back(ps);
+    }
+    for (int r = 1; r < L; ++r) {
+        s.set_max_row(r);
+        int src = r - 1;
+        for (size_t k = 0; k < starts.size(); ++k) {
+            FusedPass ps{};
+            const size_t m0 = p.mops.size();
+            const int n = s.run_pass(starts[k], starts[k] == 0, max_gates_per_pass, ps);
+            const bool done = s.row_done(r);
+            if (n == 0 && !(done && src >= 0)) { p.mops.resize(m0); continue; }
+            ps.src_buf = src; ps.dst_buf = done ? r : -1;
+            src = -1;
+            p.passes.push_back(ps);
+            if (done) break;
+        }
+        if (!s.row_done(r)) return p;          // ok stays false
+    }
+    p.ok = true;
+    return p;
+}
+
 inline std::string describe_fused(const FusedPlan& p) {
     std::string out; char line[200];
     snprintf(line, sizeof line, "fused L=%d passes=%zu mops=%zu gates=%zu\n", p.L,
@@ -467,9 +515,9 @@ inline std::string describe_fused(const FusedPlan& p) {
     out += line;
     for (size_t i = 0; i < p.passes.size(); ++i) {
         const FusedPass& ps = p.passes[i];
-        snprintf(line, sizeof line, "fpass %zu a=%d W=%d low=%d flags=%d first=%d last=%d phases=%d rounds=%d gates=%d\n", i,
+        snprintf(line, sizeof line, "fpass %zu a=%d W=%d low=%d flags=%d first=%d last=%d phases=%d rounds=%d gates=%d src=%d dst=%d\n", i,
                  ps.a, ps.W, ps.low, ps.flags, ps.first_layout, ps.last_layout, ps.n_phases, ps.n_rounds,
-                 ps.gate_end - ps.gate_begin);
+                 ps.gate_end - ps.gate_begin, ps.src_buf, ps.dst_buf);
         out += line;
         for (int k = ps.mop_begin; k < ps.mop_end; ++k) {
             const MicroOp& m = p.mops[k];

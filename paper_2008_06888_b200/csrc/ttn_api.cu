@@ -85,8 +85,8 @@ bool i16_eligible(int q, int L) {
 }
 bool fused_eligible(int q, int L, bool count, bool config) {
     if (const char* e = getenv("TTN_DEBUG_FUSED")) if (atoi(e) == 0) return false;
-    if (q != 2 || config) return false;
-    return count ? L >= ttn::CW_LOW : L >= ttn::F_WLOW;
+    if (q != 2) return false;
+    return count ? L >= ttn::CW_LOW : L >= ttn::F_WLOW;      // config: row-aligned f32 plan
 }
 
 // The op list length is bounded by L*L gates + 2*L*L diagonals.
@@ -210,10 +210,17 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
     pp.state = reinterpret_cast<float*>(P->ws + y.x);
     pp.inst_stride = y.NS;
     pp.tiles_per_inst = y.NS >> 12;
+    pp.src = pp.state; pp.src_stride = pp.inst_stride;
+    if (P->config) {           // row-aligned plan: checkpoints C_r = V''_r, [inst][L][2^L]
+        float* CK = reinterpret_cast<float*>(P->ws + y.ckpt);
+        if (ps.src_buf >= 0) { pp.src = CK + (unsigned long long)ps.src_buf * y.NS; pp.src_stride = (unsigned long long)P->L * y.NS; }
+        if (ps.dst_buf >= 0) { pp.state = CK + (unsigned long long)ps.dst_buf * y.NS; pp.inst_stride = (unsigned long long)P->L * y.NS; }
+    }
     pp.L_cols = P->L;
     if (P->i16) {           // the kernel sees the lattice of 32-bit words: column c >= 1 = word digit c - 1
         pp.L = P->L - 1; pp.a = ps.low ? 0 : ps.a - 1;
         pp.inst_stride = y.NS >> 1; pp.tiles_per_inst = y.NS >> 13;
+        pp.src = pp.state; pp.src_stride = pp.inst_stride;
     }
     const int a_mem = pp.a;
     pp.mops = reinterpret_cast<const ttn::MicroOp*>(P->ws + y.f_mops) + ps.mop_begin;
@@ -266,6 +273,7 @@ static ttn_status launch_fcount_pass(const ttn_plan* P, const ttn::FusedPass& ps
     pp.state = reinterpret_cast<float*>(P->ws + y.x);
     cp.state_n = reinterpret_cast<double*>(P->ws + y.n);
     pp.inst_stride = y.NS;
+    pp.src = pp.state; pp.src_stride = y.NS;
     pp.tiles_per_inst = y.NS >> 10;
     pp.mops = reinterpret_cast<const ttn::MicroOp*>(P->ws + y.f_mops) + ps.mop_begin;
     pp.n_mops = ps.mop_end - ps.mop_begin;
@@ -380,6 +388,32 @@ static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
     return TTN_OK;
 }
 
+static ttn_status launch_backtrace(ttn_plan* P, cudaStream_t st) {
+    {
+        const Layout& y = P->lay;
+        ttn::ArgmaxParams ap{};
+        ap.L = P->L; ap.NS = y.NS; ap.nblk = y.amax_blocks;
+        ap.c_stride = (unsigned long long)P->L * y.NS;
+        ap.Jv = reinterpret_cast<const float*>(P->ws + y.Jv);
+        ap.Jh = reinterpret_cast<const float*>(P->ws + y.Jh);
+        ap.h = P->has_field ? reinterpret_cast<const float*>(P->ws + y.h) : nullptr;
+        ap.s_next = ap.s_out = reinterpret_cast<unsigned long long*>(P->ws + y.out_s);
+        ap.part_v = reinterpret_cast<float*>(P->ws + y.amax_v);
+        ap.part_s = reinterpret_cast<unsigned long long*>(P->ws + y.amax_s);
+        ap.v_out = reinterpret_cast<float*>(P->ws + y.out_x);
+        ap.sigma = reinterpret_cast<signed char*>(P->ws + y.sigma);
+        for (int r = P->L - 1; r >= 0; --r) {
+            ap.r = r; ap.has_next = (r < P->L - 1);
+            ap.C = reinterpret_cast<const float*>(P->ws + y.ckpt) + (unsigned long long)r * y.NS;
+            ttn::argmax_partial_kernel<<<dim3(ap.nblk, P->batch), 256, 0, st>>>(ap);
+            TTN_CUDA(cudaGetLastError());
+            ttn::argmax_final_kernel<<<P->batch, 32, 0, st>>>(ap);
+            TTN_CUDA(cudaGetLastError());
+        }
+    }
+    return TTN_OK;
+}
+
 extern "C" {
 
 const char* ttn_last_error(void) { return g_err; }
@@ -405,7 +439,8 @@ long ttn_plan_describe(int q, int L, ttn_call call, char* buf, size_t n) {
     if (call == TTN_CALL_ENERGY_I16 && s.empty()) call = TTN_CALL_ENERGY;
     if (s.empty() && fused_eligible(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) {
         ttn::FusedPlan fp = call == TTN_CALL_COUNT ? ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_COUNT)
-                                                   : ttn::make_fused_plan(L, ttn::FMAX_GATES);
+                          : call == TTN_CALL_CONFIG ? ttn::make_fused_row_plan(L, ttn::FMAX_GATES)
+                                                    : ttn::make_fused_plan(L, ttn::FMAX_GATES);
         if (fp.ok) s = ttn::describe_fused(fp);
     }
     if (s.empty()) s = ttn::describe(plan_for(q, L, call, /*has_field=*/q == 2));
@@ -475,7 +510,8 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
         P->fused = P->fplan.ok;
         if (!P->fused) { delete P; return fail(TTN_EUNSUPPORTED, "no Tropical<i16> schedule"); }
     } else if (fused_eligible(q, L, count, config)) {
-        P->fplan = count ? ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_COUNT) : ttn::make_fused_plan(L, ttn::FMAX_GATES);
+        P->fplan = count ? ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_COUNT)
+                 : config ? ttn::make_fused_row_plan(L, ttn::FMAX_GATES) : ttn::make_fused_plan(L, ttn::FMAX_GATES);
         P->fused = P->fplan.ok;
     }
     if (!P->fused) P->plan = plan_for(q, L, call, P->has_field);
@@ -505,7 +541,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     if (P->fused) {
         ttn_status fs = count ? setup_fcount(P, st) : setup_fused(P, st);
         if (fs != TTN_OK) { delete P; return fs; }
-        P->launches = (int)P->fplan.passes.size() + 1;
+        P->launches = (int)P->fplan.passes.size() + (config ? 2 * L : 1);
     } else {
         ttn::GenericPrepParams gp{};
         gp.q = q; gp.L = L; gp.n_ops = (int)P->plan.ops.size();
@@ -548,6 +584,7 @@ ttn_status ttn_plan_launch(ttn_plan* P, void* stream) {
             }
             for (auto& e : ev) cudaEventDestroy(e);
         }
+        if (P->config) return launch_backtrace(P, st);
         return TTN_OK;
     }
     const bool gtiming = getenv("TTN_DEBUG_TIMING") != nullptr;      // per-pass device times on stderr
@@ -570,28 +607,7 @@ ttn_status ttn_plan_launch(ttn_plan* P, void* stream) {
         }
         for (auto& e : gev) cudaEventDestroy(e);
     }
-    if (P->config) {
-        const Layout& y = P->lay;
-        ttn::ArgmaxParams ap{};
-        ap.L = P->L; ap.NS = y.NS; ap.nblk = y.amax_blocks;
-        ap.c_stride = (unsigned long long)P->L * y.NS;
-        ap.Jv = reinterpret_cast<const float*>(P->ws + y.Jv);
-        ap.Jh = reinterpret_cast<const float*>(P->ws + y.Jh);
-        ap.h = P->has_field ? reinterpret_cast<const float*>(P->ws + y.h) : nullptr;
-        ap.s_next = ap.s_out = reinterpret_cast<unsigned long long*>(P->ws + y.out_s);
-        ap.part_v = reinterpret_cast<float*>(P->ws + y.amax_v);
-        ap.part_s = reinterpret_cast<unsigned long long*>(P->ws + y.amax_s);
-        ap.v_out = reinterpret_cast<float*>(P->ws + y.out_x);
-        ap.sigma = reinterpret_cast<signed char*>(P->ws + y.sigma);
-        for (int r = P->L - 1; r >= 0; --r) {
-            ap.r = r; ap.has_next = (r < P->L - 1);
-            ap.C = reinterpret_cast<const float*>(P->ws + y.ckpt) + (unsigned long long)r * y.NS;
-            ttn::argmax_partial_kernel<<<dim3(ap.nblk, P->batch), 256, 0, st>>>(ap);
-            TTN_CUDA(cudaGetLastError());
-            ttn::argmax_final_kernel<<<P->batch, 32, 0, st>>>(ap);
-            TTN_CUDA(cudaGetLastError());
-        }
-    }
+    if (P->config) return launch_backtrace(P, st);
     return TTN_OK;
 }
 

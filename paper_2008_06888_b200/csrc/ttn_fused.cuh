@@ -46,8 +46,10 @@ __host__ __device__ constexpr size_t fsmem_bytes(bool low) {
 
 struct FusedParams {
     int L, a, low, flags, first_layout, last_layout, batch;
-    float* state;                       // instance 0
+    float* state;                       // instance 0: where the pass WRITES (and reads, unless src is set)
     unsigned long long inst_stride;     // elements between instances
+    const float* src;                   // where the pass READS (row-aligned plans: a checkpoint); else = state
+    unsigned long long src_stride;
     unsigned long long tiles_per_inst;  // warp tiles (2^12 elements) per instance
     const MicroOp* mops; int n_mops;    // this pass's program
     const float* gate_k; int n_gates;   // [inst][all gates][8]; this pass's slice of instance 0
@@ -450,6 +452,7 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
             for (int i = tid; i < FFINAL_FLOATS; i += blockDim.x) s_fin[i] = p.final_tab[(size_t)inst * FFINAL_FLOATS + i];
         __syncthreads();
         float* S = p.state + (unsigned long long)inst * p.inst_stride;
+        float* SRC = const_cast<float*>(p.src) + (unsigned long long)inst * p.src_stride;
         float wmax = -INFINITY;
 
         // HIGH: the 4 warps of a group (one per scheduler) take 4 consecutive tiles -- the 4 sectors
@@ -467,7 +470,7 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
         const bool async_load = !LOW && !(p.flags & PASS_INIT) && p.prefetch_pc >= 0;
         if (async_load) {                               // the first tile of this warp
             group_sync(warp);
-            if (tile_of(0) < p.tiles_per_inst) pf_issue(myreg, S + high_base(tile_of(0)), lane, p.stride_bytes, p.a);
+            if (tile_of(0) < p.tiles_per_inst) pf_issue(myreg, SRC + high_base(tile_of(0)), lane, p.stride_bytes, p.a);
         }
         for (unsigned long long it = 0;; ++it) {
             const unsigned long long wt = tile_of(it);
@@ -500,11 +503,11 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
 #pragma unroll
                 for (int j = 0; j < 128; ++j) v[j] = 0.f;                         // tropical one
             } else if (LOW) {
-                gmove<LOW, 1, false>(v, S + base, lane, p.stride_bytes, p.a);
+                gmove<LOW, 1, false>(v, SRC + base, lane, p.stride_bytes, p.a);
             } else if (!async_load) {
                 group_sync(warp);
-                if (p.first_layout == 1) gmove<LOW, 1, false>(v, S + base, lane, p.stride_bytes, p.a);
-                else gmove<LOW, 0, false>(v, S + base, lane, p.stride_bytes, p.a);
+                if (p.first_layout == 1) gmove<LOW, 1, false>(v, SRC + base, lane, p.stride_bytes, p.a);
+                else gmove<LOW, 0, false>(v, SRC + base, lane, p.stride_bytes, p.a);
             } else {
                 // the tile was fetched into this warp's region while the previous tile was computed
                 asm volatile("cp.async.wait_group 0;" ::: "memory");
@@ -521,7 +524,7 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
                 if (async_load && pc == p.prefetch_pc) {    // the region is free from here on: fetch the next tile
                     const unsigned long long wn = tile_of(it + 1);
                     group_sync(warp);                       // the group's 4 sectors of every line are requested together
-                    if (wn < p.tiles_per_inst) pf_issue(myreg, S + high_base(wn), lane, p.stride_bytes, p.a);
+                    if (wn < p.tiles_per_inst) pf_issue(myreg, SRC + high_base(wn), lane, p.stride_bytes, p.a);
                 }
                 const unsigned code = op & 0xffu;
                 if (code == MC_END || code == MC_FINAL) break;

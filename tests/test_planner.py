@@ -148,7 +148,7 @@ DIGIT_OF_BIT_I16 = {(1, 0): [1 + d for d in [5, 6, 0, 1, 2, 3, 4]] + [0], (1, 1)
                     (0, 0): [4, 5, 6, 0, 1, 2, 3], (0, 1): [4, 3, 2, 8, 7, 6, 5]}
 
 
-def fused_to_gates(L, fpasses, count=False, i16=False):
+def fused_to_gates(L, fpasses, count=False, i16=False, config=False):
     """Check the structure of the micro-op program (layouts, register bits, rounds) and the
     three-point-stencil dependency rule; return the flat (r, c) gate sequence."""
     flat = []
@@ -160,7 +160,7 @@ def fused_to_gates(L, fpasses, count=False, i16=False):
         assert (low == 1 and a == 0 and Wt == wl) or (low == 0 and a >= (5 if i16 else 4) and Wt == wh)
         assert a + Wt <= L
         assert (ps["flags"] & 1) == (1 if i == 0 else 0)
-        last = i == len(fpasses) - 1
+        last = i == len(fpasses) - 1 and not config
         assert bool(ps["flags"] & 2) == last
         if low:
             assert ps["first"] == 1 and ps["last"] == 1     # coalesced global layout
@@ -250,6 +250,28 @@ def test_fused_i16_schedule_obeys_dependency_rule(L):
     assert int(head["L"]) == L
     flat = fused_to_gates(L, fpasses, i16=True)
     assert len(flat) == L * (L - 1) == len(set(flat))
+
+
+@pytest.mark.parametrize("L", [12, 13, 16, 20, 21, 22, 28])
+def test_fused_row_aligned_schedule(L):
+    """ttn_ground_config on the fused kernel: every row boundary is a checkpoint; the pass that
+    completes row r writes C_r, the next one reads it (src/dst chain)."""
+    head, fpasses = parse_fused(describe(2, L, 2, fused=True))
+    flat = fused_to_gates(L, fpasses, config=True)
+    assert len(flat) == L * (L - 1)
+    rows = [r for r, c in flat]
+    assert rows == sorted(rows)                              # no gate of row r+1 before row r is complete
+    assert fpasses[0]["gates"] == 0 and fpasses[0]["src"] == -1 and fpasses[0]["dst"] == 0
+    done, seen = 0, 0
+    for i, ps in enumerate(fpasses[1:], 1):
+        assert ps["src"] == fpasses[i - 1]["dst"]
+        seen += ps["gates"]
+        if seen == (done + 1) * L:
+            done += 1
+            assert ps["dst"] == done
+        else:
+            assert ps["dst"] == -1
+    assert done == L - 1
 
 
 @pytest.mark.parametrize("L", [12, 13, 16])
