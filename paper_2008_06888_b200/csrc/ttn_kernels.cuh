@@ -347,15 +347,30 @@ __global__ void __launch_bounds__(256) argmax_partial_kernel(const ArgmaxParams 
         kacc[c] = (float)ks;
     }
     __syncthreads();
+    // w(s) = sum_c jsig[c] sigma_c + sum_c kacc[c] sigma_c sigma_{c+1}, split into one 256-entry
+    // table per byte of s (terms inside the byte) + one sign per byte boundary
+    __shared__ float tab[4][256];                    // L <= 28 for this call
+    const int nchunk = (p.L + 7) >> 3;
+    for (int m = 0; m < nchunk; ++m) {
+        const int v = threadIdx.x;                   // blockDim.x = 256
+        float acc = 0.f;
+        for (int i = 0; i < 8 && 8 * m + i < p.L; ++i) {
+            const int c = 8 * m + i, b = (v >> i) & 1;
+            acc += b ? -jsig[c] : jsig[c];
+            if (i + 1 < 8 && c + 1 < p.L) acc += (b == ((v >> (i + 1)) & 1)) ? kacc[c] : -kacc[c];
+        }
+        tab[m][v] = acc;
+    }
+    __syncthreads();
     const float* C = p.C + inst * p.c_stride;
     float bv = -INFINITY; unsigned long long bs = ~0ull;
     for (unsigned long long s = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; s < p.NS;
          s += (unsigned long long)gridDim.x * blockDim.x) {
-        float w = 0.f;
         const unsigned long long x = s ^ (s >> 1);            // bit c set <=> sigma_c != sigma_{c+1}
-        for (int c = 0; c < p.L; ++c) {
-            w += ((s >> c) & 1ull) ? -jsig[c] : jsig[c];
-            if (c + 1 < p.L) w += ((x >> c) & 1ull) ? -kacc[c] : kacc[c];
+        float w = tab[0][s & 255u];
+        for (int m = 1; m < nchunk; ++m) {
+            w += tab[m][(s >> (8 * m)) & 255u];
+            w += ((x >> (8 * m - 1)) & 1ull) ? -kacc[8 * m - 1] : kacc[8 * m - 1];
         }
         argmax_combine(bv, bs, C[s] + w, s);
     }
