@@ -357,3 +357,40 @@ def test_i16_rejects_non_integer_and_large_couplings():
     with pytest.raises(ttn.TTNError) as e:
         ttn.sweep_energy_i16(100 * Jh, 100 * Jv)
     assert e.value.status == 1
+
+
+# ------------------------------------------------------------------ SURVEY.md NEXT-2 sizes
+def test_next2_count_32x32():
+    """Degeneracy of the 32x32 +-J instance of cfg 4 (2^32 counting elements, 51.5 GB): the paper's
+    largest entropy size.  No oracle value exists at this size (the count needs a
+    64 GB u128 frontier); pins: E0 equals the O-dp energy, the count is even (global flip, h = 0)
+    and invariant under the lattice transpose up to f64 summation order."""
+    import torch
+    L = 32
+    free, _ = torch.cuda.mem_get_info()
+    need = ttn.workspace_bytes(2, L, ttn.COUNTING_F32_F64, 1)
+    if free < need + (2 << 30):
+        pytest.skip("needs %.0f GB of free device memory" % (need / 1e9))
+    ws = ttn.alloc_workspace(need)
+    Jh, Jv, _ = config_batch(4)
+    E0, g = ttn.sweep_count(Jh, Jv, workspace=ws)
+    assert E0[0] == golden()[("ising_energy", 32, 4000)][0]
+    assert g[0] >= 2 and np.isfinite(g[0])
+    Et, gt = ttn.sweep_count(np.ascontiguousarray(Jv.transpose(0, 2, 1)),
+                             np.ascontiguousarray(Jh.transpose(0, 2, 1)), workspace=ws)
+    assert Et[0] == E0[0] and abs(gt[0] - g[0]) <= 1e-12 * g[0]
+    if g[0] < 2 ** 53:
+        assert g[0] % 2 == 0
+    del ws
+    torch.cuda.empty_cache()
+
+
+def test_next2_ground_config_24x24():
+    """Ground configuration at L = 24 (24 checkpoints of 64 MiB): the energy of the returned
+    configuration, evaluated with Eq. (1) in f64, equals the O-dp ground energy (bit-exact, +-J)."""
+    gold = golden()
+    Jh, Jv, _ = make_batch(24, [4000, 4001], "pmj")
+    E0, sig = ttn.ground_config(Jh, Jv)
+    for b, seed in enumerate((4000, 4001)):
+        assert E0[b] == gold[("ising_energy", 24, seed)][0]
+        assert oracle.ising_energy(24, Jh[b], Jv[b], None, sig[b]) == E0[b]
