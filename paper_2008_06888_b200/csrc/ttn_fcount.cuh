@@ -34,6 +34,9 @@ struct CountParams {
     double* part_n;                     // [batch][part_stride]
 };
 
+// 1.0 / 0.0 from a predicate: only the high word of the double is selected
+__device__ __forceinline__ double ind(bool p) { return __hiloint2double(p ? 0x3ff00000 : 0, 0); }
+
 // ---- counting gate on register bit K ------------------------------------------------------------------
 template <int K, int PN, int QN>
 __device__ __forceinline__ void cgate_count(float (&x)[32], double (&n)[32], const float4 c0, const float4 c1,
@@ -55,9 +58,16 @@ __device__ __forceinline__ void cgate_count(float (&x)[32], double (&n)[32], con
         const float xa = x[j], xb = x[j + B];
         const double na = n[j], nb = n[j + B];
         const float ca = xb + ka[np][nq], cb = xa + kb[np][nq];
+#ifdef TTN_COUNT_SELECT
         const double ns = na + nb;
         n[j] = ca > xa ? nb : (ca == xa ? ns : na);
         n[j + B] = cb > xb ? na : (cb == xb ? ns : nb);
+#else
+        // Eq. (4) as n' = n_keep [keep >= cand] + n_cand [cand >= keep] with 0/1 factors: the selects
+        // of 64-bit counts (alu pipe, two per count) become one FP64 multiply-add each (exact: x 1, x 0)
+        n[j] = fma(nb, ind(ca >= xa), na * ind(xa >= ca));
+        n[j + B] = fma(na, ind(cb >= xb), nb * ind(xb >= cb));
+#endif
         x[j] = fmaxf(xa, ca);
         x[j + B] = fmaxf(xb, cb);
     }
