@@ -66,6 +66,13 @@ __device__ __forceinline__ void oplus(float& x, double& n, float cx, double cn) 
     x = fmaxf(x, cx);
 }
 
+// 3-input max: one FMNMX3 on sm_100
+__device__ __forceinline__ float max3(float a, float b, float c) {
+    float r; asm("max.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c)); return r;
+}
+// 1.0 / 0.0 from a predicate (only the high word of the double is selected)
+__device__ __forceinline__ double ind01(bool p) { return __hiloint2double(p ? 0x3ff00000 : 0, 0); }
+
 // exact n / d for n * d < 2^32 with the host-side magic M = floor(2^32 / d) + 1
 __device__ __forceinline__ unsigned fastdiv(unsigned n, unsigned magic) { return __umulhi(n, magic); }
 __host__ __device__ inline unsigned fastdiv_magic(unsigned d) { return d <= 1 ? 0u : (unsigned)(0x100000000ull / d) + 1u; }
@@ -183,20 +190,24 @@ __global__ void __launch_bounds__(512) pass_kernel(const PassParams p) {
                     x[t] = sx[i0 + t * st] + R[t];
                 }
                 if (COUNT) {
+                    // Eq. (4) over three candidates: count = sum of n_t over the exact maximisers; the
+                    // 0/1 indicators make it FP64 multiply-adds instead of 64-bit selects
                     double n[3];
 #pragma unroll
                     for (int t = 0; t < 3; ++t) n[t] = sn[i0 + t * st];
 #pragma unroll
                     for (int tn = 0; tn < 3; ++tn) {
-                        float y = x[tn] + J; double m = n[tn];
+                        float c[3];
 #pragma unroll
-                        for (int t = 0; t < 3; ++t) if (t != tn) oplus<true>(y, m, x[t], n[t]);
-                        sx[i0 + tn * st] = y - R[tn]; sn[i0 + tn * st] = m;
+                        for (int t = 0; t < 3; ++t) c[t] = t == tn ? x[t] + J : x[t];
+                        const float best = max3(c[0], c[1], c[2]);
+                        const double m = fma(n[2], ind01(c[2] == best), fma(n[1], ind01(c[1] == best), n[0] * ind01(c[0] == best)));
+                        sx[i0 + tn * st] = best - R[tn]; sn[i0 + tn * st] = m;
                     }
                 } else {
-                    sx[i0] = fmaxf(x[0] + J, fmaxf(x[1], x[2])) - R[0];
-                    sx[i0 + st] = fmaxf(x[1] + J, fmaxf(x[0], x[2])) - R[1];
-                    sx[i0 + 2 * st] = fmaxf(x[2] + J, fmaxf(x[0], x[1])) - R[2];
+                    sx[i0] = max3(x[0] + J, x[1], x[2]) - R[0];
+                    sx[i0 + st] = max3(x[1] + J, x[0], x[2]) - R[1];
+                    sx[i0 + 2 * st] = max3(x[2] + J, x[0], x[1]) - R[2];
                 }
             }
         }
