@@ -28,12 +28,12 @@
 
 namespace ttn {
 
-enum OpType : uint8_t { OP_GATE = 0, OP_DH = 1, OP_DJ = 2 };
+enum OpType : uint8_t { OP_GATE = 0 };     // diagonal frame: gates are the only scheduled operation
 
 struct Op {            // 8 bytes, uploaded as-is
     uint8_t type;      // OpType
     uint8_t pos;       // GATE: tile position of the digit (0 .. T-1)
-    uint8_t c;         // global column (digit) -- DJ: left digit, pair (c, c+1)
+    uint8_t c;         // global column (digit)
     uint8_t first;     // 1 = first gate of a round (the gates of a round commute: all were legal together)
     uint16_t row;      // lattice row r of the operation
     uint16_t pad2;
@@ -173,7 +173,7 @@ inline std::string describe(const Plan& p) {
         for (int k = ps.op_begin; k < ps.op_end; ++k) {
             const Op& o = p.ops[k];
             snprintf(line, sizeof line, "op %s r=%d c=%d pos=%d\n",
-                     o.type == OP_GATE ? "g" : (o.type == OP_DH ? "dh" : "dJ"), o.row, o.c, o.pos);
+                     "g", o.row, o.c, o.pos);
             out += line;
         }
     }

@@ -89,7 +89,7 @@ bool fused_eligible(int q, int L, bool count, bool config) {
     return count ? L >= ttn::CW_LOW : L >= ttn::F_WLOW;      // config: row-aligned f32 plan
 }
 
-// The op list length is bounded by L*L gates + 2*L*L diagonals.
+// The op list of a plan holds the L(L-1) gates of the sweep (diagonal frame: no diagonal op).
 Layout make_layout(int q, int L, bool count, bool config, int batch, bool i16 = false) {
     Layout y;
     y.NS = ipow(q, L);
