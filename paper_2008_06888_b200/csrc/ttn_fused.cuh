@@ -12,11 +12,15 @@
 //     (LOW) / 64-bit (HIGH) bank-conflict-free accesses, synchronised with __syncwarp only;
 //   * the last pass adds the accumulated diagonal A_{L-1}(s) (a 128-entry table over the
 //     register digits in 4 boundary variants + a per-thread scalar) and max-reduces.
-// Global traffic goes straight between HBM and registers: the LOW tile (columns 0..11) moves
-// 128-byte lines with immediate offsets; HIGH tiles (columns a..a+8 plus the riding columns 0..2
-// on the low lane bits) move whole 32-byte sectors, four per request, one IMAD.WIDE per address.
-// The kernel is persistent (one CTA per SM); programs and gate constants are staged in shared
-// memory once per launch and instance.
+// Global traffic: the LOW tile (columns 0..11) moves 128-byte lines straight between HBM and
+// registers with immediate offsets; HIGH tiles (columns a..a+8 plus the riding columns 0..2 on
+// the low lane bits) move whole 32-byte sectors, four per request, one IMAD.WIDE per address.
+// The 4 warps of a HIGH group own the 4 sectors of every line and meet at a named barrier before
+// they touch memory; where a tile spans few pages the NEXT tile is fetched with cp.async into the
+// warp's own exchange region as soon as the last exchange of the current tile is done.
+// The kernel is persistent (one CTA per SM, 12 warps); programs and gate constants are staged in
+// shared memory once per launch and instance.  ELEM = 1 instantiates the same kernel for
+// Tropical<i16> (two elements per 32-bit word, packed VIADDMNMX gates).
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
