@@ -36,7 +36,8 @@ struct Op {            // 8 bytes, uploaded as-is
     uint8_t c;         // global column (digit)
     uint8_t first;     // 1 = first gate of a round (the gates of a round commute: all were legal together)
     uint16_t row;      // lattice row r of the operation
-    uint16_t pad2;
+    uint16_t nb;       // q = 3 (mark_gate_blocks): this gate leads a block of nb gates on adjacent columns
+                       // of one row, applied together; 0 = member of the preceding block.  1 otherwise.
 };
 
 enum PassFlags : int { PASS_INIT = 1, PASS_REDUCE = 2 };
@@ -90,7 +91,7 @@ class Scheduler {
             if (legal.empty()) break;
             bool first = true;
             for (int c : legal) {
-                ops.push_back({OP_GATE, (uint8_t)pos_of(c), (uint8_t)c, (uint8_t)(first ? 1 : 0), (uint16_t)grow_[c], 0});
+                ops.push_back({OP_GATE, (uint8_t)pos_of(c), (uint8_t)c, (uint8_t)(first ? 1 : 0), (uint16_t)grow_[c], 1});
                 first = false;
                 ++gates;
             }
@@ -159,6 +160,31 @@ inline Plan make_plan(int q, int L, bool has_field, bool row_aligned, int Tmax, 
     return best;
 }
 
+// q = 3 (ttn_potts.cuh): group the gates of every round into blocks of up to max_nb gates on
+// adjacent columns held at adjacent tile positions.  Gates legal in the same round on adjacent
+// columns belong to the same lattice row (each needs its neighbour to be at least as far), so a
+// block shares one conjugation A_{r-1}.  Runs are cut 3,3,..., with a tail of 2+2 instead of 3+1.
+inline void mark_gate_blocks(Plan& p, int max_nb = 3) {
+    for (const Pass& ps : p.passes) {
+        int k = ps.op_begin;
+        while (k < ps.op_end) {
+            int run = 1;
+            while (k + run < ps.op_end && !p.ops[k + run].first && p.ops[k + run].row == p.ops[k].row &&
+                   p.ops[k + run].c == p.ops[k + run - 1].c + 1 && p.ops[k + run].pos == p.ops[k + run - 1].pos + 1)
+                ++run;
+            int left = run, i = k;
+            while (left > 0) {
+                int nb = left < max_nb ? left : max_nb;
+                if (max_nb == 3 && left == 4) nb = 2;
+                p.ops[i].nb = (uint16_t)nb;
+                for (int j = 1; j < nb; ++j) p.ops[i + j].nb = 0;
+                i += nb; left -= nb;
+            }
+            k += run;
+        }
+    }
+}
+
 inline std::string describe(const Plan& p) {
     std::string out;
     char line[160];
@@ -172,8 +198,8 @@ inline std::string describe(const Plan& p) {
         out += line;
         for (int k = ps.op_begin; k < ps.op_end; ++k) {
             const Op& o = p.ops[k];
-            snprintf(line, sizeof line, "op %s r=%d c=%d pos=%d\n",
-                     "g", o.row, o.c, o.pos);
+            snprintf(line, sizeof line, "op %s r=%d c=%d pos=%d first=%d nb=%d\n",
+                     "g", o.row, o.c, o.pos, o.first, o.nb);
             out += line;
         }
     }

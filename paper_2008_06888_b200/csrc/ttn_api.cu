@@ -14,6 +14,7 @@
 #include "../../include/ttn.h"
 #include "planner.h"
 #include "ttn_kernels.cuh"
+#include "ttn_potts.cuh"
 #include "ttn_fused.cuh"
 #include "ttn_fcount.cuh"
 
@@ -155,7 +156,13 @@ struct ttn_plan {
 static ttn::Plan plan_for(int q, int L, ttn_call call, bool has_field) {
     const bool count = (call == TTN_CALL_COUNT);
     const TileCfg tc = tile_cfg(q, count);
-    return ttn::make_plan(q, L, has_field, call == TTN_CALL_CONFIG, tc.Tmax, tc.ride);
+    ttn::Plan p = ttn::make_plan(q, L, has_field, call == TTN_CALL_CONFIG, tc.Tmax, tc.ride);
+    if (q == 3) {
+        int max_nb = count ? ttn::POTTS_MAX_NB_COUNT : 3;
+        if (const char* e = getenv("TTN_DEBUG_NB")) { int v = atoi(e); if (v >= 1 && v <= max_nb) max_nb = v; }
+        ttn::mark_gate_blocks(p, max_nb);
+    }
+    return p;
 }
 
 template <int Q, bool COUNT>
@@ -185,12 +192,32 @@ static ttn_status launch_pass(const ttn_plan* P, const ttn::Pass& ps, cudaStream
     pp.part_x = reinterpret_cast<float*>(P->ws + y.part_x);
     pp.part_n = reinterpret_cast<double*>(P->ws + y.part_n);
     const size_t smem = (size_t)pp.n_tile * (COUNT ? 12 : 4);
-    ttn_status s = set_smem(ttn::pass_kernel<Q, COUNT>, smem);
-    if (s != TTN_OK) return s;
     const unsigned long long grid = pp.tiles_per_inst * (unsigned long long)P->batch;
     if (grid > 0x7fffffffull) return fail(TTN_EUNSUPPORTED, "grid too large");
-    unsigned threads = pp.n_tile / Q >= 512 ? 512 : (pp.n_tile / Q < 32 ? 32 : ((pp.n_tile / Q + 31) / 32 * 32));
-    ttn::pass_kernel<Q, COUNT><<<(unsigned)grid, threads, smem, st>>>(pp);
+    if constexpr (Q == 3) {    // Potts: register-blocked gates (ttn_potts.cuh)
+        // persistent CTAs, two residents per SM (ttn_potts.cuh)
+        if (pp.n_ops > ttn::POTTS_MAX_OPS) return fail(TTN_EUNSUPPORTED, "too many gates in one Potts pass");
+        static int sms = 0;
+        if (!sms) { int dev = 0; TTN_CUDA(cudaGetDevice(&dev)); TTN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)); }
+        const unsigned ctas = grid < 2ull * sms ? (unsigned)grid : 2u * (unsigned)sms;
+        const size_t psmem = ttn::potts_buf_bytes(pp.n_tile, COUNT);
+        ttn_status s = TTN_OK;
+        if (pp.n_tile / 27 <= 128) {                                   // tiny lattices
+            s = set_smem(ttn::potts_pass_kernel<COUNT, 128>, psmem);
+            if (s != TTN_OK) return s;
+            ttn::potts_pass_kernel<COUNT, 128><<<ctas, 128, psmem, st>>>(pp, (unsigned)grid);
+        } else {
+            constexpr int TH = COUNT ? ttn::POTTS_THREADS_COUNT : ttn::POTTS_THREADS;
+            s = set_smem(ttn::potts_pass_kernel<COUNT, TH>, psmem);
+            if (s != TTN_OK) return s;
+            ttn::potts_pass_kernel<COUNT, TH><<<ctas, TH, psmem, st>>>(pp, (unsigned)grid);
+        }
+    } else {
+        ttn_status s = set_smem(ttn::pass_kernel<Q, COUNT>, smem);
+        if (s != TTN_OK) return s;
+        unsigned threads = pp.n_tile / Q >= 512 ? 512 : (pp.n_tile / Q < 32 ? 32 : ((pp.n_tile / Q + 31) / 32 * 32));
+        ttn::pass_kernel<Q, COUNT><<<(unsigned)grid, threads, smem, st>>>(pp);
+    }
     TTN_CUDA(cudaGetLastError());
     if (ps.flags & ttn::PASS_REDUCE) {
         ttn::final_reduce_kernel<COUNT><<<P->batch, 256, 0, st>>>(

@@ -132,6 +132,36 @@ def test_multipass_schedules_with_small_tiles(monkeypatch, tmax, ride):
                 assert (E0[b], g[b], E1[b]) == (Eo, go, Eo)
 
 
+@pytest.mark.parametrize("tmax,ride", [(3, 1), (4, 0), (5, 2)])
+def test_potts_blocks_persistent_ctas(monkeypatch, tmax, ride):
+    """Potts tile kernel (ttn_potts.cuh): integer couplings of several magnitudes (every bond
+    constant of a 1-, 2- and 3-gate block is distinct), tiny tiles so that each persistent CTA walks
+    many tiles and crosses the instance boundary of the batch."""
+    monkeypatch.setenv("TTN_DEBUG_TMAX", str(tmax))
+    monkeypatch.setenv("TTN_DEBUG_RIDE", str(ride))
+    L, B = 9, 2                                          # 3^(9-tmax) >= 81 tiles per instance
+    rng = np.random.default_rng(777 + tmax)
+    Jh = rng.integers(-3, 4, size=(B, L, L - 1)).astype(np.float32)
+    Jv = rng.integers(-3, 4, size=(B, L - 1, L)).astype(np.float32)
+    E0, g = ttn.potts3_sweep_count(Jh, Jv)
+    E1 = ttn.potts3_sweep_energy(Jh, Jv)
+    for b in range(B):
+        Eo, go, _ = oracle.dp_potts3(L, Jh[b], Jv[b])
+        assert (E0[b], g[b], E1[b]) == (Eo, go, Eo)
+
+
+def test_potts_gaussian_energy_f32_tolerance():
+    """App. C PAPER.md:296 with real-valued couplings: f32 sweep against the f64 oracle."""
+    L = 10
+    rng = np.random.default_rng(4242)
+    Jh = rng.standard_normal((2, L, L - 1)).astype(np.float32)
+    Jv = rng.standard_normal((2, L - 1, L)).astype(np.float32)
+    E1 = ttn.potts3_sweep_energy(Jh, Jv)
+    for b in range(2):
+        Eo, _, _ = oracle.dp_potts3(L, Jh[b], Jv[b])
+        assert abs(E1[b] - Eo) <= TOL * abs(Eo)
+
+
 # ------------------------------------------------------------------ mid sizes: several tiles + ragged
 @pytest.mark.parametrize("L", [15, 16, 17, 19])
 def test_mid_ising_count_vs_oracle(L):

@@ -94,6 +94,32 @@ def test_schedule_obeys_dependency_rule(q, L, call):
     validate(q, L, passes, fields=(q == 2), row_aligned=(call == 2))
 
 
+@pytest.mark.parametrize("L,call,tmax,ride", [(18, 1, None, None), (18, 0, None, None), (12, 0, None, None),
+                                              (6, 1, 4, 1), (5, 1, 3, 0), (3, 1, None, None)])
+def test_potts_gate_blocks(L, call, tmax, ride):
+    """csrc/planner.h mark_gate_blocks (ttn_potts.cuh): the gates of a q = 3 pass are applied in
+    blocks of up to three; a block is led by a gate with nb >= 1 and followed by nb - 1 gates with
+    nb = 0 on the next columns / tile positions of the SAME row and the SAME round (so they commute,
+    PAPER.md:118, and share one conjugation A_{r-1})."""
+    _, passes = parse(describe(3, L, call, tmax=tmax, ride=ride))
+    sizes = []
+    for ps in passes:
+        ops = ps["ops"]
+        k = 0
+        while k < len(ops):
+            nb = ops[k]["nb"]
+            assert 1 <= nb <= 3 and k + nb <= len(ops)
+            for j in range(1, nb):
+                o, pr = ops[k + j], ops[k + j - 1]
+                assert o["nb"] == 0 and o["first"] == 0
+                assert o["r"] == pr["r"] and o["c"] == pr["c"] + 1 and o["pos"] == pr["pos"] + 1
+            sizes.append(nb)
+            k += nb
+    assert sum(sizes) == L * (L - 1)
+    if L >= 6:
+        assert sizes.count(1) < len(sizes) // 2          # most gates ride in blocks of 2 or 3
+
+
 def test_fusion_cuts_hbm_passes():
     # SURVEY.md 8a-S8: cross-row fusion brings L=32 from 3 passes per row (93) to ~0.5 per row
     _, passes = parse(describe(2, 32, 0))
