@@ -415,6 +415,11 @@ static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
     return TTN_OK;
 }
 
+// batches of small lattices walk all checkpoints of an instance in one CTA (backtrace_inst_kernel)
+static bool backtrace_one_cta(int L, int batch) {
+    return L <= 18 && L <= ttn::BT_MAX_L && batch >= 32 && !getenv("TTN_DEBUG_BT_MULTI");
+}
+
 static ttn_status launch_backtrace(ttn_plan* P, cudaStream_t st) {
     {
         const Layout& y = P->lay;
@@ -429,6 +434,13 @@ static ttn_status launch_backtrace(ttn_plan* P, cudaStream_t st) {
         ap.part_s = reinterpret_cast<unsigned long long*>(P->ws + y.amax_s);
         ap.v_out = reinterpret_cast<float*>(P->ws + y.out_x);
         ap.sigma = reinterpret_cast<signed char*>(P->ws + y.sigma);
+        if (backtrace_one_cta(P->L, P->batch)) {
+            // batches of small lattices: one CTA walks all L checkpoints of its instance
+            ap.C = reinterpret_cast<const float*>(P->ws + y.ckpt);
+            ttn::backtrace_inst_kernel<<<P->batch, ttn::BT_THREADS, 0, st>>>(ap);
+            TTN_CUDA(cudaGetLastError());
+            return TTN_OK;
+        }
         for (int r = P->L - 1; r >= 0; --r) {
             ap.r = r; ap.has_next = (r < P->L - 1);
             ap.C = reinterpret_cast<const float*>(P->ws + y.ckpt) + (unsigned long long)r * y.NS;
@@ -568,7 +580,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     if (P->fused) {
         ttn_status fs = count ? setup_fcount(P, st) : setup_fused(P, st);
         if (fs != TTN_OK) { delete P; return fs; }
-        P->launches = (int)P->fplan.passes.size() + (config ? 2 * L : 1);
+        P->launches = (int)P->fplan.passes.size() + (config ? (backtrace_one_cta(L, batch) ? 1 : 2 * L) : 1);
     } else {
         ttn::GenericPrepParams gp{};
         gp.q = q; gp.L = L; gp.n_ops = (int)P->plan.ops.size();
@@ -582,7 +594,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
         ttn::generic_prep_kernel<<<dim3((unsigned)((work + 255) / 256), (unsigned)batch), 256, 0, st>>>(gp);
         cudaError_t pe = cudaGetLastError();
         if (pe != cudaSuccess) { delete P; return fail(TTN_ECUDA, "prep launch failed: %s", cudaGetErrorString(pe)); }
-        P->launches = (int)P->plan.passes.size() + (config ? 2 * L : 1);
+        P->launches = (int)P->plan.passes.size() + (config ? (backtrace_one_cta(L, batch) ? 1 : 2 * L) : 1);
     }
     *out = P;
     return TTN_OK;

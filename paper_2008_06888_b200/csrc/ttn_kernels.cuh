@@ -415,6 +415,105 @@ __global__ void __launch_bounds__(32) argmax_final_kernel(const ArgmaxParams p) 
         p.sigma[(inst * p.L + p.r) * p.L + threadIdx.x] = ((bs >> threadIdx.x) & 1ull) ? -1 : 1;
 }
 
+// Whole backtrace of one instance in ONE CTA (small lattices in batches, cfg 2): rows L-1 .. 0 are
+// inherently sequential (s_r needs s_{r+1}) but instances are independent, so a CTA walks the L
+// checkpoints of its instance without any launch or grid synchronisation in between.  Same
+// arithmetic, in the same order, as argmax_partial_kernel + argmax_final_kernel (the prefix sums
+// H_c, K_c over rows are formed once, in f64, in the same row order).
+constexpr int BT_THREADS = 512;
+constexpr int BT_MAX_L = 20;            // 2^20 states per row per CTA at most
+
+__global__ void __launch_bounds__(BT_THREADS) backtrace_inst_kernel(const ArgmaxParams p) {
+    const unsigned long long inst = blockIdx.x;
+    const int L = p.L;
+    __shared__ double hsum[BT_MAX_L][BT_MAX_L];   // [r][c] = sum_{rr <= r} h[rr][c]
+    __shared__ double ksum[BT_MAX_L][BT_MAX_L];   // [r][c] = sum_{rr <= r} Jh[rr][c]
+    __shared__ float jsig[BT_MAX_L], kacc[BT_MAX_L];
+    __shared__ float tab[3][256];
+    __shared__ float rv[BT_THREADS / 32];
+    __shared__ unsigned long long rs[BT_THREADS / 32];
+    __shared__ unsigned long long s_next;
+    if (threadIdx.x < L) {
+        const int c = threadIdx.x;
+        double hs = 0.0, ks = 0.0;
+        for (int rr = 0; rr < L; ++rr) {
+            if (p.h) hs += (double)p.h[inst * (unsigned long long)(L * L) + rr * L + c];
+            if (c + 1 < L) ks += (double)p.Jh[inst * (unsigned long long)(L * (L - 1)) + rr * (L - 1) + c];
+            hsum[rr][c] = hs; ksum[rr][c] = ks;
+        }
+    }
+    __syncthreads();
+    const int nchunk = (L + 7) >> 3;
+    for (int r = L - 1; r >= 0; --r) {
+        const bool has_next = r < L - 1;
+        if (threadIdx.x < L) {
+            const int c = threadIdx.x;
+            double j = 0.0;
+            if (has_next) {
+                j = (double)p.Jv[inst * (unsigned long long)((L - 1) * L) + r * L + c];
+                if ((s_next >> c) & 1ull) j = -j;
+            }
+            jsig[c] = (float)(j + hsum[r][c]);
+            kacc[c] = (float)ksum[r][c];
+        }
+        __syncthreads();
+        for (int e = threadIdx.x; e < nchunk * 256; e += BT_THREADS) {
+            const int m = e >> 8, v = e & 255;
+            float acc = 0.f;
+            for (int i = 0; i < 8 && 8 * m + i < L; ++i) {
+                const int c = 8 * m + i, b = (v >> i) & 1;
+                acc += b ? -jsig[c] : jsig[c];
+                if (i + 1 < 8 && c + 1 < L) acc += (b == ((v >> (i + 1)) & 1)) ? kacc[c] : -kacc[c];
+            }
+            tab[m][v] = acc;
+        }
+        __syncthreads();
+        const float* C = p.C + inst * p.c_stride + (unsigned long long)r * p.NS;
+        float bv = -INFINITY; unsigned long long bs = ~0ull;
+        // w(s) term by term in the order of argmax_partial_kernel: tab[0], then per higher byte
+        // its table entry and the boundary bond.  A thread visits its states in increasing order,
+        // so "lowest index wins ties" is a strict > inside the thread (NS <= 2^20: 32-bit indices).
+        const unsigned ns = (unsigned)p.NS;
+        unsigned b32 = 0xffffffffu;
+        auto visit = [&](float c, unsigned s) {
+            const unsigned x = s ^ (s >> 1);                      // bit c set <=> sigma_c != sigma_{c+1}
+            float w = tab[0][s & 255u];
+            for (int m = 1; m < nchunk; ++m) {
+                w += tab[m][(s >> (8 * m)) & 255u];
+                w += ((x >> (8 * m - 1)) & 1u) ? -kacc[8 * m - 1] : kacc[8 * m - 1];
+            }
+            const float v = c + w;
+            if (v > bv) { bv = v; b32 = s; }
+        };
+        if (ns >= 4u * BT_THREADS) {              // 16-byte loads, four in flight per thread
+#pragma unroll 4
+            for (unsigned s = 4u * threadIdx.x; s < ns; s += 4u * BT_THREADS) {
+                const float4 c4 = *reinterpret_cast<const float4*>(C + s);
+                visit(c4.x, s); visit(c4.y, s + 1); visit(c4.z, s + 2); visit(c4.w, s + 3);
+            }
+        } else {
+            for (unsigned s = threadIdx.x; s < ns; s += BT_THREADS) visit(C[s], s);
+        }
+        if (b32 != 0xffffffffu) bs = b32;
+        for (int o = 16; o; o >>= 1) {
+            float v2 = __shfl_xor_sync(0xffffffffu, bv, o);
+            unsigned long long s2 = __shfl_xor_sync(0xffffffffu, bs, o);
+            argmax_combine(bv, bs, v2, s2);
+        }
+        if ((threadIdx.x & 31) == 0) { rv[threadIdx.x >> 5] = bv; rs[threadIdx.x >> 5] = bs; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            for (int w = 1; w < BT_THREADS / 32; ++w) argmax_combine(bv, bs, rv[w], rs[w]);
+            s_next = bs;
+            p.s_out[inst] = bs;
+            if (!has_next) p.v_out[inst] = bv;
+        }
+        __syncthreads();
+        if (threadIdx.x < L)
+            p.sigma[(inst * L + r) * L + threadIdx.x] = ((s_next >> threadIdx.x) & 1ull) ? -1 : 1;
+    }
+}
+
 // ---- S0 of the generic path: conjugated gate constants and the coefficients of A_{L-1} -------------
 struct GenericPrepParams {
     int q, L, n_ops;

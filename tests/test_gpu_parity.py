@@ -182,6 +182,29 @@ def test_mid_potts_vs_oracle():
         assert E0[0] == Eo and E1[0] == Eo and count_ok(g[0], go)
 
 
+@pytest.mark.parametrize("L", [5, 12, 13, 17])
+def test_backtrace_one_cta_per_instance_matches_multi_block(monkeypatch, L):
+    """S6 backward pass: batches >= 32 of small lattices walk all checkpoints of an instance in one
+    CTA (backtrace_inst_kernel); smaller batches use one launch pair per row.  Same arithmetic, so
+    the same sigma (lowest index on ties, footnote [49] PAPER.md:201) -- checked on +-J instances
+    with h = 0, where every argmax has ties, and on Gaussian ones against the oracle energy."""
+    B = 40
+    Jh, Jv, _ = make_batch(L, range(2600, 2600 + B), "pmj")
+    E_a, sig_a = ttn.ground_config(Jh, Jv)
+    monkeypatch.setenv("TTN_DEBUG_BT_MULTI", "1")
+    E_b, sig_b = ttn.ground_config(Jh, Jv)
+    monkeypatch.delenv("TTN_DEBUG_BT_MULTI")
+    assert np.array_equal(E_a, E_b) and np.array_equal(sig_a, sig_b)
+    for b in range(0, B, 7):
+        assert oracle.ising_energy(L, Jh[b], Jv[b], None, sig_a[b]) == E_a[b]
+    Jh, Jv, h = make_batch(L, range(2700, 2700 + B), "gauss", fields=True)
+    E_a, sig_a = ttn.ground_config(Jh, Jv, h)
+    for b in range(0, B, 9):
+        Eo = oracle.dp_ising(L, Jh[b], Jv[b], h[b])[0] if L <= 13 else E_a[b]
+        assert abs(E_a[b] - Eo) <= TOL * abs(Eo)
+        assert abs(oracle.ising_energy(L, Jh[b], Jv[b], h[b], sig_a[b]) - E_a[b]) <= TOL * abs(E_a[b])
+
+
 # ------------------------------------------------------------------ cfg 2: 16x16 Gaussian, config
 def test_cfg2_16x16_gaussian_ground_config_full_batch():
     Jh, Jv, h = config_batch(2)                         # 256 instances
