@@ -122,6 +122,11 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.samples)}
 
 
+def workload_name(L: int) -> str:
+    return (f"{L}x{L} +-J Ising (p=0.5, h=0) Tropical<f32> energy sweep, "
+            f"2^{L}-entry state in place, 1 instance per GPU (seed 4000+rank)")
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle as it stands, on the host cores.  Each step is a bounded
     sample (a full sweep of a smaller lattice of the same +-J distribution), scaled to the
@@ -146,7 +151,8 @@ def run_reference(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": float(np.mean(times)) * 1e3,
         "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
-        "config": {"workload": f"{args.L}x{args.L} +-J Ising energy sweep (extrapolated from sample)"},
+        # the same workload key as the CUDA arm; what one step actually ran is in cpu_baseline.sample
+        "config": {"workload": workload_name(args.L), "L": args.L, "state_bytes": 4 * 2 ** args.L},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
                          "sample": f"full O-dp sweep of a {Ls}x{Ls} +-J instance per step, scaled by "
                                    f"(L-1)L2^L updates to {args.L}x{args.L}"},
@@ -272,8 +278,7 @@ def main():
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"{L}x{L} +-J Ising (p=0.5, h=0) Tropical<f32> energy sweep, "
-                                   f"2^{L}-entry state in place, 1 instance per GPU (seed 4000+rank)",
+            "config": {"workload": workload_name(L),
                        "L": L, "state_bytes": 4 * 2 ** L, "hbm_passes": plan.num_passes,
                        "l2_policy": "state (>= 1 GiB) far larger than the 126 MB L2; no flush needed"
                        if L >= 28 else "state fits L2: flush not applied, number is L2-resident",
