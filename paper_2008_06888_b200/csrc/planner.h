@@ -21,6 +21,7 @@
 // Host only; no CUDA.  The same structures are dumped by ttn_plan_describe() and replayed by
 // tests/test_planner.py against an independent statement of the rule.
 #pragma once
+#include <algorithm>
 #include <cstdint>
 #include <cstdio>
 #include <string>
@@ -158,6 +159,83 @@ inline Plan make_plan(int q, int L, bool has_field, bool row_aligned, int Tmax, 
         if (!have || p.passes.size() < best.passes.size()) { best = p; have = true; }
     }
     return best;
+}
+
+// Beam search over tile sequences (any tile at any step instead of a fixed cycle): minimises the
+// number of HBM passes of a multi-pass sweep; among sequences of equal length the one with more
+// low (contiguous) tiles wins, since a strided pass costs about twice the memory time of a
+// contiguous one (profiles/r01j.md).  States are the per-column progress vectors; a layer holds
+// the `width` states with the most gates applied.  Used for the q = 3 plans, where a pass costs
+// 15-20 ms of memory time before its first gate.
+inline Plan make_plan_beam(int q, int L, int Tmax, int ride, int width = 256) {
+    const int wh = Tmax - ride;
+    std::vector<TileSpec> tiles;
+    tiles.push_back({Tmax, Tmax, Tmax});
+    for (int a = ride + 1; a + wh <= L; ++a) tiles.push_back({ride, a, a + wh});
+    struct Node { std::vector<int> grow; std::vector<int> seq; int total; int lows; };
+    auto advance = [&](const std::vector<int>& g0, const TileSpec& t, std::vector<int>& g1) {
+        g1 = g0;
+        int gates = 0;
+        auto in_tile = [&](int c) { return c < t.lo || (c >= t.a && c < t.b); };
+        for (;;) {
+            int legal[64], nl = 0;
+            for (int c = 0; c < L; ++c) {
+                if (!in_tile(c)) continue;
+                const int r = g1[c];
+                if (r >= L) continue;
+                if (c > 0 && g1[c - 1] < r) continue;
+                if (c + 1 < L && g1[c + 1] < r) continue;
+                legal[nl++] = c;
+            }
+            if (!nl) break;
+            for (int i = 0; i < nl; ++i) g1[legal[i]] += 1;
+            gates += nl;
+        }
+        return gates;
+    };
+    std::vector<Node> layer(1);
+    layer[0].grow.assign(L, 1); layer[0].total = 0; layer[0].lows = 0;
+    std::vector<int> best_seq;
+    for (int depth = 0; depth < 4 * L && best_seq.empty(); ++depth) {
+        std::vector<Node> next;
+        for (const Node& nd : layer)
+            for (size_t ti = 0; ti < tiles.size(); ++ti) {
+                Node nn;
+                const int g = advance(nd.grow, tiles[ti], nn.grow);
+                if (g == 0 && depth > 0) continue;
+                nn.seq = nd.seq; nn.seq.push_back((int)ti);
+                nn.total = nd.total + g; nn.lows = nd.lows + (ti == 0);
+                next.push_back(std::move(nn));
+            }
+        if (next.empty()) break;
+        // best first: most gates applied, then most low tiles; drop duplicates of a progress vector
+        std::stable_sort(next.begin(), next.end(), [](const Node& x, const Node& y) {
+            if (x.total != y.total) return x.total > y.total;
+            return x.lows > y.lows;
+        });
+        layer.clear();
+        for (Node& nn : next) {
+            bool dup = false;
+            for (const Node& k : layer) if (k.grow == nn.grow) { dup = true; break; }
+            if (dup) continue;
+            if (nn.total == L * (L - 1)) { if (best_seq.empty()) best_seq = nn.seq; continue; }
+            if ((int)layer.size() < width) layer.push_back(std::move(nn));
+        }
+    }
+    Plan p; p.q = q; p.L = L; p.row_aligned = false;
+    if (best_seq.empty()) return p;
+    Scheduler s(L);
+    for (size_t i = 0; i < best_seq.size(); ++i) {
+        const TileSpec& t = tiles[best_seq[i]];
+        Pass ps{t.lo, t.a, t.b, (int)p.ops.size(), 0, 0, -1, -1, 0};
+        ps.n_gates = s.run_pass(t, L, p.ops);
+        ps.op_end = (int)p.ops.size();
+        if (i == 0) ps.flags |= PASS_INIT;
+        p.passes.push_back(ps);
+    }
+    if (!s.done()) { p.passes.clear(); p.ops.clear(); return p; }
+    p.passes.back().flags |= PASS_REDUCE;
+    return p;
 }
 
 // q = 3 (ttn_potts.cuh): group the gates of every round into blocks of up to max_nb gates on

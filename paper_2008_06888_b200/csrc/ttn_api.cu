@@ -5,6 +5,9 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
+#include <mutex>
+#include <tuple>
 #include <new>
 #include <string>
 #include <vector>
@@ -157,6 +160,15 @@ static ttn::Plan plan_for(int q, int L, ttn_call call, bool has_field) {
     const bool count = (call == TTN_CALL_COUNT);
     const TileCfg tc = tile_cfg(q, count);
     ttn::Plan p = ttn::make_plan(q, L, has_field, call == TTN_CALL_CONFIG, tc.Tmax, tc.ride);
+    if (q == 3 && L > tc.Tmax && !getenv("TTN_DEBUG_NOBEAM")) {       // multi-pass Potts sweep: search the tile order
+        static std::map<std::tuple<int, int, int>, ttn::Plan> cache;
+        static std::mutex mu;
+        std::lock_guard<std::mutex> lock(mu);
+        const auto key = std::make_tuple(L, tc.Tmax, tc.ride);
+        auto it = cache.find(key);
+        if (it == cache.end()) it = cache.emplace(key, ttn::make_plan_beam(q, L, tc.Tmax, tc.ride)).first;
+        if (!it->second.passes.empty() && it->second.passes.size() < p.passes.size()) p = it->second;
+    }
     if (q == 3) {
         int max_nb = count ? ttn::POTTS_MAX_NB_COUNT : 3;
         if (const char* e = getenv("TTN_DEBUG_NB")) { int v = atoi(e); if (v >= 1 && v <= max_nb) max_nb = v; }
@@ -197,6 +209,7 @@ static ttn_status launch_pass(const ttn_plan* P, const ttn::Pass& ps, cudaStream
     if constexpr (Q == 3) {    // Potts: register-blocked gates (ttn_potts.cuh)
         // persistent CTAs, two residents per SM (ttn_potts.cuh)
         if (pp.n_ops > ttn::POTTS_MAX_OPS) return fail(TTN_EUNSUPPORTED, "too many gates in one Potts pass");
+        if (pp.T > 9) return fail(TTN_EUNSUPPORTED, "Potts tiles hold at most 3^9 elements");
         static int sms = 0;
         if (!sms) { int dev = 0; TTN_CUDA(cudaGetDevice(&dev)); TTN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)); }
         const unsigned ctas = grid < 2ull * sms ? (unsigned)grid : 2u * (unsigned)sms;

@@ -151,6 +151,7 @@ __global__ void __launch_bounds__(THREADS, 2) potts_pass_kernel(const PassParams
     __shared__ int s_dig[GMAX_L + 1];        // digits of the tile's base index; slot GMAX_L = 0 ("no such column")
     __shared__ float s_fin[GMAX_L];          // K_c of A_{L-1} (REDUCE pass)
     __shared__ float s_aout;                 // part of A_{L-1} that only involves columns outside the tile
+    __shared__ float s_tabA[81], s_tabB[243]; // A_{L-1} over the low 4 / the other <= 5 tile digits (T <= 9)
     __shared__ uint4 s_aux[POTTS_MAX_OPS];   // per gate (block leaders are the ones used)
     __shared__ float4 s_gk[POTTS_MAX_OPS];   // gate constants of the current instance
     __shared__ unsigned char s_list[POTTS_MAX_OPS];   // op index of every block leader
@@ -240,19 +241,39 @@ __global__ void __launch_bounds__(THREADS, 2) potts_pass_kernel(const PassParams
                 s_aout = acc;
             }
             __syncthreads();
-            float mx = -INFINITY;
-            for (unsigned e = threadIdx.x; e < N; e += THREADS) {
-                float acc = s_aout;
-                unsigned rest = e;
+            // A_{L-1}(s) restricted to the tile = table over the low (<= 4) tile digits + table over
+            // the other (<= 5) digits + the one bond between the two groups
+            const int GA = p.T < 4 ? p.T : 4;
+            unsigned NA = 1;
+            for (int i = 0; i < GA; ++i) NA *= Q;
+            const unsigned NBH = N / NA, m_na = fastdiv_magic(NA);
+            auto terms = [&](unsigned idx, int pos0, int pos1) {
+                float acc = 0.f;
+                unsigned rest = idx;
                 int dprev = 0, cprev = -2;
-                for (int pos = 0; pos < p.T; ++pos) {
+                for (int pos = pos0; pos < pos1; ++pos) {
                     const int d = (int)(rest % Q); rest /= Q;
                     const int c = tile_col(p, pos);
-                    if (c > 0) acc += diag2<Q>(K[c - 1], cprev == c - 1 ? dprev : s_dig[c - 1], d);
+                    if (c > 0) {
+                        if (cprev == c - 1) acc += diag2<Q>(K[c - 1], dprev, d);                 // left neighbour in this group
+                        else if (!(pos > 0 && tile_col(p, pos - 1) == c - 1)) acc += diag2<Q>(K[c - 1], s_dig[c - 1], d);   // outside the tile
+                    }                                                                            // else: the bond between the groups
                     const bool right_in = pos + 1 < p.T && tile_col(p, pos + 1) == c + 1;
                     if (c + 1 < p.L && !right_in) acc += diag2<Q>(K[c], d, s_dig[c + 1]);
                     dprev = d; cprev = c;
                 }
+                return acc;
+            };
+            for (unsigned i = threadIdx.x; i < NA; i += THREADS) s_tabA[i] = terms(i, 0, GA);
+            for (unsigned i = threadIdx.x; i < NBH; i += THREADS) s_tabB[i] = terms(i, GA, p.T);
+            const bool has_x = GA < p.T && tile_col(p, GA) == tile_col(p, GA - 1) + 1;
+            const float Kx = has_x ? K[tile_col(p, GA - 1)] : 0.f;
+            __syncthreads();
+            float mx = -INFINITY;
+            for (unsigned e = threadIdx.x; e < N; e += THREADS) {
+                const unsigned hi = NA == N ? 0u : fastdiv(e, m_na), lo = e - hi * NA;
+                float acc = s_aout + s_tabA[lo] + s_tabB[hi];
+                if (lo / (NA / Q) == hi % Q) acc += Kx;
                 const float val = sx[e] + acc;
                 sx[e] = val;
                 mx = fmaxf(mx, val);

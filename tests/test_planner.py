@@ -128,6 +128,11 @@ def test_fusion_cuts_hbm_passes():
     assert len(passes) <= 12
     head, fpasses = parse_fused(describe(2, 32, 0, fused=True))
     assert len(fpasses) <= 24
+    # q = 3: beam search over tile sequences (planner.h make_plan_beam) vs the cyclic tile order
+    _, passes = parse(describe(3, 18, 1))
+    assert len(passes) <= 12
+    _, passes = parse(describe(3, 18, 0))
+    assert len(passes) <= 8
 
 
 # ------------------------------------------------------------------ fused register-phase schedule
