@@ -447,3 +447,48 @@ def test_next2_ground_config_24x24():
     for b, seed in enumerate((4000, 4001)):
         assert E0[b] == gold[("ising_energy", 24, seed)][0]
         assert oracle.ising_energy(24, Jh[b], Jv[b], None, sig[b]) == E0[b]
+
+
+# ------------------------------------------------------------------ maximum sizes of the other calls
+def test_ground_config_28x28_planted():
+    """ttn_ground_config at its size limit (28 checkpoints of 1 GiB).  Planted instance = gauge-
+    transformed ferromagnet J_ij = eps_i eps_j: E0 = -2L(L-1) and the ground state
+    is unique up to the global flip, so the returned configuration must be +-eps itself."""
+    import torch
+    L = 28
+    free, _ = torch.cuda.mem_get_info()
+    if free < 36 * 2 ** 30:
+        pytest.skip("needs 36 GiB of free device memory")
+    rng = np.random.default_rng(28)
+    eps = rng.choice([-1.0, 1.0], size=(L, L)).astype(np.float32)
+    Jh, Jv = (eps[:, :-1] * eps[:, 1:])[None], (eps[:-1, :] * eps[1:, :])[None]
+    E0, sig = ttn.ground_config(Jh, Jv)
+    assert E0[0] == -2 * L * (L - 1)
+    s = sig[0].astype(np.float32)
+    assert np.array_equal(s, eps) or np.array_equal(s, -eps)
+    assert oracle.ising_energy(L, Jh[0], Jv[0], None, sig[0]) == E0[0]
+    torch.cuda.empty_cache()
+
+
+def test_potts_20x20_planted_count():
+    """Potts at its size limit (3^20 = 3.49e9 states: element offsets just below 2^32; 41.8 GB of
+    (x, n)).  Planted instance: draw a colouring t*, set J_ij = +1 where t*_i = t*_j and -1
+    elsewhere; E = -sum J delta >= -#(J = +1) with equality at t*, so E0 = -#(J = +1) exactly.  The
+    degeneracy is a multiple of 3 (cyclic colour shift) and at least 6 here (every
+    colour permutation of t* is a ground state and t* uses all three colours)."""
+    import torch
+    L = 20
+    free, _ = torch.cuda.mem_get_info()
+    if free < 50 * 2 ** 30:
+        pytest.skip("needs 50 GiB of free device memory")
+    rng = np.random.default_rng(2020)
+    t = rng.integers(0, 3, size=(L, L))
+    Jh = np.where(t[:, :-1] == t[:, 1:], 1.0, -1.0).astype(np.float32)[None]
+    Jv = np.where(t[:-1, :] == t[1:, :], 1.0, -1.0).astype(np.float32)[None]
+    n_plus = int((Jh > 0).sum() + (Jv > 0).sum())
+    E0, g = ttn.potts3_sweep_count(Jh, Jv)
+    assert E0[0] == -n_plus
+    assert g[0] >= 6 and g[0] < 2 ** 53 and int(g[0]) % 3 == 0
+    E1 = ttn.potts3_sweep_energy(Jh, Jv)
+    assert E1[0] == E0[0]
+    torch.cuda.empty_cache()
