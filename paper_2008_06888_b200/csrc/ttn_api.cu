@@ -286,7 +286,31 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
         if (grid > need) grid = need;
     }
     pp.part_stride = pp.cta_per_inst ? 1 : (int)grid;
-    if (P->i16) {
+    pp.igroup = 1;
+    if (pp.cta_per_inst && !P->i16 && !(ps.flags & ttn::PASS_REDUCE) && !getenv("TTN_DEBUG_NOGROUP")) {
+        // instances per CTA at a time: fewest rounds of the 12 warps (HIGH: of the 3 warp groups) over
+        // the flat tile list of K instances, times the rounds of CTA groups over the grid
+        const unsigned long long tpi = pp.tiles_per_inst, slots = ps.low ? (unsigned long long)nw : (unsigned long long)(nw / 4);
+        const unsigned long long unit = ps.low ? 1 : 4;
+        double best = 0; int bestK = 1;
+        for (int K = 1; K <= 8; ++K) {
+            if ((size_t)K * (pp.n_gates * 2 + 2) > (size_t)(ttn::FMAX_GATES + 1) * 2) break;
+            const unsigned long long groups = ((unsigned long long)P->batch + K - 1) / K;
+            const unsigned long long waves = (groups + P->fused_grid - 1) / P->fused_grid;
+            const unsigned long long rounds = ((K * tpi + unit - 1) / unit + slots - 1) / slots;
+            const double cost = (double)(waves * rounds);
+            if (K == 1 || cost < best) { best = cost; bestK = K; }
+        }
+        pp.igroup = bestK;
+        int sh = 0; while ((1ull << sh) < tpi) ++sh;
+        pp.tpi_shift = sh;
+    }
+    if (pp.igroup > 1) {
+        const unsigned long long groups = ((unsigned long long)P->batch + pp.igroup - 1) / pp.igroup;
+        grid = groups < (unsigned long long)P->fused_grid ? groups : (unsigned long long)P->fused_grid;
+        if (ps.low) ttn::fused_pass_kernel<true, 0, true><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(true), st>>>(pp);
+        else ttn::fused_pass_kernel<false, 0, true><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(false), st>>>(pp);
+    } else if (P->i16) {
         if (ps.low) ttn::fused_pass_kernel<true, 1><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(true), st>>>(pp);
         else ttn::fused_pass_kernel<false, 1><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(false), st>>>(pp);
     } else {
@@ -417,6 +441,8 @@ static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
     TTN_CUDA(cudaGetLastError());
     TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
     TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));
     int dev = 0, sms = 0, per_sm = 0, per_sm2 = 0;
     TTN_CUDA(cudaGetDevice(&dev));
     TTN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));

@@ -67,6 +67,9 @@ struct FusedParams {
                                         // tile is fetched into it asynchronously (cp.async) while the rest
                                         // of this tile's gates run
     int cta_per_inst;                   // 1: few tiles per instance -- every CTA sweeps whole instances
+    int igroup, tpi_shift;              // GROUP kernels: instances a CTA takes at a time (their tiles form one
+                                        // flat list, so 16 tiles on 12 warps do not cost two full rounds each);
+                                        // log2(tiles_per_inst)
                                         // (blockIdx.x, + gridDim.x, ...) with its own warps only
     int part_stride;                    // partials per instance: gridDim.x, or 1 when cta_per_inst
     int L_cols;                         // Tropical<i16> only: lattice L (p.L = L - 1 word digits)
@@ -426,7 +429,9 @@ __device__ __forceinline__ void group_sync(int warp) {
 
 // ELEM = 0: Tropical<f32>.  ELEM = 1: Tropical<i16>, two elements per word; then p.L, p.a and the
 // tile geometry count WORD digits (column c >= 1 = word digit c - 1) and p.L_cols = lattice L.
-template <bool LOW, int ELEM = 0>
+// GROUP (cta_per_inst passes without a reduction, f32): a CTA stages the constants of p.igroup
+// instances and walks their tiles as one list.
+template <bool LOW, int ELEM = 0, bool GROUP = false>
 __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const FusedParams p) {
     constexpr int FWARPS = fwarps(LOW);
     extern __shared__ __align__(16) unsigned char fsm_raw[];
@@ -440,23 +445,32 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
     const unsigned long long gw = p.cta_per_inst ? (unsigned long long)warp : (unsigned long long)blockIdx.x * FWARPS + warp;
     const unsigned long long nw = p.cta_per_inst ? (unsigned long long)FWARPS : (unsigned long long)gridDim.x * FWARPS;
 
-    for (int inst = p.cta_per_inst ? (int)blockIdx.x : 0; inst < p.batch; inst += p.cta_per_inst ? (int)gridDim.x : 1) {
+    const int igroup = GROUP ? p.igroup : 1;
+    const int gk_stride = p.n_gates * 2 + 2;            // float4 per instance in s_gk (GROUP)
+    for (int inst = p.cta_per_inst ? (int)blockIdx.x * igroup : 0; inst < p.batch;
+         inst += p.cta_per_inst ? (int)gridDim.x * igroup : 1) {
+        const int ng = GROUP ? (p.batch - inst < igroup ? p.batch - inst : igroup) : 1;
+        const unsigned long long ntiles = GROUP ? (unsigned long long)ng << p.tpi_shift : p.tiles_per_inst;
         // ---- stage this instance's program and gate constants (S0 outputs) into shared memory
         __syncthreads();
         for (int i = tid; i < p.n_mops; i += blockDim.x) {
             const MicroOp mo = p.mops[i];
             s_mops[i] = (unsigned)mo.code | ((unsigned)mo.mask << 8) | ((unsigned)mo.arg << 16);
         }
-        {
-            const float4* src = reinterpret_cast<const float4*>(p.gate_k + (size_t)inst * p.gate_inst_stride);
-            for (int i = tid; i < p.n_gates * 2; i += blockDim.x) s_gk[i] = src[i];
-            if (tid < 2) s_gk[p.n_gates * 2 + tid] = make_float4(0.f, 0.f, 0.f, 0.f);   // prefetch runs one ahead
+        for (int j = 0; j < ng; ++j) {
+            const float4* src = reinterpret_cast<const float4*>(p.gate_k + (size_t)(inst + j) * p.gate_inst_stride);
+            float4* dst = s_gk + j * gk_stride;
+            for (int i = tid; i < p.n_gates * 2; i += blockDim.x) dst[i] = src[i];
+            if (tid < 2) dst[p.n_gates * 2 + tid] = make_float4(0.f, 0.f, 0.f, 0.f);   // prefetch runs one ahead
         }
         if (p.flags & PASS_REDUCE)
             for (int i = tid; i < FFINAL_FLOATS; i += blockDim.x) s_fin[i] = p.final_tab[(size_t)inst * FFINAL_FLOATS + i];
         __syncthreads();
-        float* S = p.state + (unsigned long long)inst * p.inst_stride;
-        float* SRC = const_cast<float*>(p.src) + (unsigned long long)inst * p.src_stride;
+        float* S0 = p.state + (unsigned long long)inst * p.inst_stride;
+        float* SRC0 = const_cast<float*>(p.src) + (unsigned long long)inst * p.src_stride;
+        // flat tile number -> instance of the group and tile of that instance
+        auto il_of = [&](unsigned long long ft) -> unsigned long long { return GROUP ? ft >> p.tpi_shift : 0ull; };
+        auto wt_of = [&](unsigned long long ft) -> unsigned long long { return GROUP ? ft & (p.tiles_per_inst - 1) : ft; };
         float wmax = -INFINITY;
 
         // HIGH: the 4 warps of a group (one per scheduler) take 4 consecutive tiles -- the 4 sectors
@@ -474,12 +488,16 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
         const bool async_load = !LOW && !(p.flags & PASS_INIT) && p.prefetch_pc >= 0;
         if (async_load) {                               // the first tile of this warp
             group_sync(warp);
-            if (tile_of(0) < p.tiles_per_inst) pf_issue(myreg, SRC + high_base(tile_of(0)), lane, p.stride_bytes, p.a);
+            const unsigned long long f0 = tile_of(0);
+            if (f0 < ntiles) pf_issue(myreg, SRC0 + il_of(f0) * p.src_stride + high_base(wt_of(f0)), lane, p.stride_bytes, p.a);
         }
         for (unsigned long long it = 0;; ++it) {
-            const unsigned long long wt = tile_of(it);
-            if ((LOW ? wt : (wt & ~3ull)) >= p.tiles_per_inst) break;       // uniform per group
-            if (!LOW && wt >= p.tiles_per_inst) {      // L = 13: fewer than 4 tiles; keep the barrier counts equal
+            const unsigned long long ft = tile_of(it);
+            if ((LOW ? ft : (ft & ~3ull)) >= ntiles) break;                 // uniform per group
+            const unsigned long long wt = wt_of(ft);
+            float* S = S0 + il_of(ft) * p.inst_stride;
+            float* SRC = SRC0 + il_of(ft) * p.src_stride;
+            if (!LOW && ft >= ntiles) {                // L = 13: fewer than 4 tiles; keep the barrier counts equal
                 if (!(p.flags & PASS_INIT)) group_sync(warp);      // the load barrier (either flavour)
                 if (!(p.flags & PASS_REDUCE)) group_sync(warp);
                 continue;
@@ -522,13 +540,13 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
             // ---- run the program ------------------------------------------------------------------
             int pc = 0, layout = p.first_layout;
             unsigned op = s_mops[0];
-            const ulonglong2* gk = reinterpret_cast<const ulonglong2*>(s_gk);
+            const ulonglong2* gk = reinterpret_cast<const ulonglong2*>(s_gk + (GROUP ? (int)il_of(ft) * gk_stride : 0));
             ulonglong2 n0 = gk[0], n1 = gk[1];
             for (;;) {
                 if (async_load && pc == p.prefetch_pc) {    // the region is free from here on: fetch the next tile
-                    const unsigned long long wn = tile_of(it + 1);
+                    const unsigned long long fn = tile_of(it + 1);
                     group_sync(warp);                       // the group's 4 sectors of every line are requested together
-                    if (wn < p.tiles_per_inst) pf_issue(myreg, SRC + high_base(wn), lane, p.stride_bytes, p.a);
+                    if (fn < ntiles) pf_issue(myreg, SRC0 + il_of(fn) * p.src_stride + high_base(wt_of(fn)), lane, p.stride_bytes, p.a);
                 }
                 const unsigned code = op & 0xffu;
                 if (code == MC_END || code == MC_FINAL) break;
