@@ -160,6 +160,41 @@ def run_reference(args):
     }))
 
 
+def other_configs(torch):
+    """cfg 2, 3, 5 of BASELINE.json through the plan API; bytes_min as in
+    BASELINE.md section 2 (north_star roofline: (L-1) * 2 * B_e * q^L per instance)."""
+    import paper_2008_06888_b200 as ttn
+    from ttn_inputs import CONFIGS, config_batch
+    peak, _ = measured_peaks()
+    rows = {}
+    for name, cfg, q, call, be in (("cfg2_16x16_gauss_ground_config_batch256", 2, 2, ttn.CALL_CONFIG, 4),
+                                   ("cfg3_24x24_pmj_count_batch16", 3, 2, ttn.CALL_COUNT, 12),
+                                   ("cfg5_potts_18x18_pmj_count_batch4", 5, 3, ttn.CALL_COUNT, 12)):
+        try:
+            Jh, Jv, h = config_batch(cfg)
+            plan = ttn.Plan(q, call, Jh, Jv, h)
+            plan.launch()
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for _ in range(3):
+                plan.launch()
+            b.record()
+            torch.cuda.synchronize()
+            ms = a.elapsed_time(b) / 3
+            B, Lc = Jh.shape[0], CONFIGS[cfg]["L"]
+            bmin = B * (Lc - 1) * 2 * be * q ** Lc      # cfg 2: = the checkpoints written once and read back once
+            rows[name] = {"ms_total": ms, "ms_per_instance": ms / B, "batch": B, "hbm_passes": plan.num_passes,
+                          "launches": plan.num_launches,
+                          "hbm_roofline_frac": bmin / (peak * 1e9) / (ms * 1e-3)}
+            plan.close()
+            del plan
+            torch.cuda.empty_cache()
+        except ttn.TTNError as e:
+            rows[name] = {"unavailable": str(e)}
+    return rows
+
+
 def cpu_baseline(L_target: int, L_sample: int):
     import oracle
     Jh, Jv, _ = make_batch(L_sample, [4000], "pmj")
@@ -183,6 +218,7 @@ def main():
     ap.add_argument("--ref-L", type=int, default=22, dest="ref_L")
     ap.add_argument("--cpu-L", type=int, default=24, dest="cpu_L")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", dest="no_other_configs")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                   # timing rule: W >= 3
@@ -267,6 +303,12 @@ def main():
     except ttn.TTNError as e:      # e.g. L below the i16 path's limits
         i16 = {"unavailable": str(e)}
 
+    # ---- the other BASELINE.json configs, timed beside the headline (rank 0, one GPU; they are parity
+    # cases, not the metric: device time of ttn_plan_launch, couplings resident, mean of 3 launches)
+    others = None
+    if rank == 0 and world == 1 and L == 32 and not args.no_other_configs:
+        others = other_configs(torch)
+
     if rank == 0:
         peak, peak_src = measured_peaks()
         per_inst_ms = whole_job_ms_per_instance(ms_per_step, world)
@@ -302,6 +344,8 @@ def main():
                              "note": "1 FMNMX per update on the 64-lane/clk/SM alu pipe at the sampled SM clock"},
             "step_ms": step_ms, "clocks": clocks, "tropical_i16": i16,
         }
+        if others is not None:
+            out["other_configs"] = others
         if not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(L, args.cpu_L)
         print(json.dumps(out))
