@@ -75,7 +75,7 @@ bool limits_ok(int q, int L, bool count, bool config) {
 struct Layout {
     size_t x = 0, n = 0, ckpt = 0, Jh = 0, Jv = 0, h = 0, ops = 0, part_x = 0, part_n = 0,
            amax_v = 0, amax_s = 0, out_x = 0, out_n = 0, out_s = 0, sigma = 0, total = 0;
-    size_t f_mops = 0, f_gate_rc = 0, f_gate_k = 0, f_final = 0, g_gate_k = 0, g_fin = 0;
+    size_t f_mops = 0, f_gate_rc = 0, f_gate_k = 0, f_final = 0, g_gate_k = 0, g_fin = 0, f_sweep = 0;
     unsigned long long NS = 0, max_tiles = 0;
     int amax_blocks = 0;
     int f_max_gates = 0, f_max_mops = 0;
@@ -129,6 +129,7 @@ Layout make_layout(int q, int L, bool count, bool config, int batch, bool i16 = 
         y.f_gate_rc = take((size_t)y.f_max_gates * 4);
         y.f_gate_k = take((size_t)batch * y.f_max_gates * 8 * 4);
         y.f_final = take((size_t)batch * ttn::FFINAL_FLOATS * 4);
+        y.f_sweep = take((size_t)(4 * L + 8) * sizeof(ttn::FusedParams));     // fused_sweep_kernel: one entry per pass
     }
     y.total = off;
     return y;
@@ -150,6 +151,8 @@ struct ttn_plan {
     ttn::FusedPlan fplan;
     bool fused = false, i16 = false;
     int fused_grid = 0;
+    int sweep_grid = 0;             // > 0: fused_sweep_kernel runs every pass in one launch (table at lay.f_sweep)
+    std::vector<ttn::FusedParams> sweep_params;
     Layout lay;
     unsigned char* ws;
     std::vector<double> defer;     // per instance: sum of the +J constants factored out of the gates
@@ -241,7 +244,9 @@ static ttn_status launch_pass(const ttn_plan* P, const ttn::Pass& ps, cudaStream
     return TTN_OK;
 }
 
-static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps, cudaStream_t st) {
+// out_pp != NULL: only fill the parameters (force_group instances per CTA at a time) and the grid.
+static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps, cudaStream_t st,
+                                    ttn::FusedParams* out_pp = nullptr, int force_group = 0, unsigned* out_grid = nullptr) {
     const Layout& y = P->lay;
     const ttn::FusedPlan& fp = P->fplan;
     ttn::FusedParams pp{};
@@ -287,6 +292,7 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
     }
     pp.part_stride = pp.cta_per_inst ? 1 : (int)grid;
     pp.igroup = 1;
+    { int sh = 0; while ((1ull << sh) < pp.tiles_per_inst) ++sh; pp.tpi_shift = sh; }
     if (pp.cta_per_inst && !P->i16 && !(ps.flags & ttn::PASS_REDUCE) && !getenv("TTN_DEBUG_NOGROUP")) {
         // instances per CTA at a time: fewest rounds of the 12 warps (HIGH: of the 3 warp groups) over
         // the flat tile list of K instances, times the rounds of CTA groups over the grid
@@ -301,9 +307,15 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
             const double cost = (double)(waves * rounds);
             if (K == 1 || cost < best) { best = cost; bestK = K; }
         }
-        pp.igroup = bestK;
-        int sh = 0; while ((1ull << sh) < tpi) ++sh;
-        pp.tpi_shift = sh;
+        pp.igroup = force_group > 0 ? force_group : bestK;
+    }
+    if (out_pp) {
+        if (!pp.cta_per_inst || (ps.flags & ttn::PASS_REDUCE) || P->i16) return fail(TTN_EUNSUPPORTED, "pass not eligible for the one-launch sweep");
+        if ((size_t)pp.igroup * (pp.n_gates * 2 + 2) > (size_t)(ttn::FMAX_GATES + 1) * 2) return fail(TTN_EUNSUPPORTED, "instance group too large");
+        const unsigned long long groups = ((unsigned long long)P->batch + pp.igroup - 1) / pp.igroup;
+        if (out_grid) *out_grid = (unsigned)(groups < (unsigned long long)P->fused_grid ? groups : (unsigned long long)P->fused_grid);
+        *out_pp = pp;
+        return TTN_OK;
     }
     if (pp.igroup > 1) {
         const unsigned long long groups = ((unsigned long long)P->batch + pp.igroup - 1) / pp.igroup;
@@ -441,6 +453,7 @@ static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
     TTN_CUDA(cudaGetLastError());
     TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
     TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_sweep_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
     TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
     TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));
     int dev = 0, sms = 0, per_sm = 0, per_sm2 = 0;
@@ -620,6 +633,25 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
         ttn_status fs = count ? setup_fcount(P, st) : setup_fused(P, st);
         if (fs != TTN_OK) { delete P; return fs; }
         P->launches = (int)P->fplan.passes.size() + (config ? (backtrace_one_cta(L, batch) ? 1 : 2 * L) : 1);
+        if (config && !count && !P->i16 && !getenv("TTN_DEBUG_NOSWEEP") && P->fplan.passes.size() <= (size_t)(4 * L + 8)) {
+            // every pass in cta_per_inst mode: the pass table of fused_sweep_kernel (two instances per
+            // CTA at a time where the constants of every pass fit, else one)
+            std::vector<ttn::FusedParams> v(P->fplan.passes.size());
+            unsigned grid = 0;
+            bool ok = false;
+            for (int K = 2; K >= 1 && !ok; --K) {
+                ok = true;
+                for (size_t i = 0; i < v.size() && ok; ++i)
+                    ok = launch_fused_pass(P, P->fplan.passes[i], st, &v[i], K, &grid) == TTN_OK;
+            }
+            if (ok) {
+                P->sweep_params = v; P->sweep_grid = (int)grid;
+                cudaError_t ce = cudaMemcpyAsync(P->ws + lay.f_sweep, P->sweep_params.data(), v.size() * sizeof(ttn::FusedParams),
+                                                 cudaMemcpyHostToDevice, st);
+                if (ce != cudaSuccess) { delete P; return fail(TTN_ECUDA, "pass table upload failed: %s", cudaGetErrorString(ce)); }
+                P->launches = 1 + (backtrace_one_cta(L, batch) ? 1 : 2 * L);
+            }
+        }
     } else {
         ttn::GenericPrepParams gp{};
         gp.q = q; gp.L = L; gp.n_ops = (int)P->plan.ops.size();
@@ -646,6 +678,13 @@ ttn_status ttn_plan_launch(ttn_plan* P, void* stream) {
         const bool timing = getenv("TTN_DEBUG_TIMING") != nullptr;     // per-pass device times on stderr
         std::vector<cudaEvent_t> ev;
         if (timing) { ev.resize(P->fplan.passes.size() + 1); for (auto& e : ev) cudaEventCreate(&e); cudaEventRecord(ev[0], st); }
+        // batches of small lattices, no reduction pass (ttn_ground_config): all passes in one launch
+        if (P->sweep_grid > 0 && !timing) {
+            ttn::fused_sweep_kernel<0><<<(unsigned)P->sweep_grid, ttn::fwarps(true) * 32, ttn::fsmem_bytes(true), st>>>(
+                reinterpret_cast<const ttn::FusedParams*>(P->ws + P->lay.f_sweep), (int)P->sweep_params.size());
+            TTN_CUDA(cudaGetLastError());
+            return launch_backtrace(P, st);
+        }
         size_t k = 0;
         for (const ttn::FusedPass& ps : P->fplan.passes) {
             ttn_status s = P->count ? launch_fcount_pass(P, ps, st) : launch_fused_pass(P, ps, st);

@@ -431,10 +431,11 @@ __device__ __forceinline__ void group_sync(int warp) {
 // tile geometry count WORD digits (column c >= 1 = word digit c - 1) and p.L_cols = lattice L.
 // GROUP (cta_per_inst passes without a reduction, f32): a CTA stages the constants of p.igroup
 // instances and walks their tiles as one list.
-template <bool LOW, int ELEM = 0, bool GROUP = false>
-__global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const FusedParams p) {
+// The pass itself: `inst_first`, `inst_step` = the instances (GROUP: instance groups) this CTA takes.
+template <bool LOW, int ELEM, bool GROUP>
+__device__ __forceinline__ void fused_pass_body(const FusedParams& p, unsigned char* fsm_raw,
+                                                const int inst_first, const int inst_step) {
     constexpr int FWARPS = fwarps(LOW);
-    extern __shared__ __align__(16) unsigned char fsm_raw[];
     float4* regions = reinterpret_cast<float4*>(fsm_raw);                              // FWARPS * FREGION_F4
     float4* s_gk = reinterpret_cast<float4*>(fsm_raw + (size_t)FWARPS * FREGION_F4 * 16);   // (FMAX_GATES + 1) * 2
     float* s_fin = reinterpret_cast<float*>(s_gk + (FMAX_GATES + 1) * 2);               // FFINAL_FLOATS
@@ -447,8 +448,7 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
 
     const int igroup = GROUP ? p.igroup : 1;
     const int gk_stride = p.n_gates * 2 + 2;            // float4 per instance in s_gk (GROUP)
-    for (int inst = p.cta_per_inst ? (int)blockIdx.x * igroup : 0; inst < p.batch;
-         inst += p.cta_per_inst ? (int)gridDim.x * igroup : 1) {
+    for (int inst = inst_first; inst < p.batch; inst += inst_step) {
         const int ng = GROUP ? (p.batch - inst < igroup ? p.batch - inst : igroup) : 1;
         const unsigned long long ntiles = GROUP ? (unsigned long long)ng << p.tpi_shift : p.tiles_per_inst;
         // ---- stage this instance's program and gate constants (S0 outputs) into shared memory
@@ -620,6 +620,38 @@ __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const F
                 for (int w = 1; w < FWARPS; ++w) m = fmaxf(m, s_red[w]);
                 p.part_x[(size_t)inst * p.part_stride + (p.cta_per_inst ? 0 : blockIdx.x)] = m;
             }
+        }
+    }
+}
+
+template <bool LOW, int ELEM = 0, bool GROUP = false>
+__global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const FusedParams p) {
+    extern __shared__ __align__(16) unsigned char fsm_raw[];
+    const int igroup = GROUP ? p.igroup : 1;
+    fused_pass_body<LOW, ELEM, GROUP>(p, fsm_raw, p.cta_per_inst ? (int)blockIdx.x * igroup : 0,
+                                      p.cta_per_inst ? (int)gridDim.x * igroup : 1);
+}
+
+// Batches of small lattices (every pass in cta_per_inst mode, no reduction pass -- the row-aligned
+// plans of ttn_ground_config): the instances are independent, so ONE launch runs all passes; a
+// CTA takes p.igroup instances through the whole list of passes (block barrier between passes:
+// the tiles of a pass are written by other warps of the same CTA) before it moves to its next
+// instances.  Saves the launch gap and the ramp / tail of ~30 short kernels.
+template <int ELEM = 0>
+__global__ void __launch_bounds__(fwarps(true) * 32, 1) fused_sweep_kernel(const FusedParams* __restrict__ passes,
+                                                                            const int n_passes) {
+    static_assert(fwarps(true) == fwarps(false), "one CTA shape for both tile kinds");
+    extern __shared__ __align__(16) unsigned char fsm_raw[];
+    __shared__ FusedParams s_p;
+    const int igroup = passes[0].igroup, batch = passes[0].batch;
+    for (int inst = (int)blockIdx.x * igroup; inst < batch; inst += (int)gridDim.x * igroup) {
+        for (int k = 0; k < n_passes; ++k) {
+            __syncthreads();                                   // the previous pass is complete (and s_p free)
+            for (int i = threadIdx.x; i < (int)(sizeof(FusedParams) / 4); i += blockDim.x)
+                reinterpret_cast<unsigned*>(&s_p)[i] = reinterpret_cast<const unsigned*>(passes + k)[i];
+            __syncthreads();
+            if (s_p.low) fused_pass_body<true, ELEM, true>(s_p, fsm_raw, inst, 1 << 30);
+            else fused_pass_body<false, ELEM, true>(s_p, fsm_raw, inst, 1 << 30);
         }
     }
 }

@@ -365,7 +365,9 @@ def test_h_none_equals_zero_field_and_batch_independence():
 def test_plan_split_api_relaunch():
     Jh, Jv, h = make_batch(12, range(10, 14), "gauss", fields=True)
     p = ttn.Plan(2, ttn.CALL_CONFIG, Jh, Jv, h)
-    assert p.num_launches >= p.num_passes + 2 * 12
+    # forward: one launch per pass, or ONE launch for all passes (batches of small lattices);
+    # backward: a launch pair per row (batch < 32)
+    assert p.num_passes >= 12 and p.num_launches in (p.num_passes + 2 * 12, 1 + 2 * 12)
     p.launch(); E_a, _, s_a = p.read()
     p.launch(); E_b, _, s_b = p.read()
     assert np.array_equal(E_a, E_b) and np.array_equal(s_a, s_b)
