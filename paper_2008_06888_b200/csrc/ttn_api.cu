@@ -291,6 +291,7 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
         if (grid > need) grid = need;
     }
     pp.part_stride = pp.cta_per_inst ? 1 : (int)grid;
+    if (ps.low && getenv("TTN_DEBUG_NOLOWPF")) pp.prefetch_pc = -1;
     pp.igroup = 1;
     { int sh = 0; while ((1ull << sh) < pp.tiles_per_inst) ++sh; pp.tpi_shift = sh; }
     if (pp.cta_per_inst && !P->i16 && !(ps.flags & ttn::PASS_REDUCE) && !getenv("TTN_DEBUG_NOGROUP")) {

@@ -422,6 +422,22 @@ __device__ __forceinline__ void pf_read(float (&v)[128], const float4* region, i
     }
 }
 
+// LOW tiles: the same for a contiguous 16 KiB tile (no barrier: a low tile is whole lines anyway);
+// the region holds the tile linearly, read back in layout B (lanes = the 5 lowest digits).
+__device__ __forceinline__ void pf_issue_low(float4* region, const float* tile, int lane) {
+    const unsigned sbase = (unsigned)__cvta_generic_to_shared(region) + 16u * (unsigned)lane;
+    const unsigned long long g = (unsigned long long)__cvta_generic_to_global(tile + 4 * lane);
+#pragma unroll
+    for (int i = 0; i < 32; ++i)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(sbase + 512u * i), "l"(g + 512ull * i) : "memory");
+    asm volatile("cp.async.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void pf_read_low(float (&v)[128], const float4* region, int lane) {
+    const float* q = reinterpret_cast<const float*>(region) + lane;
+#pragma unroll
+    for (int j = 0; j < 128; ++j) v[j] = q[32 * ereg_low_b(j)];
+}
+
 // named barrier of one 4-warp group (barrier 0 is __syncthreads)
 __device__ __forceinline__ void group_sync(int warp) {
     asm volatile("bar.sync %0, 128;" :: "r"(1 + (warp >> 2)) : "memory");
@@ -431,205 +447,19 @@ __device__ __forceinline__ void group_sync(int warp) {
 // tile geometry count WORD digits (column c >= 1 = word digit c - 1) and p.L_cols = lattice L.
 // GROUP (cta_per_inst passes without a reduction, f32): a CTA stages the constants of p.igroup
 // instances and walks their tiles as one list.
-// The pass itself: `inst_first`, `inst_step` = the instances (GROUP: instance groups) this CTA takes.
+// One fused pass.  The body lives in ttn_fused_body.inc (see there).
 template <bool LOW, int ELEM, bool GROUP>
 __device__ __forceinline__ void fused_pass_body(const FusedParams& p, unsigned char* fsm_raw,
                                                 const int inst_first, const int inst_step) {
-    constexpr int FWARPS = fwarps(LOW);
-    float4* regions = reinterpret_cast<float4*>(fsm_raw);                              // FWARPS * FREGION_F4
-    float4* s_gk = reinterpret_cast<float4*>(fsm_raw + (size_t)FWARPS * FREGION_F4 * 16);   // (FMAX_GATES + 1) * 2
-    float* s_fin = reinterpret_cast<float*>(s_gk + (FMAX_GATES + 1) * 2);               // FFINAL_FLOATS
-    unsigned* s_mops = reinterpret_cast<unsigned*>(s_fin + FFINAL_FLOATS);              // FMAX_MOPS
-    float* s_red = reinterpret_cast<float*>(s_mops + FMAX_MOPS);                        // FWARPS (<= 16)
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    float4* myreg = regions + warp * FREGION_F4;
-    const unsigned long long gw = p.cta_per_inst ? (unsigned long long)warp : (unsigned long long)blockIdx.x * FWARPS + warp;
-    const unsigned long long nw = p.cta_per_inst ? (unsigned long long)FWARPS : (unsigned long long)gridDim.x * FWARPS;
-
-    const int igroup = GROUP ? p.igroup : 1;
-    const int gk_stride = p.n_gates * 2 + 2;            // float4 per instance in s_gk (GROUP)
-    for (int inst = inst_first; inst < p.batch; inst += inst_step) {
-        const int ng = GROUP ? (p.batch - inst < igroup ? p.batch - inst : igroup) : 1;
-        const unsigned long long ntiles = GROUP ? (unsigned long long)ng << p.tpi_shift : p.tiles_per_inst;
-        // ---- stage this instance's program and gate constants (S0 outputs) into shared memory
-        __syncthreads();
-        for (int i = tid; i < p.n_mops; i += blockDim.x) {
-            const MicroOp mo = p.mops[i];
-            s_mops[i] = (unsigned)mo.code | ((unsigned)mo.mask << 8) | ((unsigned)mo.arg << 16);
-        }
-        for (int j = 0; j < ng; ++j) {
-            const float4* src = reinterpret_cast<const float4*>(p.gate_k + (size_t)(inst + j) * p.gate_inst_stride);
-            float4* dst = s_gk + j * gk_stride;
-            for (int i = tid; i < p.n_gates * 2; i += blockDim.x) dst[i] = src[i];
-            if (tid < 2) dst[p.n_gates * 2 + tid] = make_float4(0.f, 0.f, 0.f, 0.f);   // prefetch runs one ahead
-        }
-        if (p.flags & PASS_REDUCE)
-            for (int i = tid; i < FFINAL_FLOATS; i += blockDim.x) s_fin[i] = p.final_tab[(size_t)inst * FFINAL_FLOATS + i];
-        __syncthreads();
-        float* S0 = p.state + (unsigned long long)inst * p.inst_stride;
-        float* SRC0 = const_cast<float*>(p.src) + (unsigned long long)inst * p.src_stride;
-        // flat tile number -> instance of the group and tile of that instance
-        auto il_of = [&](unsigned long long ft) -> unsigned long long { return GROUP ? ft >> p.tpi_shift : 0ull; };
-        auto wt_of = [&](unsigned long long ft) -> unsigned long long { return GROUP ? ft & (p.tiles_per_inst - 1) : ft; };
-        float wmax = -INFINITY;
-
-        // HIGH: the 4 warps of a group (one per scheduler) take 4 consecutive tiles -- the 4 sectors
-        // of every 128-byte line -- and meet at a named barrier before their loads and before their
-        // stores, so that the lines are requested whole and at the same time (scattered 32-byte
-        // sectors that arrive at different times cost DRAM efficiency); groups drift freely against
-        // each other, which is what overlaps memory phases with gate phases.
-        auto tile_of = [&](unsigned long long it) -> unsigned long long {
-            return LOW ? it * nw + gw : 4ull * (it * (nw >> 2) + (gw >> 2)) + (unsigned long long)(warp & 3);
-        };
-        auto high_base = [&](unsigned long long wt) -> unsigned long long {
-            const int amid = p.a - F_RIDE;
-            return ((wt & ((1ull << amid) - 1)) << F_RIDE) + ((wt >> amid) << (p.a + F_WHIGH));
-        };
-        const bool async_load = !LOW && !(p.flags & PASS_INIT) && p.prefetch_pc >= 0;
-        if (async_load) {                               // the first tile of this warp
-            group_sync(warp);
-            const unsigned long long f0 = tile_of(0);
-            if (f0 < ntiles) pf_issue(myreg, SRC0 + il_of(f0) * p.src_stride + high_base(wt_of(f0)), lane, p.stride_bytes, p.a);
-        }
-        for (unsigned long long it = 0;; ++it) {
-            const unsigned long long ft = tile_of(it);
-            if ((LOW ? ft : (ft & ~3ull)) >= ntiles) break;                 // uniform per group
-            const unsigned long long wt = wt_of(ft);
-            float* S = S0 + il_of(ft) * p.inst_stride;
-            float* SRC = SRC0 + il_of(ft) * p.src_stride;
-            if (!LOW && ft >= ntiles) {                // L = 13: fewer than 4 tiles; keep the barrier counts equal
-                if (!(p.flags & PASS_INIT)) group_sync(warp);      // the load barrier (either flavour)
-                if (!(p.flags & PASS_REDUCE)) group_sync(warp);
-                continue;
-            }
-            // ---- tile geometry: base index, per-thread P / Q neighbour bits per layout ---------------
-            unsigned long long base;
-            int tpA, tqA, tpB, tqB;
-            if (LOW) {
-                base = wt << 12;
-                tpA = 0;                                   // column -1 does not exist
-                tqA = lane & 1;                            // d7 (lane bit 0 in layout A)
-                tpB = (p.L > F_WLOW) ? (int)(wt & 1ull) : 0;                      // column 12
-                tqB = (lane >> 4) & 1;                     // d4 (lane bit 4 in layout B)
-            } else {
-                const int amid = p.a - F_RIDE;
-                const unsigned long long tmid = wt & ((1ull << amid) - 1), ttop = wt >> amid;
-                base = (tmid << F_RIDE) + (ttop << (p.a + F_WHIGH));
-                tpA = (int)((base >> (p.a - 1)) & 1ull);                          // column a-1 (>= 3)
-                tqA = (lane >> 3) & 1;                     // d7
-                tpB = (p.a + F_WHIGH < p.L) ? (int)(ttop & 1ull) : 0;             // column a+9
-                tqB = (lane >> 4) & 1;                     // d1
-            }
-            float v[128];
-            if (p.flags & PASS_INIT) {
-#pragma unroll
-                for (int j = 0; j < 128; ++j) v[j] = 0.f;                         // tropical one
-            } else if (LOW) {
-                gmove<LOW, 1, false>(v, SRC + base, lane, p.stride_bytes, p.a);
-            } else if (!async_load) {
-                group_sync(warp);
-                if (p.first_layout == 1) gmove<LOW, 1, false>(v, SRC + base, lane, p.stride_bytes, p.a);
-                else gmove<LOW, 0, false>(v, SRC + base, lane, p.stride_bytes, p.a);
-            } else {
-                // the tile was fetched into this warp's region while the previous tile was computed
-                asm volatile("cp.async.wait_group 0;" ::: "memory");
-                __syncwarp();
-                if (p.first_layout == 1) pf_read<1>(v, myreg, lane); else pf_read<0>(v, myreg, lane);
-                __syncwarp();
-            }
-            // ---- run the program ------------------------------------------------------------------
-            int pc = 0, layout = p.first_layout;
-            unsigned op = s_mops[0];
-            const ulonglong2* gk = reinterpret_cast<const ulonglong2*>(s_gk + (GROUP ? (int)il_of(ft) * gk_stride : 0));
-            ulonglong2 n0 = gk[0], n1 = gk[1];
-            for (;;) {
-                if (async_load && pc == p.prefetch_pc) {    // the region is free from here on: fetch the next tile
-                    const unsigned long long fn = tile_of(it + 1);
-                    group_sync(warp);                       // the group's 4 sectors of every line are requested together
-                    if (fn < ntiles) pf_issue(myreg, SRC0 + il_of(fn) * p.src_stride + high_base(wt_of(fn)), lane, p.stride_bytes, p.a);
-                }
-                const unsigned code = op & 0xffu;
-                if (code == MC_END || code == MC_FINAL) break;
-                const unsigned nxt = s_mops[pc + 1];
-                if (code == MC_ROUND) {
-                    if (ELEM == 0) fround<LOW>(v, (op >> 8) & 0x7fu, gk, n0, n1, layout ? tpB : tpA, layout ? tqB : tqA);
-                    else fround16<LOW>(v, (op >> 8) & 0xffu, reinterpret_cast<const uint4*>(s_gk) + 2 * (op >> 16), layout,
-                                       layout ? tpB : tpA, layout ? tqB : tqA, lane & 1);
-                } else if (code == MC_XAB) {
-                    __syncwarp(); xmove<LOW, 0, true>(v, myreg, lane); __syncwarp(); xmove<LOW, 1, false>(v, myreg, lane);
-                    layout = 1;
-                } else {
-                    __syncwarp(); xmove<LOW, 1, true>(v, myreg, lane); __syncwarp(); xmove<LOW, 0, false>(v, myreg, lane);
-                    layout = 0;
-                }
-                op = nxt; ++pc;
-            }
-            // ---- store, or add A_{L-1}(s) and reduce ---------------------------------------------
-            if (p.flags & PASS_REDUCE) {
-                // element index with the register digits cleared, first register column, variant
-                unsigned long long sthr; int x0, var;
-                if (LOW) {
-                    if (layout == 0) { sthr = base + ((unsigned long long)lane << 7); x0 = 0; var = tpA + 2 * tqA; }
-                    else { sthr = base + lane; x0 = 5; var = tqB + 2 * tpB; }
-                } else {
-                    if (layout == 0) { sthr = base + (lane & 7) + ((unsigned long long)(lane >> 3) << (p.a + 7)); x0 = p.a; var = tpA + 2 * tqA; }
-                    else { sthr = base + (lane & 7) + ((unsigned long long)(lane >> 3) << p.a); x0 = p.a + 2; var = tqB + 2 * tpB; }
-                }
-                if (ELEM == 0) {
-                    const float cthr = final_thread_const(s_fin, p.L, x0, sthr);
-                    const float4* T = reinterpret_cast<const float4*>(s_fin + var * 128);
-                    float mx = -INFINITY;
-#pragma unroll
-                    for (int q = 0; q < 32; ++q) {
-                        const float4 t = T[q];
-                        mx = fmaxf(mx, fmaxf(fmaxf(v[4 * q] + t.x, v[4 * q + 1] + t.y), fmaxf(v[4 * q + 2] + t.z, v[4 * q + 3] + t.w)));
-                    }
-                    wmax = fmaxf(wmax, mx + cthr);
-                } else {
-                    // per half h: element index = 2 * word index + h, register columns x0+1 .. x0+7; the
-                    // table entries and the thread constants are packed (lo = h 0, hi = h 1), all integers
-                    const int c0 = __float2int_rn(final_thread_const(s_fin, p.L_cols, x0 + 1, sthr << 1));
-                    const int c1 = __float2int_rn(final_thread_const(s_fin, p.L_cols, x0 + 1, (sthr << 1) | 1ull));
-                    const unsigned cpk = ((unsigned)c0 & 0xffffu) | ((unsigned)c1 << 16);
-                    const uint4* T = reinterpret_cast<const uint4*>(s_fin + var * 128);
-                    unsigned m2 = 0x80008000u;                    // (-32768, -32768)
-#pragma unroll
-                    for (int q = 0; q < 32; ++q) {
-                        const uint4 t = T[q];
-                        m2 = __vmaxs2(m2, __vadd2(__float_as_uint(v[4 * q]), t.x));
-                        m2 = __vmaxs2(m2, __vadd2(__float_as_uint(v[4 * q + 1]), t.y));
-                        m2 = __vmaxs2(m2, __vadd2(__float_as_uint(v[4 * q + 2]), t.z));
-                        m2 = __vmaxs2(m2, __vadd2(__float_as_uint(v[4 * q + 3]), t.w));
-                    }
-                    m2 = __vadd2(m2, cpk);
-                    const int lo = (int)(short)(m2 & 0xffffu), hi = (int)(short)(m2 >> 16);
-                    wmax = fmaxf(wmax, (float)(lo > hi ? lo : hi));
-                }
-            } else {
-                if (!LOW) group_sync(warp);
-                if (LOW || p.last_layout == 1) gmove<LOW, 1, true>(v, S + base, lane, p.stride_bytes, p.a);
-                else gmove<LOW, 0, true>(v, S + base, lane, p.stride_bytes, p.a);
-            }
-        }
-        if (p.flags & PASS_REDUCE) {
-            for (int o = 16; o; o >>= 1) wmax = fmaxf(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
-            if (lane == 0) s_red[warp] = wmax;
-            __syncthreads();
-            if (tid == 0) {
-                float m = s_red[0];
-                for (int w = 1; w < FWARPS; ++w) m = fmaxf(m, s_red[w]);
-                p.part_x[(size_t)inst * p.part_stride + (p.cta_per_inst ? 0 : blockIdx.x)] = m;
-            }
-        }
-    }
+#include "ttn_fused_body.inc"
 }
 
 template <bool LOW, int ELEM = 0, bool GROUP = false>
 __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const FusedParams p) {
     extern __shared__ __align__(16) unsigned char fsm_raw[];
-    const int igroup = GROUP ? p.igroup : 1;
-    fused_pass_body<LOW, ELEM, GROUP>(p, fsm_raw, p.cta_per_inst ? (int)blockIdx.x * igroup : 0,
-                                      p.cta_per_inst ? (int)gridDim.x * igroup : 1);
+    const int inst_first = p.cta_per_inst ? (int)blockIdx.x * (GROUP ? p.igroup : 1) : 0;
+    const int inst_step = p.cta_per_inst ? (int)gridDim.x * (GROUP ? p.igroup : 1) : 1;
+#include "ttn_fused_body.inc"
 }
 
 // Batches of small lattices (every pass in cta_per_inst mode, no reduction pass -- the row-aligned
