@@ -549,15 +549,14 @@ inline FusedPlan make_fused_plan(int L, int max_gates_per_pass, const FusedGeom&
         FusedScheduler s(L, p, G);
         bool first = true;
         while ((first || !s.done()) && p.passes.size() < 4096) {
-            int best_a = -1, best_n = -1; double best_c = 0;
+            int best_a = -1, best_n = -1;
             for (int a = 0; a + G.WHIGH <= L; a = (a == 0 ? G.AMIN : a + 1)) {
                 FusedScheduler trial = s;                       // dry run on a copy
                 FusedPlan scratch; scratch.L = L;
                 trial.rebind(scratch);
                 FusedPass ps{};
                 const int n = trial.run_pass(a, a == 0, max_gates_per_pass, ps);
-                const double c = fused_pass_cost(ps, G);
-                if (n > best_n) { best_a = a; best_n = n; best_c = c; }          // ties: the lowest start
+                if (n > best_n) { best_a = a; best_n = n; }                      // ties: the lowest start
             }
             if (best_n <= 0 && !first) break;
             FusedPass ps{};
