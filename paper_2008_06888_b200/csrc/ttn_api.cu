@@ -323,12 +323,18 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
         grid = groups < (unsigned long long)P->fused_grid ? groups : (unsigned long long)P->fused_grid;
         if (ps.low) ttn::fused_pass_kernel<true, 0, true><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(true), st>>>(pp);
         else ttn::fused_pass_kernel<false, 0, true><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(false), st>>>(pp);
-    } else if (P->i16) {
-        if (ps.low) ttn::fused_pass_kernel<true, 1><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(true), st>>>(pp);
-        else ttn::fused_pass_kernel<false, 1><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(false), st>>>(pp);
     } else {
-        if (ps.low) ttn::fused_pass_kernel<true><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(true), st>>>(pp);
-        else ttn::fused_pass_kernel<false><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(false), st>>>(pp);
+        const bool red = (ps.flags & ttn::PASS_REDUCE) != 0;
+#define TTN_FUSED_LAUNCH(LOW_, ELEM_, RED_)                                                                             \
+        ttn::fused_pass_kernel<LOW_, ELEM_, false, RED_><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(LOW_), st>>>(pp)
+        if (P->i16) {
+            if (ps.low) { if (red) TTN_FUSED_LAUNCH(true, 1, true); else TTN_FUSED_LAUNCH(true, 1, false); }
+            else { if (red) TTN_FUSED_LAUNCH(false, 1, true); else TTN_FUSED_LAUNCH(false, 1, false); }
+        } else {
+            if (ps.low) { if (red) TTN_FUSED_LAUNCH(true, 0, true); else TTN_FUSED_LAUNCH(true, 0, false); }
+            else { if (red) TTN_FUSED_LAUNCH(false, 0, true); else TTN_FUSED_LAUNCH(false, 0, false); }
+        }
+#undef TTN_FUSED_LAUNCH
     }
     TTN_CUDA(cudaGetLastError());
     if (ps.flags & ttn::PASS_REDUCE) {
@@ -446,14 +452,18 @@ static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
     if (P->i16) {
         ttn::fused16_prep_kernel<<<grid, 256, 0, st>>>(q);
         TTN_CUDA(cudaGetLastError());
-        TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
-        TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));
+        TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 1, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 1, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
+        TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false, 1, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false, 1, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));
     } else {
         ttn::fused_prep_kernel<<<grid, 256, 0, st>>>(q);
     }
     TTN_CUDA(cudaGetLastError());
-    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
-    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 0, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 0, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false, 0, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false, 0, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));
     TTN_CUDA(cudaFuncSetAttribute(ttn::fused_sweep_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
     TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
     TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));

@@ -451,10 +451,12 @@ __device__ __forceinline__ void group_sync(int warp) {
 template <bool LOW, int ELEM, bool GROUP>
 __device__ __forceinline__ void fused_pass_body(const FusedParams& p, unsigned char* fsm_raw,
                                                 const int inst_first, const int inst_step) {
+    constexpr bool RED = false;          // GROUP passes never reduce
 #include "ttn_fused_body.inc"
 }
 
-template <bool LOW, int ELEM = 0, bool GROUP = false>
+// RED = the last pass of a sweep (adds A_{L-1}(s) and reduces instead of storing)
+template <bool LOW, int ELEM = 0, bool GROUP = false, bool RED = false>
 __global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const FusedParams p) {
     extern __shared__ __align__(16) unsigned char fsm_raw[];
     const int inst_first = p.cta_per_inst ? (int)blockIdx.x * (GROUP ? p.igroup : 1) : 0;
