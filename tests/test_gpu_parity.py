@@ -205,6 +205,28 @@ def test_backtrace_one_cta_per_instance_matches_multi_block(monkeypatch, L):
         assert abs(oracle.ising_energy(L, Jh[b], Jv[b], h[b], sig_a[b]) - E_a[b]) <= TOL * abs(E_a[b])
 
 
+@pytest.mark.parametrize("L", [12, 13, 14, 16])
+def test_one_launch_forward_sweep_matches_per_pass_launches(monkeypatch, L):
+    """ttn_ground_config on a batch of small lattices runs every forward pass in one launch
+    (fused_sweep_kernel, instance groups, LOW-tile prefetch).  Same kernels' arithmetic as one
+    launch per pass without grouping: E0 and sigma must be identical bit for bit (Gaussian
+    couplings, so any reordering of an addition would show), and match the oracle."""
+    B = 37                                             # odd: the last instance group is a single instance
+    Jh, Jv, h = make_batch(L, range(2800, 2800 + B), "gauss", fields=True)
+    E_a, sig_a = ttn.ground_config(Jh, Jv, h)
+    monkeypatch.setenv("TTN_DEBUG_NOSWEEP", "1")
+    E_b, sig_b = ttn.ground_config(Jh, Jv, h)
+    monkeypatch.setenv("TTN_DEBUG_NOGROUP", "1")
+    monkeypatch.setenv("TTN_DEBUG_NOLOWPF", "1")
+    E_c, sig_c = ttn.ground_config(Jh, Jv, h)
+    assert np.array_equal(E_a, E_b) and np.array_equal(sig_a, sig_b)
+    assert np.array_equal(E_a, E_c) and np.array_equal(sig_a, sig_c)
+    for b in (0, B // 2, B - 1):
+        Eo = oracle.dp_ising(L, Jh[b], Jv[b], h[b])[0]
+        assert abs(E_a[b] - Eo) <= TOL * abs(Eo)
+        assert abs(oracle.ising_energy(L, Jh[b], Jv[b], h[b], sig_a[b]) - Eo) <= TOL * abs(Eo)
+
+
 # ------------------------------------------------------------------ cfg 2: 16x16 Gaussian, config
 def test_cfg2_16x16_gaussian_ground_config_full_batch():
     Jh, Jv, h = config_batch(2)                         # 256 instances
