@@ -281,7 +281,7 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
         if (fp.mops[k].code == ttn::MC_XAB || fp.mops[k].code == ttn::MC_XBA) pp.prefetch_pc = k - ps.mop_begin + 1;
     if (a_mem > 18) pp.prefetch_pc = -1;     // > 256 distinct 2 MiB pages per tile: synchronous loads
     unsigned long long grid = (unsigned long long)P->fused_grid;
-    const int nw = ttn::fwarps(ps.low != 0);
+    const int nw = ttn::fwarps(ps.low != 0, P->i16 ? 1 : 0);
     // batches of small lattices: one CTA per instance at a time instead of the whole grid per instance
     pp.cta_per_inst = (P->batch > 1 && pp.tiles_per_inst < (unsigned long long)nw * grid) ? 1 : 0;
     if (pp.cta_per_inst) {
@@ -326,7 +326,7 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
     } else {
         const bool red = (ps.flags & ttn::PASS_REDUCE) != 0;
 #define TTN_FUSED_LAUNCH(LOW_, ELEM_, RED_)                                                                             \
-        ttn::fused_pass_kernel<LOW_, ELEM_, false, RED_><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(LOW_), st>>>(pp)
+        ttn::fused_pass_kernel<LOW_, ELEM_, false, RED_><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(LOW_, ELEM_), st>>>(pp)
         if (P->i16) {
             if (ps.low) { if (red) TTN_FUSED_LAUNCH(true, 1, true); else TTN_FUSED_LAUNCH(true, 1, false); }
             else { if (red) TTN_FUSED_LAUNCH(false, 1, true); else TTN_FUSED_LAUNCH(false, 1, false); }
@@ -452,10 +452,10 @@ static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
     if (P->i16) {
         ttn::fused16_prep_kernel<<<grid, 256, 0, st>>>(q);
         TTN_CUDA(cudaGetLastError());
-        TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 1, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
-    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 1, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
-        TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false, 1, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));
-    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false, 1, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));
+        TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 1, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true, 1)));
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 1, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true, 1)));
+        TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false, 1, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false, 1)));
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false, 1, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false, 1)));
     } else {
         ttn::fused_prep_kernel<<<grid, 256, 0, st>>>(q);
     }

@@ -37,14 +37,20 @@ namespace ttn {
 #ifndef TTN_FWARPS_HIGH
 #define TTN_FWARPS_HIGH 12
 #endif
-constexpr int FWARPS_LOW = TTN_FWARPS_LOW, FWARPS_HIGH = TTN_FWARPS_HIGH;
+// Tropical<i16>: 8 warps of <= 255 registers.  Measured at 32x32 (profiles/r01m.md): 12 / 8 / 4 warps
+// = 220 / 202 / 210 ms; the gain is in the passes whose tiles span 512 pages (a = 23: 18.2 -> 15.9,
+// 14.6 -> 11.5, 13.8 -> 9.7 ms) and in the LOW passes; f32 is fastest with 12 (336 / 359 / 387 ms).
+#ifndef TTN_FWARPS_I16
+#define TTN_FWARPS_I16 8
+#endif
+constexpr int FWARPS_LOW = TTN_FWARPS_LOW, FWARPS_HIGH = TTN_FWARPS_HIGH, FWARPS_I16 = TTN_FWARPS_I16;
 constexpr int FREGION_F4 = 33 * 32;       // float4 per warp exchange region (low tile: padded rows)
 constexpr int FMAX_MOPS = 128;            // micro-ops per pass
 constexpr int FMAX_GATES = 160;           // gates per pass (8 constants each)
 constexpr int FFINAL_FLOATS = 4 * 128 + 2 * 64;   // final table (4 variants) + H[64] + K[64]
-__host__ __device__ constexpr int fwarps(bool low) { return low ? FWARPS_LOW : FWARPS_HIGH; }
-__host__ __device__ constexpr size_t fsmem_bytes(bool low) {
-    return (size_t)fwarps(low) * FREGION_F4 * 16 + (size_t)(FMAX_GATES + 1) * 32 + (size_t)FFINAL_FLOATS * 4 +
+__host__ __device__ constexpr int fwarps(bool low, int elem = 0) { return elem == 1 ? FWARPS_I16 : (low ? FWARPS_LOW : FWARPS_HIGH); }
+__host__ __device__ constexpr size_t fsmem_bytes(bool low, int elem = 0) {
+    return (size_t)fwarps(low, elem) * FREGION_F4 * 16 + (size_t)(FMAX_GATES + 1) * 32 + (size_t)FFINAL_FLOATS * 4 +
            (size_t)FMAX_MOPS * 4 + 64;
 }
 
@@ -457,7 +463,7 @@ __device__ __forceinline__ void fused_pass_body(const FusedParams& p, unsigned c
 
 // RED = the last pass of a sweep (adds A_{L-1}(s) and reduces instead of storing)
 template <bool LOW, int ELEM = 0, bool GROUP = false, bool RED = false>
-__global__ void __launch_bounds__(fwarps(LOW) * 32, 1) fused_pass_kernel(const FusedParams p) {
+__global__ void __launch_bounds__(fwarps(LOW, ELEM) * 32, 1) fused_pass_kernel(const FusedParams p) {
     extern __shared__ __align__(16) unsigned char fsm_raw[];
     const int inst_first = p.cta_per_inst ? (int)blockIdx.x * (GROUP ? p.igroup : 1) : 0;
     const int inst_step = p.cta_per_inst ? (int)gridDim.x * (GROUP ? p.igroup : 1) : 1;
