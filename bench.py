@@ -331,7 +331,7 @@ def main():
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak,
                          # dram__bytes_read.sum + dram__bytes_write.sum per pass launch from the ncu
-                         # --set full capture in profiles/r01l_ncu_full_summary.csv (one read + one
+                         # --set full capture in profiles/r01m_ncu_full_summary.csv (one read + one
                          # write of the state); algorithmic bytes per launch = bytes_min / passes
                          "traffic": 17.18e9 + 17.12e9 if L == 32 else None,
                          "algorithmic_bytes_per_launch": bytes_min(L) / plan.num_passes,

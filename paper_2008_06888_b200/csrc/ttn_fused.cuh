@@ -14,7 +14,7 @@
 //     register digits in 4 boundary variants + a per-thread scalar) and max-reduces.
 // Global traffic: the LOW tile (columns 0..11) moves 128-byte lines straight between HBM and
 // registers with immediate offsets; HIGH tiles (columns a..a+8 plus the riding columns 0..2 on
-// the low lane bits) move whole 32-byte sectors, four per request, one IMAD.WIDE per address.
+// the low lane bits) move whole 32-byte sectors, four per request, one mad.wide.u32 per address.
 // The 4 warps of a HIGH group own the 4 sectors of every line and meet at a named barrier before
 // they touch memory; where a tile spans few pages the NEXT tile is fetched with cp.async into the
 // warp's own exchange region as soon as the last exchange of the current tile is done.
@@ -80,7 +80,7 @@ struct FusedParams {
     int part_stride;                    // partials per instance: gridDim.x, or 1 when cta_per_inst
     int L_cols;                         // Tropical<i16> only: lattice L (p.L = L - 1 word digits)
     unsigned stride_bytes;              // HIGH: 4 << a, passed opaque so that the address math stays
-                                        // one IMAD.WIDE (32 x 32 -> 64 bit) per access
+                                        // one mad.wide.u32 (32 x 32 -> 64 bit) per access
 };
 
 // (o0, o1) = (a0 + b0, a1 + b1) in one FADD2
@@ -341,10 +341,14 @@ __host__ __device__ constexpr int ereg_high(int layout, int j) {
           64 * ((j >> 5) & 1) + 32 * ((j >> 6) & 1);
 }
 
-// address of element offset (imm * stride) from a 64-bit base in ONE fma-pipe instruction
-// (IMAD.WIDE.U32); `sb` is the stride in bytes as an opaque 32-bit value.  The result is a
-// GLOBAL-space address: the accesses below are spelled ld.global / st.global because a pointer
-// that comes out of inline asm is "generic" to the compiler (LD/ST instead of LDG/STG).
+// address of element offset (imm * stride) from a 64-bit base: mad.wide.u32; `sb` is the stride
+// in bytes as an opaque 32-bit value.  ptxas 12.9 lowers it to IMAD.WIDE.U32 (product, fma pipe) +
+// IADD3 + IMAD.X (64-bit add).  The C++ spelling `gbase + (u64)sb * imm` does become ONE
+// IMAD.WIDE.U32 with a 64-bit addend (the HIGH kernel shrinks from 5096 to 4072 SASS instructions)
+// but the sweep is SLOWER with it (32x32: 338.8 vs 336.6 ms, profiles/r01m.md), so this form stays.
+// The result is a GLOBAL-space address: the accesses below are spelled ld.global / st.global
+// because a pointer that comes out of inline asm is "generic" to the compiler (LD/ST instead of
+// LDG/STG).
 __device__ __forceinline__ unsigned long long addr_mad(unsigned long long gbase, unsigned sb, unsigned imm) {
     unsigned long long r;
     asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(r) : "r"(sb), "r"(imm), "l"(gbase));
