@@ -488,10 +488,9 @@ inline double fused_pass_cost(const FusedPass& ps, const FusedGeom& G = GEOM_F32
     if (G.kind == 2) {
         // Tropical<i16>: half the bytes and half the alu work per element; tiles whose 9 active
         // word digits reach past bit 18 (> 256 pages of 2 MiB) are bound by address translation
-        if (ps.low) { const double t = 1.2 + 0.19 * g + 0.02 * ps.n_rounds + 0.25 * x; return t > 4.0 ? t : 4.0; }
-        const double t = 3.5 + 0.135 * g + 0.06 * ps.n_rounds + 0.25 * x;
-        const double floor_ = ps.a - 1 > 18 ? 12.5 : 5.0;
-        return t > floor_ ? t : floor_;
+        if (ps.low) { const double t = 1.0 + 0.165 * g + 0.02 * ps.n_rounds + 0.25 * x; return t > 4.0 ? t : 4.0; }
+        const double t = 2.9 + 0.115 * g + 0.06 * ps.n_rounds + 0.25 * x;
+        return t > 5.0 ? t : 5.0;
     }
     if (ps.low) { const double t = 1.2 + 0.267 * g + 0.02 * ps.n_rounds + 0.25 * x; return t > 6.5 ? t : 6.5; }
     const double t = 3.5 + 0.267 * g + 0.08 * ps.n_rounds + 0.25 * x;
