@@ -21,7 +21,11 @@ namespace ttn {
 constexpr int CRB = 5;                                   // register digits
 constexpr int CW_LOW = 10, CW_HIGH = 7;
 constexpr int CREGION_BYTES = 32 * 33 * 4 + 32 * 33 * 8; // padded x plane + padded n plane
-constexpr int CWARPS = 12;
+// warps per CTA: 24x24 counting, batch 16, with 8 / 12 / 16 warps = 87.3 / 77.3 / 78.6 ms (profiles/r01m.md)
+#ifndef TTN_CWARPS
+#define TTN_CWARPS 12
+#endif
+constexpr int CWARPS = TTN_CWARPS;
 constexpr int CFINAL_FLOATS = FFINAL_FLOATS;             // same table layout (first 4 x 32 entries used)
 __host__ __device__ constexpr size_t csmem_bytes() {
     return (size_t)CWARPS * CREGION_BYTES + (size_t)(FMAX_GATES + 1) * 32 + (size_t)CFINAL_FLOATS * 4 +
