@@ -399,7 +399,7 @@ def test_plan_split_api_relaunch():
 
 
 # ------------------------------------------------------------------ Tropical<i16>
-@pytest.mark.parametrize("L", [4, 12, 13, 14, 15, 17, 19])
+@pytest.mark.parametrize("L", [4, 12, 13, 14, 15, 17, 19, 21])
 def test_i16_energy_vs_oracle(L):
     """Exact integer arithmetic in 16 bits: bit-exact against the oracle, with and without fields."""
     rng = np.random.default_rng(1600 + L)
