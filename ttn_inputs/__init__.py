@@ -105,3 +105,24 @@ def config_batch(cfg: int, L: Optional[int] = None, n: Optional[int] = None):
     if n is not None:
         seeds = seeds[:n]
     return make_batch(L or c["L"], seeds, c["kind"], c["fields"], c["q"])
+
+
+@dataclass
+class ChimeraInstance:
+    M: int                      # rows of unit cells
+    N: int                      # columns of unit cells
+    T: int                      # spins per group (4 = the D-Wave chimera cell K_{4,4})
+    K: np.ndarray               # float32 [M, N, T, T]   vertical-group spin k x horizontal-group spin l
+    Jv: np.ndarray              # float32 [M-1, N, T]    vertical group of (r, c) - vertical group of (r+1, c)
+    Jh: np.ndarray              # float32 [M, N-1, T]    horizontal group of (r, c) - horizontal group of (r, c+1)
+    seed: int
+
+
+def make_chimera_instance(M: int, N: int, seed: int, T: int = 4) -> ChimeraInstance:
+    """+-J (p = 0.5), no field, on the chimera graph of M x N unit cells (SURVEY.md
+    8f NEXT-3).  Draw order: K row-major, then Jv, then Jh."""
+    nk, nv, nh = M * N * T * T, (M - 1) * N * T, M * (N - 1) * T
+    vals = _pm_one(splitmix64(seed, nk + nv + nh))
+    return ChimeraInstance(M=M, N=N, T=T, K=vals[:nk].reshape(M, N, T, T).copy(),
+                           Jv=vals[nk:nk + nv].reshape(M - 1, N, T).copy(),
+                           Jh=vals[nk + nv:].reshape(M, N - 1, T).copy(), seed=seed)
