@@ -101,6 +101,25 @@ ttn_status ttn_potts3_sweep_count(int L, const float* Jh, const float* Jv, int b
                                   void* workspace, size_t workspace_bytes, void* stream,
                                   double* E0 /*[batch]*/, double* degeneracy /*[batch]*/);
 
+/* ---- chimera graph (Fig. 2) -------------------------
+ * +-J (any integer couplings), no field, on M x N unit cells of K_{4,4}: cell (r, c) holds a
+ * vertical group v[0..4) and a horizontal group u[0..4);
+ *   K [M][N][4][4]  K[r][c][k][l] couples v_k and u_l of the same cell,
+ *   Jv[M-1][N][4]   couples v_k of (r, c) with v_k of (r+1, c)   (may be NULL when M = 1),
+ *   Jh[M][N-1][4]   couples u_l of (r, c) with u_l of (r, c+1)   (may be NULL when N = 1),
+ * energy as Eq. (1) with h = 0.  All three are HOST pointers, row-major float32.  The sweep runs
+ * column by column at the level of single spins in Tropical<i16> (the paper's Int16):
+ * a state of 2^(4M+4) int16 elements (the 4M horizontal spins of the column front and a 4-spin
+ * ancilla for the vertical group), one HBM pass per unit cell.  Exact; couplings must be
+ * integer-valued with sum |J| <= 8000, else TTN_EINVAL.  Limits: M <= 8 (137 GB state), N <= 64;
+ * beyond them TTN_EUNSUPPORTED.  `workspace` is a DEVICE pointer of at least
+ * ttn_chimera_workspace_bytes(M, N) bytes (0 = unsupported size); E0 receives the ground-state
+ * energy; the call synchronises `stream`. */
+size_t ttn_chimera_workspace_bytes(int M, int N);
+ttn_status ttn_chimera_sweep_energy_i16(int M, int N, const float* K, const float* Jv, const float* Jh,
+                                        void* workspace, size_t workspace_bytes, void* stream,
+                                        double* E0 /*[1]*/);
+
 /* ---- split API: upload once, launch asynchronously, read later ---------------------------
  * The one-call functions above are ttn_plan_create + ttn_plan_launch + ttn_plan_read +
  * ttn_plan_destroy.  A plan holds the host-side pass schedule (which gates

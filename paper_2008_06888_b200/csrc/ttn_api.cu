@@ -20,6 +20,7 @@
 #include "ttn_potts.cuh"
 #include "ttn_fused.cuh"
 #include "ttn_fcount.cuh"
+#include "ttn_chimera.cuh"
 
 namespace {
 
@@ -807,6 +808,85 @@ ttn_status ttn_potts3_sweep_energy(int L, const float* Jh, const float* Jv, int 
 ttn_status ttn_potts3_sweep_count(int L, const float* Jh, const float* Jv, int batch, void* ws,
                                   size_t wsb, void* stream, double* E0, double* g) {
     return one_call(3, L, TTN_CALL_COUNT, Jh, Jv, nullptr, batch, ws, wsb, stream, E0, g, nullptr);
+}
+
+// ---- chimera graph, Tropical<i16> (ttn_chimera.cuh) ---------------------------
+size_t ttn_chimera_workspace_bytes(int M, int N) {
+    if (M < 1 || M > 8 || N < 1 || N > 64) return 0;
+    return align_up((size_t)2 << (4 * M + 4)) + align_up((size_t)M * N * 128 * 4) + 256;
+}
+
+ttn_status ttn_chimera_sweep_energy_i16(int M, int N, const float* K, const float* Jv, const float* Jh,
+                                        void* ws, size_t wsb, void* stream, double* E0) {
+    if (M < 1 || N < 1 || !K || !E0 || !ws || (M > 1 && !Jv) || (N > 1 && !Jh)) return fail(TTN_EINVAL, "bad argument");
+    if (M > 8 || N > 64) return fail(TTN_EUNSUPPORTED, "chimera: M <= 8 rows of cells (state 2^(4M+4) int16), N <= 64");
+    const size_t need = ttn_chimera_workspace_bytes(M, N);
+    if (wsb < need) return fail(TTN_ENOMEM, "workspace too small: %zu < %zu", wsb, need);
+    // integer-valued couplings whose absolute sum fits 16 bits with room (as ttn_sweep_energy_i16)
+    double total = 0;
+    auto scan = [&](const float* a, size_t n) {
+        for (size_t i = 0; i < n; ++i) {
+            const double x = (double)a[i];
+            if (!std::isfinite(x) || x != std::nearbyint(x)) return false;
+            total += std::fabs(x);
+        }
+        return true;
+    };
+    if (!scan(K, (size_t)M * N * 16) || (M > 1 && !scan(Jv, (size_t)(M - 1) * N * 4)) || (N > 1 && !scan(Jh, (size_t)M * (N - 1) * 4)))
+        return fail(TTN_EINVAL, "chimera i16: couplings must be finite integers");
+    if (total > 8000.0) return fail(TTN_EINVAL, "chimera i16: sum |J| = %.0f exceeds 8000", total);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    unsigned char* base = static_cast<unsigned char*>(ws);
+    unsigned* state = reinterpret_cast<unsigned*>(base);
+    const size_t state_bytes = (size_t)2 << (4 * M + 4);
+    unsigned* tables = reinterpret_cast<unsigned*>(base + align_up(state_bytes));
+    int* d_out = reinterpret_cast<int*>(base + align_up(state_bytes) + align_up((size_t)M * N * 128 * 4));
+    // the cells' tables B(u, v) = sum_kl K[k][l] s_k(v) s_l(u), packed over the lowest bit of v
+    std::vector<unsigned> tab((size_t)M * N * 128);
+    for (int r = 0; r < M; ++r)
+        for (int c = 0; c < N; ++c) {
+            const float* Kc = K + ((size_t)r * N + c) * 16;
+            for (int u = 0; u < 16; ++u)
+                for (int j = 0; j < 8; ++j) {
+                    int val[2];
+                    for (int hlf = 0; hlf < 2; ++hlf) {
+                        const int v = 2 * j + hlf;
+                        int acc = 0;
+                        for (int k = 0; k < 4; ++k)
+                            for (int l = 0; l < 4; ++l)
+                                acc += (int)Kc[k * 4 + l] * (((v >> k) & 1) ? -1 : 1) * (((u >> l) & 1) ? -1 : 1);
+                        val[hlf] = acc;
+                    }
+                    tab[(((size_t)r * N + c) * 16 + u) * 8 + j] = ((unsigned)val[0] & 0xffffu) | ((unsigned)val[1] << 16);
+                }
+        }
+    TTN_CUDA(cudaMemcpyAsync(tables, tab.data(), tab.size() * 4, cudaMemcpyHostToDevice, st));
+    const int int_min = -2147483647 - 1;
+    TTN_CUDA(cudaMemcpyAsync(d_out, &int_min, sizeof(int), cudaMemcpyHostToDevice, st));
+    TTN_CUDA(cudaMemsetAsync(state, 0, state_bytes, st));            // tropical one
+    auto pack = [](float J) { const unsigned h = (unsigned)(int)J & 0xffffu; return h | (h << 16); };
+    ttn::ChimeraCellParams q;
+    q.state = state;
+    q.groups = 1ull << (4 * M - 4);
+    const unsigned long long blocks = (q.groups + ttn::CH_THREADS - 1) / ttn::CH_THREADS;
+    for (int c = 0; c < N; ++c)
+        for (int r = 0; r < M; ++r) {
+            q.p = 4 + 4 * r;
+            for (int l = 0; l < 4; ++l) q.ju[l] = c > 0 ? pack(Jh[((size_t)r * (N - 1) + (c - 1)) * 4 + l]) : 0u;
+            for (int k = 0; k < 4; ++k) q.jv[k] = r > 0 ? pack(Jv[((size_t)(r - 1) * N + c) * 4 + k]) : 0u;
+            q.table = tables + ((size_t)r * N + c) * 128;
+            ttn::chimera_cell_kernel<<<(unsigned)blocks, ttn::CH_THREADS, 0, st>>>(q);
+            TTN_CUDA(cudaGetLastError());
+        }
+    const unsigned long long words = 1ull << (4 * M + 3);
+    const unsigned rb = (unsigned)(words / 256 < 148ull * 8 ? (words + 255) / 256 : 148ull * 8);
+    ttn::chimera_max_kernel<<<rb, 256, 0, st>>>(state, words, d_out);
+    TTN_CUDA(cudaGetLastError());
+    int mx = 0;
+    TTN_CUDA(cudaMemcpyAsync(&mx, d_out, sizeof(int), cudaMemcpyDeviceToHost, st));
+    TTN_CUDA(cudaStreamSynchronize(st));
+    *E0 = mx == 0 ? 0.0 : -(double)mx;
+    return TTN_OK;
 }
 
 }  // extern "C"

@@ -1,0 +1,132 @@
+// ttn_chimera.cuh -- Tropical<i16> sweep of the chimera-graph spin glass (
+// PAPER.md:120-126, Fig. 2: M x N unit cells of K_{4,4}, "evolution of a state", Int16 elements).
+//
+// The paper contracts a network of 16 x 16 tropical matrices (one index per group of four spins).
+// Here the same contraction runs at the level of single spins, in the circuit picture of
+// every 16 x 16 inter-cell matrix is diagonal in the pairing of spin k with spin k,
+// so it factorises into four 2 x 2 max-plus gates (A2) PAPER.md:242, and the intra-cell K_{4,4}
+// tensor is a diagonal operator (a 256-entry table over the 4 + 4 spins of the cell).
+//
+// State: 2^(4M+4) int16 elements.  Index bits 0..3 = the ANCILLA: the vertical group v of the cell
+// being processed (it is swept down the column); bits 4+4r .. 7+4r = the horizontal group u of row
+// r (the boundary of the column sweep).  Bit = 0 means spin +1.  Two elements per 32-bit word
+// (ancilla bit 0 = the half of a word), packed add / max / add-max instructions as in the
+// Tropical<i16> Ising kernels.
+//
+// One launch = one cell (r, c) = one HBM pass over the state:
+//   1. four gates on the bits of u^r with the couplings Jh[r][c-1][l] (u of column c-1 -> u of
+//      column c; J = 0 in column 0: the state is still the tropical one there);
+//   2. four gates on the ancilla bits with Jv[r-1][c][k] (v of row r-1 -> v of row r; J = 0 for
+//      r = 0, which maximises over the previous column's last v and broadcasts the result);
+//   3. x += B(u, v) = sum_kl K[r][c][k][l] s_k(v) s_l(u), the cell's table.
+// A thread owns the 256 elements that differ in the 8 active bits: 16 rows (u) of one 32-byte sector
+// (v), 128 packed registers; consecutive threads own consecutive sectors of a row.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace ttn {
+
+constexpr int CH_THREADS = 256;
+
+struct ChimeraCellParams {
+    unsigned* state;              // 2^(4M+3) words
+    int p;                        // first bit of u^r in the ELEMENT index: 4 + 4 r
+    unsigned long long groups;    // 2^(4M+4-8) threads' worth of work
+    unsigned ju[4];               // packed (J, J) per spin l of u^r, as int16 pairs
+    unsigned jv[4];               // packed (J, J) per spin k of the ancilla
+    const unsigned* table;        // [16 u][8 words]: B(u, v), v = 2 j + half  (device)
+};
+
+__device__ __forceinline__ unsigned ch_neg2(unsigned k) { return __vneg2(k); }
+
+// gate (A2) on a bit that selects between two packed words A (bit = 0) and B (bit = 1):
+//   A' = max(A + J, B - J),  B' = max(B + J, A - J)
+__device__ __forceinline__ void ch_gate(unsigned& A, unsigned& B, const unsigned jp, const unsigned jn) {
+    const unsigned ta = __vadd2(A, jp), tb = __vadd2(B, jp);
+    const unsigned na = __viaddmax_s16x2(B, jn, ta);
+    const unsigned nb = __viaddmax_s16x2(A, jn, tb);
+    A = na; B = nb;
+}
+// gate on the half of a word: w = (lo: bit = 0, hi: bit = 1)
+__device__ __forceinline__ unsigned ch_gate_half(const unsigned w, const unsigned jp, const unsigned jn) {
+    const unsigned sw = __byte_perm(w, 0u, 0x1032);
+    return __viaddmax_s16x2(sw, jn, __vadd2(w, jp));
+}
+
+__global__ void __launch_bounds__(CH_THREADS) chimera_cell_kernel(const ChimeraCellParams q) {
+    __shared__ uint4 s_tab[32];                       // 16 rows x 8 words
+    if (threadIdx.x < 32) s_tab[threadIdx.x] = reinterpret_cast<const uint4*>(q.table)[threadIdx.x];
+    __syncthreads();
+    const unsigned long long G = (unsigned long long)blockIdx.x * CH_THREADS + threadIdx.x;
+    if (G >= q.groups) return;
+    // element index of (u = 0, v = 0): bits below p (above the ancilla) = low part of G, the rest above u^r
+    const int midbits = q.p - 4;
+    const unsigned long long mid = G & ((1ull << midbits) - 1), high = G >> midbits;
+    const unsigned long long e0 = (mid << 4) + (high << (q.p + 4));
+    uint4* base = reinterpret_cast<uint4*>(q.state + (e0 >> 1));
+    const unsigned long long row_stride = (1ull << q.p) >> 3;       // uint4 (8 elements) per step of u
+    unsigned w[16][8];
+#pragma unroll
+    for (int u = 0; u < 16; ++u) {
+        const uint4 a = base[u * row_stride], b = base[u * row_stride + 1];
+        w[u][0] = a.x; w[u][1] = a.y; w[u][2] = a.z; w[u][3] = a.w;
+        w[u][4] = b.x; w[u][5] = b.y; w[u][6] = b.z; w[u][7] = b.w;
+    }
+    // 1. gates on the four bits of u^r (row index)
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+        const unsigned jp = q.ju[l], jn = ch_neg2(jp);
+#pragma unroll
+        for (int u = 0; u < 16; ++u)
+            if (!(u & (1 << l))) {
+#pragma unroll
+                for (int j = 0; j < 8; ++j) ch_gate(w[u][j], w[u | (1 << l)][j], jp, jn);
+            }
+    }
+    // 2. gates on the ancilla: bit 0 = the half, bits 1..3 = the word index
+    {
+        const unsigned jp = q.jv[0], jn = ch_neg2(jp);
+#pragma unroll
+        for (int u = 0; u < 16; ++u)
+#pragma unroll
+            for (int j = 0; j < 8; ++j) w[u][j] = ch_gate_half(w[u][j], jp, jn);
+    }
+#pragma unroll
+    for (int k = 1; k < 4; ++k) {
+        const unsigned jp = q.jv[k], jn = ch_neg2(jp);
+#pragma unroll
+        for (int u = 0; u < 16; ++u)
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+                if (!(j & (1 << (k - 1)))) ch_gate(w[u][j], w[u][j | (1 << (k - 1))], jp, jn);
+    }
+    // 3. the cell's table, and store
+#pragma unroll
+    for (int u = 0; u < 16; ++u) {
+        const uint4 ta = s_tab[2 * u], tb = s_tab[2 * u + 1];
+        uint4 a, b;
+        a.x = __vadd2(w[u][0], ta.x); a.y = __vadd2(w[u][1], ta.y); a.z = __vadd2(w[u][2], ta.z); a.w = __vadd2(w[u][3], ta.w);
+        b.x = __vadd2(w[u][4], tb.x); b.y = __vadd2(w[u][5], tb.y); b.z = __vadd2(w[u][6], tb.z); b.w = __vadd2(w[u][7], tb.w);
+        base[u * row_stride] = a; base[u * row_stride + 1] = b;
+    }
+}
+
+// max over the whole state (both halves of every word) -> *out (int, initialised to INT_MIN by the host side)
+__global__ void __launch_bounds__(256) chimera_max_kernel(const unsigned* __restrict__ state, const unsigned long long words, int* out) {
+    unsigned m2 = 0x80008000u;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < words;
+         i += (unsigned long long)gridDim.x * blockDim.x)
+        m2 = __vmaxs2(m2, state[i]);
+    int m = max((int)(short)(m2 & 0xffffu), (int)(short)(m2 >> 16));
+    for (int o = 16; o; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+    __shared__ int s[8];
+    if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int k = 1; k < 8; ++k) m = max(m, s[k]);
+        atomicMax(out, m);
+    }
+}
+
+}  // namespace ttn

@@ -22,6 +22,7 @@ EXPORTS = [
     "ttn_potts3_sweep_energy", "ttn_potts3_sweep_count", "ttn_plan_create", "ttn_plan_launch",
     "ttn_plan_read", "ttn_plan_destroy", "ttn_plan_num_launches", "ttn_plan_num_passes",
     "ttn_plan_describe", "ttn_last_error", "ttn_version",
+    "ttn_chimera_workspace_bytes", "ttn_chimera_sweep_energy_i16",
 ]
 
 _STATUS = {1: "TTN_EINVAL", 2: "TTN_EUNSUPPORTED", 3: "TTN_ENOMEM", 4: "TTN_ECUDA"}
@@ -63,6 +64,9 @@ def lib() -> ctypes.CDLL:
         L.ttn_plan_describe.argtypes = [ci, ci, ci, ctypes.c_char_p, sz]
         L.ttn_plan_describe.restype = ctypes.c_long
         L.ttn_last_error.restype = ctypes.c_char_p
+        L.ttn_chimera_workspace_bytes.argtypes = [ci, ci]
+        L.ttn_chimera_workspace_bytes.restype = sz
+        L.ttn_chimera_sweep_energy_i16.argtypes = [ci, ci, fp, fp, fp, vp, sz, vp, dp]
         _lib = L
     return _lib
 
@@ -233,3 +237,28 @@ def potts3_sweep_energy(Jh, Jv, workspace=None, stream=None) -> np.ndarray:
 
 def potts3_sweep_count(Jh, Jv, workspace=None, stream=None) -> Tuple[np.ndarray, np.ndarray]:
     return _one_call("ttn_potts3_sweep_count", 3, CALL_COUNT, Jh, Jv, None, workspace, stream)
+
+
+def chimera_workspace_bytes(M: int, N: int) -> int:
+    n = lib().ttn_chimera_workspace_bytes(M, N)
+    if n == 0:
+        raise TTNError(2, f"chimera: unsupported size M={M}, N={N}")
+    return n
+
+
+def chimera_sweep_energy_i16(K, Jv, Jh, workspace=None, stream=None) -> float:
+    """ttn_chimera_sweep_energy_i16: ground-state energy of the +-J (integer-coupling) spin glass on
+    the chimera graph of M x N unit cells; K[M,N,4,4], Jv[M-1,N,4], Jh[M,N-1,4]."""
+    K = np.ascontiguousarray(np.asarray(K, dtype=np.float32))
+    if K.ndim != 4 or K.shape[2:] != (4, 4):
+        raise ValueError(f"K: expected shape [M, N, 4, 4], got {K.shape}")
+    M, N = K.shape[:2]
+    Jv = _f32(Jv, (M - 1, N, 4), "Jv")
+    Jh = _f32(Jh, (M, N - 1, 4), "Jh")
+    need = chimera_workspace_bytes(M, N)
+    ws = workspace if workspace is not None else alloc_workspace(need)
+    E0 = np.zeros(1, dtype=np.float64)
+    _check(lib().ttn_chimera_sweep_energy_i16(M, N, _fptr(K), _fptr(Jv), _fptr(Jh), ws.data_ptr(),
+                                              ws.numel() * ws.element_size(), _stream_ptr(stream),
+                                              E0.ctypes.data_as(ctypes.POINTER(ctypes.c_double))))
+    return float(E0[0])

@@ -516,3 +516,54 @@ def test_potts_20x20_planted_count():
     E1 = ttn.potts3_sweep_energy(Jh, Jv)
     assert E1[0] == E0[0]
     torch.cuda.empty_cache()
+
+
+# ------------------------------------------------------------------ chimera graph
+def _chimera_oracle():
+    from oracle import chimera_oracle
+    return chimera_oracle
+
+
+@pytest.mark.parametrize("M,N", [(1, 1), (1, 3), (2, 1), (2, 2), (3, 2), (2, 4), (3, 3), (4, 2), (4, 4)])
+def test_chimera_energy_vs_oracle(M, N):
+    """Bit-exact ground-state energies against the group tensor-network oracle (integers)."""
+    from ttn_inputs import make_chimera_instance
+    co = _chimera_oracle()
+    rng = np.random.default_rng(50 * M + N)
+    for seed in (6000, 6001):
+        I = make_chimera_instance(M, N, seed)
+        assert ttn.chimera_sweep_energy_i16(I.K, I.Jv, I.Jh) == co.dp_chimera(M, N, 4, I.K, I.Jv, I.Jh)[0]
+    K = rng.integers(-3, 4, size=(M, N, 4, 4)).astype(np.float32)
+    Jv = rng.integers(-3, 4, size=(M - 1, N, 4)).astype(np.float32)
+    Jh = rng.integers(-3, 4, size=(M, N - 1, 4)).astype(np.float32)
+    assert ttn.chimera_sweep_energy_i16(K, Jv, Jh) == co.dp_chimera(M, N, 4, K, Jv, Jh)[0]
+
+
+@pytest.mark.parametrize("M,N", [(5, 5), (6, 6), (7, 3)])
+def test_chimera_closed_forms_beyond_the_oracle(M, N):
+    """Ferromagnet, antiferromagnet (bipartite graph) and a planted instance: E0 = -#edges."""
+    co = _chimera_oracle()
+    ne = co.n_edges(M, N, 4)
+    one = lambda *s: np.ones(s, dtype=np.float32)
+    assert ttn.chimera_sweep_energy_i16(one(M, N, 4, 4), one(M - 1, N, 4), one(M, N - 1, 4)) == -ne
+    assert ttn.chimera_sweep_energy_i16(-one(M, N, 4, 4), -one(M - 1, N, 4), -one(M, N - 1, 4)) == -ne
+    rng = np.random.default_rng(M * N)
+    ev = rng.choice([-1.0, 1.0], size=(M, N, 4)); eu = rng.choice([-1.0, 1.0], size=(M, N, 4))
+    Kp, Jvp, Jhp = co.gauge(M, N, 4, one(M, N, 4, 4), one(M - 1, N, 4), one(M, N - 1, 4), ev, eu)
+    assert ttn.chimera_sweep_energy_i16(Kp, Jvp, Jhp) == -ne
+    # gauge invariance of a seeded +-J instance
+    from ttn_inputs import make_chimera_instance
+    I = make_chimera_instance(M, N, 6300)
+    K2, Jv2, Jh2 = co.gauge(M, N, 4, I.K, I.Jv, I.Jh, ev, eu)
+    assert ttn.chimera_sweep_energy_i16(I.K, I.Jv, I.Jh) == ttn.chimera_sweep_energy_i16(K2, Jv2, Jh2)
+
+
+def test_chimera_argument_errors():
+    K = np.ones((2, 2, 4, 4), dtype=np.float32); Jv = np.ones((1, 2, 4), dtype=np.float32); Jh = np.ones((2, 1, 4), dtype=np.float32)
+    with pytest.raises(ttn.TTNError) as e:
+        ttn.chimera_sweep_energy_i16(0.5 * K, Jv, Jh)
+    assert e.value.status == 1
+    with pytest.raises(ttn.TTNError) as e:
+        ttn.chimera_sweep_energy_i16(200 * K, Jv, Jh)
+    assert e.value.status == 1
+    assert ttn.lib().ttn_chimera_workspace_bytes(9, 4) == 0
