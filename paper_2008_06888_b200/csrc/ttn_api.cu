@@ -864,7 +864,9 @@ ttn_status ttn_chimera_sweep_energy_i16(int M, int N, const float* K, const floa
     const int int_min = -2147483647 - 1;
     TTN_CUDA(cudaMemcpyAsync(d_out, &int_min, sizeof(int), cudaMemcpyHostToDevice, st));
     TTN_CUDA(cudaMemsetAsync(state, 0, state_bytes, st));            // tropical one
-    auto pack = [](float J) { const unsigned h = (unsigned)(int)J & 0xffffu; return h | (h << 16); };
+    // a gate is applied as max(A, B - 2J); its common + J is summed here and added to the maximum
+    long shift = 0;
+    auto pack = [&](float J) { shift += (long)J; const unsigned h = (unsigned)(-2 * (int)J) & 0xffffu; return h | (h << 16); };
     ttn::ChimeraCellParams q;
     q.state = state;
     q.groups = 1ull << (4 * M - 4);
@@ -885,7 +887,8 @@ ttn_status ttn_chimera_sweep_energy_i16(int M, int N, const float* K, const floa
     int mx = 0;
     TTN_CUDA(cudaMemcpyAsync(&mx, d_out, sizeof(int), cudaMemcpyDeviceToHost, st));
     TTN_CUDA(cudaStreamSynchronize(st));
-    *E0 = mx == 0 ? 0.0 : -(double)mx;
+    const long top = (long)mx + shift;
+    *E0 = top == 0 ? 0.0 : -(double)top;
     return TTN_OK;
 }
 

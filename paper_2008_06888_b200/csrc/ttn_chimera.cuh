@@ -27,31 +27,35 @@
 
 namespace ttn {
 
-constexpr int CH_THREADS = 256;
+// Small CTAs: a CTA's warps load, compute and store in phase, so what overlaps memory with the gates
+// is CTAs of one SM being in different phases (256 threads: 89 ms per cell pass at 8 x 8 cells).
+#ifndef TTN_CH_THREADS
+#define TTN_CH_THREADS 64
+#endif
+constexpr int CH_THREADS = TTN_CH_THREADS;
 
 struct ChimeraCellParams {
     unsigned* state;              // 2^(4M+3) words
     int p;                        // first bit of u^r in the ELEMENT index: 4 + 4 r
     unsigned long long groups;    // 2^(4M+4-8) threads' worth of work
-    unsigned ju[4];               // packed (J, J) per spin l of u^r, as int16 pairs
-    unsigned jv[4];               // packed (J, J) per spin k of the ancilla
+    unsigned ju[4];               // packed (-2J, -2J) per spin l of u^r, as int16 pairs
+    unsigned jv[4];               // packed (-2J, -2J) per spin k of the ancilla
     const unsigned* table;        // [16 u][8 words]: B(u, v), v = 2 j + half  (device)
 };
 
-__device__ __forceinline__ unsigned ch_neg2(unsigned k) { return __vneg2(k); }
-
 // gate (A2) on a bit that selects between two packed words A (bit = 0) and B (bit = 1):
-//   A' = max(A + J, B - J),  B' = max(B + J, A - J)
-__device__ __forceinline__ void ch_gate(unsigned& A, unsigned& B, const unsigned jp, const unsigned jn) {
-    const unsigned ta = __vadd2(A, jp), tb = __vadd2(B, jp);
-    const unsigned na = __viaddmax_s16x2(B, jn, ta);
-    const unsigned nb = __viaddmax_s16x2(A, jn, tb);
+//   A' = max(A + J, B - J) = max(A, B - 2J) + J,  B' = max(B + J, A - 2J) = max(B, A - 2J) + J.
+// The common + J is the same for every element of the state, so it is left out here and added to
+// the final maximum on the host (sum of J over all gates): one VIADDMNMX per word and gate.
+// m2 = packed (-2J, -2J).
+__device__ __forceinline__ void ch_gate(unsigned& A, unsigned& B, const unsigned m2) {
+    const unsigned na = __viaddmax_s16x2(B, m2, A);
+    const unsigned nb = __viaddmax_s16x2(A, m2, B);
     A = na; B = nb;
 }
 // gate on the half of a word: w = (lo: bit = 0, hi: bit = 1)
-__device__ __forceinline__ unsigned ch_gate_half(const unsigned w, const unsigned jp, const unsigned jn) {
-    const unsigned sw = __byte_perm(w, 0u, 0x1032);
-    return __viaddmax_s16x2(sw, jn, __vadd2(w, jp));
+__device__ __forceinline__ unsigned ch_gate_half(const unsigned w, const unsigned m2) {
+    return __viaddmax_s16x2(__byte_perm(w, 0u, 0x1032), m2, w);
 }
 
 __global__ void __launch_bounds__(CH_THREADS) chimera_cell_kernel(const ChimeraCellParams q) {
@@ -76,30 +80,30 @@ __global__ void __launch_bounds__(CH_THREADS) chimera_cell_kernel(const ChimeraC
     // 1. gates on the four bits of u^r (row index)
 #pragma unroll
     for (int l = 0; l < 4; ++l) {
-        const unsigned jp = q.ju[l], jn = ch_neg2(jp);
+        const unsigned m2 = q.ju[l];
 #pragma unroll
         for (int u = 0; u < 16; ++u)
             if (!(u & (1 << l))) {
 #pragma unroll
-                for (int j = 0; j < 8; ++j) ch_gate(w[u][j], w[u | (1 << l)][j], jp, jn);
+                for (int j = 0; j < 8; ++j) ch_gate(w[u][j], w[u | (1 << l)][j], m2);
             }
     }
     // 2. gates on the ancilla: bit 0 = the half, bits 1..3 = the word index
     {
-        const unsigned jp = q.jv[0], jn = ch_neg2(jp);
+        const unsigned m2 = q.jv[0];
 #pragma unroll
         for (int u = 0; u < 16; ++u)
 #pragma unroll
-            for (int j = 0; j < 8; ++j) w[u][j] = ch_gate_half(w[u][j], jp, jn);
+            for (int j = 0; j < 8; ++j) w[u][j] = ch_gate_half(w[u][j], m2);
     }
 #pragma unroll
     for (int k = 1; k < 4; ++k) {
-        const unsigned jp = q.jv[k], jn = ch_neg2(jp);
+        const unsigned m2 = q.jv[k];
 #pragma unroll
         for (int u = 0; u < 16; ++u)
 #pragma unroll
             for (int j = 0; j < 8; ++j)
-                if (!(j & (1 << (k - 1)))) ch_gate(w[u][j], w[u][j | (1 << (k - 1))], jp, jn);
+                if (!(j & (1 << (k - 1)))) ch_gate(w[u][j], w[u][j | (1 << (k - 1))], m2);
     }
     // 3. the cell's table, and store
 #pragma unroll
