@@ -192,6 +192,33 @@ def other_configs(torch):
             torch.cuda.empty_cache()
         except ttn.TTNError as e:
             rows[name] = {"unavailable": str(e)}
+    # +-J chimera graph, L x L unit cells (8 L^2 spins), Tropical<i16>, through the
+    # one-call C ABI (host couplings; table upload and the read-back of E0 are inside the timed region).
+    # Roofline: one read + one write of the 2^(4L+4) int16 state per unit cell.
+    from ttn_inputs import make_chimera_instance
+    for Lc, reps in ((7, 3), (8, 2)):
+        name = f"next3_chimera_{Lc}x{Lc}_cells_{8 * Lc * Lc}_spins_i16"
+        try:
+            I = make_chimera_instance(Lc, Lc, 7000 + Lc)
+            wsc = ttn.alloc_workspace(ttn.chimera_workspace_bytes(Lc, Lc))
+            E = ttn.chimera_sweep_energy_i16(I.K, I.Jv, I.Jh, workspace=wsc)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for _ in range(reps):
+                E2 = ttn.chimera_sweep_energy_i16(I.K, I.Jv, I.Jh, workspace=wsc)
+            b.record()
+            torch.cuda.synchronize()
+            assert E2 == E
+            ms = a.elapsed_time(b) / reps
+            state_bytes = 2 * 2 ** (4 * Lc + 4)
+            rows[name] = {"ms_total": ms, "E0": E, "state_bytes": state_bytes, "hbm_passes": Lc * Lc,
+                          "launches": Lc * Lc + 1,
+                          "hbm_roofline_frac": Lc * Lc * 2 * state_bytes / (peak * 1e9) / (ms * 1e-3)}
+            del wsc
+            torch.cuda.empty_cache()
+        except (ttn.TTNError, RuntimeError) as e:      # RuntimeError: torch could not allocate the state
+            rows[name] = {"unavailable": str(e).splitlines()[0][:200]}
+            torch.cuda.empty_cache()
     return rows
 
 

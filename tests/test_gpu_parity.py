@@ -567,3 +567,31 @@ def test_chimera_argument_errors():
         ttn.chimera_sweep_energy_i16(200 * K, Jv, Jh)
     assert e.value.status == 1
     assert ttn.lib().ttn_chimera_workspace_bytes(9, 4) == 0
+
+
+def test_chimera_8x8_cells_512_spins():
+    """The paper's largest chimera size (8 L^2 = 512 spins), 2^36 int16 = 137 GB of state:
+    planted instance (gauge-transformed ferromagnet, E0 = -#edges = -1472) and gauge invariance of the
+    seeded +-J instance that bench.py times."""
+    import torch
+    from ttn_inputs import make_chimera_instance
+    co = _chimera_oracle()
+    M = N = 8
+    need = ttn.chimera_workspace_bytes(M, N)
+    free, _ = torch.cuda.mem_get_info()
+    if free < need + (1 << 30):
+        pytest.skip("needs 138 GB of free device memory")
+    ws = ttn.alloc_workspace(need)
+    one = lambda *s: np.ones(s, dtype=np.float32)
+    rng = np.random.default_rng(88)
+    ev = rng.choice([-1.0, 1.0], size=(M, N, 4)); eu = rng.choice([-1.0, 1.0], size=(M, N, 4))
+    Kp, Jvp, Jhp = co.gauge(M, N, 4, one(M, N, 4, 4), one(M - 1, N, 4), one(M, N - 1, 4), ev, eu)
+    assert co.n_edges(M, N, 4) == 1472
+    assert ttn.chimera_sweep_energy_i16(Kp, Jvp, Jhp, workspace=ws) == -1472.0
+    I = make_chimera_instance(M, N, 7008)
+    E = ttn.chimera_sweep_energy_i16(I.K, I.Jv, I.Jh, workspace=ws)
+    K2, Jv2, Jh2 = co.gauge(M, N, 4, I.K, I.Jv, I.Jh, ev, eu)
+    assert ttn.chimera_sweep_energy_i16(K2, Jv2, Jh2, workspace=ws) == E
+    assert -1472 < E < -700 and E == int(E)
+    del ws
+    torch.cuda.empty_cache()
