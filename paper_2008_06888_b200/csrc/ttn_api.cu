@@ -880,9 +880,9 @@ ttn_status ttn_chimera_sweep_energy_i16(int M, int N, const float* K, const floa
             ttn::chimera_cell_kernel<<<(unsigned)blocks, ttn::CH_THREADS, 0, st>>>(q);
             TTN_CUDA(cudaGetLastError());
         }
-    const unsigned long long words = 1ull << (4 * M + 3);
-    const unsigned rb = (unsigned)(words / 256 < 148ull * 8 ? (words + 255) / 256 : 148ull * 8);
-    ttn::chimera_max_kernel<<<rb, 256, 0, st>>>(state, words, d_out);
+    const unsigned long long quads = 1ull << (4 * M + 1);           // uint4 = 8 elements
+    const unsigned rb = (unsigned)(quads / 256 < 148ull * 8 ? (quads + 255) / 256 : 148ull * 8);
+    ttn::chimera_max_kernel<<<rb, 256, 0, st>>>(reinterpret_cast<const uint4*>(state), quads, d_out);
     TTN_CUDA(cudaGetLastError());
     int mx = 0;
     TTN_CUDA(cudaMemcpyAsync(&mx, d_out, sizeof(int), cudaMemcpyDeviceToHost, st));

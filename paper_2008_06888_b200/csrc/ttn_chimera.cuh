@@ -27,12 +27,17 @@
 
 namespace ttn {
 
-// Small CTAs: a CTA's warps load, compute and store in phase, so what overlaps memory with the gates
-// is CTAs of one SM being in different phases (256 threads: 89 ms per cell pass at 8 x 8 cells).
+// One-warp CTAs: the warps of a CTA load, compute and store in phase, so what overlaps memory with
+// the gates is CTAs of one SM being in different phases.  8 x 8 cells, per cell pass: 256 threads
+// 89 ms, 128: 58.7, 64: 57.3, 32: 56.4 ms (204 registers: 10 warps per SM either way); capping the
+// registers at 168 for 12 warps spills (69 - 81 ms).  profiles/r01n.md.
 #ifndef TTN_CH_THREADS
-#define TTN_CH_THREADS 64
+#define TTN_CH_THREADS 32
 #endif
 constexpr int CH_THREADS = TTN_CH_THREADS;
+#ifndef TTN_CH_MINBLOCKS
+#define TTN_CH_MINBLOCKS 1
+#endif
 
 struct ChimeraCellParams {
     unsigned* state;              // 2^(4M+3) words
@@ -58,7 +63,7 @@ __device__ __forceinline__ unsigned ch_gate_half(const unsigned w, const unsigne
     return __viaddmax_s16x2(__byte_perm(w, 0u, 0x1032), m2, w);
 }
 
-__global__ void __launch_bounds__(CH_THREADS) chimera_cell_kernel(const ChimeraCellParams q) {
+__global__ void __launch_bounds__(CH_THREADS, TTN_CH_MINBLOCKS) chimera_cell_kernel(const ChimeraCellParams q) {
     __shared__ uint4 s_tab[32];                       // 16 rows x 8 words
     if (threadIdx.x < 32) s_tab[threadIdx.x] = reinterpret_cast<const uint4*>(q.table)[threadIdx.x];
     __syncthreads();
@@ -117,11 +122,13 @@ __global__ void __launch_bounds__(CH_THREADS) chimera_cell_kernel(const ChimeraC
 }
 
 // max over the whole state (both halves of every word) -> *out (int, initialised to INT_MIN by the host side)
-__global__ void __launch_bounds__(256) chimera_max_kernel(const unsigned* __restrict__ state, const unsigned long long words, int* out) {
+__global__ void __launch_bounds__(256) chimera_max_kernel(const uint4* __restrict__ state, const unsigned long long quads, int* out) {
     unsigned m2 = 0x80008000u;
-    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < words;
-         i += (unsigned long long)gridDim.x * blockDim.x)
-        m2 = __vmaxs2(m2, state[i]);
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < quads;
+         i += (unsigned long long)gridDim.x * blockDim.x) {
+        const uint4 t = state[i];
+        m2 = __vmaxs2(__vmaxs2(m2, t.x), __vmaxs2(__vmaxs2(t.y, t.z), t.w));
+    }
     int m = max((int)(short)(m2 & 0xffffu), (int)(short)(m2 >> 16));
     for (int o = 16; o; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
     __shared__ int s[8];
