@@ -1,8 +1,9 @@
 """CPU oracle for the chimera-graph spin glass -- TEST INFRASTRUCTURE ONLY.
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline leg may import this module.
-There is NO CUDA path for NEXT-3 yet: this file and its pins (tests/test_chimera_oracle_pins.py)
-are the groundwork the tier rules ask for before the first kernel.
+It shares no code with the CUDA path (csrc/ttn_chimera.cuh works on single spins with an ancilla;
+this file contracts the paper's group tensors) and was committed, pinned
+(tests/test_chimera_oracle_pins.py), before that kernel.
 
 The model ("+-J coupling and no external field on the chimera graph ... unit cells
 arranged in a square grid ... Each unit cell contains 8 spins forming a complete bipartite graph.

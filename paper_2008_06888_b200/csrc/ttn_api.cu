@@ -870,7 +870,17 @@ ttn_status ttn_chimera_sweep_energy_i16(int M, int N, const float* K, const floa
     ttn::ChimeraCellParams q;
     q.state = state;
     q.groups = 1ull << (4 * M - 4);
-    const unsigned long long blocks = (q.groups + ttn::CH_THREADS - 1) / ttn::CH_THREADS;
+    unsigned long long blocks = (q.groups + ttn::CH_THREADS - 1) / ttn::CH_THREADS;
+    {   // a CTA walks its groups with the stride of the grid; 512 CTAs per SM measured best at 8 x 8
+        // cells (per SM 8 / 32 / 64 / 128 / 512 CTAs: 3.27 / 3.24 / 3.19 / 3.15 / 3.12 s; one group per
+        // thread, i.e. 2^23 CTAs: 3.61 s)
+        int dev = 0, sms = 0, per_sm = 512;
+        TTN_CUDA(cudaGetDevice(&dev));
+        TTN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        if (const char* e = getenv("TTN_DEBUG_CH_PERSM")) { int v = atoi(e); if (v >= 1) per_sm = v; }
+        const unsigned long long cap = (unsigned long long)sms * (unsigned long long)per_sm;
+        if (blocks > cap) blocks = cap;
+    }
     for (int c = 0; c < N; ++c)
         for (int r = 0; r < M; ++r) {
             q.p = 4 + 4 * r;

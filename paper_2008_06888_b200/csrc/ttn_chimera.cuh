@@ -28,9 +28,10 @@
 namespace ttn {
 
 // One-warp CTAs: the warps of a CTA load, compute and store in phase, so what overlaps memory with
-// the gates is CTAs of one SM being in different phases.  8 x 8 cells, per cell pass: 256 threads
-// 89 ms, 128: 58.7, 64: 57.3, 32: 56.4 ms (204 registers: 10 warps per SM either way); capping the
-// registers at 168 for 12 warps spills (69 - 81 ms).  profiles/r01n.md.
+// the gates is CTAs of one SM being in different phases.  8 x 8 cells, per cell pass, one group per
+// thread: 256 threads 89 ms, 128: 58.7, 64: 57.3, 32: 56.4 ms; capping the registers at 168 for
+// 12 warps spills (69 - 81 ms).  With the grid-stride loop below (512 CTAs per SM): 48.7 ms.
+// profiles/r01n.md.
 #ifndef TTN_CH_THREADS
 #define TTN_CH_THREADS 32
 #endif
@@ -67,8 +68,9 @@ __global__ void __launch_bounds__(CH_THREADS, TTN_CH_MINBLOCKS) chimera_cell_ker
     __shared__ uint4 s_tab[32];                       // 16 rows x 8 words
     if (threadIdx.x < 32) s_tab[threadIdx.x] = reinterpret_cast<const uint4*>(q.table)[threadIdx.x];
     __syncthreads();
-    const unsigned long long G = (unsigned long long)blockIdx.x * CH_THREADS + threadIdx.x;
-    if (G >= q.groups) return;
+    // a CTA walks the groups with the stride of the grid (ttn_api.cu sizes the grid)
+    for (unsigned long long G = (unsigned long long)blockIdx.x * CH_THREADS + threadIdx.x; G < q.groups;
+         G += (unsigned long long)gridDim.x * CH_THREADS) {
     // element index of (u = 0, v = 0): bits below p (above the ancilla) = low part of G, the rest above u^r
     const int midbits = q.p - 4;
     const unsigned long long mid = G & ((1ull << midbits) - 1), high = G >> midbits;
@@ -118,6 +120,7 @@ __global__ void __launch_bounds__(CH_THREADS, TTN_CH_MINBLOCKS) chimera_cell_ker
         a.x = __vadd2(w[u][0], ta.x); a.y = __vadd2(w[u][1], ta.y); a.z = __vadd2(w[u][2], ta.z); a.w = __vadd2(w[u][3], ta.w);
         b.x = __vadd2(w[u][4], tb.x); b.y = __vadd2(w[u][5], tb.y); b.z = __vadd2(w[u][6], tb.z); b.w = __vadd2(w[u][7], tb.w);
         base[u * row_stride] = a; base[u * row_stride + 1] = b;
+    }
     }
 }
 

@@ -1,4 +1,4 @@
-"""Pins of the chimera oracle (SURVEY.md 8f NEXT-3 groundwork; no CUDA path yet).
+"""Pins of the chimera oracle (the CUDA path is tested in test_gpu_parity.py).
 
 oracle/chimera_oracle.py holds two independent computations: the definition (enumeration) and the
 paper's group tensor network.  Here the second is pinned to the first on every
