@@ -887,7 +887,13 @@ ttn_status ttn_chimera_sweep_energy_i16(int M, int N, const float* K, const floa
             for (int l = 0; l < 4; ++l) q.ju[l] = c > 0 ? pack(Jh[((size_t)r * (N - 1) + (c - 1)) * 4 + l]) : 0u;
             for (int k = 0; k < 4; ++k) q.jv[k] = r > 0 ? pack(Jv[((size_t)(r - 1) * N + c) * 4 + k]) : 0u;
             q.table = tables + ((size_t)r * N + c) * 128;
-            ttn::chimera_cell_kernel<<<(unsigned)blocks, ttn::CH_THREADS, 0, st>>>(q);
+            if (r == 0 && q.groups >= 32 && !getenv("TTN_DEBUG_CH_NOCELL0")) {
+                const unsigned long long tiles = q.groups >> 5, wpb = ttn::CH_THREADS / 32;
+                const unsigned long long b0 = (tiles + wpb - 1) / wpb;
+                ttn::chimera_cell0_kernel<<<(unsigned)(b0 < blocks ? b0 : blocks), ttn::CH_THREADS, 0, st>>>(q);
+            } else {
+                ttn::chimera_cell_kernel<<<(unsigned)blocks, ttn::CH_THREADS, 0, st>>>(q);
+            }
             TTN_CUDA(cudaGetLastError());
         }
     const unsigned long long quads = 1ull << (4 * M + 1);           // uint4 = 8 elements
