@@ -863,7 +863,6 @@ ttn_status ttn_chimera_sweep_energy_i16(int M, int N, const float* K, const floa
     TTN_CUDA(cudaMemcpyAsync(tables, tab.data(), tab.size() * 4, cudaMemcpyHostToDevice, st));
     const int int_min = -2147483647 - 1;
     TTN_CUDA(cudaMemcpyAsync(d_out, &int_min, sizeof(int), cudaMemcpyHostToDevice, st));
-    TTN_CUDA(cudaMemsetAsync(state, 0, state_bytes, st));            // tropical one
     // a gate is applied as max(A, B - 2J); its common + J is summed here and added to the maximum
     long shift = 0;
     auto pack = [&](float J) { shift += (long)J; const unsigned h = (unsigned)(-2 * (int)J) & 0xffffu; return h | (h << 16); };
@@ -884,6 +883,7 @@ ttn_status ttn_chimera_sweep_energy_i16(int M, int N, const float* K, const floa
     for (int c = 0; c < N; ++c)
         for (int r = 0; r < M; ++r) {
             q.p = 4 + 4 * r;
+            q.init = (c == 0 && r == 0) ? 1 : 0;      // write-only first pass: every element is written
             for (int l = 0; l < 4; ++l) q.ju[l] = c > 0 ? pack(Jh[((size_t)r * (N - 1) + (c - 1)) * 4 + l]) : 0u;
             for (int k = 0; k < 4; ++k) q.jv[k] = r > 0 ? pack(Jv[((size_t)(r - 1) * N + c) * 4 + k]) : 0u;
             q.table = tables + ((size_t)r * N + c) * 128;

@@ -15,7 +15,8 @@
 //
 // One launch = one cell (r, c) = one HBM pass over the state:
 //   1. four gates on the bits of u^r with the couplings Jh[r][c-1][l] (u of column c-1 -> u of
-//      column c; J = 0 in column 0: the state is still the tropical one there);
+//      column c; J = 0 in column 0: the state is still the tropical one there -- the very first
+//      cell does not read it at all, it starts from zeros in registers);
 //   2. four gates on the ancilla bits with Jv[r-1][c][k] (v of row r-1 -> v of row r; J = 0 for
 //      r = 0, which maximises over the previous column's last v and broadcasts the result);
 //   3. x += B(u, v) = sum_kl K[r][c][k][l] s_k(v) s_l(u), the cell's table.
@@ -43,6 +44,7 @@ constexpr int CH_THREADS = TTN_CH_THREADS;
 struct ChimeraCellParams {
     unsigned* state;              // 2^(4M+3) words
     int p;                        // first bit of u^r in the ELEMENT index: 4 + 4 r
+    int init;                     // the very first cell: the state is the tropical one (0), nothing is read
     unsigned long long groups;    // 2^(4M+4-8) threads' worth of work
     unsigned ju[4];               // packed (-2J, -2J) per spin l of u^r, as int16 pairs
     unsigned jv[4];               // packed (-2J, -2J) per spin k of the ancilla
@@ -80,7 +82,8 @@ __global__ void __launch_bounds__(CH_THREADS, TTN_CH_MINBLOCKS) chimera_cell_ker
     unsigned w[16][8];
 #pragma unroll
     for (int u = 0; u < 16; ++u) {
-        const uint4 a = base[u * row_stride], b = base[u * row_stride + 1];
+        const uint4 z = make_uint4(0u, 0u, 0u, 0u);                     // tropical one
+        const uint4 a = q.init ? z : base[u * row_stride], b = q.init ? z : base[u * row_stride + 1];
         w[u][0] = a.x; w[u][1] = a.y; w[u][2] = a.z; w[u][3] = a.w;
         w[u][4] = b.x; w[u][5] = b.y; w[u][6] = b.z; w[u][7] = b.w;
     }
@@ -141,7 +144,7 @@ __global__ void __launch_bounds__(CH_THREADS) chimera_cell0_kernel(const Chimera
         unsigned w[32][4];
 #pragma unroll
         for (int i = 0; i < 32; ++i) {
-            const uint4 a = base[32 * i];
+            const uint4 a = q.init ? make_uint4(0u, 0u, 0u, 0u) : base[32 * i];
             w[i][0] = a.x; w[i][1] = a.y; w[i][2] = a.z; w[i][3] = a.w;
         }
         // gates on u^0 (lane bits 1..4) and on ancilla bit 3 (lane bit 0)
