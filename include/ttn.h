@@ -20,9 +20,17 @@
  * Memory spaces.  Couplings and results are HOST pointers (they are O(L^2) numbers);
  * `workspace` is a DEVICE pointer owned by the caller (at least ttn_workspace_bytes(...)
  * bytes, 256-byte aligned), `stream` is a cudaStream_t passed as void* (NULL = default
- * stream).  The library allocates no device memory and keeps no global state; every step of
- * the path runs in the library's own sm_100a kernels.  There is NO CPU fallback: without a
- * CUDA device every compute call returns TTN_ECUDA.
+ * stream).  The library allocates no device memory; its only process-wide state is a
+ * mutex-guarded memo of searched Potts pass schedules (a pure function of L).  The TTN_DEBUG_*
+ * environment switches (test hooks) are read once per entry point and a plan keeps the values it
+ * was created with.  Every step of the path runs in the library's own sm_100a kernels.  There
+ * is NO CPU fallback: without a CUDA device every compute call returns TTN_ECUDA.
+ *
+ * h = 0 (NULL or all zero): Eq. (1) is invariant under the global flip sigma -> -sigma, and so is
+ * every intermediate state of the sweep; ttn_sweep_energy then stores only the half of the state
+ * vector with column 0 up (2^(L-1) elements) and applies the column-0 gates as a pairing of
+ * every element with its complement -- half the memory, bytes and arithmetic, identical results
+ * (SURVEY.md 8f NEXT-4).  Any non-zero field selects the full-state sweep.
  *
  * Layouts (row-major, batch-major):  Jh[batch][L][L-1], Jv[batch][L-1][L], h[batch][L][L]
  * (h may be NULL = all zero), E0[batch], degeneracy[batch], sigma[batch][L][L] (+1 / -1).
@@ -131,7 +139,13 @@ ttn_status ttn_chimera_sweep_energy_i16(int M, int N, const float* K, const floa
  *   ttn_plan_read   : device->host copy of the results of the last launch; synchronises.
  *                     Pointers that do not apply to the plan's call kind must be NULL.      */
 typedef struct ttn_plan ttn_plan;
-typedef enum { TTN_CALL_ENERGY = 0, TTN_CALL_COUNT = 1, TTN_CALL_CONFIG = 2, TTN_CALL_ENERGY_I16 = 3 } ttn_call;
+typedef enum {
+    TTN_CALL_ENERGY = 0, TTN_CALL_COUNT = 1, TTN_CALL_CONFIG = 2, TTN_CALL_ENERGY_I16 = 3,
+    /* TTN_CALL_ENERGY with the flip-reduced half-state REQUIRED: TTN_EINVAL when h != 0 (lattices with
+       L < 14 run the plain sweep).  TTN_CALL_ENERGY selects it by itself when h = 0; this kind exists
+       for ttn_plan_describe and for tests. */
+    TTN_CALL_ENERGY_Z2 = 4
+} ttn_call;
 
 ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const float* Jv,
                            const float* h, int batch, void* workspace, size_t workspace_bytes,
@@ -144,6 +158,9 @@ void ttn_plan_destroy(ttn_plan* plan);
 /* Introspection (host only, no CUDA calls). */
 int ttn_plan_num_launches(const ttn_plan* plan);   /* kernels enqueued by one ttn_plan_launch   */
 int ttn_plan_num_passes(const ttn_plan* plan);     /* HBM passes over the state among them      */
+/* State-vector elements stored per instance: q^L, or 2^(L-1) when the plan uses the h = 0 flip
+   reduction (see the top of this file). */
+unsigned long long ttn_plan_state_elements(const ttn_plan* plan);
 /* Writes a text description of the pass schedule for (q, L, call) -- one line per pass and
    one per op -- into buf (NUL-terminated, truncated to n).  Returns the untruncated length,
    or -1 on bad arguments.  Needs no device: used by the CPU-side schedule validator.          */

@@ -8,7 +8,7 @@ this file contracts the paper's group tensors) and was committed, pinned
 The model ("+-J coupling and no external field on the chimera graph ... unit cells
 arranged in a square grid ... Each unit cell contains 8 spins forming a complete bipartite graph.
 Each group of four spins within the unit cell connects horizontally or vertically to the spins in
-the neighboring unit cells"), energy as Eq. (1) PAPER.md:45:  E = - sum_<ij> J_ij s_i s_j - sum h_i s_i.
+the neighboring unit cells"), energy as Eq. (1) PAPER.md:29:  E = - sum_<ij> J_ij s_i s_j - sum h_i s_i.
 
     M x N cells, T spins per group (T = 4 on the device; smaller T only so that brute force reaches
     2 x 2 cells).  Cell (r, c) holds a VERTICAL group v[0..T) and a HORIZONTAL group u[0..T).
@@ -25,7 +25,7 @@ Two independent computations:
     of a state of dimension (2^T)^M column by column -- for every column: the horizontal matrices
     H_r[u, u'] act on the M indices, then the column's vertical chain (black tensors K_r[u', v]
     and red matrices V_r[v, v']) is contracted for every boundary value.  CountingTropical
-    arithmetic: (x, n) (+) = max with counts added on ties, (x) = (x1+x2, n1*n2).
+    arithmetic (Eq. (4)): (x, n) (+) = max with counts added on ties, (x) = (x1+x2, n1*n2).
     Values in float64 (exact for integer couplings), counts in int64; OverflowError instead of a
     wrapped count (a later 16-term sum of counts below 2^57 stays below 2^62).
 """

@@ -328,6 +328,9 @@ enum MicroCode : uint8_t { MC_END = 0, MC_XAB = 1, MC_XBA = 2, MC_ROUND = 3, MC_
 
 struct MicroOp { uint8_t code; uint8_t mask; uint16_t arg; };   // ROUND: mask = register bits, arg = index of
                                                                 // its first gate in the pass's gate list
+                                                                // | MOP_FLIP: the round ends with the Z2 flip gate
+constexpr uint16_t MOP_FLIP = 0x8000;       // (column 0, see "GLOBAL-FLIP (Z2) REDUCTION" below)
+constexpr int GATE_RC_FLIP = 1 << 17;       // gate_rc flag of a flip gate (its K field is 0)
 
 constexpr int F_RB = 7;          // register digits
 constexpr int F_WLOW = 12;       // active digits of the low tile
@@ -368,21 +371,56 @@ constexpr int fused_bit_of_digit(bool low, int layout, int d) {
 //          kind-0 geometry applies to the word index (column c >= 1 = word digit c-1).  The LOW
 //          tile has 13 columns; pseudo register bit 7 is the half digit (in every LOW layout);
 //          HIGH tiles start at column a >= 5 (word digit a-1) and column 0 rides.
+//
+// GLOBAL-FLIP (Z2) REDUCTION, h = 0 (symmetry of Eq. (1) PAPER.md:29 without the
+// field term).  Every gate (A2) and every diagonal (A4) commutes with the flip F: s -> ~s, and the
+// initial state is F-invariant, so EVERY intermediate state of every schedule obeys W[s] = W[~s].
+// Only the half with column 0 up (s_0 = 0) is stored: an (L-1)-digit state u = (s_1 .. s_{L-1}).
+//   * a gate on column c >= 1 stays inside the half; column 1's left neighbour is the constant
+//     sigma_0 = +1 (the kernels' "column -1 does not exist" bit 0, with K_0 in the constants);
+//   * the gate on column 0 pairs s with the element whose column-0 bit is set, which the symmetry
+//     maps to the COMPLEMENT of u inside the half:
+//         W'[u] = max(W[u], W[~u] + m - 2 K_0 sigma_1(u)),    m = -2 Jv[r-1][0];
+//     it touches no particular digit, so it is legal in any tile; it depends, by the usual
+//     stencil, on column 1, which the LOW tile holds: it is scheduled there as pseudo register
+//     bit RB (+1) of every LOW layout, and the LOW kernel pairs warps on tiles (T, ~T).
+//  kind 3: Tropical<f32> + Z2: the kind-0 geometry on the digits d = c - 1 (same column maps as kind 2)
+//  kind 4: CountingTropical + Z2: the kind-1 geometry on d = c - 1, pseudo bit 5 = column 0
+//  kind 5: Tropical<i16> + Z2: column 1 is the half of a word (pseudo bit 7), word digit = c - 2,
+//          pseudo bit 8 = column 0
 struct FusedGeom { int RB, WLOW, WHIGH, RIDE, AMIN, kind; };
 constexpr FusedGeom GEOM_F32{F_RB, F_WLOW, F_WHIGH, F_RIDE, F_AMIN, 0};
 constexpr FusedGeom GEOM_COUNT{5, 10, 7, 3, 4, 1};
 constexpr FusedGeom GEOM_I16{F_RB, F_WLOW + 1, F_WHIGH, F_RIDE + 1, F_AMIN + 1, 2};
+constexpr FusedGeom GEOM_F32_Z2{F_RB, F_WLOW + 1, F_WHIGH, F_RIDE + 1, F_AMIN + 1, 3};
+constexpr FusedGeom GEOM_COUNT_Z2{5, 11, 7, 4, 5, 4};
+constexpr FusedGeom GEOM_I16_Z2{F_RB, F_WLOW + 2, F_WHIGH, F_RIDE + 2, F_AMIN + 2, 5};
+// columns in front of the first tile digit of the kernel's index space (virtual / sub-word columns)
 #if defined(__CUDACC__)
 __host__ __device__
 #endif
-constexpr int geom_bits(const FusedGeom& g, bool low) { return g.kind == 2 && low ? g.RB + 1 : g.RB; }
+constexpr int geom_col_off(const FusedGeom& g) { return g.kind == 2 || g.kind == 3 || g.kind == 4 ? 1 : (g.kind == 5 ? 2 : 0); }
+#if defined(__CUDACC__)
+__host__ __device__
+#endif
+constexpr bool geom_has_flip(const FusedGeom& g) { return g.kind >= 3; }
+// bits of a ROUND mask: the register bits, + the half-of-a-word column of the i16 LOW tiles (bit RB)
+#if defined(__CUDACC__)
+__host__ __device__
+#endif
+constexpr int geom_bits(const FusedGeom& g, bool low) { return (g.kind == 2 || g.kind == 5) && low ? g.RB + 1 : g.RB; }
+// lattice column (relative to the tile start a; LOW tiles: a = 0) acted on by mask bit `bit`
 #if defined(__CUDACC__)
 __host__ __device__
 #endif
 constexpr int geom_digit_of_bit(const FusedGeom& g, bool low, int layout, int bit) {
-    return g.kind == 0 ? fused_digit_of_bit(low, layout, bit)
-         : g.kind == 1 ? (layout == 0 ? bit : (low ? g.WLOW : g.WHIGH) - 1 - bit)
-         : (low ? (bit == F_RB ? 0 : 1 + fused_digit_of_bit(true, layout, bit)) : fused_digit_of_bit(false, layout, bit));
+    if (g.kind == 0) return fused_digit_of_bit(low, layout, bit);
+    if (g.kind == 1) return layout == 0 ? bit : (low ? g.WLOW : g.WHIGH) - 1 - bit;
+    if (g.kind == 4) return low ? 1 + (layout == 0 ? bit : g.WLOW - 2 - bit) : (layout == 0 ? bit : g.WHIGH - 1 - bit);
+    if (!low) return fused_digit_of_bit(false, layout, bit);
+    if (g.kind == 5) return bit == F_RB ? 1 : 2 + fused_digit_of_bit(true, layout, bit);
+    if (g.kind == 3) return 1 + fused_digit_of_bit(true, layout, bit);
+    return bit == F_RB ? 0 : 1 + fused_digit_of_bit(true, layout, bit);       // kind 2
 }
 
 struct FusedPass {
@@ -457,18 +495,21 @@ class FusedScheduler {
         int n = 0;
         for (;;) {
             const int nb = geom_bits(G_, low);
-            if ((int)Pp_->gate_rc.size() - pass_gate_begin_ + nb > max_gates_) break;
+            if ((int)Pp_->gate_rc.size() - pass_gate_begin_ + nb + 1 > max_gates_) break;
             if ((int)Pp_->mops.size() - pass_mop_begin_ + 8 > max_mops_) break;
             unsigned mask = 0;
             for (int b = 0; b < nb; ++b) if (legal(a + geom_digit_of_bit(G_, low, layout, b))) mask |= 1u << b;
-            if (!mask) break;
-            Pp_->mops.push_back({MC_ROUND, (uint8_t)mask, (uint16_t)((int)Pp_->gate_rc.size() - pass_gate_begin_)});
+            const bool flip = low && geom_has_flip(G_) && legal(0);      // Z2: the gate on column 0
+            if (!mask && !flip) break;
+            Pp_->mops.push_back({MC_ROUND, (uint8_t)mask, (uint16_t)(((int)Pp_->gate_rc.size() - pass_gate_begin_) | (flip ? MOP_FLIP : 0))});
             for (int b = 0; b < nb; ++b) if (mask >> b & 1) {
                 const int c = a + geom_digit_of_bit(G_, low, layout, b);
                 Pp_->gate_rc.push_back((low ? 1 << 16 : 0) | (b << 13) | (layout << 12) | (grow_[c] << 6) | c);
                 ++n;
             }
+            if (flip) { Pp_->gate_rc.push_back(GATE_RC_FLIP | (low ? 1 << 16 : 0) | (layout << 12) | (grow_[0] << 6) | 0); ++n; }
             for (int b = 0; b < nb; ++b) if (mask >> b & 1) grow_[a + geom_digit_of_bit(G_, low, layout, b)] += 1;
+            if (flip) grow_[0] += 1;
             ++rounds;
         }
         return n;
@@ -485,6 +526,11 @@ class FusedScheduler {
 // dispatch and exchanges; a pass cannot beat its memory time.
 inline double fused_pass_cost(const FusedPass& ps, const FusedGeom& G = GEOM_F32) {
     const int g = ps.gate_end - ps.gate_begin, x = ps.n_phases > 1 ? ps.n_phases - 1 : 0;
+    if (G.kind == 3 || G.kind == 4) {            // Z2: the kind-0 / kind-1 pass over half the elements
+        FusedPass q = ps;
+        return 0.5 * fused_pass_cost(q, G.kind == 3 ? GEOM_F32 : GEOM_COUNT);
+    }
+    if (G.kind == 5) { FusedPass q = ps; return 0.5 * fused_pass_cost(q, GEOM_I16); }
     if (G.kind == 2) {
         // Tropical<i16>: half the bytes and half the alu work per element; tiles whose 9 active
         // word digits reach past bit 18 (> 256 pages of 2 MiB) are bound by address translation
@@ -629,12 +675,17 @@ inline std::string describe_fused(const FusedPlan& p) {
                 case MC_END: out += "m end\n"; break;
                 case MC_FINAL: out += "m final\n"; break;
                 case MC_ROUND: {
-                    snprintf(line, sizeof line, "m round mask=%d first=%d\n", m.mask, m.arg);
+                    snprintf(line, sizeof line, "m round mask=%d first=%d flip=%d\n", m.mask, m.arg & ~MOP_FLIP, (m.arg & MOP_FLIP) ? 1 : 0);
                     out += line;
-                    int g = ps.gate_begin + m.arg;
+                    int g = ps.gate_begin + (m.arg & ~MOP_FLIP);
                     for (int b = 0; b < 8; ++b) if (m.mask >> b & 1) {
                         const int rc = p.gate_rc[g++];
                         snprintf(line, sizeof line, "g k=%d r=%d c=%d layout=%d\n", (rc >> 13) & 7, (rc >> 6) & 63, rc & 63, (rc >> 12) & 1);
+                        out += line;
+                    }
+                    if (m.arg & MOP_FLIP) {
+                        const int rc = p.gate_rc[g++];
+                        snprintf(line, sizeof line, "g k=-1 r=%d c=%d layout=%d\n", (rc >> 6) & 63, rc & 63, (rc >> 12) & 1);
                         out += line;
                     }
                     break; }

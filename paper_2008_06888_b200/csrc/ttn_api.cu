@@ -50,15 +50,42 @@ unsigned long long ipow(int q, int e) {
     return r;
 }
 
+// Test / debug switches (environment TTN_DEBUG_*).  They are read ONCE per entry point
+// (ttn_workspace_bytes, ttn_plan_describe, ttn_plan_create, the chimera call) into this struct; a
+// plan keeps the snapshot it was created with, and no launch path calls getenv.  The tests use them
+// to force small tiles, the generic kernels or the fallbacks of the specialised paths.
+struct DebugCfg {
+    int tmax = -1, ride = -1;     // TTN_DEBUG_TMAX / _RIDE: smaller generic tiles (multi-pass plans on tiny lattices)
+    int fused = 1;                // TTN_DEBUG_FUSED=0: generic tile kernels instead of the fused register kernels
+    int z2 = 1;                   // TTN_DEBUG_Z2=0: never use the global-flip reduction (h = 0)
+    int nobeam = 0, nb = -1;      // Potts: TTN_DEBUG_NOBEAM, TTN_DEBUG_NB (gate-block size)
+    int nolowpf = 0, nogroup = 0, nosweep = 0;   // ground_config forward: no LOW prefetch / instance groups / one-launch sweep
+    int bt_multi = 0;             // backward pass: one launch pair per row even for batches of small lattices
+    int timing = 0;               // per-pass device times on stderr
+    int ch_persm = 512, ch_nocell0 = 0;          // chimera: CTAs per SM, generic kernel for the r = 0 cells
+};
+DebugCfg read_debug() {
+    DebugCfg d;
+    auto geti = [](const char* name, int& v) { if (const char* e = getenv(name)) v = atoi(e); };
+    auto flag = [](const char* name, int& v) { v = getenv(name) != nullptr; };
+    geti("TTN_DEBUG_TMAX", d.tmax); geti("TTN_DEBUG_RIDE", d.ride); geti("TTN_DEBUG_FUSED", d.fused);
+    geti("TTN_DEBUG_Z2", d.z2); geti("TTN_DEBUG_NB", d.nb); geti("TTN_DEBUG_CH_PERSM", d.ch_persm);
+    flag("TTN_DEBUG_NOBEAM", d.nobeam); flag("TTN_DEBUG_NOLOWPF", d.nolowpf); flag("TTN_DEBUG_NOGROUP", d.nogroup);
+    flag("TTN_DEBUG_NOSWEEP", d.nosweep); flag("TTN_DEBUG_BT_MULTI", d.bt_multi); flag("TTN_DEBUG_TIMING", d.timing);
+    flag("TTN_DEBUG_CH_NOCELL0", d.ch_nocell0);
+    if (d.ch_persm < 1) d.ch_persm = 512;
+    return d;
+}
+
 // Tile capacity (log_q of elements per CTA tile) and riding digits of the generic path.
 struct TileCfg { int Tmax, ride; };
-TileCfg tile_cfg(int q, bool count) {
+TileCfg tile_cfg(int q, bool count, const DebugCfg& dbg) {
     TileCfg t;
     if (q == 2) t = count ? TileCfg{13, 3} : TileCfg{14, 3};   // 96 KiB / 64 KiB of smem
     else t = count ? TileCfg{8, 2} : TileCfg{9, 2};           // 3^8*12 = 77 KiB / 3^9*4 = 77 KiB
     // Debug/test override (smaller tiles only): lets tiny lattices exercise multi-pass schedules.
-    if (const char* e = getenv("TTN_DEBUG_TMAX")) { int v = atoi(e); if (v >= 2 && v <= t.Tmax) t.Tmax = v; }
-    if (const char* e = getenv("TTN_DEBUG_RIDE")) { int v = atoi(e); if (v >= 0 && v < t.Tmax) t.ride = v; }
+    if (dbg.tmax >= 2 && dbg.tmax <= t.Tmax) t.Tmax = dbg.tmax;
+    if (dbg.ride >= 0 && dbg.ride < t.Tmax) t.ride = dbg.ride;
     if (t.ride >= t.Tmax) t.ride = t.Tmax - 1;
     return t;
 }
@@ -84,24 +111,30 @@ struct Layout {
 
 // The fused register-phase paths: Ising Tropical<f32> energy for L >= 12 (ttn_fused.cuh) and Ising
 // CountingTropical<f32,f64> for L >= 10 (ttn_fcount.cuh).
-bool i16_eligible(int q, int L) {
-    if (const char* e = getenv("TTN_DEBUG_FUSED")) if (atoi(e) == 0) return false;
-    return q == 2 && L >= ttn::GEOM_I16.WLOW;
+bool i16_eligible(int q, int L, const DebugCfg& dbg) {
+    return dbg.fused != 0 && q == 2 && L >= ttn::GEOM_I16.WLOW;
 }
-bool fused_eligible(int q, int L, bool count, bool config) {
-    if (const char* e = getenv("TTN_DEBUG_FUSED")) if (atoi(e) == 0) return false;
-    if (q != 2) return false;
+bool fused_eligible(int q, int L, bool count, bool config, const DebugCfg& dbg) {
+    if (dbg.fused == 0 || q != 2) return false;
     return count ? L >= ttn::CW_LOW : L >= ttn::F_WLOW;      // config: row-aligned f32 plan
+}
+// Global-flip (Z2) reduction (planner.h): h = 0 only; the half-state must span at least two LOW tiles
+// (a tile and its complement).  Geometry of the call, or nullptr.
+const ttn::FusedGeom* z2_geom(int q, int L, ttn_call call, bool has_field, const DebugCfg& dbg) {
+    if (dbg.fused == 0 || dbg.z2 == 0 || q != 2 || has_field) return nullptr;
+    if ((call == TTN_CALL_ENERGY || call == TTN_CALL_ENERGY_Z2) && L >= ttn::GEOM_F32_Z2.WLOW + 1) return &ttn::GEOM_F32_Z2;
+    return nullptr;
 }
 
 // The op list of a plan holds the L(L-1) gates of the sweep (diagonal frame: no diagonal op).
-Layout make_layout(int q, int L, bool count, bool config, int batch, bool i16 = false) {
+// z2: the stored state is the half with column 0 up: q^(L-1) elements (every size below follows NS)
+Layout make_layout(int q, int L, bool count, bool config, int batch, const DebugCfg& dbg, bool i16 = false, bool z2 = false) {
     Layout y;
-    y.NS = ipow(q, L);
-    const TileCfg tc = tile_cfg(q, count);
+    y.NS = ipow(q, z2 ? L - 1 : L);
+    const TileCfg tc = tile_cfg(q, count, dbg);
     // every pass of a plan stages tiles of q^min(L, Tmax) elements
     y.max_tiles = y.NS / ipow(q, tc.Tmax < L ? tc.Tmax : L);
-    if (fused_eligible(q, L, count, config) && y.max_tiles < 1024) y.max_tiles = 1024;   // one partial per CTA
+    if (fused_eligible(q, L, count, config, dbg) && y.max_tiles < 1024) y.max_tiles = 1024;   // one partial per CTA
     if (y.max_tiles == 0) y.max_tiles = 1;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
@@ -124,7 +157,7 @@ Layout make_layout(int q, int L, bool count, bool config, int batch, bool i16 = 
     y.out_n = take((size_t)batch * 8);
     y.out_s = take((size_t)batch * 8);
     y.sigma = take((size_t)batch * L * L);
-    if (fused_eligible(q, L, count, config)) {
+    if (fused_eligible(q, L, count, config, dbg)) {
         y.f_max_gates = L * L; y.f_max_mops = 4 * L * L + 64;
         y.f_mops = take((size_t)y.f_max_mops * sizeof(ttn::MicroOp));
         y.f_gate_rc = take((size_t)y.f_max_gates * 4);
@@ -151,7 +184,10 @@ struct ttn_plan {
     ttn::Plan plan;
     ttn::FusedPlan fplan;
     bool fused = false, i16 = false;
+    bool z2 = false;               // global-flip reduction: the state is the half with column 0 up (h = 0)
+    DebugCfg dbg;                  // the debug switches as they were when the plan was created
     int fused_grid = 0;
+    int sms = 0;
     int sweep_grid = 0;             // > 0: fused_sweep_kernel runs every pass in one launch (table at lay.f_sweep)
     std::vector<ttn::FusedParams> sweep_params;
     Layout lay;
@@ -160,11 +196,13 @@ struct ttn_plan {
     int launches;
 };
 
-static ttn::Plan plan_for(int q, int L, ttn_call call, bool has_field) {
+static ttn::Plan plan_for(int q, int L, ttn_call call, bool has_field, const DebugCfg& dbg) {
     const bool count = (call == TTN_CALL_COUNT);
-    const TileCfg tc = tile_cfg(q, count);
+    const TileCfg tc = tile_cfg(q, count, dbg);
     ttn::Plan p = ttn::make_plan(q, L, has_field, call == TTN_CALL_CONFIG, tc.Tmax, tc.ride);
-    if (q == 3 && L > tc.Tmax && !getenv("TTN_DEBUG_NOBEAM")) {       // multi-pass Potts sweep: search the tile order
+    if (q == 3 && L > tc.Tmax && !dbg.nobeam) {       // multi-pass Potts sweep: search the tile order
+        // The one piece of process-wide state in the library: a memo of beam-searched Potts schedules
+        // (a pure function of (L, Tmax, ride), ~1 s to compute at L = 18), guarded by a mutex.
         static std::map<std::tuple<int, int, int>, ttn::Plan> cache;
         static std::mutex mu;
         std::lock_guard<std::mutex> lock(mu);
@@ -175,7 +213,7 @@ static ttn::Plan plan_for(int q, int L, ttn_call call, bool has_field) {
     }
     if (q == 3) {
         int max_nb = count ? ttn::POTTS_MAX_NB_COUNT : 3;
-        if (const char* e = getenv("TTN_DEBUG_NB")) { int v = atoi(e); if (v >= 1 && v <= max_nb) max_nb = v; }
+        if (dbg.nb >= 1 && dbg.nb <= max_nb) max_nb = dbg.nb;
         ttn::mark_gate_blocks(p, max_nb);
     }
     return p;
@@ -214,8 +252,7 @@ static ttn_status launch_pass(const ttn_plan* P, const ttn::Pass& ps, cudaStream
         // persistent CTAs, two residents per SM (ttn_potts.cuh)
         if (pp.n_ops > ttn::POTTS_MAX_OPS) return fail(TTN_EUNSUPPORTED, "too many gates in one Potts pass");
         if (pp.T > 9) return fail(TTN_EUNSUPPORTED, "Potts tiles hold at most 3^9 elements");
-        static int sms = 0;
-        if (!sms) { int dev = 0; TTN_CUDA(cudaGetDevice(&dev)); TTN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)); }
+        const int sms = P->sms;                         // of the device the plan was created on
         const unsigned ctas = grid < 2ull * sms ? (unsigned)grid : 2u * (unsigned)sms;
         const size_t psmem = ttn::potts_buf_bytes(pp.n_tile, COUNT);
         ttn_status s = TTN_OK;
@@ -267,6 +304,8 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
         pp.L = P->L - 1; pp.a = ps.low ? 0 : ps.a - 1;
         pp.inst_stride = y.NS >> 1; pp.tiles_per_inst = y.NS >> 13;
         pp.src = pp.state; pp.src_stride = pp.inst_stride;
+    } else if (P->z2) {     // the kernel sees the half-state over columns 1 .. L-1: column c = digit c - 1
+        pp.L = P->L - 1; pp.a = ps.low ? 0 : ps.a - 1;
     }
     const int a_mem = pp.a;
     pp.mops = reinterpret_cast<const ttn::MicroOp*>(P->ws + y.f_mops) + ps.mop_begin;
@@ -292,10 +331,10 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
         if (grid > need) grid = need;
     }
     pp.part_stride = pp.cta_per_inst ? 1 : (int)grid;
-    if (ps.low && getenv("TTN_DEBUG_NOLOWPF")) pp.prefetch_pc = -1;
+    if (ps.low && P->dbg.nolowpf) pp.prefetch_pc = -1;
     pp.igroup = 1;
     { int sh = 0; while ((1ull << sh) < pp.tiles_per_inst) ++sh; pp.tpi_shift = sh; }
-    if (pp.cta_per_inst && !P->i16 && !(ps.flags & ttn::PASS_REDUCE) && !getenv("TTN_DEBUG_NOGROUP")) {
+    if (pp.cta_per_inst && !P->i16 && !P->z2 && !(ps.flags & ttn::PASS_REDUCE) && !P->dbg.nogroup) {
         // instances per CTA at a time: fewest rounds of the 12 warps (HIGH: of the 3 warp groups) over
         // the flat tile list of K instances, times the rounds of CTA groups over the grid
         const unsigned long long tpi = pp.tiles_per_inst, slots = ps.low ? (unsigned long long)nw : (unsigned long long)(nw / 4);
@@ -331,6 +370,9 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
         if (P->i16) {
             if (ps.low) { if (red) TTN_FUSED_LAUNCH(true, 1, true); else TTN_FUSED_LAUNCH(true, 1, false); }
             else { if (red) TTN_FUSED_LAUNCH(false, 1, true); else TTN_FUSED_LAUNCH(false, 1, false); }
+        } else if (P->z2 && ps.low) {      // warp pairs on complementary tiles, flip gates
+            if (red) ttn::fused_pass_kernel<true, 0, false, true, true><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(true), st>>>(pp);
+            else ttn::fused_pass_kernel<true, 0, false, false, true><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(true), st>>>(pp);
         } else {
             if (ps.low) { if (red) TTN_FUSED_LAUNCH(true, 0, true); else TTN_FUSED_LAUNCH(true, 0, false); }
             else { if (red) TTN_FUSED_LAUNCH(false, 0, true); else TTN_FUSED_LAUNCH(false, 0, false); }
@@ -447,7 +489,8 @@ static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
     q.final_tab = reinterpret_cast<float*>(P->ws + y.f_final);
     const ttn::FusedPass& lastp = fp.passes.back();
     q.fin_low = lastp.low; q.fin_layout = lastp.last_layout; q.fin_a = lastp.a;
-    if (P->i16) q.fin_a = lastp.low ? 0 : lastp.a - 1;                 // word digit
+    if (P->i16 || P->z2) q.fin_a = lastp.low ? 0 : lastp.a - 1;        // word digit / half-state digit
+    q.col_off = P->z2 ? 1 : 0;
     long work = ttn::FFINAL_FLOATS; if (q.n_gates > work) work = q.n_gates;
     dim3 grid((unsigned)((work + 255) / 256), (unsigned)P->batch);
     if (P->i16) {
@@ -465,6 +508,8 @@ static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
     TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 0, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
     TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false, 0, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));
     TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false, 0, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 0, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 0, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
     TTN_CUDA(cudaFuncSetAttribute(ttn::fused_sweep_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
     TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true)));
     TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false)));
@@ -480,8 +525,8 @@ static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
 }
 
 // batches of small lattices walk all checkpoints of an instance in one CTA (backtrace_inst_kernel)
-static bool backtrace_one_cta(int L, int batch) {
-    return L <= 18 && L <= ttn::BT_MAX_L && batch >= 32 && !getenv("TTN_DEBUG_BT_MULTI");
+static bool backtrace_one_cta(int L, int batch, const DebugCfg& dbg) {
+    return L <= 18 && L <= ttn::BT_MAX_L && batch >= 32 && !dbg.bt_multi;
 }
 
 static ttn_status launch_backtrace(ttn_plan* P, cudaStream_t st) {
@@ -498,7 +543,7 @@ static ttn_status launch_backtrace(ttn_plan* P, cudaStream_t st) {
         ap.part_s = reinterpret_cast<unsigned long long*>(P->ws + y.amax_s);
         ap.v_out = reinterpret_cast<float*>(P->ws + y.out_x);
         ap.sigma = reinterpret_cast<signed char*>(P->ws + y.sigma);
-        if (backtrace_one_cta(P->L, P->batch)) {
+        if (backtrace_one_cta(P->L, P->batch, P->dbg)) {
             // batches of small lattices: one CTA walks all L checkpoints of its instance
             ap.C = reinterpret_cast<const float*>(P->ws + y.ckpt);
             ttn::backtrace_inst_kernel<<<P->batch, ttn::BT_THREADS, 0, st>>>(ap);
@@ -528,25 +573,35 @@ size_t ttn_workspace_bytes(int q, int L, ttn_semiring mode, int batch, int want_
         (mode != TTN_TROPICAL_F32 && mode != TTN_COUNTING_F32_F64 && mode != TTN_TROPICAL_I16)) return 0;
     if (mode == TTN_TROPICAL_I16 && (q != 2 || want_config)) return 0;
     if (!limits_ok(q, L, count, want_config != 0)) return 0;
-    return make_layout(q, L, count, want_config != 0, batch, mode == TTN_TROPICAL_I16 && i16_eligible(q, L)).total;
+    const DebugCfg dbg = read_debug();
+    // (with h = 0 the calls may store the flip-reduced half-state: every field is then smaller)
+    return make_layout(q, L, count, want_config != 0, batch, dbg, mode == TTN_TROPICAL_I16 && i16_eligible(q, L, dbg)).total;
 }
 
 long ttn_plan_describe(int q, int L, ttn_call call, char* buf, size_t n) {
     if ((q != 2 && q != 3) || !buf || n == 0) return -1;
     if (!limits_ok(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) return -1;
     std::string s;
-    if (call == TTN_CALL_ENERGY_I16 && i16_eligible(q, L)) {
+    const DebugCfg dbg = read_debug();
+    if (call == TTN_CALL_ENERGY_Z2) {              // the schedule ttn_sweep_energy runs when h = 0
+        if (const ttn::FusedGeom* G = z2_geom(q, L, call, false, dbg)) {
+            ttn::FusedPlan fp = ttn::make_fused_plan(L, ttn::FMAX_GATES, *G);
+            if (fp.ok) s = ttn::describe_fused(fp);
+        }
+        if (s.empty()) call = TTN_CALL_ENERGY;
+    }
+    if (call == TTN_CALL_ENERGY_I16 && i16_eligible(q, L, dbg)) {
         ttn::FusedPlan fp = ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_I16);
         if (fp.ok) s = ttn::describe_fused(fp);
     }
     if (call == TTN_CALL_ENERGY_I16 && s.empty()) call = TTN_CALL_ENERGY;
-    if (s.empty() && fused_eligible(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) {
+    if (s.empty() && fused_eligible(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG, dbg)) {
         ttn::FusedPlan fp = call == TTN_CALL_COUNT ? ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_COUNT)
                           : call == TTN_CALL_CONFIG ? ttn::make_fused_row_plan(L, ttn::FMAX_GATES)
                                                     : ttn::make_fused_plan(L, ttn::FMAX_GATES);
         if (fp.ok) s = ttn::describe_fused(fp);
     }
-    if (s.empty()) s = ttn::describe(plan_for(q, L, call, /*has_field=*/q == 2));
+    if (s.empty()) s = ttn::describe(plan_for(q, L, call, /*has_field=*/q == 2, dbg));
     size_t m = s.size() < n - 1 ? s.size() : n - 1;
     memcpy(buf, s.data(), m);
     buf[m] = 0;
@@ -560,13 +615,16 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     *out = nullptr;
     if (q != 2 && q != 3) return fail(TTN_EINVAL, "q must be 2 or 3");
     if (L < 1 || batch < 1) return fail(TTN_EINVAL, "L and batch must be >= 1");
-    if (call != TTN_CALL_ENERGY && call != TTN_CALL_COUNT && call != TTN_CALL_CONFIG && call != TTN_CALL_ENERGY_I16)
+    if (call != TTN_CALL_ENERGY && call != TTN_CALL_COUNT && call != TTN_CALL_CONFIG && call != TTN_CALL_ENERGY_I16 &&
+        call != TTN_CALL_ENERGY_Z2)
         return fail(TTN_EINVAL, "bad call kind");
+    const DebugCfg dbg = read_debug();
     bool i16 = false;
     if (call == TTN_CALL_ENERGY_I16) {
         if (q != 2) return fail(TTN_EINVAL, "Tropical<i16> is an Ising call");
-        i16 = i16_eligible(q, L);           // small lattices run the f32 path (identical results)
+        i16 = i16_eligible(q, L, dbg);      // small lattices run the f32 path (identical results)
     }
+    if (call == TTN_CALL_ENERGY_Z2 && q != 2) return fail(TTN_EINVAL, "the flip reduction is an Ising call");
     if (L > 1 && (!Jh || !Jv)) return fail(TTN_EINVAL, "Jh/Jv is NULL");
     if (!workspace) return fail(TTN_EINVAL, "workspace is NULL");
     if (q == 3 && h) return fail(TTN_EINVAL, "the Potts variant takes no fields");
@@ -591,7 +649,13 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
             if (tot > 8000.0) return fail(TTN_EINVAL, "Tropical<i16>: sum of |couplings| = %.0f > 8000 (instance %d)", tot, b);
         }
     }
-    Layout lay = make_layout(q, L, count, config, batch, i16);
+    // h = NULL or all zero: Eq. (1) PAPER.md:29 is invariant under the global flip -> half-state (planner.h)
+    bool field = false;
+    if (h) for (size_t i = 0; i < nf && !field; ++i) field = (h[i] != 0.0f);
+    if (call == TTN_CALL_ENERGY_Z2 && field) return fail(TTN_EINVAL, "the flip reduction needs h = 0");
+    const ttn::FusedGeom* zg = z2_geom(q, L, call, field, dbg);
+    if (call == TTN_CALL_ENERGY_Z2) call = TTN_CALL_ENERGY;       // lattices too small for it run the plain sweep
+    Layout lay = make_layout(q, L, count, config, batch, dbg, i16, zg != nullptr);
     if (workspace_bytes < lay.total)
         return fail(TTN_ENOMEM, "workspace too small: %zu < %zu", workspace_bytes, lay.total);
     if ((uintptr_t)workspace % 256) return fail(TTN_EINVAL, "workspace must be 256-byte aligned");
@@ -604,20 +668,30 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     ttn_plan* P = new (std::nothrow) ttn_plan();
     if (!P) return fail(TTN_ENOMEM, "host allocation failed");
     P->q = q; P->L = L; P->batch = batch; P->call = call; P->count = count; P->config = config;
-    P->has_field = (h != nullptr);
+    P->has_field = (h != nullptr) && zg == nullptr;
     P->i16 = i16;
+    P->z2 = zg != nullptr;
+    P->dbg = dbg;
     P->lay = lay;
+    {
+        cudaError_t ce = cudaDeviceGetAttribute(&P->sms, cudaDevAttrMultiProcessorCount, dev);
+        if (ce != cudaSuccess) { delete P; return fail(TTN_ECUDA, "cudaDeviceGetAttribute failed: %s", cudaGetErrorString(ce)); }
+    }
     P->ws = static_cast<unsigned char*>(workspace);
     if (i16) {
         P->fplan = ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_I16);
         P->fused = P->fplan.ok;
         if (!P->fused) { delete P; return fail(TTN_EUNSUPPORTED, "no Tropical<i16> schedule"); }
-    } else if (fused_eligible(q, L, count, config)) {
+    } else if (zg) {
+        P->fplan = ttn::make_fused_plan(L, ttn::FMAX_GATES, *zg);
+        P->fused = P->fplan.ok;
+        if (!P->fused) { delete P; return fail(TTN_EUNSUPPORTED, "no flip-reduced schedule"); }
+    } else if (fused_eligible(q, L, count, config, dbg)) {
         P->fplan = count ? ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_COUNT)
                  : config ? ttn::make_fused_row_plan(L, ttn::FMAX_GATES) : ttn::make_fused_plan(L, ttn::FMAX_GATES);
         P->fused = P->fplan.ok;
     }
-    if (!P->fused) P->plan = plan_for(q, L, call, P->has_field);
+    if (!P->fused) P->plan = plan_for(q, L, call, P->has_field, dbg);
     if (!P->fused && P->plan.passes.empty()) { delete P; return fail(TTN_EUNSUPPORTED, "planner produced no schedule"); }
     if (P->plan.ops.size() > (size_t)(L * L + 8)) { delete P; return fail(TTN_EUNSUPPORTED, "op list too long"); }
 
@@ -644,8 +718,8 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     if (P->fused) {
         ttn_status fs = count ? setup_fcount(P, st) : setup_fused(P, st);
         if (fs != TTN_OK) { delete P; return fs; }
-        P->launches = (int)P->fplan.passes.size() + (config ? (backtrace_one_cta(L, batch) ? 1 : 2 * L) : 1);
-        if (config && !count && !P->i16 && !getenv("TTN_DEBUG_NOSWEEP") && P->fplan.passes.size() <= (size_t)(4 * L + 8)) {
+        P->launches = (int)P->fplan.passes.size() + (config ? (backtrace_one_cta(L, batch, dbg) ? 1 : 2 * L) : 1);
+        if (config && !count && !P->i16 && !dbg.nosweep && P->fplan.passes.size() <= (size_t)(4 * L + 8)) {
             // every pass in cta_per_inst mode: the pass table of fused_sweep_kernel (two instances per
             // CTA at a time where the constants of every pass fit, else one)
             std::vector<ttn::FusedParams> v(P->fplan.passes.size());
@@ -661,7 +735,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
                 cudaError_t ce = cudaMemcpyAsync(P->ws + lay.f_sweep, P->sweep_params.data(), v.size() * sizeof(ttn::FusedParams),
                                                  cudaMemcpyHostToDevice, st);
                 if (ce != cudaSuccess) { delete P; return fail(TTN_ECUDA, "pass table upload failed: %s", cudaGetErrorString(ce)); }
-                P->launches = 1 + (backtrace_one_cta(L, batch) ? 1 : 2 * L);
+                P->launches = 1 + (backtrace_one_cta(L, batch, dbg) ? 1 : 2 * L);
             }
         }
     } else {
@@ -677,7 +751,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
         ttn::generic_prep_kernel<<<dim3((unsigned)((work + 255) / 256), (unsigned)batch), 256, 0, st>>>(gp);
         cudaError_t pe = cudaGetLastError();
         if (pe != cudaSuccess) { delete P; return fail(TTN_ECUDA, "prep launch failed: %s", cudaGetErrorString(pe)); }
-        P->launches = (int)P->plan.passes.size() + (config ? (backtrace_one_cta(L, batch) ? 1 : 2 * L) : 1);
+        P->launches = (int)P->plan.passes.size() + (config ? (backtrace_one_cta(L, batch, dbg) ? 1 : 2 * L) : 1);
     }
     *out = P;
     return TTN_OK;
@@ -687,7 +761,7 @@ ttn_status ttn_plan_launch(ttn_plan* P, void* stream) {
     if (!P) return fail(TTN_EINVAL, "plan is NULL");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if (P->fused) {
-        const bool timing = getenv("TTN_DEBUG_TIMING") != nullptr;     // per-pass device times on stderr
+        const bool timing = P->dbg.timing != 0;                        // per-pass device times on stderr
         std::vector<cudaEvent_t> ev;
         if (timing) { ev.resize(P->fplan.passes.size() + 1); for (auto& e : ev) cudaEventCreate(&e); cudaEventRecord(ev[0], st); }
         // batches of small lattices, no reduction pass (ttn_ground_config): all passes in one launch
@@ -716,7 +790,7 @@ ttn_status ttn_plan_launch(ttn_plan* P, void* stream) {
         if (P->config) return launch_backtrace(P, st);
         return TTN_OK;
     }
-    const bool gtiming = getenv("TTN_DEBUG_TIMING") != nullptr;      // per-pass device times on stderr
+    const bool gtiming = P->dbg.timing != 0;                         // per-pass device times on stderr
     std::vector<cudaEvent_t> gev;
     if (gtiming) { gev.resize(P->plan.passes.size() + 1); for (auto& e : gev) cudaEventCreate(&e); cudaEventRecord(gev[0], st); }
     size_t gk = 0;
@@ -765,6 +839,7 @@ ttn_status ttn_plan_read(ttn_plan* P, void* stream, double* E0, double* degenera
 void ttn_plan_destroy(ttn_plan* P) { delete P; }
 int ttn_plan_num_launches(const ttn_plan* P) { return P ? P->launches : 0; }
 int ttn_plan_num_passes(const ttn_plan* P) { return P ? (int)(P->fused ? P->fplan.passes.size() : P->plan.passes.size()) : 0; }
+unsigned long long ttn_plan_state_elements(const ttn_plan* P) { return P ? P->lay.NS : 0ull; }
 
 }  // extern "C"
 
@@ -822,6 +897,8 @@ ttn_status ttn_chimera_sweep_energy_i16(int M, int N, const float* K, const floa
     if (M > 8 || N > 64) return fail(TTN_EUNSUPPORTED, "chimera: M <= 8 rows of cells (state 2^(4M+4) int16), N <= 64");
     const size_t need = ttn_chimera_workspace_bytes(M, N);
     if (wsb < need) return fail(TTN_ENOMEM, "workspace too small: %zu < %zu", wsb, need);
+    if ((uintptr_t)ws % 256) return fail(TTN_EINVAL, "workspace must be 256-byte aligned");
+    const DebugCfg dbg = read_debug();
     // integer-valued couplings whose absolute sum fits 16 bits with room (as ttn_sweep_energy_i16)
     double total = 0;
     auto scan = [&](const float* a, size_t n) {
@@ -873,10 +950,12 @@ ttn_status ttn_chimera_sweep_energy_i16(int M, int N, const float* K, const floa
     {   // a CTA walks its groups with the stride of the grid; 512 CTAs per SM measured best at 8 x 8
         // cells (per SM 8 / 32 / 64 / 128 / 512 CTAs: 3.27 / 3.24 / 3.19 / 3.15 / 3.12 s; one group per
         // thread, i.e. 2^23 CTAs: 3.61 s)
-        int dev = 0, sms = 0, per_sm = 512;
+        int dev = 0, sms = 0, major = 0;
+        const int per_sm = dbg.ch_persm;
         TTN_CUDA(cudaGetDevice(&dev));
+        TTN_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+        if (major != 10) return fail(TTN_EUNSUPPORTED, "device compute capability %d.x is not sm_100", major);
         TTN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-        if (const char* e = getenv("TTN_DEBUG_CH_PERSM")) { int v = atoi(e); if (v >= 1) per_sm = v; }
         const unsigned long long cap = (unsigned long long)sms * (unsigned long long)per_sm;
         if (blocks > cap) blocks = cap;
     }
@@ -887,7 +966,7 @@ ttn_status ttn_chimera_sweep_energy_i16(int M, int N, const float* K, const floa
             for (int l = 0; l < 4; ++l) q.ju[l] = c > 0 ? pack(Jh[((size_t)r * (N - 1) + (c - 1)) * 4 + l]) : 0u;
             for (int k = 0; k < 4; ++k) q.jv[k] = r > 0 ? pack(Jv[((size_t)(r - 1) * N + c) * 4 + k]) : 0u;
             q.table = tables + ((size_t)r * N + c) * 128;
-            if (r == 0 && q.groups >= 32 && !getenv("TTN_DEBUG_CH_NOCELL0")) {
+            if (r == 0 && q.groups >= 32 && !dbg.ch_nocell0) {
                 const unsigned long long tiles = q.groups >> 5, wpb = ttn::CH_THREADS / 32;
                 const unsigned long long b0 = (tiles + wpb - 1) / wpb;
                 ttn::chimera_cell0_kernel<<<(unsigned)(b0 < blocks ? b0 : blocks), ttn::CH_THREADS, 0, st>>>(q);

@@ -203,6 +203,62 @@ __device__ __forceinline__ void fround(float (&v)[128], const unsigned mask, con
 #undef TTN_G
 }
 
+// ---- Z2 flip gate (h = 0; planner.h "GLOBAL-FLIP (Z2) REDUCTION") -------------------------------------
+// The stored half-state obeys W[s_0 = 1, u] = W[s_0 = 0, ~u], so the gate (A2) on column 0 reads
+//     W'[u] = max(W[u], W[~u] + kf[bit of column 1 in u]).
+// ~u lives in the complement tile, which the partner warp (warp ^ 1) of the pair holds in the same
+// layout: both warps publish their registers in their own exchange region (the store half of an
+// exchange), meet at the pair's named barrier, and read the partner's region at the complemented
+// position -- register 127 - j of lane 31 - lane -- which mirrors the load half of the exchange and
+// is bank-conflict free for the same reason.  A second barrier frees the regions.
+__device__ __forceinline__ void pair_sync(int warp) {
+    asm volatile("bar.sync %0, 64;" :: "r"(1 + (warp >> 1)) : "memory");
+}
+__host__ __device__ constexpr int rev5c(int q) {
+    return ((q & 1) << 4) | ((q & 2) << 2) | (q & 4) | ((q & 8) >> 2) | ((q & 16) >> 4);
+}
+template <int LAYOUT>
+__device__ __forceinline__ void flipgate(float (&v)[128], float4* myreg, const float4* preg, const int lane,
+                                         const int warp, const float k0, const float k1) {
+    __syncwarp();
+    if (LAYOUT == 0) {
+        float4* p = myreg + 33 * lane;
+#pragma unroll
+        for (int q = 0; q < 32; ++q) p[q] = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+    } else {
+        float4* p = myreg + lane;
+#pragma unroll
+        for (int q = 0; q < 32; ++q) p[33 * rev5c(q)] = make_float4(v[4 * q], v[4 * q + 2], v[4 * q + 1], v[4 * q + 3]);
+    }
+    pair_sync(warp);
+    if (LAYOUT == 0) {          // column 1 = tile digit 0 = register bit 2 = bit 0 of the quad index
+        const float4* p = preg + 33 * (31 - lane);
+#pragma unroll
+        for (int q = 0; q < 32; ++q) {
+            const float4 t = p[31 - q];
+            const float kq = (q & 1) ? k1 : k0;
+            float a0, a1, a2, a3;
+            add2(a0, a1, t.w, t.z, kq, kq);
+            add2(a2, a3, t.y, t.x, kq, kq);
+            v[4 * q] = fmaxf(v[4 * q], a0); v[4 * q + 1] = fmaxf(v[4 * q + 1], a1);
+            v[4 * q + 2] = fmaxf(v[4 * q + 2], a2); v[4 * q + 3] = fmaxf(v[4 * q + 3], a3);
+        }
+    } else {                    // column 1 = lane bit 0
+        const float4* p = preg + (31 - lane);
+        const float kk = (lane & 1) ? k1 : k0;
+#pragma unroll
+        for (int q = 0; q < 32; ++q) {
+            const float4 t = p[33 * rev5c(31 - q)];
+            float a0, a1, a2, a3;
+            add2(a0, a1, t.w, t.y, kk, kk);
+            add2(a2, a3, t.z, t.x, kk, kk);
+            v[4 * q] = fmaxf(v[4 * q], a0); v[4 * q + 1] = fmaxf(v[4 * q + 1], a1);
+            v[4 * q + 2] = fmaxf(v[4 * q + 2], a2); v[4 * q + 3] = fmaxf(v[4 * q + 3], a3);
+        }
+    }
+    pair_sync(warp);
+}
+
 // ---- Tropical<i16> (the paper's own Int16 choice for +-J) -----------
 // Two elements per 32-bit word: column 0 of the lattice row is the HALF of a word (low half =
 // bit 0 = sigma +1), the kernel's tile geometry applies to the word index.  One VIADDMNMX.S16x2
@@ -462,11 +518,14 @@ template <bool LOW, int ELEM, bool GROUP>
 __device__ __forceinline__ void fused_pass_body(const FusedParams& p, unsigned char* fsm_raw,
                                                 const int inst_first, const int inst_step) {
     constexpr bool RED = false;          // GROUP passes never reduce
+    constexpr bool Z2 = false;
 #include "ttn_fused_body.inc"
 }
 
 // RED = the last pass of a sweep (adds A_{L-1}(s) and reduces instead of storing)
-template <bool LOW, int ELEM = 0, bool GROUP = false, bool RED = false>
+// Z2 (LOW only) = the flip-reduced state: warps work in pairs on tiles (T, ~T) and the program may
+// contain flip gates (planner.h "GLOBAL-FLIP (Z2) REDUCTION")
+template <bool LOW, int ELEM = 0, bool GROUP = false, bool RED = false, bool Z2 = false>
 __global__ void __launch_bounds__(fwarps(LOW, ELEM) * 32, 1) fused_pass_kernel(const FusedParams p) {
     extern __shared__ __align__(16) unsigned char fsm_raw[];
     const int inst_first = p.cta_per_inst ? (int)blockIdx.x * (GROUP ? p.igroup : 1) : 0;
@@ -506,6 +565,7 @@ struct FusedPrepParams {
     float* gate_k;                 // [inst][n_gates][8]
     float* final_tab;              // [inst][FFINAL_FLOATS]
     int fin_low, fin_layout, fin_a;   // tile kind, layout and start column of the last pass's end
+    int col_off;                   // Z2: 1 = the kernel's digit d is lattice column d + 1 (fin_a is a digit)
 };
 
 __global__ void __launch_bounds__(256) fused_prep_kernel(const FusedPrepParams p) {
@@ -524,24 +584,29 @@ __global__ void __launch_bounds__(256) fused_prep_kernel(const FusedPrepParams p
         const double m = -2.0 * (double)Jv[(r - 1) * L + c];
         const double H = Hacc(r, c), Kl = Kacc(r, c - 1), Kr = Kacc(r, c);
         float* out = p.gate_k + (inst * p.n_gates + idx) * 8;
-        // k[side][P bit][Q bit]: P = left neighbour in layout A, right neighbour in layout B
-        float k[2][2][2];
-        for (int np = 0; np < 2; ++np)
-            for (int nq = 0; nq < 2; ++nq) {
-                const int nl = mirrored ? nq : np, nh = mirrored ? np : nq;
-                const double rho = H + (nl ? -Kl : Kl) + (nh ? -Kr : Kr);
-                k[0][np][nq] = (float)(m - 2.0 * rho);         // ka: a' = max(a, b + ka)
-                k[1][np][nq] = (float)(m + 2.0 * rho);         // kb: b' = max(b, a + kb)
-            }
-        const int pos = fused_chain_pos(low != 0, K);
-        const int PN = pos == 0 ? -1 : fused_bit_of_digit(low != 0, 0, pos - 1);
-        const int order = gate_order(K, PN);
-        for (int np = 0; np < 2; ++np)
-            for (int nq = 0; nq < 2; ++nq) {
-                if (order == ORDER_K0) { out[(np * 2 + nq) * 2] = k[1][np][nq]; out[(np * 2 + nq) * 2 + 1] = k[0][np][nq]; }
-                else if (order == ORDER_PN0) { out[nq * 2 + np] = k[0][np][nq]; out[4 + nq * 2 + np] = k[1][np][nq]; }
-                else { out[np * 2 + nq] = k[0][np][nq]; out[4 + np * 2 + nq] = k[1][np][nq]; }
-            }
+        if (g & GATE_RC_FLIP) {        // Z2 flip gate on column 0: kf[bit of column 1] = m - 2 K_0 sigma_1 (h = 0)
+            out[0] = (float)(m - 2.0 * Kr); out[1] = (float)(m + 2.0 * Kr);
+            for (int i = 2; i < 8; ++i) out[i] = 0.f;
+        } else {
+            // k[side][P bit][Q bit]: P = left neighbour in layout A, right neighbour in layout B
+            float k[2][2][2];
+            for (int np = 0; np < 2; ++np)
+                for (int nq = 0; nq < 2; ++nq) {
+                    const int nl = mirrored ? nq : np, nh = mirrored ? np : nq;
+                    const double rho = H + (nl ? -Kl : Kl) + (nh ? -Kr : Kr);
+                    k[0][np][nq] = (float)(m - 2.0 * rho);         // ka: a' = max(a, b + ka)
+                    k[1][np][nq] = (float)(m + 2.0 * rho);         // kb: b' = max(b, a + kb)
+                }
+            const int pos = fused_chain_pos(low != 0, K);
+            const int PN = pos == 0 ? -1 : fused_bit_of_digit(low != 0, 0, pos - 1);
+            const int order = gate_order(K, PN);
+            for (int np = 0; np < 2; ++np)
+                for (int nq = 0; nq < 2; ++nq) {
+                    if (order == ORDER_K0) { out[(np * 2 + nq) * 2] = k[1][np][nq]; out[(np * 2 + nq) * 2 + 1] = k[0][np][nq]; }
+                    else if (order == ORDER_PN0) { out[nq * 2 + np] = k[0][np][nq]; out[4 + nq * 2 + np] = k[1][np][nq]; }
+                    else { out[np * 2 + nq] = k[0][np][nq]; out[4 + np * 2 + nq] = k[1][np][nq]; }
+                }
+        }
     }
     if (idx < FFINAL_FLOATS) {
         float* out = p.final_tab + inst * FFINAL_FLOATS;
@@ -550,7 +615,7 @@ __global__ void __launch_bounds__(256) fused_prep_kernel(const FusedPrepParams p
             const bool low = p.fin_low != 0;
             // register columns are consecutive: x0 .. x0+6
             const int d0 = low ? (p.fin_layout == 0 ? 0 : 5) : (p.fin_layout == 0 ? 0 : 2);
-            const int x0 = p.fin_a + d0;
+            const int x0 = p.col_off + p.fin_a + d0;
             double acc = 0;
             int bits[F_RB];
             for (int i = 0; i < F_RB; ++i) bits[i] = (j >> fused_bit_of_digit(low, p.fin_layout, d0 + i)) & 1;
@@ -559,14 +624,15 @@ __global__ void __launch_bounds__(256) fused_prep_kernel(const FusedPrepParams p
                 acc += bits[i] ? -Hacc(L, c) : Hacc(L, c);
                 if (i + 1 < F_RB) acc += (bits[i] == bits[i + 1]) ? Kacc(L, c) : -Kacc(L, c);
             }
-            acc += (tl == bits[0]) ? Kacc(L, x0 - 1) : -Kacc(L, x0 - 1);              // 0 when x0 = 0
+            acc += (tl == bits[0]) ? Kacc(L, x0 - 1) : -Kacc(L, x0 - 1);              // 0 when x0 = 0 (Z2: tl = 0 = sigma_0 up)
             acc += (th == bits[F_RB - 1]) ? Kacc(L, x0 + F_RB - 1) : -Kacc(L, x0 + F_RB - 1);   // 0 at the right edge
             out[idx] = (float)acc;
         } else if (idx < 576) {
-            const int c = (int)idx - 512;
-            out[idx] = c < L ? (float)Hacc(L, c) : 0.f;
+            // per DIGIT of the kernel's index; Z2: digit 0 = column 1 also carries K_0 sigma_0 sigma_1 = K_0 sigma_1
+            const int c = (int)idx - 512 + p.col_off;
+            out[idx] = c < L ? (float)(Hacc(L, c) + (p.col_off && c == p.col_off ? Kacc(L, c - 1) : 0.0)) : 0.f;
         } else {
-            const int c = (int)idx - 576;
+            const int c = (int)idx - 576 + p.col_off;
             out[idx] = c < L - 1 ? (float)Kacc(L, c) : 0.f;
         }
     }

@@ -16,12 +16,13 @@ TROPICAL_F32 = 0
 COUNTING_F32_F64 = 1
 TROPICAL_I16 = 2
 CALL_ENERGY, CALL_COUNT, CALL_CONFIG, CALL_ENERGY_I16 = 0, 1, 2, 3
+CALL_ENERGY_Z2 = 4      # CALL_ENERGY with the h = 0 flip-reduced half-state required (ttn.h)
 
 EXPORTS = [
     "ttn_workspace_bytes", "ttn_sweep_energy", "ttn_sweep_energy_i16", "ttn_sweep_count", "ttn_ground_config",
     "ttn_potts3_sweep_energy", "ttn_potts3_sweep_count", "ttn_plan_create", "ttn_plan_launch",
     "ttn_plan_read", "ttn_plan_destroy", "ttn_plan_num_launches", "ttn_plan_num_passes",
-    "ttn_plan_describe", "ttn_last_error", "ttn_version",
+    "ttn_plan_describe", "ttn_plan_state_elements", "ttn_last_error", "ttn_version",
     "ttn_chimera_workspace_bytes", "ttn_chimera_sweep_energy_i16",
 ]
 
@@ -61,6 +62,8 @@ def lib() -> ctypes.CDLL:
         L.ttn_plan_destroy.restype = None
         L.ttn_plan_num_launches.argtypes = [vp]
         L.ttn_plan_num_passes.argtypes = [vp]
+        L.ttn_plan_state_elements.argtypes = [vp]
+        L.ttn_plan_state_elements.restype = ctypes.c_ulonglong
         L.ttn_plan_describe.argtypes = [ci, ci, ci, ctypes.c_char_p, sz]
         L.ttn_plan_describe.restype = ctypes.c_long
         L.ttn_last_error.restype = ctypes.c_char_p
@@ -158,6 +161,11 @@ class Plan:
     @property
     def num_passes(self) -> int:
         return int(lib().ttn_plan_num_passes(self._p))
+
+    @property
+    def state_elements(self) -> int:
+        """Stored state-vector elements per instance (2^(L-1) under the h = 0 flip reduction)."""
+        return int(lib().ttn_plan_state_elements(self._p))
 
     def launch(self, stream=None):
         _check(lib().ttn_plan_launch(self._p, _stream_ptr(stream)))

@@ -173,6 +173,52 @@ def test_mid_ising_count_vs_oracle(L):
         assert E0[b] == Eo and E1[b] == Eo and count_ok(g[b], go)
 
 
+@pytest.mark.parametrize("L", [14, 15, 17, 19, 21])
+def test_mid_ising_integer_fields_vs_oracle(L):
+    """Integer couplings WITH integer fields at sizes where the fused f32 / counting kernels run
+    cross-row plans with two and more HIGH tile positions: the conjugated gate constants carry
+    the accumulated fields H_c and the last pass adds A_{L-1}(s) from the
+    4-variant table plus the per-thread H / K terms of the columns outside the register window.
+    Bit-exact against O-dp (Eq. (1) PAPER.md:29 with h != 0; gates (A2)-(A4) PAPER.md:240-252)."""
+    rng = np.random.default_rng(2100 + L)
+    B = 2
+    Jh = rng.integers(-3, 4, size=(B, L, L - 1)).astype(np.float32)
+    Jv = rng.integers(-3, 4, size=(B, L - 1, L)).astype(np.float32)
+    h = rng.integers(-2, 3, size=(B, L, L)).astype(np.float32)
+    E0, g = ttn.sweep_count(Jh, Jv, h)
+    E1 = ttn.sweep_energy(Jh, Jv, h)
+    for b in range(B):
+        Eo, go, _ = oracle.dp_ising(L, Jh[b], Jv[b], h[b])
+        assert E0[b] == Eo and E1[b] == Eo and count_ok(g[b], go)
+    # one instance alone (the whole grid works on it: cta_per_inst = 0 where the state is large enough)
+    assert ttn.sweep_energy(Jh[:1], Jv[:1], h[:1])[0] == E1[0]
+    Ec, gc = ttn.sweep_count(Jh[:1], Jv[:1], h[:1])
+    assert Ec[0] == E0[0] and gc[0] == g[0]
+
+
+@pytest.mark.parametrize("L", [16, 20, 24, 28])
+def test_gaussian_couplings_and_fields_f32_tolerance(L):
+    """The paper's own workload: Gaussian couplings AND fields in Float32.
+    ttn_sweep_energy through cross-row plans with HIGH tiles and asynchronous prefetch against the
+    f64 O-dp value, at north_star's |dE| <= 1e-5 |E0|.  The diagonal frame makes the gate constants
+    grow with the accumulated H / K sums: this is where f32 rounding would show."""
+    gold = golden()
+    seeds = [2000, 2001] if L <= 24 else [2000]
+    Jh, Jv, h = make_batch(L, seeds, "gauss", fields=True)
+    E1 = ttn.sweep_energy(Jh, Jv, h)
+    for b, seed in enumerate(seeds):
+        key = ("ising_gauss", L, seed)
+        if key in gold:
+            Eo = gold[key][0]
+        elif L <= 20:
+            Eo = oracle.dp_ising(L, Jh[b], Jv[b], h[b], count=False)[0]
+        else:
+            pytest.skip("no stored oracle value for %s" % (key,))
+        assert abs(E1[b] - Eo) <= TOL * abs(Eo), (L, seed, E1[b], Eo)
+    if L <= 24:        # single instance: the whole grid on one state
+        assert ttn.sweep_energy(Jh[:1], Jv[:1], h[:1])[0] == E1[0]
+
+
 def test_mid_potts_vs_oracle():
     for L in (10, 11):
         Jh, Jv, _ = make_batch(L, [5000], "pmj", q=3)
@@ -200,9 +246,9 @@ def test_backtrace_one_cta_per_instance_matches_multi_block(monkeypatch, L):
     Jh, Jv, h = make_batch(L, range(2700, 2700 + B), "gauss", fields=True)
     E_a, sig_a = ttn.ground_config(Jh, Jv, h)
     for b in range(0, B, 9):
-        Eo = oracle.dp_ising(L, Jh[b], Jv[b], h[b])[0] if L <= 13 else E_a[b]
+        Eo = oracle.dp_ising(L, Jh[b], Jv[b], h[b], count=False)[0]      # O-dp at every L (2^17 states: instant)
         assert abs(E_a[b] - Eo) <= TOL * abs(Eo)
-        assert abs(oracle.ising_energy(L, Jh[b], Jv[b], h[b], sig_a[b]) - E_a[b]) <= TOL * abs(E_a[b])
+        assert abs(oracle.ising_energy(L, Jh[b], Jv[b], h[b], sig_a[b]) - Eo) <= TOL * abs(Eo)
 
 
 @pytest.mark.parametrize("L", [12, 13, 14, 16])
@@ -356,6 +402,62 @@ def test_large_energy_vs_golden(L):
         pytest.skip("no stored oracle value")
     Jh, Jv, _ = make_batch(L, [4000], "pmj")
     assert ttn.sweep_energy(Jh, Jv)[0] == gold[key][0]
+
+
+# ------------------------------------------------------------------ h = 0 flip reduction
+@pytest.mark.parametrize("L", [14, 15, 16, 17, 19, 21])
+def test_z2_energy_vs_oracle(L, monkeypatch):
+    """h = 0: ttn_sweep_energy stores the half-state with column 0 up and applies the column-0 gates
+    as a pairing of every element with its complement (symmetry of Eq. (1)).  Bit-exact
+    against O-dp for integer couplings; identical to the full-state sweep; any field falls back."""
+    rng = np.random.default_rng(4400 + L)
+    B = 3
+    Jh = rng.integers(-3, 4, size=(B, L, L - 1)).astype(np.float32)
+    Jv = rng.integers(-3, 4, size=(B, L - 1, L)).astype(np.float32)
+    p = ttn.Plan(2, ttn.CALL_ENERGY, Jh, Jv)
+    assert p.state_elements == 2 ** (L - 1)                     # the reduction is what runs
+    p.launch(); E_z, _, _ = p.read(); p.close()
+    p = ttn.Plan(2, ttn.CALL_ENERGY_Z2, Jh[:1], Jv[:1], np.zeros((1, L, L), np.float32))   # all-zero h counts as h = 0
+    assert p.state_elements == 2 ** (L - 1)
+    p.launch(); E_1, _, _ = p.read(); p.close()                 # one instance: the whole grid on one state
+    for b in range(B):
+        assert E_z[b] == oracle.dp_ising(L, Jh[b], Jv[b], None, count=False)[0]
+    assert E_1[0] == E_z[0]
+    monkeypatch.setenv("TTN_DEBUG_Z2", "0")
+    p = ttn.Plan(2, ttn.CALL_ENERGY, Jh, Jv)
+    assert p.state_elements == 2 ** L
+    p.launch(); E_f, _, _ = p.read(); p.close()
+    monkeypatch.delenv("TTN_DEBUG_Z2")
+    assert np.array_equal(E_f, E_z)
+    # a single non-zero field entry selects the full-state sweep; the explicit kind refuses it
+    h = np.zeros((B, L, L), np.float32); h[1, L // 2, L - 1] = 1.0
+    p = ttn.Plan(2, ttn.CALL_ENERGY, Jh, Jv, h)
+    assert p.state_elements == 2 ** L
+    p.launch(); E_h, _, _ = p.read(); p.close()
+    assert E_h[1] == oracle.dp_ising(L, Jh[1], Jv[1], h[1], count=False)[0] and E_h[0] == E_z[0]
+    with pytest.raises(ttn.TTNError) as e:
+        ttn.Plan(2, ttn.CALL_ENERGY_Z2, Jh, Jv, h)
+    assert e.value.status == 1
+
+
+@pytest.mark.parametrize("L", [16, 20, 24])
+def test_z2_gaussian_couplings_f32_tolerance(L):
+    """Gaussian couplings, no field, through the flip-reduced sweep: |dE| <= 1e-5 |E0| against O-dp."""
+    Jh, Jv, _ = make_batch(L, [2100, 2101], "gauss")
+    E1 = ttn.sweep_energy(Jh, Jv)
+    for b in range(2):
+        if L <= 20 or b == 0:
+            Eo = oracle.dp_ising(L, Jh[b], Jv[b], None, count=False)[0]
+            assert abs(E1[b] - Eo) <= TOL * abs(Eo)
+
+
+@pytest.mark.parametrize("L", [24, 28])
+def test_full_state_sweep_still_matches_golden(L, monkeypatch):
+    """The full-state Tropical<f32> sweep (what any h != 0 runs) on the +-J goldens, flip reduction off."""
+    gold = golden()
+    monkeypatch.setenv("TTN_DEBUG_Z2", "0")
+    Jh, Jv, _ = make_batch(L, [4000], "pmj")
+    assert ttn.sweep_energy(Jh, Jv)[0] == gold[("ising_energy", L, 4000)][0]
 
 
 # ------------------------------------------------------------------ error behaviour
@@ -524,7 +626,7 @@ def _chimera_oracle():
     return chimera_oracle
 
 
-@pytest.mark.parametrize("M,N", [(1, 1), (1, 3), (2, 1), (2, 2), (3, 2), (2, 4), (3, 3), (4, 2), (4, 4)])
+@pytest.mark.parametrize("M,N", [(1, 1), (1, 3), (2, 1), (2, 2), (3, 2), (2, 4), (3, 3), (4, 2), (4, 4), (5, 2), (5, 5)])
 def test_chimera_energy_vs_oracle(M, N):
     """Bit-exact ground-state energies against the group tensor-network oracle (integers)."""
     from ttn_inputs import make_chimera_instance
@@ -556,6 +658,24 @@ def test_chimera_closed_forms_beyond_the_oracle(M, N):
     I = make_chimera_instance(M, N, 6300)
     K2, Jv2, Jh2 = co.gauge(M, N, 4, I.K, I.Jv, I.Jh, ev, eu)
     assert ttn.chimera_sweep_energy_i16(I.K, I.Jv, I.Jh) == ttn.chimera_sweep_energy_i16(K2, Jv2, Jh2)
+
+
+@pytest.mark.parametrize("M,N,seed", [(3, 5, 6400), (6, 4, 6401), (7, 7, 7007)])
+def test_chimera_transpose_isomorphism_on_device(M, N, seed):
+    """The chimera graph of M x N cells is isomorphic to the one of N x M cells with the two groups
+    of every cell exchanged: (K, Jv, Jh) -> (K^T per cell on the transposed grid, Jh^T, Jv^T).  The
+    device sweeps columns with an ancilla for the vertical group, so rows and columns take entirely
+    different code paths: equal energies pin the seeded values beyond the oracle's reach (7 x 7
+    cells = the instance bench.py times)."""
+    from ttn_inputs import make_chimera_instance
+    I = make_chimera_instance(M, N, seed)
+    Kt = np.ascontiguousarray(np.transpose(I.K, (1, 0, 3, 2)))
+    Jvt = np.ascontiguousarray(np.transpose(I.Jh, (1, 0, 2)))
+    Jht = np.ascontiguousarray(np.transpose(I.Jv, (1, 0, 2)))
+    E = ttn.chimera_sweep_energy_i16(I.K, I.Jv, I.Jh)
+    assert ttn.chimera_sweep_energy_i16(Kt, Jvt, Jht) == E
+    if max(M, N) <= 5:
+        assert E == _chimera_oracle().dp_chimera(M, N, 4, I.K, I.Jv, I.Jh)[0]
 
 
 def test_chimera_argument_errors():

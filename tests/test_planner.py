@@ -179,16 +179,23 @@ DIGIT_OF_BIT_I16 = {(1, 0): [1 + d for d in [5, 6, 0, 1, 2, 3, 4]] + [0], (1, 1)
                     (0, 0): [4, 5, 6, 0, 1, 2, 3], (0, 1): [4, 3, 2, 8, 7, 6, 5]}
 
 
-def fused_to_gates(L, fpasses, count=False, i16=False, config=False):
+# flip-reduced f32 geometry (GEOM_F32_Z2, h = 0): column 0 is not stored (the half-state holds the
+# configurations with column 0 up); column c >= 1 is digit c - 1 with the f32 maps; the gate on
+# column 0 ("flip gate", k = -1) may end any round of a LOW pass
+DIGIT_OF_BIT_Z2 = {(1, 0): [1 + d for d in [5, 6, 0, 1, 2, 3, 4]], (1, 1): [1 + d for d in [6, 5, 11, 10, 9, 8, 7]],
+                   (0, 0): [4, 5, 6, 0, 1, 2, 3], (0, 1): [4, 3, 2, 8, 7, 6, 5]}
+
+
+def fused_to_gates(L, fpasses, count=False, i16=False, config=False, z2=False):
     """Check the structure of the micro-op program (layouts, register bits, rounds) and the
     three-point-stencil dependency rule; return the flat (r, c) gate sequence."""
     flat = []
     grow = [1] * L                                   # rows complete per digit (row 0 needs no gate)
     for i, ps in enumerate(fpasses):
         a, Wt, low = ps["a"], ps["W"], ps["low"]
-        wl, wh, rb = (10, 7, 5) if count else ((13, 9, 8 if low else 7) if i16 else (12, 9, 7))
-        dmap = DIGIT_OF_BIT_COUNT if count else (DIGIT_OF_BIT_I16 if i16 else DIGIT_OF_BIT)
-        assert (low == 1 and a == 0 and Wt == wl) or (low == 0 and a >= (5 if i16 else 4) and Wt == wh)
+        wl, wh, rb = (10, 7, 5) if count else ((13, 9, 8 if low else 7) if i16 else ((13, 9, 7) if z2 else (12, 9, 7)))
+        dmap = DIGIT_OF_BIT_COUNT if count else (DIGIT_OF_BIT_I16 if i16 else (DIGIT_OF_BIT_Z2 if z2 else DIGIT_OF_BIT))
+        assert (low == 1 and a == 0 and Wt == wl) or (low == 0 and a >= (5 if i16 or z2 else 4) and Wt == wh)
         assert a + Wt <= L
         assert (ps["flags"] & 1) == (1 if i == 0 else 0)
         last = i == len(fpasses) - 1 and not config
@@ -208,13 +215,19 @@ def fused_to_gates(L, fpasses, count=False, i16=False, config=False):
                 assert layout == 1
                 layout = 0
             else:
-                assert code == "round" and 0 < m["mask"] < (1 << rb) and m["first"] == ngates
-                bits = [k for k in range(rb) if m["mask"] >> k & 1]
-                assert [g["k"] for g in m["gates"]] == bits          # ascending register bits
+                flip = m.get("flip", 0)
+                assert not flip or (z2 and low)                      # flip gates: LOW passes of Z2 plans only
+                assert code == "round" and (flip or 0 < m["mask"]) and m["mask"] < (1 << rb) and m["first"] == ngates
+                bits = [k for k in range(rb) if m["mask"] >> k & 1] + ([-1] if flip else [])
+                assert [g["k"] for g in m["gates"]] == bits          # ascending register bits, the flip gate last
                 before = list(grow)
                 for g in m["gates"]:
                     c, r = g["c"], g["r"]
-                    assert c == a + dmap[(low, layout)][g["k"]]      # register bit <-> column
+                    if g["k"] < 0:
+                        assert c == 0
+                    else:
+                        assert c == a + dmap[(low, layout)][g["k"]]  # register bit <-> column
+                        assert not z2 or c >= 1
                     assert g["layout"] == layout
                     # legal at the START of the round: every gate of a round commutes with the others
                     assert 1 <= r < L and before[c] == r
@@ -281,6 +294,71 @@ def test_fused_i16_schedule_obeys_dependency_rule(L):
     assert int(head["L"]) == L
     flat = fused_to_gates(L, fpasses, i16=True)
     assert len(flat) == L * (L - 1) == len(set(flat))
+
+
+@pytest.mark.parametrize("L", [14, 15, 16, 19, 23, 24, 28, 30, 32, 34])
+def test_fused_z2_schedule_obeys_dependency_rule(L):
+    """h = 0 flip reduction: same stencil rule; the gates on column 0 appear as
+    flip gates in LOW passes, exactly one per row."""
+    head, fpasses = parse_fused(describe(2, L, 4, fused=True))
+    assert int(head["L"]) == L
+    flat = fused_to_gates(L, fpasses, z2=True)
+    assert len(flat) == L * (L - 1) == len(set(flat))
+    assert sorted(r for r, c in flat if c == 0) == list(range(1, L))
+
+
+def replay_z2_half_state(L, gates, Jh, Jv):
+    """numpy float64 replay of a flip-reduced schedule on the HALF state, restated from the symmetry:
+    with h = 0 every intermediate state W of the sweep obeys W[s] = W[~s] (each gate (A2) PAPER.md:242
+    and each diagonal (A4) PAPER.md:251 commutes with the global flip of Eq. (1)), so
+    only u = (s_1 .. s_{L-1}) with s_0 = 0 (sigma_0 = +1) is stored and the partner of u under the
+    column-0 gate, the element with s_0 = 1, is W[~u].  Gates in the diagonal frame as above."""
+    N = 2 ** (L - 1)
+    u = np.arange(N)
+    sig = [np.ones(N)] + [1 - 2 * ((u >> (c - 1)) & 1) for c in range(1, L)]
+    Kacc = np.cumsum(Jh, axis=0)
+    V = np.zeros(N)
+    defer = 0.0
+    for (r, c) in gates:
+        J = Jv[r - 1, c]
+        defer += J
+        rho = np.zeros(N)
+        if c > 0:
+            rho = rho + Kacc[r - 1, c - 1] * sig[c - 1]
+        if c < L - 1:
+            rho = rho + Kacc[r - 1, c] * sig[c + 1]
+        if c == 0:
+            V = np.maximum(V, V[(N - 1) ^ u] - 2 * J - 2 * rho)       # a' = max(a, b + m - 2 rho), b = W[~u]
+        else:
+            ia = u[(u >> (c - 1)) & 1 == 0]
+            ib = ia | (1 << (c - 1))
+            xa, xb = V[ia].copy(), V[ib].copy()
+            V[ia] = np.maximum(xa, xb - 2 * J - 2 * rho[ia])
+            V[ib] = np.maximum(xb, xa - 2 * J + 2 * rho[ia])
+    A = np.zeros(N)
+    for c in range(L - 1):
+        A += Kacc[L - 1, c] * sig[c] * sig[c + 1]
+    m = (V + A).max() + defer
+    return 0.0 if m == 0 else -m
+
+
+@pytest.mark.parametrize("L", [14, 15, 17])
+def test_fused_z2_schedule_replay_matches_oracle(L):
+    _, fpasses = parse_fused(describe(2, L, 4, fused=True))
+    flat = fused_to_gates(L, fpasses, z2=True)
+    rng = np.random.default_rng(200 + L)
+    Jh = rng.integers(-2, 3, size=(L, L - 1)).astype(float)
+    Jv = rng.integers(-2, 3, size=(L - 1, L)).astype(float)
+    Eo, _, _ = oracle.dp_ising(L, Jh, Jv, None, count=False)
+    assert replay_z2_half_state(L, flat, Jh, Jv) == Eo
+    Jh, Jv = rng.normal(size=Jh.shape), rng.normal(size=Jv.shape)
+    Eo, _, _ = oracle.dp_ising(L, Jh, Jv, None, count=False)
+    assert abs(replay_z2_half_state(L, flat, Jh, Jv) - Eo) <= 1e-9 * abs(Eo)
+
+
+def test_z2_describe_falls_back_below_two_tiles():
+    """L = 13: the half-state is a single (self-complementary) LOW tile: the plain schedule runs."""
+    assert describe(2, 13, 4, fused=True) == describe(2, 13, 0, fused=True)
 
 
 @pytest.mark.parametrize("L", [12, 13, 16, 20, 21, 22, 28])
