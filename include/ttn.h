@@ -27,10 +27,11 @@
  * is NO CPU fallback: without a CUDA device every compute call returns TTN_ECUDA.
  *
  * h = 0 (NULL or all zero): Eq. (1) is invariant under the global flip sigma -> -sigma, and so is
- * every intermediate state of the sweep; ttn_sweep_energy then stores only the half of the state
- * vector with column 0 up (2^(L-1) elements) and applies the column-0 gates as a pairing of
- * every element with its complement -- half the memory, bytes and arithmetic, identical results
- * (SURVEY.md 8f NEXT-4).  Any non-zero field selects the full-state sweep.
+ * every intermediate state of the sweep; ttn_sweep_energy and ttn_sweep_count then store only the
+ * half of the state vector with column 0 up (2^(L-1) elements) and apply the column-0 gates as a
+ * pairing of every element with its complement -- half the memory, bytes and arithmetic,
+ * identical results, the degeneracy being twice the half's count.  Any
+ * non-zero field selects the full-state sweep.
  *
  * Layouts (row-major, batch-major):  Jh[batch][L][L-1], Jv[batch][L-1][L], h[batch][L][L]
  * (h may be NULL = all zero), E0[batch], degeneracy[batch], sigma[batch][L][L] (+1 / -1).
@@ -144,7 +145,8 @@ typedef enum {
     /* TTN_CALL_ENERGY with the flip-reduced half-state REQUIRED: TTN_EINVAL when h != 0 (lattices with
        L < 14 run the plain sweep).  TTN_CALL_ENERGY selects it by itself when h = 0; this kind exists
        for ttn_plan_describe and for tests. */
-    TTN_CALL_ENERGY_Z2 = 4
+    TTN_CALL_ENERGY_Z2 = 4,
+    TTN_CALL_COUNT_Z2 = 5       /* the same for TTN_CALL_COUNT (L < 12 runs the plain sweep) */
 } ttn_call;
 
 ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const float* Jv,

@@ -123,6 +123,7 @@ bool fused_eligible(int q, int L, bool count, bool config, const DebugCfg& dbg) 
 const ttn::FusedGeom* z2_geom(int q, int L, ttn_call call, bool has_field, const DebugCfg& dbg) {
     if (dbg.fused == 0 || dbg.z2 == 0 || q != 2 || has_field) return nullptr;
     if ((call == TTN_CALL_ENERGY || call == TTN_CALL_ENERGY_Z2) && L >= ttn::GEOM_F32_Z2.WLOW + 1) return &ttn::GEOM_F32_Z2;
+    if ((call == TTN_CALL_COUNT || call == TTN_CALL_COUNT_Z2) && L >= ttn::GEOM_COUNT_Z2.WLOW + 1) return &ttn::GEOM_COUNT_Z2;
     return nullptr;
 }
 
@@ -395,6 +396,7 @@ static ttn_status launch_fcount_pass(const ttn_plan* P, const ttn::FusedPass& ps
     ttn::CountParams cp{};
     ttn::FusedParams& pp = cp.f;
     pp.L = P->L; pp.a = ps.a; pp.low = ps.low; pp.flags = ps.flags; pp.batch = P->batch;
+    if (P->z2) { pp.L = P->L - 1; pp.a = ps.low ? 0 : ps.a - 1; }      // half-state: column c = digit c - 1
     pp.first_layout = ps.first_layout; pp.last_layout = ps.last_layout;
     pp.state = reinterpret_cast<float*>(P->ws + y.x);
     cp.state_n = reinterpret_cast<double*>(P->ws + y.n);
@@ -409,7 +411,7 @@ static ttn_status launch_fcount_pass(const ttn_plan* P, const ttn::FusedPass& ps
     pp.final_tab = reinterpret_cast<const float*>(P->ws + y.f_final);
     pp.part_x = reinterpret_cast<float*>(P->ws + y.part_x);
     cp.part_n = reinterpret_cast<double*>(P->ws + y.part_n);
-    pp.stride_bytes = 4u << ps.a;
+    pp.stride_bytes = 4u << pp.a;
     pp.prefetch_pc = -1;
     unsigned long long grid = (unsigned long long)P->fused_grid;
     const int nw = ttn::CWARPS;
@@ -421,7 +423,8 @@ static ttn_status launch_fcount_pass(const ttn_plan* P, const ttn::FusedPass& ps
         if (grid > need) grid = need;
     }
     pp.part_stride = pp.cta_per_inst ? 1 : (int)grid;
-    if (ps.low) ttn::fcount_pass_kernel<true><<<(unsigned)grid, nw * 32, ttn::csmem_bytes(), st>>>(cp);
+    if (ps.low && P->z2) ttn::fcount_pass_kernel<true, true><<<(unsigned)grid, nw * 32, ttn::csmem_bytes(), st>>>(cp);
+    else if (ps.low) ttn::fcount_pass_kernel<true><<<(unsigned)grid, nw * 32, ttn::csmem_bytes(), st>>>(cp);
     else ttn::fcount_pass_kernel<false><<<(unsigned)grid, nw * 32, ttn::csmem_bytes(), st>>>(cp);
     TTN_CUDA(cudaGetLastError());
     if (ps.flags & ttn::PASS_REDUCE) {
@@ -454,12 +457,15 @@ static ttn_status setup_fcount(ttn_plan* P, cudaStream_t st) {
     q.final_tab = reinterpret_cast<float*>(P->ws + y.f_final);
     const ttn::FusedPass& lastp = fp.passes.back();
     q.fin_low = lastp.low; q.fin_layout = lastp.last_layout; q.fin_a = lastp.a;
+    if (P->z2) q.fin_a = lastp.low ? 0 : lastp.a - 1;
+    q.col_off = P->z2 ? 1 : 0;
     long work = ttn::CFINAL_FLOATS; if (q.n_gates > work) work = q.n_gates;
     dim3 grid((unsigned)((work + 255) / 256), (unsigned)P->batch);
     ttn::fcount_prep_kernel<<<grid, 256, 0, st>>>(q);
     TTN_CUDA(cudaGetLastError());
     TTN_CUDA(cudaFuncSetAttribute(ttn::fcount_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::csmem_bytes()));
     TTN_CUDA(cudaFuncSetAttribute(ttn::fcount_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::csmem_bytes()));
+    TTN_CUDA(cudaFuncSetAttribute(ttn::fcount_pass_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::csmem_bytes()));
     int dev = 0, sms = 0;
     TTN_CUDA(cudaGetDevice(&dev));
     TTN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -583,12 +589,12 @@ long ttn_plan_describe(int q, int L, ttn_call call, char* buf, size_t n) {
     if (!limits_ok(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) return -1;
     std::string s;
     const DebugCfg dbg = read_debug();
-    if (call == TTN_CALL_ENERGY_Z2) {              // the schedule ttn_sweep_energy runs when h = 0
+    if (call == TTN_CALL_ENERGY_Z2 || call == TTN_CALL_COUNT_Z2) {   // the schedules the calls run when h = 0
         if (const ttn::FusedGeom* G = z2_geom(q, L, call, false, dbg)) {
             ttn::FusedPlan fp = ttn::make_fused_plan(L, ttn::FMAX_GATES, *G);
             if (fp.ok) s = ttn::describe_fused(fp);
         }
-        if (s.empty()) call = TTN_CALL_ENERGY;
+        if (s.empty()) call = call == TTN_CALL_ENERGY_Z2 ? TTN_CALL_ENERGY : TTN_CALL_COUNT;
     }
     if (call == TTN_CALL_ENERGY_I16 && i16_eligible(q, L, dbg)) {
         ttn::FusedPlan fp = ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_I16);
@@ -616,19 +622,20 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     if (q != 2 && q != 3) return fail(TTN_EINVAL, "q must be 2 or 3");
     if (L < 1 || batch < 1) return fail(TTN_EINVAL, "L and batch must be >= 1");
     if (call != TTN_CALL_ENERGY && call != TTN_CALL_COUNT && call != TTN_CALL_CONFIG && call != TTN_CALL_ENERGY_I16 &&
-        call != TTN_CALL_ENERGY_Z2)
+        call != TTN_CALL_ENERGY_Z2 && call != TTN_CALL_COUNT_Z2)
         return fail(TTN_EINVAL, "bad call kind");
+    const bool want_z2 = (call == TTN_CALL_ENERGY_Z2 || call == TTN_CALL_COUNT_Z2);
     const DebugCfg dbg = read_debug();
     bool i16 = false;
     if (call == TTN_CALL_ENERGY_I16) {
         if (q != 2) return fail(TTN_EINVAL, "Tropical<i16> is an Ising call");
         i16 = i16_eligible(q, L, dbg);      // small lattices run the f32 path (identical results)
     }
-    if (call == TTN_CALL_ENERGY_Z2 && q != 2) return fail(TTN_EINVAL, "the flip reduction is an Ising call");
+    if (want_z2 && q != 2) return fail(TTN_EINVAL, "the flip reduction is an Ising call");
     if (L > 1 && (!Jh || !Jv)) return fail(TTN_EINVAL, "Jh/Jv is NULL");
     if (!workspace) return fail(TTN_EINVAL, "workspace is NULL");
     if (q == 3 && h) return fail(TTN_EINVAL, "the Potts variant takes no fields");
-    const bool count = (call == TTN_CALL_COUNT), config = (call == TTN_CALL_CONFIG);
+    const bool count = (call == TTN_CALL_COUNT || call == TTN_CALL_COUNT_Z2), config = (call == TTN_CALL_CONFIG);
     if (!limits_ok(q, L, count, config)) return fail(TTN_EUNSUPPORTED, "L=%d beyond the limits for this call", L);
     const size_t nh = (size_t)batch * L * (L - 1), nv = (size_t)batch * (L - 1) * L, nf = (size_t)batch * L * L;
     for (size_t i = 0; i < nh; ++i) if (!std::isfinite(Jh[i])) return fail(TTN_EINVAL, "non-finite Jh[%zu]", i);
@@ -652,9 +659,9 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     // h = NULL or all zero: Eq. (1) PAPER.md:29 is invariant under the global flip -> half-state (planner.h)
     bool field = false;
     if (h) for (size_t i = 0; i < nf && !field; ++i) field = (h[i] != 0.0f);
-    if (call == TTN_CALL_ENERGY_Z2 && field) return fail(TTN_EINVAL, "the flip reduction needs h = 0");
+    if (want_z2 && field) return fail(TTN_EINVAL, "the flip reduction needs h = 0");
     const ttn::FusedGeom* zg = z2_geom(q, L, call, field, dbg);
-    if (call == TTN_CALL_ENERGY_Z2) call = TTN_CALL_ENERGY;       // lattices too small for it run the plain sweep
+    if (want_z2) call = count ? TTN_CALL_COUNT : TTN_CALL_ENERGY;  // lattices too small for it run the plain sweep
     Layout lay = make_layout(q, L, count, config, batch, dbg, i16, zg != nullptr);
     if (workspace_bytes < lay.total)
         return fail(TTN_ENOMEM, "workspace too small: %zu < %zu", workspace_bytes, lay.total);
@@ -829,6 +836,8 @@ ttn_status ttn_plan_read(ttn_plan* P, void* stream, double* E0, double* degenera
     if (P->config)
         TTN_CUDA(cudaMemcpyAsync(sigma, P->ws + P->lay.sigma, (size_t)P->batch * P->L * P->L, cudaMemcpyDeviceToHost, st));
     TTN_CUDA(cudaStreamSynchronize(st));
+    if (P->count && P->z2)                           // the stored half holds one of every flip pair (exact: x 2)
+        for (int b = 0; b < P->batch; ++b) degeneracy[b] *= 2.0;
     for (int b = 0; b < P->batch; ++b) {
         double m = (double)x[b] + P->defer[b];      // max of -E
         E0[b] = (m == 0.0) ? 0.0 : -m;              // -0.0 -> +0.0

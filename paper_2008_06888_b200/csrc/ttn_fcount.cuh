@@ -118,6 +118,31 @@ __device__ __forceinline__ void cxmove(float (&x)[32], double (&n)[32], unsigned
     }
 }
 
+// ---- Z2 flip gate (h = 0; planner.h "GLOBAL-FLIP (Z2) REDUCTION"), counting form --------------------------
+//     c = x[~u] + kf[bit of column 1 in u];   n'[u] = n[u] [x >= c] + n[~u] [c >= x];   x'[u] = max(x[u], c)
+// ~u = register 31 - j of lane 31 - lane of the partner warp (warp ^ 1), which holds the complement
+// tile in the same layout; both warps publish (x, n) in their own exchange region first.
+template <int LAYOUT>
+__device__ __forceinline__ void cflipgate(float (&x)[32], double (&n)[32], unsigned char* myreg, const unsigned char* preg,
+                                          const int lane, const int warp, const float k0, const float k1) {
+    __syncwarp();
+    cxmove<true, LAYOUT, true>(x, n, myreg, lane);
+    pair_sync(warp);
+    const float* px = reinterpret_cast<const float*>(preg);
+    const double* pn = reinterpret_cast<const double*>(preg + 32 * 33 * 4);
+    // column 1 = tile digit 0: register bit 0 in layout A, lane bit 0 in layout B
+    const float kl = (lane & 1) ? k1 : k0;
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {
+        const int i = cx_index<true, LAYOUT>(31 - lane, 31 - j);
+        const float c = px[i] + (LAYOUT == 0 ? ((j & 1) ? k1 : k0) : kl);
+        const double m = pn[i];
+        n[j] = fma(m, ind(c >= x[j]), n[j] * ind(x[j] >= c));
+        x[j] = fmaxf(x[j], c);
+    }
+    pair_sync(warp);
+}
+
 // ---- global <-> register ----------------------------------------------------------------------------
 //   LOW  B: e = lane + 32 rev5(j)
 //   HIGH A: e = j + 32 (lane >> 3);   HIGH B: e = (lane >> 3) + 4 rev5(j);   address = tile + rho + (e << a)
@@ -169,7 +194,8 @@ __device__ __forceinline__ float cfinal_thread_const(const float* s_fin, int L, 
     return acc;
 }
 
-template <bool LOW>
+// Z2 (LOW only): flip-reduced state, warp pairs on tiles (T, ~T), flip gates (ttn_fused.cuh)
+template <bool LOW, bool Z2 = false>
 __global__ void __launch_bounds__(CWARPS * 32, 1) fcount_pass_kernel(const CountParams cp) {
     const FusedParams& p = cp.f;
     extern __shared__ __align__(16) unsigned char csm_raw[];
@@ -203,8 +229,15 @@ __global__ void __launch_bounds__(CWARPS * 32, 1) fcount_pass_kernel(const Count
         float wmax = -INFINITY; double wcnt = 0.0;
 
         for (unsigned long long it = 0;; ++it) {
-            const unsigned long long wt = LOW ? it * nw + gw : 4ull * (it * (nw >> 2) + (gw >> 2)) + (unsigned long long)(warp & 3);
-            if ((LOW ? wt : (wt & ~3ull)) >= p.tiles_per_inst) break;
+            unsigned long long wt;
+            if (LOW && Z2) {                               // the pair (2k, 2k + 1) takes tile t and its complement
+                const unsigned long long t = it * (nw >> 1) + (gw >> 1);
+                if (t >= (p.tiles_per_inst >> 1)) break;
+                wt = (gw & 1ull) ? p.tiles_per_inst - 1 - t : t;
+            } else {
+                wt = LOW ? it * nw + gw : 4ull * (it * (nw >> 2) + (gw >> 2)) + (unsigned long long)(warp & 3);
+                if ((LOW ? wt : (wt & ~3ull)) >= p.tiles_per_inst) break;
+            }
             if (!LOW && wt >= p.tiles_per_inst) {          // partial last group: keep the barrier counts equal
                 if (!(p.flags & PASS_INIT)) group_sync(warp);
                 if (!(p.flags & PASS_REDUCE)) group_sync(warp);
@@ -243,8 +276,14 @@ __global__ void __launch_bounds__(CWARPS * 32, 1) fcount_pass_kernel(const Count
                 if (code == MC_END || code == MC_FINAL) break;
                 const unsigned nxt = s_mops[pc + 1];
                 if (code == MC_ROUND) {
-                    const float4* gk = s_gk + 2 * (op >> 16);
+                    const float4* gk = s_gk + 2 * ((op >> 16) & 0x7fffu);
                     cround<LOW>(x, n, (op >> 8) & 0x1fu, gk, layout ? tpB : tpA, layout ? tqB : tqA);
+                    if (LOW && Z2 && (op >> 31)) {         // the round ends with the flip gate (column 0)
+                        const float4 kf = gk[0];
+                        const unsigned char* preg = regions + (size_t)(warp ^ 1) * CREGION_BYTES;
+                        if (layout == 0) cflipgate<0>(x, n, myreg, preg, lane, warp, kf.x, kf.y);
+                        else cflipgate<1>(x, n, myreg, preg, lane, warp, kf.x, kf.y);
+                    }
                 } else if (code == MC_XAB) {
                     __syncwarp(); cxmove<LOW, 0, true>(x, n, myreg, lane); __syncwarp(); cxmove<LOW, 1, false>(x, n, myreg, lane);
                     layout = 1;
@@ -304,6 +343,7 @@ struct CountPrepParams {
     float* gate_k;                 // [inst][n_gates][8]
     float* final_tab;              // [inst][CFINAL_FLOATS]
     int fin_low, fin_layout, fin_a;
+    int col_off;                   // Z2: 1 = the kernel's digit d is lattice column d + 1 (fin_a is a digit)
 };
 
 __global__ void __launch_bounds__(256) fcount_prep_kernel(const CountPrepParams p) {
@@ -320,20 +360,25 @@ __global__ void __launch_bounds__(256) fcount_prep_kernel(const CountPrepParams 
         const double m = -2.0 * (double)Jv[(r - 1) * L + c];
         const double H = Hacc(r, c), Kl = Kacc(r, c - 1), Kr = Kacc(r, c);
         float* out = p.gate_k + (inst * p.n_gates + idx) * 8;
-        for (int np = 0; np < 2; ++np)
-            for (int nq = 0; nq < 2; ++nq) {
-                const int nl = mirrored ? nq : np, nh = mirrored ? np : nq;      // P = left in A, right in B
-                const double rho = H + (nl ? -Kl : Kl) + (nh ? -Kr : Kr);
-                out[np * 2 + nq] = (float)(m - 2.0 * rho);
-                out[4 + np * 2 + nq] = (float)(m + 2.0 * rho);
-            }
+        if (g & GATE_RC_FLIP) {        // Z2 flip gate on column 0: kf[bit of column 1] = m - 2 K_0 sigma_1 (h = 0)
+            out[0] = (float)(m - 2.0 * Kr); out[1] = (float)(m + 2.0 * Kr);
+            for (int i = 2; i < 8; ++i) out[i] = 0.f;
+        } else {
+            for (int np = 0; np < 2; ++np)
+                for (int nq = 0; nq < 2; ++nq) {
+                    const int nl = mirrored ? nq : np, nh = mirrored ? np : nq;      // P = left in A, right in B
+                    const double rho = H + (nl ? -Kl : Kl) + (nh ? -Kr : Kr);
+                    out[np * 2 + nq] = (float)(m - 2.0 * rho);
+                    out[4 + np * 2 + nq] = (float)(m + 2.0 * rho);
+                }
+        }
     }
     if (idx < CFINAL_FLOATS) {
         float* out = p.final_tab + inst * CFINAL_FLOATS;
         if (idx < 128) {
             const int var = (int)idx >> 5, j = (int)idx & 31, tl = var & 1, th = var >> 1;
             const int Wt = p.fin_low ? CW_LOW : CW_HIGH;
-            const int x0 = p.fin_a + (p.fin_layout == 0 ? 0 : Wt - CRB);       // first register column
+            const int x0 = p.col_off + p.fin_a + (p.fin_layout == 0 ? 0 : Wt - CRB);       // first register column
             int bits[CRB];
             for (int i = 0; i < CRB; ++i) bits[i] = (j >> (p.fin_layout == 0 ? i : CRB - 1 - i)) & 1;
             double acc = 0;
@@ -346,10 +391,11 @@ __global__ void __launch_bounds__(256) fcount_prep_kernel(const CountPrepParams 
             acc += (th == bits[CRB - 1]) ? Kacc(L, x0 + CRB - 1) : -Kacc(L, x0 + CRB - 1);
             out[idx] = (float)acc;
         } else if (idx >= 512 && idx < 576) {
-            const int c = (int)idx - 512;
-            out[idx] = c < L ? (float)Hacc(L, c) : 0.f;
+            // per DIGIT of the kernel's index; Z2: digit 0 = column 1 also carries K_0 sigma_0 sigma_1 = K_0 sigma_1
+            const int c = (int)idx - 512 + p.col_off;
+            out[idx] = c < L ? (float)(Hacc(L, c) + (p.col_off && c == p.col_off ? Kacc(L, c - 1) : 0.0)) : 0.f;
         } else if (idx >= 576) {
-            const int c = (int)idx - 576;
+            const int c = (int)idx - 576 + p.col_off;
             out[idx] = c < L - 1 ? (float)Kacc(L, c) : 0.f;
         } else out[idx] = 0.f;
     }

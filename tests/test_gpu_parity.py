@@ -328,6 +328,21 @@ def test_cfg3_side_sizes_exact_counts(L):
         assert go < 2 ** 53 and E0[b] == Eo and g[b] == go
 
 
+@pytest.mark.parametrize("L", [20, 26, 28])
+def test_large_counts_vs_golden(L):
+    """Degeneracies pinned by O-dp (u128 counts) beyond cfg 3's size: the > 2^53 regime closer to the
+    32x32 count, which itself stays property-pinned."""
+    gold = golden()
+    seeds = [s for s in (3000, 3001) if ("ising_count", L, s) in gold]
+    if not seeds:
+        pytest.skip("no stored oracle value")
+    Jh, Jv, _ = make_batch(L, seeds, "pmj")
+    E0, g = ttn.sweep_count(Jh, Jv)
+    for b, seed in enumerate(seeds):
+        Eo, go = gold[("ising_count", L, seed)]
+        assert E0[b] == Eo and count_ok(g[b], go)
+
+
 # ------------------------------------------------------------------ cfg 5: 18x18 Potts counting
 def test_cfg5_potts_18x18_count():
     gold = golden()
@@ -438,6 +453,54 @@ def test_z2_energy_vs_oracle(L, monkeypatch):
     with pytest.raises(ttn.TTNError) as e:
         ttn.Plan(2, ttn.CALL_ENERGY_Z2, Jh, Jv, h)
     assert e.value.status == 1
+
+
+@pytest.mark.parametrize("L", [12, 13, 14, 16, 17, 19, 21])
+def test_z2_count_vs_oracle(L, monkeypatch):
+    """h = 0: ttn_sweep_count on the flip-reduced half-state; the degeneracy is twice the half's count
+    (every ground state pairs with its global flip).  E0 and g bit-exact against O-dp (u128 counts);
+    identical to the full-state sweep; a non-zero field falls back to it."""
+    rng = np.random.default_rng(4500 + L)
+    B = 3
+    Jh = rng.integers(-2, 3, size=(B, L, L - 1)).astype(np.float32)
+    Jv = rng.integers(-2, 3, size=(B, L - 1, L)).astype(np.float32)
+    Jp, Jq, _ = make_batch(L, [3100], "pmj")
+    Jh[2], Jv[2] = Jp[0], Jq[0]
+    p = ttn.Plan(2, ttn.CALL_COUNT, Jh, Jv)
+    assert p.state_elements == 2 ** (L - 1)
+    p.launch(); E_z, g_z, _ = p.read(); p.close()
+    p = ttn.Plan(2, ttn.CALL_COUNT_Z2, Jh[2:], Jv[2:])
+    assert p.state_elements == 2 ** (L - 1)
+    p.launch(); E_1, g_1, _ = p.read(); p.close()
+    for b in range(B):
+        Eo, go, _ = oracle.dp_ising(L, Jh[b], Jv[b], None)
+        assert E_z[b] == Eo and count_ok(g_z[b], go) and go % 2 == 0
+    assert E_1[0] == E_z[2] and g_1[0] == g_z[2]
+    monkeypatch.setenv("TTN_DEBUG_Z2", "0")
+    p = ttn.Plan(2, ttn.CALL_COUNT, Jh, Jv)
+    assert p.state_elements == 2 ** L
+    p.launch(); E_f, g_f, _ = p.read(); p.close()
+    monkeypatch.delenv("TTN_DEBUG_Z2")
+    assert np.array_equal(E_f, E_z) and np.array_equal(g_f, g_z)
+    h = np.zeros((B, L, L), np.float32); h[0, 0, 0] = -1.0
+    p = ttn.Plan(2, ttn.CALL_COUNT, Jh, Jv, h)
+    assert p.state_elements == 2 ** L
+    p.launch(); E_h, g_h, _ = p.read(); p.close()
+    Eo, go, _ = oracle.dp_ising(L, Jh[0], Jv[0], h[0])
+    assert E_h[0] == Eo and g_h[0] == go and g_h[1] == g_z[1]
+    with pytest.raises(ttn.TTNError) as e:
+        ttn.Plan(2, ttn.CALL_COUNT_Z2, Jh, Jv, h)
+    assert e.value.status == 1
+
+
+def test_full_state_count_still_matches_golden(monkeypatch):
+    """cfg 3 seeds through the full-state counting sweep (flip reduction off), incl. a count above 2^53."""
+    gold = golden()
+    monkeypatch.setenv("TTN_DEBUG_Z2", "0")
+    Jh, Jv, _ = make_batch(24, [3000, 3001], "pmj")
+    E0, g = ttn.sweep_count(Jh, Jv)
+    for b, seed in enumerate((3000, 3001)):
+        assert E0[b] == gold[("ising_count", 24, seed)][0] and count_ok(g[b], gold[("ising_count", 24, seed)][1])
 
 
 @pytest.mark.parametrize("L", [16, 20, 24])

@@ -186,6 +186,11 @@ DIGIT_OF_BIT_Z2 = {(1, 0): [1 + d for d in [5, 6, 0, 1, 2, 3, 4]], (1, 1): [1 + 
                    (0, 0): [4, 5, 6, 0, 1, 2, 3], (0, 1): [4, 3, 2, 8, 7, 6, 5]}
 
 
+# flip-reduced counting geometry (GEOM_COUNT_Z2): column c >= 1 is digit c - 1 with the counting maps
+DIGIT_OF_BIT_COUNT_Z2 = {(1, 0): [1, 2, 3, 4, 5], (1, 1): [10, 9, 8, 7, 6],
+                         (0, 0): [0, 1, 2, 3, 4], (0, 1): [6, 5, 4, 3, 2]}
+
+
 def fused_to_gates(L, fpasses, count=False, i16=False, config=False, z2=False):
     """Check the structure of the micro-op program (layouts, register bits, rounds) and the
     three-point-stencil dependency rule; return the flat (r, c) gate sequence."""
@@ -193,8 +198,8 @@ def fused_to_gates(L, fpasses, count=False, i16=False, config=False, z2=False):
     grow = [1] * L                                   # rows complete per digit (row 0 needs no gate)
     for i, ps in enumerate(fpasses):
         a, Wt, low = ps["a"], ps["W"], ps["low"]
-        wl, wh, rb = (10, 7, 5) if count else ((13, 9, 8 if low else 7) if i16 else ((13, 9, 7) if z2 else (12, 9, 7)))
-        dmap = DIGIT_OF_BIT_COUNT if count else (DIGIT_OF_BIT_I16 if i16 else (DIGIT_OF_BIT_Z2 if z2 else DIGIT_OF_BIT))
+        wl, wh, rb = ((11, 7, 5) if z2 else (10, 7, 5)) if count else ((13, 9, 8 if low else 7) if i16 else ((13, 9, 7) if z2 else (12, 9, 7)))
+        dmap = (DIGIT_OF_BIT_COUNT_Z2 if z2 else DIGIT_OF_BIT_COUNT) if count else (DIGIT_OF_BIT_I16 if i16 else (DIGIT_OF_BIT_Z2 if z2 else DIGIT_OF_BIT))
         assert (low == 1 and a == 0 and Wt == wl) or (low == 0 and a >= (5 if i16 or z2 else 4) and Wt == wh)
         assert a + Wt <= L
         assert (ps["flags"] & 1) == (1 if i == 0 else 0)
@@ -307,7 +312,16 @@ def test_fused_z2_schedule_obeys_dependency_rule(L):
     assert sorted(r for r, c in flat if c == 0) == list(range(1, L))
 
 
-def replay_z2_half_state(L, gates, Jh, Jv):
+@pytest.mark.parametrize("L", [12, 13, 14, 17, 20, 24, 28, 32])
+def test_fused_count_z2_schedule_obeys_dependency_rule(L):
+    head, fpasses = parse_fused(describe(2, L, 5, fused=True))
+    assert int(head["L"]) == L
+    flat = fused_to_gates(L, fpasses, count=True, z2=True)
+    assert len(flat) == L * (L - 1) == len(set(flat))
+    assert sorted(r for r, c in flat if c == 0) == list(range(1, L))
+
+
+def replay_z2_half_state(L, gates, Jh, Jv, count=False):
     """numpy float64 replay of a flip-reduced schedule on the HALF state, restated from the symmetry:
     with h = 0 every intermediate state W of the sweep obeys W[s] = W[~s] (each gate (A2) PAPER.md:242
     and each diagonal (A4) PAPER.md:251 commutes with the global flip of Eq. (1)), so
@@ -318,7 +332,12 @@ def replay_z2_half_state(L, gates, Jh, Jv):
     sig = [np.ones(N)] + [1 - 2 * ((u >> (c - 1)) & 1) for c in range(1, L)]
     Kacc = np.cumsum(Jh, axis=0)
     V = np.zeros(N)
+    n = np.ones(N)                       # counts as float64: exact below 2^53 (the sizes replayed here)
     defer = 0.0
+
+    def oplus(xk, nk, xc, nc):           # Eq. (4): keep (+) candidate
+        return np.maximum(xk, xc), nk * (xk >= xc) + nc * (xc >= xk)
+
     for (r, c) in gates:
         J = Jv[r - 1, c]
         defer += J
@@ -328,18 +347,23 @@ def replay_z2_half_state(L, gates, Jh, Jv):
         if c < L - 1:
             rho = rho + Kacc[r - 1, c] * sig[c + 1]
         if c == 0:
-            V = np.maximum(V, V[(N - 1) ^ u] - 2 * J - 2 * rho)       # a' = max(a, b + m - 2 rho), b = W[~u]
+            co = (N - 1) ^ u                                          # a' = a (+) (b + m - 2 rho), b = W[~u]
+            V, n = oplus(V, n, V[co] - 2 * J - 2 * rho, n[co])
         else:
             ia = u[(u >> (c - 1)) & 1 == 0]
             ib = ia | (1 << (c - 1))
-            xa, xb = V[ia].copy(), V[ib].copy()
-            V[ia] = np.maximum(xa, xb - 2 * J - 2 * rho[ia])
-            V[ib] = np.maximum(xb, xa - 2 * J + 2 * rho[ia])
+            xa, xb, na, nb = V[ia].copy(), V[ib].copy(), n[ia].copy(), n[ib].copy()
+            V[ia], n[ia] = oplus(xa, na, xb - 2 * J - 2 * rho[ia], nb)
+            V[ib], n[ib] = oplus(xb, nb, xa - 2 * J + 2 * rho[ia], na)
     A = np.zeros(N)
     for c in range(L - 1):
         A += Kacc[L - 1, c] * sig[c] * sig[c + 1]
-    m = (V + A).max() + defer
-    return 0.0 if m == 0 else -m
+    x = V + A
+    m = x.max()
+    E0 = 0.0 if m + defer == 0 else -(m + defer)
+    if count:
+        return E0, 2 * int(n[x == m].sum())       # the stored half holds one of every flip pair
+    return E0
 
 
 @pytest.mark.parametrize("L", [14, 15, 17])
@@ -356,9 +380,23 @@ def test_fused_z2_schedule_replay_matches_oracle(L):
     assert abs(replay_z2_half_state(L, flat, Jh, Jv) - Eo) <= 1e-9 * abs(Eo)
 
 
+@pytest.mark.parametrize("L", [12, 13, 15])
+def test_fused_count_z2_schedule_replay_matches_oracle(L):
+    _, fpasses = parse_fused(describe(2, L, 5, fused=True))
+    flat = fused_to_gates(L, fpasses, count=True, z2=True)
+    rng = np.random.default_rng(300 + L)
+    for trial in range(2):
+        Jh = rng.integers(-1, 2, size=(L, L - 1)).astype(float)       # many ties
+        Jv = rng.integers(-1, 2, size=(L - 1, L)).astype(float)
+        Eo, go, _ = oracle.dp_ising(L, Jh, Jv, None)
+        assert go < 2 ** 53
+        assert replay_z2_half_state(L, flat, Jh, Jv, count=True) == (Eo, go)
+
+
 def test_z2_describe_falls_back_below_two_tiles():
     """L = 13: the half-state is a single (self-complementary) LOW tile: the plain schedule runs."""
     assert describe(2, 13, 4, fused=True) == describe(2, 13, 0, fused=True)
+    assert describe(2, 11, 5, fused=True) == describe(2, 11, 1, fused=True)
 
 
 @pytest.mark.parametrize("L", [12, 13, 16, 20, 21, 22, 28])
