@@ -27,7 +27,7 @@
  * is NO CPU fallback: without a CUDA device every compute call returns TTN_ECUDA.
  *
  * h = 0 (NULL or all zero): Eq. (1) is invariant under the global flip sigma -> -sigma, and so is
- * every intermediate state of the sweep; ttn_sweep_energy and ttn_sweep_count then store only the
+ * every intermediate state of the sweep; ttn_sweep_energy[_i16] and ttn_sweep_count then store only the
  * half of the state vector with column 0 up (2^(L-1) elements) and apply the column-0 gates as a
  * pairing of every element with its complement -- half the memory, bytes and arithmetic,
  * identical results, the degeneracy being twice the half's count.  Any
@@ -146,7 +146,8 @@ typedef enum {
        L < 14 run the plain sweep).  TTN_CALL_ENERGY selects it by itself when h = 0; this kind exists
        for ttn_plan_describe and for tests. */
     TTN_CALL_ENERGY_Z2 = 4,
-    TTN_CALL_COUNT_Z2 = 5       /* the same for TTN_CALL_COUNT (L < 12 runs the plain sweep) */
+    TTN_CALL_COUNT_Z2 = 5,      /* the same for TTN_CALL_COUNT (L < 12 runs the plain sweep) */
+    TTN_CALL_ENERGY_I16_Z2 = 6  /* the same for TTN_CALL_ENERGY_I16 (L < 15 runs the plain i16 sweep) */
 } ttn_call;
 
 ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const float* Jv,

@@ -124,6 +124,7 @@ const ttn::FusedGeom* z2_geom(int q, int L, ttn_call call, bool has_field, const
     if (dbg.fused == 0 || dbg.z2 == 0 || q != 2 || has_field) return nullptr;
     if ((call == TTN_CALL_ENERGY || call == TTN_CALL_ENERGY_Z2) && L >= ttn::GEOM_F32_Z2.WLOW + 1) return &ttn::GEOM_F32_Z2;
     if ((call == TTN_CALL_COUNT || call == TTN_CALL_COUNT_Z2) && L >= ttn::GEOM_COUNT_Z2.WLOW + 1) return &ttn::GEOM_COUNT_Z2;
+    if ((call == TTN_CALL_ENERGY_I16 || call == TTN_CALL_ENERGY_I16_Z2) && L >= ttn::GEOM_I16_Z2.WLOW + 1) return &ttn::GEOM_I16_Z2;
     return nullptr;
 }
 
@@ -302,7 +303,9 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
     }
     pp.L_cols = P->L;
     if (P->i16) {           // the kernel sees the lattice of 32-bit words: column c >= 1 = word digit c - 1
-        pp.L = P->L - 1; pp.a = ps.low ? 0 : ps.a - 1;
+        const int off = P->z2 ? 2 : 1;     // (flip-reduced: the half-state's column 1 is the half of a word)
+        pp.L = P->L - off; pp.a = ps.low ? 0 : ps.a - off;
+        pp.L_cols = P->L - (off - 1);      // digits of the element index
         pp.inst_stride = y.NS >> 1; pp.tiles_per_inst = y.NS >> 13;
         pp.src = pp.state; pp.src_stride = pp.inst_stride;
     } else if (P->z2) {     // the kernel sees the half-state over columns 1 .. L-1: column c = digit c - 1
@@ -368,7 +371,10 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
         const bool red = (ps.flags & ttn::PASS_REDUCE) != 0;
 #define TTN_FUSED_LAUNCH(LOW_, ELEM_, RED_)                                                                             \
         ttn::fused_pass_kernel<LOW_, ELEM_, false, RED_><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(LOW_, ELEM_), st>>>(pp)
-        if (P->i16) {
+        if (P->i16 && P->z2 && ps.low) {
+            if (red) ttn::fused_pass_kernel<true, 1, false, true, true><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(true, 1), st>>>(pp);
+            else ttn::fused_pass_kernel<true, 1, false, false, true><<<(unsigned)grid, nw * 32, ttn::fsmem_bytes(true, 1), st>>>(pp);
+        } else if (P->i16) {
             if (ps.low) { if (red) TTN_FUSED_LAUNCH(true, 1, true); else TTN_FUSED_LAUNCH(true, 1, false); }
             else { if (red) TTN_FUSED_LAUNCH(false, 1, true); else TTN_FUSED_LAUNCH(false, 1, false); }
         } else if (P->z2 && ps.low) {      // warp pairs on complementary tiles, flip gates
@@ -495,13 +501,15 @@ static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
     q.final_tab = reinterpret_cast<float*>(P->ws + y.f_final);
     const ttn::FusedPass& lastp = fp.passes.back();
     q.fin_low = lastp.low; q.fin_layout = lastp.last_layout; q.fin_a = lastp.a;
-    if (P->i16 || P->z2) q.fin_a = lastp.low ? 0 : lastp.a - 1;        // word digit / half-state digit
+    if (P->i16 || P->z2) q.fin_a = lastp.low ? 0 : lastp.a - ((P->i16 && P->z2) ? 2 : 1);   // word digit / half-state digit
     q.col_off = P->z2 ? 1 : 0;
     long work = ttn::FFINAL_FLOATS; if (q.n_gates > work) work = q.n_gates;
     dim3 grid((unsigned)((work + 255) / 256), (unsigned)P->batch);
     if (P->i16) {
         ttn::fused16_prep_kernel<<<grid, 256, 0, st>>>(q);
         TTN_CUDA(cudaGetLastError());
+        TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 1, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true, 1)));
+        TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 1, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true, 1)));
         TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 1, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true, 1)));
     TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 1, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true, 1)));
         TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false, 1, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false, 1)));
@@ -589,12 +597,12 @@ long ttn_plan_describe(int q, int L, ttn_call call, char* buf, size_t n) {
     if (!limits_ok(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) return -1;
     std::string s;
     const DebugCfg dbg = read_debug();
-    if (call == TTN_CALL_ENERGY_Z2 || call == TTN_CALL_COUNT_Z2) {   // the schedules the calls run when h = 0
+    if (call == TTN_CALL_ENERGY_Z2 || call == TTN_CALL_COUNT_Z2 || call == TTN_CALL_ENERGY_I16_Z2) {   // the schedules the calls run when h = 0
         if (const ttn::FusedGeom* G = z2_geom(q, L, call, false, dbg)) {
             ttn::FusedPlan fp = ttn::make_fused_plan(L, ttn::FMAX_GATES, *G);
             if (fp.ok) s = ttn::describe_fused(fp);
         }
-        if (s.empty()) call = call == TTN_CALL_ENERGY_Z2 ? TTN_CALL_ENERGY : TTN_CALL_COUNT;
+        if (s.empty()) call = call == TTN_CALL_ENERGY_Z2 ? TTN_CALL_ENERGY : (call == TTN_CALL_COUNT_Z2 ? TTN_CALL_COUNT : TTN_CALL_ENERGY_I16);
     }
     if (call == TTN_CALL_ENERGY_I16 && i16_eligible(q, L, dbg)) {
         ttn::FusedPlan fp = ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_I16);
@@ -622,12 +630,13 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     if (q != 2 && q != 3) return fail(TTN_EINVAL, "q must be 2 or 3");
     if (L < 1 || batch < 1) return fail(TTN_EINVAL, "L and batch must be >= 1");
     if (call != TTN_CALL_ENERGY && call != TTN_CALL_COUNT && call != TTN_CALL_CONFIG && call != TTN_CALL_ENERGY_I16 &&
-        call != TTN_CALL_ENERGY_Z2 && call != TTN_CALL_COUNT_Z2)
+        call != TTN_CALL_ENERGY_Z2 && call != TTN_CALL_COUNT_Z2 && call != TTN_CALL_ENERGY_I16_Z2)
         return fail(TTN_EINVAL, "bad call kind");
-    const bool want_z2 = (call == TTN_CALL_ENERGY_Z2 || call == TTN_CALL_COUNT_Z2);
+    const bool want_z2 = (call == TTN_CALL_ENERGY_Z2 || call == TTN_CALL_COUNT_Z2 || call == TTN_CALL_ENERGY_I16_Z2);
     const DebugCfg dbg = read_debug();
     bool i16 = false;
-    if (call == TTN_CALL_ENERGY_I16) {
+    const bool want_i16 = (call == TTN_CALL_ENERGY_I16 || call == TTN_CALL_ENERGY_I16_Z2);
+    if (want_i16) {
         if (q != 2) return fail(TTN_EINVAL, "Tropical<i16> is an Ising call");
         i16 = i16_eligible(q, L, dbg);      // small lattices run the f32 path (identical results)
     }
@@ -642,7 +651,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     for (size_t i = 0; i < nv; ++i) if (!std::isfinite(Jv[i])) return fail(TTN_EINVAL, "non-finite Jv[%zu]", i);
     if (h) for (size_t i = 0; i < nf; ++i) if (!std::isfinite(h[i])) return fail(TTN_EINVAL, "non-finite h[%zu]", i);
 
-    if (call == TTN_CALL_ENERGY_I16) {
+    if (want_i16) {
         // exactness: integer-valued couplings whose absolute sum keeps every intermediate inside 16 bits
         for (int b = 0; b < batch; ++b) {
             double tot = 0.0;
@@ -661,7 +670,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     if (h) for (size_t i = 0; i < nf && !field; ++i) field = (h[i] != 0.0f);
     if (want_z2 && field) return fail(TTN_EINVAL, "the flip reduction needs h = 0");
     const ttn::FusedGeom* zg = z2_geom(q, L, call, field, dbg);
-    if (want_z2) call = count ? TTN_CALL_COUNT : TTN_CALL_ENERGY;  // lattices too small for it run the plain sweep
+    if (want_z2) call = count ? TTN_CALL_COUNT : (want_i16 ? TTN_CALL_ENERGY_I16 : TTN_CALL_ENERGY);  // lattices too small for it run the plain sweep
     Layout lay = make_layout(q, L, count, config, batch, dbg, i16, zg != nullptr);
     if (workspace_bytes < lay.total)
         return fail(TTN_ENOMEM, "workspace too small: %zu < %zu", workspace_bytes, lay.total);
@@ -686,7 +695,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     }
     P->ws = static_cast<unsigned char*>(workspace);
     if (i16) {
-        P->fplan = ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_I16);
+        P->fplan = ttn::make_fused_plan(L, ttn::FMAX_GATES, zg ? *zg : ttn::GEOM_I16);
         P->fused = P->fplan.ok;
         if (!P->fused) { delete P; return fail(TTN_EUNSUPPORTED, "no Tropical<i16> schedule"); }
     } else if (zg) {

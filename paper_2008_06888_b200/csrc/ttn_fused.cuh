@@ -259,6 +259,45 @@ __device__ __forceinline__ void flipgate(float (&v)[128], float4* myreg, const f
     pair_sync(warp);
 }
 
+// Tropical<i16> form: column 1 is the half of a word, so ~u = the OTHER half of the complement word,
+// and the neighbour bit of the flip gate is the half itself: one PRMT + one VIADDMNMX.S16x2 per word
+// against the packed constant kpk = (lo: kf[0], hi: kf[1]).
+template <int LAYOUT>
+__device__ __forceinline__ void flipgate16(float (&v)[128], float4* myreg, const float4* preg, const int lane,
+                                           const int warp, const unsigned kpk) {
+    __syncwarp();
+    if (LAYOUT == 0) {
+        float4* p = myreg + 33 * lane;
+#pragma unroll
+        for (int q = 0; q < 32; ++q) p[q] = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+    } else {
+        float4* p = myreg + lane;
+#pragma unroll
+        for (int q = 0; q < 32; ++q) p[33 * rev5c(q)] = make_float4(v[4 * q], v[4 * q + 2], v[4 * q + 1], v[4 * q + 3]);
+    }
+    pair_sync(warp);
+    auto upd = [&](float& x, float pw) {
+        const unsigned sw = __byte_perm(__float_as_uint(pw), 0u, 0x1032);       // the partner's other half
+        x = __uint_as_float(__viaddmax_s16x2(sw, kpk, __float_as_uint(x)));
+    };
+    if (LAYOUT == 0) {
+        const float4* p = preg + 33 * (31 - lane);
+#pragma unroll
+        for (int q = 0; q < 32; ++q) {
+            const float4 t = p[31 - q];
+            upd(v[4 * q], t.w); upd(v[4 * q + 1], t.z); upd(v[4 * q + 2], t.y); upd(v[4 * q + 3], t.x);
+        }
+    } else {
+        const float4* p = preg + (31 - lane);
+#pragma unroll
+        for (int q = 0; q < 32; ++q) {
+            const float4 t = p[33 * rev5c(31 - q)];
+            upd(v[4 * q], t.w); upd(v[4 * q + 1], t.y); upd(v[4 * q + 2], t.z); upd(v[4 * q + 3], t.x);
+        }
+    }
+    pair_sync(warp);
+}
+
 // ---- Tropical<i16> (the paper's own Int16 choice for +-J) -----------
 // Two elements per 32-bit word: column 0 of the lattice row is the HALF of a word (low half =
 // bit 0 = sigma +1), the kernel's tile geometry applies to the word index.  One VIADDMNMX.S16x2
@@ -665,16 +704,19 @@ __global__ void __launch_bounds__(256) fused16_prep_kernel(const FusedPrepParams
             const double rho = H + (nl ? -Kl : Kl) + (nh ? -Kr : Kr);
             return side == 0 ? m - 2.0 * rho : m + 2.0 * rho;
         };
-        if (K == 7) {                 // column 0: kp[n] = (lo: ka, hi: kb), n = bit of column 1
+        if (g & GATE_RC_FLIP) {       // Z2 flip gate on column 0; its neighbour bit (column 1) is the half itself
             for (int i = 0; i < 8; ++i) out[i] = 0u;
+            out[0] = pack(m - 2.0 * Kr, m + 2.0 * Kr);
+        } else if (K == 7) {          // the half column (0; Z2: 1, left neighbour sigma_0 = +1): kp[n] = (lo: ka, hi: kb),
+            for (int i = 0; i < 8; ++i) out[i] = 0u;                  // n = bit of the next column
             for (int n = 0; n < 2; ++n) out[n] = pack(kval(0, 0, n), kval(1, 0, n));
         } else {
             for (int side = 0; side < 2; ++side)
                 for (int np = 0; np < 2; ++np)
                     for (int nq = 0; nq < 2; ++nq) {
                         const int nl = mirrored ? nq : np, nh = mirrored ? np : nq;
-                        // column 1: the left neighbour is the half of the word itself
-                        out[side * 4 + np * 2 + nq] = c == 1 ? pack(kval(side, 0, nh), kval(side, 1, nh))
+                        // the column after the half column: the left neighbour is the half of the word itself
+                        out[side * 4 + np * 2 + nq] = c == 1 + p.col_off ? pack(kval(side, 0, nh), kval(side, 1, nh))
                                                              : pack(kval(side, nl, nh), kval(side, nl, nh));
                     }
         }
@@ -685,7 +727,7 @@ __global__ void __launch_bounds__(256) fused16_prep_kernel(const FusedPrepParams
             const int var = (int)idx >> 7, j = (int)idx & 127, tl = var & 1, th = var >> 1;
             const bool low = p.fin_low != 0;
             const int d0 = low ? (p.fin_layout == 0 ? 0 : 5) : (p.fin_layout == 0 ? 0 : 2);
-            const int x0 = 1 + p.fin_a + d0;                    // first register COLUMN (fin_a = word digit)
+            const int x0 = p.col_off + 1 + p.fin_a + d0;        // first register COLUMN (fin_a = word digit)
             int bits[F_RB];
             for (int i = 0; i < F_RB; ++i) bits[i] = (j >> fused_bit_of_digit(low, p.fin_layout, d0 + i)) & 1;
             double acc = 0;
@@ -696,13 +738,14 @@ __global__ void __launch_bounds__(256) fused16_prep_kernel(const FusedPrepParams
             }
             acc += (th == bits[F_RB - 1]) ? Kacc(L, x0 + F_RB - 1) : -Kacc(L, x0 + F_RB - 1);
             const double kl = Kacc(L, x0 - 1);
-            const int tl0 = x0 == 1 ? 0 : tl, tl1 = x0 == 1 ? 1 : tl;     // column 0 = the half
+            const int tl0 = x0 == 1 + p.col_off ? 0 : tl, tl1 = x0 == 1 + p.col_off ? 1 : tl;     // left neighbour = the half
             reinterpret_cast<unsigned*>(out)[idx] = pack(acc + ((tl0 == bits[0]) ? kl : -kl), acc + ((tl1 == bits[0]) ? kl : -kl));
         } else if (idx < 576) {
-            const int c = (int)idx - 512;
-            out[idx] = c < L ? (float)Hacc(L, c) : 0.f;
+            // per DIGIT of the element index; Z2: digit 0 = column 1 also carries K_0 sigma_0 sigma_1 = K_0 sigma_1
+            const int c = (int)idx - 512 + p.col_off;
+            out[idx] = c < L ? (float)(Hacc(L, c) + (p.col_off && c == p.col_off ? Kacc(L, c - 1) : 0.0)) : 0.f;
         } else {
-            const int c = (int)idx - 576;
+            const int c = (int)idx - 576 + p.col_off;
             out[idx] = c < L - 1 ? (float)Kacc(L, c) : 0.f;
         }
     }

@@ -16,7 +16,7 @@ TROPICAL_F32 = 0
 COUNTING_F32_F64 = 1
 TROPICAL_I16 = 2
 CALL_ENERGY, CALL_COUNT, CALL_CONFIG, CALL_ENERGY_I16 = 0, 1, 2, 3
-CALL_ENERGY_Z2, CALL_COUNT_Z2 = 4, 5      # CALL_ENERGY / CALL_COUNT with the h = 0 flip-reduced half-state required (ttn.h)
+CALL_ENERGY_Z2, CALL_COUNT_Z2, CALL_ENERGY_I16_Z2 = 4, 5, 6      # CALL_ENERGY / CALL_COUNT / CALL_ENERGY_I16 with the h = 0 flip-reduced half-state required (ttn.h)
 
 EXPORTS = [
     "ttn_workspace_bytes", "ttn_sweep_energy", "ttn_sweep_energy_i16", "ttn_sweep_count", "ttn_ground_config",
@@ -193,7 +193,7 @@ class Plan:
 
 
 def _mode_of(call: int) -> int:
-    return {CALL_COUNT: COUNTING_F32_F64, CALL_COUNT_Z2: COUNTING_F32_F64, CALL_ENERGY_I16: TROPICAL_I16}.get(call, TROPICAL_F32)
+    return {CALL_COUNT: COUNTING_F32_F64, CALL_COUNT_Z2: COUNTING_F32_F64, CALL_ENERGY_I16: TROPICAL_I16, CALL_ENERGY_I16_Z2: TROPICAL_I16}.get(call, TROPICAL_F32)
 
 
 def _one_call(fn_name, q, call, Jh, Jv, h, workspace, stream):

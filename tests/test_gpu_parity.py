@@ -503,6 +503,37 @@ def test_full_state_count_still_matches_golden(monkeypatch):
         assert E0[b] == gold[("ising_count", 24, seed)][0] and count_ok(g[b], gold[("ising_count", 24, seed)][1])
 
 
+@pytest.mark.parametrize("L", [15, 16, 17, 19, 21])
+def test_z2_i16_energy_vs_oracle(L, monkeypatch):
+    """h = 0: Tropical<i16> on the flip-reduced half-state (column 1 is the half of a word, the
+    column-0 gate pairs a word with the swapped halves of its complement word)."""
+    rng = np.random.default_rng(4600 + L)
+    B = 3
+    Jh = rng.integers(-3, 4, size=(B, L, L - 1)).astype(np.float32)
+    Jv = rng.integers(-3, 4, size=(B, L - 1, L)).astype(np.float32)
+    p = ttn.Plan(2, ttn.CALL_ENERGY_I16, Jh, Jv)
+    assert p.state_elements == 2 ** (L - 1)
+    p.launch(); E_z, _, _ = p.read(); p.close()
+    p = ttn.Plan(2, ttn.CALL_ENERGY_I16_Z2, Jh[:1], Jv[:1])
+    p.launch(); E_1, _, _ = p.read(); p.close()
+    for b in range(B):
+        assert E_z[b] == oracle.dp_ising(L, Jh[b], Jv[b], None, count=False)[0]
+    assert E_1[0] == E_z[0]
+    monkeypatch.setenv("TTN_DEBUG_Z2", "0")
+    p = ttn.Plan(2, ttn.CALL_ENERGY_I16, Jh, Jv)
+    assert p.state_elements == 2 ** L
+    p.launch(); E_f, _, _ = p.read(); p.close()
+    monkeypatch.delenv("TTN_DEBUG_Z2")
+    assert np.array_equal(E_f, E_z)
+
+
+def test_full_state_i16_still_matches_golden(monkeypatch):
+    gold = golden()
+    monkeypatch.setenv("TTN_DEBUG_Z2", "0")
+    Jh, Jv, _ = make_batch(28, [4000], "pmj")
+    assert ttn.sweep_energy_i16(Jh, Jv)[0] == gold[("ising_energy", 28, 4000)][0]
+
+
 @pytest.mark.parametrize("L", [16, 20, 24])
 def test_z2_gaussian_couplings_f32_tolerance(L):
     """Gaussian couplings, no field, through the flip-reduced sweep: |dE| <= 1e-5 |E0| against O-dp."""

@@ -191,6 +191,12 @@ DIGIT_OF_BIT_COUNT_Z2 = {(1, 0): [1, 2, 3, 4, 5], (1, 1): [10, 9, 8, 7, 6],
                          (0, 0): [0, 1, 2, 3, 4], (0, 1): [6, 5, 4, 3, 2]}
 
 
+# flip-reduced Tropical<i16> geometry (GEOM_I16_Z2): column 1 is the half of a word (pseudo bit 7),
+# column c >= 2 is word digit c - 2
+DIGIT_OF_BIT_I16_Z2 = {(1, 0): [2 + d for d in [5, 6, 0, 1, 2, 3, 4]] + [1], (1, 1): [2 + d for d in [6, 5, 11, 10, 9, 8, 7]] + [1],
+                       (0, 0): [4, 5, 6, 0, 1, 2, 3], (0, 1): [4, 3, 2, 8, 7, 6, 5]}
+
+
 def fused_to_gates(L, fpasses, count=False, i16=False, config=False, z2=False):
     """Check the structure of the micro-op program (layouts, register bits, rounds) and the
     three-point-stencil dependency rule; return the flat (r, c) gate sequence."""
@@ -198,9 +204,11 @@ def fused_to_gates(L, fpasses, count=False, i16=False, config=False, z2=False):
     grow = [1] * L                                   # rows complete per digit (row 0 needs no gate)
     for i, ps in enumerate(fpasses):
         a, Wt, low = ps["a"], ps["W"], ps["low"]
-        wl, wh, rb = ((11, 7, 5) if z2 else (10, 7, 5)) if count else ((13, 9, 8 if low else 7) if i16 else ((13, 9, 7) if z2 else (12, 9, 7)))
-        dmap = (DIGIT_OF_BIT_COUNT_Z2 if z2 else DIGIT_OF_BIT_COUNT) if count else (DIGIT_OF_BIT_I16 if i16 else (DIGIT_OF_BIT_Z2 if z2 else DIGIT_OF_BIT))
-        assert (low == 1 and a == 0 and Wt == wl) or (low == 0 and a >= (5 if i16 or z2 else 4) and Wt == wh)
+        wl, wh, rb = ((11, 7, 5) if z2 else (10, 7, 5)) if count else ((14 if z2 else 13, 9, 8 if low else 7) if i16 else ((13, 9, 7) if z2 else (12, 9, 7)))
+        dmap = (DIGIT_OF_BIT_COUNT_Z2 if z2 else DIGIT_OF_BIT_COUNT) if count else \
+               ((DIGIT_OF_BIT_I16_Z2 if z2 else DIGIT_OF_BIT_I16) if i16 else (DIGIT_OF_BIT_Z2 if z2 else DIGIT_OF_BIT))
+        amin = 4 + (1 if i16 else 0) + (1 if z2 else 0)
+        assert (low == 1 and a == 0 and Wt == wl) or (low == 0 and a >= amin and Wt == wh)
         assert a + Wt <= L
         assert (ps["flags"] & 1) == (1 if i == 0 else 0)
         last = i == len(fpasses) - 1 and not config
@@ -321,6 +329,15 @@ def test_fused_count_z2_schedule_obeys_dependency_rule(L):
     assert sorted(r for r, c in flat if c == 0) == list(range(1, L))
 
 
+@pytest.mark.parametrize("L", [15, 16, 17, 20, 24, 28, 32, 34])
+def test_fused_i16_z2_schedule_obeys_dependency_rule(L):
+    head, fpasses = parse_fused(describe(2, L, 6, fused=True))
+    assert int(head["L"]) == L
+    flat = fused_to_gates(L, fpasses, i16=True, z2=True)
+    assert len(flat) == L * (L - 1) == len(set(flat))
+    assert sorted(r for r, c in flat if c == 0) == list(range(1, L))
+
+
 def replay_z2_half_state(L, gates, Jh, Jv, count=False):
     """numpy float64 replay of a flip-reduced schedule on the HALF state, restated from the symmetry:
     with h = 0 every intermediate state W of the sweep obeys W[s] = W[~s] (each gate (A2) PAPER.md:242
@@ -397,6 +414,7 @@ def test_z2_describe_falls_back_below_two_tiles():
     """L = 13: the half-state is a single (self-complementary) LOW tile: the plain schedule runs."""
     assert describe(2, 13, 4, fused=True) == describe(2, 13, 0, fused=True)
     assert describe(2, 11, 5, fused=True) == describe(2, 11, 1, fused=True)
+    assert describe(2, 14, 6, fused=True) == describe(2, 14, 3, fused=True)
 
 
 @pytest.mark.parametrize("L", [12, 13, 16, 20, 21, 22, 28])
