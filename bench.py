@@ -2,10 +2,12 @@
 """bench.py -- headline benchmark of the tropical transfer sweep (BASELINE.json metric:
 "Sweep time per instance & achieved HBM GB/s (frac. of peak), LxL tropical sweep").
 
-Workload at N=1: BASELINE.json configs[3] -- 32x32 +-J Ising, h=0, Tropical<f32> energy, one
-2^32-entry (16 GiB) state swept in place -- the configuration north_star's ">= 60 % of the HBM
-roofline on the 2^28..2^32-entry sweeps" is quoted on.  A "step" is one whole sweep (every pass
-kernel + the final reduction) of one instance per GPU.  With N GPUs each rank sweeps its own
+Workload at N=1: BASELINE.json configs[3] -- 32x32 +-J Ising, h=0, Tropical<f32> energy, the
+2^32-entry state vector swept in place row by row -- the configuration north_star's ">= 60 % of
+the HBM roofline on the 2^28..2^32-entry sweeps" is quoted on.  With h = 0 the library stores the
+flip-symmetric half of that vector (2^31 elements, 8 GiB; include/ttn.h) --
+the roofline below is still quoted against north_star's full-vector bytes.  A "step" is one whole
+sweep (every pass kernel + the final reduction) of one instance per GPU.  With N GPUs each rank sweeps its own
 instance (seed 4000 + rank): replicas, no data-path collective, "scaling": "weak".
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--L 32] [--impl ours|reference]
@@ -19,7 +21,9 @@ instance (seed 4000 + rank): replicas, no data-path collective, "
            (row 0 write-only, last row read-only) over the measured sweep time,
            against the measured copy bandwidth in MEASURED_PEAKS.json.
 `cpu_baseline`: the CPU oracle (oracle/, unmodified) timed on the host cores on a bounded
-           sample, scaled to the metric's unit by the update count (L-1)*L*2^L.
+           sample: one full sweep of a smaller lattice, reported UNSCALED next to the GPU time for
+           that same lattice; `value` is its extrapolation to the workload by the update count
+           (L-1)*L*2^L and is labelled as such.
 """
 from __future__ import annotations
 
@@ -112,7 +116,7 @@ class ClockSampler(threading.Thread):
                         self.reasons.add(n)
             except Exception:
                 pass
-            self._stop_evt.wait(0.2)
+            self._stop_evt.wait(0.1)
 
     def stop(self):
         self._stop_evt.set()
@@ -125,6 +129,43 @@ class ClockSampler(threading.Thread):
 def workload_name(L: int) -> str:
     return (f"{L}x{L} +-J Ising (p=0.5, h=0) Tropical<f32> energy sweep, "
             f"2^{L}-entry state in place, 1 instance per GPU (seed 4000+rank)")
+
+
+# The oracle's one full-size run: 32x32 +-J seed 4000, O-dp, 34 GB frontier.
+ORACLE_FULL_32 = {"seconds": 4776, "cores": 6, "where": "build box, round 1 (tests/golden/oracle_values.txt ising_energy 32 4000)"}
+
+
+def ncu_traffic_per_launch(summary_csv: str, kernel_substr: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch, averaged over the launches of the
+    kernel in a committed `ncu --set full` summary (profiles/*.csv: one row per metric -- name, unit,
+    one column per captured launch; units byte / Kbyte / Mbyte / Gbyte).  None when the file is
+    absent: the number is never a literal in this script."""
+    path = os.path.join(ROOT, "profiles", summary_csv)
+    if not os.path.exists(path):
+        return None, None
+    import csv
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    rows = {r[0]: r for r in csv.reader(open(path)) if r}
+    names = rows.get("Kernel Name")
+    rd, wr = rows.get("dram__bytes_read.sum"), rows.get("dram__bytes_write.sum")
+    if not (names and rd and wr):
+        return None, None
+    vals = [float(rd[i]) * scale[rd[1]] + float(wr[i]) * scale[wr[1]]
+            for i in range(2, len(names)) if kernel_substr in names[i]]
+    return (sum(vals) / len(vals) if vals else None), "profiles/" + summary_csv
+
+
+def time_plan(torch, plan, reps=3, warm=1):
+    for _ in range(warm):
+        plan.launch()
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(reps):
+        plan.launch()
+    b.record()
+    torch.cuda.synchronize()
+    return a.elapsed_time(b) / reps
 
 
 def run_reference(args):
@@ -192,6 +233,26 @@ def other_configs(torch):
             torch.cuda.empty_cache()
         except ttn.TTNError as e:
             rows[name] = {"unavailable": str(e)}
+    # the rest of north_star's "2^28..2^32-entry" band (f32, +-J, h = 0: flip-reduced like the headline) and
+    # the paper's own headline workload, 32x32 GAUSSIAN couplings and fields in Float32 (PAPER.md:118, 282:
+    # 590 s on its GPU): fields break the flip symmetry, so this leg sweeps the full 2^32-entry state
+    for name, Lc, kind, seed in (("band_28x28_pmj_f32", 28, "pmj", 4000), ("band_30x30_pmj_f32", 30, "pmj", 4000),
+                                 ("paper_32x32_gauss_J_and_h_f32", 32, "gauss", 2032)):
+        try:
+            Jh, Jv, h = make_batch(Lc, [seed], kind, fields=(kind == "gauss"))
+            plan = ttn.Plan(2, ttn.CALL_ENERGY, Jh, Jv, h)
+            ms = time_plan(torch, plan, reps=3)
+            E = float(plan.read()[0][0])
+            rows[name] = {"ms_per_instance": ms, "E0": E, "hbm_passes": plan.num_passes, "launches": plan.num_launches,
+                          "state_elements_stored": plan.state_elements,
+                          "hbm_roofline_frac": bytes_min(Lc) / (peak * 1e9) / (ms * 1e-3),
+                          "alu_roofline_frac": float(Lc) * (Lc - 1) * plan.state_elements / (ms * 1e-3) / (148 * 64 * 1.965e9)}
+            plan.close()
+            del plan
+            torch.cuda.empty_cache()
+        except (ttn.TTNError, RuntimeError) as e:
+            rows[name] = {"unavailable": str(e).splitlines()[0][:200]}
+            torch.cuda.empty_cache()
     # +-J chimera graph, L x L unit cells (8 L^2 spins), Tropical<i16>, through the
     # one-call C ABI (host couplings; table upload and the read-back of E0 are inside the timed region).
     # Roofline: one read + one write of the 2^(4L+4) int16 state per unit cell, against the MEASURED copy
@@ -224,28 +285,34 @@ def other_configs(torch):
     return rows
 
 
-def cpu_baseline(L_target: int, L_sample: int):
+def cpu_baseline(L_target: int, L_sample: int, gpu_ms_same_L=None):
+    """O-dp as it stands on the host cores: ONE full sweep of an L_sample x L_sample +-J instance
+    (a measurement), next to the GPU time for the same instance; `value` extrapolates it to the
+    workload by the update count -- an under-estimate, since the 32x32 frontier (34 GB) is far out
+    of cache while the sample's is not: the one measured full-size run is quoted beside it."""
     import oracle
     Jh, Jv, _ = make_batch(L_sample, [4000], "pmj")
     t = time.perf_counter()
-    oracle.dp_ising(L_sample, Jh[0], Jv[0], None, count=False)
+    E = oracle.dp_ising(L_sample, Jh[0], Jv[0], None, count=False)[0]
     dt = time.perf_counter() - t
     val = dt / updates(L_sample) * updates(L_target) * 1e3
     return {"value": val, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-            "sample": f"one full O-dp sweep of a {L_sample}x{L_sample} +-J instance ({dt:.1f} s), scaled by "
-                      f"(L-1)L2^L updates to {L_target}x{L_target}",
-            "sample_seconds": dt}
+            "extrapolated": True,
+            "sample": f"one full O-dp sweep of a {L_sample}x{L_sample} +-J instance (seed 4000), measured {dt:.1f} s; "
+                      f"`value` scales it by (L-1)L2^L updates to {L_target}x{L_target}",
+            "measured": {"L": L_sample, "ms": dt * 1e3, "E0": E, "gpu_ms_same_instance": gpu_ms_same_L},
+            "full_size_oracle_run": ORACLE_FULL_32 if L_target == 32 else None}
 
 
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--L", type=int, default=32)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--ref-L", type=int, default=22, dest="ref_L")
-    ap.add_argument("--cpu-L", type=int, default=24, dest="cpu_L")
+    ap.add_argument("--ref-L", type=int, default=24, dest="ref_L")
+    ap.add_argument("--cpu-L", type=int, default=28, dest="cpu_L")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true", dest="no_other_configs")
     args = ap.parse_args()
@@ -326,11 +393,19 @@ def main():
         torch.cuda.synchronize()
         E16 = p16.read()[0][0]
         assert E16 == E_dev, (E16, E_dev)
-        i16 = {"ms_per_instance": a.elapsed_time(b) / 3, "hbm_passes": p16.num_passes, "state_bytes": 2 * 2 ** L,
+        i16 = {"ms_per_instance": a.elapsed_time(b) / 3, "hbm_passes": p16.num_passes, "state_bytes": 2 * p16.state_elements,
                "note": "ttn_sweep_energy_i16 (SURVEY.md NEXT-1), same instance, E0 identical; not the headline metric"}
         p16.close()
     except ttn.TTNError as e:      # e.g. L below the i16 path's limits
         i16 = {"unavailable": str(e)}
+
+    # ---- the GPU time for the very instance the CPU baseline sweeps (same L, same seed)
+    gpu_same = None
+    if rank == 0 and not args.no_cpu_baseline:
+        Jc, Jd, _ = make_batch(args.cpu_L, [4000], "pmj")
+        pc = ttn.Plan(2, ttn.CALL_ENERGY, Jc, Jd, None, workspace=ws if args.cpu_L <= L else None)
+        gpu_same = time_plan(torch, pc, reps=3)
+        pc.close()
 
     # ---- the other BASELINE.json configs, timed beside the headline (rank 0, one GPU; they are parity
     # cases, not the metric: device time of ttn_plan_launch, couplings resident, mean of 3 launches)
@@ -340,17 +415,23 @@ def main():
 
     if rank == 0:
         peak, peak_src = measured_peaks()
+        traffic, traffic_src = ncu_traffic_per_launch("r02_ncu_full_summary.csv", "fused_pass_kernel") if L == 32 else (None, None)
         per_inst_ms = whole_job_ms_per_instance(ms_per_step, world)
         achieved = bytes_min(L) / (ms_per_step * 1e-3) / 1e9            # GB/s per GPU
         sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
         alu_peak = 148 * 64 * sm_mhz * 1e6                              # FMNMX: 64 lanes/clk/SM (alu pipe)
+        # max-plus updates the sweep executes: L (L-1) gates (L-1 of them flip gates under the h = 0
+        # reduction) over the stored state
+        upd_exec = float(L) * (L - 1) * plan.state_elements
         out = {
             "metric": METRIC, "value": per_inst_ms, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_name(L),
-                       "L": L, "state_bytes": 4 * 2 ** L, "hbm_passes": plan.num_passes,
+                       "L": L, "state_bytes": 4 * plan.state_elements, "hbm_passes": plan.num_passes,
+                       "symmetry": "h = 0: the flip-symmetric half-state (column 0 up) is stored and swept"
+                       if plan.state_elements < 2 ** L else "none",
                        "l2_policy": "state (>= 1 GiB) far larger than the 126 MB L2; no flush needed"
                        if L >= 28 else "state fits L2: flush not applied, number is L2-resident",
                        "E0": E_dev},
@@ -359,24 +440,29 @@ def main():
             "gpu_launches": plan.num_launches * args.steps,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak,
-                         # dram__bytes_read.sum + dram__bytes_write.sum per pass launch from the ncu
-                         # --set full capture in profiles/r01m_ncu_full_summary.csv (one read + one
-                         # write of the state); algorithmic bytes per launch = bytes_min / passes
-                         "traffic": 17.18e9 + 17.12e9 if L == 32 else None,
+                         # dram__bytes_read.sum + dram__bytes_write.sum per pass launch, read from the
+                         # committed ncu --set full summary of this kernel (None if absent / other L)
+                         "traffic": traffic, "traffic_source": traffic_src,
                          "algorithmic_bytes_per_launch": bytes_min(L) / plan.num_passes,
+                         "note": "algorithmic bytes are north_star's: one read + one write of the FULL 2^L f32 "
+                                 "vector per row; the sweep stores the flip-symmetric half (h = 0) and fuses rows "
+                                 "across passes, so it moves fewer bytes than that",
                          "peak_source": peak_src,
                          "algorithmic_bytes_per_sweep": bytes_min(L),
                          "kernel": "ttn::fused_pass_kernel<LOW|HIGH> (all %d pass launches of one sweep)" % plan.num_passes},
-            "alu_roofline": {"bound": "alu", "achieved": updates(L) / (ms_per_step * 1e-3),
+            "alu_roofline": {"bound": "alu", "achieved": upd_exec / (ms_per_step * 1e-3),
                              "peak": alu_peak, "unit": "max-plus updates/s",
-                             "frac": updates(L) / (ms_per_step * 1e-3) / alu_peak,
-                             "note": "1 FMNMX per update on the 64-lane/clk/SM alu pipe at the sampled SM clock"},
+                             "frac": upd_exec / (ms_per_step * 1e-3) / alu_peak,
+                             "updates_per_sweep": upd_exec,
+                             "note": "1 FMNMX per EXECUTED update (L(L-1) gates over the stored state: half of "
+                                     "north_star's full-vector count under the h = 0 flip reduction) on the "
+                                     "64-lane/clk/SM alu pipe at the sampled SM clock"},
             "step_ms": step_ms, "clocks": clocks, "tropical_i16": i16,
         }
         if others is not None:
             out["other_configs"] = others
         if not args.no_cpu_baseline:
-            out["cpu_baseline"] = cpu_baseline(L, args.cpu_L)
+            out["cpu_baseline"] = cpu_baseline(L, args.cpu_L, gpu_same)
         print(json.dumps(out))
     plan.close()
     if dist is not None:
