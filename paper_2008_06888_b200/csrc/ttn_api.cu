@@ -62,6 +62,7 @@ struct DebugCfg {
     int nolowpf = 0, nogroup = 0, nosweep = 0;   // ground_config forward: no LOW prefetch / instance groups / one-launch sweep
     int bt_multi = 0;             // backward pass: one launch pair per row even for batches of small lattices
     int timing = 0;               // per-pass device times on stderr
+    int ckpt_k = 0;               // TTN_DEBUG_CKPT_K=k: ground_config keeps a checkpoint every k rows + recompute (any L)
     int ch_persm = 512, ch_nocell0 = 0;          // chimera: CTAs per SM, generic kernel for the r = 0 cells
 };
 DebugCfg read_debug() {
@@ -70,6 +71,7 @@ DebugCfg read_debug() {
     auto flag = [](const char* name, int& v) { v = getenv(name) != nullptr; };
     geti("TTN_DEBUG_TMAX", d.tmax); geti("TTN_DEBUG_RIDE", d.ride); geti("TTN_DEBUG_FUSED", d.fused);
     geti("TTN_DEBUG_Z2", d.z2); geti("TTN_DEBUG_NB", d.nb); geti("TTN_DEBUG_CH_PERSM", d.ch_persm);
+    geti("TTN_DEBUG_CKPT_K", d.ckpt_k);
     flag("TTN_DEBUG_NOBEAM", d.nobeam); flag("TTN_DEBUG_NOLOWPF", d.nolowpf); flag("TTN_DEBUG_NOGROUP", d.nogroup);
     flag("TTN_DEBUG_NOSWEEP", d.nosweep); flag("TTN_DEBUG_BT_MULTI", d.bt_multi); flag("TTN_DEBUG_TIMING", d.timing);
     flag("TTN_DEBUG_CH_NOCELL0", d.ch_nocell0);
@@ -93,11 +95,35 @@ TileCfg tile_cfg(int q, bool count, const DebugCfg& dbg) {
 bool limits_ok(int q, int L, bool count, bool config) {
     if (L < 1) return false;
     if (q == 2) {
-        if (config) return L <= 28;
+        if (config) return L <= 32;
         return count ? L <= 32 : L <= 34;
     }
     if (q == 3) return !config && L <= 20;
     return false;
+}
+
+// Checkpoints of ttn_ground_config ("checkpointing").  k = 0: every row boundary C_r has
+// its own buffer (L buffers).  k > 1 (L > 28, where L buffers no longer fit): C_r is kept for
+// r = 0, k, 2k, ... and r = L-1 only; the backward pass re-sweeps each segment (a, b) of rows between
+// two kept checkpoints from C_a into a ring of k - 1 scratch buffers, backtracks through it, and moves
+// on to the segment below: n_stored + k - 1 buffers, k ~ sqrt(L), and one extra forward sweep in total.
+struct CkptScheme {
+    int L = 0, k = 0, n_stored = 0, n_buf = 0;
+    bool stored(int r) const { return k == 0 || r % k == 0 || r == L - 1; }
+    int stored_slot(int r) const { return k == 0 ? r : (r % k == 0 ? r / k : n_stored - 1); }
+    int prev_stored(int b) const { return k == 0 ? b - 1 : ((b - 1) / k) * k; }   // largest stored row < b
+    int ring_slot(int a, int r) const { return n_stored + (r - a - 1); }           // a < r < next stored row
+};
+CkptScheme ckpt_scheme(int L, bool fused, const DebugCfg& dbg) {
+    CkptScheme c; c.L = L; c.k = 0; c.n_stored = L; c.n_buf = L;
+    int k = 0;
+    if (fused && dbg.ckpt_k > 1) k = dbg.ckpt_k;
+    else if (fused && L > 28) { k = 1; while (k * k < L) ++k; }
+    if (k <= 1 || k >= L - 1) return c;
+    c.k = k; c.n_stored = 0;
+    for (int r = 0; r < L; ++r) if (r % k == 0 || r == L - 1) ++c.n_stored;
+    c.n_buf = c.n_stored + k - 1;
+    return c;
 }
 
 struct Layout {
@@ -107,6 +133,7 @@ struct Layout {
     unsigned long long NS = 0, max_tiles = 0;
     int amax_blocks = 0;
     int f_max_gates = 0, f_max_mops = 0;
+    CkptScheme ck;
 };
 
 // The fused register-phase paths: Ising Tropical<f32> energy for L >= 12 (ttn_fused.cuh) and Ising
@@ -142,7 +169,8 @@ Layout make_layout(int q, int L, bool count, bool config, int batch, const Debug
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
     y.x = take((size_t)batch * y.NS * (i16 ? 2 : 4));
     if (count) y.n = take((size_t)batch * y.NS * 8);
-    if (config) y.ckpt = take((size_t)batch * L * y.NS * 4);
+    y.ck = ckpt_scheme(L, config && fused_eligible(q, L, count, config, dbg), dbg);
+    if (config) y.ckpt = take((size_t)batch * y.ck.n_buf * y.NS * 4);
     y.Jh = take((size_t)batch * L * (L - 1) * 4 + 4);
     y.Jv = take((size_t)batch * (L - 1) * L * 4 + 4);
     y.h = take((size_t)batch * L * L * 4);
@@ -190,6 +218,9 @@ struct ttn_plan {
     DebugCfg dbg;                  // the debug switches as they were when the plan was created
     int fused_grid = 0;
     int sms = 0;
+    // row-aligned (config) fused plans: passes of row r = [row_pass[r], row_pass[r + 1]); buffer slot that
+    // holds C_r at the moment (-1: none -- the row's result lives in the in-place state V)
+    std::vector<int> row_pass, slot_of_row;
     int sweep_grid = 0;             // > 0: fused_sweep_kernel runs every pass in one launch (table at lay.f_sweep)
     std::vector<ttn::FusedParams> sweep_params;
     Layout lay;
@@ -233,7 +264,7 @@ static ttn_status launch_pass(const ttn_plan* P, const ttn::Pass& ps, cudaStream
     float* CK = reinterpret_cast<float*>(P->ws + y.ckpt);
     auto buf = [&](int id, unsigned long long& stride) -> float* {
         if (id < 0) { stride = y.NS; return V; }
-        stride = (unsigned long long)P->L * y.NS;
+        stride = (unsigned long long)y.ck.n_buf * y.NS;
         return CK + (unsigned long long)id * y.NS;
     };
     pp.src_x = buf(ps.src_buf, pp.src_stride);
@@ -286,7 +317,9 @@ static ttn_status launch_pass(const ttn_plan* P, const ttn::Pass& ps, cudaStream
 
 // out_pp != NULL: only fill the parameters (force_group instances per CTA at a time) and the grid.
 static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps, cudaStream_t st,
-                                    ttn::FusedParams* out_pp = nullptr, int force_group = 0, unsigned* out_grid = nullptr) {
+                                    ttn::FusedParams* out_pp = nullptr, int force_group = 0, unsigned* out_grid = nullptr);
+static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps, cudaStream_t st,
+                                    ttn::FusedParams* out_pp, int force_group, unsigned* out_grid) {
     const Layout& y = P->lay;
     const ttn::FusedPlan& fp = P->fplan;
     ttn::FusedParams pp{};
@@ -298,8 +331,10 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
     pp.src = pp.state; pp.src_stride = pp.inst_stride;
     if (P->config) {           // row-aligned plan: checkpoints C_r = V''_r, [inst][L][2^L]
         float* CK = reinterpret_cast<float*>(P->ws + y.ckpt);
-        if (ps.src_buf >= 0) { pp.src = CK + (unsigned long long)ps.src_buf * y.NS; pp.src_stride = (unsigned long long)P->L * y.NS; }
-        if (ps.dst_buf >= 0) { pp.state = CK + (unsigned long long)ps.dst_buf * y.NS; pp.inst_stride = (unsigned long long)P->L * y.NS; }
+        const unsigned long long cstride = (unsigned long long)y.ck.n_buf * y.NS;
+        const int ss = ps.src_buf >= 0 ? P->slot_of_row[ps.src_buf] : -1, ds = ps.dst_buf >= 0 ? P->slot_of_row[ps.dst_buf] : -1;
+        if (ss >= 0) { pp.src = CK + (unsigned long long)ss * y.NS; pp.src_stride = cstride; }
+        if (ds >= 0) { pp.state = CK + (unsigned long long)ds * y.NS; pp.inst_stride = cstride; }
     }
     pp.L_cols = P->L;
     if (P->i16) {           // the kernel sees the lattice of 32-bit words: column c >= 1 = word digit c - 1
@@ -548,7 +583,7 @@ static ttn_status launch_backtrace(ttn_plan* P, cudaStream_t st) {
         const Layout& y = P->lay;
         ttn::ArgmaxParams ap{};
         ap.L = P->L; ap.NS = y.NS; ap.nblk = y.amax_blocks;
-        ap.c_stride = (unsigned long long)P->L * y.NS;
+        ap.c_stride = (unsigned long long)y.ck.n_buf * y.NS;
         ap.Jv = reinterpret_cast<const float*>(P->ws + y.Jv);
         ap.Jh = reinterpret_cast<const float*>(P->ws + y.Jh);
         ap.h = P->has_field ? reinterpret_cast<const float*>(P->ws + y.h) : nullptr;
@@ -557,20 +592,42 @@ static ttn_status launch_backtrace(ttn_plan* P, cudaStream_t st) {
         ap.part_s = reinterpret_cast<unsigned long long*>(P->ws + y.amax_s);
         ap.v_out = reinterpret_cast<float*>(P->ws + y.out_x);
         ap.sigma = reinterpret_cast<signed char*>(P->ws + y.sigma);
-        if (backtrace_one_cta(P->L, P->batch, P->dbg)) {
+        if (y.ck.k == 0 && backtrace_one_cta(P->L, P->batch, P->dbg)) {
             // batches of small lattices: one CTA walks all L checkpoints of its instance
             ap.C = reinterpret_cast<const float*>(P->ws + y.ckpt);
             ttn::backtrace_inst_kernel<<<P->batch, ttn::BT_THREADS, 0, st>>>(ap);
             TTN_CUDA(cudaGetLastError());
             return TTN_OK;
         }
-        for (int r = P->L - 1; r >= 0; --r) {
+        auto bt_row = [&](int r, int slot) -> ttn_status {
             ap.r = r; ap.has_next = (r < P->L - 1);
-            ap.C = reinterpret_cast<const float*>(P->ws + y.ckpt) + (unsigned long long)r * y.NS;
+            ap.C = reinterpret_cast<const float*>(P->ws + y.ckpt) + (unsigned long long)slot * y.NS;
             ttn::argmax_partial_kernel<<<dim3(ap.nblk, P->batch), 256, 0, st>>>(ap);
             TTN_CUDA(cudaGetLastError());
             ttn::argmax_final_kernel<<<P->batch, 32, 0, st>>>(ap);
             TTN_CUDA(cudaGetLastError());
+            return TTN_OK;
+        };
+        const CkptScheme& ck = y.ck;
+        if (ck.k == 0) {
+            for (int r = P->L - 1; r >= 0; --r) { ttn_status s = bt_row(r, r); if (s != TTN_OK) return s; }
+            return TTN_OK;
+        }
+        // sqrt-spaced checkpoints: backtrack row b from its kept checkpoint, re-sweep rows a+1 .. b-1 from
+        // C_a into the ring, backtrack through them and through row a, continue below a
+        int b = P->L - 1;
+        ttn_status s = bt_row(b, ck.stored_slot(b));
+        if (s != TTN_OK) return s;
+        while (b > 0) {
+            const int a = ck.prev_stored(b);
+            for (int r = a + 1; r < b; ++r) P->slot_of_row[r] = ck.ring_slot(a, r);
+            for (int k = P->row_pass[a + 1]; k < P->row_pass[b]; ++k) {
+                s = launch_fused_pass(P, P->fplan.passes[k], st, nullptr, 0, nullptr);
+                if (s != TTN_OK) return s;
+            }
+            for (int r = b - 1; r >= a; --r) { s = bt_row(r, P->slot_of_row[r]); if (s != TTN_OK) return s; }
+            for (int r = a + 1; r < b; ++r) P->slot_of_row[r] = -1;
+            b = a;
         }
     }
     return TTN_OK;
@@ -734,8 +791,22 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     if (P->fused) {
         ttn_status fs = count ? setup_fcount(P, st) : setup_fused(P, st);
         if (fs != TTN_OK) { delete P; return fs; }
-        P->launches = (int)P->fplan.passes.size() + (config ? (backtrace_one_cta(L, batch, dbg) ? 1 : 2 * L) : 1);
-        if (config && !count && !P->i16 && !dbg.nosweep && P->fplan.passes.size() <= (size_t)(4 * L + 8)) {
+        const CkptScheme& ck = lay.ck;
+        const bool bt1 = ck.k == 0 && backtrace_one_cta(L, batch, dbg);
+        P->launches = (int)P->fplan.passes.size() + (config ? (bt1 ? 1 : 2 * L) : 1);
+        if (config) {
+            // passes of row r (row 0 = the initialising pass), and where C_r lives during the forward sweep
+            P->row_pass.assign(L + 1, 0);
+            int row = 0;
+            for (size_t i = 0; i < P->fplan.passes.size(); ++i)
+                if (P->fplan.passes[i].dst_buf >= 0) { P->row_pass[++row] = (int)i + 1; }
+            if (row != L) { delete P; return fail(TTN_EUNSUPPORTED, "row-aligned plan is incomplete"); }
+            P->slot_of_row.assign(L, -1);
+            for (int r = 0; r < L; ++r) if (ck.stored(r)) P->slot_of_row[r] = ck.stored_slot(r);
+            if (ck.k > 0)          // the backward pass re-sweeps every row that is not kept
+                for (int r = 1; r < L; ++r) if (!ck.stored(r)) P->launches += P->row_pass[r + 1] - P->row_pass[r];
+        }
+        if (config && ck.k == 0 && !count && !P->i16 && !dbg.nosweep && P->fplan.passes.size() <= (size_t)(4 * L + 8)) {
             // every pass in cta_per_inst mode: the pass table of fused_sweep_kernel (two instances per
             // CTA at a time where the constants of every pass fit, else one)
             std::vector<ttn::FusedParams> v(P->fplan.passes.size());
@@ -751,7 +822,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
                 cudaError_t ce = cudaMemcpyAsync(P->ws + lay.f_sweep, P->sweep_params.data(), v.size() * sizeof(ttn::FusedParams),
                                                  cudaMemcpyHostToDevice, st);
                 if (ce != cudaSuccess) { delete P; return fail(TTN_ECUDA, "pass table upload failed: %s", cudaGetErrorString(ce)); }
-                P->launches = 1 + (backtrace_one_cta(L, batch, dbg) ? 1 : 2 * L);
+                P->launches = 1 + (bt1 ? 1 : 2 * L);
             }
         }
     } else {
@@ -767,7 +838,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
         ttn::generic_prep_kernel<<<dim3((unsigned)((work + 255) / 256), (unsigned)batch), 256, 0, st>>>(gp);
         cudaError_t pe = cudaGetLastError();
         if (pe != cudaSuccess) { delete P; return fail(TTN_ECUDA, "prep launch failed: %s", cudaGetErrorString(pe)); }
-        P->launches = (int)P->plan.passes.size() + (config ? (backtrace_one_cta(L, batch, dbg) ? 1 : 2 * L) : 1);
+        P->launches = (int)P->plan.passes.size() + (config ? (lay.ck.k == 0 && backtrace_one_cta(L, batch, dbg) ? 1 : 2 * L) : 1);
     }
     *out = P;
     return TTN_OK;

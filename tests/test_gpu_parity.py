@@ -669,6 +669,47 @@ def test_next2_ground_config_24x24():
         assert oracle.ising_energy(24, Jh[b], Jv[b], None, sig[b]) == E0[b]
 
 
+# ------------------------------------------------------------------ sqrt-spaced checkpoints + recompute (NEXT-2)
+@pytest.mark.parametrize("L,k", [(12, 2), (13, 3), (14, 5), (16, 4), (17, 6)])
+def test_ground_config_sqrt_checkpoints_match_all_checkpoints(monkeypatch, L, k):
+    """PAPER.md:99 "checkpointing": C_r kept every k rows, the backward pass re-sweeps each segment into a
+    ring of k - 1 scratch buffers.  The re-swept checkpoints are bit-identical to the ones the forward
+    sweep would have kept, so E0 and sigma must equal the all-checkpoints run exactly (Gaussian J, h:
+    any change of arithmetic would show), and match the oracle."""
+    B = 3
+    Jh, Jv, h = make_batch(L, range(2900, 2900 + B), "gauss", fields=True)
+    E_a, sig_a = ttn.ground_config(Jh, Jv, h)
+    monkeypatch.setenv("TTN_DEBUG_CKPT_K", str(k))
+    need_k = ttn.workspace_bytes(2, L, ttn.TROPICAL_F32, B, True)
+    E_k, sig_k = ttn.ground_config(Jh, Jv, h)
+    monkeypatch.delenv("TTN_DEBUG_CKPT_K")
+    assert need_k < ttn.workspace_bytes(2, L, ttn.TROPICAL_F32, B, True)        # fewer buffers
+    assert np.array_equal(E_a, E_k) and np.array_equal(sig_a, sig_k)
+    for b in range(B):
+        Eo = oracle.dp_ising(L, Jh[b], Jv[b], h[b], count=False)[0]
+        assert abs(E_k[b] - Eo) <= TOL * abs(Eo)
+        assert abs(oracle.ising_energy(L, Jh[b], Jv[b], h[b], sig_k[b]) - Eo) <= TOL * abs(Eo)
+
+
+def test_ground_config_30x30_seeded():
+    """ttn_ground_config beyond L = 28 (where L checkpoints of 2^L floats no longer fit): sqrt-spaced
+    checkpoints + recompute.  The +-J seed-4000 30x30 instance: E0 and the Eq. (1) energy of the
+    returned configuration equal the O-dp golden value (bit-exact)."""
+    import torch
+    gold = golden()
+    L = 30
+    need = ttn.workspace_bytes(2, L, ttn.TROPICAL_F32, 1, True)
+    free, _ = torch.cuda.mem_get_info()
+    if free < need + (2 << 30):
+        pytest.skip("needs %.0f GB of free device memory" % (need / 1e9))
+    assert need < 16 * 4 * 2 ** L                     # far fewer than L buffers
+    Jh, Jv, _ = make_batch(L, [4000], "pmj")
+    E0, sig = ttn.ground_config(Jh, Jv)
+    assert E0[0] == gold[("ising_energy", L, 4000)][0]
+    assert oracle.ising_energy(L, Jh[0], Jv[0], None, sig[0]) == E0[0]
+    torch.cuda.empty_cache()
+
+
 # ------------------------------------------------------------------ maximum sizes of the other calls
 def test_ground_config_28x28_planted():
     """ttn_ground_config at its size limit (28 checkpoints of 1 GiB).  Planted instance = gauge-
