@@ -27,7 +27,7 @@
  * is NO CPU fallback: without a CUDA device every compute call returns TTN_ECUDA.
  *
  * h = 0 (NULL or all zero): Eq. (1) is invariant under the global flip sigma -> -sigma, and so is
- * every intermediate state of the sweep; ttn_sweep_energy[_i16] and ttn_sweep_count then store only the
+ * every intermediate state of the sweep; ttn_sweep_energy[_i16], ttn_sweep_count and ttn_ground_config then store only the
  * half of the state vector with column 0 up (2^(L-1) elements) and apply the column-0 gates as a
  * pairing of every element with its complement -- half the memory, bytes and arithmetic,
  * identical results, the degeneracy being twice the half's count.  Any
@@ -71,10 +71,16 @@ typedef enum {
 } ttn_semiring;
 
 /* Limits: Ising tropical L <= 34, Ising counting L <= 32, Potts L <= 20 (index fits 32 bits);
-   ttn_ground_config L <= 28 (L checkpoints of 2^L f32 each). */
+   ttn_ground_config L <= 32: L checkpoints of 2^L f32 each up to L = 28, ~2 sqrt(L) of them with a
+   re-sweep of every segment in the backward pass beyond; the workspace at L = 32 is
+   192 GiB with fields (beyond one B200) and 96 GiB for h = 0 (ttn_workspace_bytes_h0). */
 
-/* Bytes of device workspace needed.  q = 2 (Ising) or 3 (Potts).  Returns 0 on bad arguments. */
+/* Bytes of device workspace needed.  q = 2 (Ising) or 3 (Potts).  Returns 0 on bad arguments.
+   The size covers any field h.  ttn_workspace_bytes_h0 is the (smaller) size that suffices when the
+   caller will pass h = NULL or an all-zero h (the flip-reduced half-state, see the top of this file);
+   at L = 32, ttn_ground_config fits one B200 only in that case. */
 size_t ttn_workspace_bytes(int q, int L, ttn_semiring mode, int batch, int want_config);
+size_t ttn_workspace_bytes_h0(int q, int L, ttn_semiring mode, int batch, int want_config);
 
 /* ---- one-call host API (upload + sweep + read-back, synchronises `stream`) -------------- */
 
@@ -147,7 +153,8 @@ typedef enum {
        for ttn_plan_describe and for tests. */
     TTN_CALL_ENERGY_Z2 = 4,
     TTN_CALL_COUNT_Z2 = 5,      /* the same for TTN_CALL_COUNT (L < 12 runs the plain sweep) */
-    TTN_CALL_ENERGY_I16_Z2 = 6  /* the same for TTN_CALL_ENERGY_I16 (L < 15 runs the plain i16 sweep) */
+    TTN_CALL_ENERGY_I16_Z2 = 6, /* the same for TTN_CALL_ENERGY_I16 (L < 15 runs the plain i16 sweep) */
+    TTN_CALL_CONFIG_Z2 = 7      /* the same for TTN_CALL_CONFIG: checkpoints are half-states (L < 14: plain) */
 } ttn_call;
 
 ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const float* Jv,

@@ -619,16 +619,17 @@ inline FusedPlan make_fused_plan(int L, int max_gates_per_pass, const FusedGeom&
 // checkpoint C_r = V''_r.  Row r needs one pass per tile of a cover of the columns (the low tile
 // and high tiles up to column L); the pass that completes row r writes C_r, the first pass of
 // row r+1 reads it.  Pass 0 initialises C_0 (no gate: V''_0 is the tropical one everywhere).
-inline FusedPlan make_fused_row_plan(int L, int max_gates_per_pass) {
+// G = GEOM_F32, or GEOM_F32_Z2 for h = 0 (the checkpoints are then half-states).
+inline FusedPlan make_fused_row_plan(int L, int max_gates_per_pass, const FusedGeom& G = GEOM_F32) {
     FusedPlan p; p.L = L;
-    if (L < F_WLOW) return p;
+    if (L < G.WLOW) return p;
     std::vector<int> starts{0};
-    for (int x = F_WLOW; x < L; x += F_WHIGH) {
-        int a = x + F_WHIGH <= L ? x : L - F_WHIGH;
-        if (a < F_AMIN) a = F_AMIN;
+    for (int x = G.WLOW; x < L; x += G.WHIGH) {
+        int a = x + G.WHIGH <= L ? x : L - G.WHIGH;
+        if (a < G.AMIN) a = G.AMIN;
         starts.push_back(a);
     }
-    FusedScheduler s(L, p, GEOM_F32);
+    FusedScheduler s(L, p, G);
     {   // row 0: initialise
         s.set_max_row(0);
         FusedPass ps{};

@@ -149,7 +149,8 @@ bool fused_eligible(int q, int L, bool count, bool config, const DebugCfg& dbg) 
 // (a tile and its complement).  Geometry of the call, or nullptr.
 const ttn::FusedGeom* z2_geom(int q, int L, ttn_call call, bool has_field, const DebugCfg& dbg) {
     if (dbg.fused == 0 || dbg.z2 == 0 || q != 2 || has_field) return nullptr;
-    if ((call == TTN_CALL_ENERGY || call == TTN_CALL_ENERGY_Z2) && L >= ttn::GEOM_F32_Z2.WLOW + 1) return &ttn::GEOM_F32_Z2;
+    if ((call == TTN_CALL_ENERGY || call == TTN_CALL_ENERGY_Z2 || call == TTN_CALL_CONFIG || call == TTN_CALL_CONFIG_Z2) &&
+        L >= ttn::GEOM_F32_Z2.WLOW + 1) return &ttn::GEOM_F32_Z2;
     if ((call == TTN_CALL_COUNT || call == TTN_CALL_COUNT_Z2) && L >= ttn::GEOM_COUNT_Z2.WLOW + 1) return &ttn::GEOM_COUNT_Z2;
     if ((call == TTN_CALL_ENERGY_I16 || call == TTN_CALL_ENERGY_I16_Z2) && L >= ttn::GEOM_I16_Z2.WLOW + 1) return &ttn::GEOM_I16_Z2;
     return nullptr;
@@ -574,8 +575,8 @@ static ttn_status setup_fused(ttn_plan* P, cudaStream_t st) {
 }
 
 // batches of small lattices walk all checkpoints of an instance in one CTA (backtrace_inst_kernel)
-static bool backtrace_one_cta(int L, int batch, const DebugCfg& dbg) {
-    return L <= 18 && L <= ttn::BT_MAX_L && batch >= 32 && !dbg.bt_multi;
+static bool backtrace_one_cta(int L, int batch, const DebugCfg& dbg, bool z2 = false) {
+    return !z2 && L <= 18 && L <= ttn::BT_MAX_L && batch >= 32 && !dbg.bt_multi;
 }
 
 static ttn_status launch_backtrace(ttn_plan* P, cudaStream_t st) {
@@ -592,7 +593,7 @@ static ttn_status launch_backtrace(ttn_plan* P, cudaStream_t st) {
         ap.part_s = reinterpret_cast<unsigned long long*>(P->ws + y.amax_s);
         ap.v_out = reinterpret_cast<float*>(P->ws + y.out_x);
         ap.sigma = reinterpret_cast<signed char*>(P->ws + y.sigma);
-        if (y.ck.k == 0 && backtrace_one_cta(P->L, P->batch, P->dbg)) {
+        if (y.ck.k == 0 && backtrace_one_cta(P->L, P->batch, P->dbg, P->z2)) {
             // batches of small lattices: one CTA walks all L checkpoints of its instance
             ap.C = reinterpret_cast<const float*>(P->ws + y.ckpt);
             ttn::backtrace_inst_kernel<<<P->batch, ttn::BT_THREADS, 0, st>>>(ap);
@@ -602,7 +603,8 @@ static ttn_status launch_backtrace(ttn_plan* P, cudaStream_t st) {
         auto bt_row = [&](int r, int slot) -> ttn_status {
             ap.r = r; ap.has_next = (r < P->L - 1);
             ap.C = reinterpret_cast<const float*>(P->ws + y.ckpt) + (unsigned long long)slot * y.NS;
-            ttn::argmax_partial_kernel<<<dim3(ap.nblk, P->batch), 256, 0, st>>>(ap);
+            if (P->z2) ttn::argmax_partial_kernel<true><<<dim3(ap.nblk, P->batch), 256, 0, st>>>(ap);
+            else ttn::argmax_partial_kernel<false><<<dim3(ap.nblk, P->batch), 256, 0, st>>>(ap);
             TTN_CUDA(cudaGetLastError());
             ttn::argmax_final_kernel<<<P->batch, 32, 0, st>>>(ap);
             TTN_CUDA(cudaGetLastError());
@@ -649,17 +651,30 @@ size_t ttn_workspace_bytes(int q, int L, ttn_semiring mode, int batch, int want_
     return make_layout(q, L, count, want_config != 0, batch, dbg, mode == TTN_TROPICAL_I16 && i16_eligible(q, L, dbg)).total;
 }
 
+size_t ttn_workspace_bytes_h0(int q, int L, ttn_semiring mode, int batch, int want_config) {
+    const size_t full = ttn_workspace_bytes(q, L, mode, batch, want_config);
+    if (!full || q != 2) return full;
+    const DebugCfg dbg = read_debug();
+    const bool count = (mode == TTN_COUNTING_F32_F64);
+    const ttn_call call = want_config ? TTN_CALL_CONFIG : (count ? TTN_CALL_COUNT : (mode == TTN_TROPICAL_I16 ? TTN_CALL_ENERGY_I16 : TTN_CALL_ENERGY));
+    if (!z2_geom(q, L, call, false, dbg)) return full;
+    return make_layout(q, L, count, want_config != 0, batch, dbg, mode == TTN_TROPICAL_I16 && i16_eligible(q, L, dbg), true).total;
+}
+
 long ttn_plan_describe(int q, int L, ttn_call call, char* buf, size_t n) {
     if ((q != 2 && q != 3) || !buf || n == 0) return -1;
     if (!limits_ok(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) return -1;
     std::string s;
     const DebugCfg dbg = read_debug();
-    if (call == TTN_CALL_ENERGY_Z2 || call == TTN_CALL_COUNT_Z2 || call == TTN_CALL_ENERGY_I16_Z2) {   // the schedules the calls run when h = 0
+    if (call == TTN_CALL_ENERGY_Z2 || call == TTN_CALL_COUNT_Z2 || call == TTN_CALL_ENERGY_I16_Z2 || call == TTN_CALL_CONFIG_Z2) {
+        // the schedules the calls run when h = 0
         if (const ttn::FusedGeom* G = z2_geom(q, L, call, false, dbg)) {
-            ttn::FusedPlan fp = ttn::make_fused_plan(L, ttn::FMAX_GATES, *G);
+            ttn::FusedPlan fp = call == TTN_CALL_CONFIG_Z2 ? ttn::make_fused_row_plan(L, ttn::FMAX_GATES, *G)
+                                                           : ttn::make_fused_plan(L, ttn::FMAX_GATES, *G);
             if (fp.ok) s = ttn::describe_fused(fp);
         }
-        if (s.empty()) call = call == TTN_CALL_ENERGY_Z2 ? TTN_CALL_ENERGY : (call == TTN_CALL_COUNT_Z2 ? TTN_CALL_COUNT : TTN_CALL_ENERGY_I16);
+        if (s.empty()) call = call == TTN_CALL_ENERGY_Z2 ? TTN_CALL_ENERGY : (call == TTN_CALL_COUNT_Z2 ? TTN_CALL_COUNT
+                            : (call == TTN_CALL_CONFIG_Z2 ? TTN_CALL_CONFIG : TTN_CALL_ENERGY_I16));
     }
     if (call == TTN_CALL_ENERGY_I16 && i16_eligible(q, L, dbg)) {
         ttn::FusedPlan fp = ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_I16);
@@ -687,9 +702,10 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     if (q != 2 && q != 3) return fail(TTN_EINVAL, "q must be 2 or 3");
     if (L < 1 || batch < 1) return fail(TTN_EINVAL, "L and batch must be >= 1");
     if (call != TTN_CALL_ENERGY && call != TTN_CALL_COUNT && call != TTN_CALL_CONFIG && call != TTN_CALL_ENERGY_I16 &&
-        call != TTN_CALL_ENERGY_Z2 && call != TTN_CALL_COUNT_Z2 && call != TTN_CALL_ENERGY_I16_Z2)
+        call != TTN_CALL_ENERGY_Z2 && call != TTN_CALL_COUNT_Z2 && call != TTN_CALL_ENERGY_I16_Z2 && call != TTN_CALL_CONFIG_Z2)
         return fail(TTN_EINVAL, "bad call kind");
-    const bool want_z2 = (call == TTN_CALL_ENERGY_Z2 || call == TTN_CALL_COUNT_Z2 || call == TTN_CALL_ENERGY_I16_Z2);
+    const bool want_z2 = (call == TTN_CALL_ENERGY_Z2 || call == TTN_CALL_COUNT_Z2 || call == TTN_CALL_ENERGY_I16_Z2 ||
+                          call == TTN_CALL_CONFIG_Z2);
     const DebugCfg dbg = read_debug();
     bool i16 = false;
     const bool want_i16 = (call == TTN_CALL_ENERGY_I16 || call == TTN_CALL_ENERGY_I16_Z2);
@@ -701,7 +717,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     if (L > 1 && (!Jh || !Jv)) return fail(TTN_EINVAL, "Jh/Jv is NULL");
     if (!workspace) return fail(TTN_EINVAL, "workspace is NULL");
     if (q == 3 && h) return fail(TTN_EINVAL, "the Potts variant takes no fields");
-    const bool count = (call == TTN_CALL_COUNT || call == TTN_CALL_COUNT_Z2), config = (call == TTN_CALL_CONFIG);
+    const bool count = (call == TTN_CALL_COUNT || call == TTN_CALL_COUNT_Z2), config = (call == TTN_CALL_CONFIG || call == TTN_CALL_CONFIG_Z2);
     if (!limits_ok(q, L, count, config)) return fail(TTN_EUNSUPPORTED, "L=%d beyond the limits for this call", L);
     const size_t nh = (size_t)batch * L * (L - 1), nv = (size_t)batch * (L - 1) * L, nf = (size_t)batch * L * L;
     for (size_t i = 0; i < nh; ++i) if (!std::isfinite(Jh[i])) return fail(TTN_EINVAL, "non-finite Jh[%zu]", i);
@@ -727,7 +743,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     if (h) for (size_t i = 0; i < nf && !field; ++i) field = (h[i] != 0.0f);
     if (want_z2 && field) return fail(TTN_EINVAL, "the flip reduction needs h = 0");
     const ttn::FusedGeom* zg = z2_geom(q, L, call, field, dbg);
-    if (want_z2) call = count ? TTN_CALL_COUNT : (want_i16 ? TTN_CALL_ENERGY_I16 : TTN_CALL_ENERGY);  // lattices too small for it run the plain sweep
+    if (want_z2) call = count ? TTN_CALL_COUNT : (config ? TTN_CALL_CONFIG : (want_i16 ? TTN_CALL_ENERGY_I16 : TTN_CALL_ENERGY));  // lattices too small for it run the plain sweep
     Layout lay = make_layout(q, L, count, config, batch, dbg, i16, zg != nullptr);
     if (workspace_bytes < lay.total)
         return fail(TTN_ENOMEM, "workspace too small: %zu < %zu", workspace_bytes, lay.total);
@@ -756,7 +772,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
         P->fused = P->fplan.ok;
         if (!P->fused) { delete P; return fail(TTN_EUNSUPPORTED, "no Tropical<i16> schedule"); }
     } else if (zg) {
-        P->fplan = ttn::make_fused_plan(L, ttn::FMAX_GATES, *zg);
+        P->fplan = config ? ttn::make_fused_row_plan(L, ttn::FMAX_GATES, *zg) : ttn::make_fused_plan(L, ttn::FMAX_GATES, *zg);
         P->fused = P->fplan.ok;
         if (!P->fused) { delete P; return fail(TTN_EUNSUPPORTED, "no flip-reduced schedule"); }
     } else if (fused_eligible(q, L, count, config, dbg)) {
@@ -792,7 +808,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
         ttn_status fs = count ? setup_fcount(P, st) : setup_fused(P, st);
         if (fs != TTN_OK) { delete P; return fs; }
         const CkptScheme& ck = lay.ck;
-        const bool bt1 = ck.k == 0 && backtrace_one_cta(L, batch, dbg);
+        const bool bt1 = ck.k == 0 && backtrace_one_cta(L, batch, dbg, P->z2);
         P->launches = (int)P->fplan.passes.size() + (config ? (bt1 ? 1 : 2 * L) : 1);
         if (config) {
             // passes of row r (row 0 = the initialising pass), and where C_r lives during the forward sweep
@@ -806,7 +822,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
             if (ck.k > 0)          // the backward pass re-sweeps every row that is not kept
                 for (int r = 1; r < L; ++r) if (!ck.stored(r)) P->launches += P->row_pass[r + 1] - P->row_pass[r];
         }
-        if (config && ck.k == 0 && !count && !P->i16 && !dbg.nosweep && P->fplan.passes.size() <= (size_t)(4 * L + 8)) {
+        if (config && ck.k == 0 && !count && !P->i16 && !P->z2 && !dbg.nosweep && P->fplan.passes.size() <= (size_t)(4 * L + 8)) {
             // every pass in cta_per_inst mode: the pass table of fused_sweep_kernel (two instances per
             // CTA at a time where the constants of every pass fit, else one)
             std::vector<ttn::FusedParams> v(P->fplan.passes.size());

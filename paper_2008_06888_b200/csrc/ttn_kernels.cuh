@@ -338,6 +338,11 @@ __device__ __forceinline__ void argmax_combine(float& v, unsigned long long& s, 
     if (v2 > v || (v2 == v && s2 < s)) { v = v2; s = s2; }
 }
 
+// Z2 (h = 0, checkpoints are half-states over u = (s_1 .. s_{L-1}), column 0 up): the candidates of a row
+// are s = (0, u) with value C[u] + A(u) + Wj(u) and its flip (1, ~u), whose checkpoint entry is the same
+// (W[1, ~u] = W[0, u]), whose A is the same (no field) and whose bond term to the next row is -Wj(u):
+//     best of the pair = C[u] + A(u) + |Wj(u)|,   s = (0, u) if Wj(u) >= 0 else its global flip.
+template <bool Z2>
 __global__ void __launch_bounds__(256) argmax_partial_kernel(const ArgmaxParams p) {
     const unsigned long long inst = blockIdx.y;
     __shared__ float jsig[GMAX_L];      // coefficient of sigma_c: Jv sigma'_c + H_c (accumulated through row r)
@@ -360,30 +365,36 @@ __global__ void __launch_bounds__(256) argmax_partial_kernel(const ArgmaxParams 
     __syncthreads();
     // w(s) = sum_c jsig[c] sigma_c + sum_c kacc[c] sigma_c sigma_{c+1}, split into one 256-entry
     // table per byte of s (terms inside the byte) + one sign per byte boundary
-    __shared__ float tab[4][256];                    // L <= 28 for this call
+    __shared__ float tab[4][256];                    // L <= 32 (four bytes of s)
+    __shared__ float tabj[Z2 ? 4 : 1][256];          // Z2: the bond-to-next-row part on its own (tab holds A only)
     const int nchunk = (p.L + 7) >> 3;
     for (int m = 0; m < nchunk; ++m) {
         const int v = threadIdx.x;                   // blockDim.x = 256
-        float acc = 0.f;
+        float acc = 0.f, accj = 0.f;
         for (int i = 0; i < 8 && 8 * m + i < p.L; ++i) {
             const int c = 8 * m + i, b = (v >> i) & 1;
-            acc += b ? -jsig[c] : jsig[c];
+            if (Z2) accj += b ? -jsig[c] : jsig[c]; else acc += b ? -jsig[c] : jsig[c];
             if (i + 1 < 8 && c + 1 < p.L) acc += (b == ((v >> (i + 1)) & 1)) ? kacc[c] : -kacc[c];
         }
         tab[m][v] = acc;
+        if (Z2) tabj[m][v] = accj;
     }
     __syncthreads();
     const float* C = p.C + inst * p.c_stride;
     float bv = -INFINITY; unsigned long long bs = ~0ull;
-    for (unsigned long long s = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; s < p.NS;
-         s += (unsigned long long)gridDim.x * blockDim.x) {
+    const unsigned long long full = (p.L >= 64) ? ~0ull : ((1ull << p.L) - 1ull);
+    for (unsigned long long e = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; e < p.NS;
+         e += (unsigned long long)gridDim.x * blockDim.x) {
+        const unsigned long long s = Z2 ? e << 1 : e;         // Z2: e = u, the full index has column 0 up
         const unsigned long long x = s ^ (s >> 1);            // bit c set <=> sigma_c != sigma_{c+1}
-        float w = tab[0][s & 255u];
+        float w = tab[0][s & 255u], wj = Z2 ? tabj[0][s & 255u] : 0.f;
         for (int m = 1; m < nchunk; ++m) {
             w += tab[m][(s >> (8 * m)) & 255u];
+            if (Z2) wj += tabj[m][(s >> (8 * m)) & 255u];
             w += ((x >> (8 * m - 1)) & 1ull) ? -kacc[8 * m - 1] : kacc[8 * m - 1];
         }
-        argmax_combine(bv, bs, C[s] + w, s);
+        if (Z2) argmax_combine(bv, bs, C[e] + (w + fabsf(wj)), wj >= 0.f ? s : (~s & full));
+        else argmax_combine(bv, bs, C[s] + w, s);
     }
     for (int o = 16; o; o >>= 1) {
         float v2 = __shfl_xor_sync(0xffffffffu, bv, o);

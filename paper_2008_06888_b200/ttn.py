@@ -16,10 +16,10 @@ TROPICAL_F32 = 0
 COUNTING_F32_F64 = 1
 TROPICAL_I16 = 2
 CALL_ENERGY, CALL_COUNT, CALL_CONFIG, CALL_ENERGY_I16 = 0, 1, 2, 3
-CALL_ENERGY_Z2, CALL_COUNT_Z2, CALL_ENERGY_I16_Z2 = 4, 5, 6      # CALL_ENERGY / CALL_COUNT / CALL_ENERGY_I16 with the h = 0 flip-reduced half-state required (ttn.h)
+CALL_ENERGY_Z2, CALL_COUNT_Z2, CALL_ENERGY_I16_Z2, CALL_CONFIG_Z2 = 4, 5, 6, 7      # CALL_ENERGY / CALL_COUNT / CALL_ENERGY_I16 / CALL_CONFIG with the h = 0 flip-reduced half-state required (ttn.h)
 
 EXPORTS = [
-    "ttn_workspace_bytes", "ttn_sweep_energy", "ttn_sweep_energy_i16", "ttn_sweep_count", "ttn_ground_config",
+    "ttn_workspace_bytes", "ttn_workspace_bytes_h0", "ttn_sweep_energy", "ttn_sweep_energy_i16", "ttn_sweep_count", "ttn_ground_config",
     "ttn_potts3_sweep_energy", "ttn_potts3_sweep_count", "ttn_plan_create", "ttn_plan_launch",
     "ttn_plan_read", "ttn_plan_destroy", "ttn_plan_num_launches", "ttn_plan_num_passes",
     "ttn_plan_describe", "ttn_plan_state_elements", "ttn_last_error", "ttn_version",
@@ -49,6 +49,8 @@ def lib() -> ctypes.CDLL:
         vp, sz, ci = ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int
         L.ttn_workspace_bytes.argtypes = [ci, ci, ci, ci, ci]
         L.ttn_workspace_bytes.restype = sz
+        L.ttn_workspace_bytes_h0.argtypes = [ci, ci, ci, ci, ci]
+        L.ttn_workspace_bytes_h0.restype = sz
         L.ttn_sweep_energy.argtypes = [ci, fp, fp, fp, ci, vp, sz, vp, dp]
         L.ttn_sweep_energy_i16.argtypes = [ci, fp, fp, fp, ci, vp, sz, vp, dp]
         L.ttn_sweep_count.argtypes = [ci, fp, fp, fp, ci, vp, sz, vp, dp, dp]
@@ -106,8 +108,10 @@ def _couplings(Jh, Jv, h):
     return B, L, Jh, Jv, h
 
 
-def workspace_bytes(q: int, L: int, mode: int, batch: int, want_config: bool = False) -> int:
-    n = int(lib().ttn_workspace_bytes(q, L, mode, batch, int(want_config)))
+def workspace_bytes(q: int, L: int, mode: int, batch: int, want_config: bool = False, h_zero: bool = False) -> int:
+    """ttn_workspace_bytes, or ttn_workspace_bytes_h0 when the caller will pass no (or an all-zero) field."""
+    fn = lib().ttn_workspace_bytes_h0 if h_zero else lib().ttn_workspace_bytes
+    n = int(fn(q, L, mode, batch, int(want_config)))
     if n == 0:
         raise TTNError(2, f"unsupported q={q} L={L} mode={mode} batch={batch}")
     return n
@@ -144,7 +148,7 @@ class Plan:
         self.B, self.L, self.Jh, self.Jv, self.h = _couplings(Jh, Jv, h)
         self.q, self.call = q, call
         mode = _mode_of(call)
-        need = workspace_bytes(q, self.L, mode, self.B, call == CALL_CONFIG)
+        need = workspace_bytes(q, self.L, mode, self.B, call in (CALL_CONFIG, CALL_CONFIG_Z2), _h_zero(self.h))
         self.workspace = workspace if workspace is not None else alloc_workspace(need)
         if self.workspace.numel() * self.workspace.element_size() < need:
             raise TTNError(3, "workspace too small")
@@ -173,7 +177,7 @@ class Plan:
     def read(self, stream=None):
         E0 = np.zeros(self.B, dtype=np.float64)
         g = np.zeros(self.B, dtype=np.float64) if self.call in (CALL_COUNT, CALL_COUNT_Z2) else None
-        sig = np.zeros((self.B, self.L, self.L), dtype=np.int8) if self.call == CALL_CONFIG else None
+        sig = np.zeros((self.B, self.L, self.L), dtype=np.int8) if self.call in (CALL_CONFIG, CALL_CONFIG_Z2) else None
         _check(lib().ttn_plan_read(
             self._p, _stream_ptr(stream), E0.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
             g.ctypes.data_as(ctypes.POINTER(ctypes.c_double)) if g is not None else None,
@@ -192,6 +196,10 @@ class Plan:
             pass
 
 
+def _h_zero(h) -> bool:
+    return h is None or not np.any(h)
+
+
 def _mode_of(call: int) -> int:
     return {CALL_COUNT: COUNTING_F32_F64, CALL_COUNT_Z2: COUNTING_F32_F64, CALL_ENERGY_I16: TROPICAL_I16, CALL_ENERGY_I16_Z2: TROPICAL_I16}.get(call, TROPICAL_F32)
 
@@ -199,7 +207,7 @@ def _mode_of(call: int) -> int:
 def _one_call(fn_name, q, call, Jh, Jv, h, workspace, stream):
     B, L, Jh, Jv, h = _couplings(Jh, Jv, h)
     mode = _mode_of(call)
-    need = workspace_bytes(q, L, mode, B, call == CALL_CONFIG)
+    need = workspace_bytes(q, L, mode, B, call == CALL_CONFIG, q == 2 and _h_zero(h))
     ws = workspace if workspace is not None else alloc_workspace(need)
     wsb = ws.numel() * ws.element_size()
     E0 = np.zeros(B, dtype=np.float64)

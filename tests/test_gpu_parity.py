@@ -710,6 +710,56 @@ def test_ground_config_30x30_seeded():
     torch.cuda.empty_cache()
 
 
+@pytest.mark.parametrize("L", [14, 15, 16, 17, 20])
+def test_z2_ground_config_vs_oracle(L, monkeypatch):
+    """h = 0: ttn_ground_config on half-state checkpoints.  The backward pass takes, for every u, the
+    better of s = (0, u) and its global flip (same checkpoint entry, bond term to the next row of
+    opposite sign).  E0 bit-exact for +-J, Eq. (1) energy of sigma = E0; Gaussian J within tolerance."""
+    B = 3
+    Jh, Jv, _ = make_batch(L, range(4700, 4700 + B), "pmj")
+    p = ttn.Plan(2, ttn.CALL_CONFIG, Jh, Jv)
+    assert p.state_elements == 2 ** (L - 1)
+    p.launch(); E_z, _, sig = p.read(); p.close()
+    for b in range(B):
+        Eo = oracle.dp_ising(L, Jh[b], Jv[b], None, count=False)[0]
+        assert E_z[b] == Eo and oracle.ising_energy(L, Jh[b], Jv[b], None, sig[b]) == Eo
+    monkeypatch.setenv("TTN_DEBUG_CKPT_K", "4")                    # half-state checkpoints + recompute
+    E_k, sig_k = ttn.ground_config(Jh, Jv)
+    monkeypatch.delenv("TTN_DEBUG_CKPT_K")
+    assert np.array_equal(E_k, E_z) and np.array_equal(sig_k, sig)
+    Jh, Jv, _ = make_batch(L, range(4750, 4750 + B), "gauss")
+    E_g, sig_g = ttn.ground_config(Jh, Jv)
+    for b in range(B):
+        Eo = oracle.dp_ising(L, Jh[b], Jv[b], None, count=False)[0]
+        assert abs(E_g[b] - Eo) <= TOL * abs(Eo)
+        assert abs(oracle.ising_energy(L, Jh[b], Jv[b], None, sig_g[b]) - Eo) <= TOL * abs(Eo)
+    monkeypatch.setenv("TTN_DEBUG_Z2", "0")
+    E_f, sig_f = ttn.ground_config(Jh, Jv)
+    for b in range(B):                                             # full-state path: a ground state too
+        assert abs(E_f[b] - E_g[b]) <= TOL * abs(E_g[b])
+        assert abs(oracle.ising_energy(L, Jh[b], Jv[b], None, sig_f[b]) - E_g[b]) <= TOL * abs(E_g[b])
+
+
+def test_ground_config_32x32_planted():
+    """ttn_ground_config at 32 x 32 (the paper's largest lattice): h = 0, so the checkpoints
+    are half-states (8 GiB each), 7 kept + 5 ring buffers (104 GiB).  Planted instance = gauge-transformed
+    ferromagnet: E0 = -2L(L-1) and the returned configuration must be +-eps itself."""
+    import torch
+    L = 32
+    need = ttn.workspace_bytes(2, L, ttn.TROPICAL_F32, 1, True, h_zero=True)
+    free, _ = torch.cuda.mem_get_info()
+    if free < need + (2 << 30):
+        pytest.skip("needs %.0f GB of free device memory" % (need / 1e9))
+    rng = np.random.default_rng(3232)
+    eps = rng.choice([-1.0, 1.0], size=(L, L)).astype(np.float32)
+    Jh, Jv = (eps[:, :-1] * eps[:, 1:])[None], (eps[:-1, :] * eps[1:, :])[None]
+    E0, sig = ttn.ground_config(Jh, Jv)
+    assert E0[0] == -2 * L * (L - 1)
+    s = sig[0].astype(np.float32)
+    assert np.array_equal(s, eps) or np.array_equal(s, -eps)
+    torch.cuda.empty_cache()
+
+
 # ------------------------------------------------------------------ maximum sizes of the other calls
 def test_ground_config_28x28_planted():
     """ttn_ground_config at its size limit (28 checkpoints of 1 GiB).  Planted instance = gauge-

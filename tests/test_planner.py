@@ -439,6 +439,29 @@ def test_fused_row_aligned_schedule(L):
     assert done == L - 1
 
 
+@pytest.mark.parametrize("L", [14, 16, 21, 30, 32])
+def test_fused_z2_row_aligned_schedule(L):
+    """ttn_ground_config with h = 0: the row-aligned plan on the flip-reduced geometry (checkpoints are
+    half-states); rows complete in order, one flip gate (column 0) per row, src/dst chain intact."""
+    head, fpasses = parse_fused(describe(2, L, 7, fused=True))
+    flat = fused_to_gates(L, fpasses, config=True, z2=True)
+    assert len(flat) == L * (L - 1) == len(set(flat))
+    rows = [r for r, c in flat]
+    assert rows == sorted(rows)
+    assert sorted(r for r, c in flat if c == 0) == list(range(1, L))
+    assert fpasses[0]["gates"] == 0 and fpasses[0]["src"] == -1 and fpasses[0]["dst"] == 0
+    done, seen = 0, 0
+    for i, ps in enumerate(fpasses[1:], 1):
+        assert ps["src"] == fpasses[i - 1]["dst"]
+        seen += ps["gates"]
+        if seen == (done + 1) * L:
+            done += 1
+            assert ps["dst"] == done
+        else:
+            assert ps["dst"] == -1
+    assert done == L - 1
+
+
 @pytest.mark.parametrize("L", [12, 13, 16])
 def test_fused_schedule_replay_matches_oracle(L):
     _, fpasses = parse_fused(describe(2, L, 0, fused=True))
