@@ -456,6 +456,8 @@ class FusedScheduler {
         return true;
     }
     void set_max_row(int r) { max_row_ = r; }
+    // gate-row plans: the gates of the current row on columns >= c are someone else's: count them as done
+    void skip_columns_from(int c) { for (int i = c; i < L_; ++i) grow_[i] += 1; }
     int run_pass(int a, bool low, int max_gates, FusedPass& ps) {
         const int W = low ? G_.WLOW : G_.WHIGH;
         ps.a = a; ps.W = W; ps.low = low; ps.flags = 0; ps.n_phases = 0; ps.n_rounds = 0;
@@ -654,6 +656,33 @@ inline FusedPlan make_fused_row_plan(int L, int max_gates_per_pass, const FusedG
         if (!s.row_done(r)) return p;          // ok stays false
     }
     p.ok = true;
+    return p;
+}
+
+// ONE row of gates on every column of an L-column lattice (row 1 only; no INIT, no REDUCE pass): the
+// single-spin gates of the chimera sweep's horizontal couplings (ttn_chimera2.cuh), which run on the
+// Ising pass kernels.  One pass per tile of a column cover, all in place.
+// Columns >= ncols get no gate (the caller applies them elsewhere); the tiles cover [0, ncols).
+inline FusedPlan make_gate_row_plan(int L, int ncols, int max_gates_per_pass, const FusedGeom& G) {
+    FusedPlan p; p.L = L;
+    if (L < G.WLOW || ncols > L) return p;
+    std::vector<int> starts{0};
+    for (int x = G.WLOW; x < ncols; x += G.WHIGH) {
+        int a = x + G.WHIGH <= ncols ? x : ncols - G.WHIGH;
+        if (a < G.AMIN) a = G.AMIN;
+        starts.push_back(a);
+    }
+    FusedScheduler s(L, p, G);
+    s.set_max_row(1);
+    s.skip_columns_from(ncols);
+    for (size_t k = 0; k < starts.size(); ++k) {
+        FusedPass ps{};
+        const size_t m0 = p.mops.size();
+        const int n = s.run_pass(starts[k], starts[k] == 0, max_gates_per_pass, ps);
+        if (n == 0) { p.mops.resize(m0); continue; }
+        p.passes.push_back(ps);
+    }
+    p.ok = s.row_done(1);
     return p;
 }
 

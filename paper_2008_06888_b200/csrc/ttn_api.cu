@@ -21,6 +21,7 @@
 #include "ttn_fused.cuh"
 #include "ttn_fcount.cuh"
 #include "ttn_chimera.cuh"
+#include "ttn_chimera2.cuh"
 
 namespace {
 
@@ -991,8 +992,41 @@ ttn_status ttn_potts3_sweep_count(int L, const float* Jh, const float* Jv, int b
 }
 
 // ---- chimera graph, Tropical<i16> (ttn_chimera.cuh) ---------------------------
+}  // extern "C"
+
+// ---- chimera, M >= 4: the 16^M state of ttn_chimera2.cuh.  The horizontal couplings of a column are one
+// gate row of a 4M-column Ising lattice in Tropical<i16>: an internal plan drives the fused pass kernels.
+namespace {
+constexpr int CH2_MIN_M = 4;
+struct Chimera2Layout {
+    Layout lay;                 // of the internal Ising plan (state, programs; batch 1)
+    size_t fJh = 0, fJv = 0, gate_k = 0, final_tab = 0, tables = 0, out = 0, total = 0;
+};
+Chimera2Layout chimera2_layout(int M, int N, const DebugCfg& dbg) {
+    Chimera2Layout c;
+    const int NB = 4 * M, cols = N > 1 ? N - 1 : 1;
+    c.lay = make_layout(2, NB, false, false, 1, dbg, /*i16=*/true, false);
+    size_t off = c.lay.total;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+    c.fJh = take((size_t)cols * NB * (NB - 1) * 4 + 4);           // fake couplings, one "instance" per column
+    c.fJv = take((size_t)cols * (NB - 1) * NB * 4 + 4);
+    c.gate_k = take((size_t)cols * NB * 8 * 4);
+    c.final_tab = take((size_t)cols * ttn::FFINAL_FLOATS * 4);
+    c.tables = take((size_t)M * N * 128 * 4);
+    c.out = take(256);
+    c.total = off;
+    return c;
+}
+}  // namespace
+
+static ttn_status chimera2_sweep(int M, int N, const float* K, const float* Jv, const float* Jh, void* ws,
+                                 size_t wsb, void* stream, double* E0, const DebugCfg& dbg);
+
+extern "C" {
+
 size_t ttn_chimera_workspace_bytes(int M, int N) {
     if (M < 1 || M > 8 || N < 1 || N > 64) return 0;
+    if (M >= CH2_MIN_M) return chimera2_layout(M, N, read_debug()).total;
     return align_up((size_t)2 << (4 * M + 4)) + align_up((size_t)M * N * 128 * 4) + 256;
 }
 
@@ -1017,6 +1051,7 @@ ttn_status ttn_chimera_sweep_energy_i16(int M, int N, const float* K, const floa
     if (!scan(K, (size_t)M * N * 16) || (M > 1 && !scan(Jv, (size_t)(M - 1) * N * 4)) || (N > 1 && !scan(Jh, (size_t)M * (N - 1) * 4)))
         return fail(TTN_EINVAL, "chimera i16: couplings must be finite integers");
     if (total > 8000.0) return fail(TTN_EINVAL, "chimera i16: sum |J| = %.0f exceeds 8000", total);
+    if (M >= CH2_MIN_M) return chimera2_sweep(M, N, K, Jv, Jh, ws, wsb, stream, E0, dbg);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     unsigned char* base = static_cast<unsigned char*>(ws);
     unsigned* state = reinterpret_cast<unsigned*>(base);
@@ -1093,3 +1128,136 @@ ttn_status ttn_chimera_sweep_energy_i16(int M, int N, const float* K, const floa
 }
 
 }  // extern "C"
+
+// The cells' tables B(u, v) = sum_kl K[k][l] s_k(v) s_l(u), packed over the lowest bit of v: [cell][16 u][8 words]
+static void chimera_tables(int M, int N, const float* K, bool column_major, std::vector<unsigned>& tab) {
+    tab.assign((size_t)M * N * 128, 0u);
+    for (int r = 0; r < M; ++r)
+        for (int c = 0; c < N; ++c) {
+            const float* Kc = K + ((size_t)r * N + c) * 16;
+            const size_t cell = column_major ? (size_t)c * M + r : (size_t)r * N + c;
+            for (int u = 0; u < 16; ++u)
+                for (int j = 0; j < 8; ++j) {
+                    int val[2];
+                    for (int hlf = 0; hlf < 2; ++hlf) {
+                        const int v = 2 * j + hlf;
+                        int acc = 0;
+                        for (int k = 0; k < 4; ++k)
+                            for (int l = 0; l < 4; ++l)
+                                acc += (int)Kc[k * 4 + l] * (((v >> k) & 1) ? -1 : 1) * (((u >> l) & 1) ? -1 : 1);
+                        val[hlf] = acc;
+                    }
+                    tab[(cell * 16 + u) * 8 + j] = ((unsigned)val[0] & 0xffffu) | ((unsigned)val[1] << 16);
+                }
+        }
+}
+
+static ttn_status chimera2_sweep(int M, int N, const float* K, const float* Jv, const float* Jh, void* ws,
+                                 size_t wsb, void* stream, double* E0, const DebugCfg& dbg) {
+    (void)wsb;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int NB = 4 * M, cols = N - 1;
+    const Chimera2Layout cl = chimera2_layout(M, N, dbg);
+    unsigned char* base = static_cast<unsigned char*>(ws);
+    int dev = 0, major = 0, sms = 0;
+    TTN_CUDA(cudaGetDevice(&dev));
+    TTN_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10) return fail(TTN_EUNSUPPORTED, "device compute capability %d.x is not sm_100", major);
+    TTN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    // ---- tables of the cells, column-major, and the deferred constant of every gate
+    std::vector<unsigned> tab;
+    chimera_tables(M, N, K, /*column_major=*/true, tab);
+    TTN_CUDA(cudaMemcpyAsync(base + cl.tables, tab.data(), tab.size() * 4, cudaMemcpyHostToDevice, st));
+    const int int_min = -2147483647 - 1;
+    TTN_CUDA(cudaMemcpyAsync(base + cl.out, &int_min, sizeof(int), cudaMemcpyHostToDevice, st));
+    long shift = 0;
+    for (size_t i = 0; i < (size_t)(M - 1) * N * 4; ++i) shift += (long)Jv[i];
+    for (size_t i = 0; i < (size_t)M * (N - 1) * 4; ++i) shift += (long)Jh[i];
+    // ---- the internal Ising plan: one gate row over the 4M bits of u, Tropical<i16>
+    ttn_plan P{};
+    P.q = 2; P.L = NB; P.batch = 1; P.call = TTN_CALL_ENERGY_I16; P.count = false; P.config = false; P.has_field = false;
+    P.fused = true; P.i16 = true; P.z2 = false; P.dbg = dbg; P.lay = cl.lay; P.ws = base; P.sms = sms;
+    std::vector<float> fJv, fJh;
+    if (cols > 0) {
+        P.fplan = ttn::make_gate_row_plan(NB, NB - 1, ttn::FMAX_GATES, ttn::GEOM_I16);     // the top bit: column kernel
+        if (!P.fplan.ok) return fail(TTN_EUNSUPPORTED, "chimera: no gate-row schedule for %d bits", NB);
+        // fake lattice per column c >= 1: Jv[0][4 r + l] = Jh_chimera[r][c-1][l], everything else 0, so that the
+        // conjugation A_0 of the diagonal frame is the identity and gate (1, b) is the plain gate (A2) on bit b
+        fJv.assign((size_t)cols * (NB - 1) * NB, 0.f);
+        fJh.assign((size_t)cols * NB * (NB - 1), 0.f);
+        for (int c = 1; c < N; ++c)
+            for (int r = 0; r < M; ++r)
+                for (int l = 0; l < 4; ++l)
+                    fJv[(size_t)(c - 1) * (NB - 1) * NB + 4 * r + l] = Jh[((size_t)r * (N - 1) + (c - 1)) * 4 + l];
+        TTN_CUDA(cudaMemcpyAsync(base + cl.fJv, fJv.data(), fJv.size() * 4, cudaMemcpyHostToDevice, st));
+        TTN_CUDA(cudaMemcpyAsync(base + cl.fJh, fJh.data(), fJh.size() * 4, cudaMemcpyHostToDevice, st));
+        const ttn::FusedPlan& fp = P.fplan;
+        if ((int)fp.gate_rc.size() > cl.lay.f_max_gates || (int)fp.mops.size() > cl.lay.f_max_mops)
+            return fail(TTN_EUNSUPPORTED, "chimera: gate-row plan exceeds its workspace bounds");
+        TTN_CUDA(cudaMemcpyAsync(base + cl.lay.f_mops, fp.mops.data(), fp.mops.size() * sizeof(ttn::MicroOp), cudaMemcpyHostToDevice, st));
+        TTN_CUDA(cudaMemcpyAsync(base + cl.lay.f_gate_rc, fp.gate_rc.data(), fp.gate_rc.size() * 4, cudaMemcpyHostToDevice, st));
+        ttn::FusedPrepParams q{};
+        q.L = NB; q.n_gates = (int)fp.gate_rc.size();
+        q.gate_rc = reinterpret_cast<const int*>(base + cl.lay.f_gate_rc);
+        q.Jh = reinterpret_cast<const float*>(base + cl.fJh);
+        q.Jv = reinterpret_cast<const float*>(base + cl.fJv);
+        q.h = nullptr;
+        q.gate_k = reinterpret_cast<float*>(base + cl.gate_k);
+        q.final_tab = reinterpret_cast<float*>(base + cl.final_tab);
+        q.fin_low = 1; q.fin_layout = 1; q.fin_a = 0; q.col_off = 0;
+        long work = ttn::FFINAL_FLOATS; if (q.n_gates > work) work = q.n_gates;
+        ttn::fused16_prep_kernel<<<dim3((unsigned)((work + 255) / 256), (unsigned)cols), 256, 0, st>>>(q);
+        TTN_CUDA(cudaGetLastError());
+        TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<true, 1, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(true, 1)));
+        TTN_CUDA(cudaFuncSetAttribute(ttn::fused_pass_kernel<false, 1, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::fsmem_bytes(false, 1)));
+        P.fused_grid = sms;
+    }
+    ttn::ChimeraColumnParams cp{};
+    cp.state = reinterpret_cast<unsigned*>(base + cl.lay.x);
+    cp.M = M;
+    cp.tiles = 1ull << (NB - 12);
+    cp.out = reinterpret_cast<int*>(base + cl.out);
+    const unsigned long long need = ((cp.tiles >> 1) + ttn::CH2_WARPS - 1) / ttn::CH2_WARPS;      // a warp takes a tile pair
+    const unsigned cgrid = (unsigned)(need < 2ull * sms ? need : 2ull * sms);
+    std::vector<cudaEvent_t> ev;               // TTN_DEBUG_TIMING: per-launch device times on stderr
+    auto stamp = [&]() { if (dbg.timing) { cudaEvent_t e; cudaEventCreate(&e); cudaEventRecord(e, st); ev.push_back(e); } };
+    stamp();
+    for (int c = 0; c < N; ++c) {
+        if (c > 0) {
+            // the column's constants: instance c - 1 of the prep kernel's output
+            P.lay.f_gate_k = cl.gate_k + (size_t)(c - 1) * P.fplan.gate_rc.size() * 32;
+            for (const ttn::FusedPass& ps : P.fplan.passes) {
+                ttn_status s = launch_fused_pass(&P, ps, st);
+                if (s != TTN_OK) return s;
+                stamp();
+            }
+        }
+        cp.init = (c == 0); cp.reduce = (c == N - 1);
+        {
+            const int J = c > 0 ? (int)Jh[((size_t)(M - 1) * (N - 1) + (c - 1)) * 4 + 3] : 0;
+            const unsigned h = (unsigned)(-2 * J) & 0xffffu;
+            cp.ju_top = h | (h << 16);
+        }
+        cp.tables = reinterpret_cast<const unsigned*>(base + cl.tables) + (size_t)c * M * 128;
+        for (int r = 0; r < 8; ++r)
+            for (int k = 0; k < 4; ++k) {
+                const int J = (r >= 1 && r < M) ? (int)Jv[((size_t)(r - 1) * N + c) * 4 + k] : 0;
+                const unsigned h = (unsigned)(-2 * J) & 0xffffu;
+                cp.jv[r][k] = h | (h << 16);
+            }
+        ttn::chimera_column_kernel<<<cgrid, ttn::CH2_WARPS * 32, 0, st>>>(cp);
+        TTN_CUDA(cudaGetLastError());
+        stamp();
+    }
+    if (dbg.timing) {
+        cudaStreamSynchronize(st);
+        for (size_t i = 1; i < ev.size(); ++i) { float ms = 0; cudaEventElapsedTime(&ms, ev[i - 1], ev[i]); fprintf(stderr, "chimera launch %2zu : %.2f ms\n", i - 1, ms); }
+        for (auto& e : ev) cudaEventDestroy(e);
+    }
+    int mx = 0;
+    TTN_CUDA(cudaMemcpyAsync(&mx, base + cl.out, sizeof(int), cudaMemcpyDeviceToHost, st));
+    TTN_CUDA(cudaStreamSynchronize(st));
+    const long top = (long)mx + shift;
+    *E0 = top == 0 ? 0.0 : -(double)top;
+    return TTN_OK;
+}
