@@ -135,6 +135,16 @@ ttn_status ttn_chimera_sweep_energy_i16(int M, int N, const float* K, const floa
                                         void* workspace, size_t workspace_bytes, void* stream,
                                         double* E0 /*[1]*/);
 
+/* Ground-state energy AND degeneracy on the chimera graph (CountingTropical, Eq. (4) PAPER.md:78-83;
+ * the residual entropies of PAPER.md:128, Fig. 3): same arguments and conventions as
+ * ttn_chimera_sweep_energy_i16, elements (x f32, n f64), 12 bytes per state of the 16^max(M,3) column
+ * front (M = 8: 48 GiB).  Couplings must be integer-valued (exact f32 sums and exact ties), else
+ * TTN_EINVAL.  degeneracy is exact below 2^53 and a correctly rounded f64 product / sum above. */
+size_t ttn_chimera_count_workspace_bytes(int M, int N);
+ttn_status ttn_chimera_sweep_count(int M, int N, const float* K, const float* Jv, const float* Jh,
+                                   void* workspace, size_t workspace_bytes, void* stream,
+                                   double* E0 /*[1]*/, double* degeneracy /*[1]*/);
+
 /* ---- split API: upload once, launch asynchronously, read later ---------------------------
  * The one-call functions above are ttn_plan_create + ttn_plan_launch + ttn_plan_read +
  * ttn_plan_destroy.  A plan holds the host-side pass schedule (which gates

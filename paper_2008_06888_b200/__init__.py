@@ -7,5 +7,5 @@ from .ttn import (  # noqa: F401
     TROPICAL_F32, COUNTING_F32_F64, TROPICAL_I16, CALL_ENERGY, CALL_COUNT, CALL_CONFIG, CALL_ENERGY_I16, CALL_ENERGY_Z2, CALL_COUNT_Z2, CALL_ENERGY_I16_Z2, CALL_CONFIG_Z2, EXPORTS,
     TTNError, Plan, lib, workspace_bytes, alloc_workspace, plan_describe,
     sweep_energy, sweep_energy_i16, sweep_count, ground_config, potts3_sweep_energy, potts3_sweep_count,
-    chimera_workspace_bytes, chimera_sweep_energy_i16,
+    chimera_workspace_bytes, chimera_sweep_energy_i16, chimera_count_workspace_bytes, chimera_sweep_count,
 )

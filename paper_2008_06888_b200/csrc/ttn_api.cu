@@ -1022,7 +1022,35 @@ Chimera2Layout chimera2_layout(int M, int N, const DebugCfg& dbg) {
 static ttn_status chimera2_sweep(int M, int N, const float* K, const float* Jv, const float* Jh, void* ws,
                                  size_t wsb, void* stream, double* E0, const DebugCfg& dbg);
 
+// counting: rows of cells are padded with coupling-free cells up to CHC_MIN_M (each adds 8 free spins: x 2^8)
+namespace {
+constexpr int CHC_MIN_M = 3;
+struct ChimeraCountLayout {
+    Layout lay;                 // of the internal counting Ising plan (x, n, programs; batch 1)
+    size_t fJh = 0, fJv = 0, gate_k = 0, final_tab = 0, tables = 0, total = 0;
+};
+ChimeraCountLayout chimera_count_layout(int Mp, int N, const DebugCfg& dbg) {
+    ChimeraCountLayout c;
+    const int NB = 4 * Mp, cols = N > 1 ? N - 1 : 1;
+    c.lay = make_layout(2, NB, true, false, 1, dbg, false, false);
+    size_t off = c.lay.total;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+    c.fJh = take((size_t)cols * NB * (NB - 1) * 4 + 4);
+    c.fJv = take((size_t)cols * (NB - 1) * NB * 4 + 4);
+    c.gate_k = take((size_t)cols * NB * 8 * 4);
+    c.final_tab = take((size_t)cols * ttn::CFINAL_FLOATS * 4);
+    c.tables = take((size_t)Mp * N * 256 * 4);
+    c.total = off;
+    return c;
+}
+}  // namespace
+
 extern "C" {
+
+size_t ttn_chimera_count_workspace_bytes(int M, int N) {
+    if (M < 1 || M > 8 || N < 1 || N > 64) return 0;
+    return chimera_count_layout(M < CHC_MIN_M ? CHC_MIN_M : M, N, read_debug()).total;
+}
 
 size_t ttn_chimera_workspace_bytes(int M, int N) {
     if (M < 1 || M > 8 || N < 1 || N > 64) return 0;
@@ -1259,5 +1287,130 @@ static ttn_status chimera2_sweep(int M, int N, const float* K, const float* Jv, 
     TTN_CUDA(cudaStreamSynchronize(st));
     const long top = (long)mx + shift;
     *E0 = top == 0 ? 0.0 : -(double)top;
+    return TTN_OK;
+}
+
+// ---- chimera, CountingTropical (ttn_chimera2.cuh, second half) ----------------------------------------
+extern "C" ttn_status ttn_chimera_sweep_count(int M, int N, const float* K, const float* Jv, const float* Jh,
+                                               void* ws, size_t wsb, void* stream, double* E0, double* degeneracy) {
+    if (M < 1 || N < 1 || !K || !E0 || !degeneracy || !ws || (M > 1 && !Jv) || (N > 1 && !Jh)) return fail(TTN_EINVAL, "bad argument");
+    if (M > 8 || N > 64) return fail(TTN_EUNSUPPORTED, "chimera: M <= 8 rows of cells, N <= 64");
+    const size_t need = ttn_chimera_count_workspace_bytes(M, N);
+    if (wsb < need) return fail(TTN_ENOMEM, "workspace too small: %zu < %zu", wsb, need);
+    if ((uintptr_t)ws % 256) return fail(TTN_EINVAL, "workspace must be 256-byte aligned");
+    const DebugCfg dbg = read_debug();
+    double total = 0;
+    auto scan = [&](const float* a, size_t n) {
+        for (size_t i = 0; i < n; ++i) {
+            const double x = (double)a[i];
+            if (!std::isfinite(x) || x != std::nearbyint(x)) return false;
+            total += std::fabs(x);
+        }
+        return true;
+    };
+    if (!scan(K, (size_t)M * N * 16) || (M > 1 && !scan(Jv, (size_t)(M - 1) * N * 4)) || (N > 1 && !scan(Jh, (size_t)M * (N - 1) * 4)))
+        return fail(TTN_EINVAL, "chimera count: couplings must be finite integers");
+    if (total > 4.0e6) return fail(TTN_EINVAL, "chimera count: sum |J| = %.0f exceeds the exact f32 integer range", total);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int Mp = M < CHC_MIN_M ? CHC_MIN_M : M, NB = 4 * Mp, cols = N - 1;
+    const ChimeraCountLayout cl = chimera_count_layout(Mp, N, dbg);
+    unsigned char* base = static_cast<unsigned char*>(ws);
+    int dev = 0, major = 0, sms = 0;
+    TTN_CUDA(cudaGetDevice(&dev));
+    TTN_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10) return fail(TTN_EUNSUPPORTED, "device compute capability %d.x is not sm_100", major);
+    TTN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    // ---- tables B_r(u, v) of every cell as floats, column-major [c][r][16 u][16 v]; padded rows are zero
+    std::vector<float> tab((size_t)Mp * N * 256, 0.f);
+    for (int r = 0; r < M; ++r)
+        for (int c = 0; c < N; ++c) {
+            const float* Kc = K + ((size_t)r * N + c) * 16;
+            float* out = tab.data() + ((size_t)c * Mp + r) * 256;
+            for (int u = 0; u < 16; ++u)
+                for (int v = 0; v < 16; ++v) {
+                    int acc = 0;
+                    for (int k = 0; k < 4; ++k)
+                        for (int l = 0; l < 4; ++l)
+                            acc += (int)Kc[k * 4 + l] * (((v >> k) & 1) ? -1 : 1) * (((u >> l) & 1) ? -1 : 1);
+                    out[u * 16 + v] = (float)acc;
+                }
+        }
+    TTN_CUDA(cudaMemcpyAsync(base + cl.tables, tab.data(), tab.size() * 4, cudaMemcpyHostToDevice, st));
+    double shift = 0;
+    for (size_t i = 0; i < (size_t)(M - 1) * N * 4; ++i) shift += (double)Jv[i];
+    for (size_t i = 0; i < (size_t)M * (N - 1) * 4; ++i) shift += (double)Jh[i];
+    // ---- the internal counting Ising plan: one gate row over the 4 Mp bits of u
+    ttn_plan P{};
+    P.q = 2; P.L = NB; P.batch = 1; P.call = TTN_CALL_COUNT; P.count = true; P.config = false; P.has_field = false;
+    P.fused = true; P.i16 = false; P.z2 = false; P.dbg = dbg; P.lay = cl.lay; P.ws = base; P.sms = sms;
+    std::vector<float> fJv, fJh;
+    if (cols > 0) {
+        P.fplan = ttn::make_gate_row_plan(NB, NB, ttn::FMAX_GATES, ttn::GEOM_COUNT);
+        if (!P.fplan.ok) return fail(TTN_EUNSUPPORTED, "chimera count: no gate-row schedule for %d bits", NB);
+        fJv.assign((size_t)cols * (NB - 1) * NB, 0.f);
+        fJh.assign((size_t)cols * NB * (NB - 1), 0.f);
+        for (int c = 1; c < N; ++c)
+            for (int r = 0; r < M; ++r)
+                for (int l = 0; l < 4; ++l)
+                    fJv[(size_t)(c - 1) * (NB - 1) * NB + 4 * r + l] = Jh[((size_t)r * (N - 1) + (c - 1)) * 4 + l];
+        TTN_CUDA(cudaMemcpyAsync(base + cl.fJv, fJv.data(), fJv.size() * 4, cudaMemcpyHostToDevice, st));
+        TTN_CUDA(cudaMemcpyAsync(base + cl.fJh, fJh.data(), fJh.size() * 4, cudaMemcpyHostToDevice, st));
+        const ttn::FusedPlan& fp = P.fplan;
+        if ((int)fp.gate_rc.size() > cl.lay.f_max_gates || (int)fp.mops.size() > cl.lay.f_max_mops)
+            return fail(TTN_EUNSUPPORTED, "chimera count: gate-row plan exceeds its workspace bounds");
+        TTN_CUDA(cudaMemcpyAsync(base + cl.lay.f_mops, fp.mops.data(), fp.mops.size() * sizeof(ttn::MicroOp), cudaMemcpyHostToDevice, st));
+        TTN_CUDA(cudaMemcpyAsync(base + cl.lay.f_gate_rc, fp.gate_rc.data(), fp.gate_rc.size() * 4, cudaMemcpyHostToDevice, st));
+        ttn::CountPrepParams q{};
+        q.L = NB; q.n_gates = (int)fp.gate_rc.size();
+        q.gate_rc = reinterpret_cast<const int*>(base + cl.lay.f_gate_rc);
+        q.Jh = reinterpret_cast<const float*>(base + cl.fJh);
+        q.Jv = reinterpret_cast<const float*>(base + cl.fJv);
+        q.h = nullptr;
+        q.gate_k = reinterpret_cast<float*>(base + cl.gate_k);
+        q.final_tab = reinterpret_cast<float*>(base + cl.final_tab);
+        q.fin_low = 1; q.fin_layout = 1; q.fin_a = 0; q.col_off = 0;
+        long work = ttn::CFINAL_FLOATS; if (q.n_gates > work) work = q.n_gates;
+        ttn::fcount_prep_kernel<<<dim3((unsigned)((work + 255) / 256), (unsigned)cols), 256, 0, st>>>(q);
+        TTN_CUDA(cudaGetLastError());
+        TTN_CUDA(cudaFuncSetAttribute(ttn::fcount_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::csmem_bytes()));
+        TTN_CUDA(cudaFuncSetAttribute(ttn::fcount_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ttn::csmem_bytes()));
+        P.fused_grid = sms;
+    }
+    ttn::ChimeraCountParams cp{};
+    cp.x = reinterpret_cast<float*>(base + cl.lay.x);
+    cp.n = reinterpret_cast<double*>(base + cl.lay.n);
+    cp.M = Mp;
+    cp.tiles = 1ull << (NB - 12);
+    cp.part_x = reinterpret_cast<float*>(base + cl.lay.part_x);
+    cp.part_n = reinterpret_cast<double*>(base + cl.lay.part_n);
+    const unsigned long long needc = (cp.tiles + ttn::CH2C_WARPS - 1) / ttn::CH2C_WARPS;
+    const unsigned cgrid = (unsigned)(needc < (unsigned long long)sms ? needc : (unsigned long long)sms);
+    if ((unsigned long long)cgrid > cl.lay.max_tiles) return fail(TTN_EUNSUPPORTED, "chimera count: partials do not fit");
+    for (int c = 0; c < N; ++c) {
+        if (c > 0) {
+            P.lay.f_gate_k = cl.gate_k + (size_t)(c - 1) * P.fplan.gate_rc.size() * 32;
+            for (const ttn::FusedPass& ps : P.fplan.passes) {
+                ttn_status s = launch_fcount_pass(&P, ps, st);
+                if (s != TTN_OK) return s;
+            }
+        }
+        cp.init = (c == 0); cp.reduce = (c == N - 1);
+        cp.tables = reinterpret_cast<const float*>(base + cl.tables) + (size_t)c * Mp * 256;
+        for (int r = 0; r < 8; ++r)
+            for (int k = 0; k < 4; ++k)
+                cp.jv[r][k] = (r >= 1 && r < M) ? -2.f * Jv[((size_t)(r - 1) * N + c) * 4 + k] : 0.f;
+        ttn::chimera_column_count_kernel<<<cgrid, ttn::CH2C_WARPS * 32, 0, st>>>(cp);
+        TTN_CUDA(cudaGetLastError());
+    }
+    ttn::final_reduce_kernel<true><<<1, 256, 0, st>>>(cp.part_x, cp.part_n, (unsigned long long)cgrid,
+                                                     reinterpret_cast<float*>(base + cl.lay.out_x), reinterpret_cast<double*>(base + cl.lay.out_n));
+    TTN_CUDA(cudaGetLastError());
+    float mx = 0; double g = 0;
+    TTN_CUDA(cudaMemcpyAsync(&mx, base + cl.lay.out_x, sizeof(float), cudaMemcpyDeviceToHost, st));
+    TTN_CUDA(cudaMemcpyAsync(&g, base + cl.lay.out_n, sizeof(double), cudaMemcpyDeviceToHost, st));
+    TTN_CUDA(cudaStreamSynchronize(st));
+    const double top = (double)mx + shift;
+    *E0 = top == 0.0 ? 0.0 : -top;
+    *degeneracy = std::ldexp(g, -8 * N * (Mp - M));          // the padded cells' free spins (exact: a power of two)
     return TTN_OK;
 }

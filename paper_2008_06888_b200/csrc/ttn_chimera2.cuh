@@ -170,3 +170,139 @@ __global__ void __launch_bounds__(CH2_WARPS * 32, 2) chimera_column_kernel(const
 }
 
 }  // namespace ttn
+
+// =============================================================================================
+// CountingTropical form (Eq. (4); the chimera entropies of PAPER.md:128, Fig. 3): the
+// same column sweep with elements (x f32, n f64), structure of arrays.  The horizontal couplings run
+// as one gate row on the counting Ising pass kernels (ttn_fcount.cuh); the column's vertical chain
+// is contracted on the fly in CountingTropical arithmetic:
+//     (x, n) (+) (y, m) = (max, counts added on exact ties),   (x, n) (.) (y, m) = (x + y, n m),
+//     F[u] <- F[u] (.) G_c(u),   G_c(u) = (+)_{v^0..v^{M-1}} (.)_r B_r(u^r, v^r) (.) V_{r-1}(v^{r-1}, v^r).
+// Couplings are integers (the caller checks), so f32 sums are exact and ties are exact ties.
+// Same tile as the Tropical<i16> kernel: a warp owns (u^0, u^1, u^2), lane = (bit 3 of u^0, u^1), the lane's
+// elements of one u^2 value are 8 consecutive floats / doubles.
+namespace ttn {
+
+struct ChimeraCountParams {
+    float* x; double* n;          // 2^(4M) elements each
+    int M;                        // rows of cells, 3 <= M <= 8
+    int init, reduce;
+    unsigned long long tiles;     // 2^(4M-12)
+    const float* tables;          // [M rows][16 u][16 v]: B_r(u, v) of this column
+    float jv[8][4];               // [r][k] = -2 Jv[r-1][c][k]; row 0 unused
+    float* part_x; double* part_n;   // [gridDim.x] (reduce)
+};
+
+__device__ __forceinline__ double ch2_ind(bool p) { return __hiloint2double(p ? 0x3ff00000 : 0, 0); }
+
+// the four single-spin counting gates of one vertical coupling group on a 16-vector over v
+__device__ __forceinline__ void ch2_cvgates(float (&x)[16], double (&n)[16], const float* m2) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int B = 1 << k;
+        const float m = m2[k];
+#pragma unroll
+        for (int v = 0; v < 16; ++v) {
+            if (v & B) continue;
+            const float xa = x[v], xb = x[v | B];
+            const double na = n[v], nb = n[v | B];
+            const float ca = xb + m, cb = xa + m;
+            n[v] = fma(nb, ch2_ind(ca >= xa), na * ch2_ind(xa >= ca));
+            n[v | B] = fma(na, ch2_ind(cb >= xb), nb * ch2_ind(xb >= cb));
+            x[v] = fmaxf(xa, ca);
+            x[v | B] = fmaxf(xb, cb);
+        }
+    }
+}
+
+constexpr int CH2C_WARPS = 8;
+
+__global__ void __launch_bounds__(CH2C_WARPS * 32, 1) chimera_column_count_kernel(const ChimeraCountParams q) {
+    __shared__ float s_tab[8][16][16];
+    __shared__ float s_jv[8][4];
+    __shared__ float s_redx[CH2C_WARPS];
+    __shared__ double s_redn[CH2C_WARPS];
+    for (int i = threadIdx.x; i < q.M * 256; i += blockDim.x) (&s_tab[0][0][0])[i] = q.tables[i];
+    if (threadIdx.x < 32) (&s_jv[0][0])[threadIdx.x] = q.jv[threadIdx.x >> 2][threadIdx.x & 3];
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int u1 = lane >> 1, u0hi = 8 * (lane & 1);
+    float best = -INFINITY; double bcnt = 0.0;
+    const unsigned long long nw = (unsigned long long)gridDim.x * CH2C_WARPS;
+    for (unsigned long long tile = (unsigned long long)blockIdx.x * CH2C_WARPS + warp; tile < q.tiles; tile += nw) {
+        // ---- levels M-1 .. 3: uniform per tile
+        float b3x[16]; double b3n[16];
+#pragma unroll
+        for (int v = 0; v < 16; ++v) { b3x[v] = 0.f; b3n[v] = 1.0; }
+        for (int r = q.M - 1; r >= 3; --r) {
+            const int ur = (int)((tile >> (4 * (r - 3))) & 15ull);
+#pragma unroll
+            for (int v = 0; v < 16; ++v) b3x[v] += s_tab[r][ur][v];
+            ch2_cvgates(b3x, b3n, s_jv[r]);
+        }
+        float* px = q.x + (tile << 12) + 8 * lane;
+        double* pn = q.n + (tile << 12) + 8 * lane;
+#pragma unroll 1
+        for (int i = 0; i < 16; ++i) {               // u^2 = i
+            float fx[8]; double fn[8];
+            if (!q.init) {
+                const float4 a = *reinterpret_cast<const float4*>(px + 256 * i), b = *reinterpret_cast<const float4*>(px + 256 * i + 4);
+                fx[0] = a.x; fx[1] = a.y; fx[2] = a.z; fx[3] = a.w; fx[4] = b.x; fx[5] = b.y; fx[6] = b.z; fx[7] = b.w;
+#pragma unroll
+                for (int t = 0; t < 8; t += 2) {
+                    const double2 d = *reinterpret_cast<const double2*>(pn + 256 * i + t);
+                    fn[t] = d.x; fn[t + 1] = d.y;
+                }
+            } else {
+#pragma unroll
+                for (int t = 0; t < 8; ++t) { fx[t] = 0.f; fn[t] = 1.0; }
+            }
+            float x[16]; double n[16];
+#pragma unroll
+            for (int v = 0; v < 16; ++v) { x[v] = b3x[v] + s_tab[2][i][v]; n[v] = b3n[v]; }
+            ch2_cvgates(x, n, s_jv[2]);                                             // b_2 over v^1
+#pragma unroll
+            for (int v = 0; v < 16; ++v) x[v] += s_tab[1][u1][v];                   // a_1
+            ch2_cvgates(x, n, s_jv[1]);                                             // b_1 over v^0
+#pragma unroll
+            for (int t = 0; t < 8; ++t) {            // G(u) = (+)_v B_0(u^0, v) (.) b_1[v]
+                float c[16];
+                float g = -INFINITY;
+#pragma unroll
+                for (int v = 0; v < 16; ++v) { c[v] = s_tab[0][u0hi + t][v] + x[v]; g = fmaxf(g, c[v]); }
+                double gn = 0.0;
+#pragma unroll
+                for (int v = 0; v < 16; ++v) gn = fma(n[v], ch2_ind(c[v] == g), gn);
+                fx[t] += g; fn[t] *= gn;
+            }
+            if (q.reduce) {
+#pragma unroll
+                for (int t = 0; t < 8; ++t) {
+                    if (fx[t] > best) { best = fx[t]; bcnt = fn[t]; } else if (fx[t] == best) bcnt += fn[t];
+                }
+            } else {
+                *reinterpret_cast<float4*>(px + 256 * i) = make_float4(fx[0], fx[1], fx[2], fx[3]);
+                *reinterpret_cast<float4*>(px + 256 * i + 4) = make_float4(fx[4], fx[5], fx[6], fx[7]);
+#pragma unroll
+                for (int t = 0; t < 8; t += 2) *reinterpret_cast<double2*>(pn + 256 * i + t) = make_double2(fn[t], fn[t + 1]);
+            }
+        }
+    }
+    if (q.reduce) {
+        float m = best;
+        for (int o = 16; o; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+        double c = best == m ? bcnt : 0.0;
+        for (int o = 16; o; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+        if (lane == 0) { s_redx[warp] = m; s_redn[warp] = c; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            float mm = s_redx[0];
+            for (int w = 1; w < CH2C_WARPS; ++w) mm = fmaxf(mm, s_redx[w]);
+            double cc = 0.0;
+            for (int w = 0; w < CH2C_WARPS; ++w) if (s_redx[w] == mm) cc += s_redn[w];
+            q.part_x[blockIdx.x] = mm; q.part_n[blockIdx.x] = cc;
+        }
+    }
+}
+
+}  // namespace ttn

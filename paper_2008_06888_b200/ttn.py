@@ -24,6 +24,7 @@ EXPORTS = [
     "ttn_plan_read", "ttn_plan_destroy", "ttn_plan_num_launches", "ttn_plan_num_passes",
     "ttn_plan_describe", "ttn_plan_state_elements", "ttn_last_error", "ttn_version",
     "ttn_chimera_workspace_bytes", "ttn_chimera_sweep_energy_i16",
+    "ttn_chimera_count_workspace_bytes", "ttn_chimera_sweep_count",
 ]
 
 _STATUS = {1: "TTN_EINVAL", 2: "TTN_EUNSUPPORTED", 3: "TTN_ENOMEM", 4: "TTN_ECUDA"}
@@ -72,6 +73,9 @@ def lib() -> ctypes.CDLL:
         L.ttn_chimera_workspace_bytes.argtypes = [ci, ci]
         L.ttn_chimera_workspace_bytes.restype = sz
         L.ttn_chimera_sweep_energy_i16.argtypes = [ci, ci, fp, fp, fp, vp, sz, vp, dp]
+        L.ttn_chimera_count_workspace_bytes.argtypes = [ci, ci]
+        L.ttn_chimera_count_workspace_bytes.restype = sz
+        L.ttn_chimera_sweep_count.argtypes = [ci, ci, fp, fp, fp, vp, sz, vp, dp, dp]
         _lib = L
     return _lib
 
@@ -278,3 +282,29 @@ def chimera_sweep_energy_i16(K, Jv, Jh, workspace=None, stream=None) -> float:
                                               ws.numel() * ws.element_size(), _stream_ptr(stream),
                                               E0.ctypes.data_as(ctypes.POINTER(ctypes.c_double))))
     return float(E0[0])
+
+
+def chimera_count_workspace_bytes(M: int, N: int) -> int:
+    n = lib().ttn_chimera_count_workspace_bytes(M, N)
+    if n == 0:
+        raise TTNError(2, f"chimera: unsupported size M={M}, N={N}")
+    return n
+
+
+def chimera_sweep_count(K, Jv, Jh, workspace=None, stream=None) -> Tuple[float, float]:
+    """ttn_chimera_sweep_count: (E0, degeneracy) of the integer-coupling spin glass on the chimera graph."""
+    K = np.ascontiguousarray(np.asarray(K, dtype=np.float32))
+    if K.ndim != 4 or K.shape[2:] != (4, 4):
+        raise ValueError(f"K: expected shape [M, N, 4, 4], got {K.shape}")
+    M, N = K.shape[:2]
+    Jv = _f32(Jv, (M - 1, N, 4), "Jv")
+    Jh = _f32(Jh, (M, N - 1, 4), "Jh")
+    need = chimera_count_workspace_bytes(M, N)
+    ws = workspace if workspace is not None else alloc_workspace(need)
+    E0 = np.zeros(1, dtype=np.float64)
+    g = np.zeros(1, dtype=np.float64)
+    dp = ctypes.POINTER(ctypes.c_double)
+    _check(lib().ttn_chimera_sweep_count(M, N, _fptr(K), _fptr(Jv), _fptr(Jh), ws.data_ptr(),
+                                         ws.numel() * ws.element_size(), _stream_ptr(stream),
+                                         E0.ctypes.data_as(dp), g.ctypes.data_as(dp)))
+    return float(E0[0]), float(g[0])

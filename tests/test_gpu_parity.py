@@ -863,6 +863,71 @@ def test_chimera_transpose_isomorphism_on_device(M, N, seed):
         assert E == _chimera_oracle().dp_chimera(M, N, 4, I.K, I.Jv, I.Jh)[0]
 
 
+@pytest.mark.parametrize("M,N", [(1, 1), (1, 3), (2, 1), (2, 2), (3, 2), (3, 3), (4, 2), (4, 4), (5, 2)])
+def test_chimera_count_vs_oracle(M, N):
+    """CountingTropical on the chimera graph (Eq. (4); entropies of PAPER.md:128): E0 and the
+    degeneracy bit-exact against the group tensor-network oracle (int64 counts)."""
+    from ttn_inputs import make_chimera_instance
+    co = _chimera_oracle()
+    rng = np.random.default_rng(70 * M + N)
+    for seed in (6000, 6001):
+        I = make_chimera_instance(M, N, seed)
+        Eo, go = co.dp_chimera(M, N, 4, I.K, I.Jv, I.Jh)
+        E, g = ttn.chimera_sweep_count(I.K, I.Jv, I.Jh)
+        assert (E, g) == (Eo, float(go)) and go < 2 ** 53
+        assert ttn.chimera_sweep_energy_i16(I.K, I.Jv, I.Jh) == E
+    K = rng.integers(-2, 3, size=(M, N, 4, 4)).astype(np.float32)          # zeros included: more ties
+    Jv = rng.integers(-2, 3, size=(M - 1, N, 4)).astype(np.float32)
+    Jh = rng.integers(-2, 3, size=(M, N - 1, 4)).astype(np.float32)
+    Eo, go = co.dp_chimera(M, N, 4, K, Jv, Jh)
+    assert ttn.chimera_sweep_count(K, Jv, Jh) == (Eo, float(go))
+
+
+@pytest.mark.parametrize("M,N", [(2, 2), (4, 3), (5, 5), (6, 4)])
+def test_chimera_count_closed_forms_and_transpose(M, N):
+    co = _chimera_oracle()
+    ne = co.n_edges(M, N, 4)
+    one = lambda *s: np.ones(s, dtype=np.float32)
+    assert ttn.chimera_sweep_count(one(M, N, 4, 4), one(M - 1, N, 4), one(M, N - 1, 4)) == (-ne, 2.0)     # ferromagnet
+    assert ttn.chimera_sweep_count(-one(M, N, 4, 4), -one(M - 1, N, 4), -one(M, N - 1, 4)) == (-ne, 2.0)  # bipartite
+    if 8 * M * N <= 1000:
+        E, g = ttn.chimera_sweep_count(0 * one(M, N, 4, 4), 0 * one(M - 1, N, 4), 0 * one(M, N - 1, 4))
+        assert E == 0.0 and g == 2.0 ** (8 * M * N)                                                       # free spins
+    from ttn_inputs import make_chimera_instance
+    I = make_chimera_instance(M, N, 6500)
+    E, g = ttn.chimera_sweep_count(I.K, I.Jv, I.Jh)
+    Kt = np.ascontiguousarray(np.transpose(I.K, (1, 0, 3, 2)))
+    Jvt = np.ascontiguousarray(np.transpose(I.Jh, (1, 0, 2)))
+    Jht = np.ascontiguousarray(np.transpose(I.Jv, (1, 0, 2)))
+    Et, gt = ttn.chimera_sweep_count(Kt, Jvt, Jht)
+    assert Et == E and g >= 2 and (gt == g if g < 2 ** 53 else abs(gt - g) <= 1e-12 * g)
+    if g < 2 ** 53:
+        assert int(g) % 2 == 0                                                                            # global flip
+
+
+def test_chimera_count_8x8_cells():
+    """512 spins (PAPER.md:126 size): E0 equals the Tropical<i16> path, the degeneracy is invariant under the
+    row / column transpose isomorphism (entirely different code paths for the two directions)."""
+    import torch
+    from ttn_inputs import make_chimera_instance
+    M = N = 8
+    need = ttn.chimera_count_workspace_bytes(M, N)
+    free, _ = torch.cuda.mem_get_info()
+    if free < need + (2 << 30):
+        pytest.skip("needs %.0f GB of free device memory" % (need / 1e9))
+    ws = ttn.alloc_workspace(need)
+    I = make_chimera_instance(M, N, 7008)
+    E, g = ttn.chimera_sweep_count(I.K, I.Jv, I.Jh, workspace=ws)
+    assert E == ttn.chimera_sweep_energy_i16(I.K, I.Jv, I.Jh) and g >= 2 and np.isfinite(g)
+    Kt = np.ascontiguousarray(np.transpose(I.K, (1, 0, 3, 2)))
+    Jvt = np.ascontiguousarray(np.transpose(I.Jh, (1, 0, 2)))
+    Jht = np.ascontiguousarray(np.transpose(I.Jv, (1, 0, 2)))
+    Et, gt = ttn.chimera_sweep_count(Kt, Jvt, Jht, workspace=ws)
+    assert Et == E and abs(gt - g) <= 1e-12 * g
+    del ws
+    torch.cuda.empty_cache()
+
+
 def test_chimera_argument_errors():
     K = np.ones((2, 2, 4, 4), dtype=np.float32); Jv = np.ones((1, 2, 4), dtype=np.float32); Jh = np.ones((2, 1, 4), dtype=np.float32)
     with pytest.raises(ttn.TTNError) as e:
