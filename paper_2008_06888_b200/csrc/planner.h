@@ -51,8 +51,22 @@ struct Pass {
     int n_gates;
 };
 
+// COLOUR-ROTATION (Z3) REDUCTION of the Potts sweep (q = 3; there are no fields, App. C).
+// E = -sum J delta(t_i, t_j) is invariant under t -> t + 1 (mod 3) on every site, every 3 x 3 gate and
+// every diagonal commutes with that rotation rho, and the initial state is rho-invariant: every
+// intermediate state obeys W[t] = W[rho t].  Only the third with column 0 in colour 0 is stored: a state
+// over the L - 1 digits of columns 1 .. L-1 (digit d = column d + 1).  Gates on columns >= 1 stay inside
+// it (column 1's left neighbour is the constant colour 0).  The gate on column 0 acts on the triple
+// W[k, rest] = H[rho^-k rest], k = 0, 1, 2: three stored elements whose EVERY digit differs by the same
+// shift -- they live in the three tiles of a rotation orbit, which one CTA holds together.  That
+// "virtual column" gate (Op.c = Op.pos = VCOL) touches no tile digit and is legal in any pass; by the
+// three-point stencil it depends on column 1 (digit 0).  Plan::vcol: L counts the stored DIGITS, the
+// lattice has L + 1 rows.
+constexpr int VCOL = 255;
+
 struct Plan {
     int q = 2, L = 0;
+    bool vcol = false;          // Z3-reduced Potts plan (see above)
     bool row_aligned = false;   // ttn_ground_config: every row boundary is materialised
     std::vector<Pass> passes;
     std::vector<Op> ops;
@@ -64,14 +78,14 @@ struct TileSpec { int lo, a, b; };
 // gates are scheduled; g(r,c) is legal once g(r-1,c-1), g(r-1,c), g(r-1,c+1) are done.
 class Scheduler {
   public:
-    explicit Scheduler(int L) : L_(L), grow_(L, 1) {}
+    explicit Scheduler(int L, bool vcol = false) : L_(L), rows_(vcol ? L + 1 : L), vcol_(vcol), grow_(L, 1) {}
     bool done() const {
-        for (int c = 0; c < L_; ++c) if (grow_[c] != L_) return false;
-        return true;
+        for (int c = 0; c < L_; ++c) if (grow_[c] != rows_) return false;
+        return !vcol_ || vgrow_ == rows_;
     }
     bool row_done(int r) const {   // all of row r's gates applied
         for (int c = 0; c < L_; ++c) if (grow_[c] < r + 1) return false;
-        return true;
+        return !vcol_ || vgrow_ >= r + 1;
     }
     // Greedily apply everything legal for tile digits [0,lo) U [a,b) with rows <= max_row.
     // Appends to ops; returns number of gates applied.
@@ -84,24 +98,31 @@ class Scheduler {
             for (int c = 0; c < L_; ++c) {
                 if (!in_tile(c)) continue;
                 const int r = grow_[c];
-                if (r >= L_ || r > max_row) continue;
+                if (r >= rows_ || r > max_row) continue;
                 if (c > 0 && grow_[c - 1] < r) continue;
+                if (c == 0 && vcol_ && vgrow_ < r) continue;     // digit 0 = column 1: its left neighbour is column 0
                 if (c + 1 < L_ && grow_[c + 1] < r) continue;
                 legal.push_back(c);
             }
-            if (legal.empty()) break;
+            // the virtual column 0: in every tile; its only neighbour is digit 0 (column 1)
+            const bool vlegal = vcol_ && vgrow_ < rows_ && vgrow_ <= max_row && grow_[0] >= vgrow_;
+            if (legal.empty() && !vlegal) break;
             bool first = true;
             for (int c : legal) {
                 ops.push_back({OP_GATE, (uint8_t)pos_of(c), (uint8_t)c, (uint8_t)(first ? 1 : 0), (uint16_t)grow_[c], 1});
                 first = false;
                 ++gates;
             }
+            if (vlegal) { ops.push_back({OP_GATE, (uint8_t)VCOL, (uint8_t)VCOL, (uint8_t)(first ? 1 : 0), (uint16_t)vgrow_, 1}); ++gates; }
             for (int c : legal) grow_[c] += 1;
+            if (vlegal) vgrow_ += 1;
         }
         return gates;
     }
   private:
-    int L_;
+    int L_, rows_;
+    bool vcol_;
+    int vgrow_ = 1;                    // rows complete on the virtual column
     std::vector<int> grow_;            // grow[c] = rows complete on digit c (row 0 needs no gate)
 };
 
@@ -125,7 +146,7 @@ inline std::vector<TileSpec> tile_cycle(int L, int Tmax, int ride, int stride) {
 }
 
 // Build the plan.  Tmax = log_q of the tile capacity; ride = riding low digits of high tiles.
-inline Plan make_plan(int q, int L, bool has_field, bool row_aligned, int Tmax, int ride) {
+inline Plan make_plan(int q, int L, bool has_field, bool row_aligned, int Tmax, int ride, bool vcol = false) {
     Plan best;
     int wh = Tmax - ride;
     int s_lo = 1, s_hi = wh;
@@ -134,14 +155,14 @@ inline Plan make_plan(int q, int L, bool has_field, bool row_aligned, int Tmax, 
     bool have = false;
     for (int stride = s_lo; stride <= s_hi; ++stride) {
         std::vector<TileSpec> cyc = tile_cycle(L, Tmax, ride, stride);
-        Plan p; p.q = q; p.L = L; p.row_aligned = row_aligned;
-        Scheduler s(L);
+        Plan p; p.q = q; p.L = L; p.row_aligned = row_aligned; p.vcol = vcol;
+        Scheduler s(L, vcol);
         size_t k = 0; int row = 0; bool first = true; int idle = 0;
         int cur_src = -1;
         while (first || !s.done()) {   // the INIT pass exists even when there is nothing to apply
             const TileSpec& t = cyc[k % cyc.size()]; ++k;
             Pass ps{t.lo, t.a, t.b, (int)p.ops.size(), 0, 0, -1, -1, 0};
-            ps.n_gates = s.run_pass(t, row_aligned ? row : L, p.ops);
+            ps.n_gates = s.run_pass(t, row_aligned ? row : L + 1, p.ops);
             ps.op_end = (int)p.ops.size();
             if (ps.op_end == ps.op_begin && !first) { if (++idle > (int)cyc.size()) break; continue; }
             idle = 0;
@@ -167,8 +188,9 @@ inline Plan make_plan(int q, int L, bool has_field, bool row_aligned, int Tmax, 
 // contiguous one (profiles/r01j.md).  States are the per-column progress vectors; a layer holds
 // the `width` states with the most gates applied.  Used for the q = 3 plans, where a pass costs
 // 15-20 ms of memory time before its first gate.
-inline Plan make_plan_beam(int q, int L, int Tmax, int ride, int width = 256) {
+inline Plan make_plan_beam(int q, int L, int Tmax, int ride, int width = 256, bool vcol = false) {
     const int wh = Tmax - ride;
+    const int rows = vcol ? L + 1 : L;          // progress vectors carry the virtual column at index L
     std::vector<TileSpec> tiles;
     tiles.push_back({Tmax, Tmax, Tmax});
     for (int a = ride + 1; a + wh <= L; ++a) tiles.push_back({ride, a, a + wh});
@@ -182,19 +204,23 @@ inline Plan make_plan_beam(int q, int L, int Tmax, int ride, int width = 256) {
             for (int c = 0; c < L; ++c) {
                 if (!in_tile(c)) continue;
                 const int r = g1[c];
-                if (r >= L) continue;
+                if (r >= rows) continue;
                 if (c > 0 && g1[c - 1] < r) continue;
+                if (c == 0 && vcol && g1[L] < r) continue;
                 if (c + 1 < L && g1[c + 1] < r) continue;
                 legal[nl++] = c;
             }
-            if (!nl) break;
+            const bool vlegal = vcol && g1[L] < rows && g1[0] >= g1[L];
+            if (!nl && !vlegal) break;
             for (int i = 0; i < nl; ++i) g1[legal[i]] += 1;
-            gates += nl;
+            if (vlegal) g1[L] += 1;
+            gates += nl + (vlegal ? 1 : 0);
         }
         return gates;
     };
+    const int all_gates = vcol ? (L + 1) * L : L * (L - 1);
     std::vector<Node> layer(1);
-    layer[0].grow.assign(L, 1); layer[0].total = 0; layer[0].lows = 0;
+    layer[0].grow.assign(vcol ? L + 1 : L, 1); layer[0].total = 0; layer[0].lows = 0;
     std::vector<int> best_seq;
     for (int depth = 0; depth < 4 * L && best_seq.empty(); ++depth) {
         std::vector<Node> next;
@@ -218,17 +244,17 @@ inline Plan make_plan_beam(int q, int L, int Tmax, int ride, int width = 256) {
             bool dup = false;
             for (const Node& k : layer) if (k.grow == nn.grow) { dup = true; break; }
             if (dup) continue;
-            if (nn.total == L * (L - 1)) { if (best_seq.empty()) best_seq = nn.seq; continue; }
+            if (nn.total == all_gates) { if (best_seq.empty()) best_seq = nn.seq; continue; }
             if ((int)layer.size() < width) layer.push_back(std::move(nn));
         }
     }
-    Plan p; p.q = q; p.L = L; p.row_aligned = false;
+    Plan p; p.q = q; p.L = L; p.row_aligned = false; p.vcol = vcol;
     if (best_seq.empty()) return p;
-    Scheduler s(L);
+    Scheduler s(L, vcol);
     for (size_t i = 0; i < best_seq.size(); ++i) {
         const TileSpec& t = tiles[best_seq[i]];
         Pass ps{t.lo, t.a, t.b, (int)p.ops.size(), 0, 0, -1, -1, 0};
-        ps.n_gates = s.run_pass(t, L, p.ops);
+        ps.n_gates = s.run_pass(t, L + 1, p.ops);
         ps.op_end = (int)p.ops.size();
         if (i == 0) ps.flags |= PASS_INIT;
         p.passes.push_back(ps);
@@ -266,8 +292,8 @@ inline void mark_gate_blocks(Plan& p, int max_nb = 3) {
 inline std::string describe(const Plan& p) {
     std::string out;
     char line[160];
-    snprintf(line, sizeof line, "plan q=%d L=%d row_aligned=%d passes=%zu ops=%zu\n", p.q, p.L,
-             (int)p.row_aligned, p.passes.size(), p.ops.size());
+    snprintf(line, sizeof line, "plan q=%d L=%d row_aligned=%d passes=%zu ops=%zu vcol=%d\n", p.q, p.L,
+             (int)p.row_aligned, p.passes.size(), p.ops.size(), (int)p.vcol);
     out += line;
     for (size_t i = 0; i < p.passes.size(); ++i) {
         const Pass& ps = p.passes[i];

@@ -82,10 +82,12 @@ DebugCfg read_debug() {
 
 // Tile capacity (log_q of elements per CTA tile) and riding digits of the generic path.
 struct TileCfg { int Tmax, ride; };
-TileCfg tile_cfg(int q, bool count, const DebugCfg& dbg) {
+// z3: the Potts CTA holds the three member tiles of a rotation orbit: one digit less per member
+TileCfg tile_cfg(int q, bool count, const DebugCfg& dbg, bool z3 = false) {
     TileCfg t;
     if (q == 2) t = count ? TileCfg{13, 3} : TileCfg{14, 3};   // 96 KiB / 64 KiB of smem
     else t = count ? TileCfg{8, 2} : TileCfg{9, 2};           // 3^8*12 = 77 KiB / 3^9*4 = 77 KiB
+    if (q == 3 && z3) t.Tmax -= 1;
     // Debug/test override (smaller tiles only): lets tiny lattices exercise multi-pass schedules.
     if (dbg.tmax >= 2 && dbg.tmax <= t.Tmax) t.Tmax = dbg.tmax;
     if (dbg.ride >= 0 && dbg.ride < t.Tmax) t.ride = dbg.ride;
@@ -146,6 +148,13 @@ bool fused_eligible(int q, int L, bool count, bool config, const DebugCfg& dbg) 
     if (dbg.fused == 0 || q != 2) return false;
     return count ? L >= ttn::CW_LOW : L >= ttn::F_WLOW;      // config: row-aligned f32 plan
 }
+// Colour-rotation (Z3) reduction of the Potts sweeps (planner.h): always valid (no fields); used when the
+// reduced state of L - 1 digits spans more than one member tile, so that every rotation orbit has three tiles.
+bool z3_eligible(int q, int L, bool count, const DebugCfg& dbg) {
+    if (q != 3 || dbg.z2 == 0 || L < 3) return false;
+    return L - 1 > tile_cfg(3, count, dbg, true).Tmax;
+}
+
 // Global-flip (Z2) reduction (planner.h): h = 0 only; the half-state must span at least two LOW tiles
 // (a tile and its complement).  Geometry of the call, or nullptr.
 const ttn::FusedGeom* z2_geom(int q, int L, ttn_call call, bool has_field, const DebugCfg& dbg) {
@@ -162,9 +171,9 @@ const ttn::FusedGeom* z2_geom(int q, int L, ttn_call call, bool has_field, const
 Layout make_layout(int q, int L, bool count, bool config, int batch, const DebugCfg& dbg, bool i16 = false, bool z2 = false) {
     Layout y;
     y.NS = ipow(q, z2 ? L - 1 : L);
-    const TileCfg tc = tile_cfg(q, count, dbg);
+    const TileCfg tc = tile_cfg(q, count, dbg, q == 3 && z2);
     // every pass of a plan stages tiles of q^min(L, Tmax) elements
-    y.max_tiles = y.NS / ipow(q, tc.Tmax < L ? tc.Tmax : L);
+    y.max_tiles = y.NS / ipow(q, tc.Tmax < L ? tc.Tmax : L);     // (Z3: three tiles per partial: an upper bound)
     if (fused_eligible(q, L, count, config, dbg) && y.max_tiles < 1024) y.max_tiles = 1024;   // one partial per CTA
     if (y.max_tiles == 0) y.max_tiles = 1;
     size_t off = 0;
@@ -233,6 +242,24 @@ struct ttn_plan {
 
 static ttn::Plan plan_for(int q, int L, ttn_call call, bool has_field, const DebugCfg& dbg) {
     const bool count = (call == TTN_CALL_COUNT);
+    if (z3_eligible(q, L, count, dbg)) {              // Potts on the colour-rotation-reduced state: L - 1 digits + column 0
+        const TileCfg tc = tile_cfg(q, count, dbg, true);
+        const int Ld = L - 1;
+        ttn::Plan p = ttn::make_plan(q, Ld, false, false, tc.Tmax, tc.ride, /*vcol=*/true);
+        if (!dbg.nobeam) {
+            static std::map<std::tuple<int, int, int>, ttn::Plan> zcache;      // memo, as below
+            static std::mutex zmu;
+            std::lock_guard<std::mutex> lock(zmu);
+            const auto key = std::make_tuple(Ld, tc.Tmax, tc.ride);
+            auto it = zcache.find(key);
+            if (it == zcache.end()) it = zcache.emplace(key, ttn::make_plan_beam(q, Ld, tc.Tmax, tc.ride, 256, true)).first;
+            if (!it->second.passes.empty() && it->second.passes.size() < p.passes.size()) p = it->second;
+        }
+        int max_nb = count ? ttn::POTTS_MAX_NB_COUNT : 3;
+        if (dbg.nb >= 1 && dbg.nb <= max_nb) max_nb = dbg.nb;
+        ttn::mark_gate_blocks(p, max_nb);
+        return p;
+    }
     const TileCfg tc = tile_cfg(q, count, dbg);
     ttn::Plan p = ttn::make_plan(q, L, has_field, call == TTN_CALL_CONFIG, tc.Tmax, tc.ride);
     if (q == 3 && L > tc.Tmax && !dbg.nobeam) {       // multi-pass Potts sweep: search the tile order
@@ -258,7 +285,9 @@ template <int Q, bool COUNT>
 static ttn_status launch_pass(const ttn_plan* P, const ttn::Pass& ps, cudaStream_t st) {
     const Layout& y = P->lay;
     ttn::PassParams pp{};
-    pp.L = P->L; pp.lo = ps.lo; pp.a = ps.a; pp.b = ps.b; pp.T = ps.lo + (ps.b - ps.a);
+    const bool z3 = Q == 3 && P->z2;           // (the plan's "reduced by the symmetry" flag)
+    pp.z3 = z3 ? 1 : 0;
+    pp.L = z3 ? P->L - 1 : P->L; pp.lo = ps.lo; pp.a = ps.a; pp.b = ps.b; pp.T = ps.lo + (ps.b - ps.a);
     pp.P_lo = ipow(Q, ps.lo); pp.P_a = ipow(Q, ps.a); pp.P_mid = ipow(Q, ps.a - ps.lo); pp.P_b = ipow(Q, ps.b);
     pp.n_tile = (unsigned)ipow(Q, pp.T);
     pp.tiles_per_inst = y.NS / pp.n_tile;
@@ -281,7 +310,9 @@ static ttn_status launch_pass(const ttn_plan* P, const ttn::Pass& ps, cudaStream
     pp.part_x = reinterpret_cast<float*>(P->ws + y.part_x);
     pp.part_n = reinterpret_cast<double*>(P->ws + y.part_n);
     const size_t smem = (size_t)pp.n_tile * (COUNT ? 12 : 4);
-    const unsigned long long grid = pp.tiles_per_inst * (unsigned long long)P->batch;
+    // Z3: a work unit is a rotation orbit of three tiles
+    const unsigned long long units_per_inst = z3 ? pp.tiles_per_inst / 3 : pp.tiles_per_inst;
+    const unsigned long long grid = units_per_inst * (unsigned long long)P->batch;
     if (grid > 0x7fffffffull) return fail(TTN_EUNSUPPORTED, "grid too large");
     if constexpr (Q == 3) {    // Potts: register-blocked gates (ttn_potts.cuh)
         // persistent CTAs, two residents per SM (ttn_potts.cuh)
@@ -289,9 +320,9 @@ static ttn_status launch_pass(const ttn_plan* P, const ttn::Pass& ps, cudaStream
         if (pp.T > 9) return fail(TTN_EUNSUPPORTED, "Potts tiles hold at most 3^9 elements");
         const int sms = P->sms;                         // of the device the plan was created on
         const unsigned ctas = grid < 2ull * sms ? (unsigned)grid : 2u * (unsigned)sms;
-        const size_t psmem = ttn::potts_buf_bytes(pp.n_tile, COUNT);
+        const size_t psmem = z3 ? ttn::potts_z3_bytes(pp.n_tile, COUNT) : ttn::potts_buf_bytes(pp.n_tile, COUNT);
         ttn_status s = TTN_OK;
-        if (pp.n_tile / 27 <= 128) {                                   // tiny lattices
+        if (pp.n_tile * (z3 ? 3u : 1u) / 27 <= 128) {                  // tiny lattices
             s = set_smem(ttn::potts_pass_kernel<COUNT, 128>, psmem);
             if (s != TTN_OK) return s;
             ttn::potts_pass_kernel<COUNT, 128><<<ctas, 128, psmem, st>>>(pp, (unsigned)grid);
@@ -310,7 +341,7 @@ static ttn_status launch_pass(const ttn_plan* P, const ttn::Pass& ps, cudaStream
     TTN_CUDA(cudaGetLastError());
     if (ps.flags & ttn::PASS_REDUCE) {
         ttn::final_reduce_kernel<COUNT><<<P->batch, 256, 0, st>>>(
-            pp.part_x, pp.part_n, pp.tiles_per_inst, reinterpret_cast<float*>(P->ws + y.out_x),
+            pp.part_x, pp.part_n, units_per_inst, reinterpret_cast<float*>(P->ws + y.out_x),
             reinterpret_cast<double*>(P->ws + y.out_n));
         TTN_CUDA(cudaGetLastError());
     }
@@ -648,8 +679,10 @@ size_t ttn_workspace_bytes(int q, int L, ttn_semiring mode, int batch, int want_
     if (mode == TTN_TROPICAL_I16 && (q != 2 || want_config)) return 0;
     if (!limits_ok(q, L, count, want_config != 0)) return 0;
     const DebugCfg dbg = read_debug();
-    // (with h = 0 the calls may store the flip-reduced half-state: every field is then smaller)
-    return make_layout(q, L, count, want_config != 0, batch, dbg, mode == TTN_TROPICAL_I16 && i16_eligible(q, L, dbg)).total;
+    // (with h = 0 the calls may store the flip-reduced half-state: every field is then smaller; the Potts
+    // calls always run on the colour-rotation-reduced third where it applies)
+    return make_layout(q, L, count, want_config != 0, batch, dbg, mode == TTN_TROPICAL_I16 && i16_eligible(q, L, dbg),
+                       z3_eligible(q, L, count, dbg)).total;
 }
 
 size_t ttn_workspace_bytes_h0(int q, int L, ttn_semiring mode, int batch, int want_config) {
@@ -744,8 +777,9 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     if (h) for (size_t i = 0; i < nf && !field; ++i) field = (h[i] != 0.0f);
     if (want_z2 && field) return fail(TTN_EINVAL, "the flip reduction needs h = 0");
     const ttn::FusedGeom* zg = z2_geom(q, L, call, field, dbg);
+    const bool z3 = z3_eligible(q, L, count, dbg);
     if (want_z2) call = count ? TTN_CALL_COUNT : (config ? TTN_CALL_CONFIG : (want_i16 ? TTN_CALL_ENERGY_I16 : TTN_CALL_ENERGY));  // lattices too small for it run the plain sweep
-    Layout lay = make_layout(q, L, count, config, batch, dbg, i16, zg != nullptr);
+    Layout lay = make_layout(q, L, count, config, batch, dbg, i16, zg != nullptr || z3);
     if (workspace_bytes < lay.total)
         return fail(TTN_ENOMEM, "workspace too small: %zu < %zu", workspace_bytes, lay.total);
     if ((uintptr_t)workspace % 256) return fail(TTN_EINVAL, "workspace must be 256-byte aligned");
@@ -760,7 +794,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     P->q = q; P->L = L; P->batch = batch; P->call = call; P->count = count; P->config = config;
     P->has_field = (h != nullptr) && zg == nullptr;
     P->i16 = i16;
-    P->z2 = zg != nullptr;
+    P->z2 = zg != nullptr || z3;
     P->dbg = dbg;
     P->lay = lay;
     {
@@ -784,6 +818,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     if (!P->fused) P->plan = plan_for(q, L, call, P->has_field, dbg);
     if (!P->fused && P->plan.passes.empty()) { delete P; return fail(TTN_EUNSUPPORTED, "planner produced no schedule"); }
     if (P->plan.ops.size() > (size_t)(L * L + 8)) { delete P; return fail(TTN_EUNSUPPORTED, "op list too long"); }
+    if (!P->fused && z3 != P->plan.vcol) { delete P; return fail(TTN_EUNSUPPORTED, "planner / layout disagree on the Z3 reduction"); }
 
     // the +J constants factored out of the Ising gates (kernel comment at OP_GATE), in f64
     P->defer.assign(batch, 0.0);
@@ -845,6 +880,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     } else {
         ttn::GenericPrepParams gp{};
         gp.q = q; gp.L = L; gp.n_ops = (int)P->plan.ops.size();
+        gp.col_off = P->plan.vcol ? 1 : 0;
         gp.ops = reinterpret_cast<const ttn::Op*>(P->ws + lay.ops);
         gp.Jh = reinterpret_cast<const float*>(P->ws + lay.Jh);
         gp.Jv = reinterpret_cast<const float*>(P->ws + lay.Jv);
@@ -933,8 +969,8 @@ ttn_status ttn_plan_read(ttn_plan* P, void* stream, double* E0, double* degenera
     if (P->config)
         TTN_CUDA(cudaMemcpyAsync(sigma, P->ws + P->lay.sigma, (size_t)P->batch * P->L * P->L, cudaMemcpyDeviceToHost, st));
     TTN_CUDA(cudaStreamSynchronize(st));
-    if (P->count && P->z2)                           // the stored half holds one of every flip pair (exact: x 2)
-        for (int b = 0; b < P->batch; ++b) degeneracy[b] *= 2.0;
+    if (P->count && P->z2)                           // the stored half (third) holds one of every flip pair (rotation triple)
+        for (int b = 0; b < P->batch; ++b) degeneracy[b] *= (P->q == 3 ? 3.0 : 2.0);
     for (int b = 0; b < P->batch; ++b) {
         double m = (double)x[b] + P->defer[b];      // max of -E
         E0[b] = (m == 0.0) ? 0.0 : -m;              // -0.0 -> +0.0

@@ -44,6 +44,9 @@ struct PassParams {
     const float* fin;                             // [inst][2 * GMAX_L]: H_c, K_c of A_{L-1} (REDUCE pass)
     int flags;
     float* part_x; double* part_n;                // [inst][tile] partial reductions
+    int z3;                                       // q = 3, colour-rotation reduction (planner.h): L, T and every power
+                                                  // above count the STORED digits (digit d = column d + 1); a CTA holds
+                                                  // the three tiles of a rotation orbit; ops with pos = VCOL act on column 0
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -527,6 +530,7 @@ __global__ void __launch_bounds__(BT_THREADS) backtrace_inst_kernel(const Argmax
 
 // ---- S0 of the generic path: conjugated gate constants and the coefficients of A_{L-1} -------------
 struct GenericPrepParams {
+    int col_off;                   // Z3: 1 = Op.c is a stored digit, lattice column = c + 1; Op.c = VCOL is column 0
     int q, L, n_ops;
     const Op* ops;                 // [n_ops] gates in execution order
     const float* Jh; const float* Jv; const float* h;   // device couplings, per instance
@@ -545,7 +549,7 @@ __global__ void __launch_bounds__(256) generic_prep_kernel(const GenericPrepPara
     auto Kacc = [&](int R, int c) { double s = 0; if (c < 0 || c >= L - 1) return s; for (int r = 0; r < R; ++r) s += (double)Jh[r * (L - 1) + c]; return s; };
     if (idx < p.n_ops) {
         const Op op = p.ops[idx];
-        const int r = op.row, c = op.c;
+        const int r = op.row, c = op.c == VCOL ? 0 : op.c + p.col_off;          // lattice column
         float* out = p.gate_k + (inst * p.n_ops + idx) * 8;
         const double J = (double)Jv[(r - 1) * L + c], Kl = Kacc(r, c - 1), Kr = Kacc(r, c);
         if (p.q == 2) {
@@ -563,8 +567,9 @@ __global__ void __launch_bounds__(256) generic_prep_kernel(const GenericPrepPara
     }
     if (idx < 2 * GMAX_L) {
         float* out = p.fin + inst * (2 * GMAX_L);
-        const int c = (int)(idx % GMAX_L);
-        if (idx < GMAX_L) out[idx] = c < L ? (float)Hacc(L, c) : 0.f;
+        const int c = (int)(idx % GMAX_L) + p.col_off;                          // tables are per stored digit
+        if (idx < GMAX_L) out[idx] = p.col_off ? (idx == 0 ? (float)Kacc(L, 0) : 0.f)   // Z3: slot 0 = the bond column 0 - column 1
+                                               : (c < L ? (float)Hacc(L, c) : 0.f);
         else out[idx] = c < L - 1 ? (float)Kacc(L, c) : 0.f;
     }
 }

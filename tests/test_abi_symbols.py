@@ -33,7 +33,10 @@ def test_workspace_bytes_and_argument_errors_without_gpu():
     n = ttn.workspace_bytes(2, 16, ttn.TROPICAL_F32, 256, True)
     assert n >= 256 * 17 * 2**16 * 4
     n = ttn.workspace_bytes(3, 18, ttn.COUNTING_F32_F64, 1)
-    assert n >= 3**18 * 12
+    assert 3**17 * 12 <= n < 3**17 * 12 + 2**26          # Potts runs on the colour-rotation-reduced third (3^17 elements)
+    # h = 0: the flip-reduced half-state suffices (ttn_workspace_bytes_h0)
+    n = ttn.workspace_bytes(2, 32, ttn.TROPICAL_F32, 1, h_zero=True)
+    assert 8 * 2**30 <= n < 8 * 2**30 + 2**26
     lib = ttn.lib()
     assert lib.ttn_workspace_bytes(5, 8, 0, 1, 0) == 0
     assert lib.ttn_workspace_bytes(2, 0, 0, 1, 0) == 0

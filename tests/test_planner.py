@@ -49,20 +49,31 @@ def parse(txt):
     return head, passes
 
 
-def validate(q, L, passes, fields, row_aligned):
-    """Diagonal frame: only gates are scheduled; g(r,c) needs g(r-1,c-1), g(r-1,c), g(r-1,c+1)."""
+VCOL = 255      # csrc/planner.h: the virtual column 0 of a Z3-reduced Potts plan
+
+
+def validate(q, L, passes, fields, row_aligned, vcol=False):
+    """Diagonal frame: only gates are scheduled; g(r,c) needs g(r-1,c-1), g(r-1,c), g(r-1,c+1).
+    vcol (Z3-reduced Potts plan): the tiles hold the L - 1 stored digits (digit d = column d + 1); the
+    gate on column 0 is an op with c = pos = VCOL and may appear in any pass."""
     g = np.zeros((L, L), dtype=int); g[0, :] = 1          # row 0 needs no gate
     rows_done = 0
+    Ld = L - 1 if vcol else L
     for i, ps in enumerate(passes):
         lo, a, b = ps["lo"], ps["a"], ps["b"]
-        assert 0 <= lo <= a <= b <= L
+        assert 0 <= lo <= a <= b <= Ld
         tile = list(range(lo)) + list(range(a, b))
         assert len(tile) == len(set(tile)) and len(tile) >= 1
         assert (ps["flags"] & 1) == (1 if i == 0 else 0)          # INIT only on the first pass
         for op in ps["ops"]:
             r, c = op["r"], op["c"]
             assert op["type"] == "g"                               # no diagonal op is ever scheduled
-            assert c in tile and tile.index(c) == op["pos"]
+            if vcol and c == VCOL:
+                assert op["pos"] == VCOL
+                c = 0
+            else:
+                assert c in tile and tile.index(c) == op["pos"]
+                c = c + 1 if vcol else c
             assert 1 <= r < L and g[r, c] == 0 and g[r - 1, c] == 1
             if c > 0: assert g[r - 1, c - 1] == 1
             if c < L - 1: assert g[r - 1, c + 1] == 1
@@ -90,8 +101,10 @@ def validate(q, L, passes, fields, row_aligned):
                                       (3, 12, 0), (2, 34, 0), (2, 15, 0), (2, 14, 1)])
 def test_schedule_obeys_dependency_rule(q, L, call):
     head, passes = parse(describe(q, L, call))
-    assert int(head["L"]) == L and int(head["q"]) == q
-    validate(q, L, passes, fields=(q == 2), row_aligned=(call == 2))
+    vcol = int(head.get("vcol", 0)) == 1
+    assert int(head["L"]) == (L - 1 if vcol else L) and int(head["q"]) == q
+    assert vcol == (q == 3 and L >= 10)                   # Potts sweeps beyond one tile run Z3-reduced
+    validate(q, L, passes, fields=(q == 2), row_aligned=(call == 2), vcol=vcol)
 
 
 @pytest.mark.parametrize("L,call,tmax,ride", [(18, 1, None, None), (18, 0, None, None), (12, 0, None, None),
@@ -113,10 +126,11 @@ def test_potts_gate_blocks(L, call, tmax, ride):
                 o, pr = ops[k + j], ops[k + j - 1]
                 assert o["nb"] == 0 and o["first"] == 0
                 assert o["r"] == pr["r"] and o["c"] == pr["c"] + 1 and o["pos"] == pr["pos"] + 1
+                assert o["c"] != VCOL and pr["c"] != VCOL        # the column-0 gate is a block of its own
             sizes.append(nb)
             k += nb
     assert sum(sizes) == L * (L - 1)
-    if L >= 6:
+    if L >= 12:
         assert sizes.count(1) < len(sizes) // 2          # most gates ride in blocks of 2 or 3
 
 
@@ -129,10 +143,11 @@ def test_fusion_cuts_hbm_passes():
     head, fpasses = parse_fused(describe(2, 32, 0, fused=True))
     assert len(fpasses) <= 24
     # q = 3: beam search over tile sequences (planner.h make_plan_beam) vs the cyclic tile order
+    # (Z3-reduced: passes over a third of the state)
     _, passes = parse(describe(3, 18, 1))
-    assert len(passes) <= 12
+    assert len(passes) <= 15
     _, passes = parse(describe(3, 18, 0))
-    assert len(passes) <= 8
+    assert len(passes) <= 11
 
 
 # ------------------------------------------------------------------ fused register-phase schedule
@@ -541,15 +556,98 @@ def replay(q, L, passes, Jh, Jv, h):
     return (0.0 if m == 0 else -m), int(sum(n[x == m]))
 
 
+def replay_z3(L, passes, Jh, Jv):
+    """Z3-reduced Potts replay, restated from the symmetry: E = -sum J delta (App. C PAPER.md:296 in
+    BASELINE.json's reading) is invariant under t -> t + 1 (mod 3) on every site, so every intermediate
+    state W of the sweep obeys W[t] = W[rho t].  Stored: H[rest] = W[0, rest] over the digits of columns
+    1 .. L-1.  A gate on column c >= 1 acts inside H (column 1 sees colour 0 on its left).  The gate on
+    column 0 acts on x_k = W[k, rest] = H[rho^-k rest] (every digit of rest minus k), k = 0, 1, 2."""
+    Ld = L - 1
+    N = 3 ** Ld
+    x = np.zeros(N); n = np.ones(N, dtype=object)
+    idx = np.arange(N)
+    dig = [(idx // 3 ** d) % 3 for d in range(Ld)]          # dig[d] = colour of column d + 1
+    K = np.cumsum(Jh, axis=0)
+
+    def rot_minus(k):                                       # index of rho^-k rest
+        out = np.zeros(N, dtype=np.int64)
+        for d in range(Ld):
+            out += ((dig[d] - k) % 3) * 3 ** d
+        return out
+
+    rm = [idx, rot_minus(1), rot_minus(2)]
+
+    def gate3(olds, J, Rs):
+        news = []
+        for tn in range(3):
+            bx = None
+            for t in range(3):
+                cx, cn = olds[t][0] + J * (t == tn) + Rs[t] - Rs[tn], olds[t][1]
+                if bx is None:
+                    bx, bn = cx.copy(), cn.copy()
+                else:
+                    gt, eq = cx > bx, cx == bx
+                    bn = np.where(gt, cn, np.where(eq, bn + cn, bn))
+                    bx = np.maximum(bx, cx)
+            news.append((bx, bn))
+        return news
+
+    for ps in passes:
+        for op in ps["ops"]:
+            r = op["r"]
+            if op["c"] == VCOL:                             # column 0: R(t) = K_0 delta(t, colour of column 1)
+                J = Jv[r - 1, 0]
+                sel = idx                                   # every rest once, as the k = 0 member
+                olds = [(x[rm[k]].copy(), n[rm[k]].copy()) for k in range(3)]
+                Rs = [K[r - 1, 0] * (dig[0] == t) for t in range(3)]
+                news = gate3(olds, J, Rs)
+                x = news[0][0]; n = news[0][1]              # H'[rest] = W'[0, rest]; the others follow by symmetry
+                for k in (1, 2):                            # ... and must agree with what the symmetry predicts
+                    assert np.array_equal(news[k][0], x[rm[k]])
+                continue
+            d = op["c"]; c = d + 1
+            J = Jv[r - 1, c]
+            st = 3 ** d
+            base = idx[dig[d] == 0]
+            olds = [(x[base + t * st].copy(), n[base + t * st].copy()) for t in range(3)]
+            left = dig[d - 1][base] if d > 0 else np.zeros(base.size, dtype=np.int64)     # column 0 = colour 0
+            Rs = []
+            for t in range(3):
+                R = K[r - 1, c - 1] * (left == t)
+                if c < L - 1:
+                    R = R + K[r - 1, c] * (t == dig[d + 1][base])
+                Rs.append(R)
+            news = gate3(olds, J, Rs)
+            for t in range(3):
+                x[base + t * st] = news[t][0]; n[base + t * st] = news[t][1]
+    A = K[L - 1, 0] * (dig[0] == 0)
+    for d in range(Ld - 1):
+        A = A + K[L - 1, d + 1] * (dig[d] == dig[d + 1])
+    x = x + A
+    m = x.max()
+    return (0.0 if m == 0 else -m), 3 * int(sum(n[x == m]))
+
+
 @pytest.mark.parametrize("q,L,call,tmax,ride", [
     (2, 8, 1, 5, 2), (2, 9, 0, 4, 1), (2, 7, 1, 3, 1), (2, 10, 1, 6, 3), (2, 6, 2, 4, 2),
-    (3, 6, 1, 3, 1), (3, 5, 1, 2, 1), (3, 7, 0, 4, 2), (2, 8, 1, 13, 3),
+    (3, 6, 1, 3, 1), (3, 5, 1, 2, 1), (3, 7, 0, 4, 2), (2, 8, 1, 13, 3), (3, 7, 1, 3, 0), (3, 4, 1, 2, 1),
 ])
 def test_schedule_replay_matches_oracle(q, L, call, tmax, ride):
     head, passes = parse(describe(q, L, call, tmax, ride))
-    validate(q, L, passes, fields=(q == 2), row_aligned=(call == 2))
+    vcol = int(head.get("vcol", 0)) == 1
+    validate(q, L, passes, fields=(q == 2), row_aligned=(call == 2), vcol=vcol)
     if tmax < L:
         assert len(passes) > 1
+    if vcol:
+        assert q == 3
+        for seed in range(3):
+            inst = make_instance(L, 900 + seed, "pmj", q=3)
+            assert replay_z3(L, passes, inst.Jh, inst.Jv) == oracle.dp_potts3(L, inst.Jh, inst.Jv)[:2]
+        rng = np.random.default_rng(L)
+        Jh = rng.integers(-2, 3, size=(L, L - 1)).astype(float)
+        Jv = rng.integers(-2, 3, size=(L - 1, L)).astype(float)
+        assert replay_z3(L, passes, Jh, Jv) == oracle.dp_potts3(L, Jh, Jv)[:2]
+        return
     for seed in range(3):
         if q == 2:
             rng = np.random.default_rng(seed)
