@@ -227,6 +227,9 @@ def other_configs(torch):
             bmin = B * (Lc - 1) * 2 * be * q ** Lc      # cfg 2: = the checkpoints written once and read back once
             rows[name] = {"ms_total": ms, "ms_per_instance": ms / B, "batch": B, "hbm_passes": plan.num_passes,
                           "launches": plan.num_launches,
+                          # q^L, or the part of it the sweep stores: half (h = 0 flip symmetry, cfg 3), a third
+                          # (Potts colour rotation, cfg 5); the roofline bytes stay north_star's full-vector ones
+                          "state_elements_stored": plan.state_elements,
                           "hbm_roofline_frac": bmin / (peak * 1e9) / (ms * 1e-3)}
             plan.close()
             del plan
@@ -288,6 +291,26 @@ def other_configs(torch):
         except (ttn.TTNError, RuntimeError) as e:      # RuntimeError: torch could not allocate the state
             rows[name] = {"unavailable": str(e).splitlines()[0][:200]}
             torch.cuda.empty_cache()
+    # chimera counting (Fig. 3: residual entropies): CountingTropical on the same column front
+    try:
+        Lc = 8
+        I = make_chimera_instance(Lc, Lc, 7000 + Lc)
+        wsc = ttn.alloc_workspace(ttn.chimera_count_workspace_bytes(Lc, Lc))
+        E, g = ttn.chimera_sweep_count(I.K, I.Jv, I.Jh, workspace=wsc)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        E2, g2 = ttn.chimera_sweep_count(I.K, I.Jv, I.Jh, workspace=wsc)
+        b.record()
+        torch.cuda.synchronize()
+        assert (E2, g2) == (E, g)
+        rows["next3_chimera_8x8_cells_512_spins_count"] = {
+            "ms_total": a.elapsed_time(b), "E0": E, "degeneracy": g, "state_bytes": 12 * 2 ** (4 * Lc),
+            "entropy_per_spin": float(np.log(g) / (8 * Lc * Lc))}
+        del wsc
+        torch.cuda.empty_cache()
+    except (ttn.TTNError, RuntimeError) as e:
+        rows["next3_chimera_8x8_cells_512_spins_count"] = {"unavailable": str(e).splitlines()[0][:200]}
+        torch.cuda.empty_cache()
     return rows
 
 
