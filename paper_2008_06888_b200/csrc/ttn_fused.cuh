@@ -51,7 +51,7 @@ constexpr int FFINAL_FLOATS = 4 * 128 + 2 * 64;   // final table (4 variants) + 
 __host__ __device__ constexpr int fwarps(bool low, int elem = 0) { return elem == 1 ? FWARPS_I16 : (low ? FWARPS_LOW : FWARPS_HIGH); }
 __host__ __device__ constexpr size_t fsmem_bytes(bool low, int elem = 0) {
     return (size_t)fwarps(low, elem) * FREGION_F4 * 16 + (size_t)(FMAX_GATES + 1) * 32 + (size_t)FFINAL_FLOATS * 4 +
-           (size_t)FMAX_MOPS * 4 + 64;
+           (size_t)FMAX_MOPS * 4 + 64 + 256;       // + per-warp mbarriers and their phases (bulk prefetch)
 }
 
 struct FusedParams {
@@ -527,15 +527,34 @@ __device__ __forceinline__ void pf_read(float (&v)[128], const float4* region, i
     }
 }
 
-// LOW tiles: the same for a contiguous 16 KiB tile (no barrier: a low tile is whole lines anyway);
-// the region holds the tile linearly, read back in layout B (lanes = the 5 lowest digits).
-__device__ __forceinline__ void pf_issue_low(float4* region, const float* tile, int lane) {
-    const unsigned sbase = (unsigned)__cvta_generic_to_shared(region) + 16u * (unsigned)lane;
-    const unsigned long long g = (unsigned long long)__cvta_generic_to_global(tile + 4 * lane);
-#pragma unroll
-    for (int i = 0; i < 32; ++i)
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(sbase + 512u * i), "l"(g + 512ull * i) : "memory");
-    asm volatile("cp.async.commit_group;" ::: "memory");
+// LOW tiles: a contiguous 16 KiB tile is ONE bulk copy of the TMA unit (cp.async.bulk global -> shared,
+// UBLKCP in SASS) issued by lane 0 and tracked by the warp's own mbarrier: no per-lane address arithmetic,
+// no LSU instructions.  The region holds the tile linearly, read back in layout B (lanes = the 5 lowest
+// digits).  The region was last touched by generic-proxy accesses (an exchange): fence.proxy.async
+// orders them before the async-proxy write.
+__device__ __forceinline__ void mbar_init(unsigned long long* mbar) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"((unsigned)__cvta_generic_to_shared(mbar)) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void pf_issue_low(float4* region, const float* tile, int lane, unsigned long long* mbar) {
+    __syncwarp();
+    if (lane == 0) {
+        const unsigned dst = (unsigned)__cvta_generic_to_shared(region), mb = (unsigned)__cvta_generic_to_shared(mbar);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], 16384;" :: "r"(mb) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], 16384, [%2];"
+                     :: "r"(dst), "l"((unsigned long long)__cvta_generic_to_global(tile)), "r"(mb) : "memory");
+    }
+}
+__device__ __forceinline__ void pf_wait_low(unsigned long long* mbar, unsigned& phase) {
+    const unsigned mb = (unsigned)__cvta_generic_to_shared(mbar);
+    unsigned ok;
+    do {
+        asm volatile("{ .reg .pred p;\n\t"
+                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                     "selp.u32 %0, 1, 0, p; }" : "=r"(ok) : "r"(mb), "r"(phase) : "memory");
+    } while (!ok);
+    phase ^= 1u;
 }
 __device__ __forceinline__ void pf_read_low(float (&v)[128], const float4* region, int lane) {
     const float* q = reinterpret_cast<const float*>(region) + lane;
@@ -558,6 +577,7 @@ __device__ __forceinline__ void fused_pass_body(const FusedParams& p, unsigned c
                                                 const int inst_first, const int inst_step) {
     constexpr bool RED = false;          // GROUP passes never reduce
     constexpr bool Z2 = false;
+    constexpr bool INIT_MBAR = false;    // fused_sweep_kernel initialises the mbarriers once
 #include "ttn_fused_body.inc"
 }
 
@@ -569,6 +589,7 @@ __global__ void __launch_bounds__(fwarps(LOW, ELEM) * 32, 1) fused_pass_kernel(c
     extern __shared__ __align__(16) unsigned char fsm_raw[];
     const int inst_first = p.cta_per_inst ? (int)blockIdx.x * (GROUP ? p.igroup : 1) : 0;
     const int inst_step = p.cta_per_inst ? (int)gridDim.x * (GROUP ? p.igroup : 1) : 1;
+    constexpr bool INIT_MBAR = true;
 #include "ttn_fused_body.inc"
 }
 
@@ -584,6 +605,11 @@ __global__ void __launch_bounds__(fwarps(true) * 32, 1) fused_sweep_kernel(const
     extern __shared__ __align__(16) unsigned char fsm_raw[];
     __shared__ FusedParams s_p;
     const int igroup = passes[0].igroup, batch = passes[0].batch;
+    {   // the warps' mbarriers (bulk prefetch of LOW tiles) and their phases live behind s_red (ttn_fused_body.inc)
+        unsigned long long* mb = reinterpret_cast<unsigned long long*>(fsm_raw + fsmem_bytes(true) - 256);
+        if ((threadIdx.x & 31) == 0) { mbar_init(mb + (threadIdx.x >> 5)); reinterpret_cast<unsigned*>(mb + 16)[threadIdx.x >> 5] = 0u; }
+        __syncthreads();
+    }
     for (int inst = (int)blockIdx.x * igroup; inst < batch; inst += (int)gridDim.x * igroup) {
         for (int k = 0; k < n_passes; ++k) {
             __syncthreads();                                   // the previous pass is complete (and s_p free)
