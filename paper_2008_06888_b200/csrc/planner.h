@@ -350,7 +350,8 @@ inline std::string describe(const Plan& p) {
 // of each of those digits (all legal at the start of the round), in ascending bit order.  Layout
 // exchanges go through the warp's private shared-memory region.
 // =============================================================================================
-enum MicroCode : uint8_t { MC_END = 0, MC_XAB = 1, MC_XBA = 2, MC_ROUND = 3, MC_FINAL = 4 };
+enum MicroCode : uint8_t { MC_END = 0, MC_XAB = 1, MC_XBA = 2, MC_ROUND = 3, MC_FINAL = 4,
+                            MC_CKPT = 5 };   // store the tile as it stands to the pass's checkpoint buffer (merged row plans)
 
 struct MicroOp { uint8_t code; uint8_t mask; uint16_t arg; };   // ROUND: mask = register bits, arg = index of
                                                                 // its first gate in the pass's gate list
@@ -458,6 +459,7 @@ struct FusedPass {
     int gate_begin, gate_end;    // into FusedPlan::gate_rc
     int n_phases, n_rounds;
     int src_buf = -1, dst_buf = -1;   // -1 = the state V; r >= 0 = checkpoint C_r (row-aligned plans)
+    int ckpt_buf = -1;                // merged row plans: the row whose checkpoint the MC_CKPT micro-op of this pass writes
 };
 
 struct FusedPlan {
@@ -484,7 +486,10 @@ class FusedScheduler {
     void set_max_row(int r) { max_row_ = r; }
     // gate-row plans: the gates of the current row on columns >= c are someone else's: count them as done
     void skip_columns_from(int c) { for (int i = c; i < L_; ++i) grow_[i] += 1; }
-    int run_pass(int a, bool low, int max_gates, FusedPass& ps) {
+    // ckpt_row >= 0 (merged row plans): gates up to row ckpt_row, MC_CKPT (row ckpt_row is complete there: the
+    // caller guarantees it), then the tile's gates of row ckpt_row + 1.
+    int run_pass(int a, bool low, int max_gates, FusedPass& ps, int ckpt_row = -1) {
+        if (ckpt_row >= 0) max_row_ = ckpt_row;
         const int W = low ? G_.WLOW : G_.WHIGH;
         ps.a = a; ps.W = W; ps.low = low; ps.flags = 0; ps.n_phases = 0; ps.n_rounds = 0;
         ps.mop_begin = (int)Pp_->mops.size(); ps.gate_begin = (int)Pp_->gate_rc.size();
@@ -494,16 +499,29 @@ class FusedScheduler {
         ps.first_layout = layout;
         int total = 0, idle = 0;
         bool pending_x = false;                        // an exchange is owed before the next non-empty phase
-        while (idle < 2) {
-            size_t mark = Pp_->mops.size();
-            if (pending_x) Pp_->mops.push_back({(uint8_t)(layout == 1 ? MC_XAB : MC_XBA), 0, 0});
-            int rounds = 0;
-            int n = run_phase(a, low, layout, rounds);
-            if (n == 0) { Pp_->mops.resize(mark); ++idle; layout ^= 1; pending_x = !pending_x; continue; }
-            total += n; idle = 0; ++ps.n_phases; ps.n_rounds += rounds;
-            layout ^= 1; pending_x = true;
+        int cur = layout;                              // the layout the registers are in
+        for (int part = 0; part < (ckpt_row >= 0 ? 2 : 1); ++part) {
+            idle = 0;
+            while (idle < 2) {
+                size_t mark = Pp_->mops.size();
+                if (pending_x) Pp_->mops.push_back({(uint8_t)(layout == 1 ? MC_XAB : MC_XBA), 0, 0});
+                int rounds = 0;
+                int n = run_phase(a, low, layout, rounds);
+                if (n == 0) { Pp_->mops.resize(mark); ++idle; layout ^= 1; pending_x = !pending_x; continue; }
+                total += n; idle = 0; ++ps.n_phases; ps.n_rounds += rounds;
+                cur = layout;
+                layout ^= 1; pending_x = true;
+            }
+            if (part == 0 && ckpt_row >= 0) {
+                // back to "no exchange owed" relative to the layout the registers are in; LOW tiles store from B
+                if (low && cur != 1) { Pp_->mops.push_back({MC_XAB, 0, 0}); cur = 1; }
+                Pp_->mops.push_back({MC_CKPT, 0, 0});
+                ps.ckpt_buf = ckpt_row;
+                layout = cur; pending_x = false;
+                max_row_ = ckpt_row + 1;
+            }
         }
-        int last = layout ^ 1;                          // the layout of the last productive phase
+        int last = cur;                                 // the layout of the last productive phase
         if (ps.n_phases == 0) last = ps.first_layout;
         if (low && last != 1) { Pp_->mops.push_back({MC_XAB, 0, 0}); last = 1; }
         ps.last_layout = last;
@@ -712,6 +730,49 @@ inline FusedPlan make_gate_row_plan(int L, int ncols, int max_gates_per_pass, co
     return p;
 }
 
+// Merged row-aligned plan (two tile kinds: the low tile and ONE high tile, i.e. L <= WLOW + WHIGH): the tile
+// order alternates from row to row -- low, high | high, low | low, high ... -- so that the second pass of row
+// r and the first pass of row r + 1 use the same tile and merge into one pass with the checkpoint store of
+// C_r in its middle (MC_CKPT): one load of the tile for two rows of its gates, L passes instead of 2L - 1.
+// Gates of one row commute (planner.h header), so the order inside a row is free.
+inline FusedPlan make_fused_row_plan_merged(int L, int max_gates_per_pass, const FusedGeom& G = GEOM_F32) {
+    FusedPlan p; p.L = L;
+    if (L <= G.WLOW || L > G.WLOW + G.WHIGH) return p;
+    int ah = L - G.WHIGH;
+    if (ah < G.AMIN) ah = G.AMIN;
+    FusedScheduler s(L, p, G);
+    {   // row 0: initialise C_0
+        s.set_max_row(0);
+        FusedPass ps{};
+        s.run_pass(0, true, max_gates_per_pass, ps);
+        ps.flags |= PASS_INIT; ps.src_buf = -1; ps.dst_buf = 0;
+        p.passes.push_back(ps);
+    }
+    {   // first half of row 1 on the low tile
+        s.set_max_row(1);
+        FusedPass ps{};
+        s.run_pass(0, true, max_gates_per_pass, ps);
+        ps.src_buf = 0; ps.dst_buf = -1;
+        p.passes.push_back(ps);
+    }
+    bool low = false;                          // tile of the next (merged) pass
+    for (int r = 1; r < L; ++r, low = !low) {
+        FusedPass ps{};
+        if (r + 1 < L) {
+            s.run_pass(low ? 0 : ah, low, max_gates_per_pass, ps, /*ckpt_row=*/r);
+            ps.src_buf = -1; ps.dst_buf = -1;
+        } else {                               // the last row: its second half completes it
+            s.set_max_row(r);
+            s.run_pass(low ? 0 : ah, low, max_gates_per_pass, ps);
+            ps.src_buf = -1; ps.dst_buf = r;
+        }
+        p.passes.push_back(ps);
+        if (!s.row_done(r)) return p;          // ok stays false
+    }
+    p.ok = s.done();
+    return p;
+}
+
 inline std::string describe_fused(const FusedPlan& p) {
     std::string out; char line[200];
     snprintf(line, sizeof line, "fused L=%d passes=%zu mops=%zu gates=%zu\n", p.L,
@@ -719,9 +780,9 @@ inline std::string describe_fused(const FusedPlan& p) {
     out += line;
     for (size_t i = 0; i < p.passes.size(); ++i) {
         const FusedPass& ps = p.passes[i];
-        snprintf(line, sizeof line, "fpass %zu a=%d W=%d low=%d flags=%d first=%d last=%d phases=%d rounds=%d gates=%d src=%d dst=%d\n", i,
+        snprintf(line, sizeof line, "fpass %zu a=%d W=%d low=%d flags=%d first=%d last=%d phases=%d rounds=%d gates=%d src=%d dst=%d ckpt=%d\n", i,
                  ps.a, ps.W, ps.low, ps.flags, ps.first_layout, ps.last_layout, ps.n_phases, ps.n_rounds,
-                 ps.gate_end - ps.gate_begin, ps.src_buf, ps.dst_buf);
+                 ps.gate_end - ps.gate_begin, ps.src_buf, ps.dst_buf, ps.ckpt_buf);
         out += line;
         for (int k = ps.mop_begin; k < ps.mop_end; ++k) {
             const MicroOp& m = p.mops[k];
@@ -730,6 +791,7 @@ inline std::string describe_fused(const FusedPlan& p) {
                 case MC_XBA: out += "m xBA\n"; break;
                 case MC_END: out += "m end\n"; break;
                 case MC_FINAL: out += "m final\n"; break;
+                case MC_CKPT: out += "m ckpt\n"; break;
                 case MC_ROUND: {
                     snprintf(line, sizeof line, "m round mask=%d first=%d flip=%d\n", m.mask, m.arg & ~MOP_FLIP, (m.arg & MOP_FLIP) ? 1 : 0);
                     out += line;

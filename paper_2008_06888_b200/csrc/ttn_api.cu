@@ -64,6 +64,7 @@ struct DebugCfg {
     int bt_multi = 0;             // backward pass: one launch pair per row even for batches of small lattices
     int timing = 0;               // per-pass device times on stderr
     int ckpt_k = 0;               // TTN_DEBUG_CKPT_K=k: ground_config keeps a checkpoint every k rows + recompute (any L)
+    int nomerge = 0;              // TTN_DEBUG_NOMERGE: ground_config forward with one pass per tile and row (no merged passes)
     int ch_persm = 512, ch_nocell0 = 0;          // chimera: CTAs per SM, generic kernel for the r = 0 cells
 };
 DebugCfg read_debug() {
@@ -75,7 +76,7 @@ DebugCfg read_debug() {
     geti("TTN_DEBUG_CKPT_K", d.ckpt_k);
     flag("TTN_DEBUG_NOBEAM", d.nobeam); flag("TTN_DEBUG_NOLOWPF", d.nolowpf); flag("TTN_DEBUG_NOGROUP", d.nogroup);
     flag("TTN_DEBUG_NOSWEEP", d.nosweep); flag("TTN_DEBUG_BT_MULTI", d.bt_multi); flag("TTN_DEBUG_TIMING", d.timing);
-    flag("TTN_DEBUG_CH_NOCELL0", d.ch_nocell0);
+    flag("TTN_DEBUG_CH_NOCELL0", d.ch_nocell0); flag("TTN_DEBUG_NOMERGE", d.nomerge);
     if (d.ch_persm < 1) d.ch_persm = 512;
     return d;
 }
@@ -368,6 +369,7 @@ static ttn_status launch_fused_pass(const ttn_plan* P, const ttn::FusedPass& ps,
         const int ss = ps.src_buf >= 0 ? P->slot_of_row[ps.src_buf] : -1, ds = ps.dst_buf >= 0 ? P->slot_of_row[ps.dst_buf] : -1;
         if (ss >= 0) { pp.src = CK + (unsigned long long)ss * y.NS; pp.src_stride = cstride; }
         if (ds >= 0) { pp.state = CK + (unsigned long long)ds * y.NS; pp.inst_stride = cstride; }
+        if (ps.ckpt_buf >= 0) { pp.ckpt = CK + (unsigned long long)P->slot_of_row[ps.ckpt_buf] * y.NS; pp.ckpt_stride = cstride; }
     }
     pp.L_cols = P->L;
     if (P->i16) {           // the kernel sees the lattice of 32-bit words: column c >= 1 = word digit c - 1
@@ -703,8 +705,11 @@ long ttn_plan_describe(int q, int L, ttn_call call, char* buf, size_t n) {
     if (call == TTN_CALL_ENERGY_Z2 || call == TTN_CALL_COUNT_Z2 || call == TTN_CALL_ENERGY_I16_Z2 || call == TTN_CALL_CONFIG_Z2) {
         // the schedules the calls run when h = 0
         if (const ttn::FusedGeom* G = z2_geom(q, L, call, false, dbg)) {
-            ttn::FusedPlan fp = call == TTN_CALL_CONFIG_Z2 ? ttn::make_fused_row_plan(L, ttn::FMAX_GATES, *G)
-                                                           : ttn::make_fused_plan(L, ttn::FMAX_GATES, *G);
+            ttn::FusedPlan fp;
+            if (call == TTN_CALL_CONFIG_Z2) {
+                if (ckpt_scheme(L, true, dbg).k == 0 && !dbg.nomerge) fp = ttn::make_fused_row_plan_merged(L, ttn::FMAX_GATES, *G);
+                if (!fp.ok) fp = ttn::make_fused_row_plan(L, ttn::FMAX_GATES, *G);
+            } else fp = ttn::make_fused_plan(L, ttn::FMAX_GATES, *G);
             if (fp.ok) s = ttn::describe_fused(fp);
         }
         if (s.empty()) call = call == TTN_CALL_ENERGY_Z2 ? TTN_CALL_ENERGY : (call == TTN_CALL_COUNT_Z2 ? TTN_CALL_COUNT
@@ -716,9 +721,12 @@ long ttn_plan_describe(int q, int L, ttn_call call, char* buf, size_t n) {
     }
     if (call == TTN_CALL_ENERGY_I16 && s.empty()) call = TTN_CALL_ENERGY;
     if (s.empty() && fused_eligible(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG, dbg)) {
-        ttn::FusedPlan fp = call == TTN_CALL_COUNT ? ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_COUNT)
-                          : call == TTN_CALL_CONFIG ? ttn::make_fused_row_plan(L, ttn::FMAX_GATES)
-                                                    : ttn::make_fused_plan(L, ttn::FMAX_GATES);
+        ttn::FusedPlan fp;
+        if (call == TTN_CALL_CONFIG && ckpt_scheme(L, true, dbg).k == 0 && !dbg.nomerge) fp = ttn::make_fused_row_plan_merged(L, ttn::FMAX_GATES);
+        if (!fp.ok)
+            fp = call == TTN_CALL_COUNT ? ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_COUNT)
+               : call == TTN_CALL_CONFIG ? ttn::make_fused_row_plan(L, ttn::FMAX_GATES)
+                                         : ttn::make_fused_plan(L, ttn::FMAX_GATES);
         if (fp.ok) s = ttn::describe_fused(fp);
     }
     if (s.empty()) s = ttn::describe(plan_for(q, L, call, /*has_field=*/q == 2, dbg));
@@ -807,12 +815,16 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
         P->fused = P->fplan.ok;
         if (!P->fused) { delete P; return fail(TTN_EUNSUPPORTED, "no Tropical<i16> schedule"); }
     } else if (zg) {
-        P->fplan = config ? ttn::make_fused_row_plan(L, ttn::FMAX_GATES, *zg) : ttn::make_fused_plan(L, ttn::FMAX_GATES, *zg);
+        if (config && lay.ck.k == 0 && !dbg.nomerge) P->fplan = ttn::make_fused_row_plan_merged(L, ttn::FMAX_GATES, *zg);
+        if (config && !P->fplan.ok) P->fplan = ttn::make_fused_row_plan(L, ttn::FMAX_GATES, *zg);
+        if (!config) P->fplan = ttn::make_fused_plan(L, ttn::FMAX_GATES, *zg);
         P->fused = P->fplan.ok;
         if (!P->fused) { delete P; return fail(TTN_EUNSUPPORTED, "no flip-reduced schedule"); }
     } else if (fused_eligible(q, L, count, config, dbg)) {
-        P->fplan = count ? ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_COUNT)
-                 : config ? ttn::make_fused_row_plan(L, ttn::FMAX_GATES) : ttn::make_fused_plan(L, ttn::FMAX_GATES);
+        if (config && lay.ck.k == 0 && !dbg.nomerge) P->fplan = ttn::make_fused_row_plan_merged(L, ttn::FMAX_GATES);
+        if (!P->fplan.ok)
+            P->fplan = count ? ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_COUNT)
+                     : config ? ttn::make_fused_row_plan(L, ttn::FMAX_GATES) : ttn::make_fused_plan(L, ttn::FMAX_GATES);
         P->fused = P->fplan.ok;
     }
     if (!P->fused) P->plan = plan_for(q, L, call, P->has_field, dbg);
@@ -852,7 +864,7 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
             int row = 0;
             for (size_t i = 0; i < P->fplan.passes.size(); ++i)
                 if (P->fplan.passes[i].dst_buf >= 0) { P->row_pass[++row] = (int)i + 1; }
-            if (row != L) { delete P; return fail(TTN_EUNSUPPORTED, "row-aligned plan is incomplete"); }
+            if (ck.k > 0 && row != L) { delete P; return fail(TTN_EUNSUPPORTED, "row-aligned plan is incomplete"); }
             P->slot_of_row.assign(L, -1);
             for (int r = 0; r < L; ++r) if (ck.stored(r)) P->slot_of_row[r] = ck.stored_slot(r);
             if (ck.k > 0)          // the backward pass re-sweeps every row that is not kept

@@ -81,6 +81,8 @@ struct FusedParams {
     int L_cols;                         // Tropical<i16> only: lattice L (p.L = L - 1 word digits)
     unsigned stride_bytes;              // HIGH: 4 << a, passed opaque so that the address math stays
                                         // one mad.wide.u32 (32 x 32 -> 64 bit) per access
+    float* ckpt;                        // merged row plans: where MC_CKPT stores the tile (instance 0), else NULL
+    unsigned long long ckpt_stride;
 };
 
 // (o0, o1) = (a0 + b0, a1 + b1) in one FADD2

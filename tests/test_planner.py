@@ -19,10 +19,12 @@ from ttn_inputs import make_instance
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def describe(q, L, call, tmax=None, ride=None, fused=False):
+def describe(q, L, call, tmax=None, ride=None, fused=False, nomerge=False):
     """Run ttn_plan_describe in a subprocess so the debug tile overrides can be set."""
     env = dict(os.environ)
     env["TTN_DEBUG_FUSED"] = "1" if fused else "0"
+    if nomerge:
+        env["TTN_DEBUG_NOMERGE"] = "1"
     if tmax is not None:
         env["TTN_DEBUG_TMAX"] = str(tmax)
     if ride is not None:
@@ -236,6 +238,11 @@ def fused_to_gates(L, fpasses, count=False, i16=False, config=False, z2=False):
         ngates = 0
         for m in ps["mops"][:-1]:
             code = m["code"]
+            if code == "ckpt":
+                assert config and ps["ckpt"] >= 1 and (not low or layout == 1)
+                assert all(g >= ps["ckpt"] + 1 for g in grow)             # the row is complete where it is stored
+                assert all(g <= ps["ckpt"] + 1 for g in grow)             # ... and nothing of the next row is in it
+                continue
             if code == "xAB":
                 assert layout == 0
                 layout = 1
@@ -436,7 +443,7 @@ def test_z2_describe_falls_back_below_two_tiles():
 def test_fused_row_aligned_schedule(L):
     """ttn_ground_config on the fused kernel: every row boundary is a checkpoint; the pass that
     completes row r writes C_r, the next one reads it (src/dst chain)."""
-    head, fpasses = parse_fused(describe(2, L, 2, fused=True))
+    head, fpasses = parse_fused(describe(2, L, 2, fused=True, nomerge=True))
     flat = fused_to_gates(L, fpasses, config=True)
     assert len(flat) == L * (L - 1)
     rows = [r for r, c in flat]
@@ -458,7 +465,7 @@ def test_fused_row_aligned_schedule(L):
 def test_fused_z2_row_aligned_schedule(L):
     """ttn_ground_config with h = 0: the row-aligned plan on the flip-reduced geometry (checkpoints are
     half-states); rows complete in order, one flip gate (column 0) per row, src/dst chain intact."""
-    head, fpasses = parse_fused(describe(2, L, 7, fused=True))
+    head, fpasses = parse_fused(describe(2, L, 7, fused=True, nomerge=True))
     flat = fused_to_gates(L, fpasses, config=True, z2=True)
     assert len(flat) == L * (L - 1) == len(set(flat))
     rows = [r for r, c in flat]
@@ -475,6 +482,25 @@ def test_fused_z2_row_aligned_schedule(L):
         else:
             assert ps["dst"] == -1
     assert done == L - 1
+
+
+@pytest.mark.parametrize("L,call", [(13, 2), (16, 2), (20, 2), (21, 2), (14, 7), (16, 7), (22, 7)])
+def test_fused_merged_row_schedule(L, call):
+    """Merged row-aligned plan (low tile + one high tile): the tile order alternates from row to row and the
+    two passes on the same tile merge around a mid-pass checkpoint store: L passes; every C_r (0 < r < L-1)
+    is written by an MC_CKPT micro-op exactly where row r is complete and row r + 1 untouched (checked
+    inside fused_to_gates), C_0 and C_{L-1} by the first and the last pass."""
+    z2 = call == 7
+    head, fpasses = parse_fused(describe(2, L, call, fused=True))
+    flat = fused_to_gates(L, fpasses, config=True, z2=z2)
+    assert len(flat) == L * (L - 1) == len(set(flat))
+    assert len(fpasses) == L + 1
+    assert fpasses[0]["dst"] == 0 and fpasses[1]["src"] == 0 and fpasses[-1]["dst"] == L - 1
+    assert [ps["ckpt"] for ps in fpasses[2:-1]] == list(range(1, L - 1))
+    assert all(ps["src"] == -1 and ps["dst"] == -1 for ps in fpasses[2:-1])
+    assert [ps["low"] for ps in fpasses[1:]] == [(i + 1) % 2 for i in range(L)]     # low, high, low, ...
+    for ps in fpasses:
+        assert [m["code"] for m in ps["mops"]].count("ckpt") == (1 if ps["ckpt"] >= 0 else 0)
 
 
 @pytest.mark.parametrize("L", [12, 13, 16])
