@@ -443,7 +443,7 @@ __global__ void __launch_bounds__(BT_THREADS) backtrace_inst_kernel(const Argmax
     __shared__ double hsum[BT_MAX_L][BT_MAX_L];   // [r][c] = sum_{rr <= r} h[rr][c]
     __shared__ double ksum[BT_MAX_L][BT_MAX_L];   // [r][c] = sum_{rr <= r} Jh[rr][c]
     __shared__ float jsig[BT_MAX_L], kacc[BT_MAX_L];
-    __shared__ float tab[3][256];
+    __shared__ __align__(16) float tab[3][256];
     __shared__ float rv[BT_THREADS / 32];
     __shared__ unsigned long long rs[BT_THREADS / 32];
     __shared__ unsigned long long s_next;
@@ -500,10 +500,26 @@ __global__ void __launch_bounds__(BT_THREADS) backtrace_inst_kernel(const Argmax
             if (v > bv) { bv = v; b32 = s; }
         };
         if (ns >= 4u * BT_THREADS) {              // 16-byte loads, four in flight per thread
+            // The four states of a float4 differ in bits 0, 1 only: the table entries of the higher bytes and
+            // the boundary bonds are fetched once per float4, tab[0] with one 128-bit load; every element's
+            // sum is formed in the order of visit() (tab[0], then per higher byte its entry and its bond).
 #pragma unroll 4
             for (unsigned s = 4u * threadIdx.x; s < ns; s += 4u * BT_THREADS) {
                 const float4 c4 = *reinterpret_cast<const float4*>(C + s);
-                visit(c4.x, s); visit(c4.y, s + 1); visit(c4.z, s + 2); visit(c4.w, s + 3);
+                const float4 t0 = *reinterpret_cast<const float4*>(&tab[0][s & 255u]);
+                float w0 = t0.x, w1 = t0.y, w2 = t0.z, w3 = t0.w;
+                const unsigned x = s ^ (s >> 1);
+                for (int m = 1; m < nchunk; ++m) {
+                    const float tm = tab[m][(s >> (8 * m)) & 255u];
+                    const float bd = ((x >> (8 * m - 1)) & 1u) ? -kacc[8 * m - 1] : kacc[8 * m - 1];
+                    w0 += tm; w1 += tm; w2 += tm; w3 += tm;
+                    w0 += bd; w1 += bd; w2 += bd; w3 += bd;
+                }
+                const float v0 = c4.x + w0, v1 = c4.y + w1, v2 = c4.z + w2, v3 = c4.w + w3;
+                if (v0 > bv) { bv = v0; b32 = s; }
+                if (v1 > bv) { bv = v1; b32 = s + 1; }
+                if (v2 > bv) { bv = v2; b32 = s + 2; }
+                if (v3 > bv) { bv = v3; b32 = s + 3; }
             }
         } else {
             for (unsigned s = threadIdx.x; s < ns; s += BT_THREADS) visit(C[s], s);
