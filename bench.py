@@ -469,6 +469,7 @@ def main():
             "gpu_launches": plan.num_launches * args.steps,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak,
+                         "frac_vs_nominal_8TBs": achieved / 8000.0,      # north_star's nominal "~8 TB/s"
                          # dram__bytes_read.sum + dram__bytes_write.sum per pass launch, read from the
                          # committed ncu --set full summary of this kernel (None if absent / other L)
                          "traffic": traffic, "traffic_source": traffic_src,

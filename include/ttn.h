@@ -125,9 +125,13 @@ ttn_status ttn_potts3_sweep_count(int L, const float* Jh, const float* Jv, int b
  * energy as Eq. (1) with h = 0.  All three are HOST pointers, row-major float32.  The sweep runs
  * column by column at the level of single spins in Tropical<i16> (the paper's Int16):
  * a state of 2^(4M+4) int16 elements (the 4M horizontal spins of the column front and a 4-spin
- * ancilla for the vertical group), one HBM pass per unit cell.  Exact; couplings must be
- * integer-valued with sum |J| <= 8000, else TTN_EINVAL.  Limits: M <= 8 (137 GB state), N <= 64;
- * beyond them TTN_EUNSUPPORTED.  `workspace` is a DEVICE pointer of at least
+ * ancilla for the vertical group), one HBM pass per unit cell -- for M <= 3; for M >= 4 the state is
+ * the paper's 16^M column front, 2^(4M) int16 elements (M = 8: 8 GiB), swept with three gate-row
+ * passes and one vertical-chain pass per column of cells (csrc/ttn_chimera2.cuh).  Exact; couplings
+ * must be integer-valued with sum |J| <= 8000 (every intermediate then fits 16 bits), else
+ * TTN_EINVAL: for +-J couplings that bounds the number of edges, i.e. N <= 42 at M = 8 (184 edges
+ * per column of 8 cells), whatever the structural limits M <= 8, N <= 64 (beyond those:
+ * TTN_EUNSUPPORTED).  `workspace` is a DEVICE pointer of at least
  * ttn_chimera_workspace_bytes(M, N) bytes (0 = unsupported size); E0 receives the ground-state
  * energy; the call synchronises `stream`. */
 size_t ttn_chimera_workspace_bytes(int M, int N);
