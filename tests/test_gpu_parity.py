@@ -428,6 +428,27 @@ def test_L33_beyond_2_to_32_elements():
     torch.cuda.empty_cache()
 
 
+def test_beyond_2_to_32_elements_full_state_and_half_state(monkeypatch):
+    """Element indices beyond 2^32 on both paths: the FULL-state sweep at L = 33 (2^33 elements, what any
+    field selects; flip reduction switched off) and the flip-reduced sweep at L = 34 (half-state of 2^33
+    elements, warp pairs on tiles t and 2^21 - 1 - t).  Planted instances: E0 = -2L(L-1)."""
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if free < 40 * 2 ** 30:
+        pytest.skip("needs 40 GiB of free device memory")
+    rng = np.random.default_rng(3334)
+    for L, z2 in ((33, "0"), (34, "1")):
+        eps = rng.choice([-1.0, 1.0], size=(L, L)).astype(np.float32)
+        Jh, Jv = (eps[:, :-1] * eps[:, 1:])[None], (eps[:-1, :] * eps[1:, :])[None]
+        monkeypatch.setenv("TTN_DEBUG_Z2", z2)
+        p = ttn.Plan(2, ttn.CALL_ENERGY, Jh, Jv)
+        assert p.state_elements == 2 ** 33
+        p.launch(); E = p.read()[0][0]; p.close()
+        del p
+        torch.cuda.empty_cache()
+        assert E == -2 * L * (L - 1)
+
+
 @pytest.mark.parametrize("L", [24, 28, 30])
 def test_large_energy_vs_golden(L):
     gold = golden()
