@@ -170,13 +170,16 @@ __device__ __forceinline__ PottsTile potts_tile(const PassParams& p, unsigned gt
 }
 
 // Z3: work unit `gunit` = (instance, orbit); base[o] = first element of member o.  Member 0 is the tile whose
-// lowest outside digit is 0 (tile index 3 * orbit); member o adds o to every outside digit.
+// HIGHEST outside digit is 0 (the orbit index enumerates the other outside digits, lowest first); member o
+// adds o to every outside digit.  Consecutive orbits then differ in the lowest outside digit, so the units that
+// run at the same time on neighbouring CTAs cover, member by member, rows that continue one another in memory
+// (with the lowest digit fixed instead, neighbouring rows belong to far-away orbits: 3.3x read over-fetch).
 struct PottsOrbit { unsigned inst, base[3]; };
 __device__ __forceinline__ PottsOrbit potts_orbit(const PassParams& p, unsigned gunit) {
     const unsigned opi = (unsigned)(p.tiles_per_inst / 3);
     PottsOrbit t;
     t.inst = gunit / opi;
-    unsigned rest = (gunit - t.inst * opi) * 3u;
+    unsigned rest = gunit - t.inst * opi;           // the top outside digit of member 0 is 0: it runs out of `rest`
     t.base[0] = t.base[1] = t.base[2] = 0u;
     auto take = [&](unsigned pw) {
         const unsigned d = rest % 3u; rest /= 3u;
