@@ -226,6 +226,7 @@ struct ttn_plan {
     ttn::Plan plan;
     ttn::FusedPlan fplan;
     bool fused = false, i16 = false;
+    bool merged = false;           // row plan with merged passes (MC_CKPT): runs on fused_sweep_kernel only
     bool z2 = false;               // global-flip reduction: the state is the half with column 0 up (h = 0)
     DebugCfg dbg;                  // the debug switches as they were when the plan was created
     int fused_grid = 0;
@@ -706,10 +707,7 @@ long ttn_plan_describe(int q, int L, ttn_call call, char* buf, size_t n) {
         // the schedules the calls run when h = 0
         if (const ttn::FusedGeom* G = z2_geom(q, L, call, false, dbg)) {
             ttn::FusedPlan fp;
-            if (call == TTN_CALL_CONFIG_Z2) {
-                if (ckpt_scheme(L, true, dbg).k == 0 && !dbg.nomerge) fp = ttn::make_fused_row_plan_merged(L, ttn::FMAX_GATES, *G);
-                if (!fp.ok) fp = ttn::make_fused_row_plan(L, ttn::FMAX_GATES, *G);
-            } else fp = ttn::make_fused_plan(L, ttn::FMAX_GATES, *G);
+            fp = call == TTN_CALL_CONFIG_Z2 ? ttn::make_fused_row_plan(L, ttn::FMAX_GATES, *G) : ttn::make_fused_plan(L, ttn::FMAX_GATES, *G);
             if (fp.ok) s = ttn::describe_fused(fp);
         }
         if (s.empty()) call = call == TTN_CALL_ENERGY_Z2 ? TTN_CALL_ENERGY : (call == TTN_CALL_COUNT_Z2 ? TTN_CALL_COUNT
@@ -722,7 +720,10 @@ long ttn_plan_describe(int q, int L, ttn_call call, char* buf, size_t n) {
     if (call == TTN_CALL_ENERGY_I16 && s.empty()) call = TTN_CALL_ENERGY;
     if (s.empty() && fused_eligible(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG, dbg)) {
         ttn::FusedPlan fp;
-        if (call == TTN_CALL_CONFIG && ckpt_scheme(L, true, dbg).k == 0 && !dbg.nomerge) fp = ttn::make_fused_row_plan_merged(L, ttn::FMAX_GATES);
+        // (ttn_ground_config on batches of small lattices: the merged plan of the one-launch sweep; a single
+        // instance runs one pass per tile and row -- TTN_DEBUG_NOMERGE shows that schedule)
+        if (call == TTN_CALL_CONFIG && ckpt_scheme(L, true, dbg).k == 0 && !dbg.nomerge && !dbg.nosweep && !dbg.nogroup)
+            fp = ttn::make_fused_row_plan_merged(L, ttn::FMAX_GATES);
         if (!fp.ok)
             fp = call == TTN_CALL_COUNT ? ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_COUNT)
                : call == TTN_CALL_CONFIG ? ttn::make_fused_row_plan(L, ttn::FMAX_GATES)
@@ -810,18 +811,21 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
         if (ce != cudaSuccess) { delete P; return fail(TTN_ECUDA, "cudaDeviceGetAttribute failed: %s", cudaGetErrorString(ce)); }
     }
     P->ws = static_cast<unsigned char*>(workspace);
+    // merged row passes (MC_CKPT) exist in the instance-group kernels only: batches of lattices whose passes all
+    // run one CTA per instance group (the one-launch forward sweep)
+    const bool merged_ok = lay.ck.k == 0 && !dbg.nomerge && !dbg.nosweep && !dbg.nogroup && batch >= 2 &&
+                           ((lay.NS >> 12) < 12ull * 64ull);
     if (i16) {
         P->fplan = ttn::make_fused_plan(L, ttn::FMAX_GATES, zg ? *zg : ttn::GEOM_I16);
         P->fused = P->fplan.ok;
         if (!P->fused) { delete P; return fail(TTN_EUNSUPPORTED, "no Tropical<i16> schedule"); }
     } else if (zg) {
-        if (config && lay.ck.k == 0 && !dbg.nomerge) P->fplan = ttn::make_fused_row_plan_merged(L, ttn::FMAX_GATES, *zg);
-        if (config && !P->fplan.ok) P->fplan = ttn::make_fused_row_plan(L, ttn::FMAX_GATES, *zg);
+        if (config) P->fplan = ttn::make_fused_row_plan(L, ttn::FMAX_GATES, *zg);       // (no one-launch sweep for half-states)
         if (!config) P->fplan = ttn::make_fused_plan(L, ttn::FMAX_GATES, *zg);
         P->fused = P->fplan.ok;
         if (!P->fused) { delete P; return fail(TTN_EUNSUPPORTED, "no flip-reduced schedule"); }
     } else if (fused_eligible(q, L, count, config, dbg)) {
-        if (config && lay.ck.k == 0 && !dbg.nomerge) P->fplan = ttn::make_fused_row_plan_merged(L, ttn::FMAX_GATES);
+        if (config && merged_ok) { P->fplan = ttn::make_fused_row_plan_merged(L, ttn::FMAX_GATES); P->merged = P->fplan.ok; }
         if (!P->fplan.ok)
             P->fplan = count ? ttn::make_fused_plan(L, ttn::FMAX_GATES, ttn::GEOM_COUNT)
                      : config ? ttn::make_fused_row_plan(L, ttn::FMAX_GATES) : ttn::make_fused_plan(L, ttn::FMAX_GATES);
@@ -852,7 +856,12 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
     if (e == cudaSuccess) e = up(lay.ops, P->plan.ops.data(), P->plan.ops.size() * sizeof(ttn::Op));
     if (e != cudaSuccess) { delete P; return fail(TTN_ECUDA, "coupling upload failed: %s", cudaGetErrorString(e)); }
 
-    if (P->fused) {
+    for (int attempt = 0; P->fused && attempt < 2; ++attempt) {
+        if (attempt == 1) {                 // the merged plan did not fit the one-launch sweep: one pass per tile and row
+            P->fplan = ttn::make_fused_row_plan(L, ttn::FMAX_GATES);
+            P->merged = false; P->sweep_grid = 0; P->sweep_params.clear();
+            if (!P->fplan.ok) { delete P; return fail(TTN_EUNSUPPORTED, "no row-aligned schedule"); }
+        }
         ttn_status fs = count ? setup_fcount(P, st) : setup_fused(P, st);
         if (fs != TTN_OK) { delete P; return fs; }
         const CkptScheme& ck = lay.ck;
@@ -889,7 +898,9 @@ ttn_status ttn_plan_create(int q, int L, ttn_call call, const float* Jh, const f
                 P->launches = 1 + (bt1 ? 1 : 2 * L);
             }
         }
-    } else {
+        if (!(P->merged && P->sweep_grid == 0)) break;
+    }
+    if (!P->fused) {
         ttn::GenericPrepParams gp{};
         gp.q = q; gp.L = L; gp.n_ops = (int)P->plan.ops.size();
         gp.col_off = P->plan.vcol ? 1 : 0;
@@ -917,7 +928,7 @@ ttn_status ttn_plan_launch(ttn_plan* P, void* stream) {
         std::vector<cudaEvent_t> ev;
         if (timing) { ev.resize(P->fplan.passes.size() + 1); for (auto& e : ev) cudaEventCreate(&e); cudaEventRecord(ev[0], st); }
         // batches of small lattices, no reduction pass (ttn_ground_config): all passes in one launch
-        if (P->sweep_grid > 0 && !timing) {
+        if (P->sweep_grid > 0 && (!timing || P->merged)) {
             ttn::fused_sweep_kernel<0><<<(unsigned)P->sweep_grid, ttn::fwarps(true) * 32, ttn::fsmem_bytes(true), st>>>(
                 reinterpret_cast<const ttn::FusedParams*>(P->ws + P->lay.f_sweep), (int)P->sweep_params.size());
             TTN_CUDA(cudaGetLastError());

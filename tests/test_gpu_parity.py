@@ -259,6 +259,7 @@ def test_one_launch_forward_sweep_matches_per_pass_launches(monkeypatch, L):
     couplings, so any reordering of an addition would show), and match the oracle."""
     B = 37                                             # odd: the last instance group is a single instance
     Jh, Jv, h = make_batch(L, range(2800, 2800 + B), "gauss", fields=True)
+    monkeypatch.setenv("TTN_DEBUG_NOMERGE", "1")       # the same one-pass-per-tile-and-row plan in all three runs
     E_a, sig_a = ttn.ground_config(Jh, Jv, h)
     monkeypatch.setenv("TTN_DEBUG_NOSWEEP", "1")
     E_b, sig_b = ttn.ground_config(Jh, Jv, h)
