@@ -116,6 +116,32 @@ ttn_status ttn_potts3_sweep_count(int L, const float* Jh, const float* Jv, int b
                                   void* workspace, size_t workspace_bytes, void* stream,
                                   double* E0 /*[batch]*/, double* degeneracy /*[batch]*/);
 
+/* ---- for callers that cannot allocate device memory --------------------------------------
+ * ttn_sweep_energy (same sweep, same kernels, same result: PAPER.md:103-118) without the `workspace`
+ * argument.  It is meant for code that has no way to get device memory of its own -- a plug-in or
+ * callback inside a host application whose memory pool already owns the whole GPU (a raw cudaMalloc
+ * there fails and the plug-in has no handle to the pool), or a loop that must not run into the
+ * device-wide synchronisation that cudaMalloc / cudaFree imply.  The scratch memory is an array of
+ * TTN_NOALLOC_SCRATCH_BYTES that is part of the library image: every GPU that loads libttn.so holds
+ * that much from load to process exit, whether or not this function is ever called.  The call
+ * allocates and frees no device memory (the pass schedule lives on the host heap for the duration
+ * of the call; leave the TTN_DEBUG_TIMING test switch unset, it creates CUDA events).
+ *   Limit: the workspace the ordinary call would need, ttn_workspace_bytes(2, L, TTN_TROPICAL_F32,
+ *     batch, 0) -- or ttn_workspace_bytes_h0(...) when h is NULL / all zero -- must fit the array:
+ *     batch 1 up to L = 20 with a field and L = 21 without; small lattices in batches (e.g. 14
+ *     instances of 16 x 16 with fields).  Anything larger returns TTN_EUNSUPPORTED with a message
+ *     that states both sizes, before any CUDA call.
+ *   First call on a device: looks up the array's address on the CURRENT device
+ *     (cudaGetSymbolAddress) and keeps it; make that first call outside any stream capture.
+ *   Sharing: all calls on one device, from any thread or stream, use the SAME array.  Calls that
+ *     overlap on the GPU race on it and give garbage; calls on one stream, or otherwise ordered, are
+ *     safe.  The array keeps what the last call left, and no call depends on it: every byte a sweep
+ *     reads it has written first, so nothing needs clearing between calls.
+ *   Jh, Jv, h, E0 are HOST pointers with the layouts above; the call synchronises `stream`. */
+#define TTN_NOALLOC_SCRATCH_BYTES 4718592 /* 4.5 MiB */
+ttn_status ttn_sweep_energy_noalloc(int L, const float* Jh, const float* Jv, const float* h, int batch,
+                                    void* stream, double* E0 /*[batch]*/);
+
 /* ---- chimera graph (Fig. 2) -------------------------
  * +-J (any integer couplings), no field, on M x N unit cells of K_{4,4}: cell (r, c) holds a
  * vertical group v[0..4) and a horizontal group u[0..4);

@@ -8,4 +8,5 @@ from .ttn import (  # noqa: F401
     TTNError, Plan, lib, workspace_bytes, alloc_workspace, plan_describe,
     sweep_energy, sweep_energy_i16, sweep_count, ground_config, potts3_sweep_energy, potts3_sweep_count,
     chimera_workspace_bytes, chimera_sweep_energy_i16, chimera_count_workspace_bytes, chimera_sweep_count,
+    sweep_energy_noalloc, NOALLOC_SCRATCH_BYTES,
 )

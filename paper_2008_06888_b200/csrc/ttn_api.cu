@@ -1473,3 +1473,64 @@ extern "C" ttn_status ttn_chimera_sweep_count(int M, int N, const float* K, cons
     *degeneracy = std::ldexp(g, -8 * N * (Mp - M));          // the padded cells' free spins (exact: a power of two)
     return TTN_OK;
 }
+
+// ---- ttn_sweep_energy_noalloc: the energy sweep for callers that have no device memory to give -------
+//
+// Every other compute call of this library works inside a device workspace the caller allocates.  Some
+// callers cannot do that: a plug-in or callback living inside a host application that has already given
+// the whole GPU to its own memory pool (a raw cudaMalloc there fails, and the plug-in holds no handle to
+// the pool), or a loop that must never meet the device-wide synchronisation cudaMalloc / cudaFree imply.
+// For them the workspace of this one call is the array below: it is part of the library image, so every
+// GPU that loads libttn.so holds TTN_NOALLOC_SCRATCH_BYTES of it from load until the process exits.
+//
+// On the host, `g_noalloc_scratch` is only a handle for the runtime's symbol table, NOT a device address:
+// handing it to a kernel would fault (or, where the GPU can reach host memory, quietly use the wrong
+// bytes).  The device address is looked up with cudaGetSymbolAddress, once per device, with that device
+// current, by the first call made on it -- that first call should therefore happen outside any stream
+// capture.  The kernels then receive that address exactly like a caller's workspace pointer.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[TTN_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+constexpr int NOALLOC_MAX_DEVICES = 64;
+void* g_noalloc_addr[NOALLOC_MAX_DEVICES] = {};      // per device ordinal: device address of the array
+std::mutex g_noalloc_mu;
+
+ttn_status noalloc_scratch(void** out) {
+    int dev = -1;
+    TTN_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return fail(TTN_EUNSUPPORTED, "device ordinal %d beyond %d", dev, NOALLOC_MAX_DEVICES);
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    if (!g_noalloc_addr[dev]) {
+        void* p = nullptr;
+        TTN_CUDA(cudaGetSymbolAddress(&p, g_noalloc_scratch));     // the copy of the array on the current device
+        if (!p || (uintptr_t)p % 256) return fail(TTN_ECUDA, "cudaGetSymbolAddress gave an unusable address %p", p);
+        g_noalloc_addr[dev] = p;
+    }
+    *out = g_noalloc_addr[dev];
+    return TTN_OK;
+}
+}  // namespace
+
+extern "C" ttn_status ttn_sweep_energy_noalloc(int L, const float* Jh, const float* Jv, const float* h, int batch,
+                                               void* stream, double* E0) {
+    if (!E0) return fail(TTN_EINVAL, "E0 is NULL");
+    if (L < 1 || batch < 1) return fail(TTN_EINVAL, "L and batch must be >= 1");
+    if (L > 1 && (!Jh || !Jv)) return fail(TTN_EINVAL, "Jh/Jv is NULL");
+    // the size the ordinary call would ask its caller for (the smaller half-state size when there is no field)
+    bool field = false;
+    if (h) for (size_t i = 0, n = (size_t)batch * L * L; i < n && !field; ++i) field = (h[i] != 0.0f);
+    const size_t need = field ? ttn_workspace_bytes(2, L, TTN_TROPICAL_F32, batch, 0)
+                              : ttn_workspace_bytes_h0(2, L, TTN_TROPICAL_F32, batch, 0);
+    if (need == 0) return fail(TTN_EUNSUPPORTED, "L=%d beyond the limits for this call", L);
+    if (need > (size_t)TTN_NOALLOC_SCRATCH_BYTES)
+        return fail(TTN_EUNSUPPORTED, "ttn_sweep_energy_noalloc: L=%d, batch=%d needs %zu bytes of scratch, the built-in array holds %zu "
+                    "(L <= 20 with a field, L <= 21 without, batch 1); use ttn_sweep_energy with a workspace of your own",
+                    L, batch, need, (size_t)TTN_NOALLOC_SCRATCH_BYTES);
+    void* scratch = nullptr;
+    ttn_status s = noalloc_scratch(&scratch);
+    if (s != TTN_OK) return s;
+    // Nothing in the array has to start at zero: the first pass of a sweep writes every state element without
+    // reading it, the tables are uploaded or computed by the prep kernel, and every partial is written before the
+    // final reduction reads it -- so what the previous call left behind is never read.
+    return one_call(2, L, TTN_CALL_ENERGY, Jh, Jv, h, batch, scratch, (size_t)TTN_NOALLOC_SCRATCH_BYTES, stream, E0, nullptr, nullptr);
+}

@@ -25,7 +25,9 @@ EXPORTS = [
     "ttn_plan_describe", "ttn_plan_state_elements", "ttn_last_error", "ttn_version",
     "ttn_chimera_workspace_bytes", "ttn_chimera_sweep_energy_i16",
     "ttn_chimera_count_workspace_bytes", "ttn_chimera_sweep_count",
+    "ttn_sweep_energy_noalloc",
 ]
+NOALLOC_SCRATCH_BYTES = 4718592      # TTN_NOALLOC_SCRATCH_BYTES of include/ttn.h
 
 _STATUS = {1: "TTN_EINVAL", 2: "TTN_EUNSUPPORTED", 3: "TTN_ENOMEM", 4: "TTN_ECUDA"}
 
@@ -54,6 +56,7 @@ def lib() -> ctypes.CDLL:
         L.ttn_workspace_bytes_h0.restype = sz
         L.ttn_sweep_energy.argtypes = [ci, fp, fp, fp, ci, vp, sz, vp, dp]
         L.ttn_sweep_energy_i16.argtypes = [ci, fp, fp, fp, ci, vp, sz, vp, dp]
+        L.ttn_sweep_energy_noalloc.argtypes = [ci, fp, fp, fp, ci, vp, dp]
         L.ttn_sweep_count.argtypes = [ci, fp, fp, fp, ci, vp, sz, vp, dp, dp]
         L.ttn_ground_config.argtypes = [ci, fp, fp, fp, ci, vp, sz, vp, dp, i8]
         L.ttn_potts3_sweep_energy.argtypes = [ci, fp, fp, ci, vp, sz, vp, dp]
@@ -234,6 +237,19 @@ def _one_call(fn_name, q, call, Jh, Jv, h, workspace, stream):
 def sweep_energy(Jh, Jv, h=None, workspace=None, stream=None) -> np.ndarray:
     """ttn_sweep_energy: ground-state energies E0[batch] (Tropical<f32> sweep)."""
     return _one_call("ttn_sweep_energy", 2, CALL_ENERGY, Jh, Jv, h, workspace, stream)[0]
+
+
+def sweep_energy_noalloc(Jh, Jv, h=None, stream=None) -> np.ndarray:
+    """ttn_sweep_energy_noalloc: the E0[batch] of sweep_energy, for callers that cannot allocate device memory
+    (a plug-in inside an application whose pool owns the GPU, a loop that must not meet cudaMalloc's
+    device-wide synchronisation).  No workspace is passed or allocated: the sweep runs in a
+    NOALLOC_SCRATCH_BYTES array built into libttn.so, which bounds the size (one lattice up to L = 20 with a
+    field, L = 21 without) and which all calls on a device share -- do not overlap them.  See include/ttn.h."""
+    B, L, Jh, Jv, h = _couplings(Jh, Jv, h)
+    E0 = np.zeros(B, dtype=np.float64)
+    _check(lib().ttn_sweep_energy_noalloc(L, _fptr(Jh), _fptr(Jv), _fptr(h), B, _stream_ptr(stream),
+                                          E0.ctypes.data_as(ctypes.POINTER(ctypes.c_double))))
+    return E0
 
 
 def sweep_energy_i16(Jh, Jv, h=None, workspace=None, stream=None) -> np.ndarray:
