@@ -22,8 +22,8 @@
  * bytes, 256-byte aligned), `stream` is a cudaStream_t passed as void* (NULL = default
  * stream).  The library allocates no device memory; its only process-wide state is a
  * mutex-guarded memo of searched Potts pass schedules (a pure function of L).  The TTN_DEBUG_*
- * environment switches (test hooks) are read once per entry point and a plan keeps the values it
- * was created with.  Every step of the path runs in the library's own sm_100a kernels.  There
+ * environment switches are test hooks: they are ignored unless TTN_ENABLE_DEBUG=1 is also set (the
+ * test suite sets it), are read once per entry point, and a plan keeps the values it was created with.  Every step of the path runs in the library's own sm_100a kernels.  There
  * is NO CPU fallback: without a CUDA device every compute call returns TTN_ECUDA.
  *
  * h = 0 (NULL or all zero): Eq. (1) is invariant under the global flip sigma -> -sigma, and so is
@@ -73,7 +73,8 @@ typedef enum {
 /* Limits: Ising tropical L <= 34, Ising counting L <= 32, Potts L <= 20 (index fits 32 bits);
    ttn_ground_config L <= 32: L checkpoints of 2^L f32 each up to L = 28, ~2 sqrt(L) of them with a
    re-sweep of every segment in the backward pass beyond; the workspace at L = 32 is
-   192 GiB with fields (beyond one B200) and 96 GiB for h = 0 (ttn_workspace_bytes_h0). */
+   208 GiB with fields (12 checkpoint buffers + the state; beyond one B200) and 104 GiB for h = 0
+   (ttn_workspace_bytes_h0). */
 
 /* Bytes of device workspace needed.  q = 2 (Ising) or 3 (Potts).  Returns 0 on bad arguments.
    The size covers any field h.  ttn_workspace_bytes_h0 is the (smaller) size that suffices when the

@@ -51,7 +51,7 @@ unsigned long long ipow(int q, int e) {
     return r;
 }
 
-// Test / debug switches (environment TTN_DEBUG_*).  They are read ONCE per entry point
+// Test / debug switches (environment TTN_DEBUG_*, honoured only when TTN_ENABLE_DEBUG=1).  They are read ONCE per entry point
 // (ttn_workspace_bytes, ttn_plan_describe, ttn_plan_create, the chimera call) into this struct; a
 // plan keeps the snapshot it was created with, and no launch path calls getenv.  The tests use them
 // to force small tiles, the generic kernels or the fallbacks of the specialised paths.
@@ -69,6 +69,9 @@ struct DebugCfg {
 };
 DebugCfg read_debug() {
     DebugCfg d;
+    // opt-in: without TTN_ENABLE_DEBUG=1 (set by tests/conftest.py) no TTN_DEBUG_* variable is looked at, so a
+    // stray one in a user's environment cannot change a workspace size or a kernel path
+    { const char* en = getenv("TTN_ENABLE_DEBUG"); if (!en || atoi(en) != 1) return d; }
     auto geti = [](const char* name, int& v) { if (const char* e = getenv(name)) v = atoi(e); };
     auto flag = [](const char* name, int& v) { v = getenv(name) != nullptr; };
     geti("TTN_DEBUG_TMAX", d.tmax); geti("TTN_DEBUG_RIDE", d.ride); geti("TTN_DEBUG_FUSED", d.fused);
@@ -700,7 +703,15 @@ size_t ttn_workspace_bytes_h0(int q, int L, ttn_semiring mode, int batch, int wa
 
 long ttn_plan_describe(int q, int L, ttn_call call, char* buf, size_t n) {
     if ((q != 2 && q != 3) || !buf || n == 0) return -1;
-    if (!limits_ok(q, L, call == TTN_CALL_COUNT, call == TTN_CALL_CONFIG)) return -1;
+    {   // the limits of the call kind, plain or *_Z2, as ttn_plan_create derives them; the flip reduction is Ising only
+        const bool z2_kind = (call == TTN_CALL_ENERGY_Z2 || call == TTN_CALL_COUNT_Z2 || call == TTN_CALL_ENERGY_I16_Z2 ||
+                              call == TTN_CALL_CONFIG_Z2);
+        if (call < TTN_CALL_ENERGY || call > TTN_CALL_CONFIG_Z2) return -1;
+        if (q == 3 && (z2_kind || call == TTN_CALL_ENERGY_I16)) return -1;
+        const bool count = (call == TTN_CALL_COUNT || call == TTN_CALL_COUNT_Z2);
+        const bool config = (call == TTN_CALL_CONFIG || call == TTN_CALL_CONFIG_Z2);
+        if (!limits_ok(q, L, count, config)) return -1;
+    }
     std::string s;
     const DebugCfg dbg = read_debug();
     if (call == TTN_CALL_ENERGY_Z2 || call == TTN_CALL_COUNT_Z2 || call == TTN_CALL_ENERGY_I16_Z2 || call == TTN_CALL_CONFIG_Z2) {
@@ -1064,7 +1075,8 @@ struct Chimera2Layout {
 Chimera2Layout chimera2_layout(int M, int N, const DebugCfg& dbg) {
     Chimera2Layout c;
     const int NB = 4 * M, cols = N > 1 ? N - 1 : 1;
-    c.lay = make_layout(2, NB, false, false, 1, dbg, /*i16=*/true, false);
+    DebugCfg d = dbg; d.fused = 1;           // the gate rows always run on the fused pass kernels, whatever TTN_DEBUG_FUSED says
+    c.lay = make_layout(2, NB, false, false, 1, d, /*i16=*/true, false);
     size_t off = c.lay.total;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
     c.fJh = take((size_t)cols * NB * (NB - 1) * 4 + 4);           // fake couplings, one "instance" per column
@@ -1091,7 +1103,8 @@ struct ChimeraCountLayout {
 ChimeraCountLayout chimera_count_layout(int Mp, int N, const DebugCfg& dbg) {
     ChimeraCountLayout c;
     const int NB = 4 * Mp, cols = N > 1 ? N - 1 : 1;
-    c.lay = make_layout(2, NB, true, false, 1, dbg, false, false);
+    DebugCfg d = dbg; d.fused = 1;           // (as chimera2_layout)
+    c.lay = make_layout(2, NB, true, false, 1, d, false, false);
     size_t off = c.lay.total;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
     c.fJh = take((size_t)cols * NB * (NB - 1) * 4 + 4);
@@ -1442,6 +1455,9 @@ extern "C" ttn_status ttn_chimera_sweep_count(int M, int N, const float* K, cons
     cp.tiles = 1ull << (NB - 12);
     cp.part_x = reinterpret_cast<float*>(base + cl.lay.part_x);
     cp.part_n = reinterpret_cast<double*>(base + cl.lay.part_n);
+    // every padded cell carries 8 free spins, a factor 2^8 on the count per column: taken out column by column (an
+    // exact power-of-two scaling) so that the running count never holds 2^(8 N (Mp - M)) -- 2^1024 at M = 1, N = 64
+    cp.n_scale = std::ldexp(1.0, -8 * (Mp - M));
     const unsigned long long needc = (cp.tiles + ttn::CH2C_WARPS - 1) / ttn::CH2C_WARPS;
     const unsigned cgrid = (unsigned)(needc < (unsigned long long)sms ? needc : (unsigned long long)sms);
     if ((unsigned long long)cgrid > cl.lay.max_tiles) return fail(TTN_EUNSUPPORTED, "chimera count: partials do not fit");
@@ -1470,7 +1486,7 @@ extern "C" ttn_status ttn_chimera_sweep_count(int M, int N, const float* K, cons
     TTN_CUDA(cudaStreamSynchronize(st));
     const double top = (double)mx + shift;
     *E0 = top == 0.0 ? 0.0 : -top;
-    *degeneracy = std::ldexp(g, -8 * N * (Mp - M));          // the padded cells' free spins (exact: a power of two)
+    *degeneracy = g;                                         // (the padded cells' free spins were divided out per column)
     return TTN_OK;
 }
 

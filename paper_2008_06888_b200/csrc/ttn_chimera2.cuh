@@ -191,6 +191,7 @@ struct ChimeraCountParams {
     const float* tables;          // [M rows][16 u][16 v]: B_r(u, v) of this column
     float jv[8][4];               // [r][k] = -2 Jv[r-1][c][k]; row 0 unused
     float* part_x; double* part_n;   // [gridDim.x] (reduce)
+    double n_scale;               // a power of two put on every count of this column (1.0, or 2^-8p for p padded rows)
 };
 
 __device__ __forceinline__ double ch2_ind(bool p) { return __hiloint2double(p ? 0x3ff00000 : 0, 0); }
@@ -233,7 +234,7 @@ __global__ void __launch_bounds__(CH2C_WARPS * 32, 1) chimera_column_count_kerne
         // ---- levels M-1 .. 3: uniform per tile
         float b3x[16]; double b3n[16];
 #pragma unroll
-        for (int v = 0; v < 16; ++v) { b3x[v] = 0.f; b3n[v] = 1.0; }
+        for (int v = 0; v < 16; ++v) { b3x[v] = 0.f; b3n[v] = q.n_scale; }     // every count below is linear in it
         for (int r = q.M - 1; r >= 3; --r) {
             const int ur = (int)((tile >> (4 * (r - 3))) & 15ull);
 #pragma unroll

@@ -3,6 +3,9 @@ import sys
 
 import pytest
 
+# the TTN_DEBUG_* switches the tests use (small tiles, forced fallbacks) are honoured only with this opt-in (ttn.h)
+os.environ.setdefault("TTN_ENABLE_DEBUG", "1")
+
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)

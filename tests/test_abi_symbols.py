@@ -57,3 +57,37 @@ def test_no_cpu_fallback():
     import numpy as np
     with pytest.raises(ttn.TTNError):
         ttn.sweep_energy(np.ones((3, 2)), np.ones((2, 3)))
+
+
+def test_plan_describe_limits_follow_the_call_kind():
+    """ttn_plan_describe applies the limits ttn_plan_create applies: counting and config stop at L = 32 for the
+    plain and the *_Z2 kinds alike, and the flip-reduced kinds are Ising calls."""
+    lib = ttn.lib()
+    buf = ctypes.create_string_buffer(16)
+    assert lib.ttn_plan_describe(2, 33, ttn.CALL_ENERGY_Z2, buf, 16) > 0          # energy: L <= 34
+    for call in (ttn.CALL_COUNT, ttn.CALL_COUNT_Z2, ttn.CALL_CONFIG, ttn.CALL_CONFIG_Z2):
+        assert lib.ttn_plan_describe(2, 33, call, buf, 16) == -1, call
+        assert lib.ttn_plan_describe(2, 20, call, buf, 16) > 0, call
+    for call in (ttn.CALL_ENERGY_Z2, ttn.CALL_COUNT_Z2, ttn.CALL_ENERGY_I16_Z2, ttn.CALL_CONFIG_Z2, ttn.CALL_ENERGY_I16, ttn.CALL_CONFIG):
+        assert lib.ttn_plan_describe(3, 8, call, buf, 16) == -1, call
+    assert lib.ttn_plan_describe(3, 8, ttn.CALL_COUNT, buf, 16) > 0
+    assert lib.ttn_plan_describe(2, 8, 99, buf, 16) == -1
+
+
+def test_debug_switches_need_the_opt_in(monkeypatch):
+    """A stray TTN_DEBUG_* variable changes nothing unless TTN_ENABLE_DEBUG=1 is set too (conftest.py sets it)."""
+    half = ttn.workspace_bytes(2, 20, ttn.TROPICAL_F32, 1, h_zero=True)
+    full = ttn.workspace_bytes(2, 20, ttn.TROPICAL_F32, 1)
+    assert half < full
+    monkeypatch.setenv("TTN_DEBUG_Z2", "0")
+    assert ttn.workspace_bytes(2, 20, ttn.TROPICAL_F32, 1, h_zero=True) == full     # opted in: the switch acts
+    monkeypatch.delenv("TTN_ENABLE_DEBUG")
+    assert ttn.workspace_bytes(2, 20, ttn.TROPICAL_F32, 1, h_zero=True) == half     # not opted in: ignored
+    monkeypatch.setenv("TTN_DEBUG_FUSED", "0")
+    assert ttn.workspace_bytes(2, 20, ttn.TROPICAL_F32, 1) == full
+    # the chimera layouts do not depend on TTN_DEBUG_FUSED even when opted in (their gate rows always run fused)
+    monkeypatch.setenv("TTN_ENABLE_DEBUG", "1")
+    a = ttn.chimera_workspace_bytes(4, 3), ttn.chimera_count_workspace_bytes(3, 3)
+    monkeypatch.delenv("TTN_DEBUG_FUSED")
+    monkeypatch.delenv("TTN_DEBUG_Z2")
+    assert a == (ttn.chimera_workspace_bytes(4, 3), ttn.chimera_count_workspace_bytes(3, 3))

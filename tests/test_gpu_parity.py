@@ -219,6 +219,20 @@ def test_gaussian_couplings_and_fields_f32_tolerance(L):
         assert ttn.sweep_energy(Jh[:1], Jv[:1], h[:1])[0] == E1[0]
 
 
+def test_paper_headline_32x32_gaussian_J_and_h():
+    """The paper's own headline workload at full size: 32x32, Gaussian couplings AND fields, Float32
+    ("1024 spins with external fields"; Fig. 7a), the instance bench.py times as
+    paper_32x32_gauss_J_and_h_f32 (seed 2032).  The full 2^32-element state, 19 passes, against the f64 O-dp
+    value written by tests/golden/make_golden.py ising_gauss 32 2032 2033, at north_star's 1e-5 |E0|."""
+    gold = golden()
+    key = ("ising_gauss", 32, 2032)
+    if key not in gold:
+        pytest.skip("no stored oracle value for %s" % (key,))
+    Jh, Jv, h = make_batch(32, [2032], "gauss", fields=True)
+    E = ttn.sweep_energy(Jh, Jv, h)
+    assert abs(E[0] - gold[key][0]) <= TOL * abs(gold[key][0]), (E[0], gold[key][0])
+
+
 def test_mid_potts_vs_oracle():
     for L in (10, 11):
         Jh, Jv, _ = make_batch(L, [5000], "pmj", q=3)
@@ -568,11 +582,16 @@ def test_z2_i16_energy_vs_oracle(L, monkeypatch):
     assert np.array_equal(E_f, E_z)
 
 
-def test_full_state_i16_still_matches_golden(monkeypatch):
+@pytest.mark.parametrize("L", [28, 32])
+def test_full_state_i16_still_matches_golden(L, monkeypatch):
+    """Full-state Tropical<i16> (flip reduction off) on the +-J goldens; L = 32 is the 2^32-element plan (8 GiB)."""
     gold = golden()
     monkeypatch.setenv("TTN_DEBUG_Z2", "0")
-    Jh, Jv, _ = make_batch(28, [4000], "pmj")
-    assert ttn.sweep_energy_i16(Jh, Jv)[0] == gold[("ising_energy", 28, 4000)][0]
+    Jh, Jv, _ = make_batch(L, [4000], "pmj")
+    p = ttn.Plan(2, ttn.CALL_ENERGY_I16, Jh, Jv)
+    assert p.state_elements == 2 ** L
+    p.launch(); E, _, _ = p.read(); p.close()
+    assert E[0] == gold[("ising_energy", L, 4000)][0]
 
 
 @pytest.mark.parametrize("L", [16, 20, 24])
@@ -586,13 +605,41 @@ def test_z2_gaussian_couplings_f32_tolerance(L):
             assert abs(E1[b] - Eo) <= TOL * abs(Eo)
 
 
-@pytest.mark.parametrize("L", [24, 28])
+@pytest.mark.parametrize("L", [24, 28, 32])
 def test_full_state_sweep_still_matches_golden(L, monkeypatch):
-    """The full-state Tropical<f32> sweep (what any h != 0 runs) on the +-J goldens, flip reduction off."""
+    """The full-state Tropical<f32> sweep (what any h != 0 runs) on the +-J goldens, flip reduction off.
+    L = 32: the 19-pass plan over 2^32 elements (16 GiB in place) that every caller with a field runs at the
+    headline size, against the O-dp value of cfg 4."""
     gold = golden()
     monkeypatch.setenv("TTN_DEBUG_Z2", "0")
     Jh, Jv, _ = make_batch(L, [4000], "pmj")
-    assert ttn.sweep_energy(Jh, Jv)[0] == gold[("ising_energy", L, 4000)][0]
+    p = ttn.Plan(2, ttn.CALL_ENERGY, Jh, Jv)
+    assert p.state_elements == 2 ** L
+    p.launch(); E, _, _ = p.read(); p.close()
+    assert E[0] == gold[("ising_energy", L, 4000)][0]
+
+
+def test_full_state_count_32x32(monkeypatch):
+    """ttn_sweep_count at 32x32 with the flip reduction off: 2^32 counting elements (51.5 GB).  E0 is the O-dp
+    golden of cfg 4; the degeneracy has no oracle value at this size (test_next2_count_32x32) and is compared with
+    the flip-reduced sweep's (2 x the half's count), which sums the same integers in another order."""
+    import torch
+    L = 32
+    free, _ = torch.cuda.mem_get_info()
+    need = ttn.workspace_bytes(2, L, ttn.COUNTING_F32_F64, 1)
+    if free < need + (2 << 30):
+        pytest.skip("needs %.0f GB of free device memory" % (need / 1e9))
+    ws = ttn.alloc_workspace(need)
+    Jh, Jv, _ = config_batch(4)
+    E_z, g_z = ttn.sweep_count(Jh, Jv, workspace=ws)
+    monkeypatch.setenv("TTN_DEBUG_Z2", "0")
+    p = ttn.Plan(2, ttn.CALL_COUNT, Jh, Jv, workspace=ws)
+    assert p.state_elements == 2 ** L
+    p.launch(); E_f, g_f, _ = p.read(); p.close()
+    assert E_f[0] == golden()[("ising_energy", 32, 4000)][0] and E_z[0] == E_f[0]
+    assert count_ok(g_f[0], int(g_z[0])), (g_f, g_z)
+    del ws
+    torch.cuda.empty_cache()
 
 
 # ------------------------------------------------------------------ error behaviour
@@ -947,6 +994,34 @@ def test_chimera_count_closed_forms_and_transpose(M, N):
     assert Et == E and g >= 2 and (gt == g if g < 2 ** 53 else abs(gt - g) <= 1e-12 * g)
     if g < 2 ** 53:
         assert int(g) % 2 == 0                                                                            # global flip
+
+
+def test_chimera_count_single_row_of_64_cells():
+    """M = 1 is padded to three rows of cells; the padding's free spins are divided out column by column, so the
+    running count stays finite at the documented maximum N = 64 (it used to carry 2^(16 N) = 2^1024)."""
+    co = _chimera_oracle()
+    M, N = 1, 64
+    one = lambda *s: np.ones(s, dtype=np.float32)
+    ne = co.n_edges(M, N, 4)
+    assert ttn.chimera_sweep_count(one(M, N, 4, 4), one(M - 1, N, 4), one(M, N - 1, 4)) == (-ne, 2.0)       # ferromagnet
+    E, g = ttn.chimera_sweep_count(0 * one(M, N, 4, 4), 0 * one(M - 1, N, 4), 0 * one(M, N - 1, 4))
+    assert E == 0.0 and g == 2.0 ** (8 * M * N)                                                           # 512 free spins
+    assert ttn.chimera_sweep_count(one(2, N, 4, 4), one(1, N, 4), one(2, N - 1, 4)) == (-co.n_edges(2, N, 4), 2.0)
+    from ttn_inputs import make_chimera_instance
+    I = make_chimera_instance(1, 6, 6600)                       # seeded +-J strip against the oracle (int64 counts)
+    Eo, go = co.dp_chimera(1, 6, 4, I.K, I.Jv, I.Jh)
+    assert ttn.chimera_sweep_count(I.K, I.Jv, I.Jh) == (Eo, float(go))
+
+
+def test_chimera_does_not_depend_on_the_fused_switch(monkeypatch):
+    """TTN_DEBUG_FUSED=0 selects the generic Ising kernels; the chimera gate rows always run on the fused pass
+    kernels and their workspace layout says so (it used to return TTN_EUNSUPPORTED for M >= 4)."""
+    from ttn_inputs import make_chimera_instance
+    I = make_chimera_instance(4, 3, 6601)
+    ref = ttn.chimera_sweep_energy_i16(I.K, I.Jv, I.Jh), ttn.chimera_sweep_count(I.K, I.Jv, I.Jh)
+    monkeypatch.setenv("TTN_DEBUG_FUSED", "0")
+    assert (ttn.chimera_sweep_energy_i16(I.K, I.Jv, I.Jh), ttn.chimera_sweep_count(I.K, I.Jv, I.Jh)) == ref
+    assert ref[0] == ref[1][0]
 
 
 def test_chimera_count_8x8_cells():
