@@ -471,7 +471,7 @@ def main():
 
     if rank == 0:
         peak, peak_src = measured_peaks()
-        traffic, traffic_src = ncu_traffic_per_launch("r02_ncu_full_summary.csv", "fused_pass_kernel") if L == 32 else (None, None)
+        traffic, traffic_src = ncu_traffic_per_launch("r03b_ncu_full_sweep_summary.csv", "fused_pass_kernel") if L == 32 else (None, None)
         per_inst_ms = whole_job_ms_per_instance(ms_per_step, world)
         moved = bytes_moved(4, plan.state_elements, plan.num_passes)    # bytes one sweep really moves (computed)
         achieved = moved / (ms_per_step * 1e-3) / 1e9                   # GB/s per GPU
@@ -503,8 +503,8 @@ def main():
                          "updates_per_sweep": upd_exec,
                          "peak_source": "148 SMs x 64 FMNMX lanes/clk/SM (profiles/r01_ubench.md) x the SM clock sampled "
                                         "during the timed region (DESIGN.md section 6)",
-                         # dram__bytes_read.sum + dram__bytes_write.sum per pass launch, read from the committed
-                         # ncu --set full summary of this kernel (None if absent / other L)
+                         # dram__bytes_read.sum + dram__bytes_write.sum per pass launch, mean over ALL 19 pass launches of
+                         # one sweep, read from the committed ncu --set full summary (None if absent / other L)
                          "traffic": traffic, "traffic_source": traffic_src,
                          "traffic_computed_per_launch": moved / plan.num_passes,
                          "note": "1 FMNMX per EXECUTED update: L(L-1) gates over the stored state (half of north_star's "
