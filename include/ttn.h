@@ -20,8 +20,9 @@
  * Memory spaces.  Couplings and results are HOST pointers (they are O(L^2) numbers);
  * `workspace` is a DEVICE pointer owned by the caller (at least ttn_workspace_bytes(...)
  * bytes, 256-byte aligned), `stream` is a cudaStream_t passed as void* (NULL = default
- * stream).  The library allocates no device memory; its only process-wide state is a
- * mutex-guarded memo of searched Potts pass schedules (a pure function of L).  The TTN_DEBUG_*
+ * stream).  The library allocates no device memory; its process-wide state is a mutex-guarded
+ * memo of searched Potts pass schedules (a pure function of L) and, for ttn_sweep_energy_noalloc
+ * only, the built-in scratch array with its per-device address table (see that call).  The TTN_DEBUG_*
  * environment switches are test hooks: they are ignored unless TTN_ENABLE_DEBUG=1 is also set (the
  * test suite sets it), are read once per entry point, and a plan keeps the values it was created with.  Every step of the path runs in the library's own sm_100a kernels.  There
  * is NO CPU fallback: without a CUDA device every compute call returns TTN_ECUDA.

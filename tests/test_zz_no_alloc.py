@@ -50,6 +50,14 @@ def test_noalloc_equals_workspace_path_on_consecutive_calls():
     again = ttn.sweep_energy_noalloc(Jh, Jv, h)
     assert np.array_equal(again, first), (again, first)
 
+    # degenerate sizes: a single spin, a 2x2 and a 5x5 lattice (batches of 3, integer couplings and fields)
+    rng = np.random.default_rng(7350)
+    for Ls in (1, 2, 5):
+        Jhs = rng.integers(-3, 4, size=(3, Ls, Ls - 1)).astype(np.float32)
+        Jvs = rng.integers(-3, 4, size=(3, Ls - 1, Ls)).astype(np.float32)
+        hs = rng.integers(-2, 3, size=(3, Ls, Ls)).astype(np.float32)
+        assert np.array_equal(ttn.sweep_energy_noalloc(Jhs, Jvs, hs), ttn.sweep_energy(Jhs, Jvs, hs)), Ls
+
     # the largest field-free lattice that fits (21x21, half-state of 2^20 elements)
     L4 = 21
     Jh4, Jv4, _ = make_batch(L4, [7400], "pmj")
