@@ -97,7 +97,7 @@ def _matvec(x, n, axis, W):
 def dp_chimera(M, N, T, K, Jv, Jh, hv=None, hu=None) -> Tuple[float, int]:
     """(E0, degeneracy) by the column-by-column contraction of the group tensor network."""
     D = 1 << T
-    assert D ** (M + 1) <= 1 << 26, "oracle sizes only"
+    assert D ** (M + 1) <= 1 << 28, "oracle sizes only"             # 6 x N cells of K_{4,4}: a few GB and minutes
     S = _spins(T)                                                   # [D, T]
     K = np.asarray(K, dtype=np.float64).reshape(M, N, T, T)
     Jv = np.asarray(Jv, dtype=np.float64).reshape(max(M - 1, 0), N, T)

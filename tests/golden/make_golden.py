@@ -6,6 +6,7 @@ path.  Usage:
     python tests/golden/make_golden.py ising_energy 32 4000 4001    # cfg 4 (34 GB, ~hours)
     python tests/golden/make_golden.py potts_count 18 5000 5004     # cfg 5
     python tests/golden/make_golden.py ising_gauss 16 2000 2256     # cfg 2 (E0 + sigma energy)
+    python tests/golden/make_golden.py chimera 6 7006 7007          # chimera graph, 6 x 6 cells (L = M = N), dp_chimera
 
 Each run appends/updates lines "kind L seed E0 g" in tests/golden/oracle_values.txt (g = -1
 when not computed; E0 printed with repr() so float64 round-trips exactly).
@@ -24,7 +25,8 @@ OUT = os.path.join(os.path.dirname(os.path.abspath(__file__)), "oracle_values.tx
 HEADER = (
     "# kind L seed E0 g  -- written by tests/golden/make_golden.py from oracle/ (O-dp) on\n"
     "# ttn_inputs.make_instance(L, seed, ...).  kinds: ising_count/ising_energy = +-J h=0 (cfg 3/4\n"
-    "# distribution), potts_count = +-J 3-state Potts (cfg 5), ising_gauss = Gaussian J,h (cfg 2).\n"
+    "# distribution), potts_count = +-J 3-state Potts (cfg 5), ising_gauss = Gaussian J,h (cfg 2),\n"
+    "# chimera = +-J chimera graph of L x L unit cells, ttn_inputs.make_chimera_instance(L, L, seed), oracle.chimera_oracle.dp_chimera.\n"
 )
 
 
@@ -66,6 +68,11 @@ def main():
             i = make_instance(L, seed, "gauss", fields=True)
             E0, g, _ = oracle.dp_ising(L, i.Jh, i.Jv, i.h, count=False)
             g = -1
+        elif kind == "chimera":
+            from oracle import chimera_oracle
+            from ttn_inputs import make_chimera_instance
+            i = make_chimera_instance(L, L, seed)
+            E0, g = chimera_oracle.dp_chimera(L, L, 4, i.K, i.Jv, i.Jh)
         else:
             raise SystemExit("unknown kind")
         rows = load()

@@ -996,6 +996,22 @@ def test_chimera_count_closed_forms_and_transpose(M, N):
         assert int(g) % 2 == 0                                                                            # global flip
 
 
+def test_chimera_6x6_cells_vs_oracle_golden():
+    """288 spins, one size beyond what the oracle contracts inside the test suite: E0 and the degeneracy of the
+    seeded 6 x 6 instance against the dp_chimera value stored by tests/golden/make_golden.py chimera 6 7006 7007,
+    through both the Tropical<i16> and the counting path."""
+    from ttn_inputs import make_chimera_instance
+    key = ("chimera", 6, 7006)
+    gold = golden()
+    if key not in gold:
+        pytest.skip("no stored oracle value for %s" % (key,))
+    Eo, go = gold[key]
+    I = make_chimera_instance(6, 6, 7006)
+    assert ttn.chimera_sweep_energy_i16(I.K, I.Jv, I.Jh) == Eo
+    E, g = ttn.chimera_sweep_count(I.K, I.Jv, I.Jh)
+    assert E == Eo and count_ok(g, go), (E, g, Eo, go)
+
+
 def test_chimera_count_single_row_of_64_cells():
     """M = 1 is padded to three rows of cells; the padding's free spins are divided out column by column, so the
     running count stays finite at the documented maximum N = 64 (it used to carry 2^(16 N) = 2^1024)."""
